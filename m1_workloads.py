@@ -1,0 +1,115 @@
+"""Seeded synthetic inputs for the M1 radiative-transfer step — shared by the oracle tests and the CUDA tests/bench.
+
+This module holds NONE of the method's arithmetic (no closure, no fluxes, no solver): it only draws the
+initial fields, opacities and grids that BASELINE.json's configs describe.  Everything is host numpy, fp64,
+planes of shape [ny, nx] (x fastest); F has shape [2, ny, nx] = (Fx, Fy).
+
+The paper (arXiv 2011.13926) uses analytic set-ups, not datasets; these generators restate BASELINE.json's
+five configs.  Recipes (also in DESIGN.md, "Input recipe"):
+
+  config 1  gaussian_diffusion   : 64^2 unit box, periodic, E = exp(-r^2/(2 s0^2)) + 1e-6, s0 = 0.05, F = 0,
+                                   sigma_s = 1e3, sigma_a = 0.
+  config 2  opacity_jump         : 256^2 unit box, sigma_a = 0, sigma_s = 1 (x < 1/2) | 1e3 (x >= 1/2), F0 = 0.1;
+                                   the discrete steady profile itself is computed by oracle/steady_profile.py.
+  config 3/4 random_medium       : draw order with numpy.random.default_rng(seed):
+                                   (1) log10 sigma_a ~ U[-3,3]  [ny,nx]   (2) log10 sigma_s ~ U[-3,3]  [ny,nx]
+                                   (3) g ~ N(0,1) -> E = exp(g)  (4) u ~ U[0,0.9]  (5) theta ~ U[0,2pi)
+                                   both log10-opacity fields are smoothed with a separable periodic 5x5 box mean
+                                   (applied to the log field) and exponentiated; |F| = u c E, direction theta.
+  config 5  stratified_coupled   : see the function docstring.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+CFL_EXPLICIT = 0.4  # explicit dt = CFL * min(dx, dy) / c  (reading R3)
+
+
+def explicit_dt(dx, dy, c=1.0, cfl=CFL_EXPLICIT):
+    return cfl * min(dx, dy) / c
+
+
+def cell_centres(nx, ny, lx=1.0, ly=1.0):
+    dx, dy = lx / nx, ly / ny
+    x = (np.arange(nx) + 0.5) * dx
+    y = (np.arange(ny) + 0.5) * dy
+    return x, y, dx, dy
+
+
+def gaussian_diffusion(n=64, sigma_s=1e3, s0=0.05, floor=1e-6):
+    """BASELINE.json configs[0]."""
+    x, y, dx, dy = cell_centres(n, n)
+    X, Y = np.meshgrid(x, y)
+    r2 = (X - 0.5) ** 2 + (Y - 0.5) ** 2
+    E = np.exp(-r2 / (2.0 * s0 * s0)) + floor
+    F = np.zeros((2, n, n))
+    return dict(nx=n, ny=n, dx=dx, dy=dy, c=1.0, bc=(0, 0, 0, 0), E=E, F=F,
+                sigma_a=np.zeros((n, n)), sigma_s=np.full((n, n), float(sigma_s)), s0=s0, floor=floor)
+
+
+def opacity_jump(n=256, sig_lo=1.0, sig_hi=1e3, F0=0.1, E_out=100.0):
+    """BASELINE.json configs[1]: the opacity field and the boundary data of the constant-flux steady state.
+    The discrete steady profile E(x) is NOT computed here (it needs the scheme: oracle/steady_profile.py)."""
+    x, y, dx, dy = cell_centres(n, n)
+    sig_line = np.where(x < 0.5, sig_lo, sig_hi)
+    return dict(nx=n, ny=n, dx=dx, dy=dy, c=1.0, bc=(1, 1, 0, 0), x=x,
+                sigma_a=np.zeros((n, n)), sigma_s=np.tile(sig_line, (n, 1)), sigma_line=sig_line,
+                sigma_ghost=(sig_lo, sig_hi), F0=F0, E_out=E_out)
+
+
+def _box5_periodic(a):
+    out = np.zeros_like(a)
+    for s in (-2, -1, 0, 1, 2):
+        out += np.roll(a, s, axis=1)
+    a = out / 5.0
+    out = np.zeros_like(a)
+    for s in (-2, -1, 0, 1, 2):
+        out += np.roll(a, s, axis=0)
+    return out / 5.0
+
+
+def random_medium(n=1024, seed=1234, c=1.0, ny=None):
+    """BASELINE.json configs[2] and configs[3] (same generator, n = 1024 and 4096)."""
+    nx, ny = n, (n if ny is None else ny)
+    rng = np.random.default_rng(seed)
+    lsa = rng.uniform(-3.0, 3.0, size=(ny, nx))
+    lss = rng.uniform(-3.0, 3.0, size=(ny, nx))
+    g = rng.standard_normal(size=(ny, nx))
+    u = rng.uniform(0.0, 0.9, size=(ny, nx))
+    th = rng.uniform(0.0, 2.0 * np.pi, size=(ny, nx))
+    sigma_a = 10.0 ** _box5_periodic(lsa)
+    sigma_s = 10.0 ** _box5_periodic(lss)
+    E = np.exp(g)
+    F = np.empty((2, ny, nx))
+    F[0] = u * c * E * np.cos(th)
+    F[1] = u * c * E * np.sin(th)
+    dx, dy = 1.0 / nx, 1.0 / ny
+    return dict(nx=nx, ny=ny, dx=dx, dy=dy, c=c, bc=(0, 0, 0, 0), E=E, F=F, sigma_a=sigma_a, sigma_s=sigma_s, seed=seed)
+
+
+def stratified_coupled(n=2048, seed=4321, c=1.0, gamma=5.0 / 3.0, H=0.1, kappa=1e3, u_rms=1e-3, a_r=1.0):
+    """BASELINE.json configs[4] (stage 2).  Draw order with default_rng(seed):
+    (1) xi ~ N(0,1) [ny,nx] density perturbation  (2) g ~ N(0, 0.1^2) -> T = exp(g)  (3) psi ~ N(0,1) stream function.
+    rho = exp(-y/H)(1 + 0.01 xi); rho c_v = rho/(gamma-1) (k_b/(mu m_H) = 1); sigma_a = sigma_s = kappa rho;
+    E = a_r T^4, F = 0; velocity = curl of the 5x5-box-smoothed (three passes) periodic stream function by central
+    differences, rescaled to rms |u| = u_rms c; source_E = Q in the 2x2 central cells, Q = 100/dt_explicit."""
+    nx = ny = n
+    x, y, dx, dy = cell_centres(nx, ny)
+    rng = np.random.default_rng(seed)
+    xi = rng.standard_normal(size=(ny, nx))
+    g = 0.1 * rng.standard_normal(size=(ny, nx))
+    psi = rng.standard_normal(size=(ny, nx))
+    rho = np.exp(-y / H)[:, None] * (1.0 + 0.01 * xi)
+    T = np.exp(g)
+    for _ in range(3):
+        psi = _box5_periodic(psi)
+    ux = (np.roll(psi, -1, axis=0) - np.roll(psi, 1, axis=0)) / (2.0 * dy)
+    uy = -(np.roll(psi, -1, axis=1) - np.roll(psi, 1, axis=1)) / (2.0 * dx)
+    scale = u_rms * c / np.sqrt(np.mean(ux * ux + uy * uy))
+    ux, uy = ux * scale, uy * scale
+    E = a_r * T ** 4
+    src = np.zeros((ny, nx))
+    src[ny // 2 - 1: ny // 2 + 1, nx // 2 - 1: nx // 2 + 1] = 100.0 / explicit_dt(dx, dy, c)
+    return dict(nx=nx, ny=ny, dx=dx, dy=dy, c=c, bc=(0, 0, 0, 0), E=E, F=np.zeros((2, ny, nx)), T=T,
+                sigma_a=kappa * rho, sigma_s=kappa * rho, rho_cv=rho / (gamma - 1.0), ux=ux, uy=uy, source_E=src,
+                a_r=a_r, seed=seed)

@@ -1,0 +1,44 @@
+"""Helpers shared by the tests: build an oracle (or a CUDA solver) from a workload dict."""
+import numpy as np
+
+
+def make_oracle(w, options=None):
+    from oracle.oracle_m1 import OracleM1
+    o = OracleM1(w["nx"], w["ny"], w["dx"], w["dy"], w.get("c", 1.0), bc=w.get("bc", (0, 0, 0, 0)))
+    for k, v in (options or {}).items():
+        o.set_option(k, v)
+    o.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"], w.get("T"))
+    for name in ("rho_cv", "ux", "uy", "source_E"):
+        if w.get(name) is not None:
+            o.set_field(name, w[name])
+    for side, g in (w.get("ghosts") or {}).items():
+        o.set_boundary(side, *g)
+    return o
+
+
+def rel_l2(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def small_random_state(nx, ny, seed, fmax=0.9, dx=None, dy=None, c=1.0, bc=(0, 0, 0, 0), sig_range=(-1.0, 2.0)):
+    """A small rough state for operator/assembly checks (not one of BASELINE's configs)."""
+    rng = np.random.default_rng(seed)
+    E = np.exp(rng.standard_normal((ny, nx)))
+    u = rng.uniform(0.0, fmax, (ny, nx))
+    th = rng.uniform(0.0, 2 * np.pi, (ny, nx))
+    F = np.stack((u * c * E * np.cos(th), u * c * E * np.sin(th)))
+    sa = 10.0 ** rng.uniform(*sig_range, (ny, nx))
+    ss = 10.0 ** rng.uniform(*sig_range, (ny, nx))
+    w = dict(nx=nx, ny=ny, dx=dx or 1.0 / nx, dy=dy or 1.0 / ny, c=c, bc=bc, E=E, F=F, sigma_a=sa, sigma_s=ss)
+    ghosts = {}
+    for side in range(4):
+        if bc[side] == 1:
+            n = ny if side < 2 else nx
+            Eg = np.exp(rng.standard_normal(n))
+            ug = rng.uniform(0.0, fmax, n)
+            tg = rng.uniform(0.0, 2 * np.pi, n)
+            Fg = np.stack((ug * c * Eg * np.cos(tg), ug * c * Eg * np.sin(tg)))
+            ghosts[side] = (Eg, Fg, 10.0 ** rng.uniform(*sig_range, n), 10.0 ** rng.uniform(*sig_range, n))
+    w["ghosts"] = ghosts
+    return w

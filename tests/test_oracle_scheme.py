@@ -1,0 +1,206 @@
+"""Pins for the oracle's fluxes, AP factor, WB source and explicit step (Eqs. 12-14, 18-19, 25, C.7-C.10)."""
+import math
+
+import numpy as np
+import pytest
+
+import m1_workloads as wl
+from oracle.oracle_m1 import OracleM1, BC_DIRICHLET, XLO, XHI
+from helpers import make_oracle, small_random_state
+
+
+def test_alpha_limits_and_c7():
+    o = OracleM1(8, 8, 0.125, 0.125, 1.0)
+    UL = [1.0, 0.0, 0.0, 0.0, 0.0]
+    # sigma dx -> 0 : alpha -> 1
+    assert o.face_point(UL, UL, 0)["alpha"] == 1.0
+    # f = 0 on both sides: lambda = +-c/sqrt(3), Eq. 25 reduces to Eq. C.7 alpha = 1/(1 + sqrt(3) sigma dx/2)
+    for sig in (0.1, 3.0, 1e3, 1e6):
+        U = [1.0, 0.0, 0.0, 0.0, sig]
+        a = o.face_point(U, U, 0)["alpha"]
+        assert a == pytest.approx(1.0 / (1.0 + math.sqrt(3.0) * sig * 0.125 / 2.0), rel=1e-14)
+    # Eq. C.10: alpha ~ 2/(sqrt(3) sigma dx) for sigma dx >> 1
+    U = [1.0, 0.0, 0.0, 0.0, 1e9]
+    assert o.face_point(U, U, 0)["alpha"] == pytest.approx(2.0 / (math.sqrt(3.0) * 1e9 * 0.125), rel=1e-7)
+    # sigma_{i+1/2} is the arithmetic mean (Eq. 19); 0 < alpha <= 1
+    f = o.face_point([1.0, 0.3, 0.1, 0.0, 2.0], [2.0, -0.5, 0.2, 0.0, 6.0], 1)
+    assert f["sig"] == 4.0 and 0.0 < f["alpha"] <= 1.0
+    assert f["ap"] + f["am"] == pytest.approx(1.0, abs=1e-15) and f["Lam"] <= 0.0
+
+
+def test_alpha_uses_mean_of_scalar_f_and_1_minus_f2():
+    # Eq. 25 with f_{i+1/2} = (f_i + f_{i+1})/2 of the scalar norms: opposite fluxes do not cancel.
+    o = OracleM1(8, 8, 0.125, 0.125, 1.0)
+    UL, UR = [1.0, 0.6, 0.0, 0.0, 50.0], [1.0, -0.6, 0.0, 0.0, 50.0]
+    fc = o.face_point(UL, UR, 0)
+    expect = 1.0 / (1.0 - 3.0 * 50.0 * 0.125 * (1.0 - 0.36) * fc["Lam"] / 1.0)
+    assert fc["alpha"] == pytest.approx(expect, rel=1e-14)
+    o.set_option("ap_mode", 2)     # Eq. C.8: no (1 - f^2)
+    assert o.face_point(UL, UR, 0)["alpha"] == pytest.approx(1.0 / (1.0 - 3.0 * 50.0 * 0.125 * fc["Lam"]), rel=1e-14)
+    o.set_option("ap_mode", 0)
+    assert o.face_point(UL, UR, 0)["alpha"] == 1.0
+
+
+def test_face_speeds_one_sided_and_degenerate():
+    o = OracleM1(8, 8, 0.125, 0.125, 1.0)
+    # both states stream in +x at f = 1: lambda^- = 0 -> pure upwinding a+ = 1, a- = 0, Lambda = 0
+    U = [1.0, 1.0, 0.0, 0.0, 0.0]
+    f = o.face_point(U, U, 0)
+    assert (f["ap"], f["am"], f["Lam"]) == (1.0, 0.0, 0.0)
+    # the same states seen by a y-face are tangential: lambda^+ = lambda^- = 0 -> guarded (a+ = a- = 1/2, Lambda = 0)
+    f = o.face_point(U, U, 1)
+    assert (f["ap"], f["am"], f["Lam"]) == (0.5, 0.5, 0.0) and f["alpha"] == 1.0
+    # two-sided bounds: the face takes the max/min over both neighbours and 0
+    qL = o.closure_point(1.0, 0.5, 0.0)
+    qR = o.closure_point(1.0, -0.5, 0.0)
+    f = o.face_point([1.0, 0.5, 0.0, 0, 0], [1.0, -0.5, 0.0, 0, 0], 0)
+    lp, lm = max(0, qL["lmax_x"], qR["lmax_x"]), min(0, qL["lmin_x"], qR["lmin_x"])
+    assert f["ap"] == pytest.approx(lp / (lp - lm), rel=1e-15)
+    assert f["Lam"] == pytest.approx(lp * lm / (lp - lm), rel=1e-15)
+    # eigenvalue floor of PAPER.md:426
+    o.set_option("eig_floor", 0.1)
+    f = o.face_point(U, U, 1)
+    assert f["Lam"] == pytest.approx(-0.05, rel=1e-15)
+
+
+def test_uniform_state_is_steady():
+    n = 8
+    w = dict(nx=n, ny=n, dx=1 / n, dy=1 / n, c=1.0, bc=(0, 0, 0, 0), E=np.full((n, n), 2.5), F=np.zeros((2, n, n)),
+             sigma_a=np.zeros((n, n)), sigma_s=np.random.default_rng(0).uniform(0, 100, (n, n)))
+    RE, RF = make_oracle(w).residual()
+    assert np.max(np.abs(RE)) == 0.0 and np.max(np.abs(RF)) < 1e-13
+
+
+def test_explicit_conservation_periodic():
+    # sigma_a = 0, periodic: sum(E) is conserved to round-off; sigma = 0: sum(F) too (telescoping fluxes)
+    w = small_random_state(24, 17, seed=3)
+    w["sigma_a"][:] = 0.0
+    o = make_oracle(w)
+    dt = wl.explicit_dt(w["dx"], w["dy"])
+    E0 = w["E"].sum()
+    for _ in range(5):
+        o.step_explicit(dt)
+    E, F = o.get_state()
+    assert E.sum() == pytest.approx(E0, rel=1e-13)
+    w["sigma_s"][:] = 0.0
+    o = make_oracle(w)
+    for _ in range(5):
+        o.step_explicit(dt)
+    E, F = o.get_state()
+    assert E.sum() == pytest.approx(E0, rel=1e-13)
+    assert F[0].sum() == pytest.approx(w["F"][0].sum(), rel=1e-12, abs=1e-12)
+    assert F[1].sum() == pytest.approx(w["F"][1].sum(), rel=1e-12, abs=1e-12)
+
+
+def test_absorption_decay_rate():
+    # uniform state, F = 0, sigma_a > 0, no T: dE/dt = -c sigma_a E exactly -> forward Euler factor (1 - c sigma_a dt)
+    n = 6
+    w = dict(nx=n, ny=n, dx=1 / n, dy=1 / n, c=2.0, bc=(0, 0, 0, 0), E=np.full((n, n), 3.0), F=np.zeros((2, n, n)),
+             sigma_a=np.full((n, n), 0.7), sigma_s=np.full((n, n), 5.0))
+    o = make_oracle(w)
+    o.step_explicit(0.01)
+    E, F = o.get_state()
+    assert E == pytest.approx(3.0 * (1 - 2.0 * 0.7 * 0.01), rel=1e-15)
+    assert np.max(np.abs(F)) < 1e-14
+
+
+@pytest.mark.parametrize("direction", [0, 1])
+def test_free_streaming_slab_moves_at_c(direction):
+    # sigma = 0, slab with f = 1 along +x (or +y): P = E, lambda = c: first-order upwind advection at speed c.
+    # Sum E and sum F are conserved, so the centroid of E moves by exactly c t (P4).
+    n, m = 200, 4
+    nx, ny = (n, m) if direction == 0 else (m, n)
+    dx = 1.0 / n
+    s = (np.arange(n) + 0.5) * dx
+    prof = np.where((s > 0.2) & (s < 0.3), 1.0, 0.0) + 1e-8
+    E = np.tile(prof, (m, 1)) if direction == 0 else np.tile(prof[:, None], (1, m))
+    F = np.zeros((2, ny, nx))
+    F[direction] = E
+    w = dict(nx=nx, ny=ny, dx=dx, dy=dx, c=1.0, bc=(0, 0, 0, 0), E=E, F=F, sigma_a=np.zeros((ny, nx)), sigma_s=np.zeros((ny, nx)))
+    o = make_oracle(w)
+    dt = 0.4 * dx
+    nsteps = 150
+    for _ in range(nsteps):
+        o.step_explicit(dt)
+    E1, F1 = o.get_state()
+    line0 = prof - 1e-8
+    line1 = (E1[0] if direction == 0 else E1[:, 0]) - 1e-8
+    shift = (line1 * s).sum() / line1.sum() - (line0 * s).sum() / line0.sum()
+    assert shift == pytest.approx(nsteps * dt, abs=1e-6)
+    f = np.hypot(F1[0], F1[1]) / E1
+    assert f.max() <= 1.0 + 1e-12 and E1.min() > 0        # realizability (P7)
+    assert np.max(np.abs(F1[1 - direction])) == 0.0
+
+
+def test_symmetry_gaussian():
+    # config-1 data are symmetric under x<->y and reflections; the explicit scheme must keep that to round-off (P12)
+    w = wl.gaussian_diffusion(32, sigma_s=10.0)
+    o = make_oracle(w)
+    for _ in range(10):
+        o.step_explicit(wl.explicit_dt(w["dx"], w["dy"]))
+    E, F = o.get_state()
+    assert np.max(np.abs(E - E.T)) < 1e-15
+    assert np.max(np.abs(E - E[::-1, :])) < 1e-15 and np.max(np.abs(E - E[:, ::-1])) < 1e-15
+    assert np.max(np.abs(F[0] - F[1].T)) < 1e-15
+    assert np.max(np.abs(F[0] + F[0][:, ::-1])) < 1e-15
+
+
+def _p1_profile(n, sig_line, sg, F0, E_out, dx, c):
+    sig_ext = np.concatenate(([sg[0]], sig_line, [sg[1]]))
+    E_ext = np.empty(n + 2)
+    E_ext[-1] = E_out
+    for k in range(n, -1, -1):
+        E_ext[k] = E_ext[k + 1] + 3.0 * 0.5 * (sig_ext[k] + sig_ext[k + 1]) * dx * F0 / c
+    return E_ext
+
+
+@pytest.mark.parametrize("c", [1.0, 2.5])
+def test_wb_exact_fixed_point_p1(c):
+    # P5(ii): P1 closure, lambda = +-c/sqrt(3), alpha of Eq. C.8  =>  F == F0, E_{i+1} = E_i - 3 sigma_{i+1/2} dx F0/c
+    # is a fixed point to round-off with the WB source (both face relations, Eq. 23 and Eq. C.4, coincide);
+    # the cell-centred source Eq. 16 is NOT steady on it at the opacity jump.
+    n, F0 = 40, 0.1
+    dx = 1.0 / n
+    x = (np.arange(n) + 0.5) * dx
+    sig_line = np.where(x < 0.5, 1.0, 1e3)
+    E_ext = _p1_profile(n, sig_line, (1.0, 1e3), F0, 50.0, dx, c)
+    ny = 3
+    w = dict(nx=n, ny=ny, dx=dx, dy=dx, c=c, bc=(1, 1, 0, 0), E=np.tile(E_ext[1:-1], (ny, 1)),
+             F=np.stack((np.full((ny, n), F0), np.zeros((ny, n)))), sigma_a=np.zeros((ny, n)), sigma_s=np.tile(sig_line, (ny, 1)))
+    one = np.ones(ny)
+    w["ghosts"] = {XLO: (E_ext[0] * one, np.stack((F0 * one, 0 * one)), 0 * one, 1.0 * one),
+                   XHI: (E_ext[-1] * one, np.stack((F0 * one, 0 * one)), 0 * one, 1e3 * one)}
+    opts = dict(closure=1, eig_mode=2, ap_mode=2)
+    RE, RF = make_oracle(w, opts).residual()
+    scale = E_ext.max() * c * c / dx
+    assert np.max(np.abs(RE)) < 1e-14 * scale and np.max(np.abs(RF)) < 1e-14 * scale
+    RE, RF = make_oracle(w, dict(opts, well_balanced=0)).residual()
+    assert np.max(np.abs(RF[0])) > 1.0        # O(c sigma F0) imbalance at the jump without the WB source
+
+
+def test_wb_source_weights_appendix_b():
+    # Eq. B.1: the implicit WB source couples F_j to F_{j-1}, F_j, F_{j+1} with weights
+    # r_{j-1/2}, r_{j-1/2}+r_{j+1/2}, r_{j+1/2}, r = c sigma_face dt/4.  Isolated by differencing the assembled
+    # Fx rows with and without opacity (the hyperbolic part of the F rows does not depend on sigma).
+    n = 7
+    rng = np.random.default_rng(5)
+    w = small_random_state(n, 1, seed=9, dy=1.0)
+    w["sigma_a"][:] = 0.0
+    dt, c = 0.37, 1.0
+    A1, col, _ = make_oracle(w).assemble(dt)
+    w0 = dict(w, sigma_s=np.zeros((1, n)))
+    A0, _, _ = make_oracle(w0).assemble(dt)
+    st = w["sigma_s"][0]
+    for i in range(n):
+        r_w = c * dt * 0.5 * (st[i - 1] + st[i]) / 4
+        r_e = c * dt * 0.5 * (st[i] + st[(i + 1) % n]) / 4
+        d = A1[i] - A0[i]
+        assert d[0, 1, 1] == pytest.approx(r_w + r_e, rel=1e-12)     # centre block, Fx-Fx
+        assert d[1, 1, 1] == pytest.approx(r_w, rel=1e-12)           # west
+        assert d[2, 1, 1] == pytest.approx(r_e, rel=1e-12)           # east
+        assert abs(d[3, 1, 1]) < 1e-13 and abs(d[4, 1, 1]) < 1e-13   # Fx source has no y coupling (dimension by dimension)
+        # |A(k)| <= 1 (Eq. B.7-B.8) for every Fourier mode
+        for k in range(n):
+            ph = 2 * math.pi * k / n
+            amp = 1.0 / (1 + r_w * np.exp(-1j * ph) + r_w + r_e + r_e * np.exp(1j * ph))
+            assert abs(amp) <= 1.0 + 1e-15
