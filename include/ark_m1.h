@@ -1,0 +1,149 @@
+/* ark_m1.h — C ABI of libark_m1.so: the radiative-transfer step of the asymptotic-preserving (AP),
+ * well-balanced (WB) M1 scheme of arXiv 2011.13926 (ARK-RT), hand-written CUDA for NVIDIA B200 (sm_100a), fp64.
+ *
+ * What one handle is: one uniform 2-D grid of nx*ny cells carrying the radiative energy E, the radiative flux
+ * F = (Fx, Fy), the absorption and scattering opacities sigma_a, sigma_s (sigma_t = sigma_a + sigma_s) and,
+ * optionally, a gas temperature T.  PAPER.md:64-69 (Eq. 3) is the system advanced; PAPER.md:142 the grid.
+ *
+ * Layout.  Every field is a row-major plane [ny][nx] of doubles, x fastest.  F = [Fx plane | Fy plane]
+ * (2*nx*ny doubles).  A solver vector is [E | Fx | Fy] (3*nx*ny doubles).
+ *
+ * Pointers.  Every `const double*` / `double*` array argument may be a DEVICE pointer (cudaMalloc, e.g. a
+ * torch tensor's data_ptr()) or a HOST pointer (pinned or pageable): the library copies with
+ * cudaMemcpyAsync(cudaMemcpyDefault) on the handle's stream.  The library never keeps a caller pointer after
+ * the call returns: set_* calls copy in (for pageable host memory the copy has completed on return; for pinned
+ * or device memory it is ordered on the handle's stream, so the caller must not overwrite the source before
+ * that stream reaches it), get_* calls copy out and synchronise the stream before returning.  All device
+ * memory the handle allocates is owned by the handle and freed by ark_m1_destroy.
+ *
+ * Errors.  Functions returning int return 0 (or a non-negative count) on success and a negative ARK_M1_E_*
+ * code on failure; ark_m1_last_error(h) then holds a message.  Non-convergence of the linear solver is NOT an
+ * error (see ark_m1_step_implicit).  No call ever falls back to a CPU computation.
+ *
+ * Threading.  A handle is not thread-safe; different handles are independent.
+ */
+#ifndef ARK_M1_H
+#define ARK_M1_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define ARK_M1_API __attribute__((visibility("default")))
+#else
+#define ARK_M1_API
+#endif
+
+typedef struct ark_m1 ark_m1; /* opaque */
+
+/* Boundary condition of one side (PAPER.md:142 ghost cells; Eq. 24, for the given-state form). */
+enum { ARK_M1_BC_PERIODIC = 0, ARK_M1_BC_DIRICHLET = 1, ARK_M1_BC_OUTFLOW = 2 };
+/* Side indices for ark_m1_set_boundary. */
+enum { ARK_M1_XLO = 0, ARK_M1_XHI = 1, ARK_M1_YLO = 2, ARK_M1_YHI = 3 };
+typedef struct { int xlo, xhi, ylo, yhi; } ark_m1_bc;
+
+/* Error codes. */
+enum {
+    ARK_M1_OK = 0,
+    ARK_M1_E_ARG = -1,      /* bad argument (NULL, dt <= 0, tol <= 0, restart < 1, unknown key, ...) */
+    ARK_M1_E_CUDA = -2,     /* a CUDA runtime call failed (message holds cudaGetErrorString) */
+    ARK_M1_E_ALLOC = -3,    /* device allocation failed */
+    ARK_M1_E_NOTSET = -4,   /* step called before ark_m1_set_state */
+    ARK_M1_E_NONFINITE = -5,/* the solver met a non-finite norm (state or opacity holds NaN/Inf) */
+    ARK_M1_E_UNSUPPORTED = -6
+};
+
+/* Create a solver for an nx*ny grid with cell sizes dx, dy and speed of light c.
+ * bc == NULL means periodic on all sides; periodic must be set on both sides of a direction.
+ * Uses the current CUDA device and the legacy default stream until ark_m1_set_stream.
+ * Returns NULL on bad arguments or when no CUDA device is usable. */
+ARK_M1_API ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_m1_bc* bc);
+ARK_M1_API void    ark_m1_destroy(ark_m1* h);
+
+/* All later work of this handle is enqueued on `cuda_stream` (a cudaStream_t, e.g. torch's current stream). */
+ARK_M1_API int ark_m1_set_stream(ark_m1* h, void* cuda_stream);
+
+/* Copy in the state and the opacities (north_star: ark_m1_set_state(E, F, sigma_a, sigma_s[, T])).
+ * T == NULL: no emission and no matter coupling (pure radiation, dE/dt + div F = -c sigma_a E).
+ * T != NULL: emission c sigma_a a_r T^4 and the matter-energy equation (Eq. 4) are switched on. */
+ARK_M1_API int ark_m1_set_state(ark_m1* h, const double* E, const double* F, const double* sigma_a, const double* sigma_s,
+                     const double* T);
+
+/* One Dirichlet ghost line on `side` (used only where that side's bc is ARK_M1_BC_DIRICHLET): ny values per
+ * array for XLO/XHI, nx values for YLO/YHI; F_g = [Fx line | Fy line].  The ghost cell enters the face fluxes
+ * and the WB source exactly like an interior cell (Eq. 24) and is constant in time. */
+ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const double* F_g, const double* sigma_a_g,
+                        const double* sigma_s_g);
+
+/* Scheme switches (defaults = the paper's scheme):
+ *   "well_balanced" 1: Eqs. 18-19          0: Eq. 16, cell-centred source
+ *   "ap_mode"       1: alpha of Eq. 25         0: alpha = 1 (standard HLL)   2: Eq. C.8
+ *   "eig_mode"      0: Eq. 14                  1: fixed +-c                  2: fixed +-c/sqrt(3)
+ *   "closure"       0: M1 chi(f)                1: P1, chi = 1/3
+ *   "linearisation" 0: analytic pressure Jacobian (Newton)   1: frozen Eddington tensor
+ *   "eig_floor"     x: lambda+ >= x c, lambda- <= -x c; default 0
+ *   "a_r"           radiation constant (default 1)
+ *   "orthogonalisation" 1: one-pass classical Gram-Schmidt (default)   2: CGS2 (re-orthogonalise once)
+ *   "explicit_kernel"   0: one-thread-per-cell kernel   1: row-marching kernel (default)
+ *   "operator"          0: block-stencil (BSR 3x3, pre-multiplied by M^-1) (default)   1: matrix-free coefficient planes
+ * Unknown key or unsupported value: ARK_M1_E_ARG. */
+ARK_M1_API int ark_m1_set_option(ark_m1* h, const char* key, double value);
+
+/* Stage-2 fields, one plane each: "rho_cv" (rho c_v of Eq. 4; default 1), "ux", "uy" (gas velocity of Eq. 6),
+ * "source_E" (constant source added to the E equation).  plane == NULL removes the field. */
+ARK_M1_API int ark_m1_set_field(ark_m1* h, const char* name, const double* plane);
+
+/* Copy out E [nx*ny], F [2*nx*ny] and, if T != NULL and a temperature was set, T [nx*ny].  Synchronises. */
+ARK_M1_API int ark_m1_get_state(ark_m1* h, double* E, double* F, double* T);
+
+/* Explicit step (rows a1-a4 of the hot path): U^{n+1} = U^n - dt R(U^n), R = divergence of the AP HLL fluxes
+ * (Eqs. 12-14, 25) minus the sources (WB Eqs. 18-19 and -c sigma_a E).  One fused
+ * kernel; asynchronous (no host synchronisation).  dt <= 0: ARK_M1_E_ARG. */
+ARK_M1_API int ark_m1_step_explicit(ark_m1* h, double dt);
+
+/* `nsteps` explicit steps of the same dt enqueued back to back (no host work in between). */
+ARK_M1_API int ark_m1_steps_explicit(ark_m1* h, double dt, int nsteps);
+
+/* Implicit step (rows a5-a7): assembles the linearised system (I + dt L_n) U^{n+1} = U^n + affine terms on the
+ * 5-point stencil with 3 unknowns per cell (coefficients frozen at t^n) and solves it with
+ * restarted GMRES(restart), right-preconditioned by the 3x3 block-Jacobi inverse (Eq. 27,
+ * PAPER.md:269-272, taken block-wise), initial guess U^n, stopping when ||b - A x||_2 <= tol ||b||_2 or after
+ * `maxit` inner iterations in total.  Returns the number of inner iterations (>= 0) or a negative error code;
+ * *final_residual (host pointer, may be NULL) receives the TRUE relative residual ||b - A x||/||b|| recomputed
+ * at exit.  Not converging is not an error: the return value is then >= maxit and *final_residual > tol.
+ * Synchronises the stream.  dt <= 0, tol <= 0, restart < 1, maxit < 0: ARK_M1_E_ARG. */
+ARK_M1_API int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual);
+
+/* Step 3 of the operator splitting: explicit addition of the velocity sources of Eq. 6
+ * using the fields "ux", "uy".  ARK_M1_E_NOTSET if they are missing. */
+ARK_M1_API int ark_m1_add_velocity_sources(ark_m1* h, double dt);
+
+/* Guards of PAPER.md:245, 513 (row a7): number of cells with E <= 0 and with |F| > cE.  Synchronises. */
+ARK_M1_API int ark_m1_count_unrealizable(ark_m1* h, long long* n_E_nonpositive, long long* n_f_above_one);
+
+/* R(U^n) of the stored state: RE [nx*ny], RF [2*nx*ny].  Synchronises. */
+ARK_M1_API int ark_m1_residual(ark_m1* h, double* RE, double* RF);
+
+/* out = A V with A = I + dt L_n assembled from the stored state (3*nx*ny doubles each), through the same
+ * assembly and operator kernels the solver uses; b_out (may be NULL) receives the right-hand side. Synchronises. */
+ARK_M1_API int ark_m1_apply_operator(ark_m1* h, double dt, const double* V, double* out, double* b_out);
+
+/* Relative residual history of the last implicit solve: entry 0 = true residual of the initial guess, then one
+ * estimate per inner iteration.  Copies min(cap, n) values into buf (host) and returns n. */
+ARK_M1_API int ark_m1_get_history(ark_m1* h, double* buf, int cap);
+
+/* Timings of the last implicit solve in milliseconds (CUDA events on the handle's stream):
+ * out[0] = assembly, out[1] = Krylov iterations (everything after assembly), out[2] = total. */
+ARK_M1_API int ark_m1_get_timings(ark_m1* h, double* out3);
+
+/* Device bytes currently allocated by the handle. */
+ARK_M1_API long long ark_m1_device_bytes(const ark_m1* h);
+
+ARK_M1_API const char* ark_m1_last_error(const ark_m1* h);
+ARK_M1_API const char* ark_m1_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARK_M1_H */

@@ -1,0 +1,213 @@
+"""Thin ctypes binding of libark_m1.so (include/ark_m1.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/.  There is no CPU fallback: if the shared library is
+missing or cannot be loaded this module raises.  torch is used only for device memory and streams; array
+arguments may be torch tensors (cuda or cpu, float64, contiguous) or numpy float64 arrays — their raw pointers
+are passed straight to the C ABI, which accepts host and device pointers alike.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libark_m1.so")
+
+BC_PERIODIC, BC_DIRICHLET, BC_OUTFLOW = 0, 1, 2
+XLO, XHI, YLO, YHI = 0, 1, 2, 3
+
+# every symbol include/ark_m1.h declares
+SYMBOLS = [
+    "ark_m1_create", "ark_m1_destroy", "ark_m1_set_stream", "ark_m1_set_state", "ark_m1_set_boundary",
+    "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
+    "ark_m1_step_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
+    "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_device_bytes",
+    "ark_m1_last_error", "ark_m1_version",
+]
+
+
+class ArkBc(C.Structure):
+    _fields_ = [("xlo", C.c_int), ("xhi", C.c_int), ("ylo", C.c_int), ("yhi", C.c_int)]
+
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH):
+    """dlopen libark_m1.so and declare the prototypes.  Raises if the library is missing (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} not found: build it with `python -m paper_2011_13926_b200.build` "
+                           "(the CUDA library is the only implementation; there is no CPU fallback)")
+    L = C.CDLL(path)
+    vp, dp, d, i = C.c_void_p, C.c_void_p, C.c_double, C.c_int   # array pointers are passed as raw addresses
+    L.ark_m1_create.restype = vp
+    L.ark_m1_create.argtypes = [i, i, d, d, d, C.POINTER(ArkBc)]
+    L.ark_m1_destroy.restype = None
+    L.ark_m1_destroy.argtypes = [vp]
+    L.ark_m1_set_stream.argtypes = [vp, vp]
+    L.ark_m1_set_state.argtypes = [vp, dp, dp, dp, dp, dp]
+    L.ark_m1_set_boundary.argtypes = [vp, i, dp, dp, dp, dp]
+    L.ark_m1_set_option.argtypes = [vp, C.c_char_p, d]
+    L.ark_m1_set_field.argtypes = [vp, C.c_char_p, dp]
+    L.ark_m1_get_state.argtypes = [vp, dp, dp, dp]
+    L.ark_m1_step_explicit.argtypes = [vp, d]
+    L.ark_m1_steps_explicit.argtypes = [vp, d, i]
+    L.ark_m1_step_implicit.argtypes = [vp, d, d, i, i, C.POINTER(C.c_double)]
+    L.ark_m1_add_velocity_sources.argtypes = [vp, d]
+    L.ark_m1_count_unrealizable.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    L.ark_m1_residual.argtypes = [vp, dp, dp]
+    L.ark_m1_apply_operator.argtypes = [vp, d, dp, dp, dp]
+    L.ark_m1_get_history.argtypes = [vp, C.POINTER(C.c_double), i]
+    L.ark_m1_get_timings.argtypes = [vp, C.POINTER(C.c_double)]
+    L.ark_m1_device_bytes.restype = C.c_longlong
+    L.ark_m1_device_bytes.argtypes = [vp]
+    L.ark_m1_last_error.restype = C.c_char_p
+    L.ark_m1_last_error.argtypes = [vp]
+    L.ark_m1_version.restype = C.c_char_p
+    L.ark_m1_version.argtypes = []
+    for name in SYMBOLS:
+        getattr(L, name)
+    _lib = L
+    return L
+
+
+def _ptr(a, nelem=None):
+    """Raw address of a float64 contiguous torch tensor / numpy array (None -> NULL).  Returns (address, keepalive)."""
+    if a is None:
+        return None, None
+    try:
+        import torch
+    except ImportError:  # numpy-only callers
+        torch = None
+    if torch is not None and isinstance(a, torch.Tensor):
+        if a.dtype != torch.float64 or not a.is_contiguous():
+            raise TypeError("tensor arguments must be contiguous float64")
+        if nelem is not None and a.numel() != nelem:
+            raise ValueError(f"expected {nelem} elements, got {a.numel()}")
+        return a.data_ptr(), a
+    arr = np.ascontiguousarray(a, dtype=np.float64)
+    if nelem is not None and arr.size != nelem:
+        raise ValueError(f"expected {nelem} elements, got {arr.size}")
+    return arr.ctypes.data, arr
+
+
+class ArkM1:
+    """One solver handle.  Method names follow include/ark_m1.h without the ark_m1_ prefix."""
+
+    def __init__(self, nx, ny, dx, dy, c=1.0, bc=(0, 0, 0, 0), stream=None):
+        self._L = load_library()
+        self.nx, self.ny, self.dx, self.dy, self.c = int(nx), int(ny), float(dx), float(dy), float(c)
+        self.bc = tuple(int(b) for b in bc)
+        b = ArkBc(*self.bc)
+        self._h = self._L.ark_m1_create(self.nx, self.ny, self.dx, self.dy, self.c, C.byref(b))
+        if not self._h:
+            raise ValueError("ark_m1_create failed (bad arguments or no CUDA device)")
+        if stream is not None:
+            self.set_stream(stream)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.ark_m1_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _check(self, rc):
+        if rc < 0:
+            raise RuntimeError(f"ark_m1 error {rc}: {self._L.ark_m1_last_error(self._h).decode()}")
+        return rc
+
+    @property
+    def N(self):
+        return self.nx * self.ny
+
+    def set_stream(self, stream):
+        """stream: a torch.cuda.Stream, or a raw cudaStream_t address."""
+        addr = getattr(stream, "cuda_stream", stream)
+        self._check(self._L.ark_m1_set_stream(self._h, C.c_void_p(addr)))
+
+    def set_state(self, E, F, sigma_a, sigma_s, T=None):
+        N = self.N
+        pe, k0 = _ptr(E, N); pf, k1 = _ptr(F, 2 * N); pa, k2 = _ptr(sigma_a, N); ps, k3 = _ptr(sigma_s, N); pt, k4 = _ptr(T, N)
+        self._check(self._L.ark_m1_set_state(self._h, pe, pf, pa, ps, pt))
+        self._keep = (k0, k1, k2, k3, k4)   # sources of asynchronous copies stay alive until the next call
+
+    def set_boundary(self, side, E_g, F_g, sigma_a_g, sigma_s_g):
+        n = self.ny if side < 2 else self.nx
+        pe, k0 = _ptr(E_g, n); pf, k1 = _ptr(F_g, 2 * n); pa, k2 = _ptr(sigma_a_g, n); ps, k3 = _ptr(sigma_s_g, n)
+        self._check(self._L.ark_m1_set_boundary(self._h, int(side), pe, pf, pa, ps))
+        self._keep_b = getattr(self, "_keep_b", []) + [(k0, k1, k2, k3)]
+
+    def set_option(self, key, value):
+        self._check(self._L.ark_m1_set_option(self._h, key.encode(), float(value)))
+
+    def set_field(self, name, plane):
+        p, k = _ptr(plane, self.N)
+        self._check(self._L.ark_m1_set_field(self._h, name.encode(), p))
+        self._keep_f = getattr(self, "_keep_f", []) + [k]
+
+    def get_state(self, with_T=False, out=None):
+        """Returns numpy arrays E[ny,nx], F[2,ny,nx] (and T) unless `out` = (E, F[, T]) buffers are given."""
+        if out is None:
+            E = np.empty((self.ny, self.nx)); F = np.empty((2, self.ny, self.nx))
+            T = np.empty((self.ny, self.nx)) if with_T else None
+        else:
+            E, F = out[0], out[1]
+            T = out[2] if len(out) > 2 else None
+        pe, _ = _ptr(E, self.N); pf, _ = _ptr(F, 2 * self.N); pt, _ = _ptr(T, self.N)
+        self._check(self._L.ark_m1_get_state(self._h, pe, pf, pt))
+        return (E, F, T) if (with_T or (out is not None and len(out) > 2)) else (E, F)
+
+    def step_explicit(self, dt):
+        self._check(self._L.ark_m1_step_explicit(self._h, float(dt)))
+
+    def steps_explicit(self, dt, nsteps):
+        self._check(self._L.ark_m1_steps_explicit(self._h, float(dt), int(nsteps)))
+
+    def step_implicit(self, dt, tol=1e-10, restart=30, maxit=4000):
+        res = C.c_double(0.0)
+        its = self._check(self._L.ark_m1_step_implicit(self._h, float(dt), float(tol), int(restart), int(maxit), C.byref(res)))
+        return its, res.value
+
+    def add_velocity_sources(self, dt):
+        self._check(self._L.ark_m1_add_velocity_sources(self._h, float(dt)))
+
+    def count_unrealizable(self):
+        a, b = C.c_longlong(0), C.c_longlong(0)
+        self._check(self._L.ark_m1_count_unrealizable(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def residual(self):
+        RE = np.empty((self.ny, self.nx)); RF = np.empty((2, self.ny, self.nx))
+        self._check(self._L.ark_m1_residual(self._h, RE.ctypes.data, RF.ctypes.data))
+        return RE, RF
+
+    def apply_operator(self, dt, V, with_b=False):
+        p, keep = _ptr(V, 3 * self.N)
+        out = np.empty((3, self.ny, self.nx))
+        b = np.empty((3, self.ny, self.nx)) if with_b else None
+        self._check(self._L.ark_m1_apply_operator(self._h, float(dt), p, out.ctypes.data, None if b is None else b.ctypes.data))
+        return (out, b) if with_b else out
+
+    def history(self):
+        n = self._L.ark_m1_get_history(self._h, None, 0)
+        buf = (C.c_double * max(n, 1))()
+        self._L.ark_m1_get_history(self._h, buf, n)
+        return np.array(buf[:n])
+
+    def timings(self):
+        buf = (C.c_double * 3)()
+        self._check(self._L.ark_m1_get_timings(self._h, buf))
+        return dict(assembly_ms=buf[0], krylov_ms=buf[1], total_ms=buf[2])
+
+    def device_bytes(self):
+        return int(self._L.ark_m1_device_bytes(self._h))
+
+
+def version():
+    return load_library().ark_m1_version().decode()

@@ -1,0 +1,462 @@
+// ark_m1_api.cu — the C ABI of include/ark_m1.h: handle, device memory, step drivers.
+// Host logic only; every arithmetic step of the path runs in the kernels of this directory.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+#include "../../include/ark_m1.h"
+#include "ark_m1_internal.h"
+
+using namespace ark;
+
+struct ark_m1 {
+    Grid g;
+    Scheme s;
+    cudaStream_t st;
+    int device, sm_count;
+    long long N;
+    long long bytes;
+    bool have_state, have_T;
+    // state: two buffers of 3N doubles [E | Fx | Fy]; U[cur] is current
+    double* U[2];
+    int cur;
+    double *sa, *ss_tmp, *stot, *T[2];
+    double* gh[4][5];
+    double *rho_cv, *ux, *uy, *source_E;
+    unsigned long long* counts;   // 2
+    // options
+    int ortho, explicit_kernel, op_kind;
+    // implicit workspace (lazy)
+    BlockMatrix A;
+    double* V;         // (m+1) vectors of `stride` doubles
+    double* tvec;      // 3N
+    long long stride;
+    int m_alloc, maxit_alloc;
+    GmresWork W;
+    void* wblock;      // allocation behind W
+    GmresCtl* ctl_host;  // pinned
+    std::vector<double>* hist_host;
+    cudaEvent_t ev[3];
+    double timings[3];
+    char err[512];
+};
+
+static int fail(ark_m1* h, int code, const char* fmt, const char* detail)
+{
+    if (h) snprintf(h->err, sizeof h->err, fmt, detail ? detail : "");
+    return code;
+}
+#define CU(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(h, ARK_M1_E_CUDA, #call ": %s", cudaGetErrorString(e__)); } while (0)
+
+static int dmalloc(ark_m1* h, void** p, size_t bytes)
+{
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return fail(h, ARK_M1_E_ALLOC, "cudaMalloc: %s", cudaGetErrorString(e)); }
+    h->bytes += (long long)bytes;
+    return 0;
+}
+
+static Fields fields_of(const ark_m1* h)
+{
+    Fields f;
+    const double* U = h->U[h->cur];
+    f.E = U; f.Fx = U + h->N; f.Fy = U + 2 * h->N; f.sa = h->sa; f.st = h->stot;
+    for (int s = 0; s < 4; ++s) for (int k = 0; k < 5; ++k) f.gh[s][k] = h->gh[s][k];
+    f.T = h->have_T ? h->T[h->cur] : nullptr;
+    f.rho_cv = h->rho_cv; f.source_E = h->source_E;
+    return f;
+}
+
+extern "C" {
+
+const char* ark_m1_version(void) { return "ark_m1 0.1 (sm_100a, fp64)"; }
+
+ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_m1_bc* bc)
+{
+    if (nx < 1 || ny < 1 || !(dx > 0) || !(dy > 0) || !(c > 0)) return nullptr;
+    int b[4] = { 0, 0, 0, 0 };
+    if (bc) { b[0] = bc->xlo; b[1] = bc->xhi; b[2] = bc->ylo; b[3] = bc->yhi; }
+    for (int s = 0; s < 4; ++s) if (b[s] < 0 || b[s] > 2) return nullptr;
+    if ((b[0] == BC_PERIODIC) != (b[1] == BC_PERIODIC) || (b[2] == BC_PERIODIC) != (b[3] == BC_PERIODIC)) return nullptr;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    ark_m1* h = new (std::nothrow) ark_m1;
+    if (!h) return nullptr;
+    memset(h, 0, sizeof *h);
+    h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
+    for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
+    h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0;
+    h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 0;
+    h->device = dev; h->N = (long long)nx * ny; h->st = 0;
+    cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    h->hist_host = new std::vector<double>();
+    const size_t N = (size_t)h->N;
+    bool ok = true;
+    for (int k = 0; k < 2 && ok; ++k) ok = dmalloc(h, (void**)&h->U[k], 3 * N * sizeof(double)) == 0;
+    ok = ok && dmalloc(h, (void**)&h->sa, N * sizeof(double)) == 0;
+    ok = ok && dmalloc(h, (void**)&h->ss_tmp, N * sizeof(double)) == 0;
+    ok = ok && dmalloc(h, (void**)&h->stot, N * sizeof(double)) == 0;
+    ok = ok && dmalloc(h, (void**)&h->counts, 2 * sizeof(unsigned long long)) == 0;
+    for (int s = 0; s < 4 && ok; ++s) {
+        const size_t len = (s < 2) ? ny : nx;
+        for (int k = 0; k < 5 && ok; ++k) {
+            ok = dmalloc(h, (void**)&h->gh[s][k], len * sizeof(double)) == 0;
+            if (ok) cudaMemset(h->gh[s][k], 0, len * sizeof(double));
+        }
+    }
+    ok = ok && cudaMallocHost((void**)&h->ctl_host, sizeof(GmresCtl)) == cudaSuccess;
+    for (int k = 0; k < 3 && ok; ++k) ok = cudaEventCreate(&h->ev[k]) == cudaSuccess;
+    if (!ok) { ark_m1_destroy(h); return nullptr; }
+    return h;
+}
+
+static void free_implicit(ark_m1* h)
+{
+    cudaFree(h->A.off); cudaFree(h->A.C); cudaFree(h->A.Minv); cudaFree(h->A.b); cudaFree(h->V); cudaFree(h->tvec); cudaFree(h->wblock);
+    h->A.off = h->A.C = h->A.Minv = h->A.b = nullptr; h->V = h->tvec = nullptr; h->wblock = nullptr; h->m_alloc = 0;
+}
+
+void ark_m1_destroy(ark_m1* h)
+{
+    if (!h) return;
+    cudaStreamSynchronize(h->st);
+    for (int k = 0; k < 2; ++k) { cudaFree(h->U[k]); cudaFree(h->T[k]); }
+    cudaFree(h->sa); cudaFree(h->ss_tmp); cudaFree(h->stot); cudaFree(h->counts);
+    for (int s = 0; s < 4; ++s) for (int k = 0; k < 5; ++k) cudaFree(h->gh[s][k]);
+    cudaFree(h->rho_cv); cudaFree(h->ux); cudaFree(h->uy); cudaFree(h->source_E);
+    free_implicit(h);
+    if (h->ctl_host) cudaFreeHost(h->ctl_host);
+    for (int k = 0; k < 3; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
+    delete h->hist_host;
+    cudaGetLastError();
+    delete h;
+}
+
+int ark_m1_set_stream(ark_m1* h, void* cuda_stream)
+{
+    if (!h) return ARK_M1_E_ARG;
+    CU(cudaStreamSynchronize(h->st));
+    h->st = (cudaStream_t)cuda_stream;
+    return 0;
+}
+
+int ark_m1_set_state(ark_m1* h, const double* E, const double* F, const double* sigma_a, const double* sigma_s, const double* T)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!E || !F || !sigma_a || !sigma_s) return fail(h, ARK_M1_E_ARG, "set_state: NULL array%s", "");
+    const size_t N = (size_t)h->N, B = N * sizeof(double);
+    double* U = h->U[h->cur];
+    CU(cudaMemcpyAsync(U, E, B, cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(U + N, F, 2 * B, cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(h->sa, sigma_a, B, cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(h->ss_tmp, sigma_s, B, cudaMemcpyDefault, h->st));
+    CU(launch_add_planes(h->stot, h->sa, h->ss_tmp, (long long)N, h->st));
+    if (T) {
+        for (int k = 0; k < 2; ++k) if (!h->T[k]) { int rc = dmalloc(h, (void**)&h->T[k], B); if (rc) return rc; }
+        CU(cudaMemcpyAsync(h->T[h->cur], T, B, cudaMemcpyDefault, h->st));
+    }
+    h->have_T = (T != nullptr);
+    h->have_state = true;
+    return 0;
+}
+
+int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const double* F_g, const double* sa_g, const double* ss_g)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (side < 0 || side > 3 || !E_g || !F_g || !sa_g || !ss_g) return fail(h, ARK_M1_E_ARG, "set_boundary: bad argument%s", "");
+    const size_t len = (side < 2) ? h->g.ny : h->g.nx, B = len * sizeof(double);
+    CU(cudaMemcpyAsync(h->gh[side][0], E_g, B, cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(h->gh[side][1], F_g, B, cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(h->gh[side][2], F_g + len, B, cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(h->gh[side][3], sa_g, B, cudaMemcpyDefault, h->st));
+    // sigma_t ghost = sigma_a + sigma_s: stage sigma_s in the sigma_t line, then add in place
+    CU(cudaMemcpyAsync(h->gh[side][4], ss_g, B, cudaMemcpyDefault, h->st));
+    CU(launch_add_planes(h->gh[side][4], h->gh[side][3], h->gh[side][4], (long long)len, h->st));
+    return 0;
+}
+
+int ark_m1_set_option(ark_m1* h, const char* key, double value)
+{
+    if (!h || !key) return ARK_M1_E_ARG;
+    const int iv = (int)value;
+    if (!strcmp(key, "well_balanced")) h->s.wb = (value != 0.0);
+    else if (!strcmp(key, "ap_mode")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "ap_mode must be 0, 1 or 2%s", ""); h->s.ap = iv; }
+    else if (!strcmp(key, "eig_mode")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "eig_mode must be 0, 1 or 2%s", ""); h->s.eig = iv; }
+    else if (!strcmp(key, "closure")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "closure must be 0 or 1%s", ""); h->s.closure = iv; }
+    else if (!strcmp(key, "linearisation")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "linearisation must be 0 or 1%s", ""); h->s.lin = iv; }
+    else if (!strcmp(key, "eig_floor")) { if (!(value >= 0.0)) return fail(h, ARK_M1_E_ARG, "eig_floor must be >= 0%s", ""); h->s.eig_floor = value; }
+    else if (!strcmp(key, "a_r")) h->s.a_r = value;
+    else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
+    else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0 or 1%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "operator")) { if (iv != 0) return fail(h, ARK_M1_E_ARG, "operator: only 0 (block-stencil) is built%s", ""); h->op_kind = iv; }
+    else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
+    return 0;
+}
+
+int ark_m1_set_field(ark_m1* h, const char* name, const double* plane)
+{
+    if (!h || !name) return ARK_M1_E_ARG;
+    double** dst = nullptr;
+    if (!strcmp(name, "rho_cv")) dst = &h->rho_cv; else if (!strcmp(name, "ux")) dst = &h->ux;
+    else if (!strcmp(name, "uy")) dst = &h->uy; else if (!strcmp(name, "source_E")) dst = &h->source_E;
+    else return fail(h, ARK_M1_E_ARG, "unknown field %s", name);
+    const size_t B = (size_t)h->N * sizeof(double);
+    if (!plane) { CU(cudaStreamSynchronize(h->st)); if (*dst) { cudaFree(*dst); h->bytes -= (long long)B; } *dst = nullptr; return 0; }
+    if (!*dst) { int rc = dmalloc(h, (void**)dst, B); if (rc) return rc; }
+    CU(cudaMemcpyAsync(*dst, plane, B, cudaMemcpyDefault, h->st));
+    return 0;
+}
+
+int ark_m1_get_state(ark_m1* h, double* E, double* F, double* T)
+{
+    if (!h || !E || !F) return ARK_M1_E_ARG;
+    const size_t N = (size_t)h->N, B = N * sizeof(double);
+    const double* U = h->U[h->cur];
+    CU(cudaMemcpyAsync(E, U, B, cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(F, U + N, 2 * B, cudaMemcpyDefault, h->st));
+    if (T && h->have_T) CU(cudaMemcpyAsync(T, h->T[h->cur], B, cudaMemcpyDefault, h->st));
+    CU(cudaStreamSynchronize(h->st));
+    return 0;
+}
+
+static int explicit_once(ark_m1* h, double dt)
+{
+    const Fields f = fields_of(h);
+    double* O = h->U[h->cur ^ 1];
+    const bool plain = !h->have_T && !h->source_E;
+    if (h->explicit_kernel == 1 && plain) {
+        CU(launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
+    } else {
+        CU(launch_explicit_cell(h->g, h->s, f, dt, 0, O, O + h->N, O + 2 * h->N, h->have_T ? h->T[h->cur ^ 1] : nullptr, h->st));
+    }
+    h->cur ^= 1;
+    return 0;
+}
+
+int ark_m1_step_explicit(ark_m1* h, double dt)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "step_explicit: dt must be > 0%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_explicit: no state set%s", "");
+    return explicit_once(h, dt);
+}
+
+int ark_m1_steps_explicit(ark_m1* h, double dt, int nsteps)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!(dt > 0.0) || nsteps < 0) return fail(h, ARK_M1_E_ARG, "steps_explicit: dt must be > 0 and nsteps >= 0%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "steps_explicit: no state set%s", "");
+    for (int k = 0; k < nsteps; ++k) { int rc = explicit_once(h, dt); if (rc) return rc; }
+    return 0;
+}
+
+int ark_m1_residual(ark_m1* h, double* RE, double* RF)
+{
+    if (!h || !RE || !RF) return ARK_M1_E_ARG;
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "residual: no state set%s", "");
+    const Fields f = fields_of(h);
+    double* O = h->U[h->cur ^ 1];
+    const size_t N = (size_t)h->N;
+    CU(launch_explicit_cell(h->g, h->s, f, 0.0, 1, O, O + N, O + 2 * N, nullptr, h->st));
+    CU(cudaMemcpyAsync(RE, O, N * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(RF, O + N, 2 * N * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(cudaStreamSynchronize(h->st));
+    return 0;
+}
+
+int ark_m1_add_velocity_sources(ark_m1* h, double dt)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!h->have_state || !h->ux || !h->uy) return fail(h, ARK_M1_E_NOTSET, "add_velocity_sources: state, ux, uy must be set%s", "");
+    const Fields f = fields_of(h);
+    double* U = h->U[h->cur];
+    CU(launch_velocity_sources(h->g, h->s, f, h->ux, h->uy, dt, U, U + h->N, U + 2 * h->N, h->st));
+    return 0;
+}
+
+int ark_m1_count_unrealizable(ark_m1* h, long long* nE, long long* nf)
+{
+    if (!h || !nE || !nf) return ARK_M1_E_ARG;
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "count_unrealizable: no state set%s", "");
+    CU(cudaMemsetAsync(h->counts, 0, 2 * sizeof(unsigned long long), h->st));
+    CU(launch_count_unrealizable(h->g, fields_of(h), h->counts, h->st));
+    unsigned long long out[2];
+    CU(cudaMemcpyAsync(out, h->counts, sizeof out, cudaMemcpyDeviceToHost, h->st));
+    CU(cudaStreamSynchronize(h->st));
+    *nE = (long long)out[0]; *nf = (long long)out[1];
+    return 0;
+}
+
+long long ark_m1_device_bytes(const ark_m1* h) { return h ? h->bytes : 0; }
+const char* ark_m1_last_error(const ark_m1* h) { return h ? h->err : "null handle"; }
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------
+// Implicit step
+// ---------------------------------------------------------------------------------------------------------
+static int ensure_implicit(ark_m1* h, int m, int maxit)
+{
+    const size_t N = (size_t)h->N, n = 3 * N;
+    if (h->m_alloc >= m && h->maxit_alloc >= maxit) return 0;
+    CU(cudaStreamSynchronize(h->st));
+    const long long before = h->bytes;
+    (void)before;
+    if (h->A.off == nullptr) {
+        int rc;
+        if ((rc = dmalloc(h, (void**)&h->A.off, 36 * N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->A.C, 9 * N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->A.Minv, 9 * N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->A.b, n * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->tvec, n * sizeof(double)))) return rc;
+    }
+    h->stride = (long long)((n + 31) / 32 * 32);
+    if (h->m_alloc < m) {
+        if (h->V) { cudaFree(h->V); h->bytes -= (long long)((size_t)(h->m_alloc + 1) * h->stride * sizeof(double)); h->V = nullptr; }
+        int rc = dmalloc(h, (void**)&h->V, (size_t)(m + 1) * h->stride * sizeof(double));
+        if (rc) { h->m_alloc = 0; return rc; }
+    }
+    const int mm = m > h->m_alloc ? m : h->m_alloc;
+    const int mi = maxit > h->maxit_alloc ? maxit : h->maxit_alloc;
+    // small block: ctl | H | cs | sn | g | y | scale | coef | hist | partial
+    if (h->wblock) { cudaFree(h->wblock); h->wblock = nullptr; }
+    const int caphist = mi + mi / (mm > 0 ? mm : 1) + 8;
+    const size_t nd = (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 2 * (size_t)(mm + 1) + caphist
+                      + (size_t)krylov_max_blocks(h->sm_count) * MAXV;
+    const size_t ctl_bytes = (sizeof(GmresCtl) + 255) / 256 * 256;
+    if (cudaMalloc(&h->wblock, ctl_bytes + nd * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(h, ARK_M1_E_ALLOC, "cudaMalloc (solver scalars)%s", ""); }
+    CU(cudaMemset(h->wblock, 0, ctl_bytes + nd * sizeof(double)));
+    GmresWork& W = h->W;
+    W.ctl = (GmresCtl*)h->wblock;
+    double* p = (double*)((char*)h->wblock + ctl_bytes);
+    W.H = p; p += (size_t)(mm + 1) * mm;
+    W.cs = p; p += mm; W.sn = p; p += mm; W.g = p; p += mm + 1; W.y = p; p += mm;
+    W.scale = p; p += mm + 1; W.coef = p; p += mm + 1; W.hist = p; p += caphist; W.partial = p;
+    W.caphist = caphist;
+    h->m_alloc = mm; h->maxit_alloc = mi;
+    return 0;
+}
+
+// V0 <- b - A x  (A x = Ahat (C x)), then its norm with the DOT_RNORM epilogue.
+static int true_residual(ark_m1* h, const double* x)
+{
+    const long long n = 3 * h->N;
+    CU(launch_diag_mul(h->g, h->A.C, x, h->tvec, h->st));
+    CU(launch_spmv_hat(h->g, h->A.off, h->tvec, h->V, nullptr, h->A.b, -1.0, nullptr, h->st));
+    CU(launch_multi_dot(h->V, h->V, h->stride, 1, 0, n, h->W, DOT_RNORM, h->sm_count, h->st));
+    return 0;
+}
+
+static int fetch_ctl(ark_m1* h)
+{
+    CU(cudaMemcpyAsync(h->ctl_host, h->W.ctl, sizeof(GmresCtl), cudaMemcpyDeviceToHost, h->st));
+    CU(cudaStreamSynchronize(h->st));
+    return 0;
+}
+
+static int assemble_system(ark_m1* h, double dt)
+{
+    const Fields f = fields_of(h);
+    CU(launch_assemble(h->g, h->s, f, dt, h->A, h->st));
+    CU(launch_scale_offdiag(h->g, h->A, h->st));
+    return 0;
+}
+
+extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit: no state set%s", "");
+    int rc = ensure_implicit(h, restart, maxit);
+    if (rc) return rc;
+    const int m = restart;
+    const long long n = 3 * h->N, S = h->stride;
+    const int sm = h->sm_count;
+    double* x = h->U[h->cur];          // initial guess U^n, solution in place
+    GmresWork W = h->W;
+    const int* stop = &W.ctl->inner_stop;
+
+    CU(cudaEventRecord(h->ev[0], h->st));
+    if ((rc = assemble_system(h, dt))) return rc;
+    CU(cudaEventRecord(h->ev[1], h->st));
+    CU(launch_begin_solve(W, tol, m, maxit, h->st));
+    CU(launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
+    if ((rc = true_residual(h, x))) return rc;
+    if ((rc = fetch_ctl(h))) return rc;
+    while (!h->ctl_host->inner_stop) {
+        for (int j = 0; j < m; ++j) {
+            double* w = h->V + (size_t)(j + 1) * S;
+            CU(launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
+            for (int pass = 0; pass < h->ortho; ++pass) {
+                for (int c0 = 0; c0 <= j; c0 += MAXV) {
+                    const int nv = (j + 1 - c0) < MAXV ? (j + 1 - c0) : MAXV;
+                    CU(launch_multi_dot(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, pass == 0 ? DOT_H : DOT_H2, sm, h->st));
+                }
+                for (int c0 = 0; c0 <= j; c0 += MAXV) {
+                    const int nv = (j + 1 - c0) < MAXV ? (j + 1 - c0) : MAXV;
+                    const int last = (c0 + MAXV > j) && (pass == h->ortho - 1);
+                    CU(launch_update(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, last, sm, h->st));
+                }
+            }
+        }
+        CU(launch_solve_y(W, h->st));
+        CU(launch_combine(h->g, h->V, S, h->A.Minv, x, W, sm, h->st));
+        if ((rc = true_residual(h, x))) return rc;
+        if ((rc = fetch_ctl(h))) return rc;
+    }
+    CU(cudaEventRecord(h->ev[2], h->st));
+    const GmresCtl c = *h->ctl_host;
+    // history
+    const int nh = c.nhist < W.caphist ? c.nhist : W.caphist;
+    h->hist_host->assign((size_t)nh, 0.0);
+    if (nh > 0) CU(cudaMemcpyAsync(h->hist_host->data(), W.hist, (size_t)nh * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (h->have_T && !c.nonfinite) {
+        CU(launch_matter_update(h->g, h->s, dt, h->sa, h->rho_cv, x, h->T[h->cur], h->st));
+    }
+    CU(cudaStreamSynchronize(h->st));
+    float ms01 = 0, ms12 = 0;
+    cudaEventElapsedTime(&ms01, h->ev[0], h->ev[1]); cudaEventElapsedTime(&ms12, h->ev[1], h->ev[2]);
+    h->timings[0] = ms01; h->timings[1] = ms12; h->timings[2] = (double)ms01 + ms12;
+    if (c.nonfinite) return fail(h, ARK_M1_E_NONFINITE, "step_implicit: non-finite norm in the solver (state or opacity holds NaN/Inf?)%s", "");
+    if (final_residual) *final_residual = (c.bnorm > 0.0) ? c.rnorm / c.bnorm : c.rnorm;
+    return c.its;
+}
+
+extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, double* out, double* b_out)
+{
+    if (!h || !Vin || !out) return ARK_M1_E_ARG;
+    if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "apply_operator: dt must be > 0%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "apply_operator: no state set%s", "");
+    int rc = ensure_implicit(h, 1, 1);
+    if (rc) return rc;
+    const size_t n = 3 * (size_t)h->N;
+    if ((rc = assemble_system(h, dt))) return rc;
+    double* vin = h->V;                       // slot 0 as staging for the input, slot 1 for the output
+    double* vout = h->V + h->stride;
+    CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(launch_diag_mul(h->g, h->A.C, vin, h->tvec, h->st));
+    CU(launch_spmv_hat(h->g, h->A.off, h->tvec, vout, nullptr, nullptr, 1.0, nullptr, h->st));
+    CU(cudaMemcpyAsync(out, vout, n * sizeof(double), cudaMemcpyDefault, h->st));
+    if (b_out) CU(cudaMemcpyAsync(b_out, h->A.b, n * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(cudaStreamSynchronize(h->st));
+    return 0;
+}
+
+extern "C" int ark_m1_get_history(ark_m1* h, double* buf, int cap)
+{
+    if (!h) return ARK_M1_E_ARG;
+    const int n = (int)h->hist_host->size();
+    if (buf) for (int k = 0; k < n && k < cap; ++k) buf[k] = (*h->hist_host)[k];
+    return n;
+}
+
+extern "C" int ark_m1_get_timings(ark_m1* h, double* out3)
+{
+    if (!h || !out3) return ARK_M1_E_ARG;
+    for (int k = 0; k < 3; ++k) out3[k] = h->timings[k];
+    return 0;
+}

@@ -1,0 +1,91 @@
+// ark_m1_internal.h — handle layout and kernel launchers shared by the .cu files of libark_m1.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "m1_device.cuh"
+
+namespace ark {
+
+// ---------------------------------------------------------------------------------------------------------
+// Device-resident control block of one GMRES solve.  Every Krylov kernel reads it; the "last block done"
+// epilogues of the reduction kernels update it, so that a whole restart cycle is enqueued without a host
+// round trip.
+// ---------------------------------------------------------------------------------------------------------
+struct GmresCtl {
+    double bnorm, target, rnorm;   // ||b||, tol*||b||, last TRUE residual norm
+    double est;                    // last residual estimate |g_{j+1}|
+    int m, maxit;
+    int its;                       // inner iterations so far (all cycles)
+    int j;                         // inner iterations in the current cycle
+    int inner_stop;                // 1: skip the remaining inner kernels of this cycle
+    int converged;                 // 1: true residual <= target
+    int nonfinite;                 // 1: a norm was NaN/Inf
+    int nhist;
+    unsigned int ticket;           // "last block" counter of the reduction kernels
+    int pad;
+};
+
+struct GmresWork {                 // device pointers into one small allocation
+    GmresCtl* ctl;
+    double* H;      // (m+1) x m, row-major H[i*m + j]
+    double* cs;     // m
+    double* sn;     // m
+    double* g;      // m+1
+    double* y;      // m
+    double* scale;  // m+1 : v_i = scale[i] * V_i (basis stored unnormalised)
+    double* coef;   // m+1 : coefficients of the pending update / combination
+    double* hist;   // caphist
+    double* partial;// [max_blocks][MAXV] block partial sums
+    int caphist;
+};
+
+enum { MAXV = 16 };                // basis vectors handled per pass of the multi-vector kernels
+
+enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5 };
+
+// ---------------------------------------------------------------------------------------------------------
+// Launchers (each enqueues on `st`, returns cudaGetLastError()).
+// ---------------------------------------------------------------------------------------------------------
+// explicit_kernels.cu
+cudaError_t launch_explicit_cell(const Grid& g, const Scheme& s, const Fields& f, double dt, int mode,
+                                 double* outE, double* outFx, double* outFy, double* outT, cudaStream_t st);
+cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& f, double dt,
+                                  double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st);
+cudaError_t launch_velocity_sources(const Grid& g, const Scheme& s, const Fields& f, const double* ux, const double* uy,
+                                    double dt, double* E, double* Fx, double* Fy, cudaStream_t st);
+cudaError_t launch_count_unrealizable(const Grid& g, const Fields& f, unsigned long long* counts2, cudaStream_t st);
+cudaError_t launch_add_planes(double* st_out, const double* a, const double* b, long long n, cudaStream_t st);
+
+// implicit_kernels.cu
+struct BlockMatrix {      // SoA planes of N doubles each
+    double* off;          // 36 planes: block k in {W,E,S,N}, entry (r,c): plane k*9 + r*3 + c   (A_k M_nbr^-1 after scaling)
+    double* C;            // 9 planes: diagonal block
+    double* Minv;         // 9 planes: inverse of the diagonal block
+    double* b;            // 3 planes: right-hand side
+};
+cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, cudaStream_t st);
+cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, cudaStream_t st);
+// t = C x
+cudaError_t launch_diag_mul(const Grid& g, const double* Cblk, const double* x, double* t, cudaStream_t st);
+// out = sgn*(s*(v + sum_k Ahat_k v_nbr)) + (add ? add : 0);  s = *scale_ptr[scale_idx] if scale_ptr else 1
+cudaError_t launch_spmv_hat(const Grid& g, const double* off, const double* v, double* out, const double* scale_ptr,
+                            const double* add, double sgn, const int* skip_flag, cudaStream_t st);
+cudaError_t launch_matter_update(const Grid& g, const Scheme& s, double dt, const double* sa, const double* rho_cv,
+                                 const double* Enew, double* T, cudaStream_t st);
+
+// krylov_kernels.cu
+int  krylov_max_blocks(int sm_count);
+// dots of w with nv vectors V0 + k*stride (k < nv) -> epilogue `mode`; col0 = index of the first vector in the basis
+cudaError_t launch_multi_dot(const double* w, const double* V0, long long stride, int nv, int col0, long long n,
+                             GmresWork W, int mode, int sm_count, cudaStream_t st);
+// w -= sum_k coef[col0+k] V_k ; if with_norm: ||w||^2 -> epilogue DOT_UPD
+cudaError_t launch_update(double* w, const double* V0, long long stride, int nv, int col0, long long n,
+                          GmresWork W, int with_norm, int sm_count, cudaStream_t st);
+// the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
+cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
+// x += Minv * (sum_{k<ctl->j} coef[k] V_k)  per cell
+cudaError_t launch_combine(const Grid& g, const double* V, long long stride, const double* Minv, double* x,
+                           GmresWork W, int sm_count, cudaStream_t st);
+cudaError_t launch_begin_solve(GmresWork W, double tol, int m, int maxit, cudaStream_t st);
+
+}  // namespace ark

@@ -1,0 +1,296 @@
+// krylov_kernels.cu — row a6: the vector kernels of restarted GMRES(m) with right block-Jacobi preconditioning
+// (Krylov solve of the linearised system, "solve A K^-1 y = b and then K x = y").
+//
+// Design:
+//  * The Arnoldi basis is stored UNNORMALISED: v_i = scale[i] * V_i.  The operator, the dots and the updates
+//    carry scale[i] as a scalar, so no pass over memory is spent on normalisation.
+//  * Orthogonalisation = one-pass classical Gram-Schmidt: one multi-dot kernel (w read once against up to MAXV
+//    basis vectors per pass) and one multi-axpy kernel fused with the norm of the result (CGS2 optional).
+//  * Reductions are deterministic: block partial sums -> fixed-order final sum by the last block to finish
+//    (ticket counter), whose thread 0 then runs the scalar epilogue (Hessenberg column, Givens rotations,
+//    residual estimate, stop flag) on the device.  A whole restart cycle is enqueued without host round trips;
+//    kernels of a cycle that has already met its stop criterion return immediately (ctl->inner_stop).
+#include "ark_m1_internal.h"
+
+namespace ark {
+
+static constexpr int KTHREADS = 256;
+
+int krylov_max_blocks(int sm_count) { return sm_count * 4; }
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ void hist_push(const GmresWork& W, GmresCtl* c, double r)
+{
+    if (c->nhist < W.caphist) W.hist[c->nhist] = (c->bnorm > 0.0) ? r / c->bnorm : r;
+    c->nhist++;
+}
+
+// Scalar epilogues, run by one thread after a reduction has produced d[0..nv).
+__device__ void epilogue(const GmresWork& W, int mode, const double* d, int nv, int col0)
+{
+    GmresCtl* c = W.ctl;
+    const int m = c->m;
+    if (mode == DOT_BNORM) {
+        c->bnorm = sqrt(d[0]);
+        c->target = c->est * c->bnorm;      // est holds tol until the first residual (set by begin_solve)
+        if (!isfinite(c->bnorm)) c->nonfinite = 1;
+    } else if (mode == DOT_RNORM) {         // true residual at the start of a cycle
+        const double r = sqrt(d[0]);
+        c->rnorm = r; c->est = r;
+        hist_push(W, c, r);
+        if (!isfinite(r)) c->nonfinite = 1;
+        c->converged = (r <= c->target) ? 1 : 0;
+        c->inner_stop = (c->converged || c->its >= c->maxit || c->nonfinite) ? 1 : 0;
+        c->j = 0;
+        W.scale[0] = 1.0 / r;
+        W.g[0] = r;
+        for (int k = 1; k <= m; ++k) W.g[k] = 0.0;
+    } else if (mode == DOT_H || mode == DOT_H2) {   // h_i = <w, v_i>, v_i = scale_i V_i
+        const int j = c->j;
+        for (int k = 0; k < nv; ++k) {
+            const int i = col0 + k;
+            const double h = d[k] * W.scale[i];
+            if (mode == DOT_H) W.H[i * m + j] = h; else W.H[i * m + j] += h;
+            W.coef[i] = h * W.scale[i];
+        }
+    } else if (mode == DOT_UPD) {           // h_{j+1,j} = ||w||, Givens rotations (Saad 2003, Sect. 6.5.3)
+        const int j = c->j;
+        const double hn = sqrt(d[0]);
+        double* H = W.H;
+        H[(j + 1) * m + j] = hn;
+        for (int i = 0; i < j; ++i) {
+            const double a = H[i * m + j], b = H[(i + 1) * m + j];
+            H[i * m + j] = W.cs[i] * a + W.sn[i] * b;
+            H[(i + 1) * m + j] = -W.sn[i] * a + W.cs[i] * b;
+        }
+        const double a = H[j * m + j], b = H[(j + 1) * m + j];
+        const double r = hypot(a, b);
+        W.cs[j] = a / r; W.sn[j] = b / r;
+        H[j * m + j] = r; H[(j + 1) * m + j] = 0.0;
+        W.g[j + 1] = -W.sn[j] * W.g[j];
+        W.g[j] = W.cs[j] * W.g[j];
+        W.scale[j + 1] = 1.0 / hn;
+        c->j = j + 1; c->its += 1;
+        c->est = fabs(W.g[j + 1]);
+        hist_push(W, c, c->est);
+        if (!isfinite(hn) || !isfinite(c->est)) c->nonfinite = 1;
+        if (c->est <= c->target || hn == 0.0 || c->its >= c->maxit || j + 1 >= m || c->nonfinite) c->inner_stop = 1;
+    }
+}
+
+// Block reduction of acc[0..NV) -> partial[block][.]; the last block sums the partials in a fixed order and
+// runs the epilogue.
+template <int NV>
+__device__ __forceinline__ void reduce_and_finish(double (&acc)[NV], const GmresWork& W, int mode, int col0)
+{
+    __shared__ double sh[KTHREADS / 32][MAXV];
+    __shared__ double dres[MAXV];
+    __shared__ bool is_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        const double s = warp_sum(acc[k]);
+        if (lane == 0) sh[warp][k] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < NV) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < KTHREADS / 32; ++w) s += sh[w][threadIdx.x];
+        W.partial[(size_t)blockIdx.x * MAXV + threadIdx.x] = s;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int t = atomicInc(&W.ctl->ticket, gridDim.x - 1);   // wraps to 0 after the last block
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    for (int k = warp; k < NV; k += KTHREADS / 32) {
+        double s = 0.0;
+        for (unsigned int b = lane; b < gridDim.x; b += 32) s += __ldcg(&W.partial[(size_t)b * MAXV + k]);
+        s = warp_sum(s);
+        if (lane == 0) dres[k] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) epilogue(W, mode, dres, NV, col0);
+}
+
+template <int NV>
+__global__ void __launch_bounds__(KTHREADS) multi_dot_kernel(const double* __restrict__ w, const double* __restrict__ V0,
+                                                             long long stride, long long n, GmresWork W, int mode, int col0)
+{
+    if (mode >= DOT_H && W.ctl->inner_stop) return;
+    double acc[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) acc[k] = 0.0;
+    const long long n2 = n >> 1;
+    const double2* w2 = reinterpret_cast<const double2*>(w);
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
+        const double2 a = w2[e];
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
+            acc[k] += a.x * b.x + a.y * b.y;
+        }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) acc[k] += w[n - 1] * V0[k * stride + n - 1];
+    }
+    reduce_and_finish<NV>(acc, W, mode, col0);
+}
+
+template <int NV, bool WITH_NORM>
+__global__ void __launch_bounds__(KTHREADS) update_kernel(double* __restrict__ w, const double* __restrict__ V0,
+                                                          long long stride, long long n, GmresWork W, int col0)
+{
+    if (W.ctl->inner_stop) return;
+    double cf[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) cf[k] = W.coef[col0 + k];
+    double acc[1] = { 0.0 };
+    const long long n2 = n >> 1;
+    double2* w2 = reinterpret_cast<double2*>(w);
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
+        double2 a = w2[e];
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
+            a.x -= cf[k] * b.x; a.y -= cf[k] * b.y;
+        }
+        w2[e] = a;
+        if (WITH_NORM) acc[0] += a.x * a.x + a.y * a.y;
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        double a = w[n - 1];
+#pragma unroll
+        for (int k = 0; k < NV; ++k) a -= cf[k] * V0[k * stride + n - 1];
+        w[n - 1] = a;
+        if (WITH_NORM) acc[0] += a * a;
+    }
+    if (WITH_NORM) reduce_and_finish<1>(acc, W, DOT_UPD, 0);
+}
+
+static int grid_for(long long n, int sm_count)
+{
+    const long long need = ((n >> 1) + KTHREADS - 1) / KTHREADS;
+    const long long cap = krylov_max_blocks(sm_count);
+    return (int)(need < 1 ? 1 : (need < cap ? need : cap));
+}
+
+template <int NV>
+static void dot_launch(int grd, const double* w, const double* V0, long long stride, long long n, GmresWork W, int mode,
+                       int col0, cudaStream_t st)
+{
+    multi_dot_kernel<NV><<<grd, KTHREADS, 0, st>>>(w, V0, stride, n, W, mode, col0);
+}
+
+cudaError_t launch_multi_dot(const double* w, const double* V0, long long stride, int nv, int col0, long long n,
+                             GmresWork W, int mode, int sm_count, cudaStream_t st)
+{
+    const int grd = grid_for(n, sm_count);
+    switch (nv) {
+#define ARK_CASE(K) case K: dot_launch<K>(grd, w, V0, stride, n, W, mode, col0, st); break;
+        ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
+        ARK_CASE(9) ARK_CASE(10) ARK_CASE(11) ARK_CASE(12) ARK_CASE(13) ARK_CASE(14) ARK_CASE(15) ARK_CASE(16)
+#undef ARK_CASE
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+template <int NV>
+static void upd_launch(int grd, double* w, const double* V0, long long stride, long long n, GmresWork W, int col0,
+                       int with_norm, cudaStream_t st)
+{
+    if (with_norm) update_kernel<NV, true><<<grd, KTHREADS, 0, st>>>(w, V0, stride, n, W, col0);
+    else update_kernel<NV, false><<<grd, KTHREADS, 0, st>>>(w, V0, stride, n, W, col0);
+}
+
+cudaError_t launch_update(double* w, const double* V0, long long stride, int nv, int col0, long long n,
+                          GmresWork W, int with_norm, int sm_count, cudaStream_t st)
+{
+    const int grd = grid_for(n, sm_count);
+    switch (nv) {
+#define ARK_CASE(K) case K: upd_launch<K>(grd, w, V0, stride, n, W, col0, with_norm, st); break;
+        ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
+        ARK_CASE(9) ARK_CASE(10) ARK_CASE(11) ARK_CASE(12) ARK_CASE(13) ARK_CASE(14) ARK_CASE(15) ARK_CASE(16)
+#undef ARK_CASE
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+// Cycle end: back substitution H y = g over the ctl->j columns built in this cycle; coef_i = y_i scale_i.
+__global__ void solve_y_kernel(GmresWork W)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int jj = W.ctl->j, m = W.ctl->m;
+    for (int i = jj - 1; i >= 0; --i) {
+        double s = W.g[i];
+        for (int k = i + 1; k < jj; ++k) s -= W.H[i * m + k] * W.y[k];
+        W.y[i] = s / W.H[i * m + i];
+        W.coef[i] = W.y[i] * W.scale[i];
+    }
+}
+
+cudaError_t launch_solve_y(GmresWork W, cudaStream_t st)
+{
+    solve_y_kernel<<<1, 32, 0, st>>>(W);
+    return cudaGetLastError();
+}
+
+// x += M^-1 (V y)  ("K x = y"), per cell.
+__global__ void __launch_bounds__(KTHREADS) combine_kernel(long long N, const double* __restrict__ V, long long stride,
+                                                           const double* __restrict__ Minv, double* __restrict__ x, GmresWork W)
+{
+    const int jj = W.ctl->j;
+    if (jj == 0) return;
+    for (long long id = blockIdx.x * (long long)KTHREADS + threadIdx.x; id < N; id += (long long)gridDim.x * KTHREADS) {
+        double u0 = 0.0, u1 = 0.0, u2 = 0.0;
+#pragma unroll 4
+        for (int k = 0; k < jj; ++k) {
+            const double cf = W.coef[k];
+            const double* v = V + k * stride;
+            u0 += cf * v[id]; u1 += cf * v[N + id]; u2 += cf * v[2 * N + id];
+        }
+        x[id]         += Minv[0 * N + id] * u0 + Minv[1 * N + id] * u1 + Minv[2 * N + id] * u2;
+        x[N + id]     += Minv[3 * N + id] * u0 + Minv[4 * N + id] * u1 + Minv[5 * N + id] * u2;
+        x[2 * N + id] += Minv[6 * N + id] * u0 + Minv[7 * N + id] * u1 + Minv[8 * N + id] * u2;
+    }
+}
+
+cudaError_t launch_combine(const Grid& g, const double* V, long long stride, const double* Minv, double* x,
+                           GmresWork W, int sm_count, cudaStream_t st)
+{
+    const long long N = (long long)g.nx * g.ny;
+    const long long need = (N + KTHREADS - 1) / KTHREADS, cap = (long long)sm_count * 8;
+    combine_kernel<<<(int)(need < cap ? need : cap), KTHREADS, 0, st>>>(N, V, stride, Minv, x, W);
+    return cudaGetLastError();
+}
+
+__global__ void begin_solve_kernel(GmresWork W, double tol, int m, int maxit)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    GmresCtl* c = W.ctl;
+    c->bnorm = 0.0; c->target = 0.0; c->rnorm = 0.0; c->est = tol;
+    c->m = m; c->maxit = maxit; c->its = 0; c->j = 0; c->inner_stop = 0; c->converged = 0; c->nonfinite = 0;
+    c->nhist = 0; c->ticket = 0;
+}
+
+cudaError_t launch_begin_solve(GmresWork W, double tol, int m, int maxit, cudaStream_t st)
+{
+    begin_solve_kernel<<<1, 32, 0, st>>>(W, tol, m, maxit);
+    return cudaGetLastError();
+}
+
+}  // namespace ark

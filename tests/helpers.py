@@ -16,6 +16,26 @@ def make_oracle(w, options=None):
     return o
 
 
+def make_gpu(w, options=None):
+    """The CUDA solver (through the C ABI binding) on the same workload dict.  Fails loudly without the library/GPU."""
+    import paper_2011_13926_b200 as ark
+    g = ark.ArkM1(w["nx"], w["ny"], w["dx"], w["dy"], w.get("c", 1.0), bc=w.get("bc", (0, 0, 0, 0)))
+    for k, v in (options or {}).items():
+        g.set_option(k, v)
+    g.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"], w.get("T"))
+    for name in ("rho_cv", "ux", "uy", "source_E"):
+        if w.get(name) is not None:
+            g.set_field(name, w[name])
+    for side, gh in (w.get("ghosts") or {}).items():
+        g.set_boundary(side, *gh)
+    return g
+
+
+def state_rel_l2(got, want):
+    """max over the fields (E, F[, T]) of the relative L2 difference."""
+    return max(rel_l2(a, b) for a, b in zip(got, want) if a is not None and b is not None)
+
+
 def rel_l2(a, b):
     a, b = np.asarray(a), np.asarray(b)
     return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
