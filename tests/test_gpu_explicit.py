@@ -57,8 +57,13 @@ def test_clamped_and_degenerate_cells():
     # |F| > cE in many cells (closure clamp), F = 0 cells, f = 1 exactly tangential to a face
     w = small_random_state(48, 33, seed=9, fmax=1.7)
     w["F"][:, 3, :] = 0.0
+    # f = 1 exactly, along y: lambda+- = 0 on the x-faces between such cells (the a+- = 1/2, Lambda = 0 guard).
+    # E is a power of two there so that F/(cE) is exactly 1 however the division is carried out: Eq. 14 has a
+    # square-root singularity at f = 1 (d lambda/d f ~ (1-f)^-1/2), so one ulp in f would move lambda by 1e-8
+    # (DESIGN.md "Conditioning at f = 1").
+    w["E"][5, :] = 2.0 ** np.random.default_rng(1).integers(-2, 3, w["nx"])
     w["F"][0, 5, :] = 0.0
-    w["F"][1, 5, :] = w["E"][5, :]      # f = 1 along y: lambda+- = 0 on x-faces between such cells
+    w["F"][1, 5, :] = w["E"][5, :]
     o, g = make_oracle(w), make_gpu(w)
     assert o.count_unrealizable() == g.count_unrealizable()
     assert o.count_unrealizable()[1] > 0
