@@ -1,0 +1,375 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the M1 radiative-transfer hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 4096] [--no-sweep]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+Workload (BASELINE.json configs[3]): the seeded random medium of m1_workloads.random_medium at 4096 x 4096
+(16.8 M cells, 3 fp64 unknowns per cell).  One STEP = one pass of the whole hot path from the same initial state:
+    reset state (device-to-device) -> 1 explicit step at CFL 0.4 (rows a1-a4)
+                                   -> 1 implicit step at dt = 10 x explicit (rows a5-a7: assembly, GMRES(30)+block-Jacobi to 1e-10)
+`value` = cells updated per second by the whole step = 2 N K / T (N cells, K steps, T = timed region, CUDA events).
+The JSON line also carries, each measured in the same run with CUDA events:
+    explicit  : cell-updates/s of the explicit kernel alone (>= 20 back-to-back steps), fraction of the HBM roofline (64 B/cell)
+    implicit  : per dt ratio 10/50/100/200: iterations, ms, cell-updates/s, cell-iterations/s, bytes/iteration, HBM fraction
+    break_even: T_implicit(K)/T_explicit vs K (implicit pays off where the ratio < K), beside the paper's 50-100x
+    roofline  : the dominant kernel class of the step (by device time), from per-launch CUDA events inside the timed region
+    kernels   : the same for every kernel class
+    e2e       : the same step through the C ABI with HOST (pinned) buffers: H2D of the 5 input planes and D2H of the 3
+                state planes inside the timed region
+    cpu_baseline : the oracle (oracle/oracle_m1.c, as it stands) on a bounded sample of the same workload
+Multi-GPU (torchrun): the path does not exchange data between GPUs (one-GPU north star): every rank runs an independent
+replica with its own seed, value = sum of units / max-over-ranks time ("scaling": "weak", no collective on the data path).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import m1_workloads as wl  # noqa: E402
+
+METRIC = "M1 cell-updates/s (explicit step + implicit step per pass)"
+UNIT = "cell-updates/s"
+TOL, RESTART, MAXIT = 1e-10, 30, 4000
+BENCH_DT_RATIO = 10.0
+SWEEP = (10.0, 50.0, 100.0, 200.0)
+PAPER_BREAK_EVEN = "50-100x (relaxation preconditioner; CPU 50, K80 GPU 100; PAPER.md:369)"
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# --------------------------------------------------------------------------------------------------------------
+# clocks
+# --------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 7:
+                    continue
+                try:
+                    sm.append(float(p[0])); mx.append(float(p[1]))
+                except ValueError:
+                    continue
+                for k, nm in enumerate(names):
+                    if p[3 + k].lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# --------------------------------------------------------------------------------------------------------------
+# reference arm / cpu baseline: the oracle on a bounded sample
+# --------------------------------------------------------------------------------------------------------------
+def oracle_step_time(n_sample, seed, steps, warmup):
+    """Times `steps` passes (explicit step + implicit 10x step from the same state) of the oracle at n_sample^2."""
+    from oracle.oracle_m1 import OracleM1, num_threads
+    w = wl.random_medium(n_sample, seed=seed)
+    dt = wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    o = OracleM1(w["nx"], w["ny"], w["dx"], w["dy"], w["c"], bc=w["bc"])
+    times, its = [], 0
+    for k in range(warmup + steps):
+        o.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
+        t0 = time.perf_counter()
+        o.step_explicit(dt)
+        its, _ = o.step_implicit(BENCH_DT_RATIO * dt, TOL, RESTART, MAXIT)
+        t1 = time.perf_counter()
+        if k >= warmup:
+            times.append(t1 - t0)
+    total = float(sum(times))
+    return dict(seconds=total, per_step=total / max(steps, 1), cells=n_sample * n_sample, iterations=its, cores=num_threads())
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    n_s = args.ref_n
+    r = oracle_step_time(n_s, args.seed, args.steps, args.warmup)
+    value = 2.0 * r["cells"] * args.steps / r["seconds"]
+    sample = (f"{n_s}x{n_s} grid of the same seeded random-medium generator ({r['cells'] / (args.n * args.n):.4f} of the "
+              f"{args.n}x{args.n} workload's cells) per step, {r['iterations']} GMRES iterations per implicit step")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * r["per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"M1 random medium (BASELINE.json configs[3]) {args.n}x{args.n}, fp64, periodic; reference arm = "
+                               f"CPU oracle on a bounded sample", "step": "1 explicit step (CFL 0.4) + 1 implicit step (dt = 10x, "
+                               "GMRES(30) + block-Jacobi, tol 1e-10)", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------------------
+def aggregate_over_ranks(elapsed_s, units, dist=None):
+    """(max elapsed over ranks, total units over ranks).  `dist` = torch.distributed or None for one process."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return elapsed_s, units
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([elapsed_s], dtype=torch.float64, device=dev)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def iteration_bytes_per_cell(iters, m=RESTART):
+    """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
+    operator 336; one-pass classical Gram-Schmidt at inner index j: dots 24 (j+2), update+norm 24 (j+3); one extra read of
+    w per 16-vector pass; per cycle: combine 8 (3 jj + 15) + diag_mul 120 + residual spmv 360 + norm 24."""
+    total, done = 0.0, 0
+    while done < iters:
+        jj = min(m, iters - done)
+        for j in range(jj):
+            passes = j // 16 + 1
+            total += 336.0 + 24.0 * (j + 1 + passes) + 24.0 * (j + 1 + 2 * passes)
+        total += 8.0 * (3 * jj + 15) + 120.0 + 360.0 + 24.0
+        done += jj
+    return total
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2011_13926_b200 as ark
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the CUDA library is the only implementation (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    peak_gbs, peak_src = peaks()
+
+    n = args.n
+    N = n * n
+    w = wl.random_medium(n, seed=args.seed + rank)
+    dt_e = wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    host = {k: torch.from_numpy(np.ascontiguousarray(w[k])).pin_memory() for k in ("E", "F", "sigma_a", "sigma_s")}
+    devt = {k: v.to(dev) for k, v in host.items()}
+    out_E = torch.empty((n, n), dtype=torch.float64).pin_memory()
+    out_F = torch.empty((2, n, n), dtype=torch.float64).pin_memory()
+    stream = torch.cuda.current_stream()
+    g = ark.ArkM1(n, n, w["dx"], w["dy"], w["c"], bc=w["bc"], stream=stream)
+
+    def reset_device():
+        g.set_state(devt["E"], devt["F"], devt["sigma_a"], devt["sigma_s"])
+
+    def one_step(ratio=BENCH_DT_RATIO):
+        g.step_explicit(dt_e)
+        return g.step_implicit(ratio * dt_e, TOL, RESTART, MAXIT)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- main timed region: W warm-up + exactly K steps, inputs resident in HBM ----------------------------------
+    for _ in range(args.warmup):
+        reset_device(); one_step()
+    g.set_option("kernel_timing", 1)
+    sampler = ClockSampler(local)
+    launches0 = g.kernel_launches()
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    its_main = 0
+    for _ in range(args.steps):
+        reset_device()
+        its_main, res_main = one_step()
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    elapsed = e0.elapsed_time(e1) * 1e-3
+    launches = g.kernel_launches() - launches0
+    stats = g.kernel_stats()
+    g.set_option("kernel_timing", 0)
+    t_max, units = aggregate_over_ranks(elapsed, 2.0 * N * args.steps, dist if world > 1 else None)
+    value = units / t_max
+
+    # ---- e2e: same step through the C ABI with pinned HOST buffers -------------------------------------------------
+    def e2e_step():
+        g.set_state(host["E"], host["F"], host["sigma_a"], host["sigma_s"])
+        one_step()
+        g.get_state(out=(out_E, out_F))
+    e2e_step()
+    barrier()
+    k_e2e = max(1, min(args.steps, 3))
+    e0.record(stream)
+    for _ in range(k_e2e):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    t_e2e, u_e2e = aggregate_over_ranks(e0.elapsed_time(e1) * 1e-3, 2.0 * N * k_e2e, dist if world > 1 else None)
+    e2e = {"value": u_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": 5 * N * 8, "d2h_bytes_per_step": 3 * N * 8, "steps": k_e2e}
+
+    line_extra = {}
+    if rank == 0:
+        # ---- explicit kernel alone -----------------------------------------------------------------------------
+        reset_device()
+        g.steps_explicit(dt_e, 5)
+        torch.cuda.synchronize()
+        n_exp = max(20, 4 * args.steps)
+        e0.record(stream)
+        g.steps_explicit(dt_e, n_exp)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms_exp = e0.elapsed_time(e1) / n_exp
+        exp_rate = N / (ms_exp * 1e-3)
+        exp_gbs = 64.0 * N / (ms_exp * 1e-3) / 1e9
+        line_extra["explicit"] = {"cell_updates_per_s": exp_rate, "ms_per_step": ms_exp, "steps_timed": n_exp, "bytes_per_cell": 64,
+                                  "achieved_gbs": exp_gbs, "hbm_frac": exp_gbs / peak_gbs}
+        # ---- implicit sweep ----------------------------------------------------------------------------------------
+        imp, brk = {}, {}
+        ratios = SWEEP if not args.no_sweep else (BENCH_DT_RATIO,)
+        for ratio in ratios:
+            reset_device()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            its, res = g.step_implicit(ratio * dt_e, TOL, RESTART, MAXIT)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            tm = g.timings()
+            nE, nf = g.count_unrealizable()
+            bpc = iteration_bytes_per_cell(its)
+            kry_gbs = bpc * N / (tm["krylov_ms"] * 1e-3) / 1e9 if its > 0 else None
+            imp[f"{ratio:g}x"] = {"iterations": its, "final_residual": res, "ms": ms, "assembly_ms": tm["assembly_ms"], "krylov_ms": tm["krylov_ms"],
+                                  "ms_per_iteration": tm["krylov_ms"] / max(its, 1), "cell_updates_per_s": N / (ms * 1e-3),
+                                  "cell_iterations_per_s": N * its / (ms * 1e-3), "bytes_per_cell_per_iteration": bpc / max(its, 1),
+                                  "krylov_achieved_gbs": kry_gbs, "krylov_hbm_frac": (kry_gbs / peak_gbs) if kry_gbs else None,
+                                  "cells_E_nonpositive": nE, "cells_f_above_one": nf}
+            brk[f"{ratio:g}x"] = {"T_implicit_over_T_explicit": ms / ms_exp, "implicit_wins": bool(ms / ms_exp < ratio)}
+        line_extra["implicit"] = imp
+        wins = [k for k, v in brk.items() if v["implicit_wins"]]
+        line_extra["break_even"] = {"per_ratio": brk, "reached_in_sweep": bool(wins), "first_winning_ratio": wins[0] if wins else None,
+                                    "paper": PAPER_BREAK_EVEN}
+        # ---- roofline of the dominant kernel class ---------------------------------------------------------------
+        traffic = {}
+        tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+        if os.path.exists(tpath):
+            with open(tpath) as f:
+                traffic = json.load(f)
+        tot_ms = sum(v["ms"] for v in stats.values()) or 1.0
+        kern = {}
+        for name, v in stats.items():
+            if v["launches"] == 0:
+                continue
+            gbs = v["bytes"] / (v["ms"] * 1e-3) / 1e9 if v["ms"] > 0 else 0.0
+            kern[name] = {"launches": v["launches"], "ms_total": v["ms"], "share": v["ms"] / tot_ms, "achieved_gbs": gbs, "hbm_frac": gbs / peak_gbs,
+                          "alg_bytes_per_launch": v["bytes"] / v["launches"]}
+        dom = max((k for k in kern if k != "small"), key=lambda k: kern[k]["ms_total"])
+        tr = traffic.get(dom, {}) if (n == 4096) else {}
+        line_extra["roofline"] = {"kernel": dom, "bound": "hbm", "achieved": kern[dom]["achieved_gbs"], "peak": peak_gbs, "unit": "GB/s",
+                                  "frac": kern[dom]["hbm_frac"], "traffic": tr.get("dram_bytes_per_launch"), "peak_source": peak_src,
+                                  "share_of_step": kern[dom]["share"], "alg_bytes_per_launch": kern[dom]["alg_bytes_per_launch"],
+                                  "traffic_note": tr.get("note")}
+        line_extra["kernels"] = kern
+        # ---- cpu baseline ------------------------------------------------------------------------------------------
+        if world == 1 and not args.no_cpu_baseline:
+            n_s = args.cpu_n
+            r = oracle_step_time(n_s, args.seed, 1, 0)
+            line_extra["cpu_baseline"] = {"value": 2.0 * r["cells"] / r["seconds"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+                                          "sample": f"1 step (explicit + implicit 10x, {r['iterations']} GMRES iterations) on a {n_s}x{n_s} grid of "
+                                                    f"the same generator = {r['cells'] / N:.4f} of the workload's cells; {r['seconds']:.1f} s"}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"M1 random medium (BASELINE.json configs[3]) {n}x{n}, fp64, periodic, c=1, seed {args.seed}(+rank)",
+                       "step": "state reset (D2D) + 1 explicit step (CFL 0.4) + 1 implicit step (dt = 10x explicit, GMRES(30) + block-Jacobi, tol 1e-10)",
+                       "iterations_per_implicit_step": its_main, "parallelism": "replicas only (one independent problem per GPU)" if world > 1 else "1 GPU",
+                       "l2": f"inputs larger than L2 (state+opacity {5 * N * 8 / 1e6:.0f} MB, Krylov basis {31 * 3 * N * 8 / 1e9:.1f} GB vs 126 MB L2)",
+                       "device_bytes": g.device_bytes()},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        }
+        line.update(line_extra)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=4096, help="grid size (BASELINE.json configs[3]: 4096)")
+    ap.add_argument("--seed", type=int, default=1234)
+    ap.add_argument("--no-sweep", action="store_true", help="skip the dt = 50/100/200x implicit solves")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-n", type=int, default=2048, help="grid size of the oracle's bounded sample (cpu_baseline)")
+    ap.add_argument("--ref-n", type=int, default=1024, help="grid size of the oracle's bounded sample per step (--impl reference)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print(f"bench.py: note: warmup {args.warmup} < 3 (timing rule wants >= 3)", file=sys.stderr)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

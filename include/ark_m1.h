@@ -85,6 +85,7 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *   "eig_floor"     x: lambda+ >= x c, lambda- <= -x c; default 0
  *   "a_r"           radiation constant (default 1)
  *   "orthogonalisation" 1: one-pass classical Gram-Schmidt (default)   2: CGS2 (re-orthogonalise once)
+ *   "kernel_timing"     1: time every kernel launch with CUDA events (see ark_m1_get_kernel_stats); default 0
  *   "explicit_kernel"   0: one-thread-per-cell kernel   1: row-marching kernel (default)
  *   "operator"          0: block-stencil (BSR 3x3, pre-multiplied by M^-1) (default)   1: matrix-free coefficient planes
  * Unknown key or unsupported value: ARK_M1_E_ARG. */
@@ -136,6 +137,14 @@ ARK_M1_API int ark_m1_get_history(ark_m1* h, double* buf, int cap);
 /* Timings of the last implicit solve in milliseconds (CUDA events on the handle's stream):
  * out[0] = assembly, out[1] = Krylov iterations (everything after assembly), out[2] = total. */
 ARK_M1_API int ark_m1_get_timings(ark_m1* h, double* out3);
+
+/* Launch statistics.  After ark_m1_set_option(h, "kernel_timing", 1) every kernel launch of the handle is
+ * bracketed by CUDA events on the handle's stream; out[3k .. 3k+2] = number of launches, total milliseconds and
+ * total ALGORITHMIC bytes of kernel class k.  Returns the number of classes; names from
+ * ark_m1_kernel_class_name(k).  ark_m1_kernel_launches = kernels launched by the handle since creation. */
+ARK_M1_API int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap);
+ARK_M1_API const char* ark_m1_kernel_class_name(int k);
+ARK_M1_API long long ark_m1_kernel_launches(const ark_m1* h);
 
 /* Device bytes currently allocated by the handle. */
 ARK_M1_API long long ark_m1_device_bytes(const ark_m1* h);

@@ -23,7 +23,8 @@ SYMBOLS = [
     "ark_m1_create", "ark_m1_destroy", "ark_m1_set_stream", "ark_m1_set_state", "ark_m1_set_boundary",
     "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
     "ark_m1_step_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
-    "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_device_bytes",
+    "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
+    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
 ]
 
@@ -64,6 +65,11 @@ def load_library(path: str = LIB_PATH):
     L.ark_m1_apply_operator.argtypes = [vp, d, dp, dp, dp]
     L.ark_m1_get_history.argtypes = [vp, C.POINTER(C.c_double), i]
     L.ark_m1_get_timings.argtypes = [vp, C.POINTER(C.c_double)]
+    L.ark_m1_get_kernel_stats.argtypes = [vp, C.POINTER(C.c_double), i]
+    L.ark_m1_kernel_class_name.restype = C.c_char_p
+    L.ark_m1_kernel_class_name.argtypes = [i]
+    L.ark_m1_kernel_launches.restype = C.c_longlong
+    L.ark_m1_kernel_launches.argtypes = [vp]
     L.ark_m1_device_bytes.restype = C.c_longlong
     L.ark_m1_device_bytes.argtypes = [vp]
     L.ark_m1_last_error.restype = C.c_char_p
@@ -204,6 +210,16 @@ class ArkM1:
         buf = (C.c_double * 3)()
         self._check(self._L.ark_m1_get_timings(self._h, buf))
         return dict(assembly_ms=buf[0], krylov_ms=buf[1], total_ms=buf[2])
+
+    def kernel_stats(self):
+        """{class name: dict(launches, ms, bytes)} since set_option("kernel_timing", 1)."""
+        buf = (C.c_double * 64)()
+        n = self._check(self._L.ark_m1_get_kernel_stats(self._h, buf, 64))
+        return {self._L.ark_m1_kernel_class_name(k).decode(): dict(launches=int(buf[3 * k]), ms=buf[3 * k + 1], bytes=buf[3 * k + 2])
+                for k in range(n)}
+
+    def kernel_launches(self):
+        return int(self._L.ark_m1_kernel_launches(self._h))
 
     def device_bytes(self):
         return int(self._L.ark_m1_device_bytes(self._h))

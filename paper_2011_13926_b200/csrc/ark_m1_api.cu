@@ -13,6 +13,11 @@
 
 using namespace ark;
 
+// kernel classes for the launch statistics
+enum { KC_EXPLICIT = 0, KC_ASSEMBLE, KC_SCALE, KC_DIAGMUL, KC_SPMV, KC_DOT, KC_UPDATE, KC_COMBINE, KC_SMALL, KC_COUNT };
+static const char* const kc_names[KC_COUNT] = { "explicit", "assemble", "scale_offdiag", "diag_mul", "spmv_hat", "multi_dot",
+                                                 "update_norm", "combine", "small" };
+
 struct ark_m1 {
     Grid g;
     Scheme s;
@@ -42,6 +47,14 @@ struct ark_m1 {
     std::vector<double>* hist_host;
     cudaEvent_t ev[3];
     double timings[3];
+    // per-kernel-class timing (option "kernel_timing"): one event before every launch + one at the end
+    int ktiming;
+    std::vector<cudaEvent_t>* kev;
+    std::vector<int>* kcls;
+    std::vector<double>* kbytes;
+    size_t kused;
+    double kstat[KC_COUNT][3];   // launches, milliseconds, algorithmic bytes
+    long long launches;          // kernels launched by this handle
     char err[512];
 };
 
@@ -51,6 +64,31 @@ static int fail(ark_m1* h, int code, const char* fmt, const char* detail)
     return code;
 }
 #define CU(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(h, ARK_M1_E_CUDA, #call ": %s", cudaGetErrorString(e__)); } while (0)
+
+// Record the start of a launch of class `cls` moving `bytes` algorithmic bytes (only when kernel timing is on).
+static void kmark(ark_m1* h, int cls, double bytes)
+{
+    h->launches++;
+    if (!h->ktiming) return;
+    if (h->kused == h->kev->size()) { cudaEvent_t e; cudaEventCreate(&e); h->kev->push_back(e); }
+    cudaEventRecord((*h->kev)[h->kused++], h->st);
+    h->kcls->push_back(cls); h->kbytes->push_back(bytes);
+}
+// Close the open series: one final event, then (after a sync) accumulate per-class elapsed times.
+static void kflush(ark_m1* h)
+{
+    if (!h->ktiming || h->kcls->empty()) return;
+    if (h->kused == h->kev->size()) { cudaEvent_t e; cudaEventCreate(&e); h->kev->push_back(e); }
+    cudaEventRecord((*h->kev)[h->kused], h->st);
+    cudaStreamSynchronize(h->st);
+    for (size_t k = 0; k < h->kcls->size(); ++k) {
+        float ms = 0.f; cudaEventElapsedTime(&ms, (*h->kev)[k], (*h->kev)[k + 1]);
+        const int c = (*h->kcls)[k];
+        h->kstat[c][0] += 1.0; h->kstat[c][1] += ms; h->kstat[c][2] += (*h->kbytes)[k];
+    }
+    h->kcls->clear(); h->kbytes->clear(); h->kused = 0;
+}
+#define KL(cls, bytes, call) do { kmark(h, (cls), (double)(bytes)); CU(call); } while (0)
 
 static int dmalloc(ark_m1* h, void** p, size_t bytes)
 {
@@ -94,6 +132,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     h->hist_host = new std::vector<double>();
+    h->kev = new std::vector<cudaEvent_t>(); h->kcls = new std::vector<int>(); h->kbytes = new std::vector<double>();
     const size_t N = (size_t)h->N;
     bool ok = true;
     for (int k = 0; k < 2 && ok; ++k) ok = dmalloc(h, (void**)&h->U[k], 3 * N * sizeof(double)) == 0;
@@ -132,6 +171,8 @@ void ark_m1_destroy(ark_m1* h)
     if (h->ctl_host) cudaFreeHost(h->ctl_host);
     for (int k = 0; k < 3; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
     delete h->hist_host;
+    if (h->kev) for (cudaEvent_t e : *h->kev) cudaEventDestroy(e);
+    delete h->kev; delete h->kcls; delete h->kbytes;
     cudaGetLastError();
     delete h;
 }
@@ -192,6 +233,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
     else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0 or 1%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv != 0) return fail(h, ARK_M1_E_ARG, "operator: only 0 (block-stencil) is built%s", ""); h->op_kind = iv; }
     else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
     return 0;
@@ -229,9 +271,9 @@ static int explicit_once(ark_m1* h, double dt)
     double* O = h->U[h->cur ^ 1];
     const bool plain = !h->have_T && !h->source_E;
     if (h->explicit_kernel == 1 && plain) {
-        CU(launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
+        KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
     } else {
-        CU(launch_explicit_cell(h->g, h->s, f, dt, 0, O, O + h->N, O + 2 * h->N, h->have_T ? h->T[h->cur ^ 1] : nullptr, h->st));
+        KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_cell(h->g, h->s, f, dt, 0, O, O + h->N, O + 2 * h->N, h->have_T ? h->T[h->cur ^ 1] : nullptr, h->st));
     }
     h->cur ^= 1;
     return 0;
@@ -261,7 +303,7 @@ int ark_m1_residual(ark_m1* h, double* RE, double* RF)
     const Fields f = fields_of(h);
     double* O = h->U[h->cur ^ 1];
     const size_t N = (size_t)h->N;
-    CU(launch_explicit_cell(h->g, h->s, f, 0.0, 1, O, O + N, O + 2 * N, nullptr, h->st));
+    KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_cell(h->g, h->s, f, 0.0, 1, O, O + N, O + 2 * N, nullptr, h->st));
     CU(cudaMemcpyAsync(RE, O, N * sizeof(double), cudaMemcpyDefault, h->st));
     CU(cudaMemcpyAsync(RF, O + N, 2 * N * sizeof(double), cudaMemcpyDefault, h->st));
     CU(cudaStreamSynchronize(h->st));
@@ -274,7 +316,7 @@ int ark_m1_add_velocity_sources(ark_m1* h, double dt)
     if (!h->have_state || !h->ux || !h->uy) return fail(h, ARK_M1_E_NOTSET, "add_velocity_sources: state, ux, uy must be set%s", "");
     const Fields f = fields_of(h);
     double* U = h->U[h->cur];
-    CU(launch_velocity_sources(h->g, h->s, f, h->ux, h->uy, dt, U, U + h->N, U + 2 * h->N, h->st));
+    KL(KC_SMALL, 88.0 * h->N, launch_velocity_sources(h->g, h->s, f, h->ux, h->uy, dt, U, U + h->N, U + 2 * h->N, h->st));
     return 0;
 }
 
@@ -283,7 +325,7 @@ int ark_m1_count_unrealizable(ark_m1* h, long long* nE, long long* nf)
     if (!h || !nE || !nf) return ARK_M1_E_ARG;
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "count_unrealizable: no state set%s", "");
     CU(cudaMemsetAsync(h->counts, 0, 2 * sizeof(unsigned long long), h->st));
-    CU(launch_count_unrealizable(h->g, fields_of(h), h->counts, h->st));
+    KL(KC_SMALL, 24.0 * h->N, launch_count_unrealizable(h->g, fields_of(h), h->counts, h->st));
     unsigned long long out[2];
     CU(cudaMemcpyAsync(out, h->counts, sizeof out, cudaMemcpyDeviceToHost, h->st));
     CU(cudaStreamSynchronize(h->st));
@@ -345,9 +387,9 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
 static int true_residual(ark_m1* h, const double* x)
 {
     const long long n = 3 * h->N;
-    CU(launch_diag_mul(h->g, h->A.C, x, h->tvec, h->st));
-    CU(launch_spmv_hat(h->g, h->A.off, h->tvec, h->V, nullptr, h->A.b, -1.0, nullptr, h->st));
-    CU(launch_multi_dot(h->V, h->V, h->stride, 1, 0, n, h->W, DOT_RNORM, h->sm_count, h->st));
+    KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, x, h->tvec, h->st));
+    KL(KC_SPMV, 360.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->tvec, h->V, nullptr, h->A.b, -1.0, nullptr, h->st));
+    KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->V, h->V, h->stride, 1, 0, n, h->W, DOT_RNORM, h->sm_count, h->st));
     return 0;
 }
 
@@ -361,8 +403,8 @@ static int fetch_ctl(ark_m1* h)
 static int assemble_system(ark_m1* h, double dt)
 {
     const Fields f = fields_of(h);
-    CU(launch_assemble(h->g, h->s, f, dt, h->A, h->st));
-    CU(launch_scale_offdiag(h->g, h->A, h->st));
+    KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->st));
+    KL(KC_SCALE, 648.0 * h->N, launch_scale_offdiag(h->g, h->A, h->st));
     return 0;
 }
 
@@ -383,28 +425,28 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
     CU(cudaEventRecord(h->ev[0], h->st));
     if ((rc = assemble_system(h, dt))) return rc;
     CU(cudaEventRecord(h->ev[1], h->st));
-    CU(launch_begin_solve(W, tol, m, maxit, h->st));
-    CU(launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
+    KL(KC_SMALL, 0.0, launch_begin_solve(W, tol, m, maxit, h->st));
+    KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
     if ((rc = true_residual(h, x))) return rc;
     if ((rc = fetch_ctl(h))) return rc;
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
-            CU(launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
+            KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
             for (int pass = 0; pass < h->ortho; ++pass) {
                 for (int c0 = 0; c0 <= j; c0 += MAXV) {
                     const int nv = (j + 1 - c0) < MAXV ? (j + 1 - c0) : MAXV;
-                    CU(launch_multi_dot(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, pass == 0 ? DOT_H : DOT_H2, sm, h->st));
+                    KL(KC_DOT, 24.0 * (nv + 1) * h->N, launch_multi_dot(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, pass == 0 ? DOT_H : DOT_H2, sm, h->st));
                 }
                 for (int c0 = 0; c0 <= j; c0 += MAXV) {
                     const int nv = (j + 1 - c0) < MAXV ? (j + 1 - c0) : MAXV;
                     const int last = (c0 + MAXV > j) && (pass == h->ortho - 1);
-                    CU(launch_update(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, last, sm, h->st));
+                    KL(KC_UPDATE, 24.0 * (nv + 2) * h->N, launch_update(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, last, sm, h->st));
                 }
             }
         }
-        CU(launch_solve_y(W, h->st));
-        CU(launch_combine(h->g, h->V, S, h->A.Minv, x, W, sm, h->st));
+        KL(KC_SMALL, 0.0, launch_solve_y(W, h->st));
+        KL(KC_COMBINE, 8.0 * (3.0 * m + 15.0) * h->N, launch_combine(h->g, h->V, S, h->A.Minv, x, W, sm, h->st));
         if ((rc = true_residual(h, x))) return rc;
         if ((rc = fetch_ctl(h))) return rc;
     }
@@ -415,9 +457,10 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
     h->hist_host->assign((size_t)nh, 0.0);
     if (nh > 0) CU(cudaMemcpyAsync(h->hist_host->data(), W.hist, (size_t)nh * sizeof(double), cudaMemcpyDeviceToHost, h->st));
     if (h->have_T && !c.nonfinite) {
-        CU(launch_matter_update(h->g, h->s, dt, h->sa, h->rho_cv, x, h->T[h->cur], h->st));
+        KL(KC_SMALL, 40.0 * h->N, launch_matter_update(h->g, h->s, dt, h->sa, h->rho_cv, x, h->T[h->cur], h->st));
     }
     CU(cudaStreamSynchronize(h->st));
+    kflush(h);
     float ms01 = 0, ms12 = 0;
     cudaEventElapsedTime(&ms01, h->ev[0], h->ev[1]); cudaEventElapsedTime(&ms12, h->ev[1], h->ev[2]);
     h->timings[0] = ms01; h->timings[1] = ms12; h->timings[2] = (double)ms01 + ms12;
@@ -438,8 +481,8 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
     double* vin = h->V;                       // slot 0 as staging for the input, slot 1 for the output
     double* vout = h->V + h->stride;
     CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
-    CU(launch_diag_mul(h->g, h->A.C, vin, h->tvec, h->st));
-    CU(launch_spmv_hat(h->g, h->A.off, h->tvec, vout, nullptr, nullptr, 1.0, nullptr, h->st));
+    KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, vin, h->tvec, h->st));
+    KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->tvec, vout, nullptr, nullptr, 1.0, nullptr, h->st));
     CU(cudaMemcpyAsync(out, vout, n * sizeof(double), cudaMemcpyDefault, h->st));
     if (b_out) CU(cudaMemcpyAsync(b_out, h->A.b, n * sizeof(double), cudaMemcpyDefault, h->st));
     CU(cudaStreamSynchronize(h->st));
@@ -460,3 +503,15 @@ extern "C" int ark_m1_get_timings(ark_m1* h, double* out3)
     for (int k = 0; k < 3; ++k) out3[k] = h->timings[k];
     return 0;
 }
+
+// Per-kernel-class statistics since "kernel_timing" was switched on: out[3*k + 0..2] = launches, milliseconds,
+// algorithmic bytes of class k (k < ark_m1_kernel_classes()).  Synchronises.
+extern "C" int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap)
+{
+    if (!h || !out) return ARK_M1_E_ARG;
+    kflush(h);
+    for (int k = 0; k < KC_COUNT && 3 * k + 2 < cap; ++k) for (int q = 0; q < 3; ++q) out[3 * k + q] = h->kstat[k][q];
+    return KC_COUNT;
+}
+extern "C" const char* ark_m1_kernel_class_name(int k) { return (k >= 0 && k < KC_COUNT) ? kc_names[k] : ""; }
+extern "C" long long ark_m1_kernel_launches(const ark_m1* h) { return h ? h->launches : 0; }
