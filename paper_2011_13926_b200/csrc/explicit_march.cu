@@ -18,19 +18,120 @@ static constexpr int TX = 128;
 
 struct Raw { double E, Fx, Fy, st, sa; };
 
-// Row loader with boundary handling.  i may be -1 or nx (x ghost), j may be -1 or ny (y ghost), never both.
-__device__ __forceinline__ Raw load_raw(const Fields& f, const Grid& g, int i, int j, bool col_active)
+// Row loader with boundary handling.  The column is resolved once per thread (xmode/ii), so that the common case
+// (interior row) costs one multiply-add and five loads.
+//   xmode 0: column ii of the grid (after periodic wrap / outflow clamp);  1: Dirichlet x-ghost of side xside;  2: inactive.
+// j may be -1 or ny (y ghost).  Corner ghosts are never used by a 5-point stencil and return a dummy state.
+__device__ __forceinline__ Raw load_row(const Fields& f, const Grid& g, int xmode, int ii, int xside, int j)
 {
     Raw r; r.E = 1.0; r.Fx = 0.0; r.Fy = 0.0; r.st = 0.0; r.sa = 0.0;
-    if (!col_active) return r;
-    const bool xout = (i < 0 || i >= g.nx), yout = (j < 0 || j >= g.ny);
-    if (xout && yout) return r;          // corner ghosts are never used by a 5-point stencil
-    CellU u; fetch_cell(f, g, i, j, u);
-    r.E = u.E; r.Fx = u.Fx; r.Fy = u.Fy; r.st = u.st; r.sa = u.sa;
+    if (xmode == 2) return r;
+    if (j >= 0 && j < g.ny) {
+        if (xmode == 0) {
+            const long long id = (long long)j * g.nx + ii;
+            r.E = f.E[id]; r.Fx = f.Fx[id]; r.Fy = f.Fy[id]; r.st = f.st[id]; r.sa = f.sa[id];
+        } else {
+            r.E = f.gh[xside][0][j]; r.Fx = f.gh[xside][1][j]; r.Fy = f.gh[xside][2][j]; r.sa = f.gh[xside][3][j]; r.st = f.gh[xside][4][j];
+        }
+        return r;
+    }
+    if (xmode != 0) return r;                       // corner
+    const int side = (j < 0) ? YLO : YHI;
+    const int bc = g.bc[side];
+    if (bc == BC_DIRICHLET) {
+        r.E = f.gh[side][0][ii]; r.Fx = f.gh[side][1][ii]; r.Fy = f.gh[side][2][ii]; r.sa = f.gh[side][3][ii]; r.st = f.gh[side][4][ii];
+        return r;
+    }
+    const int jj = (bc == BC_PERIODIC) ? ((j < 0) ? g.ny - 1 : 0) : ((j < 0) ? 0 : g.ny - 1);
+    const long long id = (long long)jj * g.nx + ii;
+    r.E = f.E[id]; r.Fx = f.Fx[id]; r.Fy = f.Fy[id]; r.st = f.st[id]; r.sa = f.sa[id];
     return r;
 }
 
 struct XPub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };   // what the west neighbour needs for its east face
+
+// What the march kernel keeps per cell: pressure, Eq. 14 eigenvalues for both face orientations, |f|.
+struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };
+
+// Default-scheme closure with 2 reciprocals and 4 reciprocal square roots per cell:
+//   1/(cE);  rs = 1/sqrt(4 - 3 f^2) gives xi = s rs and 1/xi = rs;  one reciprocal of (2+xi)(5+2xi) gives both
+//   1/(5+2xi) (for chi) and 1/(2+xi) (for the anisotropic part and the eigenvalue prefactor);  |f| and the two
+//   eigenvalue roots as x rsqrt(x).
+__device__ __forceinline__ void closure_fast(double c, double E, double Fx, double Fy, CloF& q)
+{
+    const double Es = (E > ARK_E_FLOOR) ? E : ARK_E_FLOOR;
+    const double ice = rcp_fast(c * Es);
+    double fx = Fx * ice, fy = Fy * ice;
+    double f2 = fx * fx + fy * fy;
+    if (f2 > 1.0) {                        // PAPER.md:513 (rare: non-realizable cell)
+        const double r = rsqrt_fast(f2);
+        fx *= r; fy *= r; f2 = 1.0;
+    }
+    const double s = 4.0 - 3.0 * f2;       // >= 1
+    const double rs = rsqrt_fast(s);
+    const double xi = s * rs;
+    const double t2 = 2.0 + xi, t5 = 5.0 + 2.0 * xi;
+    const double rp = rcp_fast(t2 * t5);
+    const double i2 = rp * t5, i5 = rp * t2;            // 1/(2+xi), 1/(5+2xi)
+    const double chi = (3.0 + 4.0 * f2) * i5;
+    const double q3 = 3.0 * i2;
+    const double iso = 0.5 - 0.5 * chi;
+    const double Eq = E * q3;
+    q.Pxx = fma(Eq * fx, fx, E * iso); q.Pxy = Eq * fx * fy; q.Pyy = fma(Eq * fy, fy, E * iso);
+    q.f = sqrt_fast(f2);
+    // Eq. 14
+    const double a = (xi - 1.0) * t2;
+    const double k = 0.81649658092772603273 * rs * i2 * c;   // c sqrt(2/3)/(xi (xi+2))
+    const double a2 = a + a;
+    const double rx = k * sqrt_fast(a * fma(3.0 * fy, fy, a2));
+    const double ry = k * sqrt_fast(a * fma(3.0 * fx, fx, a2));
+    const double mx = c * fx * rs, my = c * fy * rs;
+    q.lmaxx = mx + rx; q.lminx = mx - rx;
+    q.lmaxy = my + ry; q.lminy = my - ry;
+}
+
+// Face coefficients with ONE reciprocal: with D = dl - kk l+ l- (kk = 3 sigma_f delta (1 - f_f^2)/c >= 0, l+ l- <= 0),
+//   1/dl = D/(dl D),  alpha = 1/(1 - kk Lambda) = dl/D = dl^2/(dl D).
+__device__ __forceinline__ void face_fast(double k3, double lminL, double lmaxL, double fL, double stL,
+                                          double lminR, double lmaxR, double fR, double stR, Face& fc)
+{
+    const double lp = fmax(0.0, fmax(lmaxL, lmaxR));
+    const double lm = fmin(0.0, fmin(lminL, lminR));
+    const double dl = lp - lm;
+    fc.sig = 0.5 * (stL + stR);
+    const double ff = 0.5 * (fL + fR);
+    const double kk = k3 * fc.sig * fma(-ff, ff, 1.0);
+    const bool ok = dl > 0.0;
+    const double dls = ok ? dl : 1.0;
+    const double lplm = lp * lm;
+    const double D = fma(-kk, lplm, dls);
+    const double qq = rcp_fast(dls * D);
+    const double idl = qq * D;
+    fc.ap = ok ? lp * idl : 0.5;
+    fc.am = ok ? -lm * idl : 0.5;
+    fc.Lam = lplm * idl;                   // 0 when dl == 0 (then l+ = l- = 0)
+    fc.alpha = dls * dls * qq;             // 1 when dl == 0
+}
+
+// Scheme dispatch: the default scheme uses the fast forms above, every other switch combination the generic ones.
+template <bool SD>
+__device__ __forceinline__ void cell_closure(const Scheme& s, double c, const Raw& u, CloF& q)
+{
+    if (SD) closure_fast(c, u.E, u.Fx, u.Fy, q);
+    else {
+        Clo t; closure_eval<false, false>(s, c, u.E, u.Fx, u.Fy, t, nullptr);
+        q.Pxx = t.Pxx; q.Pxy = t.Pxy; q.Pyy = t.Pyy; q.f = t.f;
+        q.lminx = t.lmin[0]; q.lmaxx = t.lmax[0]; q.lminy = t.lmin[1]; q.lmaxy = t.lmax[1];
+    }
+}
+template <bool SD>
+__device__ __forceinline__ void cell_face(const Scheme& s, double c, double delta, double k3,
+                                          double lminL, double lmaxL, double fL, double stL,
+                                          double lminR, double lmaxR, double fR, double stR, Face& fc)
+{
+    if (SD) face_fast(k3, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, fc);
+    else face_eval<false>(s, c, delta, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, fc);
+}
 
 template <bool SD>
 __global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
@@ -46,19 +147,32 @@ __global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fi
     const bool upd = (t >= 1 && t <= TX - 2 && i >= 0 && i < g.nx);
     const double c = g.c, c2 = c * c;
     const double rdx = dt / g.dx, rdy = dt / g.dy;
+    const double k3x = 3.0 * g.dx / c, k3y = 3.0 * g.dy / c;   // Eq. 25: 3 sigma dx (1-f^2)/c = k3 sigma (1-f^2)
+    const double qc = 0.25 * c * dt;                            // WB source weight (Eqs. 18-19) times dt
     const bool wb = SD ? true : (s.wb != 0);
 
+    // resolve the column once
+    int xmode = 0, ii = i, xside = 0;
+    if (!col_active) xmode = 2;
+    else if (i < 0 || i >= g.nx) {
+        xside = (i < 0) ? XLO : XHI;
+        const int bc = g.bc[xside];
+        if (bc == BC_DIRICHLET) { xmode = 1; ii = 0; }
+        else if (bc == BC_PERIODIC) ii = (i < 0) ? g.nx - 1 : 0;
+        else ii = (i < 0) ? 0 : g.nx - 1;
+    }
+
     // prologue: rows j0-1 (south) and j0 (centre); flux through the south face of row j0
-    Raw uS = load_raw(f, g, i, j0 - 1, col_active);
-    Raw uC = load_raw(f, g, i, j0, col_active);
-    Raw uN = load_raw(f, g, i, j0 + 1, col_active && (j0 + 1 <= g.ny));
-    Clo qS, qC;
-    closure_eval<false, SD>(s, c, uS.E, uS.Fx, uS.Fy, qS, nullptr);
-    closure_eval<false, SD>(s, c, uC.E, uC.Fx, uC.Fy, qC, nullptr);
+    Raw uS = load_row(f, g, xmode, ii, xside, j0 - 1);
+    Raw uC = load_row(f, g, xmode, ii, xside, j0);
+    Raw uN = load_row(f, g, xmode, ii, xside, j0 + 1);
+    CloF qS, qC;
+    cell_closure<SD>(s, c, uS, qS);
+    cell_closure<SD>(s, c, uC, qC);
     double Hs0, Hs1, Hs2, Ss;   // south flux and sigma_s (Fy_{j-1} + Fy_j)
     {
         Face fs;
-        face_eval<SD>(s, c, g.dy, qS.lmin[1], qS.lmax[1], qS.f, uS.st, qC.lmin[1], qC.lmax[1], qC.f, uC.st, fs);
+        cell_face<SD>(s, c, g.dy, k3y, qS.lminy, qS.lmaxy, qS.f, uS.st, qC.lminy, qC.lmaxy, qC.f, uC.st, fs);
         Hs0 = fs.alpha * (fs.ap * uS.Fy + fs.am * uC.Fy + fs.Lam * (uC.E - uS.E));
         Hs1 = c2 * (fs.ap * qS.Pxy + fs.am * qC.Pxy) + fs.Lam * (uC.Fx - uS.Fx);
         Hs2 = c2 * (fs.ap * qS.Pyy + fs.am * qC.Pyy) + fs.Lam * (uC.Fy - uS.Fy);
@@ -67,27 +181,27 @@ __global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fi
 
     for (int j = j0; j < j1; ++j) {
         // prefetch the raw state two rows ahead
-        const Raw uNN = load_raw(f, g, i, j + 2, col_active && (j + 2 <= g.ny) && (j + 1 < j1));
-        // closure of the north cell, north face
-        Clo qN;
-        closure_eval<false, SD>(s, c, uN.E, uN.Fx, uN.Fy, qN, nullptr);
+        const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
+        // publish the x-face data of this cell (computed one row ago)
+        XPub me; me.E = uC.E; me.Fx = uC.Fx; me.Fy = uC.Fy; me.Pxx = qC.Pxx; me.Pxy = qC.Pxy;
+        me.lmin = qC.lminx; me.lmax = qC.lmaxx; me.f = qC.f; me.st = uC.st;
+        pub[t] = me;
+        // closure of the north cell, north face (independent of the neighbours: overlaps the barrier)
+        CloF qN;
+        cell_closure<SD>(s, c, uN, qN);
         Face fn;
-        face_eval<SD>(s, c, g.dy, qC.lmin[1], qC.lmax[1], qC.f, uC.st, qN.lmin[1], qN.lmax[1], qN.f, uN.st, fn);
+        cell_face<SD>(s, c, g.dy, k3y, qC.lminy, qC.lmaxy, qC.f, uC.st, qN.lminy, qN.lmaxy, qN.f, uN.st, fn);
         const double Hn0 = fn.alpha * (fn.ap * uC.Fy + fn.am * uN.Fy + fn.Lam * (uN.E - uC.E));
         const double Hn1 = c2 * (fn.ap * qC.Pxy + fn.am * qN.Pxy) + fn.Lam * (uN.Fx - uC.Fx);
         const double Hn2 = c2 * (fn.ap * qC.Pyy + fn.am * qN.Pyy) + fn.Lam * (uN.Fy - uC.Fy);
         const double Sn = fn.sig * (uC.Fy + uN.Fy);
-
-        // publish the x-face data of this cell, read the east neighbour's
-        XPub me; me.E = uC.E; me.Fx = uC.Fx; me.Fy = uC.Fy; me.Pxx = qC.Pxx; me.Pxy = qC.Pxy;
-        me.lmin = qC.lmin[0]; me.lmax = qC.lmax[0]; me.f = qC.f; me.st = uC.st;
-        pub[t] = me;
         __syncthreads();
+        // east face from the east neighbour's published data
         double Ge0 = 0.0, Ge1 = 0.0, Ge2 = 0.0, Se = 0.0;
         if (t < TX - 1) {
             const XPub R = pub[t + 1];
             Face fe;
-            face_eval<SD>(s, c, g.dx, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
+            cell_face<SD>(s, c, g.dx, k3x, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
             Ge0 = fe.alpha * (fe.ap * me.Fx + fe.am * R.Fx + fe.Lam * (R.E - me.E));
             Ge1 = c2 * (fe.ap * me.Pxx + fe.am * R.Pxx) + fe.Lam * (R.Fx - me.Fx);
             Ge2 = c2 * (fe.ap * me.Pxy + fe.am * R.Pxy) + fe.Lam * (R.Fy - me.Fy);
@@ -97,14 +211,14 @@ __global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fi
         __syncthreads();
         if (upd) {
             const double Gw0 = flx[0][t - 1], Gw1 = flx[1][t - 1], Gw2 = flx[2][t - 1], Sw = flx[3][t - 1];
-            double SFx, SFy;
-            if (wb) { SFx = -0.25 * c * (Se + Sw); SFy = -0.25 * c * (Sn + Ss); }
-            else { SFx = -c * uC.st * uC.Fx; SFy = -c * uC.st * uC.Fy; }
-            const double SE = -c * uC.sa * uC.E;
+            double dSFx, dSFy;   // dt * S^F
+            if (wb) { dSFx = -qc * (Se + Sw); dSFy = -qc * (Sn + Ss); }
+            else { dSFx = -dt * c * uC.st * uC.Fx; dSFy = -dt * c * uC.st * uC.Fy; }
+            const double dSE = -dt * c * uC.sa * uC.E;
             const long long id = (long long)j * g.nx + i;
-            oE[id]  = uC.E  - (rdx * (Ge0 - Gw0) + rdy * (Hn0 - Hs0) - dt * SE);
-            oFx[id] = uC.Fx - (rdx * (Ge1 - Gw1) + rdy * (Hn1 - Hs1) - dt * SFx);
-            oFy[id] = uC.Fy - (rdx * (Ge2 - Gw2) + rdy * (Hn2 - Hs2) - dt * SFy);
+            oE[id]  = uC.E  - (rdx * (Ge0 - Gw0) + rdy * (Hn0 - Hs0) - dSE);
+            oFx[id] = uC.Fx - (rdx * (Ge1 - Gw1) + rdy * (Hn1 - Hs1) - dSFx);
+            oFy[id] = uC.Fy - (rdx * (Ge2 - Gw2) + rdy * (Hn2 - Hs2) - dSFy);
         }
         // shift the window north
         uC = uN; qC = qN; uN = uNN;
