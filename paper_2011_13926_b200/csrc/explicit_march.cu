@@ -14,7 +14,20 @@
 
 namespace ark {
 
-static constexpr int TX = 128;
+// tuning knobs (defaults chosen by measurement on B200)
+#ifndef ARK_MARCH_TX
+#define ARK_MARCH_TX 128
+#endif
+#ifndef ARK_MARCH_UNROLL
+#define ARK_MARCH_UNROLL 1
+#endif
+#ifndef ARK_MARCH_MINB
+#define ARK_MARCH_MINB 4
+#endif
+#ifndef ARK_MARCH_RY
+#define ARK_MARCH_RY 32
+#endif
+static constexpr int TX = ARK_MARCH_TX;
 
 struct Raw { double E, Fx, Fy, st, sa; };
 
@@ -28,7 +41,7 @@ __device__ __forceinline__ Raw load_row(const Fields& f, const Grid& g, int xmod
     if (xmode == 2) return r;
     if (j >= 0 && j < g.ny) {
         if (xmode == 0) {
-            const long long id = (long long)j * g.nx + ii;
+            const unsigned int id = (unsigned int)j * (unsigned int)g.nx + (unsigned int)ii;
             r.E = f.E[id]; r.Fx = f.Fx[id]; r.Fy = f.Fy[id]; r.st = f.st[id]; r.sa = f.sa[id];
         } else {
             r.E = f.gh[xside][0][j]; r.Fx = f.gh[xside][1][j]; r.Fy = f.gh[xside][2][j]; r.sa = f.gh[xside][3][j]; r.st = f.gh[xside][4][j];
@@ -51,7 +64,7 @@ __device__ __forceinline__ Raw load_row(const Fields& f, const Grid& g, int xmod
 struct XPub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };   // what the west neighbour needs for its east face
 
 // What the march kernel keeps per cell: pressure, Eq. 14 eigenvalues for both face orientations, |f|.
-struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };
+struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };   // Pxx.. hold c^2 P (what the flux needs)
 
 // Default-scheme closure with 2 reciprocals and 4 reciprocal square roots per cell:
 //   1/(cE);  rs = 1/sqrt(4 - 3 f^2) gives xi = s rs and 1/xi = rs;  one reciprocal of (2+xi)(5+2xi) gives both
@@ -62,11 +75,15 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double Es = (E > ARK_E_FLOOR) ? E : ARK_E_FLOOR;
     const double ice = rcp_fast(c * Es);
     double fx = Fx * ice, fy = Fy * ice;
-    double f2 = fx * fx + fy * fy;
-    if (f2 > 1.0) {                        // PAPER.md:513 (rare: non-realizable cell)
-        const double r = rsqrt_fast(f2);
-        fx *= r; fy *= r; f2 = 1.0;
-    }
+    const double f2raw = fx * fx + fy * fy;
+    // |f| and the clamp of PAPER.md:513, branch-free: one rsqrt serves both (f = f2 rsqrt(f2); rescale by rsqrt(f2) if f2 > 1)
+    const bool tiny = !(f2raw > 1e-290);
+    const double rf = rsqrt_fast(tiny ? 1.0 : f2raw);
+    const bool clamp = f2raw > 1.0;
+    const double sc = clamp ? rf : 1.0;
+    fx *= sc; fy *= sc;
+    const double f2 = clamp ? 1.0 : f2raw;
+    q.f = clamp ? 1.0 : (tiny ? 0.0 : f2raw * rf);
     const double s = 4.0 - 3.0 * f2;       // >= 1
     const double rs = rsqrt_fast(s);
     const double xi = s * rs;
@@ -76,24 +93,27 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double chi = (3.0 + 4.0 * f2) * i5;
     const double q3 = 3.0 * i2;
     const double iso = 0.5 - 0.5 * chi;
-    const double Eq = E * q3;
-    q.Pxx = fma(Eq * fx, fx, E * iso); q.Pxy = Eq * fx * fy; q.Pyy = fma(Eq * fy, fy, E * iso);
-    q.f = sqrt_fast(f2);
+    const double Ec = (c * c) * E;                      // c^2 folded into the stored pressure
+    const double Eq = Ec * q3, Ei = Ec * iso;
+    q.Pxx = fma(Eq * fx, fx, Ei); q.Pxy = Eq * fx * fy; q.Pyy = fma(Eq * fy, fy, Ei);
     // Eq. 14
     const double a = (xi - 1.0) * t2;
-    const double k = 0.81649658092772603273 * rs * i2 * c;   // c sqrt(2/3)/(xi (xi+2))
+    const double crs = c * rs;                                // c/xi
+    const double k = 0.81649658092772603273 * crs * i2;       // c sqrt(2/3)/(xi (xi+2))
     const double a2 = a + a;
     const double rx = k * sqrt_fast(a * fma(3.0 * fy, fy, a2));
     const double ry = k * sqrt_fast(a * fma(3.0 * fx, fx, a2));
-    const double mx = c * fx * rs, my = c * fy * rs;
+    const double mx = fx * crs, my = fy * crs;
     q.lmaxx = mx + rx; q.lminx = mx - rx;
     q.lmaxy = my + ry; q.lminy = my - ry;
 }
 
-// Face coefficients with ONE reciprocal: with D = dl - kk l+ l- (kk = 3 sigma_f delta (1 - f_f^2)/c >= 0, l+ l- <= 0),
-//   1/dl = D/(dl D),  alpha = 1/(1 - kk Lambda) = dl/D = dl^2/(dl D).
+// Face coefficients with ONE reciprocal.  With D = dl - kk l+ l- (kk = 3 sigma_f delta (1 - f_f^2)/c >= 0, l+ l- <= 0):
+//   1/dl = D/(dl D),  alpha = 1/(1 - kk Lambda) = dl/D = dl^2/(dl D).   a- = 1 - a+ is never formed: the fluxes use
+//   a+ x_L + a- x_R = x_R + a+ (x_L - x_R).
+struct FaceF { double ap, Lam, alpha, sig; };
 __device__ __forceinline__ void face_fast(double k3, double lminL, double lmaxL, double fL, double stL,
-                                          double lminR, double lmaxR, double fR, double stR, Face& fc)
+                                          double lminR, double lmaxR, double fR, double stR, FaceF& fc)
 {
     const double lp = fmax(0.0, fmax(lmaxL, lmaxR));
     const double lm = fmin(0.0, fmin(lminL, lminR));
@@ -103,14 +123,12 @@ __device__ __forceinline__ void face_fast(double k3, double lminL, double lmaxL,
     const double kk = k3 * fc.sig * fma(-ff, ff, 1.0);
     const bool ok = dl > 0.0;
     const double dls = ok ? dl : 1.0;
-    const double lplm = lp * lm;
-    const double D = fma(-kk, lplm, dls);
+    const double D = fma(-kk * lp, lm, dls);
     const double qq = rcp_fast(dls * D);
-    const double idl = qq * D;
-    fc.ap = ok ? lp * idl : 0.5;
-    fc.am = ok ? -lm * idl : 0.5;
-    fc.Lam = lplm * idl;                   // 0 when dl == 0 (then l+ = l- = 0)
-    fc.alpha = dls * dls * qq;             // 1 when dl == 0
+    const double apv = lp * (qq * D);
+    fc.ap = ok ? apv : 0.5;
+    fc.Lam = lm * apv;                     // l+ l-/dl; 0 when dl == 0 (then l+ = l- = 0)
+    fc.alpha = dls * (dls * qq);           // 1 when dl == 0
 }
 
 // Scheme dispatch: the default scheme uses the fast forms above, every other switch combination the generic ones.
@@ -120,24 +138,39 @@ __device__ __forceinline__ void cell_closure(const Scheme& s, double c, const Ra
     if (SD) closure_fast(c, u.E, u.Fx, u.Fy, q);
     else {
         Clo t; closure_eval<false, false>(s, c, u.E, u.Fx, u.Fy, t, nullptr);
-        q.Pxx = t.Pxx; q.Pxy = t.Pxy; q.Pyy = t.Pyy; q.f = t.f;
+        const double c2 = c * c;
+        q.Pxx = c2 * t.Pxx; q.Pxy = c2 * t.Pxy; q.Pyy = c2 * t.Pyy; q.f = t.f;
         q.lminx = t.lmin[0]; q.lmaxx = t.lmax[0]; q.lminy = t.lmin[1]; q.lmaxy = t.lmax[1];
     }
 }
 template <bool SD>
 __device__ __forceinline__ void cell_face(const Scheme& s, double c, double delta, double k3,
                                           double lminL, double lmaxL, double fL, double stL,
-                                          double lminR, double lmaxR, double fR, double stR, Face& fc)
+                                          double lminR, double lmaxR, double fR, double stR, FaceF& fc)
 {
     if (SD) face_fast(k3, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, fc);
-    else face_eval<false>(s, c, delta, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, fc);
+    else {
+        Face t; face_eval<false>(s, c, delta, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, t);
+        fc.ap = t.ap; fc.Lam = t.Lam; fc.alpha = t.alpha; fc.sig = t.sig;     // a+ + a- = 1 in every scheme variant
+    }
 }
 
+// Flux of Eq. 13 through one face (normal component Fn, pressures already times c^2):
+//   G0 = alpha (a+ Fn_L + a- Fn_R + Lam (E_R - E_L)),  G1/G2 = a+ P_L + a- P_R + Lam (F_R - F_L),  S = sigma_f (Fn_L + Fn_R)
+#define ARK_FACE_FLUX(fc, EL, ER, FnL, FnR, FtL, FtR, PnL, PnR, PtL, PtR, G0, Gn, Gt, S)              \
+    do {                                                                                             \
+        const double dFn_ = (FnR) - (FnL);                                                           \
+        G0 = (fc).alpha * fma((fc).Lam, (ER) - (EL), fma(-(fc).ap, dFn_, (FnR)));                    \
+        Gn = fma((fc).Lam, dFn_, fma((fc).ap, (PnL) - (PnR), (PnR)));                                \
+        Gt = fma((fc).Lam, (FtR) - (FtL), fma((fc).ap, (PtL) - (PtR), (PtR)));                       \
+        S = (fc).sig * ((FnL) + (FnR));                                                              \
+    } while (0)
+
 template <bool SD>
-__global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
+__global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
                                                             double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
 {
-    __shared__ XPub pub[TX];
+    __shared__ XPub pub[TX + 1];   // +1: the last thread reads a (unused) right neighbour
     __shared__ double flx[4][TX];
     const int t = threadIdx.x;
     const int i = blockIdx.x * (TX - 2) - 1 + t;
@@ -145,7 +178,7 @@ __global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fi
     const int j1 = min(j0 + RY, g.ny);
     const bool col_active = (i <= g.nx);                    // i in [-1, nx]
     const bool upd = (t >= 1 && t <= TX - 2 && i >= 0 && i < g.nx);
-    const double c = g.c, c2 = c * c;
+    const double c = g.c, cdt = c * dt;
     const double rdx = dt / g.dx, rdy = dt / g.dy;
     const double k3x = 3.0 * g.dx / c, k3y = 3.0 * g.dy / c;   // Eq. 25: 3 sigma dx (1-f^2)/c = k3 sigma (1-f^2)
     const double qc = 0.25 * c * dt;                            // WB source weight (Eqs. 18-19) times dt
@@ -171,14 +204,16 @@ __global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fi
     cell_closure<SD>(s, c, uC, qC);
     double Hs0, Hs1, Hs2, Ss;   // south flux and sigma_s (Fy_{j-1} + Fy_j)
     {
-        Face fs;
+        FaceF fs;
         cell_face<SD>(s, c, g.dy, k3y, qS.lminy, qS.lmaxy, qS.f, uS.st, qC.lminy, qC.lmaxy, qC.f, uC.st, fs);
-        Hs0 = fs.alpha * (fs.ap * uS.Fy + fs.am * uC.Fy + fs.Lam * (uC.E - uS.E));
-        Hs1 = c2 * (fs.ap * qS.Pxy + fs.am * qC.Pxy) + fs.Lam * (uC.Fx - uS.Fx);
-        Hs2 = c2 * (fs.ap * qS.Pyy + fs.am * qC.Pyy) + fs.Lam * (uC.Fy - uS.Fy);
-        Ss = fs.sig * (uS.Fy + uC.Fy);
+        // y-face: normal = y.  (G0, Gn, Gt) = (E, Fy, Fx) fluxes
+        ARK_FACE_FLUX(fs, uS.E, uC.E, uS.Fy, uC.Fy, uS.Fx, uC.Fx, qS.Pyy, qC.Pyy, qS.Pxy, qC.Pxy, Hs0, Hs2, Hs1, Ss);
     }
+    // 32-bit in-plane offsets (host guarantees nx*ny < 2^31)
+    unsigned int row_off = (unsigned int)j0 * (unsigned int)g.nx + (unsigned int)(i < 0 ? 0 : i);
 
+    constexpr int kUnroll = ARK_MARCH_UNROLL;
+#pragma unroll kUnroll
     for (int j = j0; j < j1; ++j) {
         // prefetch the raw state two rows ahead
         const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
@@ -189,37 +224,34 @@ __global__ void __launch_bounds__(TX) explicit_march_kernel(Grid g, Scheme s, Fi
         // closure of the north cell, north face (independent of the neighbours: overlaps the barrier)
         CloF qN;
         cell_closure<SD>(s, c, uN, qN);
-        Face fn;
+        FaceF fn;
         cell_face<SD>(s, c, g.dy, k3y, qC.lminy, qC.lmaxy, qC.f, uC.st, qN.lminy, qN.lmaxy, qN.f, uN.st, fn);
-        const double Hn0 = fn.alpha * (fn.ap * uC.Fy + fn.am * uN.Fy + fn.Lam * (uN.E - uC.E));
-        const double Hn1 = c2 * (fn.ap * qC.Pxy + fn.am * qN.Pxy) + fn.Lam * (uN.Fx - uC.Fx);
-        const double Hn2 = c2 * (fn.ap * qC.Pyy + fn.am * qN.Pyy) + fn.Lam * (uN.Fy - uC.Fy);
-        const double Sn = fn.sig * (uC.Fy + uN.Fy);
+        double Hn0, Hn1, Hn2, Sn;
+        ARK_FACE_FLUX(fn, uC.E, uN.E, uC.Fy, uN.Fy, uC.Fx, uN.Fx, qC.Pyy, qN.Pyy, qC.Pxy, qN.Pxy, Hn0, Hn2, Hn1, Sn);
         __syncthreads();
         // east face from the east neighbour's published data
-        double Ge0 = 0.0, Ge1 = 0.0, Ge2 = 0.0, Se = 0.0;
-        if (t < TX - 1) {
+        double Ge0, Ge1, Ge2, Se;
+        {
             const XPub R = pub[t + 1];
-            Face fe;
+            FaceF fe;
             cell_face<SD>(s, c, g.dx, k3x, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
-            Ge0 = fe.alpha * (fe.ap * me.Fx + fe.am * R.Fx + fe.Lam * (R.E - me.E));
-            Ge1 = c2 * (fe.ap * me.Pxx + fe.am * R.Pxx) + fe.Lam * (R.Fx - me.Fx);
-            Ge2 = c2 * (fe.ap * me.Pxy + fe.am * R.Pxy) + fe.Lam * (R.Fy - me.Fy);
-            Se = fe.sig * (me.Fx + R.Fx);
+            ARK_FACE_FLUX(fe, me.E, R.E, me.Fx, R.Fx, me.Fy, R.Fy, me.Pxx, R.Pxx, me.Pxy, R.Pxy, Ge0, Ge1, Ge2, Se);
         }
         flx[0][t] = Ge0; flx[1][t] = Ge1; flx[2][t] = Ge2; flx[3][t] = Se;
         __syncthreads();
-        if (upd) {
-            const double Gw0 = flx[0][t - 1], Gw1 = flx[1][t - 1], Gw2 = flx[2][t - 1], Sw = flx[3][t - 1];
-            double dSFx, dSFy;   // dt * S^F
-            if (wb) { dSFx = -qc * (Se + Sw); dSFy = -qc * (Sn + Ss); }
-            else { dSFx = -dt * c * uC.st * uC.Fx; dSFy = -dt * c * uC.st * uC.Fy; }
-            const double dSE = -dt * c * uC.sa * uC.E;
-            const long long id = (long long)j * g.nx + i;
-            oE[id]  = uC.E  - (rdx * (Ge0 - Gw0) + rdy * (Hn0 - Hs0) - dSE);
-            oFx[id] = uC.Fx - (rdx * (Ge1 - Gw1) + rdy * (Hn1 - Hs1) - dSFx);
-            oFy[id] = uC.Fy - (rdx * (Ge2 - Gw2) + rdy * (Hn2 - Hs2) - dSFy);
+        {
+            const int tw = (t > 0) ? t - 1 : 0;
+            const double Gw0 = flx[0][tw], Gw1 = flx[1][tw], Gw2 = flx[2][tw], Sw = flx[3][tw];
+            double dSFx, dSFy;   // -dt * S^F
+            if (wb) { dSFx = qc * (Se + Sw); dSFy = qc * (Sn + Ss); }
+            else { dSFx = dt * c * uC.st * uC.Fx; dSFy = dt * c * uC.st * uC.Fy; }
+            const double dSE = cdt * uC.sa * uC.E;
+            const double nE  = uC.E  - fma(rdx, Ge0 - Gw0, fma(rdy, Hn0 - Hs0, dSE));
+            const double nFx = uC.Fx - fma(rdx, Ge1 - Gw1, fma(rdy, Hn1 - Hs1, dSFx));
+            const double nFy = uC.Fy - fma(rdx, Ge2 - Gw2, fma(rdy, Hn2 - Hs2, dSFy));
+            if (upd) { oE[row_off] = nE; oFx[row_off] = nFx; oFy[row_off] = nFy; }
         }
+        row_off += (unsigned int)g.nx;
         // shift the window north
         uC = uN; qC = qN; uN = uNN;
         Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
@@ -232,7 +264,7 @@ cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& 
     const int strips = (g.nx + (TX - 2) - 1) / (TX - 2);
     // rows per block: enough blocks for ~8 per SM, between 4 and 64 rows
     long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
-    int RY = (int)(want < 4 ? 4 : (want > 64 ? 64 : want));
+    int RY = (int)(want < 4 ? 4 : (want > ARK_MARCH_RY ? ARK_MARCH_RY : want));
     if (RY > g.ny) RY = g.ny;
     dim3 grd(strips, (g.ny + RY - 1) / RY);
     if (s.is_default()) explicit_march_kernel<true><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
