@@ -232,7 +232,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "eig_floor")) { if (!(value >= 0.0)) return fail(h, ARK_M1_E_ARG, "eig_floor must be >= 0%s", ""); h->s.eig_floor = value; }
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
-    else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0 or 1%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1 or 2%s", ""); h->explicit_kernel = iv; }
     else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv != 0) return fail(h, ARK_M1_E_ARG, "operator: only 0 (block-stencil) is built%s", ""); h->op_kind = iv; }
     else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
@@ -270,7 +270,9 @@ static int explicit_once(ark_m1* h, double dt)
     const Fields f = fields_of(h);
     double* O = h->U[h->cur ^ 1];
     const bool plain = !h->have_T && !h->source_E;
-    if (h->explicit_kernel == 1 && plain && h->N < (1LL << 31)) {   // the march kernel uses 32-bit in-plane offsets
+    if (h->explicit_kernel == 2 && plain && h->N < (1LL << 31)) {
+        KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_warp(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
+    } else if (h->explicit_kernel == 1 && plain && h->N < (1LL << 31)) {   // the march kernels use 32-bit in-plane offsets
         KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
     } else {
         KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_cell(h->g, h->s, f, dt, 0, O, O + h->N, O + 2 * h->N, h->have_T ? h->T[h->cur ^ 1] : nullptr, h->st));

@@ -258,6 +258,109 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Barrier-free variant: a WARP owns 30 columns (+1 halo lane each side) and exchanges the x-face data with
+// __shfl_down/__shfl_up, so warps never wait for one another and the row body is one basic block.
+// ---------------------------------------------------------------------------------------------------------
+#ifndef ARK_WARP_WPB
+#define ARK_WARP_WPB 4      // warps per block
+#endif
+#ifndef ARK_WARP_MINB
+#define ARK_WARP_MINB 4
+#endif
+static constexpr int WPB = ARK_WARP_WPB;
+static constexpr int WCOLS = 30;
+
+__device__ __forceinline__ double shfl_dn(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+
+template <bool SD>
+__global__ void __launch_bounds__(32 * WPB, ARK_WARP_MINB) explicit_warp_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
+                                                            double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int i = (blockIdx.x * WPB + warp) * WCOLS - 1 + lane;
+    const int j0 = blockIdx.y * RY;
+    const int j1 = min(j0 + RY, g.ny);
+    const bool col_active = (i <= g.nx);
+    const bool upd = (lane >= 1 && lane <= WCOLS && i >= 0 && i < g.nx);
+    const double c = g.c, cdt = c * dt;
+    const double rdx = dt / g.dx, rdy = dt / g.dy;
+    const double k3x = 3.0 * g.dx / c, k3y = 3.0 * g.dy / c;
+    const double qc = 0.25 * c * dt;
+    const bool wb = SD ? true : (s.wb != 0);
+
+    int xmode = 0, ii = i, xside = 0;
+    if (!col_active) xmode = 2;
+    else if (i < 0 || i >= g.nx) {
+        xside = (i < 0) ? XLO : XHI;
+        const int bc = g.bc[xside];
+        if (bc == BC_DIRICHLET) { xmode = 1; ii = 0; }
+        else if (bc == BC_PERIODIC) ii = (i < 0) ? g.nx - 1 : 0;
+        else ii = (i < 0) ? 0 : g.nx - 1;
+    }
+    Raw uS = load_row(f, g, xmode, ii, xside, j0 - 1);
+    Raw uC = load_row(f, g, xmode, ii, xside, j0);
+    Raw uN = load_row(f, g, xmode, ii, xside, j0 + 1);
+    CloF qS, qC;
+    cell_closure<SD>(s, c, uS, qS);
+    cell_closure<SD>(s, c, uC, qC);
+    double Hs0, Hs1, Hs2, Ss;
+    {
+        FaceF fs;
+        cell_face<SD>(s, c, g.dy, k3y, qS.lminy, qS.lmaxy, qS.f, uS.st, qC.lminy, qC.lmaxy, qC.f, uC.st, fs);
+        ARK_FACE_FLUX(fs, uS.E, uC.E, uS.Fy, uC.Fy, uS.Fx, uC.Fx, qS.Pyy, qC.Pyy, qS.Pxy, qC.Pxy, Hs0, Hs2, Hs1, Ss);
+    }
+    unsigned int row_off = (unsigned int)j0 * (unsigned int)g.nx + (unsigned int)(i < 0 ? 0 : i);
+
+    for (int j = j0; j < j1; ++j) {
+        const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
+        // east neighbour's x-face data (lane + 1)
+        const double RE = shfl_dn(uC.E), RFx = shfl_dn(uC.Fx), RFy = shfl_dn(uC.Fy), RPxx = shfl_dn(qC.Pxx), RPxy = shfl_dn(qC.Pxy);
+        const double Rlmin = shfl_dn(qC.lminx), Rlmax = shfl_dn(qC.lmaxx), Rf = shfl_dn(qC.f), Rst = shfl_dn(uC.st);
+        // north cell closure + north face
+        CloF qN;
+        cell_closure<SD>(s, c, uN, qN);
+        FaceF fn;
+        cell_face<SD>(s, c, g.dy, k3y, qC.lminy, qC.lmaxy, qC.f, uC.st, qN.lminy, qN.lmaxy, qN.f, uN.st, fn);
+        double Hn0, Hn1, Hn2, Sn;
+        ARK_FACE_FLUX(fn, uC.E, uN.E, uC.Fy, uN.Fy, uC.Fx, uN.Fx, qC.Pyy, qN.Pyy, qC.Pxy, qN.Pxy, Hn0, Hn2, Hn1, Sn);
+        // east face
+        double Ge0, Ge1, Ge2, Se;
+        {
+            FaceF fe;
+            cell_face<SD>(s, c, g.dx, k3x, qC.lminx, qC.lmaxx, qC.f, uC.st, Rlmin, Rlmax, Rf, Rst, fe);
+            ARK_FACE_FLUX(fe, uC.E, RE, uC.Fx, RFx, uC.Fy, RFy, qC.Pxx, RPxx, qC.Pxy, RPxy, Ge0, Ge1, Ge2, Se);
+        }
+        // west flux = east flux of lane - 1
+        const double Gw0 = shfl_up(Ge0), Gw1 = shfl_up(Ge1), Gw2 = shfl_up(Ge2), Sw = shfl_up(Se);
+        double dSFx, dSFy;
+        if (wb) { dSFx = qc * (Se + Sw); dSFy = qc * (Sn + Ss); }
+        else { dSFx = dt * c * uC.st * uC.Fx; dSFy = dt * c * uC.st * uC.Fy; }
+        const double dSE = cdt * uC.sa * uC.E;
+        const double nE  = uC.E  - fma(rdx, Ge0 - Gw0, fma(rdy, Hn0 - Hs0, dSE));
+        const double nFx = uC.Fx - fma(rdx, Ge1 - Gw1, fma(rdy, Hn1 - Hs1, dSFx));
+        const double nFy = uC.Fy - fma(rdx, Ge2 - Gw2, fma(rdy, Hn2 - Hs2, dSFy));
+        if (upd) { oE[row_off] = nE; oFx[row_off] = nFx; oFy[row_off] = nFy; }
+        row_off += (unsigned int)g.nx;
+        uC = uN; qC = qN; uN = uNN;
+        Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
+    }
+}
+
+cudaError_t launch_explicit_warp(const Grid& g, const Scheme& s, const Fields& f, double dt,
+                                 double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st)
+{
+    const int strips = (g.nx + WCOLS * WPB - 1) / (WCOLS * WPB);
+    long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
+    int RY = (int)(want < 4 ? 4 : (want > ARK_MARCH_RY ? ARK_MARCH_RY : want));
+    if (RY > g.ny) RY = g.ny;
+    dim3 grd(strips, (g.ny + RY - 1) / RY);
+    if (s.is_default()) explicit_warp_kernel<true><<<grd, 32 * WPB, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
+    else explicit_warp_kernel<false><<<grd, 32 * WPB, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& f, double dt,
                                   double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st)
 {
