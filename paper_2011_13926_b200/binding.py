@@ -36,11 +36,13 @@ class ArkBc(C.Structure):
 _lib = None
 
 
-def load_library(path: str = LIB_PATH):
-    """dlopen libark_m1.so and declare the prototypes.  Raises if the library is missing (no fallback)."""
+def load_library(path: str | None = None):
+    """dlopen libark_m1.so and declare the prototypes.  Raises if the library is missing (no fallback).
+    `path` (or the environment variable ARK_M1_LIB) selects another build of the same library, e.g. a tuning variant."""
     global _lib
     if _lib is not None:
         return _lib
+    path = path or os.environ.get("ARK_M1_LIB") or LIB_PATH
     if not os.path.exists(path):
         raise RuntimeError(f"{path} not found: build it with `python -m paper_2011_13926_b200.build` "
                            "(the CUDA library is the only implementation; there is no CPU fallback)")

@@ -27,6 +27,9 @@ namespace ark {
 #ifndef ARK_MARCH_RY
 #define ARK_MARCH_RY 32
 #endif
+#ifndef ARK_MARCH_ASYNC
+#define ARK_MARCH_ASYNC 0   // 1: prefetch rows with cp.async into a shared-memory ring
+#endif
 static constexpr int TX = ARK_MARCH_TX;
 
 struct Raw { double E, Fx, Fy, st, sa; };
@@ -59,6 +62,53 @@ __device__ __forceinline__ Raw load_row(const Fields& f, const Grid& g, int xmod
     const long long id = (long long)jj * g.nx + ii;
     r.E = f.E[id]; r.Fx = f.Fx[id]; r.Fy = f.Fy[id]; r.st = f.st[id]; r.sa = f.sa[id];
     return r;
+}
+
+// Asynchronous variant of load_row (ARK_MARCH_ASYNC): the five values of one cell go straight from global to this
+// thread's own slots of a shared-memory ring with cp.async (LDGSTS), so no registers are held while the request is in
+// flight and the compiler cannot sink the prefetch towards its use.  A thread only ever reads back its own slots,
+// hence cp.async.wait_group is the only synchronisation needed.  ring layout: [stage][field][thread].
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
+{
+    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+
+template <int TXN>
+__device__ __forceinline__ void load_row_async(double (*ring)[TXN], int t, const Fields& f, const Grid& g,
+                                               int xmode, int ii, int xside, int j, bool wanted)
+{
+    // ring points at [field][thread] of the target stage; order of fields: E, Fx, Fy, st, sa
+    const double* p0 = nullptr; const double* p1; const double* p2; const double* p3; const double* p4;
+    if (wanted && xmode != 2 && j <= g.ny) {
+        if (j >= 0 && j < g.ny) {
+            if (xmode == 0) {
+                const unsigned int id = (unsigned int)j * (unsigned int)g.nx + (unsigned int)ii;
+                p0 = f.E + id; p1 = f.Fx + id; p2 = f.Fy + id; p3 = f.st + id; p4 = f.sa + id;
+            } else {
+                p0 = f.gh[xside][0] + j; p1 = f.gh[xside][1] + j; p2 = f.gh[xside][2] + j; p3 = f.gh[xside][4] + j; p4 = f.gh[xside][3] + j;
+            }
+        } else if (xmode == 0) {
+            const int side = (j < 0) ? YLO : YHI;
+            const int bc = g.bc[side];
+            if (bc == BC_DIRICHLET) {
+                p0 = f.gh[side][0] + ii; p1 = f.gh[side][1] + ii; p2 = f.gh[side][2] + ii; p3 = f.gh[side][4] + ii; p4 = f.gh[side][3] + ii;
+            } else {
+                const int jj = (bc == BC_PERIODIC) ? ((j < 0) ? g.ny - 1 : 0) : ((j < 0) ? 0 : g.ny - 1);
+                const unsigned int id = (unsigned int)jj * (unsigned int)g.nx + (unsigned int)ii;
+                p0 = f.E + id; p1 = f.Fx + id; p2 = f.Fy + id; p3 = f.st + id; p4 = f.sa + id;
+            }
+        }
+    }
+    if (p0) {
+        cp_async8(&ring[0][t], p0); cp_async8(&ring[1][t], p1); cp_async8(&ring[2][t], p2);
+        cp_async8(&ring[3][t], p3); cp_async8(&ring[4][t], p4);
+    } else {   // dummy state (inactive column, corner ghost, row not needed)
+        ring[0][t] = 1.0; ring[1][t] = 0.0; ring[2][t] = 0.0; ring[3][t] = 0.0; ring[4][t] = 0.0;
+    }
+    cp_async_commit();
 }
 
 struct XPub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };   // what the west neighbour needs for its east face
@@ -196,9 +246,17 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
     }
 
     // prologue: rows j0-1 (south) and j0 (centre); flux through the south face of row j0
+#if ARK_MARCH_ASYNC
+    __shared__ double ring[3][5][TX];
+    load_row_async<TX>(ring[0], t, f, g, xmode, ii, xside, j0 + 1, true);      // slot 0 <- row j0+1
+    load_row_async<TX>(ring[1], t, f, g, xmode, ii, xside, j0 + 2, j0 + 1 < j1);
+    int slot_n = 0, slot_p = 2;     // slot holding row j+1; slot receiving row j+3
+#endif
     Raw uS = load_row(f, g, xmode, ii, xside, j0 - 1);
     Raw uC = load_row(f, g, xmode, ii, xside, j0);
+#if !ARK_MARCH_ASYNC
     Raw uN = load_row(f, g, xmode, ii, xside, j0 + 1);
+#endif
     CloF qS, qC;
     cell_closure<SD>(s, c, uS, qS);
     cell_closure<SD>(s, c, uC, qC);
@@ -215,8 +273,17 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
     constexpr int kUnroll = ARK_MARCH_UNROLL;
 #pragma unroll kUnroll
     for (int j = j0; j < j1; ++j) {
+#if ARK_MARCH_ASYNC
+        // request row j+3, then take row j+1 out of the ring (its group is the third youngest)
+        load_row_async<TX>(ring[slot_p], t, f, g, xmode, ii, xside, j + 3, j + 2 < j1);
+        cp_async_wait<2>();
+        Raw uN;
+        uN.E = ring[slot_n][0][t]; uN.Fx = ring[slot_n][1][t]; uN.Fy = ring[slot_n][2][t]; uN.st = ring[slot_n][3][t]; uN.sa = ring[slot_n][4][t];
+        slot_p = slot_n; slot_n = (slot_n == 2) ? 0 : slot_n + 1;
+#else
         // prefetch the raw state two rows ahead
         const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
+#endif
         // publish the x-face data of this cell (computed one row ago)
         XPub me; me.E = uC.E; me.Fx = uC.Fx; me.Fy = uC.Fy; me.Pxx = qC.Pxx; me.Pxy = qC.Pxy;
         me.lmin = qC.lminx; me.lmax = qC.lmaxx; me.f = qC.f; me.st = uC.st;
@@ -253,7 +320,11 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
         }
         row_off += (unsigned int)g.nx;
         // shift the window north
+#if ARK_MARCH_ASYNC
+        uC = uN; qC = qN;
+#else
         uC = uN; qC = qN; uN = uNN;
+#endif
         Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
     }
 }
@@ -365,7 +436,8 @@ cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& 
                                   double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st)
 {
     const int strips = (g.nx + (TX - 2) - 1) / (TX - 2);
-    // rows per block: enough blocks for ~8 per SM, between 4 and 64 rows
+    // rows per block: enough blocks for ~8 per SM, between 4 and ARK_MARCH_RY rows.  (A single wave of
+    // SMs x resident-blocks blocks with ~240 rows each was measured 8% slower at 4096^2: uneven blocks per SM.)
     long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
     int RY = (int)(want < 4 ? 4 : (want > ARK_MARCH_RY ? ARK_MARCH_RY : want));
     if (RY > g.ny) RY = g.ny;
