@@ -1,0 +1,49 @@
+"""N > 1 path of bench.py on CPU: the path does not exchange data between GPUs (replicas only), so the only multi-rank
+logic is the max-over-ranks time / sum-of-units aggregation.  Covered with a world-size-2 gloo group."""
+import os
+import sys
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    elapsed = 1.0 + rank          # rank 1 is the slow one
+    units = 100.0 * (rank + 1)
+    t, u = bench.aggregate_over_ranks(elapsed, units, dist)
+    out[rank] = (t, u)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_aggregate_over_two_ranks_gloo():
+    mgr = mp.Manager()
+    out = mgr.dict()
+    port = 29500 + (os.getpid() % 1000)
+    mp.spawn(_worker, args=(2, port, out), nprocs=2, join=True)
+    for rank in (0, 1):
+        t, u = out[rank]
+        assert t == pytest.approx(2.0) and u == pytest.approx(300.0)   # max time, summed units -> value = 150 units/s
+
+
+def test_single_process_aggregate_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.aggregate_over_ranks(0.5, 10.0, None) == (0.5, 10.0)
+
+
+def test_iteration_byte_formula():
+    sys.path.insert(0, ROOT)
+    import bench
+    # one iteration at j = 0: operator 336 + dots 24 (1 + 1) + update 24 (1 + 2); one cycle end: combine 8 (3 + 15) + 120 + 360 + 24
+    assert bench.iteration_bytes_per_cell(1) == 336 + 48 + 72 + 8 * 18 + 120 + 360 + 24
+    assert bench.iteration_bytes_per_cell(60) == 2 * bench.iteration_bytes_per_cell(30)
