@@ -37,6 +37,7 @@ struct ark_m1 {
     int ortho, explicit_kernel, op_kind;
     // implicit workspace (lazy)
     BlockMatrix A;
+    MfPlanes mf;       // matrix-free coefficient planes (op_kind == 1)
     double* V;         // (m+1) vectors of `stride` doubles
     double* tvec;      // 3N
     long long stride;
@@ -156,7 +157,9 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
 static void free_implicit(ark_m1* h)
 {
     cudaFree(h->A.off); cudaFree(h->A.C); cudaFree(h->A.Minv); cudaFree(h->A.b); cudaFree(h->V); cudaFree(h->tvec); cudaFree(h->wblock);
-    h->A.off = h->A.C = h->A.Minv = h->A.b = nullptr; h->V = h->tvec = nullptr; h->wblock = nullptr; h->m_alloc = 0;
+    cudaFree(h->mf.J); cudaFree(h->mf.fE); cudaFree(h->mf.fN); cudaFree(h->mf.dE); cudaFree(h->mf.dF); cudaFree(h->mf.xlo); cudaFree(h->mf.ylo);
+    memset(&h->mf, 0, sizeof h->mf);
+    h->A.off = h->A.C = h->A.Minv = h->A.b = nullptr; h->V = h->tvec = nullptr; h->wblock = nullptr; h->m_alloc = 0; h->maxit_alloc = 0;
 }
 
 void ark_m1_destroy(ark_m1* h)
@@ -234,7 +237,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
     else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1 or 2%s", ""); h->explicit_kernel = iv; }
     else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
-    else if (!strcmp(key, "operator")) { if (iv != 0) return fail(h, ARK_M1_E_ARG, "operator: only 0 (block-stencil) is built%s", ""); h->op_kind = iv; }
+    else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
     else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
     return 0;
 }
@@ -346,17 +349,31 @@ const char* ark_m1_last_error(const ark_m1* h) { return h ? h->err : "null handl
 static int ensure_implicit(ark_m1* h, int m, int maxit)
 {
     const size_t N = (size_t)h->N, n = 3 * N;
-    if (h->m_alloc >= m && h->maxit_alloc >= maxit) return 0;
+    const bool have_op = (h->op_kind == 0) ? (h->A.off != nullptr) : (h->mf.J != nullptr);
+    if (h->m_alloc >= m && h->maxit_alloc >= maxit && have_op) return 0;
     CU(cudaStreamSynchronize(h->st));
     const long long before = h->bytes;
     (void)before;
-    if (h->A.off == nullptr) {
+    if (h->A.Minv == nullptr) {
         int rc;
-        if ((rc = dmalloc(h, (void**)&h->A.off, 36 * N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->A.C, 9 * N * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->A.Minv, 9 * N * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->A.b, n * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->tvec, n * sizeof(double)))) return rc;
+    }
+    if (h->op_kind == 0 && h->A.off == nullptr) {
+        int rc;
+        if ((rc = dmalloc(h, (void**)&h->A.off, 36 * N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->A.C, 9 * N * sizeof(double)))) return rc;
+    }
+    if (h->op_kind == 1 && h->mf.J == nullptr) {
+        int rc;
+        if ((rc = dmalloc(h, (void**)&h->mf.J, 9 * N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->mf.fE, 4 * N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->mf.fN, 4 * N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->mf.dE, N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->mf.dF, N * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->mf.xlo, 4 * (size_t)h->g.ny * sizeof(double)))) return rc;
+        if ((rc = dmalloc(h, (void**)&h->mf.ylo, 4 * (size_t)h->g.nx * sizeof(double)))) return rc;
     }
     h->stride = (long long)((n + 31) / 32 * 32);
     if (h->m_alloc < m) {
@@ -389,8 +406,12 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
 static int true_residual(ark_m1* h, const double* x)
 {
     const long long n = 3 * h->N;
-    KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, x, h->tvec, h->st));
-    KL(KC_SPMV, 360.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->tvec, h->V, nullptr, h->A.b, -1.0, nullptr, h->st));
+    if (h->op_kind == 1) {
+        KL(KC_SPMV, 216.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, x, h->V, nullptr, h->A.b, -1.0, nullptr, 0, h->sm_count, h->st));
+    } else {
+        KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, x, h->tvec, h->st));
+        KL(KC_SPMV, 360.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->tvec, h->V, nullptr, h->A.b, -1.0, nullptr, h->st));
+    }
     KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->V, h->V, h->stride, 1, 0, n, h->W, DOT_RNORM, h->sm_count, h->st));
     return 0;
 }
@@ -405,8 +426,14 @@ static int fetch_ctl(ark_m1* h)
 static int assemble_system(ark_m1* h, double dt)
 {
     const Fields f = fields_of(h);
-    KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->st));
-    KL(KC_SCALE, 648.0 * h->N, launch_scale_offdiag(h->g, h->A, h->st));
+    if (h->op_kind == 1) {
+        h->mf.rx = dt / h->g.dx; h->mf.ry = dt / h->g.dy;
+        KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->mf, h->st));
+    } else {
+        MfPlanes none; memset(&none, 0, sizeof none);
+        KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, none, h->st));
+        KL(KC_SCALE, 648.0 * h->N, launch_scale_offdiag(h->g, h->A, h->st));
+    }
     return 0;
 }
 
@@ -434,7 +461,10 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
-            KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
+            if (h->op_kind == 1)
+                KL(KC_SPMV, 264.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
+            else
+                KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
             for (int pass = 0; pass < h->ortho; ++pass) {
                 for (int c0 = 0; c0 <= j; c0 += MAXV) {
                     const int nv = (j + 1 - c0) < MAXV ? (j + 1 - c0) : MAXV;
@@ -483,8 +513,12 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
     double* vin = h->V;                       // slot 0 as staging for the input, slot 1 for the output
     double* vout = h->V + h->stride;
     CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
-    KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, vin, h->tvec, h->st));
-    KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->tvec, vout, nullptr, nullptr, 1.0, nullptr, h->st));
+    if (h->op_kind == 1) {
+        KL(KC_SPMV, 192.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, nullptr, 0, h->sm_count, h->st));
+    } else {
+        KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, vin, h->tvec, h->st));
+        KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->tvec, vout, nullptr, nullptr, 1.0, nullptr, h->st));
+    }
     CU(cudaMemcpyAsync(out, vout, n * sizeof(double), cudaMemcpyDefault, h->st));
     if (b_out) CU(cudaMemcpyAsync(b_out, h->A.b, n * sizeof(double), cudaMemcpyDefault, h->st));
     CU(cudaStreamSynchronize(h->st));

@@ -65,7 +65,23 @@ struct BlockMatrix {      // SoA planes of N doubles each
     double* Minv;         // 9 planes: inverse of the diagonal block
     double* b;            // 3 planes: right-hand side
 };
-cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, cudaStream_t st);
+// Matrix-free operator storage (option "operator" = 1): coefficient planes instead of assembled blocks.
+struct MfPlanes {
+    double* J;     // 9 planes: dP_ab/dU of the cell, rows xx, xy, yy
+    double* fE;    // 4 planes: a+, Lambda, alpha, c dt sigma_f/4 of the EAST face of the cell
+    double* fN;    // 4 planes: the same for the NORTH face
+    double* dE;    // 1 plane : c dt sigma_a eta
+    double* dF;    // 1 plane : c dt sigma_t when the source is cell-centred (Eq. 16), 0 with the WB source
+    double* xlo;   // [4][ny] : west face of column 0 (non-periodic x)
+    double* ylo;   // [4][nx] : south face of row 0 (non-periodic y)
+    double rx, ry; // dt/dx, dt/dy of the assembled step
+};
+// A.off / A.C may be null when mf.J is set (then only Minv, b and the coefficient planes are written)
+cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf, cudaStream_t st);
+// out = sgn * s * (A [M^-1] v) + add, flux form from the coefficient planes; precond = 1 applies M^-1 (Minv) first
+cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
+                         const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
+                         int sm_count, cudaStream_t st);
 cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, cudaStream_t st);
 // t = C x
 cudaError_t launch_diag_mul(const Grid& g, const double* Cblk, const double* x, double* t, cudaStream_t st);

@@ -61,7 +61,7 @@ __device__ __forceinline__ void inv3(const Blk& B, Blk& I)
 }
 
 template <bool SD>
-__global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields f, double dt, BlockMatrix A)
+__global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields f, double dt, BlockMatrix A, MfPlanes mf)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -126,20 +126,35 @@ __global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields 
         }
     }
     Blk Mi; inv3(B[0], Mi);
+    A.b[id] = b[0]; A.b[N + id] = b[1]; A.b[2 * N + id] = b[2];
 #pragma unroll
-    for (int e = 0; e < 9; ++e) { A.C[e * N + id] = B[0].a[e]; A.Minv[e * N + id] = Mi.a[e]; }
+    for (int e = 0; e < 9; ++e) A.Minv[e * N + id] = Mi.a[e];
+    if (mf.J) {
+        // matrix-free storage: the centre cell's Jacobian, its east and north face coefficients, the source weights
+#pragma unroll
+        for (int e = 0; e < 3; ++e) { mf.J[e * N + id] = J[0].xx[e]; mf.J[(3 + e) * N + id] = J[0].xy[e]; mf.J[(6 + e) * N + id] = J[0].yy[e]; }
+        const double qw = wb ? 0.25 * c * dt : 0.0;
+        mf.fE[id] = fe.ap; mf.fE[N + id] = fe.Lam; mf.fE[2 * N + id] = fe.alpha; mf.fE[3 * N + id] = qw * fe.sig;
+        mf.fN[id] = fn.ap; mf.fN[N + id] = fn.Lam; mf.fN[2 * N + id] = fn.alpha; mf.fN[3 * N + id] = qw * fn.sig;
+        mf.dE[id] = c * dt * u[0].sa * eta;
+        mf.dF[id] = wb ? 0.0 : c * dt * u[0].st;
+        if (i == 0) { mf.xlo[j] = fw.ap; mf.xlo[g.ny + j] = fw.Lam; mf.xlo[2 * g.ny + j] = fw.alpha; mf.xlo[3 * g.ny + j] = qw * fw.sig; }
+        if (j == 0) { mf.ylo[i] = fs.ap; mf.ylo[g.nx + i] = fs.Lam; mf.ylo[2 * g.nx + i] = fs.alpha; mf.ylo[3 * g.nx + i] = qw * fs.sig; }
+        return;
+    }
+#pragma unroll
+    for (int e = 0; e < 9; ++e) A.C[e * N + id] = B[0].a[e];
 #pragma unroll
     for (int k = 1; k < 5; ++k)
 #pragma unroll
         for (int e = 0; e < 9; ++e) A.off[((k - 1) * 9 + e) * N + id] = B[k].a[e];
-    A.b[id] = b[0]; A.b[N + id] = b[1]; A.b[2 * N + id] = b[2];
 }
 
-cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, cudaStream_t st)
+cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf, cudaStream_t st)
 {
     dim3 blk(32, 4), grd((g.nx + 31) / 32, (g.ny + 3) / 4);
-    if (s.is_default()) assemble_kernel<true><<<grd, blk, 0, st>>>(g, s, f, dt, A);
-    else assemble_kernel<false><<<grd, blk, 0, st>>>(g, s, f, dt, A);
+    if (s.is_default()) assemble_kernel<true><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf);
+    else assemble_kernel<false><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf);
     return cudaGetLastError();
 }
 

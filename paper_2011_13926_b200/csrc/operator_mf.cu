@@ -1,0 +1,163 @@
+// operator_mf.cu — matrix-free form of the implicit operator (row a6, option "operator" = 1).
+//
+// out = sgn * s * A [M^-1] v + add,  A = I + dt L_n in FLUX form (Eqs. 12-13 with the pressures
+// replaced by J.z, see implicit_kernels.cu) evaluated from coefficient planes written by the assembly kernel:
+//   per cell  : J (9), east-face and north-face coefficients (a+, Lambda, alpha, c dt sigma_f/4) (8), c dt sigma_a eta (1)
+//   = 18 doubles against the 36 of the pre-multiplied block stencil; with M^-1 (9), v (3) and out (3):
+//   264 B per cell per application instead of 336.
+//
+// Organisation = the explicit march kernel's: a block owns a strip of TXO-2 columns (+1 halo column each side) and
+// marches over the rows; a thread keeps z = M^-1 v and Pi = c^2 J z of its cell in rows j and j+1 in registers (the
+// y-face flux needs no other thread; the north flux of row j is the south flux of row j+1); x-faces go through
+// shared memory: publish (z, Pi_xx, Pi_xy), compute the EAST flux, publish it, read the WEST flux from the left thread.
+#include "ark_m1_internal.h"
+
+namespace ark {
+
+static constexpr int TXO = 128;
+
+struct ZP { double zE, zFx, zFy, Pxx, Pxy, Pyy; };   // z and c^2 J z of one cell
+struct FC { double ap, Lam, alpha, sw; };            // face coefficients; sw = c dt sigma_f / 4
+
+// Linear flux through one face (normal component n, tangential t); same algebra as the explicit kernel.
+#define ARK_LIN_FLUX(fc, EL, ER, FnL, FnR, FtL, FtR, PnL, PnR, PtL, PtR, G0, Gn, Gt, S)               \
+    do {                                                                                             \
+        const double dFn_ = (FnR) - (FnL);                                                           \
+        G0 = (fc).alpha * fma((fc).Lam, (ER) - (EL), fma(-(fc).ap, dFn_, (FnR)));                    \
+        Gn = fma((fc).Lam, dFn_, fma((fc).ap, (PnL) - (PnR), (PnR)));                                \
+        Gt = fma((fc).Lam, (FtR) - (FtL), fma((fc).ap, (PtL) - (PtR), (PtR)));                       \
+        S = (fc).sw * ((FnL) + (FnR));                                                               \
+    } while (0)
+
+// z and Pi of the cell in column (xmode, ii) and row j (j may be -1 or ny).  Dirichlet ghosts carry z = 0 (their
+// contribution is in b), outflow ghosts copy the adjacent cell, periodic ghosts wrap (R9).
+template <bool PRECOND>
+__device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const double* __restrict__ v, const double* __restrict__ Minv,
+                                      const double* __restrict__ J, double c2, int xmode, int ii, int j)
+{
+    ZP r; r.zE = 0.0; r.zFx = 0.0; r.zFy = 0.0; r.Pxx = 0.0; r.Pxy = 0.0; r.Pyy = 0.0;
+    if (xmode != 0) return r;
+    int jj = j;
+    if (j < 0 || j >= g.ny) {
+        const int bc = g.bc[(j < 0) ? YLO : YHI];
+        if (bc == BC_DIRICHLET) return r;
+        jj = (bc == BC_PERIODIC) ? ((j < 0) ? g.ny - 1 : 0) : ((j < 0) ? 0 : g.ny - 1);
+    }
+    const long long id = (long long)jj * g.nx + ii;
+    const double v0 = v[id], v1 = v[N + id], v2 = v[2 * N + id];
+    if (PRECOND) {
+        r.zE  = Minv[0 * N + id] * v0 + Minv[1 * N + id] * v1 + Minv[2 * N + id] * v2;
+        r.zFx = Minv[3 * N + id] * v0 + Minv[4 * N + id] * v1 + Minv[5 * N + id] * v2;
+        r.zFy = Minv[6 * N + id] * v0 + Minv[7 * N + id] * v1 + Minv[8 * N + id] * v2;
+    } else { r.zE = v0; r.zFx = v1; r.zFy = v2; }
+    r.Pxx = c2 * (J[0 * N + id] * r.zE + J[1 * N + id] * r.zFx + J[2 * N + id] * r.zFy);
+    r.Pxy = c2 * (J[3 * N + id] * r.zE + J[4 * N + id] * r.zFx + J[5 * N + id] * r.zFy);
+    r.Pyy = c2 * (J[6 * N + id] * r.zE + J[7 * N + id] * r.zFx + J[8 * N + id] * r.zFy);
+    return r;
+}
+
+__device__ __forceinline__ FC load_fc(const double* __restrict__ p, long long stride, long long k)
+{
+    FC f; f.ap = p[k]; f.Lam = p[stride + k]; f.alpha = p[2 * stride + k]; f.sw = p[3 * stride + k];
+    return f;
+}
+
+struct ZPub { double zE, zFx, zFy, Pxx, Pxy; };
+
+template <bool PRECOND>
+__global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const double* __restrict__ v,
+                                                    double* __restrict__ out, const double* __restrict__ scale_ptr,
+                                                    const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
+                                                    int RY, double rx, double ry, double c2)
+{
+    if (skip_flag && *skip_flag) return;
+    __shared__ ZPub pub[TXO + 1];
+    __shared__ double flx[4][TXO];
+    const int t = threadIdx.x;
+    const int i = blockIdx.x * (TXO - 2) - 1 + t;
+    const int j0 = blockIdx.y * RY;
+    const int j1 = min(j0 + RY, g.ny);
+    const long long N = (long long)g.nx * g.ny;
+    const bool upd = (t >= 1 && t <= TXO - 2 && i >= 0 && i < g.nx);
+    // column resolution: 0 = grid column ii, 1 = Dirichlet ghost (z = 0), 2 = inactive
+    int xmode = 0, ii = i;
+    bool use_xlo = false;
+    if (i > g.nx) xmode = 2;
+    else if (i < 0 || i >= g.nx) {
+        const int bc = g.bc[(i < 0) ? XLO : XHI];
+        if (bc == BC_DIRICHLET) { xmode = 1; ii = 0; }
+        else if (bc == BC_PERIODIC) ii = (i < 0) ? g.nx - 1 : 0;
+        else ii = (i < 0) ? 0 : g.nx - 1;
+        use_xlo = (i < 0) && (bc != BC_PERIODIC);
+    }
+    const bool east_valid = (i < g.nx) && (xmode != 2);    // this thread owns the face between columns i and i+1
+    const double sc = sgn * (scale_ptr ? *scale_ptr : 1.0);
+
+    ZP zS = load_zp<PRECOND>(g, N, v, Minv, mf.J, c2, xmode, ii, j0 - 1);
+    ZP zC = load_zp<PRECOND>(g, N, v, Minv, mf.J, c2, xmode, ii, j0);
+    double Hs0 = 0.0, Hs1 = 0.0, Hs2 = 0.0, Ss = 0.0;
+    if (upd) {
+        // south face of row j0: the north face of row j0-1, or the stored low-side line / the wrapped last row
+        FC fs;
+        if (j0 > 0) fs = load_fc(mf.fN, N, (long long)(j0 - 1) * g.nx + i);
+        else if (g.bc[YLO] == BC_PERIODIC) fs = load_fc(mf.fN, N, (long long)(g.ny - 1) * g.nx + i);
+        else fs = load_fc(mf.ylo, g.nx, i);
+        ARK_LIN_FLUX(fs, zS.zE, zC.zE, zS.zFy, zC.zFy, zS.zFx, zC.zFx, zS.Pyy, zC.Pyy, zS.Pxy, zC.Pxy, Hs0, Hs2, Hs1, Ss);
+    }
+
+    for (int j = j0; j < j1; ++j) {
+        const ZP zN = load_zp<PRECOND>(g, N, v, Minv, mf.J, c2, xmode, ii, j + 1);
+        ZPub me; me.zE = zC.zE; me.zFx = zC.zFx; me.zFy = zC.zFy; me.Pxx = zC.Pxx; me.Pxy = zC.Pxy;
+        pub[t] = me;
+        // north face (own column)
+        double Hn0 = 0.0, Hn1 = 0.0, Hn2 = 0.0, Sn = 0.0;
+        const long long id = (long long)j * g.nx + (upd ? i : 0);
+        if (upd) {
+            const FC fn = load_fc(mf.fN, N, id);
+            ARK_LIN_FLUX(fn, zC.zE, zN.zE, zC.zFy, zN.zFy, zC.zFx, zN.zFx, zC.Pyy, zN.Pyy, zC.Pxy, zN.Pxy, Hn0, Hn2, Hn1, Sn);
+        }
+        // east face coefficients of this thread's column
+        FC fe; fe.ap = 0.5; fe.Lam = 0.0; fe.alpha = 1.0; fe.sw = 0.0;
+        if (east_valid) {
+            if (use_xlo || xmode == 1) { if (i < 0) fe = load_fc(mf.xlo, g.ny, j); }
+            else fe = load_fc(mf.fE, N, (long long)j * g.nx + ii);
+        }
+        __syncthreads();
+        double Ge0, Ge1, Ge2, Se;
+        {
+            const ZPub R = pub[t + 1];
+            ARK_LIN_FLUX(fe, me.zE, R.zE, me.zFx, R.zFx, me.zFy, R.zFy, me.Pxx, R.Pxx, me.Pxy, R.Pxy, Ge0, Ge1, Ge2, Se);
+        }
+        flx[0][t] = Ge0; flx[1][t] = Ge1; flx[2][t] = Ge2; flx[3][t] = Se;
+        __syncthreads();
+        if (upd) {
+            const double Gw0 = flx[0][t - 1], Gw1 = flx[1][t - 1], Gw2 = flx[2][t - 1], Sw = flx[3][t - 1];
+            const double dE = mf.dE[id], dF = mf.dF[id];
+            double o0 = zC.zE  + fma(rx, Ge0 - Gw0, fma(ry, Hn0 - Hs0, dE * zC.zE));
+            double o1 = zC.zFx + fma(rx, Ge1 - Gw1, fma(ry, Hn1 - Hs1, fma(dF, zC.zFx, Se + Sw)));
+            double o2 = zC.zFy + fma(rx, Ge2 - Gw2, fma(ry, Hn2 - Hs2, fma(dF, zC.zFy, Sn + Ss)));
+            o0 *= sc; o1 *= sc; o2 *= sc;
+            if (add) { o0 += add[id]; o1 += add[N + id]; o2 += add[2 * N + id]; }
+            out[id] = o0; out[N + id] = o1; out[2 * N + id] = o2;
+        }
+        zC = zN;
+        Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
+    }
+}
+
+cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
+                         const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
+                         int sm_count, cudaStream_t st)
+{
+    const int strips = (g.nx + (TXO - 2) - 1) / (TXO - 2);
+    long long want = ((long long)g.ny * strips + (long long)sm_count * 16 - 1) / ((long long)sm_count * 16);
+    int RY = (int)(want < 4 ? 4 : (want > 64 ? 64 : want));
+    if (RY > g.ny) RY = g.ny;
+    dim3 grd(strips, (g.ny + RY - 1) / RY);
+    const double c2 = g.c * g.c;
+    if (precond) op_mf_kernel<true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2);
+    else op_mf_kernel<false><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2);
+    return cudaGetLastError();
+}
+
+}  // namespace ark

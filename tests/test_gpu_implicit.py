@@ -18,12 +18,16 @@ def _dt(w, k=1.0):
     return k * wl.explicit_dt(w["dx"], w["dy"], w["c"])
 
 
+OPS = [0, 1]   # 0: pre-multiplied block stencil, 1: matrix-free coefficient planes
+
+
+@pytest.mark.parametrize("op", OPS)
 @pytest.mark.parametrize("bc", BCS)
 @pytest.mark.parametrize("wb", [1, 0])
-def test_operator_and_rhs_match_oracle(bc, wb):
+def test_operator_and_rhs_match_oracle(bc, wb, op):
     # A V (assembly kernel + scaled block-stencil + diagonal multiply) vs the oracle's flux-form operator
     w = small_random_state(41, 23, seed=31, dx=0.013, dy=0.021, c=1.3, bc=bc)
-    o, g = make_oracle(w, dict(well_balanced=wb)), make_gpu(w, dict(well_balanced=wb))
+    o, g = make_oracle(w, dict(well_balanced=wb)), make_gpu(w, dict(well_balanced=wb, operator=op))
     dt = _dt(w, 30.0)
     rng = np.random.default_rng(5)
     V = rng.standard_normal((3, w["ny"], w["nx"]))
@@ -35,18 +39,20 @@ def test_operator_and_rhs_match_oracle(bc, wb):
     assert rel_l2(b, want_b) <= 1e-13
 
 
-def test_operator_with_clamped_cells_and_tiny_grids():
-    for (nx, ny, fmax) in [(6, 5, 1.6), (1, 7, 0.9), (7, 1, 0.9), (2, 2, 0.9), (1, 1, 0.5)]:
+@pytest.mark.parametrize("op", OPS)
+def test_operator_with_clamped_cells_and_tiny_grids(op):
+    for (nx, ny, fmax) in [(6, 5, 1.6), (1, 7, 0.9), (7, 1, 0.9), (2, 2, 0.9), (1, 1, 0.5), (300, 3, 0.9), (127, 70, 0.9)]:
         w = small_random_state(nx, ny, seed=22 + nx, fmax=fmax)
-        o, g = make_oracle(w), make_gpu(w)
+        o, g = make_oracle(w), make_gpu(w, dict(operator=op))
         V = np.random.default_rng(1).standard_normal((3, ny, nx))
         assert rel_l2(g.apply_operator(0.3, V), o.apply_linear(0.3, V)) <= 1e-13
 
 
+@pytest.mark.parametrize("op", OPS)
 @pytest.mark.parametrize("bc", BCS)
-def test_implicit_step_small_all_boundaries(bc):
+def test_implicit_step_small_all_boundaries(bc, op):
     w = small_random_state(37, 29, seed=41, bc=bc, sig_range=(-1.0, 2.0))
-    o, g = make_oracle(w), make_gpu(w)
+    o, g = make_oracle(w), make_gpu(w, dict(operator=op))
     dt = _dt(w, 50.0)
     io, ro = o.step_implicit(dt, 1e-10, 30, 4000)
     ig, rg = g.step_implicit(dt, 1e-10, 30, 4000)
@@ -101,10 +107,11 @@ def test_steady_state_returns_zero_iterations():
     assert its == 0 and res <= 1e-10
 
 
-def test_config1_gaussian_diffusion_20_steps():
+@pytest.mark.parametrize("op", OPS)
+def test_config1_gaussian_diffusion_20_steps(op):
     # BASELINE.json configs[0]: 64^2, sigma_s = 1e3, 20 implicit steps at 10x the explicit dt
     w = wl.gaussian_diffusion(64)
-    o, g = make_oracle(w), make_gpu(w)
+    o, g = make_oracle(w), make_gpu(w, dict(operator=op))
     dt = _dt(w, 10.0)
     for _ in range(20):
         io, ro = o.step_implicit(dt, 1e-10, 30, 4000)
@@ -155,11 +162,12 @@ def test_config2_opacity_jump_implicit_steady_and_restoring():
     assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_IMPLICIT
 
 
+@pytest.mark.parametrize("op", OPS)
 @pytest.mark.parametrize("k", [50.0, 100.0])
-def test_config3_random_medium_256_window(k):
+def test_config3_random_medium_256_window(k, op):
     # the config-3 generator on a 256^2 grid (the oracle finishes in seconds), dt = 50x and 100x
     w = wl.random_medium(256, seed=1234)
-    o, g = make_oracle(w), make_gpu(w)
+    o, g = make_oracle(w), make_gpu(w, dict(operator=op))
     dt = _dt(w, k)
     io, ro = o.step_implicit(dt, 1e-10, 30, 4000)
     ig, rg = g.step_implicit(dt, 1e-10, 30, 4000)

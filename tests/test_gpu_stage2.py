@@ -36,10 +36,11 @@ def test_explicit_step_with_temperature(bc):
     assert state_rel_l2(g.get_state(with_T=True), o.get_state(with_T=True)) <= 1e-11
 
 
+@pytest.mark.parametrize("op", [0, 1])
 @pytest.mark.parametrize("bc", [(0, 0, 0, 0), (1, 1, 0, 0), (2, 2, 1, 1)])
-def test_implicit_step_with_temperature(bc):
+def test_implicit_step_with_temperature(bc, op):
     w = _coupled_state(37, 29, seed=5, bc=bc)
-    o, g = make_oracle(w, dict(a_r=0.7)), make_gpu(w, dict(a_r=0.7))
+    o, g = make_oracle(w, dict(a_r=0.7)), make_gpu(w, dict(a_r=0.7, operator=op))
     dt = _dt(w, 40.0)
     for _ in range(2):
         io, ro = o.step_implicit(dt, 1e-10, 30, 4000)
