@@ -169,17 +169,20 @@ def aggregate_over_ranks(elapsed_s, units, dist=None):
     return float(t.item()), float(u.item())
 
 
-def iteration_bytes_per_cell(iters, m=RESTART):
+def iteration_bytes_per_cell(iters, m=RESTART, operator=0):
     """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
-    operator 336; one-pass classical Gram-Schmidt at inner index j: dots 24 (j+2), update+norm 24 (j+3); one extra read of
-    w per 16-vector pass; per cycle: combine 8 (3 jj + 15) + diag_mul 120 + residual spmv 360 + norm 24."""
+    operator 336 (block stencil) or 264 (matrix-free); one-pass classical Gram-Schmidt at inner index j: dots 24 (j+2),
+    update+norm 24 (j+3); one extra read of w per 16-vector pass; per cycle: combine 8 (3 jj + 15) + true residual
+    (block stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24."""
+    op = 336.0 if operator == 0 else 264.0
+    res = 480.0 if operator == 0 else 216.0
     total, done = 0.0, 0
     while done < iters:
         jj = min(m, iters - done)
         for j in range(jj):
             passes = j // 16 + 1
-            total += 336.0 + 24.0 * (j + 1 + passes) + 24.0 * (j + 1 + 2 * passes)
-        total += 8.0 * (3 * jj + 15) + 120.0 + 360.0 + 24.0
+            total += op + 24.0 * (j + 1 + passes) + 24.0 * (j + 1 + 2 * passes)
+        total += 8.0 * (3 * jj + 15) + res + 24.0
         done += jj
     return total
 
@@ -210,6 +213,7 @@ def run_ours(args):
     out_F = torch.empty((2, n, n), dtype=torch.float64).pin_memory()
     stream = torch.cuda.current_stream()
     g = ark.ArkM1(n, n, w["dx"], w["dy"], w["c"], bc=w["bc"], stream=stream)
+    g.set_option("operator", args.operator)
 
     def reset_device():
         g.set_state(devt["E"], devt["F"], devt["sigma_a"], devt["sigma_s"])
@@ -292,7 +296,7 @@ def run_ours(args):
             ms = e0.elapsed_time(e1)
             tm = g.timings()
             nE, nf = g.count_unrealizable()
-            bpc = iteration_bytes_per_cell(its)
+            bpc = iteration_bytes_per_cell(its, operator=args.operator)
             kry_gbs = bpc * N / (tm["krylov_ms"] * 1e-3) / 1e9 if its > 0 else None
             imp[f"{ratio:g}x"] = {"iterations": its, "final_residual": res, "ms": ms, "assembly_ms": tm["assembly_ms"], "krylov_ms": tm["krylov_ms"],
                                   "ms_per_iteration": tm["krylov_ms"] / max(its, 1), "cell_updates_per_s": N / (ms * 1e-3),
@@ -338,7 +342,8 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"M1 random medium (BASELINE.json configs[3]) {n}x{n}, fp64, periodic, c=1, seed {args.seed}(+rank)",
                        "step": "state reset (D2D) + 1 explicit step (CFL 0.4) + 1 implicit step (dt = 10x explicit, GMRES(30) + block-Jacobi, tol 1e-10)",
-                       "iterations_per_implicit_step": its_main, "parallelism": "replicas only (one independent problem per GPU)" if world > 1 else "1 GPU",
+                       "iterations_per_implicit_step": its_main,
+                       "operator": "matrix-free coefficient planes" if args.operator == 1 else "pre-multiplied block stencil (BSR 3x3)", "parallelism": "replicas only (one independent problem per GPU)" if world > 1 else "1 GPU",
                        "l2": f"inputs larger than L2 (state+opacity {5 * N * 8 / 1e6:.0f} MB, Krylov basis {31 * 3 * N * 8 / 1e9:.1f} GB vs 126 MB L2)",
                        "device_bytes": g.device_bytes()},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
@@ -359,6 +364,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=4096, help="grid size (BASELINE.json configs[3]: 4096)")
     ap.add_argument("--seed", type=int, default=1234)
+    ap.add_argument("--operator", type=int, default=1, choices=[0, 1],
+                    help="implicit operator: 0 = pre-multiplied block stencil, 1 = matrix-free coefficient planes (default, DESIGN.md)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the dt = 50/100/200x implicit solves")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-n", type=int, default=2048, help="grid size of the oracle's bounded sample (cpu_baseline)")

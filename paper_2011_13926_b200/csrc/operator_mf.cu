@@ -106,22 +106,24 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
     }
 
     for (int j = j0; j < j1; ++j) {
+        // issue every global load of this row first (north cell, face coefficients, source weights); they are consumed
+        // after the two barriers of the x-face exchange, which needs only data already in registers
         const ZP zN = load_zp<PRECOND>(g, N, v, Minv, mf.J, c2, xmode, ii, j + 1);
-        ZPub me; me.zE = zC.zE; me.zFx = zC.zFx; me.zFy = zC.zFy; me.Pxx = zC.Pxx; me.Pxy = zC.Pxy;
-        pub[t] = me;
-        // north face (own column)
-        double Hn0 = 0.0, Hn1 = 0.0, Hn2 = 0.0, Sn = 0.0;
         const long long id = (long long)j * g.nx + (upd ? i : 0);
+        FC fn; fn.ap = 0.5; fn.Lam = 0.0; fn.alpha = 1.0; fn.sw = 0.0;
+        double dE = 0.0, dF = 0.0, a0 = 0.0, a1 = 0.0, a2 = 0.0;
         if (upd) {
-            const FC fn = load_fc(mf.fN, N, id);
-            ARK_LIN_FLUX(fn, zC.zE, zN.zE, zC.zFy, zN.zFy, zC.zFx, zN.zFx, zC.Pyy, zN.Pyy, zC.Pxy, zN.Pxy, Hn0, Hn2, Hn1, Sn);
+            fn = load_fc(mf.fN, N, id);
+            dE = mf.dE[id]; dF = mf.dF[id];
+            if (add) { a0 = add[id]; a1 = add[N + id]; a2 = add[2 * N + id]; }
         }
-        // east face coefficients of this thread's column
         FC fe; fe.ap = 0.5; fe.Lam = 0.0; fe.alpha = 1.0; fe.sw = 0.0;
         if (east_valid) {
             if (use_xlo || xmode == 1) { if (i < 0) fe = load_fc(mf.xlo, g.ny, j); }
             else fe = load_fc(mf.fE, N, (long long)j * g.nx + ii);
         }
+        ZPub me; me.zE = zC.zE; me.zFx = zC.zFx; me.zFy = zC.zFy; me.Pxx = zC.Pxx; me.Pxy = zC.Pxy;
+        pub[t] = me;
         __syncthreads();
         double Ge0, Ge1, Ge2, Se;
         {
@@ -130,15 +132,16 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
         }
         flx[0][t] = Ge0; flx[1][t] = Ge1; flx[2][t] = Ge2; flx[3][t] = Se;
         __syncthreads();
+        const int tw = (t > 0) ? t - 1 : 0;
+        const double Gw0 = flx[0][tw], Gw1 = flx[1][tw], Gw2 = flx[2][tw], Sw = flx[3][tw];
+        // north face (own column)
+        double Hn0, Hn1, Hn2, Sn;
+        ARK_LIN_FLUX(fn, zC.zE, zN.zE, zC.zFy, zN.zFy, zC.zFx, zN.zFx, zC.Pyy, zN.Pyy, zC.Pxy, zN.Pxy, Hn0, Hn2, Hn1, Sn);
         if (upd) {
-            const double Gw0 = flx[0][t - 1], Gw1 = flx[1][t - 1], Gw2 = flx[2][t - 1], Sw = flx[3][t - 1];
-            const double dE = mf.dE[id], dF = mf.dF[id];
             double o0 = zC.zE  + fma(rx, Ge0 - Gw0, fma(ry, Hn0 - Hs0, dE * zC.zE));
             double o1 = zC.zFx + fma(rx, Ge1 - Gw1, fma(ry, Hn1 - Hs1, fma(dF, zC.zFx, Se + Sw)));
             double o2 = zC.zFy + fma(rx, Ge2 - Gw2, fma(ry, Hn2 - Hs2, fma(dF, zC.zFy, Sn + Ss)));
-            o0 *= sc; o1 *= sc; o2 *= sc;
-            if (add) { o0 += add[id]; o1 += add[N + id]; o2 += add[2 * N + id]; }
-            out[id] = o0; out[N + id] = o1; out[2 * N + id] = o2;
+            out[id] = fma(sc, o0, a0); out[N + id] = fma(sc, o1, a1); out[2 * N + id] = fma(sc, o2, a2);
         }
         zC = zN;
         Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
