@@ -172,7 +172,7 @@ def aggregate_over_ranks(elapsed_s, units, dist=None):
 def iteration_bytes_per_cell(iters, m=RESTART, operator=0):
     """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
     operator 336 (block stencil) or 264 (matrix-free); one-pass classical Gram-Schmidt at inner index j: dots 24 (j+2),
-    update+norm 24 (j+3); one extra read of w per 16-vector pass; per cycle: combine 8 (3 jj + 15) + true residual
+    update+norm 24 (j+3); one extra read of w per 16-vector pass (option vectors_per_pass, default 16 by measurement); per cycle: combine 8 (3 jj + 15) + true residual
     (block stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24."""
     op = 336.0 if operator == 0 else 264.0
     res = 480.0 if operator == 0 else 216.0

@@ -34,7 +34,7 @@ struct ark_m1 {
     double *rho_cv, *ux, *uy, *source_E;
     unsigned long long* counts;   // 2
     // options
-    int ortho, explicit_kernel, op_kind;
+    int ortho, explicit_kernel, op_kind, maxv, basis_pad;
     // implicit workspace (lazy)
     BlockMatrix A;
     MfPlanes mf;       // matrix-free coefficient planes (op_kind == 1)
@@ -129,7 +129,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0;
-    h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1;
+    h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     h->hist_host = new std::vector<double>();
@@ -236,6 +236,8 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
     else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1 or 2%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 32]%s", ""); h->maxv = iv; }
+    else if (!strcmp(key, "basis_pad")) { if (iv < 0 || (iv & 31)) return fail(h, ARK_M1_E_ARG, "basis_pad must be a non-negative multiple of 32 doubles%s", ""); if (iv != h->basis_pad) { cudaStreamSynchronize(h->st); free_implicit(h); } h->basis_pad = iv; }
     else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
     else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
@@ -375,7 +377,7 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
         if ((rc = dmalloc(h, (void**)&h->mf.xlo, 4 * (size_t)h->g.ny * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->mf.ylo, 4 * (size_t)h->g.nx * sizeof(double)))) return rc;
     }
-    h->stride = (long long)((n + 31) / 32 * 32);
+    h->stride = (long long)((n + 31) / 32 * 32) + h->basis_pad;
     if (h->m_alloc < m) {
         if (h->V) { cudaFree(h->V); h->bytes -= (long long)((size_t)(h->m_alloc + 1) * h->stride * sizeof(double)); h->V = nullptr; }
         int rc = dmalloc(h, (void**)&h->V, (size_t)(m + 1) * h->stride * sizeof(double));
@@ -450,6 +452,7 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
     double* x = h->U[h->cur];          // initial guess U^n, solution in place
     GmresWork W = h->W;
     const int* stop = &W.ctl->inner_stop;
+    const int MV = h->maxv;            // basis vectors per pass of the multi-vector kernels
 
     CU(cudaEventRecord(h->ev[0], h->st));
     if ((rc = assemble_system(h, dt))) return rc;
@@ -466,13 +469,13 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
             else
                 KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
             for (int pass = 0; pass < h->ortho; ++pass) {
-                for (int c0 = 0; c0 <= j; c0 += MAXV) {
-                    const int nv = (j + 1 - c0) < MAXV ? (j + 1 - c0) : MAXV;
+                for (int c0 = 0; c0 <= j; c0 += MV) {
+                    const int nv = (j + 1 - c0) < MV ? (j + 1 - c0) : MV;
                     KL(KC_DOT, 24.0 * (nv + 1) * h->N, launch_multi_dot(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, pass == 0 ? DOT_H : DOT_H2, sm, h->st));
                 }
-                for (int c0 = 0; c0 <= j; c0 += MAXV) {
-                    const int nv = (j + 1 - c0) < MAXV ? (j + 1 - c0) : MAXV;
-                    const int last = (c0 + MAXV > j) && (pass == h->ortho - 1);
+                for (int c0 = 0; c0 <= j; c0 += MV) {
+                    const int nv = (j + 1 - c0) < MV ? (j + 1 - c0) : MV;
+                    const int last = (c0 + MV > j) && (pass == h->ortho - 1);
                     KL(KC_UPDATE, 24.0 * (nv + 2) * h->N, launch_update(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, last, sm, h->st));
                 }
             }

@@ -39,7 +39,7 @@ struct GmresWork {                 // device pointers into one small allocation
     int caphist;
 };
 
-enum { MAXV = 16 };                // basis vectors handled per pass of the multi-vector kernels
+enum { MAXV = 32 };                // basis vectors handled per pass of the multi-vector kernels
 
 enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5 };
 

@@ -202,6 +202,8 @@ cudaError_t launch_multi_dot(const double* w, const double* V0, long long stride
 #define ARK_CASE(K) case K: dot_launch<K>(grd, w, V0, stride, n, W, mode, col0, st); break;
         ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
         ARK_CASE(9) ARK_CASE(10) ARK_CASE(11) ARK_CASE(12) ARK_CASE(13) ARK_CASE(14) ARK_CASE(15) ARK_CASE(16)
+        ARK_CASE(17) ARK_CASE(18) ARK_CASE(19) ARK_CASE(20) ARK_CASE(21) ARK_CASE(22) ARK_CASE(23) ARK_CASE(24)
+        ARK_CASE(25) ARK_CASE(26) ARK_CASE(27) ARK_CASE(28) ARK_CASE(29) ARK_CASE(30) ARK_CASE(31) ARK_CASE(32)
 #undef ARK_CASE
         default: return cudaErrorInvalidValue;
     }
@@ -224,6 +226,8 @@ cudaError_t launch_update(double* w, const double* V0, long long stride, int nv,
 #define ARK_CASE(K) case K: upd_launch<K>(grd, w, V0, stride, n, W, col0, with_norm, st); break;
         ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
         ARK_CASE(9) ARK_CASE(10) ARK_CASE(11) ARK_CASE(12) ARK_CASE(13) ARK_CASE(14) ARK_CASE(15) ARK_CASE(16)
+        ARK_CASE(17) ARK_CASE(18) ARK_CASE(19) ARK_CASE(20) ARK_CASE(21) ARK_CASE(22) ARK_CASE(23) ARK_CASE(24)
+        ARK_CASE(25) ARK_CASE(26) ARK_CASE(27) ARK_CASE(28) ARK_CASE(29) ARK_CASE(30) ARK_CASE(31) ARK_CASE(32)
 #undef ARK_CASE
         default: return cudaErrorInvalidValue;
     }

@@ -45,5 +45,6 @@ def test_iteration_byte_formula():
     sys.path.insert(0, ROOT)
     import bench
     # one iteration at j = 0: operator 336 + dots 24 (1 + 1) + update 24 (1 + 2); one cycle end: combine 8 (3 + 15) + 120 + 360 + 24
-    assert bench.iteration_bytes_per_cell(1) == 336 + 48 + 72 + 8 * 18 + 120 + 360 + 24
+    assert bench.iteration_bytes_per_cell(1, operator=0) == 336 + 48 + 72 + 8 * 18 + 120 + 360 + 24
+    assert bench.iteration_bytes_per_cell(1, operator=1) == 264 + 48 + 72 + 8 * 18 + 216 + 24
     assert bench.iteration_bytes_per_cell(60) == 2 * bench.iteration_bytes_per_cell(30)

@@ -77,7 +77,7 @@ def test_gmres_solution_matches_dense_direct_solve():
 @pytest.mark.parametrize("ortho", [1, 2])
 @pytest.mark.parametrize("restart", [5, 17, 30, 40])
 def test_restart_lengths_and_orthogonalisation(restart, ortho):
-    # restart > 16 exercises the two-pass multi-vector kernels
+    # restart > 16 (vectors_per_pass) exercises the two-pass multi-vector kernels
     w = small_random_state(50, 34, seed=43)
     o, g = make_oracle(w), make_gpu(w, dict(orthogonalisation=ortho))
     dt = _dt(w, 40.0)
