@@ -354,8 +354,9 @@ def run_ours(args):
                           "alg_bytes_per_launch": v["bytes"] / v["launches"]}
         dom = max((k for k in kern if k != "small"), key=lambda k: kern[k]["ms_total"])
         tr = traffic.get(dom, {}) if (n == 4096) else {}
+        tr_bytes = tr["ratio"] * kern[dom]["alg_bytes_per_launch"] if "ratio" in tr else None
         line_extra["roofline"] = {"kernel": dom, "bound": "hbm", "achieved": kern[dom]["achieved_gbs"], "peak": peak_gbs, "unit": "GB/s",
-                                  "frac": kern[dom]["hbm_frac"], "traffic": tr.get("dram_bytes_per_launch"), "peak_source": peak_src,
+                                  "frac": kern[dom]["hbm_frac"], "traffic": tr_bytes, "peak_source": peak_src,
                                   "share_of_step": kern[dom]["share"], "alg_bytes_per_launch": kern[dom]["alg_bytes_per_launch"],
                                   "traffic_note": tr.get("note")}
         line_extra["kernels"] = kern
