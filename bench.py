@@ -338,6 +338,34 @@ def run_ours(args):
                                                           "per_ratio": sm_out, "closest": best_k, "closest_T_implicit_over_K_T_explicit": sm_out[best_k]["over_K"],
                                                           "reached": bool(any(v["implicit_wins"] for v in sm_out.values()))}
             del devs
+        # ---- stage 2 (row a8, BASELINE.json configs[4]): matter coupling + point source + velocity sources at 2048^2 ----------
+        if not args.no_sweep and not args.no_stage2:
+            w5 = wl.stratified_coupled(2048, seed=4321)
+            N5 = w5["nx"] * w5["ny"]
+            dt5 = 100.0 * wl.explicit_dt(w5["dx"], w5["dy"], w5["c"])
+            g5 = ark.ArkM1(w5["nx"], w5["ny"], w5["dx"], w5["dy"], w5["c"], bc=w5["bc"], stream=stream)
+            g5.set_option("operator", args.operator)
+            d5 = {k: torch.from_numpy(np.ascontiguousarray(w5[k])).to(dev) for k in ("E", "F", "sigma_a", "sigma_s", "T", "rho_cv", "ux", "uy", "source_E")}
+            for name in ("rho_cv", "ux", "uy", "source_E"):
+                g5.set_field(name, d5[name])
+            g5.set_state(d5["E"], d5["F"], d5["sigma_a"], d5["sigma_s"], d5["T"])
+            g5.step_implicit(dt5, TOL, RESTART, 30)          # warm-up (allocations), then the timed step from the same state
+            g5.set_state(d5["E"], d5["F"], d5["sigma_a"], d5["sigma_s"], d5["T"])
+            torch.cuda.synchronize()
+            e0.record(stream)
+            its5, res5 = g5.step_implicit(dt5, TOL, RESTART, MAXIT)
+            g5.add_velocity_sources(dt5)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms5 = e0.elapsed_time(e1)
+            tm5 = g5.timings()
+            bpc5 = iteration_bytes_per_cell(its5, operator=args.operator)
+            line_extra["stage2"] = {"workload": "BASELINE.json configs[4]: 2048x2048 grey radiation-matter coupling, implicit step at 100x explicit dt + velocity sources",
+                                    "iterations": its5, "final_residual": res5, "ms": ms5, "cell_updates_per_s": N5 / (ms5 * 1e-3),
+                                    "ms_per_iteration": tm5["krylov_ms"] / max(its5, 1),
+                                    "krylov_hbm_frac": (bpc5 * N5 / (tm5["krylov_ms"] * 1e-3) / 1e9 / peak_gbs) if its5 > 0 else None}
+            g5.close()
+            del d5
         # ---- roofline of the dominant kernel class ---------------------------------------------------------------
         traffic = {}
         tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
@@ -399,6 +427,7 @@ def main():
                     help="implicit operator: 0 = pre-multiplied block stencil, 1 = matrix-free coefficient planes (default, DESIGN.md)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the dt = 50/100/200x implicit solves")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stage2", action="store_true", help="skip the config-5 (2048^2, matter coupling) implicit step")
     ap.add_argument("--cpu-n", type=int, default=2048, help="grid size of the oracle's bounded sample (cpu_baseline)")
     ap.add_argument("--ref-n", type=int, default=1024, help="grid size of the oracle's bounded sample per step (--impl reference)")
     args = ap.parse_args()
