@@ -378,7 +378,7 @@ static void add_block(double *dst, const double *src) { for (int k = 0; k < 9; +
 /* The matrix "update" of PAPER.md:315-321: the graph is fixed, the values follow the entries listed in
  * DESIGN.md ("Implicit system"), obtained by collecting the coefficients of U_i, U_{i+-1}, U_{j+-1} in
  * apply_cell.  b = U^n + affine terms. */
-static void assemble_cell(const oracle_m1 *h, double dt, int i, int j, double A[5][9], long col[5], double b[3])
+static void assemble_cell(const oracle_m1 *h, double dt, const double *base, int i, int j, double A[5][9], long col[5], double b[3])
 {
     cell_t u[5]; closure_t q[5];
     const int di[5] = { 0, -1, 1, 0, 0 }, dj[5] = { 0, 0, 0, -1, 1 };
@@ -420,8 +420,11 @@ static void assemble_cell(const oracle_m1 *h, double dt, int i, int j, double A[
     M(Nb, 1, 1) += ry * fn.Lam;             M(Nb, 2, 2) += ry * fn.Lam + sn;
     M(S, 1, 1) += ry * fs.Lam;              M(S, 2, 2) += ry * fs.Lam + ss;
     #undef M
-    /* right-hand side: U^n, emission and sources */
-    b[0] = u[0].E; b[1] = u[0].Fx; b[2] = u[0].Fy;
+    /* right-hand side: U^n, emission and sources.  base == NULL: U^n is the stored state (one linearised step);
+     * otherwise the stored state is a Newton iterate U^k that only supplies the coefficients and base = [E|Fx|Fy]
+     * holds U^n (oracle_m1_step_implicit_newton below). */
+    if (base) { const long N_ = (long)h->nx * h->ny; b[0] = base[u[0].idx]; b[1] = base[N_ + u[0].idx]; b[2] = base[2 * N_ + u[0].idx]; }
+    else { b[0] = u[0].E; b[1] = u[0].Fx; b[2] = u[0].Fy; }
     if (h->has_T) { const double T = h->T[u[0].idx]; b[0] += c * dt * u[0].sa * eta * h->a_r * T * T * T * T; }
     if (h->source_E) b[0] += dt * h->source_E[u[0].idx];
     /* boundaries (R9) */
@@ -439,7 +442,7 @@ static void assemble_cell(const oracle_m1 *h, double dt, int i, int j, double A[
     }
 }
 
-static int system_build(const oracle_m1 *h, double dt, system_t *s)
+static int system_build(const oracle_m1 *h, double dt, const double *base, system_t *s)
 {
     const long N = (long)h->nx * h->ny;
     s->N = N;
@@ -452,7 +455,7 @@ static int system_build(const oracle_m1 *h, double dt, system_t *s)
         for (int i = 0; i < h->nx; ++i) {
             const long id = (long)j * h->nx + i;
             double b[3];
-            assemble_cell(h, dt, i, j, (double (*)[9])(s->A + 45 * id), s->col + 5 * id, b);
+            assemble_cell(h, dt, base, i, j, (double (*)[9])(s->A + 45 * id), s->col + 5 * id, b);
             s->b[id] = b[0]; s->b[N + id] = b[1]; s->b[2 * N + id] = b[2];
         }
     return 0;
@@ -462,7 +465,7 @@ static void system_free(system_t *s) { free(s->A); free(s->col); free(s->b); }
 /* Test hook: the assembled blocks A[N][5][3][3] (centre, west, east, south, north), their column cells and b. */
 ORACLE_API int oracle_m1_assemble(oracle_m1 *h, double dt, double *A, long *col, double *b)
 {
-    system_t s; const int rc = system_build(h, dt, &s); if (rc) return rc;
+    system_t s; const int rc = system_build(h, dt, NULL, &s); if (rc) return rc;
     memcpy(A, s.A, sizeof(double) * 45 * s.N); memcpy(col, s.col, sizeof(long) * 5 * s.N);
     memcpy(b, s.b, sizeof(double) * 3 * s.N);
     system_free(&s); return 0;
@@ -604,7 +607,7 @@ static int gmres(oracle_m1 *h, const system_t *s, double *x, double tol, int m, 
 ORACLE_API int oracle_m1_step_implicit(oracle_m1 *h, double dt, double tol, int restart, int maxit, double *final_residual)
 {
     if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) { snprintf(h->err, sizeof h->err, "bad argument"); return -1; }
-    system_t s; const int rc = system_build(h, dt, &s); if (rc) return rc;
+    system_t s; const int rc = system_build(h, dt, NULL, &s); if (rc) return rc;
     const long N = s.N;
     double *x = (double *)malloc(sizeof(double) * 3 * N);
     memcpy(x, h->E, sizeof(double) * N); memcpy(x + N, h->Fx, sizeof(double) * N); memcpy(x + 2 * N, h->Fy, sizeof(double) * N);
@@ -624,6 +627,55 @@ ORACLE_API int oracle_m1_step_implicit(oracle_m1 *h, double dt, double tol, int 
     }
     free(x); system_free(&s);
     return its;
+}
+
+/* Newton-Raphson on the implicit step ("the system is non-linear ... we use a Newton-Raphson method ... a
+ * linear system has to be solved at each iteration").  With the Jacobian of DESIGN.md reading R4 (analytic pressure
+ * Jacobian, derivatives of a+-, Lambda, alpha dropped) and P homogeneous of degree 1, the Newton update
+ *   J_k (U^{k+1} - U^k) = -(U^k - U^n + dt R(U^k)),  J_k = I + dt L_{U^k},  L_{U^k} U^k = R(U^k)
+ * is the same as   (I + dt L_{U^k}) U^{k+1} = U^n + affine terms:
+ * re-assemble with the coefficients of the iterate, keep U^n on the right-hand side, start GMRES from U^k.
+ * The first iteration is exactly oracle_m1_step_implicit.  Stops when ||U^{k+1} - U^k||_2 <= newton_tol ||U^{k+1}||_2
+ * or after max_newton iterations.  The temperature is linearised about T^n throughout and updated once at the end.
+ * Returns the total number of GMRES iterations. */
+ORACLE_API int oracle_m1_step_implicit_newton(oracle_m1 *h, double dt, double tol, int restart, int maxit, double newton_tol,
+                                              int max_newton, int *newton_iterations, double *final_residual, double *final_update)
+{
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0 || !(newton_tol >= 0.0) || max_newton < 1) { snprintf(h->err, sizeof h->err, "bad argument"); return -1; }
+    const long N = (long)h->nx * h->ny;
+    double *base = (double *)malloc(sizeof(double) * 3 * N), *x = (double *)malloc(sizeof(double) * 3 * N);
+    if (!base || !x) return -3;
+    memcpy(base, h->E, sizeof(double) * N); memcpy(base + N, h->Fx, sizeof(double) * N); memcpy(base + 2 * N, h->Fy, sizeof(double) * N);
+    int total = 0, k = 0; double rel = 0.0, upd = 0.0;
+    for (k = 0; k < max_newton; ++k) {
+        system_t s; const int rc = system_build(h, dt, base, &s); if (rc) { free(base); free(x); return rc; }
+        memcpy(x, h->E, sizeof(double) * N); memcpy(x + N, h->Fx, sizeof(double) * N); memcpy(x + 2 * N, h->Fy, sizeof(double) * N);
+        const int its = gmres(h, &s, x, tol, restart, maxit, &rel);
+        system_free(&s);
+        if (its < 0) { free(base); free(x); return its; }
+        total += its;
+        double d2 = 0.0, n2 = 0.0;
+        for (long id = 0; id < N; ++id) {
+            const double dE = x[id] - h->E[id], dFx = x[N + id] - h->Fx[id], dFy = x[2 * N + id] - h->Fy[id];
+            d2 += dE * dE + dFx * dFx + dFy * dFy;
+            n2 += x[id] * x[id] + x[N + id] * x[N + id] + x[2 * N + id] * x[2 * N + id];
+        }
+        memcpy(h->E, x, sizeof(double) * N); memcpy(h->Fx, x + N, sizeof(double) * N); memcpy(h->Fy, x + 2 * N, sizeof(double) * N);
+        upd = (n2 > 0.0) ? sqrt(d2 / n2) : sqrt(d2);
+        if (upd <= newton_tol) { ++k; break; }
+    }
+    if (h->has_T) {
+        for (long id = 0; id < N; ++id) {
+            const double T = h->T[id], rcv = h->rho_cv ? h->rho_cv[id] : 1.0;
+            const double Theta = h->a_r * T * T * T * T;
+            h->T[id] = T + h->c * h->sa[id] * dt * (h->E[id] - Theta) / (rcv + 4.0 * h->a_r * h->c * h->sa[id] * dt * T * T * T);
+        }
+    }
+    if (newton_iterations) *newton_iterations = k;
+    if (final_residual) *final_residual = rel;
+    if (final_update) *final_update = upd;
+    free(base); free(x);
+    return total;
 }
 
 /* Step 3 of the operator splitting: explicit addition of the velocity-dependent sources of

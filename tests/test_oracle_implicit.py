@@ -190,3 +190,35 @@ def test_matter_coupling_0d_energy_and_closed_form():
         gap.append(abs(a_r * T[0, 0] ** 4 - E[0, 0]))
         assert E[0, 0] + rcv * T[0, 0] == pytest.approx(E0 + rcv * T0, rel=1e-13)
     assert all(g1 < 0.2 * g0 for g0, g1 in zip(gap, gap[1:])) and gap[-1] < 1e-6
+
+
+def test_newton_iteration_converges_to_the_nonlinear_backward_euler_solution():
+    # Newton-Raphson on the non-linear implicit system.  Pin: the converged iterate satisfies
+    # U - U^n + dt R(U) = 0 with R the (separately pinned) non-linear residual; one linearised step does not.
+    w = small_random_state(24, 20, seed=3, sig_range=(-1.0, 1.5))
+    U0 = np.concatenate((w["E"][None], w["F"]))
+    for K in (2.0, 50.0):
+        dt = K * wl.explicit_dt(w["dx"], w["dy"])
+        o = make_oracle(w)
+        its, nn, res, upd = o.step_implicit_newton(dt, 1e-12, 30, 4000, 1e-11, 40)
+        assert 2 <= nn < 40 and upd <= 1e-11 and res <= 1e-12
+        E, F = o.get_state()
+        RE, RF = o.residual()
+        U, R = np.concatenate((E[None], F)), np.concatenate((RE[None], RF))
+        assert np.linalg.norm(U - U0 + dt * R) <= 1e-10 * np.linalg.norm(U)
+        o1 = make_oracle(w)
+        o1.step_implicit(dt, 1e-12, 30, 4000)
+        E1, F1 = o1.get_state()
+        R1E, R1F = o1.residual()
+        U1, R1 = np.concatenate((E1[None], F1)), np.concatenate((R1E[None], R1F))
+        assert np.linalg.norm(U1 - U0 + dt * R1) > 1e-3 * np.linalg.norm(U1)
+
+
+def test_newton_first_iteration_is_the_linearised_step():
+    w = small_random_state(14, 11, seed=4, bc=(1, 2, 0, 0))
+    dt = 20.0 * wl.explicit_dt(w["dx"], w["dy"])
+    o1, o2 = make_oracle(w), make_oracle(w)
+    i1, r1 = o1.step_implicit(dt, 1e-11, 30, 4000)
+    i2, nn, r2, upd = o2.step_implicit_newton(dt, 1e-11, 30, 4000, 0.0, 1)
+    assert nn == 1 and i1 == i2
+    assert all(np.array_equal(a, b) for a, b in zip(o1.get_state(), o2.get_state()))
