@@ -221,4 +221,5 @@ def test_newton_first_iteration_is_the_linearised_step():
     i1, r1 = o1.step_implicit(dt, 1e-11, 30, 4000)
     i2, nn, r2, upd = o2.step_implicit_newton(dt, 1e-11, 30, 4000, 0.0, 1)
     assert nn == 1 and i1 == i2
-    assert all(np.array_equal(a, b) for a, b in zip(o1.get_state(), o2.get_state()))
+    # (OpenMP reductions are not bitwise reproducible run to run, hence a round-off tolerance)
+    assert all(rel_l2(a, b) <= 1e-12 for a, b in zip(o1.get_state(), o2.get_state()))
