@@ -118,6 +118,16 @@ ARK_M1_API int ark_m1_steps_explicit(ark_m1* h, double dt, int nsteps);
  * Synchronises the stream.  dt <= 0, tol <= 0, restart < 1, maxit < 0: ARK_M1_E_ARG. */
 ARK_M1_API int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual);
 
+/* Newton-Raphson on the non-linear implicit system ("we use a Newton-Raphson method ... a linear system has
+ * to be solved at each iteration").  Iteration k re-assembles the operator with the coefficients of the iterate U^k, keeps
+ * U^n (+ affine terms) on the right-hand side and runs GMRES from U^k; the first iteration is
+ * ark_m1_step_implicit.  Stops when ||U^{k+1} - U^k||_2 <= newton_tol ||U^{k+1}||_2 or after max_newton iterations (not an
+ * error).  Returns the total number of GMRES iterations or a negative error code; *newton_iterations, *final_residual (true
+ * relative residual of the last linear solve) and *final_update (last relative update) are host pointers and may be NULL.
+ * A temperature, if set, is linearised about T^n throughout and updated once at the end. */
+ARK_M1_API int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int restart, int maxit, double newton_tol,
+                                           int max_newton, int* newton_iterations, double* final_residual, double* final_update);
+
 /* Step 3 of the operator splitting: explicit addition of the velocity sources of Eq. 6
  * using the fields "ux", "uy".  ARK_M1_E_NOTSET if they are missing. */
 ARK_M1_API int ark_m1_add_velocity_sources(ark_m1* h, double dt);

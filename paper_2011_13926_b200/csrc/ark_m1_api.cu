@@ -40,6 +40,7 @@ struct ark_m1 {
     MfPlanes mf;       // matrix-free coefficient planes (op_kind == 1)
     double* V;         // (m+1) vectors of `stride` doubles
     double* tvec;      // 3N
+    double* nprev;     // 3N, previous Newton iterate (lazy)
     long long stride;
     int m_alloc, maxit_alloc;
     GmresWork W;
@@ -156,7 +157,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
 
 static void free_implicit(ark_m1* h)
 {
-    cudaFree(h->A.off); cudaFree(h->A.C); cudaFree(h->A.Minv); cudaFree(h->A.b); cudaFree(h->V); cudaFree(h->tvec); cudaFree(h->wblock);
+    cudaFree(h->A.off); cudaFree(h->A.C); cudaFree(h->A.Minv); cudaFree(h->A.b); cudaFree(h->V); cudaFree(h->tvec); cudaFree(h->wblock); cudaFree(h->nprev); h->nprev = nullptr;
     cudaFree(h->mf.J); cudaFree(h->mf.fE); cudaFree(h->mf.fN); cudaFree(h->mf.dE); cudaFree(h->mf.dF); cudaFree(h->mf.xlo); cudaFree(h->mf.ylo);
     memset(&h->mf, 0, sizeof h->mf);
     h->A.off = h->A.C = h->A.Minv = h->A.b = nullptr; h->V = h->tvec = nullptr; h->wblock = nullptr; h->m_alloc = 0; h->maxit_alloc = 0;
@@ -425,38 +426,31 @@ static int fetch_ctl(ark_m1* h)
     return 0;
 }
 
-static int assemble_system(ark_m1* h, double dt)
+static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
 {
     const Fields f = fields_of(h);
     if (h->op_kind == 1) {
         h->mf.rx = dt / h->g.dx; h->mf.ry = dt / h->g.dy;
-        KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->mf, h->st));
+        KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->st));
     } else {
         MfPlanes none; memset(&none, 0, sizeof none);
-        KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, none, h->st));
+        KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, none, bsrc, h->st));
         KL(KC_SCALE, 648.0 * h->N, launch_scale_offdiag(h->g, h->A, h->st));
     }
     return 0;
 }
 
-extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual)
+// Restarted GMRES(m) on the assembled system, x = U[cur] in place (initial guess on entry).  Leaves the final control
+// block in h->ctl_host.
+static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
 {
-    if (!h) return ARK_M1_E_ARG;
-    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit: no state set%s", "");
-    int rc = ensure_implicit(h, restart, maxit);
-    if (rc) return rc;
-    const int m = restart;
+    int rc;
     const long long n = 3 * h->N, S = h->stride;
     const int sm = h->sm_count;
-    double* x = h->U[h->cur];          // initial guess U^n, solution in place
+    double* x = h->U[h->cur];
     GmresWork W = h->W;
     const int* stop = &W.ctl->inner_stop;
     const int MV = h->maxv;            // basis vectors per pass of the multi-vector kernels
-
-    CU(cudaEventRecord(h->ev[0], h->st));
-    if ((rc = assemble_system(h, dt))) return rc;
-    CU(cudaEventRecord(h->ev[1], h->st));
     KL(KC_SMALL, 0.0, launch_begin_solve(W, tol, m, maxit, h->st));
     KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
     if ((rc = true_residual(h, x))) return rc;
@@ -485,14 +479,19 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
         if ((rc = true_residual(h, x))) return rc;
         if ((rc = fetch_ctl(h))) return rc;
     }
-    CU(cudaEventRecord(h->ev[2], h->st));
+    return 0;
+}
+
+// History copy, matter update, timings, error mapping shared by the implicit entry points.
+static int finish_implicit(ark_m1* h, double dt, double* final_residual)
+{
+    GmresWork W = h->W;
     const GmresCtl c = *h->ctl_host;
-    // history
     const int nh = c.nhist < W.caphist ? c.nhist : W.caphist;
     h->hist_host->assign((size_t)nh, 0.0);
     if (nh > 0) CU(cudaMemcpyAsync(h->hist_host->data(), W.hist, (size_t)nh * sizeof(double), cudaMemcpyDeviceToHost, h->st));
     if (h->have_T && !c.nonfinite) {
-        KL(KC_SMALL, 40.0 * h->N, launch_matter_update(h->g, h->s, dt, h->sa, h->rho_cv, x, h->T[h->cur], h->st));
+        KL(KC_SMALL, 40.0 * h->N, launch_matter_update(h->g, h->s, dt, h->sa, h->rho_cv, h->U[h->cur], h->T[h->cur], h->st));
     }
     CU(cudaStreamSynchronize(h->st));
     kflush(h);
@@ -501,7 +500,65 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
     h->timings[0] = ms01; h->timings[1] = ms12; h->timings[2] = (double)ms01 + ms12;
     if (c.nonfinite) return fail(h, ARK_M1_E_NONFINITE, "step_implicit: non-finite norm in the solver (state or opacity holds NaN/Inf?)%s", "");
     if (final_residual) *final_residual = (c.bnorm > 0.0) ? c.rnorm / c.bnorm : c.rnorm;
-    return c.its;
+    return 0;
+}
+
+extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit: no state set%s", "");
+    int rc = ensure_implicit(h, restart, maxit);
+    if (rc) return rc;
+    CU(cudaEventRecord(h->ev[0], h->st));
+    if ((rc = assemble_system(h, dt))) return rc;
+    CU(cudaEventRecord(h->ev[1], h->st));
+    if ((rc = gmres_solve(h, tol, restart, maxit))) return rc;
+    CU(cudaEventRecord(h->ev[2], h->st));
+    if ((rc = finish_implicit(h, dt, final_residual))) return rc;
+    return h->ctl_host->its;
+}
+
+// Newton-Raphson on the implicit step.  With the Jacobian of DESIGN.md reading R4 and P homogeneous of
+// degree 1 the Newton update J_k (U^{k+1} - U^k) = -(U^k - U^n + dt R(U^k)) equals (I + dt L_{U^k}) U^{k+1} = U^n + affine:
+// re-assemble with the coefficients of the iterate, keep U^n on the right-hand side, start GMRES from U^k.
+extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int restart, int maxit, double newton_tol, int max_newton,
+                                           int* newton_iterations, double* final_residual, double* final_update)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0 || !(newton_tol >= 0.0) || max_newton < 1)
+        return fail(h, ARK_M1_E_ARG, "step_implicit_newton: need dt > 0, tol > 0, restart >= 1, maxit >= 0, newton_tol >= 0, max_newton >= 1%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit_newton: no state set%s", "");
+    int rc = ensure_implicit(h, restart, maxit);
+    if (rc) return rc;
+    const size_t n = 3 * (size_t)h->N;
+    if (!h->nprev && (rc = dmalloc(h, (void**)&h->nprev, n * sizeof(double)))) return rc;
+    double* x = h->U[h->cur];
+    double* base = h->U[h->cur ^ 1];                 // U^n lives in the other state buffer during the iteration
+    CU(cudaMemcpyAsync(base, x, n * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
+    CU(cudaEventRecord(h->ev[0], h->st));
+    CU(cudaEventRecord(h->ev[1], h->st));
+    int total = 0, k = 0;
+    double upd = 0.0;
+    for (k = 0; k < max_newton; ++k) {
+        CU(cudaMemcpyAsync(h->nprev, x, n * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
+        if ((rc = assemble_system(h, dt, base))) return rc;
+        if ((rc = gmres_solve(h, tol, restart, maxit))) return rc;
+        total += h->ctl_host->its;
+        if (h->ctl_host->nonfinite) break;
+        KL(KC_SMALL, 72.0 * h->N, launch_sub(h->nprev, x, h->nprev, (long long)n, h->st));
+        KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->nprev, h->nprev, 0, 1, 0, (long long)n, h->W, DOT_AUX0, h->sm_count, h->st));
+        KL(KC_DOT, 24.0 * h->N, launch_multi_dot(x, x, 0, 1, 0, (long long)n, h->W, DOT_AUX1, h->sm_count, h->st));
+        if ((rc = fetch_ctl(h))) return rc;
+        const double d = h->ctl_host->aux[0], nrm = h->ctl_host->aux[1];
+        upd = (nrm > 0.0) ? d / nrm : d;
+        if (upd <= newton_tol) { ++k; break; }
+    }
+    CU(cudaEventRecord(h->ev[2], h->st));
+    if ((rc = finish_implicit(h, dt, final_residual))) return rc;
+    if (newton_iterations) *newton_iterations = k;
+    if (final_update) *final_update = upd;
+    return total;
 }
 
 extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, double* out, double* b_out)

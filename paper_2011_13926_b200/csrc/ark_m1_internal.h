@@ -23,6 +23,7 @@ struct GmresCtl {
     int nhist;
     unsigned int ticket;           // "last block" counter of the reduction kernels
     int pad;
+    double aux[2];                 // scratch norms (Newton update size)
 };
 
 struct GmresWork {                 // device pointers into one small allocation
@@ -41,7 +42,7 @@ struct GmresWork {                 // device pointers into one small allocation
 
 enum { MAXV = 32 };                // basis vectors handled per pass of the multi-vector kernels
 
-enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5 };
+enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5, DOT_AUX0 = 6, DOT_AUX1 = 7 };
 
 // ---------------------------------------------------------------------------------------------------------
 // Launchers (each enqueues on `st`, returns cudaGetLastError()).
@@ -77,7 +78,10 @@ struct MfPlanes {
     double rx, ry; // dt/dx, dt/dy of the assembled step
 };
 // A.off / A.C may be null when mf.J is set (then only Minv, b and the coefficient planes are written)
-cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf, cudaStream_t st);
+// bsrc: planes [E|Fx|Fy] that supply the U^n part of the right-hand side (null: the state in `f`; non-null in Newton
+// iterations, where `f` is the iterate that only supplies the coefficients)
+cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf,
+                            const double* bsrc, cudaStream_t st);
 // out = sgn * s * (A [M^-1] v) + add, flux form from the coefficient planes; precond = 1 applies M^-1 (Minv) first
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
@@ -104,6 +108,7 @@ cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
 // x += Minv * (sum_{k<ctl->j} coef[k] V_k)  per cell
 cudaError_t launch_combine(const Grid& g, const double* V, long long stride, const double* Minv, double* x,
                            GmresWork W, int sm_count, cudaStream_t st);
+cudaError_t launch_sub(double* out, const double* a, const double* b, long long n, cudaStream_t st);   // out = a - b
 cudaError_t launch_begin_solve(GmresWork W, double tol, int m, int maxit, cudaStream_t st);
 
 }  // namespace ark

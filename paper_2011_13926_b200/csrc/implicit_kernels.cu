@@ -61,7 +61,8 @@ __device__ __forceinline__ void inv3(const Blk& B, Blk& I)
 }
 
 template <bool SD>
-__global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields f, double dt, BlockMatrix A, MfPlanes mf)
+__global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields f, double dt, BlockMatrix A, MfPlanes mf,
+                                                       const double* __restrict__ bsrc)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -109,6 +110,7 @@ __global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields 
     }
     // right-hand side
     double b[3] = { u[0].E, u[0].Fx, u[0].Fy };
+    if (bsrc) { b[0] = bsrc[id]; b[1] = bsrc[N + id]; b[2] = bsrc[2 * N + id]; }   // Newton iterate: U^n comes from bsrc
     if (f.T) b[0] += c * dt * u[0].sa * eta * Theta;
     if (f.source_E) b[0] += dt * f.source_E[id];
     // boundaries (R9): a Dirichlet ghost is known -> block x ghost moves to b; a neighbour that is this
@@ -150,11 +152,12 @@ __global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields 
         for (int e = 0; e < 9; ++e) A.off[((k - 1) * 9 + e) * N + id] = B[k].a[e];
 }
 
-cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf, cudaStream_t st)
+cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf,
+                            const double* bsrc, cudaStream_t st)
 {
     dim3 blk(32, 4), grd((g.nx + 31) / 32, (g.ny + 3) / 4);
-    if (s.is_default()) assemble_kernel<true><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf);
-    else assemble_kernel<false><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf);
+    if (s.is_default()) assemble_kernel<true><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf, bsrc);
+    else assemble_kernel<false><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf, bsrc);
     return cudaGetLastError();
 }
 

@@ -59,6 +59,8 @@ __device__ void epilogue(const GmresWork& W, int mode, const double* d, int nv, 
             if (mode == DOT_H) W.H[i * m + j] = h; else W.H[i * m + j] += h;
             W.coef[i] = h * W.scale[i];
         }
+    } else if (mode == DOT_AUX0 || mode == DOT_AUX1) {
+        c->aux[mode - DOT_AUX0] = sqrt(d[0]);
     } else if (mode == DOT_UPD) {           // h_{j+1,j} = ||w||, Givens rotations (Saad 2003, Sect. 6.5.3)
         const int j = c->j;
         const double hn = sqrt(d[0]);
@@ -128,7 +130,7 @@ template <int NV>
 __global__ void __launch_bounds__(KTHREADS) multi_dot_kernel(const double* __restrict__ w, const double* __restrict__ V0,
                                                              long long stride, long long n, GmresWork W, int mode, int col0)
 {
-    if (mode >= DOT_H && W.ctl->inner_stop) return;
+    if ((mode == DOT_H || mode == DOT_H2) && W.ctl->inner_stop) return;
     double acc[NV];
 #pragma unroll
     for (int k = 0; k < NV; ++k) acc[k] = 0.0;
@@ -279,6 +281,18 @@ cudaError_t launch_combine(const Grid& g, const double* V, long long stride, con
     const long long N = (long long)g.nx * g.ny;
     const long long need = (N + KTHREADS - 1) / KTHREADS, cap = (long long)sm_count * 8;
     combine_kernel<<<(int)(need < cap ? need : cap), KTHREADS, 0, st>>>(N, V, stride, Minv, x, W);
+    return cudaGetLastError();
+}
+
+__global__ void sub_kernel(double* __restrict__ o, const double* __restrict__ a, const double* __restrict__ b, long long n)
+{
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) o[k] = a[k] - b[k];
+}
+
+cudaError_t launch_sub(double* out, const double* a, const double* b, long long n, cudaStream_t st)
+{
+    const long long need = (n + 255) / 256;
+    sub_kernel<<<(int)(need < 148 * 8 ? need : 148 * 8), 256, 0, st>>>(out, a, b, n);
     return cudaGetLastError();
 }
 
