@@ -62,6 +62,7 @@ typedef struct oracle_m1 {
     int eig;         /* 0: Eq. 14 (default), 1: fixed +-c, 2: fixed +-c/sqrt(3) */
     int closure;     /* 0: M1 (default), 1: P1 (chi = 1/3) */
     int lin;         /* 0: analytic pressure Jacobian (default, R4), 1: frozen Eddington tensor */
+    int krylov;      /* 0: restarted GMRES (north_star, default), 1: BiCGStab (the paper's solver) */
     double eig_floor;/* lambda^+ >= floor*c, lambda^- <= -floor*c; default 0 */
     double a_r;      /* radiation constant, default 1 */
     double *rho_cv, *ux, *uy, *source_E; /* stage-2 fields (may be NULL) */
@@ -603,6 +604,57 @@ static int gmres(oracle_m1 *h, const system_t *s, double *x, double tol, int m, 
     return its;
 }
 
+/* BiCGStab (van der Vorst 1992; the paper's Krylov method, "BiCGStab"), right-preconditioned with the same
+ * block-Jacobi M: p^ = M^-1 p, v = A p^, s^ = M^-1 s, t = A s^, x += alpha p^ + omega s^.
+ * Stops when the recursive residual satisfies ||r|| <= tol ||b||; the TRUE residual is then recomputed and, if it is still
+ * above the target (drift), the iteration restarts from it.  One iteration = two operator applications.
+ * `restart` is unused.  Returns the number of iterations; *relres = true relative residual at exit. */
+static int bicgstab(oracle_m1 *h, const system_t *s, double *x, double tol, int maxit, double *relres)
+{
+    const long n = 3 * s->N;
+    double *r = (double *)malloc(sizeof(double) * n), *rh = (double *)malloc(sizeof(double) * n), *p = (double *)malloc(sizeof(double) * n);
+    double *v = (double *)malloc(sizeof(double) * n), *t = (double *)malloc(sizeof(double) * n), *ph = (double *)malloc(sizeof(double) * n);
+    double *sh = (double *)malloc(sizeof(double) * n);
+    if (!r || !rh || !p || !v || !t || !ph || !sh) return -3;
+    const double bnorm = sqrt(dot(s->b, s->b, n)), target = tol * bnorm;
+    int its = 0; double rnorm;
+    h->nhist = 0;
+    for (;;) {
+        spmv(s, x, r);
+        for (long k = 0; k < n; ++k) r[k] = s->b[k] - r[k];
+        rnorm = sqrt(dot(r, r, n));
+        hist_push(h, bnorm > 0 ? rnorm / bnorm : rnorm);
+        if (rnorm <= target || its >= maxit) break;
+        memcpy(rh, r, sizeof(double) * n);
+        memset(p, 0, sizeof(double) * n); memset(v, 0, sizeof(double) * n);
+        double rho = 1.0, alpha = 1.0, omega = 1.0;
+        const int its0 = its;
+        while (its < maxit) {
+            const double rho_new = dot(rh, r, n);
+            if (rho_new == 0.0 || omega == 0.0) break;                 /* breakdown: restart from the true residual */
+            const double beta = (rho_new / rho) * (alpha / omega);
+            for (long k = 0; k < n; ++k) p[k] = r[k] + beta * (p[k] - omega * v[k]);
+            precond(s, p, ph); spmv(s, ph, v);
+            const double rhv = dot(rh, v, n);
+            if (rhv == 0.0) break;
+            alpha = rho_new / rhv;
+            for (long k = 0; k < n; ++k) r[k] -= alpha * v[k];          /* s, stored in r */
+            precond(s, r, sh); spmv(s, sh, t);
+            const double tt = dot(t, t, n);
+            omega = (tt > 0.0) ? dot(t, r, n) / tt : 0.0;
+            for (long k = 0; k < n; ++k) { x[k] += alpha * ph[k] + omega * sh[k]; r[k] -= omega * t[k]; }
+            rho = rho_new; ++its;
+            const double rn = sqrt(dot(r, r, n));
+            hist_push(h, bnorm > 0 ? rn / bnorm : rn);
+            if (rn <= target) break;
+        }
+        if (its == its0) break;                                           /* no progress possible */
+    }
+    *relres = bnorm > 0 ? rnorm / bnorm : rnorm;
+    free(r); free(rh); free(p); free(v); free(t); free(ph); free(sh);
+    return its;
+}
+
 /* One linearised implicit step (R4): (I + dt L_n) U^{n+1} = U^n + affine terms; then the T update (R10). */
 ORACLE_API int oracle_m1_step_implicit(oracle_m1 *h, double dt, double tol, int restart, int maxit, double *final_residual)
 {
@@ -612,7 +664,7 @@ ORACLE_API int oracle_m1_step_implicit(oracle_m1 *h, double dt, double tol, int 
     double *x = (double *)malloc(sizeof(double) * 3 * N);
     memcpy(x, h->E, sizeof(double) * N); memcpy(x + N, h->Fx, sizeof(double) * N); memcpy(x + 2 * N, h->Fy, sizeof(double) * N);
     double rel = 0.0;
-    const int its = gmres(h, &s, x, tol, restart, maxit, &rel);
+    const int its = h->krylov == 1 ? bicgstab(h, &s, x, tol, maxit, &rel) : gmres(h, &s, x, tol, restart, maxit, &rel);
     if (its >= 0) {
         if (h->has_T) {
             #pragma omp parallel for schedule(static)
@@ -650,7 +702,7 @@ ORACLE_API int oracle_m1_step_implicit_newton(oracle_m1 *h, double dt, double to
     for (k = 0; k < max_newton; ++k) {
         system_t s; const int rc = system_build(h, dt, base, &s); if (rc) { free(base); free(x); return rc; }
         memcpy(x, h->E, sizeof(double) * N); memcpy(x + N, h->Fx, sizeof(double) * N); memcpy(x + 2 * N, h->Fy, sizeof(double) * N);
-        const int its = gmres(h, &s, x, tol, restart, maxit, &rel);
+        const int its = h->krylov == 1 ? bicgstab(h, &s, x, tol, maxit, &rel) : gmres(h, &s, x, tol, restart, maxit, &rel);
         system_free(&s);
         if (its < 0) { free(base); free(x); return its; }
         total += its;
@@ -763,6 +815,7 @@ ORACLE_API int oracle_m1_set_option(oracle_m1 *h, const char *key, double value)
     else if (!strcmp(key, "closure")) h->closure = (int)value;
     else if (!strcmp(key, "linearisation")) h->lin = (int)value;
     else if (!strcmp(key, "eig_floor")) h->eig_floor = value;
+    else if (!strcmp(key, "krylov")) h->krylov = (int)value;
     else if (!strcmp(key, "a_r")) h->a_r = value;
     else { snprintf(h->err, sizeof h->err, "unknown option %s", key); return -1; }
     return 0;

@@ -223,3 +223,32 @@ def test_newton_first_iteration_is_the_linearised_step():
     assert nn == 1 and i1 == i2
     # (OpenMP reductions are not bitwise reproducible run to run, hence a round-off tolerance)
     assert all(rel_l2(a, b) <= 1e-12 for a, b in zip(o1.get_state(), o2.get_state()))
+
+
+@pytest.mark.parametrize("bc", BCS)
+def test_bicgstab_matches_dense_direct_solve(bc):
+    # the paper's Krylov method, right-preconditioned with the same block-Jacobi: dense LU pin
+    w = small_random_state(9, 8, seed=77, bc=bc)
+    o = make_oracle(w, dict(krylov=1))
+    dt = 100.0 * wl.explicit_dt(w["dx"], w["dy"])
+    M, b = o.dense_matrix(dt)
+    x = np.linalg.solve(M, b).reshape(3, w["ny"], w["nx"])
+    its, res = o.step_implicit(dt, 1e-12, 30, 2000)
+    E, F = o.get_state()
+    assert 0 < its < 2000 and res <= 1e-12
+    assert rel_l2(np.concatenate((E[None], F)), x) <= 1e-10
+    h = o.history()
+    assert h[-1] <= 1e-12 and len(h) >= its + 1
+
+
+def test_bicgstab_and_gmres_agree_and_maxit_semantics():
+    w = wl.random_medium(96, seed=5)
+    dt = 50.0 * wl.explicit_dt(w["dx"], w["dy"])
+    og, ob = make_oracle(w), make_oracle(w, dict(krylov=1))
+    ig, rg = og.step_implicit(dt, 1e-11, 30, 4000)
+    ib, rb = ob.step_implicit(dt, 1e-11, 30, 4000)
+    assert rb <= 1e-11 and ib < ig            # one BiCGStab iteration = two operator applications
+    assert max(rel_l2(a, c) for a, c in zip(ob.get_state(), og.get_state())) <= 1e-8
+    o2 = make_oracle(w, dict(krylov=1))
+    its, res = o2.step_implicit(dt, 1e-14, 30, 5)
+    assert its == 5 and res > 1e-14
