@@ -85,6 +85,9 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *   "eig_floor"     x: lambda+ >= x c, lambda- <= -x c; default 0
  *   "a_r"           radiation constant (default 1)
  *   "orthogonalisation" 1: one-pass classical Gram-Schmidt (default)   2: CGS2 (re-orthogonalise once)
+ *   "krylov"            0: restarted GMRES(restart) (north_star, default)   1: BiCGStab, the paper's solver,
+ *                       right-preconditioned with the same block-Jacobi; `restart` is then ignored and the returned count is in
+ *                       BiCGStab iterations (two operator applications each)
  *   "vectors_per_pass"  basis vectors handled per pass of the multi-dot / multi-axpy kernels, 1..32 (default 16, by measurement)
  *   "kernel_timing"     1: time every kernel launch with CUDA events (see ark_m1_get_kernel_stats); default 0
  *   "explicit_kernel"   0: one-thread-per-cell kernel   1: row-marching kernel (default)   2: barrier-free warp-shuffle kernel

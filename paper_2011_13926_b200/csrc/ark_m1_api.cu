@@ -34,7 +34,7 @@ struct ark_m1 {
     double *rho_cv, *ux, *uy, *source_E;
     unsigned long long* counts;   // 2
     // options
-    int ortho, explicit_kernel, op_kind, maxv, basis_pad;
+    int ortho, explicit_kernel, op_kind, maxv, basis_pad, krylov;
     // implicit workspace (lazy)
     BlockMatrix A;
     MfPlanes mf;       // matrix-free coefficient planes (op_kind == 1)
@@ -237,6 +237,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
     else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1 or 2%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "krylov")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "krylov must be 0 (GMRES) or 1 (BiCGStab)%s", ""); h->krylov = iv; }
     else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 32]%s", ""); h->maxv = iv; }
     else if (!strcmp(key, "basis_pad")) { if (iv < 0 || (iv & 31)) return fail(h, ARK_M1_E_ARG, "basis_pad must be a non-negative multiple of 32 doubles%s", ""); if (iv != h->basis_pad) { cudaStreamSynchronize(h->st); free_implicit(h); } h->basis_pad = iv; }
     else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
@@ -482,6 +483,56 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
     return 0;
 }
 
+// Right-preconditioned BiCGStab (the paper's Krylov method) on the assembled system; same conventions as
+// gmres_solve.  Vector slots of h->V: 0 = r (and s), 1 = t, 2 = r^, 3 = p, 4 = v, 5 = y (x = x0 + M^-1 y).
+// Iterations are enqueued in batches of 8 without host round trips; one iteration = two operator applications.
+static int op_apply_hat(ark_m1* h, const double* vin, double* vout, const int* stop)
+{
+    if (h->op_kind == 1)
+        KL(KC_SPMV, 264.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, stop, 1, h->sm_count, h->st));
+    else
+        KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, vin, vout, nullptr, nullptr, 1.0, stop, h->st));
+    return 0;
+}
+
+static int bicgstab_solve(ark_m1* h, double tol, int maxit)
+{
+    int rc;
+    const long long n = 3 * h->N, S = h->stride;
+    const int sm = h->sm_count;
+    double* x = h->U[h->cur];
+    GmresWork W = h->W;
+    const int* stop = &W.ctl->inner_stop;
+    double *r = h->V, *t = h->V + S, *rh = h->V + 2 * S, *p = h->V + 3 * S, *v = h->V + 4 * S, *y = h->V + 5 * S;
+    KL(KC_SMALL, 0.0, launch_begin_solve(W, tol, 1, maxit, h->st));
+    KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
+    CU(cudaMemsetAsync(y, 0, (size_t)n * sizeof(double), h->st));
+    if ((rc = true_residual(h, x))) return rc;
+    if ((rc = fetch_ctl(h))) return rc;
+    while (!h->ctl_host->inner_stop) {
+        const int its0 = h->ctl_host->its;
+        KL(KC_UPDATE, 96.0 * h->N, launch_bicg_begin(r, rh, p, v, n, W, h->st));
+        for (;;) {
+            for (int k = 0; k < 8; ++k) {
+                KL(KC_UPDATE, 96.0 * h->N, launch_bicg_p(r, p, v, n, W, h->st));
+                if ((rc = op_apply_hat(h, p, v, stop))) return rc;
+                KL(KC_DOT, 48.0 * h->N, launch_multi_dot(v, rh, S, 1, 0, n, W, BICG_ALPHA, sm, h->st));
+                KL(KC_UPDATE, 72.0 * h->N, launch_bicg_s(r, v, n, W, h->st));
+                if ((rc = op_apply_hat(h, r, t, stop))) return rc;
+                KL(KC_DOT, 72.0 * h->N, launch_multi_dot(t, r, S, 2, 0, n, W, BICG_OMEGA, sm, h->st));
+                KL(KC_UPDATE, 168.0 * h->N, launch_bicg_xr(y, p, r, t, rh, n, W, sm, h->st));
+            }
+            if ((rc = fetch_ctl(h))) return rc;
+            if (h->ctl_host->inner_stop) break;
+        }
+        KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, y, x, h->st));
+        if ((rc = true_residual(h, x))) return rc;      // resets inner_stop unless converged / out of iterations
+        if ((rc = fetch_ctl(h))) return rc;
+        if (h->ctl_host->its == its0) break;            // breakdown without progress
+    }
+    return 0;
+}
+
 // History copy, matter update, timings, error mapping shared by the implicit entry points.
 static int finish_implicit(ark_m1* h, double dt, double* final_residual)
 {
@@ -508,12 +559,12 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
     if (!h) return ARK_M1_E_ARG;
     if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit: no state set%s", "");
-    int rc = ensure_implicit(h, restart, maxit);
+    int rc = ensure_implicit(h, (h->krylov == 1 && restart < 5) ? 5 : restart, maxit);
     if (rc) return rc;
     CU(cudaEventRecord(h->ev[0], h->st));
     if ((rc = assemble_system(h, dt))) return rc;
     CU(cudaEventRecord(h->ev[1], h->st));
-    if ((rc = gmres_solve(h, tol, restart, maxit))) return rc;
+    if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : gmres_solve(h, tol, restart, maxit))) return rc;
     CU(cudaEventRecord(h->ev[2], h->st));
     if ((rc = finish_implicit(h, dt, final_residual))) return rc;
     return h->ctl_host->its;
@@ -529,7 +580,7 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
     if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0 || !(newton_tol >= 0.0) || max_newton < 1)
         return fail(h, ARK_M1_E_ARG, "step_implicit_newton: need dt > 0, tol > 0, restart >= 1, maxit >= 0, newton_tol >= 0, max_newton >= 1%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit_newton: no state set%s", "");
-    int rc = ensure_implicit(h, restart, maxit);
+    int rc = ensure_implicit(h, (h->krylov == 1 && restart < 5) ? 5 : restart, maxit);
     if (rc) return rc;
     const size_t n = 3 * (size_t)h->N;
     if (!h->nprev && (rc = dmalloc(h, (void**)&h->nprev, n * sizeof(double)))) return rc;
@@ -543,7 +594,7 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
     for (k = 0; k < max_newton; ++k) {
         CU(cudaMemcpyAsync(h->nprev, x, n * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
         if ((rc = assemble_system(h, dt, base))) return rc;
-        if ((rc = gmres_solve(h, tol, restart, maxit))) return rc;
+        if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : gmres_solve(h, tol, restart, maxit))) return rc;
         total += h->ctl_host->its;
         if (h->ctl_host->nonfinite) break;
         KL(KC_SMALL, 72.0 * h->N, launch_sub(h->nprev, x, h->nprev, (long long)n, h->st));

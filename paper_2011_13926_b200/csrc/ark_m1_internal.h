@@ -24,6 +24,7 @@ struct GmresCtl {
     unsigned int ticket;           // "last block" counter of the reduction kernels
     int pad;
     double aux[2];                 // scratch norms (Newton update size)
+    double bs[8];                  // BiCGStab scalars: rho, alpha, omega, rho_new, ||r|| (recursive), flag "restart after this iteration"
 };
 
 struct GmresWork {                 // device pointers into one small allocation
@@ -42,7 +43,9 @@ struct GmresWork {                 // device pointers into one small allocation
 
 enum { MAXV = 32 };                // basis vectors handled per pass of the multi-vector kernels
 
-enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5, DOT_AUX0 = 6, DOT_AUX1 = 7 };
+enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5, DOT_AUX0 = 6, DOT_AUX1 = 7,
+               BICG_ALPHA = 8, BICG_OMEGA = 9, BICG_RHO = 10 };
+enum { BS_RHO = 0, BS_ALPHA = 1, BS_OMEGA = 2, BS_RHO_NEW = 3, BS_RN = 4, BS_RESTART = 5 };
 
 // ---------------------------------------------------------------------------------------------------------
 // Launchers (each enqueues on `st`, returns cudaGetLastError()).
@@ -108,6 +111,13 @@ cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
 // x += Minv * (sum_{k<ctl->j} coef[k] V_k)  per cell
 cudaError_t launch_combine(const Grid& g, const double* V, long long stride, const double* Minv, double* x,
                            GmresWork W, int sm_count, cudaStream_t st);
+// BiCGStab vector kernels (krylov_kernels.cu); every one returns at once when ctl->inner_stop is set
+cudaError_t launch_bicg_begin(double* r, double* rhat, double* p, double* v, long long n, GmresWork W, cudaStream_t st);
+cudaError_t launch_bicg_p(const double* r, double* p, const double* v, long long n, GmresWork W, cudaStream_t st);      // p = r + beta (p - omega v)
+cudaError_t launch_bicg_s(double* r, const double* v, long long n, GmresWork W, cudaStream_t st);                        // r -= alpha v
+cudaError_t launch_bicg_xr(double* y, const double* p, double* r, const double* t, const double* rhat, long long n,
+                           GmresWork W, int sm_count, cudaStream_t st);   // y += alpha p + omega r; r -= omega t; rho, ||r||
+cudaError_t launch_combine_y(const Grid& g, const double* Minv, double* y, double* x, cudaStream_t st);                  // x += M^-1 y; y = 0
 cudaError_t launch_sub(double* out, const double* a, const double* b, long long n, cudaStream_t st);   // out = a - b
 cudaError_t launch_begin_solve(GmresWork W, double tol, int m, int maxit, cudaStream_t st);
 

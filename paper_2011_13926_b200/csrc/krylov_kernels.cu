@@ -59,6 +59,24 @@ __device__ void epilogue(const GmresWork& W, int mode, const double* d, int nv, 
             if (mode == DOT_H) W.H[i * m + j] = h; else W.H[i * m + j] += h;
             W.coef[i] = h * W.scale[i];
         }
+    } else if (mode == BICG_ALPHA) {        // alpha = rho_new / <r^, v>
+        const double rhv = d[0];
+        if (rhv == 0.0 || !isfinite(rhv)) { c->inner_stop = 1; if (!isfinite(rhv)) c->nonfinite = 1; }
+        else c->bs[BS_ALPHA] = c->bs[BS_RHO_NEW] / rhv;
+    } else if (mode == BICG_OMEGA) {        // omega = <t, s> / <t, t>
+        const double ts = d[0], tt = d[1];
+        c->bs[BS_OMEGA] = (tt > 0.0) ? ts / tt : 0.0;
+        c->bs[BS_RESTART] = (c->bs[BS_OMEGA] == 0.0 || !isfinite(c->bs[BS_OMEGA])) ? 1.0 : 0.0;
+        if (!isfinite(c->bs[BS_OMEGA])) { c->nonfinite = 1; c->inner_stop = 1; }
+    } else if (mode == BICG_RHO) {          // end of a BiCGStab iteration: rho <- rho_new, rho_new = <r^, r>, ||r||
+        c->bs[BS_RHO] = c->bs[BS_RHO_NEW];
+        c->bs[BS_RHO_NEW] = d[0];
+        const double rn = sqrt(d[1]);
+        c->bs[BS_RN] = rn; c->est = rn;
+        c->its += 1;
+        hist_push(W, c, rn);
+        if (!isfinite(rn) || !isfinite(d[0])) c->nonfinite = 1;
+        if (rn <= c->target || c->its >= c->maxit || d[0] == 0.0 || c->bs[BS_RESTART] != 0.0 || c->nonfinite) c->inner_stop = 1;
     } else if (mode == DOT_AUX0 || mode == DOT_AUX1) {
         c->aux[mode - DOT_AUX0] = sqrt(d[0]);
     } else if (mode == DOT_UPD) {           // h_{j+1,j} = ||w||, Givens rotations (Saad 2003, Sect. 6.5.3)
@@ -130,7 +148,7 @@ template <int NV>
 __global__ void __launch_bounds__(KTHREADS) multi_dot_kernel(const double* __restrict__ w, const double* __restrict__ V0,
                                                              long long stride, long long n, GmresWork W, int mode, int col0)
 {
-    if ((mode == DOT_H || mode == DOT_H2) && W.ctl->inner_stop) return;
+    if ((mode == DOT_H || mode == DOT_H2 || mode == BICG_ALPHA || mode == BICG_OMEGA) && W.ctl->inner_stop) return;
     double acc[NV];
 #pragma unroll
     for (int k = 0; k < NV; ++k) acc[k] = 0.0;
@@ -281,6 +299,126 @@ cudaError_t launch_combine(const Grid& g, const double* V, long long stride, con
     const long long N = (long long)g.nx * g.ny;
     const long long need = (N + KTHREADS - 1) / KTHREADS, cap = (long long)sm_count * 8;
     combine_kernel<<<(int)(need < cap ? need : cap), KTHREADS, 0, st>>>(N, V, stride, Minv, x, W);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// BiCGStab (the paper's Krylov method), right-preconditioned on A M^-1 like the GMRES path; the
+// solution is accumulated in y (x = x0 + M^-1 y at the end of a cycle).  Scalars live in ctl->bs.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(KTHREADS) bicg_begin_kernel(double* __restrict__ r, double* __restrict__ rhat, double* __restrict__ p,
+                                                              double* __restrict__ v, long long n, GmresWork W)
+{
+    GmresCtl* c = W.ctl;
+    if (c->inner_stop) return;
+    for (long long k = blockIdx.x * (long long)KTHREADS + threadIdx.x; k < n; k += (long long)gridDim.x * KTHREADS) {
+        rhat[k] = r[k]; p[k] = 0.0; v[k] = 0.0;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        c->bs[BS_RHO] = 1.0; c->bs[BS_ALPHA] = 1.0; c->bs[BS_OMEGA] = 1.0;
+        c->bs[BS_RHO_NEW] = c->rnorm * c->rnorm;      // <r^, r> with r^ = r
+        c->bs[BS_RN] = c->rnorm; c->bs[BS_RESTART] = 0.0;
+    }
+}
+
+__global__ void __launch_bounds__(KTHREADS) bicg_p_kernel(const double* __restrict__ r, double* __restrict__ p, const double* __restrict__ v,
+                                                          long long n, GmresWork W)
+{
+    const GmresCtl* c = W.ctl;
+    if (c->inner_stop) return;
+    const double omega = c->bs[BS_OMEGA];
+    const double beta = (c->bs[BS_RHO_NEW] / c->bs[BS_RHO]) * (c->bs[BS_ALPHA] / omega);
+    const long long n2 = n >> 1;
+    const double2* r2 = reinterpret_cast<const double2*>(r); const double2* v2 = reinterpret_cast<const double2*>(v);
+    double2* p2 = reinterpret_cast<double2*>(p);
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
+        const double2 a = r2[e], b = v2[e]; double2 q = p2[e];
+        q.x = fma(beta, fma(-omega, b.x, q.x), a.x); q.y = fma(beta, fma(-omega, b.y, q.y), a.y);
+        p2[e] = q;
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) p[n - 1] = r[n - 1] + beta * (p[n - 1] - omega * v[n - 1]);
+}
+
+__global__ void __launch_bounds__(KTHREADS) bicg_s_kernel(double* __restrict__ r, const double* __restrict__ v, long long n, GmresWork W)
+{
+    const GmresCtl* c = W.ctl;
+    if (c->inner_stop) return;
+    const double alpha = c->bs[BS_ALPHA];
+    const long long n2 = n >> 1;
+    double2* r2 = reinterpret_cast<double2*>(r); const double2* v2 = reinterpret_cast<const double2*>(v);
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
+        double2 a = r2[e]; const double2 b = v2[e];
+        a.x = fma(-alpha, b.x, a.x); a.y = fma(-alpha, b.y, a.y);
+        r2[e] = a;
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) r[n - 1] -= alpha * v[n - 1];
+}
+
+__global__ void __launch_bounds__(KTHREADS) bicg_xr_kernel(double* __restrict__ y, const double* __restrict__ p, double* __restrict__ r,
+                                                           const double* __restrict__ t, const double* __restrict__ rhat, long long n, GmresWork W)
+{
+    const GmresCtl* c = W.ctl;
+    if (c->inner_stop) return;
+    const double alpha = c->bs[BS_ALPHA], omega = c->bs[BS_OMEGA];
+    double acc[2] = { 0.0, 0.0 };
+    const long long n2 = n >> 1;
+    double2* y2 = reinterpret_cast<double2*>(y); double2* r2 = reinterpret_cast<double2*>(r);
+    const double2* p2 = reinterpret_cast<const double2*>(p); const double2* t2 = reinterpret_cast<const double2*>(t);
+    const double2* h2 = reinterpret_cast<const double2*>(rhat);
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
+        double2 yy = y2[e], s = r2[e]; const double2 pp = p2[e], tt = t2[e], hh = h2[e];
+        yy.x = fma(alpha, pp.x, fma(omega, s.x, yy.x)); yy.y = fma(alpha, pp.y, fma(omega, s.y, yy.y));
+        s.x = fma(-omega, tt.x, s.x); s.y = fma(-omega, tt.y, s.y);
+        y2[e] = yy; r2[e] = s;
+        acc[0] += hh.x * s.x + hh.y * s.y; acc[1] += s.x * s.x + s.y * s.y;
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const long long k = n - 1;
+        y[k] += alpha * p[k] + omega * r[k];
+        r[k] -= omega * t[k];
+        acc[0] += rhat[k] * r[k]; acc[1] += r[k] * r[k];
+    }
+    reduce_and_finish<2>(acc, W, BICG_RHO, 0);
+}
+
+// x += M^-1 y, y = 0 (end of a BiCGStab cycle; "K x = y")
+__global__ void __launch_bounds__(KTHREADS) combine_y_kernel(long long N, const double* __restrict__ Minv, double* __restrict__ y, double* __restrict__ x)
+{
+    for (long long id = blockIdx.x * (long long)KTHREADS + threadIdx.x; id < N; id += (long long)gridDim.x * KTHREADS) {
+        const double u0 = y[id], u1 = y[N + id], u2 = y[2 * N + id];
+        x[id]         += Minv[0 * N + id] * u0 + Minv[1 * N + id] * u1 + Minv[2 * N + id] * u2;
+        x[N + id]     += Minv[3 * N + id] * u0 + Minv[4 * N + id] * u1 + Minv[5 * N + id] * u2;
+        x[2 * N + id] += Minv[6 * N + id] * u0 + Minv[7 * N + id] * u1 + Minv[8 * N + id] * u2;
+        y[id] = 0.0; y[N + id] = 0.0; y[2 * N + id] = 0.0;
+    }
+}
+
+cudaError_t launch_bicg_begin(double* r, double* rhat, double* p, double* v, long long n, GmresWork W, cudaStream_t st)
+{
+    bicg_begin_kernel<<<148 * 4, KTHREADS, 0, st>>>(r, rhat, p, v, n, W);
+    return cudaGetLastError();
+}
+cudaError_t launch_bicg_p(const double* r, double* p, const double* v, long long n, GmresWork W, cudaStream_t st)
+{
+    bicg_p_kernel<<<148 * 4, KTHREADS, 0, st>>>(r, p, v, n, W);
+    return cudaGetLastError();
+}
+cudaError_t launch_bicg_s(double* r, const double* v, long long n, GmresWork W, cudaStream_t st)
+{
+    bicg_s_kernel<<<148 * 4, KTHREADS, 0, st>>>(r, v, n, W);
+    return cudaGetLastError();
+}
+cudaError_t launch_bicg_xr(double* y, const double* p, double* r, const double* t, const double* rhat, long long n,
+                           GmresWork W, int sm_count, cudaStream_t st)
+{
+    bicg_xr_kernel<<<grid_for(n, sm_count), KTHREADS, 0, st>>>(y, p, r, t, rhat, n, W);
+    return cudaGetLastError();
+}
+cudaError_t launch_combine_y(const Grid& g, const double* Minv, double* y, double* x, cudaStream_t st)
+{
+    const long long N = (long long)g.nx * g.ny;
+    const long long need = (N + KTHREADS - 1) / KTHREADS;
+    combine_y_kernel<<<(int)(need < 148 * 8 ? need : 148 * 8), KTHREADS, 0, st>>>(N, Minv, y, x);
     return cudaGetLastError();
 }
 
