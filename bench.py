@@ -187,6 +187,15 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0):
     return total
 
 
+def bicgstab_bytes_per_cell(iters, operator=1):
+    """Algorithmic bytes per cell of `iters` BiCGStab iterations as built: two operator applications + p update (96) +
+    <r^,v> (48) + s update (72) + <t,s>,<t,t> (72) + y/r update with rho, ||r|| (168); one cycle end: x += M^-1 y (168),
+    true residual, norm (24), cycle start (96)."""
+    op = 336.0 if operator == 0 else 264.0
+    res = 480.0 if operator == 0 else 216.0
+    return iters * (2.0 * op + 456.0) + 168.0 + res + 24.0 + 96.0
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -338,6 +347,33 @@ def run_ours(args):
                                                           "per_ratio": sm_out, "closest": best_k, "closest_T_implicit_over_K_T_explicit": sm_out[best_k]["over_K"],
                                                           "reached": bool(any(v["implicit_wins"] for v in sm_out.values()))}
             del devs
+        # ---- BiCGStab (the paper's Krylov method): same sweeps, option krylov = 1 -------------------------
+        if not args.no_sweep:
+            g.set_option("krylov", 1)
+            bi = {"rough_medium": {}, "smooth_problem": {}}
+            for label, tensors, ratios in (("rough_medium", devt, (10.0, 50.0, 100.0, 200.0)),
+                                           ("smooth_problem", None, (50.0, 100.0, 200.0, 1000.0, 2000.0))):
+                if tensors is None:
+                    ws = wl.gaussian_diffusion(n)
+                    tensors = {k: torch.from_numpy(np.ascontiguousarray(ws[k])).to(dev) for k in ("E", "F", "sigma_a", "sigma_s")}
+                for ratio in ratios:
+                    g.set_state(tensors["E"], tensors["F"], tensors["sigma_a"], tensors["sigma_s"])
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    its, res = g.step_implicit(ratio * dt_e, TOL, RESTART, MAXIT)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1)
+                    tm = g.timings()
+                    gbs = bicgstab_bytes_per_cell(its, args.operator) * N / (tm["krylov_ms"] * 1e-3) / 1e9 if its > 0 else None
+                    bi[label][f"{ratio:g}x"] = {"iterations": its, "operator_applications": 2 * its, "final_residual": res, "ms": ms,
+                                                "ms_per_iteration": tm["krylov_ms"] / max(its, 1), "krylov_hbm_frac": (gbs / peak_gbs) if gbs else None,
+                                                "T_implicit_over_T_explicit": ms / ms_exp, "over_K": ms / ms_exp / ratio,
+                                                "implicit_wins": bool(ms / ms_exp < ratio)}
+            wins = [f"{lab}:{k}" for lab, d in bi.items() for k, v in d.items() if v["implicit_wins"]]
+            bi["break_even_reached_at"] = wins
+            line_extra["bicgstab"] = bi
+            g.set_option("krylov", 0)
         # ---- stage 2 (row a8, BASELINE.json configs[4]): matter coupling + point source + velocity sources at 2048^2 ----------
         if not args.no_sweep and not args.no_stage2:
             w5 = wl.stratified_coupled(2048, seed=4321)

@@ -128,9 +128,10 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double f2raw = fx * fx + fy * fy;
     // |f| and the clamp of PAPER.md:513, branch-free: one rsqrt serves both (f = f2 rsqrt(f2); rescale by rsqrt(f2) if f2 > 1)
     const bool tiny = !(f2raw > 1e-290);
-    const double rf = rsqrt_fast(tiny ? 1.0 : f2raw);
+    const bool huge = !(f2raw <= 1e300);          // E <= 0 (floored): F/(cE) overflows; 1/sqrt(inf) = 0 like IEEE
+    const double rf = rsqrt_fast((tiny || huge) ? 1.0 : f2raw);
     const bool clamp = f2raw > 1.0;
-    const double sc = clamp ? rf : 1.0;
+    const double sc = clamp ? (huge ? 0.0 : rf) : 1.0;
     fx *= sc; fy *= sc;
     const double f2 = clamp ? 1.0 : f2raw;
     q.f = clamp ? 1.0 : (tiny ? 0.0 : f2raw * rf);

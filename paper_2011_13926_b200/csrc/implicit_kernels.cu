@@ -54,7 +54,7 @@ __device__ __forceinline__ void inv3(const Blk& B, Blk& I)
     const double* a = B.a;
     const double c00 = a[4] * a[8] - a[5] * a[7], c01 = a[5] * a[6] - a[3] * a[8], c02 = a[3] * a[7] - a[4] * a[6];
     const double det = a[0] * c00 + a[1] * c01 + a[2] * c02;
-    const double id = 1.0 / det;
+    const double id = rcp_fast(det);
     I.a[0] = c00 * id; I.a[1] = (a[2] * a[7] - a[1] * a[8]) * id; I.a[2] = (a[1] * a[5] - a[2] * a[4]) * id;
     I.a[3] = c01 * id; I.a[4] = (a[0] * a[8] - a[2] * a[6]) * id; I.a[5] = (a[2] * a[3] - a[0] * a[5]) * id;
     I.a[6] = c02 * id; I.a[7] = (a[1] * a[6] - a[0] * a[7]) * id; I.a[8] = (a[0] * a[4] - a[1] * a[3]) * id;
@@ -75,12 +75,12 @@ __global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields 
     fetch_cell(f, g, i, j - 1, u[3]);
     fetch_cell(f, g, i, j + 1, u[4]);
 #pragma unroll
-    for (int k = 0; k < 5; ++k) closure_eval<true, SD>(s, g.c, u[k].E, u[k].Fx, u[k].Fy, q[k], &J[k]);
+    for (int k = 0; k < 5; ++k) closure_eval<true, SD, true>(s, g.c, u[k].E, u[k].Fx, u[k].Fy, q[k], &J[k]);
     Face fw, fe, fs, fn;
-    face_eval<SD>(s, g.c, g.dx, q[1].lmin[0], q[1].lmax[0], q[1].f, u[1].st, q[0].lmin[0], q[0].lmax[0], q[0].f, u[0].st, fw);
-    face_eval<SD>(s, g.c, g.dx, q[0].lmin[0], q[0].lmax[0], q[0].f, u[0].st, q[2].lmin[0], q[2].lmax[0], q[2].f, u[2].st, fe);
-    face_eval<SD>(s, g.c, g.dy, q[3].lmin[1], q[3].lmax[1], q[3].f, u[3].st, q[0].lmin[1], q[0].lmax[1], q[0].f, u[0].st, fs);
-    face_eval<SD>(s, g.c, g.dy, q[0].lmin[1], q[0].lmax[1], q[0].f, u[0].st, q[4].lmin[1], q[4].lmax[1], q[4].f, u[4].st, fn);
+    face_eval<SD, true>(s, g.c, g.dx, q[1].lmin[0], q[1].lmax[0], q[1].f, u[1].st, q[0].lmin[0], q[0].lmax[0], q[0].f, u[0].st, fw);
+    face_eval<SD, true>(s, g.c, g.dx, q[0].lmin[0], q[0].lmax[0], q[0].f, u[0].st, q[2].lmin[0], q[2].lmax[0], q[2].f, u[2].st, fe);
+    face_eval<SD, true>(s, g.c, g.dy, q[3].lmin[1], q[3].lmax[1], q[3].f, u[3].st, q[0].lmin[1], q[0].lmax[1], q[0].f, u[0].st, fs);
+    face_eval<SD, true>(s, g.c, g.dy, q[0].lmin[1], q[0].lmax[1], q[0].f, u[0].st, q[4].lmin[1], q[4].lmax[1], q[4].f, u[4].st, fn);
 
     const double c = g.c, c2 = c * c, rx = dt / g.dx, ry = dt / g.dy;
     Blk B[5];

@@ -99,31 +99,37 @@ __device__ __forceinline__ double rsqrt_fast(double x)
 // sqrt(x) for x >= 0; exactly 0 for x below 1e-290 (the seed flushes subnormals)
 __device__ __forceinline__ double sqrt_fast(double x) { return (x > 1e-290) ? x * rsqrt_fast(x) : 0.0; }
 
+// IEEE or fast (<= 1 ulp) reciprocal / square root, selected at compile time (FAST is used by the assembly kernel).
+template <bool FAST> __device__ __forceinline__ double rcp_sel(double x) { return FAST ? rcp_fast(x) : 1.0 / x; }
+template <bool FAST> __device__ __forceinline__ double sqrt_sel(double x) { return FAST ? sqrt_fast(x) : sqrt(x); }
+template <bool FAST> __device__ __forceinline__ double rsqrt_sel(double x) { return FAST ? rsqrt_fast(x) : 1.0 / sqrt(x); }
+
 // PAPER.md:79, 170, 513.  SCHEME_DEFAULT folds the scheme switches at compile time.
-template <bool WITH_JAC, bool SCHEME_DEFAULT>
+template <bool WITH_JAC, bool SCHEME_DEFAULT, bool FAST = false>
 __device__ __forceinline__ void closure_eval(const Scheme& s, double c, double E, double Fx, double Fy, Clo& q, Jac* J)
 {
     const double Es = (E > ARK_E_FLOOR) ? E : ARK_E_FLOOR;
-    const double ice = 1.0 / (c * Es);
+    const double ice = rcp_sel<FAST>(c * Es);
     double fx = Fx * ice, fy = Fy * ice;
     double f2 = fx * fx + fy * fy;
     const bool clamped = f2 > 1.0;
     if (clamped) {
-        const double r = 1.0 / sqrt(f2);
+        // f2 = inf happens when E <= 0 (floored to 1e-300): 1/sqrt(inf) = 0 like the IEEE sequence, not NaN
+        const double r = (FAST && !(f2 <= 1e300)) ? 0.0 : rsqrt_sel<FAST>(f2);
         fx *= r; fy *= r; f2 = 1.0;
     }
     const bool p1 = !SCHEME_DEFAULT && s.closure == 1;
     double xi, chi, q3;  // q3 = 3/(2+xi): (3chi-1)/2 n_a n_b = q3 f_a f_b
     if (p1) { xi = 2.0; chi = 1.0 / 3.0; q3 = 0.0; }
     else {
-        xi = sqrt(4.0 - 3.0 * f2);
-        chi = (3.0 + 4.0 * f2) / (5.0 + 2.0 * xi);
-        q3 = 3.0 / (2.0 + xi);
+        xi = sqrt_sel<FAST>(4.0 - 3.0 * f2);
+        chi = (3.0 + 4.0 * f2) * rcp_sel<FAST>(5.0 + 2.0 * xi);
+        q3 = 3.0 * rcp_sel<FAST>(2.0 + xi);
     }
     const double iso = 0.5 * (1.0 - chi);
     const double Dxx = iso + q3 * fx * fx, Dxy = q3 * fx * fy, Dyy = iso + q3 * fy * fy;
     q.Pxx = Dxx * E; q.Pxy = Dxy * E; q.Pyy = Dyy * E;
-    q.f = sqrt(f2);
+    q.f = sqrt_sel<FAST>(f2);
 
     const int eig = SCHEME_DEFAULT ? 0 : s.eig;
     if (eig == 1) { q.lmax[0] = q.lmax[1] = c; q.lmin[0] = q.lmin[1] = -c; }
@@ -132,10 +138,10 @@ __device__ __forceinline__ void closure_eval(const Scheme& s, double c, double E
         q.lmax[0] = q.lmax[1] = l; q.lmin[0] = q.lmin[1] = -l;
     } else {  // Eq. 14: normal component f_n, tangential f_t
         const double a = (xi - 1.0) * (xi + 2.0);
-        const double ixi = 1.0 / xi;
-        const double k = 0.81649658092772603273 * ixi / (xi + 2.0);  // sqrt(2/3)/(xi (xi+2))
-        const double rx = k * sqrt(a * (2.0 * a + 3.0 * fy * fy));
-        const double ry = k * sqrt(a * (2.0 * a + 3.0 * fx * fx));
+        const double ixi = rcp_sel<FAST>(xi);
+        const double k = 0.81649658092772603273 * ixi * rcp_sel<FAST>(xi + 2.0);  // sqrt(2/3)/(xi (xi+2))
+        const double rx = k * sqrt_sel<FAST>(a * (2.0 * a + 3.0 * fy * fy));
+        const double ry = k * sqrt_sel<FAST>(a * (2.0 * a + 3.0 * fx * fx));
         const double mx = fx * ixi, my = fy * ixi;
         q.lmax[0] = c * (mx + rx); q.lmin[0] = c * (mx - rx);
         q.lmax[1] = c * (my + ry); q.lmin[1] = c * (my - ry);
@@ -149,13 +155,13 @@ __device__ __forceinline__ void closure_eval(const Scheme& s, double c, double E
             J->yy[0] = Dyy; J->yy[1] = 0.0; J->yy[2] = 0.0;
         } else if (clamped) {
             // clamped closure P = E n(x)n, n = F/|F|: dP_ab/dE = n_a n_b, dP_ab/dF_k = (E/|F|)(d_ak n_b + d_bk n_a - 2 n_a n_b n_k)
-            const double g = E / sqrt(Fx * Fx + Fy * Fy);
+            const double g = E * rsqrt_sel<FAST>(Fx * Fx + Fy * Fy);
             const double nx = fx, ny = fy;  // unit vector after the clamp
             J->xx[0] = nx * nx; J->xx[1] = g * (2.0 * nx - 2.0 * nx * nx * nx); J->xx[2] = g * (-2.0 * nx * nx * ny);
             J->xy[0] = nx * ny; J->xy[1] = g * (ny - 2.0 * nx * ny * nx);       J->xy[2] = g * (nx - 2.0 * nx * ny * ny);
             J->yy[0] = ny * ny; J->yy[1] = g * (-2.0 * ny * ny * nx);           J->yy[2] = g * (2.0 * ny - 2.0 * ny * ny * ny);
         } else {
-            const double ixi = 1.0 / xi, ic = 1.0 / c;
+            const double ixi = rcp_sel<FAST>(xi), ic = rcp_sel<FAST>(c);
             // (3/xi - 2 q)/f^2 with 2 - xi = 3 f^2/(2 + xi)  ==>  q^2/xi: no division by f^2, no cancellation
             const double t3 = q3 * q3 * ixi;                  // multiplies f_a f_b f_k
             // d/dE
@@ -176,7 +182,7 @@ __device__ __forceinline__ void closure_eval(const Scheme& s, double c, double E
 // Face coefficients a+ = l+/(l+ - l-), a- = -l-/(l+ - l-), Lambda = l+ l-/(l+ - l-), alpha (Eq. 25), sigma_f (Eq. 19).
 struct Face { double ap, am, Lam, alpha, sig; };
 
-template <bool SCHEME_DEFAULT>
+template <bool SCHEME_DEFAULT, bool FAST = false>
 __device__ __forceinline__ void face_eval(const Scheme& s, double c, double delta,
                                           double lminL, double lmaxL, double fL, double stL,
                                           double lminR, double lmaxR, double fR, double stR, Face& fc)
@@ -186,7 +192,7 @@ __device__ __forceinline__ void face_eval(const Scheme& s, double c, double delt
     const double lm = fmin(-fl, fmin(lminL, lminR));
     const double dl = lp - lm;
     if (dl > 0.0) {
-        const double idl = 1.0 / dl;
+        const double idl = rcp_sel<FAST>(dl);
         fc.ap = lp * idl; fc.am = -lm * idl; fc.Lam = lp * lm * idl;
     } else { fc.ap = 0.5; fc.am = 0.5; fc.Lam = 0.0; }  // l+ = l- = 0 (f = 1 tangential to the face)
     fc.sig = 0.5 * (stL + stR);
@@ -195,7 +201,7 @@ __device__ __forceinline__ void face_eval(const Scheme& s, double c, double delt
     if (ap == 0) fc.alpha = 1.0;
     else {
         const double w = (ap == 2) ? 1.0 : (1.0 - ff * ff);
-        fc.alpha = 1.0 / (1.0 - 3.0 * fc.sig * delta * w * fc.Lam / c);
+        fc.alpha = FAST ? rcp_fast(1.0 - 3.0 * fc.sig * delta * w * fc.Lam * rcp_fast(c)) : 1.0 / (1.0 - 3.0 * fc.sig * delta * w * fc.Lam / c);
     }
 }
 

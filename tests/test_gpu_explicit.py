@@ -162,3 +162,21 @@ def test_device_and_host_pointers_give_the_same_result():
     g2.get_state(out=(E2, F2))
     E1, F1 = g1.get_state()
     assert np.array_equal(E1, E2.cpu().numpy()) and np.array_equal(F1, F2.cpu().numpy())
+
+
+def test_nonpositive_energy_cells_do_not_poison_the_step():
+    # E <= 0 (positivity is not guaranteed): E is floored in the division only, F/(cE) overflows and the
+    # clamp must give the same finite result as the oracle's IEEE sequence (1/sqrt(inf) = 0), in every kernel
+    w = small_random_state(40, 28, seed=19)
+    w["E"][7, 9] = -0.3
+    w["E"][20, 3] = 0.0
+    for kernel in (0, 1, 2):
+        o, g = make_oracle(w), make_gpu(w, dict(explicit_kernel=kernel))
+        o.step_explicit(1e-3)
+        g.step_explicit(1e-3)
+        Eg, Fg = g.get_state()
+        assert np.all(np.isfinite(Eg)) and np.all(np.isfinite(Fg))
+        assert state_rel_l2((Eg, Fg), o.get_state()) <= TOL_EXPLICIT
+    o, g = make_oracle(w), make_gpu(w)
+    V = np.random.default_rng(2).standard_normal((3, 28, 40))
+    assert rel_l2(g.apply_operator(0.02, V), o.apply_linear(0.02, V)) <= 1e-12
