@@ -60,22 +60,64 @@ __device__ __forceinline__ void inv3(const Blk& B, Blk& I)
     I.a[6] = c02 * id; I.a[7] = (a[1] * a[6] - a[0] * a[7]) * id; I.a[8] = (a[0] * a[4] - a[1] * a[3]) * id;
 }
 
+// Tile assembly: a block owns ATX x ATY cells.  Phase 1 evaluates closure + pressure Jacobian ONCE per cell of the tile and
+// of its one-cell halo (corners excluded) into shared memory; phase 2 builds the five blocks of each cell from the five
+// shared entries.  (The first version evaluated five closures per cell: 3.5 ms at 4096^2; fast reciprocals: 2.4 ms.)
+#ifndef ARK_ASM_TY
+#define ARK_ASM_TY 4
+#endif
+static constexpr int ATX = 32, ATY = ARK_ASM_TY, AW = ATX + 2, AH = ATY + 2, ACELLS = AW * AH;
+enum { TC_E = 0, TC_FX, TC_FY, TC_SA, TC_ST, TC_F, TC_LMINX, TC_LMAXX, TC_LMINY, TC_LMAXY, TC_J0, TC_FIELDS = TC_J0 + 9 };
+
 template <bool SD>
-__global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields f, double dt, BlockMatrix A, MfPlanes mf,
-                                                       const double* __restrict__ bsrc)
+__global__ void __launch_bounds__(ATX * ATY) assemble_kernel(Grid g, Scheme s, Fields f, double dt, BlockMatrix A, MfPlanes mf,
+                                                             const double* __restrict__ bsrc)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    extern __shared__ double tile[];                 // [TC_FIELDS][ACELLS] doubles, then ACELLS long long cell indices
+    long long* tidx = reinterpret_cast<long long*>(tile + TC_FIELDS * ACELLS);
+    const int i0 = blockIdx.x * ATX, j0 = blockIdx.y * ATY;
+    const int tid = threadIdx.y * ATX + threadIdx.x;
+    for (int cidx = tid; cidx < ACELLS; cidx += ATX * ATY) {
+        const int cx = cidx % AW, cy = cidx / AW;
+        const bool corner = (cx == 0 || cx == AW - 1) && (cy == 0 || cy == AH - 1);
+        const int ci = i0 - 1 + cx, cj = j0 - 1 + cy;
+        if (corner || ci > g.nx || cj > g.ny) continue;
+        if ((ci < 0 || ci >= g.nx) && (cj < 0 || cj >= g.ny)) continue;      // domain corner ghosts are never used
+        CellU u; Clo q; Jac J;
+        fetch_cell(f, g, ci, cj, u);
+        closure_eval<true, SD, true>(s, g.c, u.E, u.Fx, u.Fy, q, &J);
+        tile[TC_E * ACELLS + cidx] = u.E; tile[TC_FX * ACELLS + cidx] = u.Fx; tile[TC_FY * ACELLS + cidx] = u.Fy;
+        tile[TC_SA * ACELLS + cidx] = u.sa; tile[TC_ST * ACELLS + cidx] = u.st; tile[TC_F * ACELLS + cidx] = q.f;
+        tile[TC_LMINX * ACELLS + cidx] = q.lmin[0]; tile[TC_LMAXX * ACELLS + cidx] = q.lmax[0];
+        tile[TC_LMINY * ACELLS + cidx] = q.lmin[1]; tile[TC_LMAXY * ACELLS + cidx] = q.lmax[1];
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            tile[(TC_J0 + e) * ACELLS + cidx] = J.xx[e]; tile[(TC_J0 + 3 + e) * ACELLS + cidx] = J.xy[e]; tile[(TC_J0 + 6 + e) * ACELLS + cidx] = J.yy[e];
+        }
+        tidx[cidx] = u.idx;
+    }
+    __syncthreads();
+    const int i = i0 + threadIdx.x, j = j0 + threadIdx.y;
     if (i >= g.nx || j >= g.ny) return;
     const long long N = (long long)g.nx * g.ny, id = (long long)j * g.nx + i;
     CellU u[5]; Clo q[5]; Jac J[5];   // centre, west, east, south, north
-    fetch_cell(f, g, i, j, u[0]);
-    fetch_cell(f, g, i - 1, j, u[1]);
-    fetch_cell(f, g, i + 1, j, u[2]);
-    fetch_cell(f, g, i, j - 1, u[3]);
-    fetch_cell(f, g, i, j + 1, u[4]);
+    {
+        const int cc = (threadIdx.y + 1) * AW + threadIdx.x + 1;
+        const int where[5] = { cc, cc - 1, cc + 1, cc - AW, cc + AW };
 #pragma unroll
-    for (int k = 0; k < 5; ++k) closure_eval<true, SD, true>(s, g.c, u[k].E, u[k].Fx, u[k].Fy, q[k], &J[k]);
+        for (int k = 0; k < 5; ++k) {
+            const int w = where[k];
+            u[k].E = tile[TC_E * ACELLS + w]; u[k].Fx = tile[TC_FX * ACELLS + w]; u[k].Fy = tile[TC_FY * ACELLS + w];
+            u[k].sa = tile[TC_SA * ACELLS + w]; u[k].st = tile[TC_ST * ACELLS + w]; u[k].idx = tidx[w];
+            q[k].f = tile[TC_F * ACELLS + w];
+            q[k].lmin[0] = tile[TC_LMINX * ACELLS + w]; q[k].lmax[0] = tile[TC_LMAXX * ACELLS + w];
+            q[k].lmin[1] = tile[TC_LMINY * ACELLS + w]; q[k].lmax[1] = tile[TC_LMAXY * ACELLS + w];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) {
+                J[k].xx[e] = tile[(TC_J0 + e) * ACELLS + w]; J[k].xy[e] = tile[(TC_J0 + 3 + e) * ACELLS + w]; J[k].yy[e] = tile[(TC_J0 + 6 + e) * ACELLS + w];
+            }
+        }
+    }
     Face fw, fe, fs, fn;
     face_eval<SD, true>(s, g.c, g.dx, q[1].lmin[0], q[1].lmax[0], q[1].f, u[1].st, q[0].lmin[0], q[0].lmax[0], q[0].f, u[0].st, fw);
     face_eval<SD, true>(s, g.c, g.dx, q[0].lmin[0], q[0].lmax[0], q[0].f, u[0].st, q[2].lmin[0], q[2].lmax[0], q[2].f, u[2].st, fe);
@@ -155,9 +197,16 @@ __global__ void __launch_bounds__(128) assemble_kernel(Grid g, Scheme s, Fields 
 cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf,
                             const double* bsrc, cudaStream_t st)
 {
-    dim3 blk(32, 4), grd((g.nx + 31) / 32, (g.ny + 3) / 4);
-    if (s.is_default()) assemble_kernel<true><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf, bsrc);
-    else assemble_kernel<false><<<grd, blk, 0, st>>>(g, s, f, dt, A, mf, bsrc);
+    dim3 blk(ATX, ATY), grd((g.nx + ATX - 1) / ATX, (g.ny + ATY - 1) / ATY);
+    const size_t smem = (size_t)ACELLS * (TC_FIELDS * sizeof(double) + sizeof(long long));
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncSetAttribute(assemble_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(assemble_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        attr_done = true;
+    }
+    if (s.is_default()) assemble_kernel<true><<<grd, blk, smem, st>>>(g, s, f, dt, A, mf, bsrc);
+    else assemble_kernel<false><<<grd, blk, smem, st>>>(g, s, f, dt, A, mf, bsrc);
     return cudaGetLastError();
 }
 
