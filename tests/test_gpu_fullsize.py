@@ -1,0 +1,43 @@
+"""GPU parity at BASELINE.json's full bench size (configs[3], 4096 x 4096), in the launch configuration bench.py times.
+
+Explicit: the oracle still finishes one step at this size in seconds, so every element is compared.  Implicit: the
+oracle's solve would take minutes; instead the CUDA solution is substituted into the ORACLE's flux-form operator (one
+application) and the oracle's residual of the linear system is checked — a property that holds at any size."""
+import numpy as np
+import pytest
+
+import m1_workloads as wl
+from helpers import make_oracle, make_gpu, rel_l2, state_rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def w4096():
+    return wl.random_medium(4096, seed=1234)
+
+
+def test_explicit_step_4096_every_element(w4096):
+    w = w4096
+    dt = wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    o, g = make_oracle(w), make_gpu(w)
+    o.step_explicit(dt)
+    g.step_explicit(dt)
+    assert state_rel_l2(g.get_state(), o.get_state()) <= 1e-11
+
+
+@pytest.mark.parametrize("krylov", [0, 1])
+def test_implicit_step_4096_satisfies_the_oracles_linear_system(w4096, krylov):
+    w = w4096
+    dt = 10.0 * wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    g = make_gpu(w, dict(krylov=krylov))
+    its, res = g.step_implicit(dt, 1e-10, 30, 4000)
+    assert res <= 1e-10 and 0 < its < 4000
+    E, F = g.get_state()
+    x = np.concatenate((E[None], F))
+    o = make_oracle(w)                                   # holds U^n: the coefficients of the linearisation
+    Ax = o.apply_linear(dt, x, mode=0)
+    b = np.concatenate((w["E"][None], w["F"]))           # periodic, no T: b = U^n
+    assert np.linalg.norm((b - Ax).ravel()) <= 2e-10 * np.linalg.norm(b.ravel())
+    # sampled cells: the implicit update is not the identity and not the explicit update
+    assert rel_l2(x, b) > 1e-3
