@@ -57,6 +57,24 @@ def opacity_jump(n=256, sig_lo=1.0, sig_hi=1e3, F0=0.1, E_out=100.0):
                 sigma_ghost=(sig_lo, sig_hi), F0=F0, E_out=E_out)
 
 
+def beam(n=128, angle_deg=45.0, E_beam=1.0, T_ratio=0.3):
+    """Beam test of the paper (Sect. 5.3): box [-1,1]^2, n x n cells, sigma = 0, background in equilibrium at
+    T0 = T_ratio * T_beam (E = T_ratio^4 E_beam, F = 0); a beam with f = 1 enters through x = -1, y in [-0.875, -0.75] at
+    `angle_deg`.  Boundaries: Dirichlet on x = -1 (beam / background ghosts), outflow elsewhere.  Units c = 1."""
+    dx = dy = 2.0 / n
+    y = -1.0 + (np.arange(n) + 0.5) * dy
+    E_bg = E_beam * T_ratio ** 4
+    E = np.full((n, n), E_bg)
+    F = np.zeros((2, n, n))
+    inb = (y >= -0.875) & (y <= -0.75)
+    th = np.deg2rad(angle_deg)
+    Eg = np.where(inb, E_beam, E_bg)
+    Fg = np.stack((np.where(inb, E_beam * np.cos(th), 0.0), np.where(inb, E_beam * np.sin(th), 0.0)))
+    zeros = np.zeros(n)
+    return dict(nx=n, ny=n, dx=dx, dy=dy, c=1.0, bc=(1, 2, 2, 2), E=E, F=F, sigma_a=np.zeros((n, n)), sigma_s=np.zeros((n, n)),
+                ghosts={0: (Eg, Fg, zeros, zeros)}, inflow_cells=int(inb.sum()), E_bg=E_bg)
+
+
 def _box5_periodic(a):
     out = np.zeros_like(a)
     for s in (-2, -1, 0, 1, 2):

@@ -180,3 +180,29 @@ def test_nonpositive_energy_cells_do_not_poison_the_step():
     o, g = make_oracle(w), make_gpu(w)
     V = np.random.default_rng(2).standard_normal((3, 28, 40))
     assert rel_l2(g.apply_operator(0.02, V), o.apply_linear(0.02, V)) <= 1e-12
+
+
+def test_beam_test_of_the_paper():
+    # PAPER.md:410-416 (Sect. 5.3): Dirichlet inflow + outflow boundaries, sigma = 0, both eigenvalue modes.
+    # (a) parity with the oracle after 300 steps, inflow at f = 0.999 (at f = 1 exactly Eq. 14 is ill-conditioned);
+    # (b) the CUDA path alone at f = 1: the beam is narrower with the eigenvalues of Eq. 14 than with +-c (paper: ~24 vs ~30).
+    w = wl.beam(128)
+    dt = _dt(w)
+    w2 = dict(w)
+    Eg, Fg, za, zs = w["ghosts"][0]
+    w2["ghosts"] = {0: (Eg, 0.999 * Fg, za, zs)}
+    for eig in (0, 1):
+        o, g = make_oracle(w2, dict(eig_mode=eig)), make_gpu(w2, dict(eig_mode=eig))
+        for _ in range(300):
+            o.step_explicit(dt)
+        g.steps_explicit(dt, 300)
+        assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+    width = {}
+    for eig in (0, 1):
+        g = make_gpu(w, dict(eig_mode=eig))
+        g.steps_explicit(dt, 1400)
+        E, F = g.get_state()
+        cut = E[64, :] - w["E_bg"]
+        width[eig] = int((cut > 0.5 * cut.max()).sum())
+        assert g.count_unrealizable() == (0, 0)
+    assert width[0] < width[1] and 0.7 <= width[0] / width[1] <= 0.9
