@@ -75,6 +75,18 @@ def beam(n=128, angle_deg=45.0, E_beam=1.0, T_ratio=0.3):
                 ghosts={0: (Eg, Fg, zeros, zeros)}, inflow_cells=int(inb.sum()), E_bg=E_bg)
 
 
+def marshak(nx=400, sigma=1e4, rho_cv=1.0, T0=0.3, T_left=1.0):
+    """Marshak wave of the paper (Sect. 5.1) in non-dimensional units (c = a_r = 1, unit length):
+    nx x 1 cells, sigma dx = 25, medium in equilibrium at T0 (E = T0^4, F = 0), a source at T_left lit at the left boundary
+    (Dirichlet ghost E = T_left^4, F = 0), zero-gradient on the right, frozen hydrodynamics, constant rho c_v."""
+    dx = 1.0 / nx
+    one = np.ones((1, nx))
+    return dict(nx=nx, ny=1, dx=dx, dy=1.0, c=1.0, bc=(1, 2, 0, 0), E=T0 ** 4 * one, F=np.zeros((2, 1, nx)), T=T0 * one,
+                sigma_a=sigma * one, sigma_s=0.0 * one, rho_cv=rho_cv * one,
+                ghosts={0: (np.array([T_left ** 4]), np.zeros((2, 1)), np.array([sigma]), np.array([0.0]))},
+                sigma=sigma, T0=T0, T_left=T_left, a_r=1.0)
+
+
 def _box5_periodic(a):
     out = np.zeros_like(a)
     for s in (-2, -1, 0, 1, 2):

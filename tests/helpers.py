@@ -62,3 +62,31 @@ def small_random_state(nx, ny, seed, fmax=0.9, dx=None, dy=None, c=1.0, bc=(0, 0
             ghosts[side] = (Eg, Fg, 10.0 ** rng.uniform(*sig_range, n), 10.0 ** rng.uniform(*sig_range, n))
     w["ghosts"] = ghosts
     return w
+
+
+def marshak_diffusion_reference(w, dt, nsteps):
+    """Reference of PAPER.md:383: "a standard discretization of Eq. 11", d/dt (a_r T^4 + rho c_v T) = d/dx ( c/(3 sigma) d/dx a_r T^4 ),
+    backward Euler with Newton to convergence on the same grid; ghost T = T_left left, zero gradient right.  Independent of
+    the oracle and of the CUDA path (numpy + a banded solve)."""
+    from scipy.linalg import solve_banded
+    nx, dx = w["nx"], w["dx"]
+    D = w["c"] / (3.0 * w["sigma"])
+    rcv = float(w["rho_cv"][0, 0])
+    T = np.full(nx, w["T0"])
+    for _ in range(nsteps):
+        e_old = T ** 4 + rcv * T
+        for _it in range(60):
+            U = T ** 4
+            Ug = np.concatenate(([w["T_left"] ** 4], U, [U[-1]]))
+            Fv = U + rcv * T - e_old - dt * D * (Ug[2:] - 2.0 * Ug[1:-1] + Ug[:-2]) / dx ** 2
+            dU = 4.0 * T ** 3
+            ab = np.zeros((3, nx))
+            ab[1] = dU + rcv + 2.0 * dt * D * dU / dx ** 2
+            ab[1, -1] -= dt * D * dU[-1] / dx ** 2
+            ab[0, 1:] = -dt * D * dU[1:] / dx ** 2
+            ab[2, :-1] = -dt * D * dU[:-1] / dx ** 2
+            d = solve_banded((1, 1), ab, -Fv)
+            T = T + d
+            if np.max(np.abs(d)) < 1e-13:
+                break
+    return T

@@ -94,3 +94,25 @@ def test_config5_stratified_coupled_window():
     o.add_velocity_sources(dt)
     g.add_velocity_sources(dt)
     assert state_rel_l2(g.get_state(with_T=True), o.get_state(with_T=True)) <= 1e-8
+
+
+def test_marshak_wave_on_the_gpu():
+    # the CUDA path itself against the independent discretisation of Eq. 11 (1.1 % bound of the paper) and
+    # against the oracle; 400 x 1 grid, Dirichlet source on the left, outflow on the right, matter coupling, BiCGStab.
+    from helpers import marshak_diffusion_reference
+    w = wl.marshak(400)
+    nsteps, dt = 300, 10.0
+    Tref = marshak_diffusion_reference(w, dt, nsteps)
+    o, g = make_oracle(w, dict(krylov=1)), make_gpu(w, dict(krylov=1))
+    for _ in range(nsteps):
+        o.step_implicit(dt, 1e-11, 30, 20000)
+        its, res = g.step_implicit(dt, 1e-11, 30, 20000)
+        assert res <= 1e-10
+    Eg, Fg, Tg = g.get_state(with_T=True)
+    assert rel_l2(Tg[0], Tref) <= 0.011
+    Eo, Fo, To = o.get_state(with_T=True)
+    assert rel_l2(Tg, To) <= 1e-7 and rel_l2(Eg, Eo) <= 1e-7
+    g0 = make_gpu(w, dict(krylov=1, ap_mode=0))
+    for _ in range(nsteps):
+        g0.step_implicit(dt, 1e-10, 30, 20000)
+    assert rel_l2(g0.get_state(with_T=True)[2][0], Tref) >= 0.5
