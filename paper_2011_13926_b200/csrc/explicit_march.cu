@@ -38,6 +38,20 @@ struct Raw { double E, Fx, Fy, st, sa; };
 // (interior row) costs one multiply-add and five loads.
 //   xmode 0: column ii of the grid (after periodic wrap / outflow clamp);  1: Dirichlet x-ghost of side xside;  2: inactive.
 // j may be -1 or ny (y ghost).  Corner ghosts are never used by a 5-point stencil and return a dummy state.
+#ifndef ARK_MARCH_PINLOAD
+#define ARK_MARCH_PINLOAD 0     // 1: the hot-path loads are volatile asm, so that ptxas cannot sink the prefetch
+#endif
+__device__ __forceinline__ double ld_pinned(const double* p)
+{
+#if ARK_MARCH_PINLOAD
+    double x;
+    asm volatile("ld.global.f64 %0, [%1];" : "=d"(x) : "l"(p) : "memory");
+    return x;
+#else
+    return *p;
+#endif
+}
+
 __device__ __forceinline__ Raw load_row(const Fields& f, const Grid& g, int xmode, int ii, int xside, int j)
 {
     Raw r; r.E = 1.0; r.Fx = 0.0; r.Fy = 0.0; r.st = 0.0; r.sa = 0.0;
@@ -45,7 +59,7 @@ __device__ __forceinline__ Raw load_row(const Fields& f, const Grid& g, int xmod
     if (j >= 0 && j < g.ny) {
         if (xmode == 0) {
             const unsigned int id = (unsigned int)j * (unsigned int)g.nx + (unsigned int)ii;
-            r.E = f.E[id]; r.Fx = f.Fx[id]; r.Fy = f.Fy[id]; r.st = f.st[id]; r.sa = f.sa[id];
+            r.E = ld_pinned(f.E + id); r.Fx = ld_pinned(f.Fx + id); r.Fy = ld_pinned(f.Fy + id); r.st = ld_pinned(f.st + id); r.sa = ld_pinned(f.sa + id);
         } else {
             r.E = f.gh[xside][0][j]; r.Fx = f.gh[xside][1][j]; r.Fy = f.gh[xside][2][j]; r.sa = f.gh[xside][3][j]; r.st = f.gh[xside][4][j];
         }
