@@ -206,3 +206,24 @@ def test_beam_test_of_the_paper():
         width[eig] = int((cut > 0.5 * cut.max()).sum())
         assert g.count_unrealizable() == (0, 0)
     assert width[0] < width[1] and 0.7 <= width[0] / width[1] <= 0.9
+
+
+def test_side_stream_and_two_handles():
+    # the handle enqueues on the stream it was given (torch side stream here); two handles are independent
+    import torch
+    import paper_2011_13926_b200 as ark
+    w = small_random_state(96, 64, seed=23)
+    ref = make_gpu(w)
+    ref.steps_explicit(1e-3, 3)
+    ref.step_implicit(0.05, 1e-10, 30, 500)
+    want = ref.get_state()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        dev = {k: torch.from_numpy(np.ascontiguousarray(w[k])).cuda() for k in ("E", "F", "sigma_a", "sigma_s")}
+        g = ark.ArkM1(w["nx"], w["ny"], w["dx"], w["dy"], w["c"], bc=w["bc"], stream=side)
+        g.set_state(dev["E"], dev["F"], dev["sigma_a"], dev["sigma_s"])
+        g.steps_explicit(1e-3, 3)
+        g.step_implicit(0.05, 1e-10, 30, 500)
+        got = g.get_state()
+    assert all(np.array_equal(a, b) for a, b in zip(got, want))
+    assert g.kernel_launches() == ref.kernel_launches() and g.device_bytes() == ref.device_bytes() > 0
