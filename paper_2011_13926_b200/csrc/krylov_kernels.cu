@@ -182,11 +182,11 @@ __global__ void __launch_bounds__(KTHREADS) update_kernel(double* __restrict__ w
     double2* w2 = reinterpret_cast<double2*>(w);
     for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
         double2 a = w2[e];
+        double2 b[NV];
 #pragma unroll
-        for (int k = 0; k < NV; ++k) {
-            const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
-            a.x -= cf[k] * b.x; a.y -= cf[k] * b.y;
-        }
+        for (int k = 0; k < NV; ++k) b[k] = reinterpret_cast<const double2*>(V0 + k * stride)[e];
+#pragma unroll
+        for (int k = 0; k < NV; ++k) { a.x = fma(-cf[k], b[k].x, a.x); a.y = fma(-cf[k], b[k].y, a.y); }
         w2[e] = a;
         if (WITH_NORM) acc[0] += a.x * a.x + a.y * a.y;
     }
