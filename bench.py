@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — throughput of the M1 radiative-transfer hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 4096] [--no-sweep]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--grid 4096] [--no-sweep]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 Workload (BASELINE.json configs[3]): the seeded random medium of m1_workloads.random_medium at 4096 x 4096
@@ -206,9 +206,17 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device — the CUDA library is the only implementation (no CPU fallback)")
+    # ARK_BENCH_SHARE_GPU=1 (test only): all ranks use cuda:0 and rendezvous over gloo, to exercise the N > 1 code path on a
+    # one-GPU box; the replicas never wait on one another on the device (no data-path collective)
+    share = os.environ.get("ARK_BENCH_SHARE_GPU") == "1"
+    if share:
+        local = 0
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if share:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
     peak_gbs, peak_src = peaks()
 
@@ -457,7 +465,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--n", type=int, default=4096, help="grid size (BASELINE.json configs[3]: 4096)")
+    ap.add_argument("--grid", "--n", dest="n", type=int, default=4096, help="grid size (BASELINE.json configs[3]: 4096); use --grid under torchrun (--n is ambiguous there)")
     ap.add_argument("--seed", type=int, default=1234)
     ap.add_argument("--operator", type=int, default=1, choices=[0, 1],
                     help="implicit operator: 0 = pre-multiplied block stencil, 1 = matrix-free coefficient planes (default, DESIGN.md)")
