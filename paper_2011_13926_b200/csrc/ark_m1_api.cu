@@ -236,7 +236,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "eig_floor")) { if (!(value >= 0.0)) return fail(h, ARK_M1_E_ARG, "eig_floor must be >= 0%s", ""); h->s.eig_floor = value; }
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
-    else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1 or 2%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 3) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1, 2 or 3%s", ""); h->explicit_kernel = iv; }
     else if (!strcmp(key, "krylov")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "krylov must be 0 (GMRES) or 1 (BiCGStab)%s", ""); h->krylov = iv; }
     else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 32]%s", ""); h->maxv = iv; }
     else if (!strcmp(key, "basis_pad")) { if (iv < 0 || (iv & 31)) return fail(h, ARK_M1_E_ARG, "basis_pad must be a non-negative multiple of 32 doubles%s", ""); if (iv != h->basis_pad) { cudaStreamSynchronize(h->st); free_implicit(h); } h->basis_pad = iv; }
@@ -277,7 +277,9 @@ static int explicit_once(ark_m1* h, double dt)
     const Fields f = fields_of(h);
     double* O = h->U[h->cur ^ 1];
     const bool plain = !h->have_T && !h->source_E;
-    if (h->explicit_kernel == 2 && plain && h->N < (1LL << 31)) {
+    if (h->explicit_kernel == 3 && plain && h->N < (1LL << 31)) {
+        KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
+    } else if (h->explicit_kernel == 2 && plain && h->N < (1LL << 31)) {
         KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_warp(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
     } else if (h->explicit_kernel == 1 && plain && h->N < (1LL << 31)) {   // the march kernels use 32-bit in-plane offsets
         KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));

@@ -18,7 +18,7 @@ def _dt(w):
     return wl.explicit_dt(w["dx"], w["dy"], w["c"])
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
 @pytest.mark.parametrize("bc", BCS)
 def test_explicit_step_small_all_boundaries(bc, kernel):
     # 37 x 29: ragged in both directions, dx != dy, c != 1
@@ -31,7 +31,7 @@ def test_explicit_step_small_all_boundaries(bc, kernel):
     assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
 @pytest.mark.parametrize("shape", [(300, 70), (127, 5), (126, 64), (1, 40), (40, 1), (2, 2), (253, 131)])
 def test_explicit_step_ragged_shapes(shape, kernel):
     # several 126-column strips plus a ragged tail; degenerate one-cell-wide grids
@@ -67,7 +67,7 @@ def test_clamped_and_degenerate_cells():
     o, g = make_oracle(w), make_gpu(w)
     assert o.count_unrealizable() == g.count_unrealizable()
     assert o.count_unrealizable()[1] > 0
-    for kernel in (0, 1, 2):
+    for kernel in (0, 1, 2, 3):
         o, g = make_oracle(w), make_gpu(w, dict(explicit_kernel=kernel))
         o.step_explicit(1e-3)
         g.step_explicit(1e-3)
@@ -76,7 +76,7 @@ def test_clamped_and_degenerate_cells():
 
 @pytest.mark.parametrize("opts", [dict(well_balanced=0), dict(ap_mode=0), dict(ap_mode=2), dict(eig_mode=1), dict(eig_mode=2),
                                   dict(closure=1), dict(eig_floor=0.1)])
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
 def test_scheme_switches(opts, kernel):
     w = small_random_state(45, 31, seed=13, bc=(1, 1, 0, 0), sig_range=(-1.0, 1.0))
     o, g = make_oracle(w, opts), make_gpu(w, dict(opts, explicit_kernel=kernel))
@@ -170,7 +170,7 @@ def test_nonpositive_energy_cells_do_not_poison_the_step():
     w = small_random_state(40, 28, seed=19)
     w["E"][7, 9] = -0.3
     w["E"][20, 3] = 0.0
-    for kernel in (0, 1, 2):
+    for kernel in (0, 1, 2, 3):
         o, g = make_oracle(w), make_gpu(w, dict(explicit_kernel=kernel))
         o.step_explicit(1e-3)
         g.step_explicit(1e-3)
