@@ -360,7 +360,7 @@ def run_ours(args):
             g.set_option("krylov", 1)
             bi = {"rough_medium": {}, "smooth_problem": {}}
             for label, tensors, ratios in (("rough_medium", devt, (10.0, 50.0, 100.0, 200.0)),
-                                           ("smooth_problem", None, (50.0, 100.0, 200.0, 1000.0, 2000.0))):
+                                           ("smooth_problem", None, (50.0, 100.0, 200.0, 300.0, 500.0, 1000.0, 2000.0))):
                 if tensors is None:
                     ws = wl.gaussian_diffusion(n)
                     tensors = {k: torch.from_numpy(np.ascontiguousarray(ws[k])).to(dev) for k in ("E", "F", "sigma_a", "sigma_s")}
