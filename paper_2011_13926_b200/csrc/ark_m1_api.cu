@@ -393,7 +393,7 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
     if (h->wblock) { cudaFree(h->wblock); h->wblock = nullptr; }
     const int caphist = mi + mi / (mm > 0 ? mm : 1) + 8;
     const size_t nd = (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 2 * (size_t)(mm + 1) + caphist
-                      + (size_t)krylov_max_blocks(h->sm_count) * MAXV;
+                      + (size_t)(krylov_max_blocks(h->sm_count) > op_mf_blocks(h->g, h->sm_count) ? krylov_max_blocks(h->sm_count) : op_mf_blocks(h->g, h->sm_count)) * MAXV;
     const size_t ctl_bytes = (sizeof(GmresCtl) + 255) / 256 * 256;
     if (cudaMalloc(&h->wblock, ctl_bytes + nd * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(h, ARK_M1_E_ALLOC, "cudaMalloc (solver scalars)%s", ""); }
     CU(cudaMemset(h->wblock, 0, ctl_bytes + nd * sizeof(double)));
@@ -517,11 +517,17 @@ static int bicgstab_solve(ark_m1* h, double tol, int maxit)
         for (;;) {
             for (int k = 0; k < 8; ++k) {
                 KL(KC_UPDATE, 96.0 * h->N, launch_bicg_p(r, p, v, n, W, h->st));
-                if ((rc = op_apply_hat(h, p, v, stop))) return rc;
-                KL(KC_DOT, 48.0 * h->N, launch_multi_dot(v, rh, S, 1, 0, n, W, BICG_ALPHA, sm, h->st));
-                KL(KC_UPDATE, 72.0 * h->N, launch_bicg_s(r, v, n, W, h->st));
-                if ((rc = op_apply_hat(h, r, t, stop))) return rc;
-                KL(KC_DOT, 72.0 * h->N, launch_multi_dot(t, r, S, 2, 0, n, W, BICG_OMEGA, sm, h->st));
+                if (h->op_kind == 1) {   // matrix-free operator with the reductions fused in
+                    KL(KC_SPMV, 288.0 * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, p, v, stop, 1, rh, W, sm, h->st));
+                    KL(KC_UPDATE, 72.0 * h->N, launch_bicg_s(r, v, n, W, h->st));
+                    KL(KC_SPMV, 264.0 * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, r, t, stop, 2, nullptr, W, sm, h->st));
+                } else {
+                    if ((rc = op_apply_hat(h, p, v, stop))) return rc;
+                    KL(KC_DOT, 48.0 * h->N, launch_multi_dot(v, rh, S, 1, 0, n, W, BICG_ALPHA, sm, h->st));
+                    KL(KC_UPDATE, 72.0 * h->N, launch_bicg_s(r, v, n, W, h->st));
+                    if ((rc = op_apply_hat(h, r, t, stop))) return rc;
+                    KL(KC_DOT, 72.0 * h->N, launch_multi_dot(t, r, S, 2, 0, n, W, BICG_OMEGA, sm, h->st));
+                }
                 KL(KC_UPDATE, 168.0 * h->N, launch_bicg_xr(y, p, r, t, rh, n, W, sm, h->st));
             }
             if ((rc = fetch_ctl(h))) return rc;

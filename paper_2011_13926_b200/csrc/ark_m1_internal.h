@@ -97,6 +97,9 @@ cudaError_t launch_diag_mul(const Grid& g, const double* Cblk, const double* x, 
 // out = sgn*(s*(v + sum_k Ahat_k v_nbr)) + (add ? add : 0);  s = *scale_ptr[scale_idx] if scale_ptr else 1
 cudaError_t launch_spmv_hat(const Grid& g, const double* off, const double* v, double* out, const double* scale_ptr,
                             const double* add, double sgn, const int* skip_flag, cudaStream_t st);
+int op_mf_blocks(const Grid& g, int sm_count);      // grid size of the matrix-free operator (sizes the partial-sum buffer)
+cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
+                             const int* skip_flag, int dot, const double* aux, GmresWork W, int sm_count, cudaStream_t st);
 cudaError_t launch_matter_update(const Grid& g, const Scheme& s, double dt, const double* sa, const double* rho_cv,
                                  const double* Enew, double* T, cudaStream_t st);
 

@@ -10,139 +10,11 @@
 //    (ticket counter), whose thread 0 then runs the scalar epilogue (Hessenberg column, Givens rotations,
 //    residual estimate, stop flag) on the device.  A whole restart cycle is enqueued without host round trips;
 //    kernels of a cycle that has already met its stop criterion return immediately (ctl->inner_stop).
-#include "ark_m1_internal.h"
+#include "krylov_device.cuh"
 
 namespace ark {
 
-static constexpr int KTHREADS = 256;
-
 int krylov_max_blocks(int sm_count) { return sm_count * 4; }
-
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    return v;
-}
-
-__device__ __forceinline__ void hist_push(const GmresWork& W, GmresCtl* c, double r)
-{
-    if (c->nhist < W.caphist) W.hist[c->nhist] = (c->bnorm > 0.0) ? r / c->bnorm : r;
-    c->nhist++;
-}
-
-// Scalar epilogues, run by one thread after a reduction has produced d[0..nv).
-__device__ void epilogue(const GmresWork& W, int mode, const double* d, int nv, int col0)
-{
-    GmresCtl* c = W.ctl;
-    const int m = c->m;
-    if (mode == DOT_BNORM) {
-        c->bnorm = sqrt(d[0]);
-        c->target = c->est * c->bnorm;      // est holds tol until the first residual (set by begin_solve)
-        if (!isfinite(c->bnorm)) c->nonfinite = 1;
-    } else if (mode == DOT_RNORM) {         // true residual at the start of a cycle
-        const double r = sqrt(d[0]);
-        c->rnorm = r; c->est = r;
-        hist_push(W, c, r);
-        if (!isfinite(r)) c->nonfinite = 1;
-        c->converged = (r <= c->target) ? 1 : 0;
-        c->inner_stop = (c->converged || c->its >= c->maxit || c->nonfinite) ? 1 : 0;
-        c->j = 0;
-        W.scale[0] = 1.0 / r;
-        W.g[0] = r;
-        for (int k = 1; k <= m; ++k) W.g[k] = 0.0;
-    } else if (mode == DOT_H || mode == DOT_H2) {   // h_i = <w, v_i>, v_i = scale_i V_i
-        const int j = c->j;
-        for (int k = 0; k < nv; ++k) {
-            const int i = col0 + k;
-            const double h = d[k] * W.scale[i];
-            if (mode == DOT_H) W.H[i * m + j] = h; else W.H[i * m + j] += h;
-            W.coef[i] = h * W.scale[i];
-        }
-    } else if (mode == BICG_ALPHA) {        // alpha = rho_new / <r^, v>
-        const double rhv = d[0];
-        if (rhv == 0.0 || !isfinite(rhv)) { c->inner_stop = 1; if (!isfinite(rhv)) c->nonfinite = 1; }
-        else c->bs[BS_ALPHA] = c->bs[BS_RHO_NEW] / rhv;
-    } else if (mode == BICG_OMEGA) {        // omega = <t, s> / <t, t>
-        const double ts = d[0], tt = d[1];
-        c->bs[BS_OMEGA] = (tt > 0.0) ? ts / tt : 0.0;
-        c->bs[BS_RESTART] = (c->bs[BS_OMEGA] == 0.0 || !isfinite(c->bs[BS_OMEGA])) ? 1.0 : 0.0;
-        if (!isfinite(c->bs[BS_OMEGA])) { c->nonfinite = 1; c->inner_stop = 1; }
-    } else if (mode == BICG_RHO) {          // end of a BiCGStab iteration: rho <- rho_new, rho_new = <r^, r>, ||r||
-        c->bs[BS_RHO] = c->bs[BS_RHO_NEW];
-        c->bs[BS_RHO_NEW] = d[0];
-        const double rn = sqrt(d[1]);
-        c->bs[BS_RN] = rn; c->est = rn;
-        c->its += 1;
-        hist_push(W, c, rn);
-        if (!isfinite(rn) || !isfinite(d[0])) c->nonfinite = 1;
-        if (rn <= c->target || c->its >= c->maxit || d[0] == 0.0 || c->bs[BS_RESTART] != 0.0 || c->nonfinite) c->inner_stop = 1;
-    } else if (mode == DOT_AUX0 || mode == DOT_AUX1) {
-        c->aux[mode - DOT_AUX0] = sqrt(d[0]);
-    } else if (mode == DOT_UPD) {           // h_{j+1,j} = ||w||, Givens rotations (Saad 2003, Sect. 6.5.3)
-        const int j = c->j;
-        const double hn = sqrt(d[0]);
-        double* H = W.H;
-        H[(j + 1) * m + j] = hn;
-        for (int i = 0; i < j; ++i) {
-            const double a = H[i * m + j], b = H[(i + 1) * m + j];
-            H[i * m + j] = W.cs[i] * a + W.sn[i] * b;
-            H[(i + 1) * m + j] = -W.sn[i] * a + W.cs[i] * b;
-        }
-        const double a = H[j * m + j], b = H[(j + 1) * m + j];
-        const double r = hypot(a, b);
-        W.cs[j] = a / r; W.sn[j] = b / r;
-        H[j * m + j] = r; H[(j + 1) * m + j] = 0.0;
-        W.g[j + 1] = -W.sn[j] * W.g[j];
-        W.g[j] = W.cs[j] * W.g[j];
-        W.scale[j + 1] = 1.0 / hn;
-        c->j = j + 1; c->its += 1;
-        c->est = fabs(W.g[j + 1]);
-        hist_push(W, c, c->est);
-        if (!isfinite(hn) || !isfinite(c->est)) c->nonfinite = 1;
-        if (c->est <= c->target || hn == 0.0 || c->its >= c->maxit || j + 1 >= m || c->nonfinite) c->inner_stop = 1;
-    }
-}
-
-// Block reduction of acc[0..NV) -> partial[block][.]; the last block sums the partials in a fixed order and
-// runs the epilogue.
-template <int NV>
-__device__ __forceinline__ void reduce_and_finish(double (&acc)[NV], const GmresWork& W, int mode, int col0)
-{
-    __shared__ double sh[KTHREADS / 32][MAXV];
-    __shared__ double dres[MAXV];
-    __shared__ bool is_last;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int k = 0; k < NV; ++k) {
-        const double s = warp_sum(acc[k]);
-        if (lane == 0) sh[warp][k] = s;
-    }
-    __syncthreads();
-    if (threadIdx.x < NV) {
-        double s = 0.0;
-#pragma unroll
-        for (int w = 0; w < KTHREADS / 32; ++w) s += sh[w][threadIdx.x];
-        W.partial[(size_t)blockIdx.x * MAXV + threadIdx.x] = s;
-    }
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned int t = atomicInc(&W.ctl->ticket, gridDim.x - 1);   // wraps to 0 after the last block
-        is_last = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!is_last) return;
-    __threadfence();
-    for (int k = warp; k < NV; k += KTHREADS / 32) {
-        double s = 0.0;
-        for (unsigned int b = lane; b < gridDim.x; b += 32) s += __ldcg(&W.partial[(size_t)b * MAXV + k]);
-        s = warp_sum(s);
-        if (lane == 0) dres[k] = s;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) epilogue(W, mode, dres, NV, col0);
-}
 
 template <int NV>
 __global__ void __launch_bounds__(KTHREADS) multi_dot_kernel(const double* __restrict__ w, const double* __restrict__ V0,

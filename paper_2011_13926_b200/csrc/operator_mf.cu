@@ -10,13 +10,14 @@
 // marches over the rows; a thread keeps z = M^-1 v and Pi = c^2 J z of its cell in rows j and j+1 in registers (the
 // y-face flux needs no other thread; the north flux of row j is the south flux of row j+1); x-faces go through
 // shared memory: publish (z, Pi_xx, Pi_xy), compute the EAST flux, publish it, read the WEST flux from the left thread.
-#include "ark_m1_internal.h"
+#include <string.h>
+#include "krylov_device.cuh"
 
 namespace ark {
 
 static constexpr int TXO = 128;
 
-struct ZP { double zE, zFx, zFy, Pxx, Pxy, Pyy; };   // z and c^2 J z of one cell
+struct ZP { double zE, zFx, zFy, Pxx, Pxy, Pyy, v0, v1, v2; };   // z = [M^-1] v, c^2 J z and the raw input v of one cell
 struct FC { double ap, Lam, alpha, sw; };            // face coefficients; sw = c dt sigma_f / 4
 
 // Linear flux through one face (normal component n, tangential t); same algebra as the explicit kernel.
@@ -35,7 +36,7 @@ template <bool PRECOND>
 __device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const double* __restrict__ v, const double* __restrict__ Minv,
                                       const double* __restrict__ J, double c2, int xmode, int ii, int j)
 {
-    ZP r; r.zE = 0.0; r.zFx = 0.0; r.zFy = 0.0; r.Pxx = 0.0; r.Pxy = 0.0; r.Pyy = 0.0;
+    ZP r; r.zE = 0.0; r.zFx = 0.0; r.zFy = 0.0; r.Pxx = 0.0; r.Pxy = 0.0; r.Pyy = 0.0; r.v0 = 0.0; r.v1 = 0.0; r.v2 = 0.0;
     if (xmode != 0) return r;
     int jj = j;
     if (j < 0 || j >= g.ny) {
@@ -45,6 +46,7 @@ __device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const double* 
     }
     const long long id = (long long)jj * g.nx + ii;
     const double v0 = v[id], v1 = v[N + id], v2 = v[2 * N + id];
+    r.v0 = v0; r.v1 = v1; r.v2 = v2;
     if (PRECOND) {
         r.zE  = Minv[0 * N + id] * v0 + Minv[1 * N + id] * v1 + Minv[2 * N + id] * v2;
         r.zFx = Minv[3 * N + id] * v0 + Minv[4 * N + id] * v1 + Minv[5 * N + id] * v2;
@@ -64,13 +66,16 @@ __device__ __forceinline__ FC load_fc(const double* __restrict__ p, long long st
 
 struct ZPub { double zE, zFx, zFy, Pxx, Pxy; };
 
-template <bool PRECOND>
+// DOT (BiCGStab fusions, saving the separate reduction passes): 0 none; 1: <out, aux> -> epilogue BICG_ALPHA;
+// 2: <out, v>, <out, out> -> epilogue BICG_OMEGA (v = the kernel's own input, already in registers).
+template <bool PRECOND, int DOT>
 __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const double* __restrict__ v,
                                                     double* __restrict__ out, const double* __restrict__ scale_ptr,
                                                     const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
-                                                    int RY, double rx, double ry, double c2)
+                                                    int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W)
 {
     if (skip_flag && *skip_flag) return;
+    double acc[2] = { 0.0, 0.0 };
     __shared__ ZPub pub[TXO + 1];
     __shared__ double flx[4][TXO];
     const int t = threadIdx.x;
@@ -117,6 +122,8 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
             dE = mf.dE[id]; dF = mf.dF[id];
             if (add) { a0 = add[id]; a1 = add[N + id]; a2 = add[2 * N + id]; }
         }
+        double x0 = 0.0, x1 = 0.0, x2 = 0.0;
+        if (DOT == 1 && upd) { x0 = aux[id]; x1 = aux[N + id]; x2 = aux[2 * N + id]; }
         FC fe; fe.ap = 0.5; fe.Lam = 0.0; fe.alpha = 1.0; fe.sw = 0.0;
         if (east_valid) {
             if (use_xlo || xmode == 1) { if (i < 0) fe = load_fc(mf.xlo, g.ny, j); }
@@ -141,25 +148,50 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
             double o0 = zC.zE  + fma(rx, Ge0 - Gw0, fma(ry, Hn0 - Hs0, dE * zC.zE));
             double o1 = zC.zFx + fma(rx, Ge1 - Gw1, fma(ry, Hn1 - Hs1, fma(dF, zC.zFx, Se + Sw)));
             double o2 = zC.zFy + fma(rx, Ge2 - Gw2, fma(ry, Hn2 - Hs2, fma(dF, zC.zFy, Sn + Ss)));
-            out[id] = fma(sc, o0, a0); out[N + id] = fma(sc, o1, a1); out[2 * N + id] = fma(sc, o2, a2);
+            o0 = fma(sc, o0, a0); o1 = fma(sc, o1, a1); o2 = fma(sc, o2, a2);
+            out[id] = o0; out[N + id] = o1; out[2 * N + id] = o2;
+            if (DOT == 1) acc[0] += o0 * x0 + o1 * x1 + o2 * x2;
+            if (DOT == 2) { acc[0] += o0 * zC.v0 + o1 * zC.v1 + o2 * zC.v2; acc[1] += o0 * o0 + o1 * o1 + o2 * o2; }
         }
         zC = zN;
         Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
     }
+    if (DOT == 1) reduce_and_finish<2, TXO>(acc, W, BICG_ALPHA, 0);
+    if (DOT == 2) reduce_and_finish<2, TXO>(acc, W, BICG_OMEGA, 0);
+}
+
+static dim3 op_mf_grid(const Grid& g, int sm_count, int* RYout)
+{
+    const int strips = (g.nx + (TXO - 2) - 1) / (TXO - 2);
+    long long want = ((long long)g.ny * strips + (long long)sm_count * 16 - 1) / ((long long)sm_count * 16);
+    int RY = (int)(want < 4 ? 4 : (want > 64 ? 64 : want));
+    if (RY > g.ny) RY = g.ny;
+    *RYout = RY;
+    return dim3(strips, (g.ny + RY - 1) / RY);
+}
+
+int op_mf_blocks(const Grid& g, int sm_count) { int RY; const dim3 d = op_mf_grid(g, sm_count, &RY); return (int)(d.x * d.y); }
+
+// v_out = A M^-1 v_in fused with the BiCGStab reduction `dot` (1: alpha with aux = r^; 2: omega)
+cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
+                             const int* skip_flag, int dot, const double* aux, GmresWork W, int sm_count, cudaStream_t st)
+{
+    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY);
+    const double c2 = g.c * g.c;
+    if (dot == 1) op_mf_kernel<true, 1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+    else op_mf_kernel<true, 2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
                          int sm_count, cudaStream_t st)
 {
-    const int strips = (g.nx + (TXO - 2) - 1) / (TXO - 2);
-    long long want = ((long long)g.ny * strips + (long long)sm_count * 16 - 1) / ((long long)sm_count * 16);
-    int RY = (int)(want < 4 ? 4 : (want > 64 ? 64 : want));
-    if (RY > g.ny) RY = g.ny;
-    dim3 grd(strips, (g.ny + RY - 1) / RY);
+    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY);
     const double c2 = g.c * g.c;
-    if (precond) op_mf_kernel<true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2);
-    else op_mf_kernel<false><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2);
+    GmresWork none; memset(&none, 0, sizeof none);
+    if (precond) op_mf_kernel<true, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    else op_mf_kernel<false, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     return cudaGetLastError();
 }
 
