@@ -85,6 +85,7 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *   "eig_floor"     x: lambda+ >= x c, lambda- <= -x c; default 0
  *   "a_r"           radiation constant (default 1)
  *   "orthogonalisation" 1: one-pass classical Gram-Schmidt (default)   2: CGS2 (re-orthogonalise once)
+ *   "assembly_kernel"   1: marching assembly for the matrix-free operator (default)   0: tile assembly (always used by operator 0)
  *   "krylov"            0: restarted GMRES(restart) (north_star, default)   1: BiCGStab, the paper's solver,
  *                       right-preconditioned with the same block-Jacobi; `restart` is then ignored and the returned count is in
  *                       BiCGStab iterations (two operator applications each)

@@ -34,7 +34,7 @@ struct ark_m1 {
     double *rho_cv, *ux, *uy, *source_E;
     unsigned long long* counts;   // 2
     // options
-    int ortho, explicit_kernel, op_kind, maxv, basis_pad, krylov;
+    int ortho, explicit_kernel, op_kind, maxv, basis_pad, krylov, asm_kernel;
     // implicit workspace (lazy)
     BlockMatrix A;
     MfPlanes mf;       // matrix-free coefficient planes (op_kind == 1)
@@ -130,7 +130,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0;
-    h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0;
+    h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0; h->asm_kernel = 1;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     h->hist_host = new std::vector<double>();
@@ -237,6 +237,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
     else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 3) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1, 2 or 3%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "assembly_kernel")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "assembly_kernel must be 0 (tile) or 1 (marching)%s", ""); h->asm_kernel = iv; }
     else if (!strcmp(key, "krylov")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "krylov must be 0 (GMRES) or 1 (BiCGStab)%s", ""); h->krylov = iv; }
     else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 32]%s", ""); h->maxv = iv; }
     else if (!strcmp(key, "basis_pad")) { if (iv < 0 || (iv & 31)) return fail(h, ARK_M1_E_ARG, "basis_pad must be a non-negative multiple of 32 doubles%s", ""); if (iv != h->basis_pad) { cudaStreamSynchronize(h->st); free_implicit(h); } h->basis_pad = iv; }
@@ -434,7 +435,10 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
     const Fields f = fields_of(h);
     if (h->op_kind == 1) {
         h->mf.rx = dt / h->g.dx; h->mf.ry = dt / h->g.dy;
-        KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->st));
+        if (h->asm_kernel == 1 && h->N < (1LL << 31))
+            KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble_march(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->sm_count, h->st));
+        else
+            KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->st));
     } else {
         MfPlanes none; memset(&none, 0, sizeof none);
         KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, none, bsrc, h->st));

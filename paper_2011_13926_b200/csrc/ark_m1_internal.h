@@ -87,6 +87,9 @@ struct MfPlanes {
 // iterations, where `f` is the iterate that only supplies the coefficients)
 cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf,
                             const double* bsrc, cudaStream_t st);
+// same outputs for the matrix-free storage from the marching kernel (assemble_march.cu)
+cudaError_t launch_assemble_march(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf,
+                                  const double* bsrc, int sm_count, cudaStream_t st);
 // out = sgn * s * (A [M^-1] v) + add, flux form from the coefficient planes; precond = 1 applies M^-1 (Minv) first
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
