@@ -90,3 +90,16 @@ def marshak_diffusion_reference(w, dt, nsteps):
             if np.max(np.abs(d)) < 1e-13:
                 break
     return T
+
+
+def paper_values():
+    """tests/golden/paper_fixed_values.txt: values the paper prints, one per line with its citation."""
+    import os
+    vals = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_fixed_values.txt")) as fh:
+        for line in fh:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split()
+                vals[k] = float(v)
+    return vals
