@@ -409,6 +409,18 @@ def run_ours(args):
                                     "iterations": its5, "final_residual": res5, "ms": ms5, "cell_updates_per_s": N5 / (ms5 * 1e-3),
                                     "ms_per_iteration": tm5["krylov_ms"] / max(its5, 1),
                                     "krylov_hbm_frac": (bpc5 * N5 / (tm5["krylov_ms"] * 1e-3) / 1e9 / peak_gbs) if its5 > 0 else None}
+            # explicit step of the coupled system (marching kernel with emission, source and the Eq. 4 update)
+            g5.set_state(d5["E"], d5["F"], d5["sigma_a"], d5["sigma_s"], d5["T"])
+            dte5 = wl.explicit_dt(w5["dx"], w5["dy"], w5["c"])
+            g5.steps_explicit(dte5, 5)
+            torch.cuda.synchronize()
+            e0.record(stream)
+            g5.steps_explicit(dte5, 40)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms5e = e0.elapsed_time(e1) / 40
+            line_extra["stage2"]["explicit"] = {"ms_per_step": ms5e, "cell_updates_per_s": N5 / (ms5e * 1e-3), "bytes_per_cell": 96,
+                                                "hbm_frac": 96.0 * N5 / (ms5e * 1e-3) / 1e9 / peak_gbs}
             g5.close()
             del d5
         # ---- roofline of the dominant kernel class ---------------------------------------------------------------

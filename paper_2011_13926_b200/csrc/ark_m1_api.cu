@@ -282,8 +282,9 @@ static int explicit_once(ark_m1* h, double dt)
         KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
     } else if (h->explicit_kernel == 2 && plain && h->N < (1LL << 31)) {
         KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_warp(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
-    } else if (h->explicit_kernel == 1 && plain && h->N < (1LL << 31)) {   // the march kernels use 32-bit in-plane offsets
-        KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
+    } else if (h->explicit_kernel >= 1 && h->N < (1LL << 31)) {   // the march kernels use 32-bit in-plane offsets
+        KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N,
+                                                                                  h->have_T ? h->T[h->cur ^ 1] : nullptr, h->sm_count, h->st));
     } else {
         KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_cell(h->g, h->s, f, dt, 0, O, O + h->N, O + 2 * h->N, h->have_T ? h->T[h->cur ^ 1] : nullptr, h->st));
     }

@@ -54,7 +54,7 @@ enum { BS_RHO = 0, BS_ALPHA = 1, BS_OMEGA = 2, BS_RHO_NEW = 3, BS_RN = 4, BS_RES
 cudaError_t launch_explicit_cell(const Grid& g, const Scheme& s, const Fields& f, double dt, int mode,
                                  double* outE, double* outFx, double* outFy, double* outT, cudaStream_t st);
 cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& f, double dt,
-                                  double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st);
+                                  double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st);
 cudaError_t launch_explicit_march3(const Grid& g, const Scheme& s, const Fields& f, double dt,
                                    double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st);
 cudaError_t launch_explicit_warp(const Grid& g, const Scheme& s, const Fields& f, double dt,

@@ -14,9 +14,11 @@
 
 namespace ark {
 
-template <bool SD>
+// COUPLED: stage-2 terms of the cell kernel (emission c sigma_a a_r T^4, source_E, explicit matter-energy update of Eq. 4).
+template <bool SD, bool COUPLED>
 __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
-                                                            double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
+                                                            double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy,
+                                                            double* __restrict__ oT)
 {
     __shared__ XPub pub[TX + 1];   // +1: the last thread reads a (unused) right neighbour
     __shared__ double flx[4][TX];
@@ -110,7 +112,16 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
             double dSFx, dSFy;   // -dt * S^F
             if (wb) { dSFx = qc * (Se + Sw); dSFy = qc * (Sn + Ss); }
             else { dSFx = dt * c * uC.st * uC.Fx; dSFy = dt * c * uC.st * uC.Fy; }
-            const double dSE = cdt * uC.sa * uC.E;
+            double dSE = cdt * uC.sa * uC.E;        // -dt * S^E
+            if (COUPLED && upd) {
+                if (f.T) {
+                    const double T = f.T[row_off], rcv = f.rho_cv ? f.rho_cv[row_off] : 1.0;
+                    const double Theta = s.a_r * (T * T) * (T * T);
+                    dSE -= cdt * uC.sa * Theta;
+                    if (oT) oT[row_off] = T - cdt * uC.sa * (Theta - uC.E) / rcv;      // Eq. 4, explicit
+                }
+                if (f.source_E) dSE -= dt * f.source_E[row_off];
+            }
             const double nE  = uC.E  - fma(rdx, Ge0 - Gw0, fma(rdy, Hn0 - Hs0, dSE));
             const double nFx = uC.Fx - fma(rdx, Ge1 - Gw1, fma(rdy, Hn1 - Hs1, dSFx));
             const double nFy = uC.Fy - fma(rdx, Ge2 - Gw2, fma(rdy, Hn2 - Hs2, dSFy));
@@ -231,7 +242,7 @@ cudaError_t launch_explicit_warp(const Grid& g, const Scheme& s, const Fields& f
 }
 
 cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& f, double dt,
-                                  double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st)
+                                  double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st)
 {
     const int strips = (g.nx + (TX - 2) - 1) / (TX - 2);
     // rows per block: enough blocks for ~8 per SM, between 4 and ARK_MARCH_RY rows.  (A single wave of
@@ -240,8 +251,14 @@ cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& 
     int RY = (int)(want < 4 ? 4 : (want > ARK_MARCH_RY ? ARK_MARCH_RY : want));
     if (RY > g.ny) RY = g.ny;
     dim3 grd(strips, (g.ny + RY - 1) / RY);
-    if (s.is_default()) explicit_march_kernel<true><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
-    else explicit_march_kernel<false><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
+    const bool coupled = (f.T != nullptr) || (f.source_E != nullptr);
+    if (coupled) {
+        if (s.is_default()) explicit_march_kernel<true, true><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, outT);
+        else explicit_march_kernel<false, true><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, outT);
+    } else {
+        if (s.is_default()) explicit_march_kernel<true, false><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, nullptr);
+        else explicit_march_kernel<false, false><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, nullptr);
+    }
     return cudaGetLastError();
 }
 
