@@ -62,6 +62,8 @@ typedef struct oracle_m1 {
     int eig;         /* 0: Eq. 14 (default), 1: fixed +-c, 2: fixed +-c/sqrt(3) */
     int closure;     /* 0: M1 (default), 1: P1 (chi = 1/3) */
     int lin;         /* 0: analytic pressure Jacobian (default, R4), 1: frozen Eddington tensor */
+    int src_off;     /* internal (semi-implicit step): 1 drops the source terms from the residual */
+    int hyp_off;     /* internal (semi-implicit step): 1 drops the flux-divergence terms from the assembled operator */
     int krylov;      /* 0: restarted GMRES (north_star, default), 1: BiCGStab (the paper's solver) */
     double eig_floor;/* lambda^+ >= floor*c, lambda^- <= -floor*c; default 0 */
     double a_r;      /* radiation constant, default 1 */
@@ -254,6 +256,7 @@ static void residual_cell(const oracle_m1 *h, int i, int j, double R[3])
     } else {      /* Eq. 16 */
         SFx = -c * u[0].st * u[0].Fx; SFy = -c * u[0].st * u[0].Fy;
     }
+    if (h->src_off) { SE = 0.0; SFx = 0.0; SFy = 0.0; }
     R[0] = (Ge[0] - Gw[0]) / h->dx + (Hn[0] - Hs[0]) / h->dy - SE;
     R[1] = (Ge[1] - Gw[1]) / h->dx + (Hn[1] - Hs[1]) / h->dy - SFx;
     R[2] = (Ge[2] - Gw[2]) / h->dx + (Hn[2] - Hs[2]) / h->dy - SFy;
@@ -282,7 +285,7 @@ ORACLE_API int oracle_m1_step_explicit(oracle_m1 *h, double dt)
     oracle_m1_residual(h, R, R + N);
     #pragma omp parallel for schedule(static)
     for (long id = 0; id < N; ++id) {
-        if (h->has_T) {
+        if (h->has_T && !h->src_off) {
             const double T = h->T[id];
             const double rcv = h->rho_cv ? h->rho_cv[id] : 1.0;
             h->T[id] = T - dt * h->c * h->sa[id] * (h->a_r * T * T * T * T - h->E[id]) / rcv;   /* Eq. 4 */
@@ -389,7 +392,7 @@ static void assemble_cell(const oracle_m1 *h, double dt, const double *base, int
     face_eval(h, &u[0], &q[0], &u[2], &q[2], 0, &fe);
     face_eval(h, &u[3], &q[3], &u[0], &q[0], 1, &fs);
     face_eval(h, &u[0], &q[0], &u[4], &q[4], 1, &fn);
-    const double c = h->c, c2 = c * c, rx = dt / h->dx, ry = dt / h->dy;
+    const double c = h->c, c2 = c * c, rx = h->hyp_off ? 0.0 : dt / h->dx, ry = h->hyp_off ? 0.0 : dt / h->dy;
     const double eta = eta_cell(h, u[0].idx, dt);
     double se = 0, sw = 0, sn = 0, ss = 0, sc = 0;
     if (h->wb) { se = c * dt * fe.sig / 4; sw = c * dt * fw.sig / 4; sn = c * dt * fn.sig / 4; ss = c * dt * fs.sig / 4; }
@@ -728,6 +731,26 @@ ORACLE_API int oracle_m1_step_implicit_newton(oracle_m1 *h, double dt, double to
     if (final_update) *final_update = upd;
     free(base); free(x);
     return total;
+}
+
+/* Semi-implicit step ("source terms remain implicit, but the hyperbolic part is time-explicit"; used by the
+ * paper for the beam and shadow tests):
+ *   U* = U^n - dt [flux divergence](U^n)            (Eq. 12 without its right-hand side, alpha etc. at t^n)
+ *   (I + dt S) U^{n+1} = U* + affine terms          (S = the source operator: c sigma_a eta on E; the WB weights of Eqs. 18-19 or,
+ *                                                    with well_balanced = 0, c sigma_t on F (Eq. 16); Eq. B.1 is its F row)
+ * The second line is the assembled system of the implicit step with the flux terms switched off; it depends on the
+ * opacities only, so nothing is linearised.  Solved with the same Krylov method and preconditioner. */
+ORACLE_API int oracle_m1_step_semi_implicit(oracle_m1 *h, double dt, double tol, int restart, int maxit, double *final_residual)
+{
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) { snprintf(h->err, sizeof h->err, "bad argument"); return -1; }
+    h->src_off = 1;
+    int rc = oracle_m1_step_explicit(h, dt);
+    h->src_off = 0;
+    if (rc) return rc;
+    h->hyp_off = 1;
+    rc = oracle_m1_step_implicit(h, dt, tol, restart, maxit, final_residual);
+    h->hyp_off = 0;
+    return rc;
 }
 
 /* Step 3 of the operator splitting: explicit addition of the velocity-dependent sources of

@@ -48,6 +48,7 @@ def lib():
         L.oracle_m1_get_state.argtypes = [C.c_void_p, dp, dp, dp]
         L.oracle_m1_step_explicit.argtypes = [C.c_void_p, C.c_double]
         L.oracle_m1_step_implicit.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, dp]
+        L.oracle_m1_step_semi_implicit.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, dp]
         L.oracle_m1_step_implicit_newton.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_int, ip, dp, dp]
         L.oracle_m1_add_velocity_sources.argtypes = [C.c_void_p, C.c_double]
         L.oracle_m1_residual.argtypes = [C.c_void_p, dp, dp]
@@ -133,6 +134,11 @@ class OracleM1:
     def step_implicit(self, dt, tol=1e-10, restart=30, maxit=4000):
         res = C.c_double(0.0)
         its = self._check(lib().oracle_m1_step_implicit(self._h, float(dt), float(tol), int(restart), int(maxit), C.byref(res)))
+        return its, res.value
+
+    def step_semi_implicit(self, dt, tol=1e-12, restart=30, maxit=4000):
+        res = C.c_double(0.0)
+        its = self._check(lib().oracle_m1_step_semi_implicit(self._h, float(dt), float(tol), int(restart), int(maxit), C.byref(res)))
         return its, res.value
 
     def step_implicit_newton(self, dt, tol=1e-10, restart=30, maxit=4000, newton_tol=1e-8, max_newton=20):

@@ -257,3 +257,46 @@ def test_marshak_wave_ap_scheme_recovers_the_diffusion_limit():
     pv = paper_values()
     assert err[1] <= pv["marshak_ap_rel_l2"]                  # the paper's 1.1 % (measured: 2e-5)
     assert abs(err[0] - pv["marshak_hll_rel_l2"]) <= 0.1      # standard HLL: numerical diffusion dominates (paper: 84 %, here 82 %)
+
+
+def test_semi_implicit_step_pins():
+    # explicit hyperbolic part, implicit sources.
+    from helpers import rel_l2
+    # (i) sigma = 0: identical to the explicit step
+    w = small_random_state(17, 13, seed=81)
+    w["sigma_a"][:] = 0.0
+    w["sigma_s"][:] = 0.0
+    dt = wl.explicit_dt(w["dx"], w["dy"])
+    o1, o2 = make_oracle(w), make_oracle(w)
+    o1.step_explicit(dt)
+    its, res = o2.step_semi_implicit(dt)
+    assert its == 0
+    assert all(rel_l2(a, b) <= 1e-14 for a, b in zip(o2.get_state(), o1.get_state()))
+    # (ii) uniform state and opacity: no flux divergence; closed form E/(1 + c dt sigma_a), F/(1 + c dt sigma_t) for BOTH source
+    #      discretisations (Eq. 16 and Eqs. 18-19: the face means of a uniform field are the field), even for c sigma dt >> 1
+    for wbflag in (1, 0):
+        n = 12
+        w = dict(nx=n, ny=n, dx=1.0 / n, dy=1.0 / n, c=1.3, bc=(0, 0, 0, 0), E=np.full((n, n), 2.0),
+                 F=np.stack((np.full((n, n), 0.4), np.full((n, n), -0.3))), sigma_a=np.full((n, n), 5.0), sigma_s=np.full((n, n), 70.0))
+        o = make_oracle(w, dict(well_balanced=wbflag))
+        dts = 3.0                                       # c sigma_t dt = 292: far beyond the explicit limit
+        o.step_semi_implicit(dts, 1e-13, 30, 500)
+        E, F = o.get_state()
+        assert np.allclose(E, 2.0 / (1.0 + 1.3 * dts * 5.0), rtol=1e-11)
+        assert np.allclose(F[0], 0.4 / (1.0 + 1.3 * dts * 75.0), rtol=1e-10) and np.allclose(F[1], -0.3 / (1.0 + 1.3 * dts * 75.0), rtol=1e-10)
+    # (iii) App. B: the implicit WB source sub-step is unconditionally stable: |F| does not grow for rough F
+    w = small_random_state(24, 18, seed=82, sig_range=(1.0, 3.0))
+    o = make_oracle(w)
+    n0 = np.linalg.norm(w["F"])
+    for _ in range(5):
+        o.step_semi_implicit(wl.explicit_dt(w["dx"], w["dy"]), 1e-12, 30, 2000)
+    assert np.linalg.norm(o.get_state()[1]) < n0
+    # (iv) consistency: for small dt the semi-implicit and the explicit step agree to O(dt^2)
+    w = small_random_state(20, 16, seed=83, sig_range=(-1.0, 0.5))
+    d = []
+    for dt in (1e-4, 5e-5):
+        oa, ob = make_oracle(w), make_oracle(w)
+        oa.step_explicit(dt)
+        ob.step_semi_implicit(dt, 1e-14, 30, 500)
+        d.append(max(rel_l2(a, b) for a, b in zip(ob.get_state(), oa.get_state())))
+    assert 3.0 < d[0] / d[1] < 5.0
