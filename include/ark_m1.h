@@ -133,6 +133,14 @@ ARK_M1_API int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
 ARK_M1_API int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int restart, int maxit, double newton_tol,
                                            int max_newton, int* newton_iterations, double* final_residual, double* final_update);
 
+/* Semi-implicit step ("source terms remain implicit, but the hyperbolic part is time-explicit"; the paper uses it
+ * for its beam and shadow tests): U* = U^n - dt [flux divergence](U^n) with the marching explicit kernel,
+ * then (I + dt S) U^{n+1} = U* + affine terms, S = the source operator only (c sigma_a eta on E; the WB weights of Eqs. 18-19
+ * — Eq. B.1 — or c sigma_t with "well_balanced" 0).  The second system is the implicit step's with its flux terms switched off
+ * and is solved by the same Krylov method (a few iterations: it is strictly diagonally dominant).  Same arguments, return
+ * value and error behaviour as ark_m1_step_implicit. */
+ARK_M1_API int ark_m1_step_semi_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual);
+
 /* Step 3 of the operator splitting: explicit addition of the velocity sources of Eq. 6
  * using the fields "ux", "uy".  ARK_M1_E_NOTSET if they are missing. */
 ARK_M1_API int ark_m1_add_velocity_sources(ark_m1* h, double dt);

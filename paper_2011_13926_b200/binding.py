@@ -22,7 +22,7 @@ XLO, XHI, YLO, YHI = 0, 1, 2, 3
 SYMBOLS = [
     "ark_m1_create", "ark_m1_destroy", "ark_m1_set_stream", "ark_m1_set_state", "ark_m1_set_boundary",
     "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
-    "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
+    "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_step_semi_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
     "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
@@ -61,6 +61,7 @@ def load_library(path: str | None = None):
     L.ark_m1_step_explicit.argtypes = [vp, d]
     L.ark_m1_steps_explicit.argtypes = [vp, d, i]
     L.ark_m1_step_implicit.argtypes = [vp, d, d, i, i, C.POINTER(C.c_double)]
+    L.ark_m1_step_semi_implicit.argtypes = [vp, d, d, i, i, C.POINTER(C.c_double)]
     L.ark_m1_step_implicit_newton.argtypes = [vp, d, d, i, i, d, i, C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.ark_m1_add_velocity_sources.argtypes = [vp, d]
     L.ark_m1_count_unrealizable.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
@@ -181,6 +182,11 @@ class ArkM1:
     def step_implicit(self, dt, tol=1e-10, restart=30, maxit=4000):
         res = C.c_double(0.0)
         its = self._check(self._L.ark_m1_step_implicit(self._h, float(dt), float(tol), int(restart), int(maxit), C.byref(res)))
+        return its, res.value
+
+    def step_semi_implicit(self, dt, tol=1e-12, restart=30, maxit=4000):
+        res = C.c_double(0.0)
+        its = self._check(self._L.ark_m1_step_semi_implicit(self._h, float(dt), float(tol), int(restart), int(maxit), C.byref(res)))
         return its, res.value
 
     def step_implicit_newton(self, dt, tol=1e-10, restart=30, maxit=4000, newton_tol=1e-8, max_newton=20):

@@ -129,7 +129,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     memset(h, 0, sizeof *h);
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
-    h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0;
+    h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
     h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0; h->asm_kernel = 1;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -435,7 +435,7 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
 {
     const Fields f = fields_of(h);
     if (h->op_kind == 1) {
-        h->mf.rx = dt / h->g.dx; h->mf.ry = dt / h->g.dy;
+        h->mf.rx = h->s.hyp_off ? 0.0 : dt / h->g.dx; h->mf.ry = h->s.hyp_off ? 0.0 : dt / h->g.dy;
         if (h->asm_kernel == 1 && h->N < (1LL << 31))
             KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble_march(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->sm_count, h->st));
         else
@@ -623,6 +623,31 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
     if (newton_iterations) *newton_iterations = k;
     if (final_update) *final_update = upd;
     return total;
+}
+
+// Semi-implicit step: explicit flux step without sources, then the source-only linear system (the assembled
+// implicit system with its flux terms switched off; it depends on the opacities only).
+extern "C" int ark_m1_step_semi_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual)
+{
+    if (!h) return ARK_M1_E_ARG;
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_semi_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_semi_implicit: no state set%s", "");
+    if (h->N >= (1LL << 31)) return fail(h, ARK_M1_E_UNSUPPORTED, "step_semi_implicit: grid too large for the marching kernels%s", "");
+    {   // U* = U^n - dt div(flux): marching kernel with the sources off (T untouched)
+        h->s.src_off = 1;
+        const Fields f = fields_of(h);
+        double* O = h->U[h->cur ^ 1];
+        kmark(h, KC_EXPLICIT, 64.0 * h->N);
+        cudaError_t e = launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, nullptr, h->sm_count, h->st);
+        h->s.src_off = 0;
+        if (e != cudaSuccess) return fail(h, ARK_M1_E_CUDA, "launch_explicit_march: %s", cudaGetErrorString(e));
+        if (h->have_T) CU(cudaMemcpyAsync(h->T[h->cur ^ 1], h->T[h->cur], (size_t)h->N * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
+        h->cur ^= 1;
+    }
+    h->s.hyp_off = 1;
+    const int rc = ark_m1_step_implicit(h, dt, tol, restart, maxit, final_residual);
+    h->s.hyp_off = 0;
+    return rc;
 }
 
 extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, double* out, double* b_out)

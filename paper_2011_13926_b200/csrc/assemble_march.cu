@@ -49,7 +49,8 @@ __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, F
     const int j1 = min(j0 + RY, g.ny);
     const long long N = (long long)g.nx * g.ny;
     const bool upd = (t >= 1 && t <= TXA - 2 && i >= 0 && i < g.nx);
-    const double c = g.c, c2 = c * c, rx = dt / g.dx, ry = dt / g.dy, cdt = c * dt;
+    const bool hyp = SD ? true : (s.hyp_off == 0);       // semi-implicit step: source-only system
+    const double c = g.c, c2 = c * c, rx = hyp ? dt / g.dx : 0.0, ry = hyp ? dt / g.dy : 0.0, cdt = c * dt;
     const bool wb = SD ? true : (s.wb != 0);
     const double qw = wb ? 0.25 * cdt : 0.0;
     int xmode = 0, ii = i, xside = 0;

@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
             if (wb) { dSFx = qc * (Se + Sw); dSFy = qc * (Sn + Ss); }
             else { dSFx = dt * c * uC.st * uC.Fx; dSFy = dt * c * uC.st * uC.Fy; }
             double dSE = cdt * uC.sa * uC.E;        // -dt * S^E
-            if (COUPLED && upd) {
+            if (COUPLED && upd && !(!SD && s.src_off)) {
                 if (f.T) {
                     const double T = f.T[row_off], rcv = f.rho_cv ? f.rho_cv[row_off] : 1.0;
                     const double Theta = s.a_r * (T * T) * (T * T);
@@ -122,6 +122,7 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
                 }
                 if (f.source_E) dSE -= dt * f.source_E[row_off];
             }
+            if (!SD && s.src_off) { dSE = 0.0; dSFx = 0.0; dSFy = 0.0; }     // semi-implicit step: hyperbolic part only
             const double nE  = uC.E  - fma(rdx, Ge0 - Gw0, fma(rdy, Hn0 - Hs0, dSE));
             const double nFx = uC.Fx - fma(rdx, Ge1 - Gw1, fma(rdy, Hn1 - Hs1, dSFx));
             const double nFy = uC.Fy - fma(rdx, Ge2 - Gw2, fma(rdy, Hn2 - Hs2, dSFy));

@@ -85,7 +85,8 @@ __global__ void __launch_bounds__(ATX * ATY) assemble_kernel(Grid g, Scheme s, F
     face_eval<SD, true>(s, g.c, g.dy, q[3].lmin[1], q[3].lmax[1], q[3].f, u[3].st, q[0].lmin[1], q[0].lmax[1], q[0].f, u[0].st, fs);
     face_eval<SD, true>(s, g.c, g.dy, q[0].lmin[1], q[0].lmax[1], q[0].f, u[0].st, q[4].lmin[1], q[4].lmax[1], q[4].f, u[4].st, fn);
 
-    const double c = g.c, c2 = c * c, rx = dt / g.dx, ry = dt / g.dy;
+    const bool hyp = SD ? true : (s.hyp_off == 0);       // semi-implicit step: source-only system
+    const double c = g.c, c2 = c * c, rx = hyp ? dt / g.dx : 0.0, ry = hyp ? dt / g.dy : 0.0;
     Blk B[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) blk_zero(B[k]);

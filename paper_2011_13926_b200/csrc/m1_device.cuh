@@ -31,8 +31,10 @@ struct Scheme {
     int lin;           // 0: Newton (analytic pressure Jacobian), 1: frozen Eddington tensor
     double eig_floor;
     double a_r;
+    int src_off;       // internal (semi-implicit step): 1 drops the source terms from the explicit update
+    int hyp_off;       // internal (semi-implicit step): 1 drops the flux-divergence terms from the assembled operator
     __host__ __device__ bool is_default() const {
-        return wb == 1 && ap == 1 && eig == 0 && closure == 0 && lin == 0 && eig_floor == 0.0;
+        return wb == 1 && ap == 1 && eig == 0 && closure == 0 && lin == 0 && eig_floor == 0.0 && src_off == 0 && hyp_off == 0;
     }
 };
 
