@@ -311,6 +311,15 @@ def run_ours(args):
     if rank == 0:
         line_extra["explicit"] = explicit_info
         ms_exp = explicit_info["ms_per_step"]
+        _tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+        if os.path.exists(_tp) and n == 4096:
+            with open(_tp) as f:
+                _te = json.load(f).get("explicit", {})
+            if "fp64_pipe_busy_frac" in _te:   # the kernel is ALU bound: fp64 pipe occupancy from the committed ncu capture
+                explicit_info["alu"] = {"bound": "alu", "pipe": "fp64", "frac": _te["fp64_pipe_busy_frac"],
+                                        "issue_slots_frac": _te.get("issue_slots_busy_frac"),
+                                        "peak": "148 SMs x 64 fp64 lanes/clk x SM clock (DESIGN.md section 6)", "source": _te.get("alu_note")}
+                explicit_info["traffic"] = _te.get("dram_bytes")
         # ---- implicit sweep ----------------------------------------------------------------------------------------
         imp, brk = {}, {}
         ratios = SWEEP if not args.no_sweep else (BENCH_DT_RATIO,)
