@@ -393,7 +393,9 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
     const int mi = maxit > h->maxit_alloc ? maxit : h->maxit_alloc;
     // small block: ctl | H | cs | sn | g | y | scale | coef | hist | partial
     if (h->wblock) { cudaFree(h->wblock); h->wblock = nullptr; }
-    const int caphist = mi + mi / (mm > 0 ? mm : 1) + 8;
+    long long caph = (long long)mi + mi / (mm > 0 ? mm : 1) + 8;
+    if (caph > (1LL << 20)) caph = (1LL << 20);     // the history keeps at most 2^20 entries (later ones are counted, not stored)
+    const int caphist = (int)caph;
     const size_t nd = (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 2 * (size_t)(mm + 1) + caphist
                       + (size_t)(krylov_max_blocks(h->sm_count) > op_mf_blocks(h->g, h->sm_count) ? krylov_max_blocks(h->sm_count) : op_mf_blocks(h->g, h->sm_count)) * MAXV;
     const size_t ctl_bytes = (sizeof(GmresCtl) + 255) / 256 * 256;

@@ -183,3 +183,21 @@ def test_nonfinite_state_is_reported():
     g = make_gpu(w)
     with pytest.raises(RuntimeError, match="non-finite"):
         g.step_implicit(_dt(w, 10.0), 1e-10, 30, 100)
+
+
+def test_huge_maxit_and_option_switching_on_one_handle():
+    # history capacity is capped (2^20 entries); operator / Krylov method / restart can change between solves of one handle
+    w = small_random_state(24, 20, seed=47)
+    g = make_gpu(w)
+    o = make_oracle(w)
+    dt = _dt(w, 30.0)
+    o.step_implicit(dt, 1e-11, 30, 4000)
+    want = o.get_state()
+    for opts in (dict(operator=1, krylov=0), dict(operator=0, krylov=0), dict(operator=0, krylov=1), dict(operator=1, krylov=1)):
+        g.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
+        for k, v in opts.items():
+            g.set_option(k, v)
+        its, res = g.step_implicit(dt, 1e-11, 7 if opts["operator"] else 30, 3_000_000)
+        assert res <= 1e-11 and its > 0
+        assert state_rel_l2(g.get_state(), want) <= TOL_IMPLICIT
+        assert len(g.history()) >= 2
