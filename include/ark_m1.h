@@ -90,6 +90,7 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                       right-preconditioned with the same block-Jacobi; `restart` is then ignored and the returned count is in
  *                       BiCGStab iterations (two operator applications each)
  *   "vectors_per_pass"  basis vectors handled per pass of the multi-dot / multi-axpy kernels, 1..32 (default 16, by measurement)
+ *   "basis_pad"         extra doubles (multiple of 32) between consecutive Krylov basis vectors (default 0; measured: no effect)
  *   "kernel_timing"     1: time every kernel launch with CUDA events (see ark_m1_get_kernel_stats); default 0
  *   "explicit_kernel"   0: one-thread-per-cell kernel   1: row-marching kernel (default)   2: barrier-free warp-shuffle kernel
  *                       3: row-marching kernel with a three-slot register rotation (no window copies)
