@@ -47,6 +47,23 @@ SWEEP = (10.0, 50.0, 100.0, 200.0)
 PAPER_BREAK_EVEN = "50-100x (relaxation preconditioner; CPU 50, K80 GPU 100; PAPER.md:369)"
 
 
+def load_ncu_traffic():
+    """profiles/ncu_traffic.csv: measured DRAM bytes over algorithmic bytes per kernel class (copied from the ncu captures)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    out = {}
+    if os.path.exists(path):
+        with open(path, newline="") as f:
+            for row in csv.DictReader(f):
+                d = {"captured": row["captured"], "dram_bytes": float(row["dram_bytes"]), "alg_bytes": float(row["alg_bytes"]),
+                     "ratio": float(row["ratio"]), "note": row["note"], "alu_note": row["note"]}
+                if row["fp64_pipe_busy_frac"]:
+                    d["fp64_pipe_busy_frac"] = float(row["fp64_pipe_busy_frac"])
+                    d["issue_slots_busy_frac"] = float(row["issue_slots_busy_frac"])
+                out[row["class"]] = d
+    return out
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -311,10 +328,9 @@ def run_ours(args):
     if rank == 0:
         line_extra["explicit"] = explicit_info
         ms_exp = explicit_info["ms_per_step"]
-        _tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")
-        if os.path.exists(_tp) and n == 4096:
-            with open(_tp) as f:
-                _te = json.load(f).get("explicit", {})
+        traffic = load_ncu_traffic()
+        if n == 4096:
+            _te = traffic.get("explicit", {})
             if "fp64_pipe_busy_frac" in _te:   # the kernel is ALU bound: fp64 pipe occupancy from the committed ncu capture
                 explicit_info["alu"] = {"bound": "alu", "pipe": "fp64", "frac": _te["fp64_pipe_busy_frac"],
                                         "issue_slots_frac": _te.get("issue_slots_busy_frac"),
@@ -433,11 +449,6 @@ def run_ours(args):
             g5.close()
             del d5
         # ---- roofline of the dominant kernel class ---------------------------------------------------------------
-        traffic = {}
-        tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
-        if os.path.exists(tpath):
-            with open(tpath) as f:
-                traffic = json.load(f)
         tot_ms = sum(v["ms"] for v in stats.values()) or 1.0
         kern = {}
         for name, v in stats.items():
