@@ -6,6 +6,7 @@
 namespace ark {
 
 static constexpr int KTHREADS = 256;
+static constexpr int EPI_MAX = 128;      // Hessenberg columns up to this length are staged in shared memory for the Givens epilogue
 
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -22,7 +23,8 @@ __device__ __forceinline__ void hist_push(const GmresWork& W, GmresCtl* c, doubl
 }
 
 // Scalar epilogues, run by one thread after a reduction has produced d[0..nv).
-__device__ __forceinline__ void epilogue(const GmresWork& W, int mode, const double* d, int nv, int col0)
+__device__ __forceinline__ void epilogue(const GmresWork& W, int mode, const double* d, int nv, int col0,
+                                         const double* hcol = nullptr, const double* ccs = nullptr, const double* ssn = nullptr)
 {
     GmresCtl* c = W.ctl;
     const int m = c->m;
@@ -74,10 +76,22 @@ __device__ __forceinline__ void epilogue(const GmresWork& W, int mode, const dou
         const double hn = sqrt(d[0]);
         double* H = W.H;
         H[(j + 1) * m + j] = hn;
-        for (int i = 0; i < j; ++i) {
-            const double a = H[i * m + j], b = H[(i + 1) * m + j];
-            H[i * m + j] = W.cs[i] * a + W.sn[i] * b;
-            H[(i + 1) * m + j] = -W.sn[i] * a + W.cs[i] * b;
+        if (hcol) {
+            // column j, cs, sn were staged in shared memory by the whole block: the rotation chain runs on registers and
+            // shared memory instead of a dependent global load/store pair per step (it was ~1 us per previous rotation)
+            double carry = hcol[0];
+            for (int i = 0; i < j; ++i) {
+                const double nxt = hcol[i + 1];
+                H[i * m + j] = ccs[i] * carry + ssn[i] * nxt;
+                carry = -ssn[i] * carry + ccs[i] * nxt;
+            }
+            H[j * m + j] = carry;
+        } else {
+            for (int i = 0; i < j; ++i) {
+                const double a = H[i * m + j], b = H[(i + 1) * m + j];
+                H[i * m + j] = W.cs[i] * a + W.sn[i] * b;
+                H[(i + 1) * m + j] = -W.sn[i] * a + W.cs[i] * b;
+            }
         }
         const double a = H[j * m + j], b = H[(j + 1) * m + j];
         const double r = hypot(a, b);
@@ -131,6 +145,16 @@ __device__ __forceinline__ void reduce_and_finish(double (&acc)[NV], const Gmres
         for (unsigned int b = lane; b < nb; b += 32) s += __ldcg(&W.partial[(size_t)b * MAXV + k]);
         s = warp_sum(s);
         if (lane == 0) dres[k] = s;
+    }
+    if (mode == DOT_UPD) {
+        // stage column j of H (rows 0..j; row j+1 is ||w|| itself), cs and sn for the scalar epilogue
+        __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
+        const int j = W.ctl->j, m = W.ctl->m;
+        const bool staged = (j < EPI_MAX);
+        if (staged) for (int i = threadIdx.x; i <= j; i += NT) { hcol[i] = W.H[i * m + j]; if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; } }
+        __syncthreads();
+        if (threadIdx.x == 0) epilogue(W, mode, dres, NV, col0, staged ? hcol : nullptr, ccs, ssn);
+        return;
     }
     __syncthreads();
     if (threadIdx.x == 0) epilogue(W, mode, dres, NV, col0);
