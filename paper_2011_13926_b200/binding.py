@@ -24,7 +24,7 @@ SYMBOLS = [
     "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
     "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_step_semi_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
-    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_device_bytes",
+    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_fastmath_errors", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
 ]
 
@@ -74,6 +74,7 @@ def load_library(path: str | None = None):
     L.ark_m1_kernel_class_name.argtypes = [i]
     L.ark_m1_kernel_launches.restype = C.c_longlong
     L.ark_m1_kernel_launches.argtypes = [vp]
+    L.ark_m1_fastmath_errors.argtypes = [i, C.POINTER(C.c_double)]
     L.ark_m1_device_bytes.restype = C.c_longlong
     L.ark_m1_device_bytes.argtypes = [vp]
     L.ark_m1_last_error.restype = C.c_char_p
@@ -239,6 +240,15 @@ class ArkM1:
 
     def device_bytes(self):
         return int(self._L.ark_m1_device_bytes(self._h))
+
+
+def fastmath_errors(n=1 << 20):
+    """Max relative errors (rcp_fast, rsqrt_fast, sqrt via rsqrt) of the kernels' fast fp64 forms against IEEE, measured on the GPU."""
+    buf = (C.c_double * 3)()
+    rc = load_library().ark_m1_fastmath_errors(int(n), buf)
+    if rc < 0:
+        raise RuntimeError(f"ark_m1_fastmath_errors failed ({rc})")
+    return tuple(buf)
 
 
 def version():

@@ -702,3 +702,17 @@ extern "C" int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap)
 }
 extern "C" const char* ark_m1_kernel_class_name(int k) { return (k >= 0 && k < KC_COUNT) ? kc_names[k] : ""; }
 extern "C" long long ark_m1_kernel_launches(const ark_m1* h) { return h ? h->launches : 0; }
+
+// Self-test of the fast reciprocal / reciprocal square root used by the hot kernels: max relative errors against the IEEE
+// sequences over n samples in 200 binades.  No handle needed.  Returns 0 or ARK_M1_E_CUDA.
+extern "C" int ark_m1_fastmath_errors(int n, double* out3)
+{
+    if (!out3 || n < 1) return ARK_M1_E_ARG;
+    double* d = nullptr;
+    if (cudaMalloc((void**)&d, 3 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return ARK_M1_E_ALLOC; }
+    cudaError_t e = cudaMemset(d, 0, 3 * sizeof(double));
+    if (e == cudaSuccess) e = launch_fastmath_selftest(n, d, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(out3, d, 3 * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    return e == cudaSuccess ? 0 : ARK_M1_E_CUDA;
+}

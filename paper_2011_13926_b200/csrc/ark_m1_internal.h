@@ -62,6 +62,7 @@ cudaError_t launch_explicit_warp(const Grid& g, const Scheme& s, const Fields& f
 cudaError_t launch_velocity_sources(const Grid& g, const Scheme& s, const Fields& f, const double* ux, const double* uy,
                                     double dt, double* E, double* Fx, double* Fy, cudaStream_t st);
 cudaError_t launch_count_unrealizable(const Grid& g, const Fields& f, unsigned long long* counts2, cudaStream_t st);
+cudaError_t launch_fastmath_selftest(int n, double* out3, cudaStream_t st);
 cudaError_t launch_add_planes(double* st_out, const double* a, const double* b, long long n, cudaStream_t st);
 
 // implicit_kernels.cu
