@@ -49,6 +49,7 @@ enum { BLK_C = 0, BLK_W = 1, BLK_E = 2, BLK_S = 3, BLK_N = 4 };
 
 #define E_FLOOR 1e-300   /* R1: E <= 0 is only guarded in the division f = |F|/(cE) */
 
+struct mg_hier;
 typedef struct oracle_m1 {
     int nx, ny;
     double dx, dy, c;
@@ -65,6 +66,10 @@ typedef struct oracle_m1 {
     int src_off;     /* internal (semi-implicit step): 1 drops the source terms from the residual */
     int hyp_off;     /* internal (semi-implicit step): 1 drops the flux-divergence terms from the assembled operator */
     int krylov;      /* 0: restarted GMRES (north_star, default), 1: BiCGStab (the paper's solver) */
+    int precond_kind;/* 0: 3x3 block-Jacobi (north_star, default), 1: multigrid V-cycle (R12) */
+    double mg_omega; /* damping of the block-Jacobi smoother, default 0.8 */
+    int mg_coarse_sweeps; /* smoother sweeps on the coarsest (1x1) level, default 2 */
+    struct mg_hier *mg;   /* hierarchy of the solve in progress (built by mg_build, freed after the solve) */
     double eig_floor;/* lambda^+ >= floor*c, lambda^- <= -floor*c; default 0 */
     double a_r;      /* radiation constant, default 1 */
     double *rho_cv, *ux, *uy, *source_E; /* stage-2 fields (may be NULL) */
@@ -516,6 +521,145 @@ static void precond(const system_t *s, const double *v, double *z)
         z[id] = zz[0]; z[N + id] = zz[1]; z[2 * N + id] = zz[2];
     }
 }
+/* ------------------------------------------------------------------------------------------------ */
+/* Multigrid preconditioner (the five steps quoted from Saad 2003; R12)  */
+/* ------------------------------------------------------------------------------------------------ */
+/* The paper uses an algebraic multigrid from a library (MueLu) and does not specify it.  On this structured grid the
+ * hierarchy is geometric: aggregates of 2x2 cells (the last one in a direction is 1 wide when the size is odd), down to
+ * a single cell.  On every level, with D = the 3x3 diagonal blocks:
+ *   restriction        R = P0^T   (sum over the aggregate; P0 = piecewise-constant injection, per component)
+ *   interpolation      P = D^-1 P0   (piecewise constant in the block-Jacobi-scaled variable D x)
+ *   coarse operator    R A P   ("R A P y = R r~") -- again a 5-point stencil of 3x3 blocks
+ *   smoother           damped block-Jacobi, z += omega D^-1 (r - A z)   ("a simple method such as Jacobi")
+ * One V-cycle, zero initial guess, one pre- and one post-smoothing sweep (steps 1-5 of PAPER.md:283-287); on the
+ * coarsest level `mg_coarse_sweeps` smoother sweeps replace the direct solve of step 3. */
+typedef struct mg_hier {
+    int nlev;
+    int nx[32], ny[32];
+    system_t lev[32];            /* lev[0] aliases the fine system (not owned); b unused on coarse levels */
+    double *r[32], *z[32], *t[32];   /* work vectors per level (r[0] unused) */
+} mg_hier;
+
+static void inv3(const double *B, double *Bi)   /* Bi = B^-1 by three solves (Gaussian elimination with pivoting) */
+{
+    for (int k = 0; k < 3; ++k) {
+        const double e[3] = { k == 0, k == 1, k == 2 }; double z[3];
+        solve3(B, e, z);
+        for (int r = 0; r < 3; ++r) Bi[3 * r + k] = z[r];
+    }
+}
+
+/* Coarse system R A P of one level. */
+static int mg_coarsen(const system_t *f, int nx, int ny, system_t *c, int *cnx, int *cny)
+{
+    const int cx = (nx + 1) / 2, cy = (ny + 1) / 2;
+    const long Nc = (long)cx * cy;
+    c->N = Nc; c->b = NULL;
+    c->A = (double *)calloc((size_t)45 * Nc, sizeof(double));
+    c->col = (long *)malloc(sizeof(long) * 5 * Nc);
+    if (!c->A || !c->col) return -3;
+    for (long k = 0; k < 5 * Nc; ++k) c->col[k] = -1;
+    for (long a = 0; a < Nc; ++a) c->col[5 * a + BLK_C] = a;
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            const long id = (long)j * nx + i, a = (long)(j / 2) * cx + i / 2;
+            for (int k = 0; k < 5; ++k) {
+                const long cj = f->col[5 * id + k]; if (cj < 0) continue;
+                double Di[9], B[9];
+                inv3(f->A + 45 * cj, Di);                       /* D^-1 of the column cell */
+                const double *Ak = f->A + 45 * id + 9 * k;
+                for (int r = 0; r < 3; ++r) for (int q = 0; q < 3; ++q)
+                    B[3 * r + q] = Ak[3 * r] * Di[q] + Ak[3 * r + 1] * Di[3 + q] + Ak[3 * r + 2] * Di[6 + q];
+                const long ac = (cj / nx / 2) * cx + (cj % nx) / 2;     /* aggregate of the column cell */
+                const int kc = (ac == a) ? BLK_C : k;           /* inside the aggregate -> diagonal block */
+                add_block(c->A + 45 * a + 9 * kc, B);
+                c->col[5 * a + kc] = ac;
+            }
+        }
+    *cnx = cx; *cny = cy;
+    return 0;
+}
+
+static void mg_free(mg_hier *m)
+{
+    if (!m) return;
+    for (int l = 0; l < m->nlev; ++l) {
+        if (l > 0) { free(m->lev[l].A); free(m->lev[l].col); }
+        free(m->r[l]); free(m->z[l]); free(m->t[l]);
+    }
+    free(m);
+}
+
+static mg_hier *mg_build(const oracle_m1 *h, const system_t *s)
+{
+    mg_hier *m = (mg_hier *)calloc(1, sizeof(mg_hier));
+    if (!m) return NULL;
+    m->lev[0] = *s; m->nx[0] = h->nx; m->ny[0] = h->ny; m->nlev = 1;
+    while ((m->nx[m->nlev - 1] > 1 || m->ny[m->nlev - 1] > 1) && m->nlev < 32) {
+        const int l = m->nlev;
+        if (mg_coarsen(&m->lev[l - 1], m->nx[l - 1], m->ny[l - 1], &m->lev[l], &m->nx[l], &m->ny[l])) { m->nlev = l + 1; mg_free(m); return NULL; }
+        m->nlev = l + 1;
+    }
+    for (int l = 0; l < m->nlev; ++l) {
+        const size_t n = 3 * (size_t)m->lev[l].N;
+        m->r[l] = (double *)malloc(sizeof(double) * n); m->z[l] = (double *)malloc(sizeof(double) * n); m->t[l] = (double *)malloc(sizeof(double) * n);
+        if (!m->r[l] || !m->z[l] || !m->t[l]) { mg_free(m); return NULL; }
+    }
+    return m;
+}
+
+/* z += omega D^-1 (r - A z); `first` = 1: z = omega D^-1 r (zero initial guess).  t: work vector. */
+static void mg_smooth(const system_t *s, double omega, const double *r, double *z, double *t, int first)
+{
+    const long n = 3 * s->N;
+    if (first) { precond(s, r, z); for (long k = 0; k < n; ++k) z[k] *= omega; return; }
+    spmv(s, z, t);
+    for (long k = 0; k < n; ++k) t[k] = r[k] - t[k];
+    double *d = (double *)malloc(sizeof(double) * n);
+    precond(s, t, d);
+    for (long k = 0; k < n; ++k) z[k] += omega * d[k];
+    free(d);
+}
+
+/* One V-cycle on level l: z ~ A_l^-1 r (steps 1-5 of PAPER.md:283-287). */
+static void mg_vcycle(const oracle_m1 *h, mg_hier *m, int l, const double *r, double *z)
+{
+    const system_t *s = &m->lev[l];
+    const long N = s->N;
+    double *t = m->t[l];
+    mg_smooth(s, h->mg_omega, r, z, t, 1);                                   /* 1. pre-smoothing */
+    if (l == m->nlev - 1) {                                                  /* coarsest level: more sweeps instead of a direct solve */
+        for (int k = 1; k < h->mg_coarse_sweeps; ++k) mg_smooth(s, h->mg_omega, r, z, t, 0);
+        return;
+    }
+    const int nx = m->nx[l], ny = m->ny[l], cx = m->nx[l + 1];
+    const long Nc = m->lev[l + 1].N;
+    double *rc = m->r[l + 1], *zc = m->z[l + 1];
+    spmv(s, z, t);                                                           /* 2. residual, restricted: rc = P0^T (r - A z) */
+    memset(rc, 0, sizeof(double) * 3 * Nc);
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            const long id = (long)j * nx + i, a = (long)(j / 2) * cx + i / 2;
+            for (int q = 0; q < 3; ++q) rc[q * Nc + a] += r[q * N + id] - t[q * N + id];
+        }
+    mg_vcycle(h, m, l + 1, rc, zc);                                          /* 3. coarse problem, recursively */
+    for (int j = 0; j < ny; ++j)                                             /* 4. interpolation: z += D^-1 P0 zc */
+        for (int i = 0; i < nx; ++i) {
+            const long id = (long)j * nx + i, a = (long)(j / 2) * cx + i / 2;
+            const double e[3] = { zc[a], zc[Nc + a], zc[2 * Nc + a] }; double d[3];
+            solve3(s->A + 45 * id, e, d);
+            for (int q = 0; q < 3; ++q) z[q * N + id] += d[q];
+        }
+    mg_smooth(s, h->mg_omega, r, z, t, 0);                                   /* 5. post-smoothing */
+}
+
+/* The right preconditioner of the Krylov solvers: block-Jacobi (Eq. 27 block-wise) or one multigrid V-cycle. */
+static void apply_precond(const oracle_m1 *h, const system_t *s, const double *v, double *z)
+{
+    if (h->precond_kind == 1 && h->mg) mg_vcycle(h, h->mg, 0, v, z);
+    else precond(s, v, z);
+}
+
 static double dot(const double *a, const double *b, long n)
 {
     double sacc = 0.0;
@@ -562,7 +706,7 @@ static int gmres(oracle_m1 *h, const system_t *s, double *x, double tol, int m, 
         int j = 0;
         for (; j < m && its < maxit; ) {
             double *vj = V + (size_t)j * n, *vn = V + (size_t)(j + 1) * n;
-            precond(s, vj, z);
+            apply_precond(h, s, vj, z);
             spmv(s, z, vn);
             for (int i = 0; i <= j; ++i) {                       /* modified Gram-Schmidt */
                 const double *vi = V + (size_t)i * n;
@@ -597,7 +741,7 @@ static int gmres(oracle_m1 *h, const system_t *s, double *x, double tol, int m, 
         }
         #pragma omp parallel for schedule(static)
         for (long k = 0; k < n; ++k) { double sacc = 0.0; for (int i = 0; i < j; ++i) sacc += y[i] * V[(size_t)i * n + k]; w[k] = sacc; }
-        precond(s, w, z);                                        /* x += M^-1 (V y) */
+        apply_precond(h, s, w, z);                                        /* x += M^-1 (V y) */
         #pragma omp parallel for schedule(static)
         for (long k = 0; k < n; ++k) x[k] += z[k];
     }
@@ -637,12 +781,12 @@ static int bicgstab(oracle_m1 *h, const system_t *s, double *x, double tol, int 
             if (rho_new == 0.0 || omega == 0.0) break;                 /* breakdown: restart from the true residual */
             const double beta = (rho_new / rho) * (alpha / omega);
             for (long k = 0; k < n; ++k) p[k] = r[k] + beta * (p[k] - omega * v[k]);
-            precond(s, p, ph); spmv(s, ph, v);
+            apply_precond(h, s, p, ph); spmv(s, ph, v);
             const double rhv = dot(rh, v, n);
             if (rhv == 0.0) break;
             alpha = rho_new / rhv;
             for (long k = 0; k < n; ++k) r[k] -= alpha * v[k];          /* s, stored in r */
-            precond(s, r, sh); spmv(s, sh, t);
+            apply_precond(h, s, r, sh); spmv(s, sh, t);
             const double tt = dot(t, t, n);
             omega = (tt > 0.0) ? dot(t, r, n) / tt : 0.0;
             for (long k = 0; k < n; ++k) { x[k] += alpha * ph[k] + omega * sh[k]; r[k] -= omega * t[k]; }
@@ -658,6 +802,43 @@ static int bicgstab(oracle_m1 *h, const system_t *s, double *x, double tol, int 
     return its;
 }
 
+/* Krylov solve of one assembled system with the chosen method and preconditioner. */
+static int solve_linear(oracle_m1 *h, const system_t *s, double *x, double tol, int restart, int maxit, double *relres)
+{
+    h->mg = NULL;
+    if (h->precond_kind == 1 && !(h->mg = mg_build(h, s))) return -3;
+    const int its = h->krylov == 1 ? bicgstab(h, s, x, tol, maxit, relres) : gmres(h, s, x, tol, restart, maxit, relres);
+    mg_free(h->mg); h->mg = NULL;
+    return its;
+}
+
+/* Test hooks for the multigrid preconditioner: one V-cycle z = M^-1 r on the system assembled for dt ... */
+ORACLE_API int oracle_m1_mg_apply(oracle_m1 *h, double dt, const double *r, double *z)
+{
+    system_t s; int rc = system_build(h, dt, NULL, &s); if (rc) return rc;
+    mg_hier *m = mg_build(h, &s);
+    if (!m) { system_free(&s); return -3; }
+    mg_vcycle(h, m, 0, r, z);
+    mg_free(m); system_free(&s);
+    return 0;
+}
+/* ... and the blocks of level `level` (0 = fine): returns the number of levels; dims = {nx, ny} of that level; A, col may
+ * be NULL to query the sizes only. */
+ORACLE_API int oracle_m1_mg_level(oracle_m1 *h, double dt, int level, double *A, long *col, int *dims)
+{
+    system_t s; int rc = system_build(h, dt, NULL, &s); if (rc) return rc;
+    mg_hier *m = mg_build(h, &s);
+    if (!m) { system_free(&s); return -3; }
+    const int nlev = m->nlev;
+    if (level >= 0 && level < nlev) {
+        dims[0] = m->nx[level]; dims[1] = m->ny[level];
+        if (A) memcpy(A, m->lev[level].A, sizeof(double) * 45 * m->lev[level].N);
+        if (col) memcpy(col, m->lev[level].col, sizeof(long) * 5 * m->lev[level].N);
+    }
+    mg_free(m); system_free(&s);
+    return nlev;
+}
+
 /* One linearised implicit step (R4): (I + dt L_n) U^{n+1} = U^n + affine terms; then the T update (R10). */
 ORACLE_API int oracle_m1_step_implicit(oracle_m1 *h, double dt, double tol, int restart, int maxit, double *final_residual)
 {
@@ -667,7 +848,7 @@ ORACLE_API int oracle_m1_step_implicit(oracle_m1 *h, double dt, double tol, int 
     double *x = (double *)malloc(sizeof(double) * 3 * N);
     memcpy(x, h->E, sizeof(double) * N); memcpy(x + N, h->Fx, sizeof(double) * N); memcpy(x + 2 * N, h->Fy, sizeof(double) * N);
     double rel = 0.0;
-    const int its = h->krylov == 1 ? bicgstab(h, &s, x, tol, maxit, &rel) : gmres(h, &s, x, tol, restart, maxit, &rel);
+    const int its = solve_linear(h, &s, x, tol, restart, maxit, &rel);
     if (its >= 0) {
         if (h->has_T) {
             #pragma omp parallel for schedule(static)
@@ -705,7 +886,7 @@ ORACLE_API int oracle_m1_step_implicit_newton(oracle_m1 *h, double dt, double to
     for (k = 0; k < max_newton; ++k) {
         system_t s; const int rc = system_build(h, dt, base, &s); if (rc) { free(base); free(x); return rc; }
         memcpy(x, h->E, sizeof(double) * N); memcpy(x + N, h->Fx, sizeof(double) * N); memcpy(x + 2 * N, h->Fy, sizeof(double) * N);
-        const int its = h->krylov == 1 ? bicgstab(h, &s, x, tol, maxit, &rel) : gmres(h, &s, x, tol, restart, maxit, &rel);
+        const int its = solve_linear(h, &s, x, tol, restart, maxit, &rel);
         system_free(&s);
         if (its < 0) { free(base); free(x); return its; }
         total += its;
@@ -795,7 +976,7 @@ ORACLE_API oracle_m1 *oracle_m1_create(int nx, int ny, double dx, double dy, dou
     h->E = (double *)calloc(N, sizeof(double)); h->Fx = (double *)calloc(N, sizeof(double)); h->Fy = (double *)calloc(N, sizeof(double));
     h->sa = (double *)calloc(N, sizeof(double)); h->st = (double *)calloc(N, sizeof(double)); h->T = (double *)calloc(N, sizeof(double));
     for (int s = 0; s < 4; ++s) { const size_t len = (s < 2) ? ny : nx; for (int k = 0; k < 5; ++k) h->gh[s][k] = (double *)calloc(len, sizeof(double)); }
-    h->wb = 1; h->ap = 1; h->eig = 0; h->closure = 0; h->lin = 0; h->eig_floor = 0.0; h->a_r = 1.0;
+    h->wb = 1; h->ap = 1; h->eig = 0; h->closure = 0; h->lin = 0; h->eig_floor = 0.0; h->a_r = 1.0; h->mg_omega = 0.8; h->mg_coarse_sweeps = 2;
     return h;
 }
 
@@ -839,6 +1020,9 @@ ORACLE_API int oracle_m1_set_option(oracle_m1 *h, const char *key, double value)
     else if (!strcmp(key, "linearisation")) h->lin = (int)value;
     else if (!strcmp(key, "eig_floor")) h->eig_floor = value;
     else if (!strcmp(key, "krylov")) h->krylov = (int)value;
+    else if (!strcmp(key, "preconditioner")) h->precond_kind = (int)value;
+    else if (!strcmp(key, "mg_omega")) h->mg_omega = value;
+    else if (!strcmp(key, "mg_coarse_sweeps")) h->mg_coarse_sweeps = (int)value;
     else if (!strcmp(key, "a_r")) h->a_r = value;
     else { snprintf(h->err, sizeof h->err, "unknown option %s", key); return -1; }
     return 0;

@@ -55,6 +55,8 @@ def lib():
         L.oracle_m1_apply_linear.argtypes = [C.c_void_p, C.c_double, dp, dp, C.c_int]
         L.oracle_m1_assemble.argtypes = [C.c_void_p, C.c_double, dp, lp, dp]
         L.oracle_m1_count_unrealizable.argtypes = [C.c_void_p, lp, lp]
+        L.oracle_m1_mg_apply.argtypes = [C.c_void_p, C.c_double, dp, dp]
+        L.oracle_m1_mg_level.argtypes = [C.c_void_p, C.c_double, C.c_int, dp, lp, ip]
         L.oracle_m1_get_history.argtypes = [C.c_void_p, dp, C.c_int]
         L.oracle_m1_last_error.restype = C.c_char_p
         L.oracle_m1_last_error.argtypes = [C.c_void_p]
@@ -187,6 +189,23 @@ class OracleM1:
                     for s in range(3):
                         M[r * N + cell, s * N + cj] += A[cell, k, r, s]
         return M, b.reshape(-1)
+
+    def mg_apply(self, dt, R):
+        """One multigrid V-cycle z = M^-1 r on the system assembled for dt (planes [3, ny, nx])."""
+        R = _f64(R, (3,) + self.shape)
+        out = np.empty_like(R)
+        self._check(lib().oracle_m1_mg_apply(self._h, float(dt), _p(R), _p(out)))
+        return out
+
+    def mg_level(self, dt, level):
+        """(number of levels, nx_l, ny_l, A[N_l,5,3,3], col[N_l,5]) of one level of the multigrid hierarchy."""
+        dims = (C.c_int * 2)()
+        n = lib().oracle_m1_mg_level(self._h, float(dt), int(level), None, None, dims)
+        self._check(min(n, 0))
+        nx, ny = dims[0], dims[1]
+        A = np.empty((nx * ny, 5, 3, 3)); col = np.empty((nx * ny, 5), dtype=np.int64)
+        lib().oracle_m1_mg_level(self._h, float(dt), int(level), _p(A), col.ctypes.data_as(C.POINTER(C.c_long)), dims)
+        return n, nx, ny, A, col
 
     def count_unrealizable(self):
         a, b = C.c_long(0), C.c_long(0)
