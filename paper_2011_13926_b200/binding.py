@@ -24,7 +24,7 @@ SYMBOLS = [
     "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
     "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_step_semi_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
-    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_fastmath_errors", "ark_m1_device_bytes",
+    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_fastmath_errors", "ark_m1_apply_preconditioner", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
 ]
 
@@ -67,6 +67,7 @@ def load_library(path: str | None = None):
     L.ark_m1_count_unrealizable.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.ark_m1_residual.argtypes = [vp, dp, dp]
     L.ark_m1_apply_operator.argtypes = [vp, d, dp, dp, dp]
+    L.ark_m1_apply_preconditioner.argtypes = [vp, d, dp, dp]
     L.ark_m1_get_history.argtypes = [vp, C.POINTER(C.c_double), i]
     L.ark_m1_get_timings.argtypes = [vp, C.POINTER(C.c_double)]
     L.ark_m1_get_kernel_stats.argtypes = [vp, C.POINTER(C.c_double), i]
@@ -216,6 +217,12 @@ class ArkM1:
         b = np.empty((3, self.ny, self.nx)) if with_b else None
         self._check(self._L.ark_m1_apply_operator(self._h, float(dt), p, out.ctypes.data, None if b is None else b.ctypes.data))
         return (out, b) if with_b else out
+
+    def apply_preconditioner(self, dt, V):
+        p, keep = _ptr(V, 3 * self.N)
+        out = np.empty((3, self.ny, self.nx))
+        self._check(self._L.ark_m1_apply_preconditioner(self._h, float(dt), p, out.ctypes.data))
+        return out
 
     def history(self):
         n = self._L.ark_m1_get_history(self._h, None, 0)

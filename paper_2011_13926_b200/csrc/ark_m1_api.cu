@@ -14,9 +14,9 @@
 using namespace ark;
 
 // kernel classes for the launch statistics
-enum { KC_EXPLICIT = 0, KC_ASSEMBLE, KC_SCALE, KC_DIAGMUL, KC_SPMV, KC_DOT, KC_UPDATE, KC_COMBINE, KC_SMALL, KC_COUNT };
+enum { KC_EXPLICIT = 0, KC_ASSEMBLE, KC_SCALE, KC_DIAGMUL, KC_SPMV, KC_DOT, KC_UPDATE, KC_COMBINE, KC_SMALL, KC_MG, KC_MGSETUP, KC_COUNT };
 static const char* const kc_names[KC_COUNT] = { "explicit", "assemble", "scale_offdiag", "diag_mul", "spmv_hat", "multi_dot",
-                                                 "update_norm", "combine", "small" };
+                                                 "update_norm", "combine", "small", "mg_vcycle", "mg_setup" };
 
 struct ark_m1 {
     Grid g;
@@ -35,6 +35,10 @@ struct ark_m1 {
     unsigned long long* counts;   // 2
     // options
     int ortho, explicit_kernel, op_kind, maxv, basis_pad, krylov, asm_kernel;
+    int precond;       // 0: 3x3 block-Jacobi, 1: multigrid V-cycle (forces the assembled block-stencil operator)
+    MgHier mg;         // hierarchy (levels >= 1 allocated lazily)
+    double* mgz;       // 3N: V-cycle output (hat variable)
+    double mg_cells;   // sum over levels of cells / N (for the byte counts)
     // implicit workspace (lazy)
     BlockMatrix A;
     MfPlanes mf;       // matrix-free coefficient planes (op_kind == 1)
@@ -100,6 +104,9 @@ static int dmalloc(ark_m1* h, void** p, size_t bytes)
     return 0;
 }
 
+// the multigrid hierarchy is built from assembled blocks: it overrides the matrix-free operator
+static inline int opk(const ark_m1* h) { return h->precond == 1 ? 0 : h->op_kind; }
+
 static Fields fields_of(const ark_m1* h)
 {
     Fields f;
@@ -131,6 +138,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
     h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0; h->asm_kernel = 1;
+    h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     h->hist_host = new std::vector<double>();
@@ -157,6 +165,8 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
 
 static void free_implicit(ark_m1* h)
 {
+    for (int l = 1; l < h->mg.nlev; ++l) { cudaFree(h->mg.lev[l].off); cudaFree(h->mg.lev[l].Dinv); cudaFree(h->mg.lev[l].r); cudaFree(h->mg.lev[l].e); }
+    h->mg.nlev = 0; cudaFree(h->mgz); h->mgz = nullptr;
     cudaFree(h->A.off); cudaFree(h->A.C); cudaFree(h->A.Minv); cudaFree(h->A.b); cudaFree(h->V); cudaFree(h->tvec); cudaFree(h->wblock); cudaFree(h->nprev); h->nprev = nullptr;
     cudaFree(h->mf.J); cudaFree(h->mf.fE); cudaFree(h->mf.fN); cudaFree(h->mf.dE); cudaFree(h->mf.dF); cudaFree(h->mf.xlo); cudaFree(h->mf.ylo);
     memset(&h->mf, 0, sizeof h->mf);
@@ -243,6 +253,9 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "basis_pad")) { if (iv < 0 || (iv & 31)) return fail(h, ARK_M1_E_ARG, "basis_pad must be a non-negative multiple of 32 doubles%s", ""); if (iv != h->basis_pad) { cudaStreamSynchronize(h->st); free_implicit(h); } h->basis_pad = iv; }
     else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
+    else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
+    else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
+    else if (!strcmp(key, "mg_coarse_sweeps")) { if (iv < 1) return fail(h, ARK_M1_E_ARG, "mg_coarse_sweeps must be >= 1%s", ""); h->mg.coarse_sweeps = iv; }
     else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
     return 0;
 }
@@ -357,8 +370,8 @@ const char* ark_m1_last_error(const ark_m1* h) { return h ? h->err : "null handl
 static int ensure_implicit(ark_m1* h, int m, int maxit)
 {
     const size_t N = (size_t)h->N, n = 3 * N;
-    const bool have_op = (h->op_kind == 0) ? (h->A.off != nullptr) : (h->mf.J != nullptr);
-    if (h->m_alloc >= m && h->maxit_alloc >= maxit && have_op) return 0;
+    const bool have_op = (opk(h) == 0) ? (h->A.off != nullptr) : (h->mf.J != nullptr);
+    if (h->m_alloc >= m && h->maxit_alloc >= maxit && have_op && (h->precond == 0 || h->mg.nlev > 0)) return 0;
     CU(cudaStreamSynchronize(h->st));
     const long long before = h->bytes;
     (void)before;
@@ -368,12 +381,12 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
         if ((rc = dmalloc(h, (void**)&h->A.b, n * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->tvec, n * sizeof(double)))) return rc;
     }
-    if (h->op_kind == 0 && h->A.off == nullptr) {
+    if (opk(h) == 0 && h->A.off == nullptr) {
         int rc;
         if ((rc = dmalloc(h, (void**)&h->A.off, 36 * N * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->A.C, 9 * N * sizeof(double)))) return rc;
     }
-    if (h->op_kind == 1 && h->mf.J == nullptr) {
+    if (opk(h) == 1 && h->mf.J == nullptr) {
         int rc;
         if ((rc = dmalloc(h, (void**)&h->mf.J, 9 * N * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->mf.fE, 4 * N * sizeof(double)))) return rc;
@@ -382,6 +395,28 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
         if ((rc = dmalloc(h, (void**)&h->mf.dF, N * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->mf.xlo, 4 * (size_t)h->g.ny * sizeof(double)))) return rc;
         if ((rc = dmalloc(h, (void**)&h->mf.ylo, 4 * (size_t)h->g.nx * sizeof(double)))) return rc;
+    }
+    if (h->precond == 1 && h->mg.nlev == 0) {       // levels 1.. of the multigrid hierarchy (about 1/3 of the fine storage)
+        int rc;
+        if ((rc = dmalloc(h, (void**)&h->mgz, n * sizeof(double)))) return rc;
+        MgHier& H = h->mg;
+        H.lev[0].g = h->g; H.lev[0].off = nullptr; H.lev[0].Dinv = nullptr; H.lev[0].r = nullptr; H.lev[0].e = nullptr;
+        int L = 1; double cells = 1.0;
+        while ((H.lev[L - 1].g.nx > 1 || H.lev[L - 1].g.ny > 1) && L < MG_MAXLEV) {
+            MgLevel& c = H.lev[L];
+            c.g = H.lev[L - 1].g; c.g.nx = (c.g.nx + 1) / 2; c.g.ny = (c.g.ny + 1) / 2;
+            const size_t Nc = (size_t)c.g.nx * c.g.ny;
+            c.off = c.Dinv = c.r = c.e = nullptr;
+            H.nlev = L + 1;                          // so that a failure below frees what was allocated
+            if ((rc = dmalloc(h, (void**)&c.off, 36 * Nc * sizeof(double)))) return rc;
+            if ((rc = dmalloc(h, (void**)&c.Dinv, 9 * Nc * sizeof(double)))) return rc;
+            if ((rc = dmalloc(h, (void**)&c.r, 3 * Nc * sizeof(double)))) return rc;
+            if ((rc = dmalloc(h, (void**)&c.e, 3 * Nc * sizeof(double)))) return rc;
+            cells += (double)Nc / (double)N;
+            ++L;
+        }
+        if (H.lev[L - 1].g.nx > 1 || H.lev[L - 1].g.ny > 1) return fail(h, ARK_M1_E_UNSUPPORTED, "multigrid: grid too large for %s levels", "24");
+        H.nlev = L; h->mg_cells = cells;
     }
     h->stride = (long long)((n + 31) / 32 * 32) + h->basis_pad;
     if (h->m_alloc < m) {
@@ -416,7 +451,7 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
 static int true_residual(ark_m1* h, const double* x)
 {
     const long long n = 3 * h->N;
-    if (h->op_kind == 1) {
+    if (opk(h) == 1) {
         KL(KC_SPMV, 216.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, x, h->V, nullptr, h->A.b, -1.0, nullptr, 0, h->sm_count, h->st));
     } else {
         KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, x, h->tvec, h->st));
@@ -436,7 +471,7 @@ static int fetch_ctl(ark_m1* h)
 static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
 {
     const Fields f = fields_of(h);
-    if (h->op_kind == 1) {
+    if (opk(h) == 1) {
         h->mf.rx = h->s.hyp_off ? 0.0 : dt / h->g.dx; h->mf.ry = h->s.hyp_off ? 0.0 : dt / h->g.dy;
         if (h->asm_kernel == 1 && h->N < (1LL << 31))
             KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble_march(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->sm_count, h->st));
@@ -447,6 +482,25 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
         KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, none, bsrc, h->st));
         KL(KC_SCALE, 648.0 * h->N, launch_scale_offdiag(h->g, h->A, h->st));
     }
+    if (h->precond == 1) {       // Galerkin hierarchy: each level reads 36 doubles per finer cell, writes 45 (+ the scaling pass) per cell
+        h->mg.lev[0].off = h->A.off;
+        for (int l = 1; l < h->mg.nlev; ++l) {
+            const MgLevel& f = h->mg.lev[l - 1]; const MgLevel& c = h->mg.lev[l];
+            const double Nf = (double)f.g.nx * f.g.ny, Nc = (double)c.g.nx * c.g.ny;
+            h->launches++;      // two kernels per level
+            KL(KC_MGSETUP, 288.0 * Nf + (360.0 + 648.0) * Nc, launch_mg_galerkin(f.g, f.off, c.g, c.off, c.Dinv, h->st));
+        }
+    }
+    return 0;
+}
+
+// z^ = Mhat^-1 v: one V-cycle in the hat variable (v, zhat: 3N, distinct).  Two stencil passes per level.
+static int mg_apply(ark_m1* h, const double* v, double* zhat, const int* stop)
+{
+    int nl = 0;
+    kmark(h, KC_MG, (312.0 + 336.0) * h->N * h->mg_cells);
+    CU(launch_mg_vcycle(h->mg, v, zhat, stop, h->st, &nl));
+    h->launches += nl - 1;
     return 0;
 }
 
@@ -468,7 +522,10 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
-            if (h->op_kind == 1)
+            if (h->precond == 1) {          // w = Ahat Mhat^-1 (scale_j v_j): the V-cycle is linear, the scale goes on last
+                if ((rc = mg_apply(h, h->V + (size_t)j * S, h->mgz, stop))) return rc;
+                KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->mgz, w, W.scale + j, nullptr, 1.0, stop, h->st));
+            } else if (opk(h) == 1)
                 KL(KC_SPMV, 264.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
             else
                 KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
@@ -485,7 +542,12 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
             }
         }
         KL(KC_SMALL, 0.0, launch_solve_y(W, h->st));
-        KL(KC_COMBINE, 8.0 * (3.0 * m + 15.0) * h->N, launch_combine(h->g, h->V, S, h->A.Minv, x, W, sm, h->st));
+        if (h->precond == 1) {              // x += D^-1 Mhat^-1 (V y)
+            KL(KC_COMBINE, 8.0 * (3.0 * m + 3.0) * h->N, launch_combine(h->g, h->V, S, nullptr, h->tvec, W, sm, h->st));
+            if ((rc = mg_apply(h, h->tvec, h->mgz, nullptr))) return rc;
+            KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, h->mgz, x, h->st));
+        } else
+            KL(KC_COMBINE, 8.0 * (3.0 * m + 15.0) * h->N, launch_combine(h->g, h->V, S, h->A.Minv, x, W, sm, h->st));
         if ((rc = true_residual(h, x))) return rc;
         if ((rc = fetch_ctl(h))) return rc;
     }
@@ -497,7 +559,13 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
 // Iterations are enqueued in batches of 8 without host round trips; one iteration = two operator applications.
 static int op_apply_hat(ark_m1* h, const double* vin, double* vout, const int* stop)
 {
-    if (h->op_kind == 1)
+    if (h->precond == 1) {
+        int rc = mg_apply(h, vin, h->mgz, stop);
+        if (rc) return rc;
+        KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->mgz, vout, nullptr, nullptr, 1.0, stop, h->st));
+        return 0;
+    }
+    if (opk(h) == 1)
         KL(KC_SPMV, 264.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, stop, 1, h->sm_count, h->st));
     else
         KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, vin, vout, nullptr, nullptr, 1.0, stop, h->st));
@@ -524,7 +592,7 @@ static int bicgstab_solve(ark_m1* h, double tol, int maxit)
         for (;;) {
             for (int k = 0; k < 8; ++k) {
                 KL(KC_UPDATE, 96.0 * h->N, launch_bicg_p(r, p, v, n, W, h->st));
-                if (h->op_kind == 1) {   // matrix-free operator with the reductions fused in
+                if (opk(h) == 1) {   // matrix-free operator with the reductions fused in
                     KL(KC_SPMV, 288.0 * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, p, v, stop, 1, rh, W, sm, h->st));
                     KL(KC_UPDATE, 72.0 * h->N, launch_bicg_s(r, v, n, W, h->st));
                     KL(KC_SPMV, 264.0 * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, r, t, stop, 2, nullptr, W, sm, h->st));
@@ -540,7 +608,12 @@ static int bicgstab_solve(ark_m1* h, double tol, int maxit)
             if ((rc = fetch_ctl(h))) return rc;
             if (h->ctl_host->inner_stop) break;
         }
-        KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, y, x, h->st));
+        if (h->precond == 1) {
+            if ((rc = mg_apply(h, y, h->mgz, nullptr))) return rc;
+            KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, h->mgz, x, h->st));
+            CU(cudaMemsetAsync(y, 0, (size_t)n * sizeof(double), h->st));
+        } else
+            KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, y, x, h->st));
         if ((rc = true_residual(h, x))) return rc;      // resets inner_stop unless converged / out of iterations
         if ((rc = fetch_ctl(h))) return rc;
         if (h->ctl_host->its == its0) break;            // breakdown without progress
@@ -664,7 +737,7 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
     double* vin = h->V;                       // slot 0 as staging for the input, slot 1 for the output
     double* vout = h->V + h->stride;
     CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
-    if (h->op_kind == 1) {
+    if (opk(h) == 1) {
         KL(KC_SPMV, 192.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, nullptr, 0, h->sm_count, h->st));
     } else {
         KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, vin, h->tvec, h->st));
@@ -673,6 +746,33 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
     CU(cudaMemcpyAsync(out, vout, n * sizeof(double), cudaMemcpyDefault, h->st));
     if (b_out) CU(cudaMemcpyAsync(b_out, h->A.b, n * sizeof(double), cudaMemcpyDefault, h->st));
     CU(cudaStreamSynchronize(h->st));
+    return 0;
+}
+
+// out = M^-1 V with the right preconditioner the solver would use for a step dt: the inverse 3x3 diagonal blocks
+// (block-Jacobi) or D^-1 times one multigrid V-cycle ("preconditioner" = 1).
+extern "C" int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* Vin, double* out)
+{
+    if (!h || !Vin || !out) return ARK_M1_E_ARG;
+    if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "apply_preconditioner: dt must be > 0%s", "");
+    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "apply_preconditioner: no state set%s", "");
+    int rc = ensure_implicit(h, 1, 1);
+    if (rc) return rc;
+    const size_t n = 3 * (size_t)h->N;
+    if ((rc = assemble_system(h, dt))) return rc;
+    double* vin = h->V;
+    double* vout = h->V + h->stride;
+    CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(cudaMemsetAsync(vout, 0, n * sizeof(double), h->st));
+    if (h->precond == 1) {
+        if ((rc = mg_apply(h, vin, h->mgz, nullptr))) return rc;
+        KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, h->mgz, vout, h->st));
+    } else {
+        KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, vin, vout, h->st));
+    }
+    CU(cudaMemcpyAsync(out, vout, n * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(cudaStreamSynchronize(h->st));
+    kflush(h);
     return 0;
 }
 

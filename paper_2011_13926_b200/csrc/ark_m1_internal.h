@@ -107,6 +107,21 @@ cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Mi
 cudaError_t launch_matter_update(const Grid& g, const Scheme& s, double dt, const double* sa, const double* rho_cv,
                                  const double* Enew, double* T, cudaStream_t st);
 
+// multigrid.cu — V-cycle preconditioner in the block-Jacobi-scaled variable (option "preconditioner" = 1)
+#define MG_MAXLEV 24
+struct MgLevel {
+    Grid g;          // nx, ny of the level; spacing unused; boundary kinds of the fine grid
+    double* off;     // 36 planes: scaled neighbour blocks of the level (level 0: the fine A.off)
+    double* Dinv;    // 9 planes: inverse diagonal block of the level's Galerkin operator (level 0: unused)
+    double* r;       // 3 planes: restricted residual = right-hand side of the level (level 0: the caller's vector)
+    double* e;       // 3 planes: the level's correction Dinv z^ handed to the finer level (level 0: the caller's output)
+};
+struct MgHier { int nlev; MgLevel lev[MG_MAXLEV]; double omega; int coarse_sweeps; };
+// coarse blocks of one level from the finer one (Galerkin, 2x2 aggregates): writes coff (scaled) and cDinv
+cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc, double* coff, double* cDinv, cudaStream_t st);
+// zhat_out = one V-cycle on r_in (level-0 vectors of 3N doubles, distinct); *nl = kernels launched
+cudaError_t launch_mg_vcycle(const MgHier& H, const double* r_in, double* zhat_out, const int* skip_flag, cudaStream_t st, int* nl);
+
 // krylov_kernels.cu
 int  krylov_max_blocks(int sm_count);
 // dots of w with nv vectors V0 + k*stride (k < nv) -> epilogue `mode`; col0 = index of the first vector in the basis
@@ -117,7 +132,7 @@ cudaError_t launch_update(double* w, const double* V0, long long stride, int nv,
                           GmresWork W, int with_norm, int sm_count, cudaStream_t st);
 // the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
 cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
-// x += Minv * (sum_{k<ctl->j} coef[k] V_k)  per cell
+// x += Minv * (sum_{k<ctl->j} coef[k] V_k)  per cell;  Minv == nullptr: x = sum_{k<ctl->j} coef[k] V_k
 cudaError_t launch_combine(const Grid& g, const double* V, long long stride, const double* Minv, double* x,
                            GmresWork W, int sm_count, cudaStream_t st);
 // BiCGStab vector kernels (krylov_kernels.cu); every one returns at once when ctl->inner_stop is set

@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(KTHREADS) combine_kernel(long long N, const do
                                                            const double* __restrict__ Minv, double* __restrict__ x, GmresWork W)
 {
     const int jj = W.ctl->j;
-    if (jj == 0) return;
+    if (jj == 0 && Minv) return;
     for (long long id = blockIdx.x * (long long)KTHREADS + threadIdx.x; id < N; id += (long long)gridDim.x * KTHREADS) {
         double u0 = 0.0, u1 = 0.0, u2 = 0.0;
 #pragma unroll 4
@@ -159,6 +159,7 @@ __global__ void __launch_bounds__(KTHREADS) combine_kernel(long long N, const do
             const double* v = V + k * stride;
             u0 += cf * v[id]; u1 += cf * v[N + id]; u2 += cf * v[2 * N + id];
         }
+        if (!Minv) { x[id] = u0; x[N + id] = u1; x[2 * N + id] = u2; continue; }   // plain combination (multigrid path)
         x[id]         += Minv[0 * N + id] * u0 + Minv[1 * N + id] * u1 + Minv[2 * N + id] * u2;
         x[N + id]     += Minv[3 * N + id] * u0 + Minv[4 * N + id] * u1 + Minv[5 * N + id] * u2;
         x[2 * N + id] += Minv[6 * N + id] * u0 + Minv[7 * N + id] * u1 + Minv[8 * N + id] * u2;

@@ -1,0 +1,208 @@
+// multigrid.cu — geometric-aggregation multigrid V-cycle as the right preconditioner of the Krylov solvers
+// (pre-smoothing, restricted residual equation "R A P y = R r~", coarse solve, interpolation,
+// post-smoothing; the paper takes an algebraic multigrid from a library, reading R12 fixes this one).
+//
+// Everything runs in the block-Jacobi-scaled ("hat") variable of the Krylov core: on level l the operator is
+//   Ahat_l = A_l D_l^-1 = I + sum_k off_k(.)            (unit diagonal blocks, four scaled neighbour blocks, like the fine level)
+// so the damped block-Jacobi smoother is a damped Richardson sweep  z^ += omega (r - Ahat z^)  that never touches D, and
+//   coarse operator  A_{l+1} = P0^T Ahat_l P0  (2x2 aggregates, 1 wide at an odd end; again a 5-point stencil of 3x3 blocks)
+//   restriction      r_{l+1} = P0^T (r - Ahat z^)
+//   interpolation    z^ += P0 e_{l+1},  e_{l+1} = D_{l+1}^-1 z^_{l+1}
+// (in the unscaled variable: R = P0^T, P = D^-1 P0, smoother omega D^-1 — the form the oracle is written in).
+// One V-cycle from a zero initial guess with one pre- and one post-sweep costs two stencil passes per level:
+//   pass 1 (restrict)      : r_c = P0^T ((1 - omega) r - omega sum_k off_k r_nbr)            reads 36 + 3 doubles per cell
+//   pass 2 (prolong+smooth): t = omega r + P0 e_c;  z^ = t + omega (r - t - sum_k off_k t_nbr)   reads 36 + 3, writes 3
+// The hierarchy ends at a single cell, where `coarse_sweeps` Richardson sweeps stand in for the direct solve.
+#include "implicit_device.cuh"
+
+namespace ark {
+
+__device__ __forceinline__ long long mg_nbr(const Grid& g, int i, int j, int k)
+{
+    int ii = i + (k == 0 ? -1 : (k == 1 ? 1 : 0));
+    int jj = j + (k == 2 ? -1 : (k == 3 ? 1 : 0));
+    if (ii < 0) ii = (g.bc[XLO] == BC_PERIODIC) ? g.nx - 1 : 0;
+    if (ii >= g.nx) ii = (g.bc[XHI] == BC_PERIODIC) ? 0 : g.nx - 1;
+    if (jj < 0) jj = (g.bc[YLO] == BC_PERIODIC) ? g.ny - 1 : 0;
+    if (jj >= g.ny) jj = (g.bc[YHI] == BC_PERIODIC) ? 0 : g.ny - 1;
+    return (long long)jj * g.nx + ii;
+}
+
+// ---- set-up: coarse blocks of one level --------------------------------------------------------------------------
+// One thread per coarse cell: D_c = sum over the aggregate of (I + blocks whose neighbour lies in the same aggregate),
+// C_k = sum of the blocks that leave the aggregate in direction k.  Writes Dinv_c = D_c^-1 and the raw C_k;
+// launch_scale_offdiag then turns C_k into C_k Dinv_c(neighbour k).
+__global__ void __launch_bounds__(128) mg_galerkin_kernel(Grid gf, const double* __restrict__ off, Grid gc,
+                                                          double* __restrict__ coff, double* __restrict__ cDinv)
+{
+    const int I = blockIdx.x * blockDim.x + threadIdx.x;
+    const int J = blockIdx.y * blockDim.y + threadIdx.y;
+    if (I >= gc.nx || J >= gc.ny) return;
+    const long long N = (long long)gf.nx * gf.ny, Nc = (long long)gc.nx * gc.ny, a = (long long)J * gc.nx + I;
+    Blk D, Ck[4];
+    blk_zero(D);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) blk_zero(Ck[k]);
+    for (int dj = 0; dj < 2; ++dj)
+        for (int di = 0; di < 2; ++di) {
+            const int i = 2 * I + di, j = 2 * J + dj;
+            if (i >= gf.nx || j >= gf.ny) continue;
+            const long long id = (long long)j * gf.nx + i;
+            D.a[0] += 1.0; D.a[4] += 1.0; D.a[8] += 1.0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const long long nb = mg_nbr(gf, i, j, k);
+                const long long anb = (nb / gf.nx / 2) * gc.nx + (nb % gf.nx) / 2;
+                const bool inside = (anb == a);
+#pragma unroll
+                for (int e = 0; e < 9; ++e) {
+                    const double v = off[(long long)(k * 9 + e) * N + id];
+                    if (inside) D.a[e] += v; else Ck[k].a[e] += v;
+                }
+            }
+        }
+    Blk Di; inv3(D, Di);
+#pragma unroll
+    for (int e = 0; e < 9; ++e) cDinv[e * Nc + a] = Di.a[e];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+        for (int e = 0; e < 9; ++e) coff[(long long)(k * 9 + e) * Nc + a] = Ck[k].a[e];
+}
+
+cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc, double* coff, double* cDinv, cudaStream_t st)
+{
+    dim3 blk(32, 4), grd((gc.nx + 31) / 32, (gc.ny + 3) / 4);
+    mg_galerkin_kernel<<<grd, blk, 0, st>>>(gf, off, gc, coff, cDinv);
+    if (cudaGetLastError() != cudaSuccess) return cudaErrorLaunchFailure;
+    BlockMatrix C; C.off = coff; C.C = nullptr; C.Minv = cDinv; C.b = nullptr;
+    return launch_scale_offdiag(gc, C, st);
+}
+
+// ---- V-cycle pass 1: r_c = P0^T ((1 - omega) r - omega sum_k off_k r_nbr) --------------------------------------------
+// Thread (i, J) handles the fine cells (i, 2J) and (i, 2J+1); lane pairs (i even, i+1) add up through a shuffle.
+__global__ void __launch_bounds__(128) mg_restrict_kernel(Grid g, const double* __restrict__ off, const double* __restrict__ r,
+                                                          double omega, int cnx, double* __restrict__ rc,
+                                                          const int* __restrict__ skip_flag)
+{
+    if (skip_flag && *skip_flag) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int J = blockIdx.y * blockDim.y + threadIdx.y;
+    const long long N = (long long)g.nx * g.ny;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    const int cny = (g.ny + 1) / 2;
+    if (i < g.nx && J < cny) {
+#pragma unroll
+        for (int dj = 0; dj < 2; ++dj) {
+            const int j = 2 * J + dj;
+            if (j >= g.ny) continue;
+            const long long id = (long long)j * g.nx + i;
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const long long nb = mg_nbr(g, i, j, k);
+                const double x0 = r[nb], x1 = r[N + nb], x2 = r[2 * N + nb];
+                const double* a = off + (long long)(k * 9) * N + id;
+                a0 += a[0 * N] * x0 + a[1 * N] * x1 + a[2 * N] * x2;
+                a1 += a[3 * N] * x0 + a[4 * N] * x1 + a[5 * N] * x2;
+                a2 += a[6 * N] * x0 + a[7 * N] * x1 + a[8 * N] * x2;
+            }
+            s0 += (1.0 - omega) * r[id] - omega * a0;
+            s1 += (1.0 - omega) * r[N + id] - omega * a1;
+            s2 += (1.0 - omega) * r[2 * N + id] - omega * a2;
+        }
+    }
+    s0 += __shfl_xor_sync(0xffffffffu, s0, 1); s1 += __shfl_xor_sync(0xffffffffu, s1, 1); s2 += __shfl_xor_sync(0xffffffffu, s2, 1);
+    if ((i & 1) == 0 && i < g.nx && J < cny) {
+        const long long Nc = (long long)cnx * cny, a = (long long)J * cnx + (i >> 1);
+        rc[a] = s0; rc[Nc + a] = s1; rc[2 * Nc + a] = s2;
+    }
+}
+
+// ---- V-cycle pass 2: t = omega r + P0 e_c;  z^ = t + omega (r - t - sum_k off_k t_nbr);  out = Dinv z^ (coarse levels) or z^ ----
+__global__ void __launch_bounds__(128) mg_prolong_smooth_kernel(Grid g, const double* __restrict__ off, const double* __restrict__ r,
+                                                                double omega, int cnx, const double* __restrict__ ec,
+                                                                const double* __restrict__ Dinv, double* __restrict__ out,
+                                                                const int* __restrict__ skip_flag)
+{
+    if (skip_flag && *skip_flag) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= g.nx || j >= g.ny) return;
+    const long long N = (long long)g.nx * g.ny, id = (long long)j * g.nx + i;
+    const long long Nc = (long long)cnx * ((g.ny + 1) / 2);
+    const long long a = (long long)(j >> 1) * cnx + (i >> 1);
+    const double r0 = r[id], r1 = r[N + id], r2 = r[2 * N + id];
+    const double t0 = omega * r0 + ec[a], t1 = omega * r1 + ec[Nc + a], t2 = omega * r2 + ec[2 * Nc + a];
+    double q0 = t0, q1 = t1, q2 = t2;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const long long nb = mg_nbr(g, i, j, k);
+        const long long an = (nb / g.nx / 2) * cnx + (nb % g.nx) / 2;
+        const double x0 = omega * r[nb] + ec[an], x1 = omega * r[N + nb] + ec[Nc + an], x2 = omega * r[2 * N + nb] + ec[2 * Nc + an];
+        const double* b = off + (long long)(k * 9) * N + id;
+        q0 += b[0 * N] * x0 + b[1 * N] * x1 + b[2 * N] * x2;
+        q1 += b[3 * N] * x0 + b[4 * N] * x1 + b[5 * N] * x2;
+        q2 += b[6 * N] * x0 + b[7 * N] * x1 + b[8 * N] * x2;
+    }
+    const double z0 = t0 + omega * (r0 - q0), z1 = t1 + omega * (r1 - q1), z2 = t2 + omega * (r2 - q2);
+    if (Dinv) {
+        out[id]         = Dinv[0 * N + id] * z0 + Dinv[1 * N + id] * z1 + Dinv[2 * N + id] * z2;
+        out[N + id]     = Dinv[3 * N + id] * z0 + Dinv[4 * N + id] * z1 + Dinv[5 * N + id] * z2;
+        out[2 * N + id] = Dinv[6 * N + id] * z0 + Dinv[7 * N + id] * z1 + Dinv[8 * N + id] * z2;
+    } else {
+        out[id] = z0; out[N + id] = z1; out[2 * N + id] = z2;
+    }
+}
+
+// ---- coarsest level (a single cell): z^ = omega r, then sweeps-1 times z^ += omega (r - Ahat z^);  out = Dinv z^ ----------
+__global__ void mg_coarsest_kernel(Grid g, const double* __restrict__ off, const double* __restrict__ r, double omega, int sweeps,
+                                   const double* __restrict__ Dinv, double* __restrict__ out, const int* __restrict__ skip_flag)
+{
+    if (skip_flag && *skip_flag) return;
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double Ah[9] = { 1, 0, 0, 0, 1, 0, 0, 0, 1 };       // N = 1: every neighbour is the cell itself (or the block is zero)
+    for (int k = 0; k < 4; ++k)
+        for (int e = 0; e < 9; ++e) Ah[e] += off[k * 9 + e];
+    const double rr[3] = { r[0], r[1], r[2] };
+    double z[3] = { omega * rr[0], omega * rr[1], omega * rr[2] };
+    for (int s = 1; s < sweeps; ++s) {
+        double q[3];
+        for (int a = 0; a < 3; ++a) q[a] = Ah[3 * a] * z[0] + Ah[3 * a + 1] * z[1] + Ah[3 * a + 2] * z[2];
+        for (int a = 0; a < 3; ++a) z[a] += omega * (rr[a] - q[a]);
+    }
+    for (int a = 0; a < 3; ++a) out[a] = Dinv ? (Dinv[3 * a] * z[0] + Dinv[3 * a + 1] * z[1] + Dinv[3 * a + 2] * z[2]) : z[a];
+}
+
+// One V-cycle: zhat_out = Mhat^-1 r_in on level 0 (both 3N planes; may not alias).  Returns the number of launches in *nl.
+cudaError_t launch_mg_vcycle(const MgHier& H, const double* r_in, double* zhat_out, const int* skip_flag, cudaStream_t st, int* nl)
+{
+    int launches = 0;
+    const int L = H.nlev;
+    for (int l = 0; l + 1 < L; ++l) {                     // downward: restricted residuals
+        const MgLevel& f = H.lev[l];
+        const double* r = (l == 0) ? r_in : f.r;
+        dim3 blk(32, 4), grd((f.g.nx + 31) / 32, ((f.g.ny + 1) / 2 + 3) / 4);
+        mg_restrict_kernel<<<grd, blk, 0, st>>>(f.g, f.off, r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].r, skip_flag);
+        ++launches;
+    }
+    {
+        const MgLevel& c = H.lev[L - 1];
+        const double* r = (L == 1) ? r_in : c.r;
+        mg_coarsest_kernel<<<1, 32, 0, st>>>(c.g, c.off, r, H.omega, H.coarse_sweeps, (L == 1) ? nullptr : c.Dinv,
+                                             (L == 1) ? zhat_out : c.e, skip_flag);
+        ++launches;
+    }
+    for (int l = L - 2; l >= 0; --l) {                    // upward: interpolation + post-smoothing
+        const MgLevel& f = H.lev[l];
+        const double* r = (l == 0) ? r_in : f.r;
+        dim3 blk(32, 4), grd((f.g.nx + 31) / 32, (f.g.ny + 3) / 4);
+        mg_prolong_smooth_kernel<<<grd, blk, 0, st>>>(f.g, f.off, r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].e,
+                                                      (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
+        ++launches;
+    }
+    if (nl) *nl = launches;
+    return cudaGetLastError();
+}
+
+}  // namespace ark
