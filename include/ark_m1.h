@@ -100,6 +100,8 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                       1: multigrid V-cycle (R12): 2x2 cell aggregates down to one cell, Galerkin
  *                          coarse operators, one damped block-Jacobi sweep before and after; uses the block-stencil operator
  *   "mg_omega"          damping of the multigrid smoother, in (0, 2) (default 0.8)
+ *   "mg_precision"      64 (default) or 32: storage precision of the multigrid's matrix blocks; the cycle itself runs in fp64
+ *                       on fp64 vectors, so it stays a fixed linear operator and the solve still meets the fp64 tolerance
  *   "mg_coarse_sweeps"  smoother sweeps on the coarsest (one-cell) level, >= 1 (default 2)
  * Unknown key or unsupported value: ARK_M1_E_ARG. */
 ARK_M1_API int ark_m1_set_option(ark_m1* h, const char* key, double value);

@@ -138,7 +138,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
     h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0; h->asm_kernel = 1;
-    h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0;
+    h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     h->hist_host = new std::vector<double>();
@@ -165,6 +165,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
 
 static void free_implicit(ark_m1* h)
 {
+    for (int l = 0; l < h->mg.nlev; ++l) { cudaFree(h->mg.lev[l].off32); h->mg.lev[l].off32 = nullptr; }
     for (int l = 1; l < h->mg.nlev; ++l) { cudaFree(h->mg.lev[l].off); cudaFree(h->mg.lev[l].Dinv); cudaFree(h->mg.lev[l].r); cudaFree(h->mg.lev[l].e); }
     h->mg.nlev = 0; cudaFree(h->mgz); h->mgz = nullptr;
     cudaFree(h->A.off); cudaFree(h->A.C); cudaFree(h->A.Minv); cudaFree(h->A.b); cudaFree(h->V); cudaFree(h->tvec); cudaFree(h->wblock); cudaFree(h->nprev); h->nprev = nullptr;
@@ -256,6 +257,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
     else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
     else if (!strcmp(key, "mg_coarse_sweeps")) { if (iv < 1) return fail(h, ARK_M1_E_ARG, "mg_coarse_sweeps must be >= 1%s", ""); h->mg.coarse_sweeps = iv; }
+    else if (!strcmp(key, "mg_precision")) { if (iv != 32 && iv != 64) return fail(h, ARK_M1_E_ARG, "mg_precision must be 64 or 32%s", ""); h->mg.precision = iv; }
     else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
     return 0;
 }
@@ -371,7 +373,7 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
 {
     const size_t N = (size_t)h->N, n = 3 * N;
     const bool have_op = (opk(h) == 0) ? (h->A.off != nullptr) : (h->mf.J != nullptr);
-    if (h->m_alloc >= m && h->maxit_alloc >= maxit && have_op && (h->precond == 0 || h->mg.nlev > 0)) return 0;
+    if (h->m_alloc >= m && h->maxit_alloc >= maxit && have_op && (h->precond == 0 || (h->mg.nlev > 0 && (h->mg.precision == 64 || h->mg.lev[0].off32)))) return 0;
     CU(cudaStreamSynchronize(h->st));
     const long long before = h->bytes;
     (void)before;
@@ -400,13 +402,13 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
         int rc;
         if ((rc = dmalloc(h, (void**)&h->mgz, n * sizeof(double)))) return rc;
         MgHier& H = h->mg;
-        H.lev[0].g = h->g; H.lev[0].off = nullptr; H.lev[0].Dinv = nullptr; H.lev[0].r = nullptr; H.lev[0].e = nullptr;
+        H.lev[0].g = h->g; H.lev[0].off = nullptr; H.lev[0].off32 = nullptr; H.lev[0].Dinv = nullptr; H.lev[0].r = nullptr; H.lev[0].e = nullptr;
         int L = 1; double cells = 1.0;
         while ((H.lev[L - 1].g.nx > 1 || H.lev[L - 1].g.ny > 1) && L < MG_MAXLEV) {
             MgLevel& c = H.lev[L];
             c.g = H.lev[L - 1].g; c.g.nx = (c.g.nx + 1) / 2; c.g.ny = (c.g.ny + 1) / 2;
             const size_t Nc = (size_t)c.g.nx * c.g.ny;
-            c.off = c.Dinv = c.r = c.e = nullptr;
+            c.off = c.Dinv = c.r = c.e = nullptr; c.off32 = nullptr;
             H.nlev = L + 1;                          // so that a failure below frees what was allocated
             if ((rc = dmalloc(h, (void**)&c.off, 36 * Nc * sizeof(double)))) return rc;
             if ((rc = dmalloc(h, (void**)&c.Dinv, 9 * Nc * sizeof(double)))) return rc;
@@ -417,6 +419,13 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
         }
         if (H.lev[L - 1].g.nx > 1 || H.lev[L - 1].g.ny > 1) return fail(h, ARK_M1_E_UNSUPPORTED, "multigrid: grid too large for %s levels", "24");
         H.nlev = L; h->mg_cells = cells;
+    }
+    if (h->precond == 1 && h->mg.precision == 32 && h->mg.lev[0].off32 == nullptr) {
+        for (int l = 0; l < h->mg.nlev; ++l) {
+            const size_t Nl = (size_t)h->mg.lev[l].g.nx * h->mg.lev[l].g.ny;
+            int rc = dmalloc(h, (void**)&h->mg.lev[l].off32, 36 * Nl * sizeof(float));
+            if (rc) return rc;
+        }
     }
     h->stride = (long long)((n + 31) / 32 * 32) + h->basis_pad;
     if (h->m_alloc < m) {
@@ -490,6 +499,11 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
             h->launches++;      // two kernels per level
             KL(KC_MGSETUP, 288.0 * Nf + (360.0 + 648.0) * Nc, launch_mg_galerkin(f.g, f.off, c.g, c.off, c.Dinv, h->st));
         }
+        if (h->mg.precision == 32)
+            for (int l = 0; l < h->mg.nlev; ++l) {
+                const long long cnt = 36LL * h->mg.lev[l].g.nx * h->mg.lev[l].g.ny;
+                KL(KC_MGSETUP, 12.0 * cnt, launch_mg_to_float(h->mg.lev[l].off, h->mg.lev[l].off32, cnt, h->st));
+            }
     }
     return 0;
 }
@@ -498,7 +512,7 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
 static int mg_apply(ark_m1* h, const double* v, double* zhat, const int* stop)
 {
     int nl = 0;
-    kmark(h, KC_MG, (312.0 + 336.0) * h->N * h->mg_cells);
+    kmark(h, KC_MG, (h->mg.precision == 32 ? (168.0 + 192.0) : (312.0 + 336.0)) * h->N * h->mg_cells);
     CU(launch_mg_vcycle(h->mg, v, zhat, stop, h->st, &nl));
     h->launches += nl - 1;
     return 0;

@@ -112,13 +112,15 @@ cudaError_t launch_matter_update(const Grid& g, const Scheme& s, double dt, cons
 struct MgLevel {
     Grid g;          // nx, ny of the level; spacing unused; boundary kinds of the fine grid
     double* off;     // 36 planes: scaled neighbour blocks of the level (level 0: the fine A.off)
+    float* off32;    // the same in single precision (option "mg_precision" = 32; null otherwise)
     double* Dinv;    // 9 planes: inverse diagonal block of the level's Galerkin operator (level 0: unused)
     double* r;       // 3 planes: restricted residual = right-hand side of the level (level 0: the caller's vector)
     double* e;       // 3 planes: the level's correction Dinv z^ handed to the finer level (level 0: the caller's output)
 };
-struct MgHier { int nlev; MgLevel lev[MG_MAXLEV]; double omega; int coarse_sweeps; };
+struct MgHier { int nlev; MgLevel lev[MG_MAXLEV]; double omega; int coarse_sweeps; int precision; };
 // coarse blocks of one level from the finer one (Galerkin, 2x2 aggregates): writes coff (scaled) and cDinv
 cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc, double* coff, double* cDinv, cudaStream_t st);
+cudaError_t launch_mg_to_float(const double* a, float* b, long long n, cudaStream_t st);
 // zhat_out = one V-cycle on r_in (level-0 vectors of 3N doubles, distinct); *nl = kernels launched
 cudaError_t launch_mg_vcycle(const MgHier& H, const double* r_in, double* zhat_out, const int* skip_flag, cudaStream_t st, int* nl);
 

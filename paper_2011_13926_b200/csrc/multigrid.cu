@@ -17,7 +17,9 @@
 
 namespace ark {
 
-__device__ __forceinline__ long long mg_nbr(const Grid& g, int i, int j, int k)
+// Neighbour k (0: W, 1: E, 2: S, 3: N) of cell (i, j): its index on the level and, through `agg`, its aggregate on the next
+// coarser level (cnx aggregates per row).  Non-periodic sides clamp (the block there is zero).
+__device__ __forceinline__ long long mg_nbr(const Grid& g, int i, int j, int k, int cnx, long long& agg)
 {
     int ii = i + (k == 0 ? -1 : (k == 1 ? 1 : 0));
     int jj = j + (k == 2 ? -1 : (k == 3 ? 1 : 0));
@@ -25,6 +27,7 @@ __device__ __forceinline__ long long mg_nbr(const Grid& g, int i, int j, int k)
     if (ii >= g.nx) ii = (g.bc[XHI] == BC_PERIODIC) ? 0 : g.nx - 1;
     if (jj < 0) jj = (g.bc[YLO] == BC_PERIODIC) ? g.ny - 1 : 0;
     if (jj >= g.ny) jj = (g.bc[YHI] == BC_PERIODIC) ? 0 : g.ny - 1;
+    agg = (long long)(jj >> 1) * cnx + (ii >> 1);
     return (long long)jj * g.nx + ii;
 }
 
@@ -51,8 +54,8 @@ __global__ void __launch_bounds__(128) mg_galerkin_kernel(Grid gf, const double*
             D.a[0] += 1.0; D.a[4] += 1.0; D.a[8] += 1.0;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const long long nb = mg_nbr(gf, i, j, k);
-                const long long anb = (nb / gf.nx / 2) * gc.nx + (nb % gf.nx) / 2;
+                long long anb;
+                mg_nbr(gf, i, j, k, gc.nx, anb);
                 const bool inside = (anb == a);
 #pragma unroll
                 for (int e = 0; e < 9; ++e) {
@@ -81,7 +84,8 @@ cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc
 
 // ---- V-cycle pass 1: r_c = P0^T ((1 - omega) r - omega sum_k off_k r_nbr) --------------------------------------------
 // Thread (i, J) handles the fine cells (i, 2J) and (i, 2J+1); lane pairs (i even, i+1) add up through a shuffle.
-__global__ void __launch_bounds__(128) mg_restrict_kernel(Grid g, const double* __restrict__ off, const double* __restrict__ r,
+template <typename TB>
+__global__ void __launch_bounds__(128) mg_restrict_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                           double omega, int cnx, double* __restrict__ rc,
                                                           const int* __restrict__ skip_flag)
 {
@@ -100,12 +104,13 @@ __global__ void __launch_bounds__(128) mg_restrict_kernel(Grid g, const double* 
             double a0 = 0.0, a1 = 0.0, a2 = 0.0;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const long long nb = mg_nbr(g, i, j, k);
+                long long an;
+                const long long nb = mg_nbr(g, i, j, k, cnx, an);
                 const double x0 = r[nb], x1 = r[N + nb], x2 = r[2 * N + nb];
-                const double* a = off + (long long)(k * 9) * N + id;
-                a0 += a[0 * N] * x0 + a[1 * N] * x1 + a[2 * N] * x2;
-                a1 += a[3 * N] * x0 + a[4 * N] * x1 + a[5 * N] * x2;
-                a2 += a[6 * N] * x0 + a[7 * N] * x1 + a[8 * N] * x2;
+                const TB* a = off + (long long)(k * 9) * N + id;
+                a0 += (double)a[0 * N] * x0 + (double)a[1 * N] * x1 + (double)a[2 * N] * x2;
+                a1 += (double)a[3 * N] * x0 + (double)a[4 * N] * x1 + (double)a[5 * N] * x2;
+                a2 += (double)a[6 * N] * x0 + (double)a[7 * N] * x1 + (double)a[8 * N] * x2;
             }
             s0 += (1.0 - omega) * r[id] - omega * a0;
             s1 += (1.0 - omega) * r[N + id] - omega * a1;
@@ -120,7 +125,8 @@ __global__ void __launch_bounds__(128) mg_restrict_kernel(Grid g, const double* 
 }
 
 // ---- V-cycle pass 2: t = omega r + P0 e_c;  z^ = t + omega (r - t - sum_k off_k t_nbr);  out = Dinv z^ (coarse levels) or z^ ----
-__global__ void __launch_bounds__(128) mg_prolong_smooth_kernel(Grid g, const double* __restrict__ off, const double* __restrict__ r,
+template <typename TB>
+__global__ void __launch_bounds__(128) mg_prolong_smooth_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                                 double omega, int cnx, const double* __restrict__ ec,
                                                                 const double* __restrict__ Dinv, double* __restrict__ out,
                                                                 const int* __restrict__ skip_flag)
@@ -137,13 +143,13 @@ __global__ void __launch_bounds__(128) mg_prolong_smooth_kernel(Grid g, const do
     double q0 = t0, q1 = t1, q2 = t2;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const long long nb = mg_nbr(g, i, j, k);
-        const long long an = (nb / g.nx / 2) * cnx + (nb % g.nx) / 2;
+        long long an;
+        const long long nb = mg_nbr(g, i, j, k, cnx, an);
         const double x0 = omega * r[nb] + ec[an], x1 = omega * r[N + nb] + ec[Nc + an], x2 = omega * r[2 * N + nb] + ec[2 * Nc + an];
-        const double* b = off + (long long)(k * 9) * N + id;
-        q0 += b[0 * N] * x0 + b[1 * N] * x1 + b[2 * N] * x2;
-        q1 += b[3 * N] * x0 + b[4 * N] * x1 + b[5 * N] * x2;
-        q2 += b[6 * N] * x0 + b[7 * N] * x1 + b[8 * N] * x2;
+        const TB* b = off + (long long)(k * 9) * N + id;
+        q0 += (double)b[0 * N] * x0 + (double)b[1 * N] * x1 + (double)b[2 * N] * x2;
+        q1 += (double)b[3 * N] * x0 + (double)b[4 * N] * x1 + (double)b[5 * N] * x2;
+        q2 += (double)b[6 * N] * x0 + (double)b[7 * N] * x1 + (double)b[8 * N] * x2;
     }
     const double z0 = t0 + omega * (r0 - q0), z1 = t1 + omega * (r1 - q1), z2 = t2 + omega * (r2 - q2);
     if (Dinv) {
@@ -156,14 +162,15 @@ __global__ void __launch_bounds__(128) mg_prolong_smooth_kernel(Grid g, const do
 }
 
 // ---- coarsest level (a single cell): z^ = omega r, then sweeps-1 times z^ += omega (r - Ahat z^);  out = Dinv z^ ----------
-__global__ void mg_coarsest_kernel(Grid g, const double* __restrict__ off, const double* __restrict__ r, double omega, int sweeps,
+template <typename TB>
+__global__ void mg_coarsest_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r, double omega, int sweeps,
                                    const double* __restrict__ Dinv, double* __restrict__ out, const int* __restrict__ skip_flag)
 {
     if (skip_flag && *skip_flag) return;
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     double Ah[9] = { 1, 0, 0, 0, 1, 0, 0, 0, 1 };       // N = 1: every neighbour is the cell itself (or the block is zero)
     for (int k = 0; k < 4; ++k)
-        for (int e = 0; e < 9; ++e) Ah[e] += off[k * 9 + e];
+        for (int e = 0; e < 9; ++e) Ah[e] += (double)off[k * 9 + e];
     const double rr[3] = { r[0], r[1], r[2] };
     double z[3] = { omega * rr[0], omega * rr[1], omega * rr[2] };
     for (int s = 1; s < sweeps; ++s) {
@@ -175,33 +182,59 @@ __global__ void mg_coarsest_kernel(Grid g, const double* __restrict__ off, const
 }
 
 // One V-cycle: zhat_out = Mhat^-1 r_in on level 0 (both 3N planes; may not alias).  Returns the number of launches in *nl.
-cudaError_t launch_mg_vcycle(const MgHier& H, const double* r_in, double* zhat_out, const int* skip_flag, cudaStream_t st, int* nl)
+// TB = float reads the single-precision copies of the blocks (option "mg_precision" = 32): the cycle is still a fixed linear
+// operator evaluated in fp64, only its matrix entries are rounded to 24 bits.
+template <typename TB>
+static cudaError_t vcycle_t(const MgHier& H, const double* r_in, double* zhat_out, const int* skip_flag, cudaStream_t st, int* nl)
 {
     int launches = 0;
     const int L = H.nlev;
+    auto blocks = [](const MgLevel& lv) -> const TB* {
+        if (sizeof(TB) == sizeof(float)) return reinterpret_cast<const TB*>(lv.off32);
+        return reinterpret_cast<const TB*>(lv.off);
+    };
     for (int l = 0; l + 1 < L; ++l) {                     // downward: restricted residuals
         const MgLevel& f = H.lev[l];
         const double* r = (l == 0) ? r_in : f.r;
         dim3 blk(32, 4), grd((f.g.nx + 31) / 32, ((f.g.ny + 1) / 2 + 3) / 4);
-        mg_restrict_kernel<<<grd, blk, 0, st>>>(f.g, f.off, r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].r, skip_flag);
+        mg_restrict_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].r, skip_flag);
         ++launches;
     }
     {
         const MgLevel& c = H.lev[L - 1];
         const double* r = (L == 1) ? r_in : c.r;
-        mg_coarsest_kernel<<<1, 32, 0, st>>>(c.g, c.off, r, H.omega, H.coarse_sweeps, (L == 1) ? nullptr : c.Dinv,
-                                             (L == 1) ? zhat_out : c.e, skip_flag);
+        mg_coarsest_kernel<TB><<<1, 32, 0, st>>>(c.g, blocks(c), r, H.omega, H.coarse_sweeps, (L == 1) ? nullptr : c.Dinv,
+                                                 (L == 1) ? zhat_out : c.e, skip_flag);
         ++launches;
     }
     for (int l = L - 2; l >= 0; --l) {                    // upward: interpolation + post-smoothing
         const MgLevel& f = H.lev[l];
         const double* r = (l == 0) ? r_in : f.r;
         dim3 blk(32, 4), grd((f.g.nx + 31) / 32, (f.g.ny + 3) / 4);
-        mg_prolong_smooth_kernel<<<grd, blk, 0, st>>>(f.g, f.off, r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].e,
-                                                      (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
+        mg_prolong_smooth_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].e,
+                                                          (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
         ++launches;
     }
     if (nl) *nl = launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_mg_vcycle(const MgHier& H, const double* r_in, double* zhat_out, const int* skip_flag, cudaStream_t st, int* nl)
+{
+    return H.precision == 32 ? vcycle_t<float>(H, r_in, zhat_out, skip_flag, st, nl)
+                             : vcycle_t<double>(H, r_in, zhat_out, skip_flag, st, nl);
+}
+
+// single-precision copy of a level's scaled blocks
+__global__ void mg_to_float_kernel(const double* __restrict__ a, float* __restrict__ b, long long n)
+{
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) b[k] = (float)a[k];
+}
+
+cudaError_t launch_mg_to_float(const double* a, float* b, long long n, cudaStream_t st)
+{
+    const long long need = (n + 255) / 256;
+    mg_to_float_kernel<<<(int)(need < 148 * 16 ? need : 148 * 16), 256, 0, st>>>(a, b, n);
     return cudaGetLastError();
 }
 

@@ -137,3 +137,32 @@ def test_multigrid_maxit_and_steady_state():
     gz = make_gpu(wz, MG)
     its, res = gz.step_implicit(_dt(wz, 100.0), 1e-10, 30, 100)
     assert its == 0
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0, 0), (1, 2, 2, 1)])
+def test_single_precision_blocks_change_the_cycle_only_at_rounding_level(bc):
+    # mg_precision = 32 rounds the stored blocks to 24 bits; vectors and arithmetic stay fp64
+    w = small_random_state(96, 80, seed=17, bc=bc)
+    o, g = make_oracle(w, MG), make_gpu(w, dict(preconditioner=1, mg_precision=32))
+    dt = _dt(w, 80.0)
+    R = np.random.default_rng(7).standard_normal((3, 80, 96))
+    d = rel_l2(g.apply_preconditioner(dt, R), o.mg_apply(dt, R))
+    assert 1e-12 < d <= 1e-5
+
+
+@pytest.mark.parametrize("krylov", [0, 1])
+def test_single_precision_multigrid_solve_meets_the_fp64_tolerance(krylov):
+    w = wl.random_medium(128, seed=1234)
+    opts = dict(preconditioner=1, krylov=krylov)
+    o, g = make_oracle(w, opts), make_gpu(w, dict(opts, mg_precision=32))
+    dt = _dt(w, 100.0)
+    io, ro = o.step_implicit(dt, 1e-10, 30, 1000)
+    ig, rg = g.step_implicit(dt, 1e-10, 30, 1000)
+    assert ro <= 1e-10 and rg <= 1e-10
+    assert state_rel_l2(g.get_state(), o.get_state()) <= 1e-8
+    assert abs(ig - io) <= max(3, 0.15 * io)
+    # switching back to fp64 blocks on the same handle
+    g.set_option("mg_precision", 64)
+    g.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
+    ig2, rg2 = g.step_implicit(dt, 1e-10, 30, 1000)
+    assert rg2 <= 1e-10 and abs(ig2 - io) <= max(3, 0.15 * io)
