@@ -408,6 +408,35 @@ def run_ours(args):
             bi["break_even_reached_at"] = wins
             line_extra["bicgstab"] = bi
             g.set_option("krylov", 0)
+        # ---- multigrid preconditioner (SURVEY 8(f) row 4 "stronger preconditioner"): option preconditioner = 1,
+        #      blocks stored in fp32 (mg_precision = 32); BiCGStab on the rough medium, GMRES(30) on the smooth problem ----------------
+        if not args.no_sweep:
+            g.set_option("preconditioner", 1); g.set_option("mg_precision", 32)
+            mgo = {"rough_medium": {}, "smooth_problem": {}, "options": {"preconditioner": 1, "mg_precision": 32, "mg_omega": 0.8,
+                                                                         "rough_medium_krylov": "bicgstab", "smooth_problem_krylov": "gmres(30)"}}
+            for label, tensors, ratios, kry in (("rough_medium", devt, (10.0, 50.0, 100.0, 200.0), 1),
+                                                ("smooth_problem", None, (50.0, 100.0, 200.0, 300.0, 500.0, 1000.0, 2000.0), 0)):
+                g.set_option("krylov", kry)
+                if tensors is None:
+                    ws = wl.gaussian_diffusion(n)
+                    tensors = {k: torch.from_numpy(np.ascontiguousarray(ws[k])).to(dev) for k in ("E", "F", "sigma_a", "sigma_s")}
+                for ratio in ratios:
+                    g.set_state(tensors["E"], tensors["F"], tensors["sigma_a"], tensors["sigma_s"])
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    its, res = g.step_implicit(ratio * dt_e, TOL, RESTART, 400)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1)
+                    tm = g.timings()
+                    mgo[label][f"{ratio:g}x"] = {"iterations": its, "preconditioner_applications": (2 if kry else 1) * its, "final_residual": res,
+                                                 "converged": bool(res <= TOL), "ms": ms, "setup_ms": tm["assembly_ms"],
+                                                 "ms_per_iteration": tm["krylov_ms"] / max(its, 1),
+                                                 "T_implicit_over_T_explicit": ms / ms_exp, "over_K": ms / ms_exp / ratio,
+                                                 "implicit_wins": bool(res <= TOL and ms / ms_exp < ratio)}
+            mgo["break_even_reached_at"] = [f"{lab}:{k}" for lab in ("rough_medium", "smooth_problem") for k, v in mgo[lab].items() if v["implicit_wins"]]
+            line_extra["multigrid"] = mgo
+            g.set_option("preconditioner", 0); g.set_option("krylov", 0)
         # ---- stage 2 (row a8, BASELINE.json configs[4]): matter coupling + point source + velocity sources at 2048^2 ----------
         if not args.no_sweep and not args.no_stage2:
             w5 = wl.stratified_coupled(2048, seed=4321)

@@ -6,7 +6,10 @@
 namespace ark {
 
 static constexpr int KTHREADS = 256;
-static constexpr int EPI_MAX = 128;      // Hessenberg columns up to this length are staged in shared memory for the Givens epilogue
+#ifndef ARK_EPI_MAX
+#define ARK_EPI_MAX 128
+#endif
+static constexpr int EPI_MAX = ARK_EPI_MAX;      // Hessenberg columns up to this length are staged in shared memory for the Givens epilogue
 
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -111,7 +114,10 @@ __device__ __forceinline__ void epilogue(const GmresWork& W, int mode, const dou
 // Block reduction of acc[0..NV) -> partial[block][.]; the last block sums the partials in a fixed order and
 // runs the epilogue.
 // NT = threads per block; blocks may be a 2-D grid (linear block id).
-template <int NV, int NT = KTHREADS>
+// STAGE: the kernel may run the DOT_UPD epilogue, whose Hessenberg column is staged in shared memory.  Only the update kernel
+// asks for it: the 3 KB of static shared memory cost the multi-dot kernels 15 % of their bandwidth (measured 6.60 -> 5.63 TB/s at
+// 4096^2 when they carried it too), while the update kernel is a little faster with it.
+template <int NV, int NT = KTHREADS, bool STAGE = false>
 __device__ __forceinline__ void reduce_and_finish(double (&acc)[NV], const GmresWork& W, int mode, int col0)
 {
     __shared__ double sh[NT / 32][MAXV];
@@ -146,7 +152,7 @@ __device__ __forceinline__ void reduce_and_finish(double (&acc)[NV], const Gmres
         s = warp_sum(s);
         if (lane == 0) dres[k] = s;
     }
-    if (mode == DOT_UPD) {
+    if constexpr (STAGE) if (mode == DOT_UPD) {
         // stage column j of H (rows 0..j; row j+1 is ||w|| itself), cs and sn for the scalar epilogue
         __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
         const int j = W.ctl->j, m = W.ctl->m;

@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(KTHREADS) update_kernel(double* __restrict__ w
         w[n - 1] = a;
         if (WITH_NORM) acc[0] += a * a;
     }
-    if (WITH_NORM) reduce_and_finish<1>(acc, W, DOT_UPD, 0);
+    if (WITH_NORM) reduce_and_finish<1, KTHREADS, true>(acc, W, DOT_UPD, 0);
 }
 
 static int grid_for(long long n, int sm_count)
