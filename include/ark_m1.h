@@ -97,7 +97,7 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *   "operator"          1: matrix-free coefficient planes, flux form (default: 5% faster per solve at 4096^2)
  *                       0: block stencil (BSR 3x3 on the 5-point graph, pre-multiplied by M^-1)
  *   "preconditioner"    0: 3x3 block-Jacobi (north_star; default)
- *                       1: multigrid V-cycle (R12): 2x2 cell aggregates down to one cell, Galerkin
+ *                       1: multigrid V-cycle (R15): 2x2 cell aggregates down to one cell, Galerkin
  *                          coarse operators, one damped block-Jacobi sweep before and after; uses the block-stencil operator
  *   "mg_omega"          damping of the multigrid smoother, in (0, 2) (default 0.8)
  *   "mg_precision"      64 (default) or 32: storage precision of the multigrid's matrix blocks; the cycle itself runs in fp64
@@ -165,7 +165,7 @@ ARK_M1_API int ark_m1_apply_operator(ark_m1* h, double dt, const double* V, doub
 
 /* out = M^-1 V, M^-1 = the right preconditioner the solver uses for a step dt ("A K^-1 y = b, K x = y"):
  * the inverse 3x3 diagonal blocks (Eq. 27 block-wise; option "preconditioner" = 0, default) or one multigrid V-cycle
- * ("preconditioner" = 1, R12).  V, out: 3*nx*ny doubles, host or device.  Synchronises. */
+ * ("preconditioner" = 1, R15).  V, out: 3*nx*ny doubles, host or device.  Synchronises. */
 ARK_M1_API int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* V, double* out);
 
 /* Relative residual history of the last implicit solve: entry 0 = true residual of the initial guess, then one

@@ -66,7 +66,7 @@ typedef struct oracle_m1 {
     int src_off;     /* internal (semi-implicit step): 1 drops the source terms from the residual */
     int hyp_off;     /* internal (semi-implicit step): 1 drops the flux-divergence terms from the assembled operator */
     int krylov;      /* 0: restarted GMRES (north_star, default), 1: BiCGStab (the paper's solver) */
-    int precond_kind;/* 0: 3x3 block-Jacobi (north_star, default), 1: multigrid V-cycle (R12) */
+    int precond_kind;/* 0: 3x3 block-Jacobi (north_star, default), 1: multigrid V-cycle (R15) */
     double mg_omega; /* damping of the block-Jacobi smoother, default 0.8 */
     int mg_coarse_sweeps; /* smoother sweeps on the coarsest (1x1) level, default 2 */
     struct mg_hier *mg;   /* hierarchy of the solve in progress (built by mg_build, freed after the solve) */
@@ -522,7 +522,7 @@ static void precond(const system_t *s, const double *v, double *z)
     }
 }
 /* ------------------------------------------------------------------------------------------------ */
-/* Multigrid preconditioner (the five steps quoted from Saad 2003; R12)  */
+/* Multigrid preconditioner (the five steps quoted from Saad 2003; R15)  */
 /* ------------------------------------------------------------------------------------------------ */
 /* The paper uses an algebraic multigrid from a library (MueLu) and does not specify it.  On this structured grid the
  * hierarchy is geometric: aggregates of 2x2 cells (the last one in a direction is 1 wide when the size is odd), down to

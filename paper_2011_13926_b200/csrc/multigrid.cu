@@ -1,6 +1,6 @@
 // multigrid.cu — geometric-aggregation multigrid V-cycle as the right preconditioner of the Krylov solvers
 // (pre-smoothing, restricted residual equation "R A P y = R r~", coarse solve, interpolation,
-// post-smoothing; the paper takes an algebraic multigrid from a library, reading R12 fixes this one).
+// post-smoothing; the paper takes an algebraic multigrid from a library, reading R15 fixes this one).
 //
 // Everything runs in the block-Jacobi-scaled ("hat") variable of the Krylov core: on level l the operator is
 //   Ahat_l = A_l D_l^-1 = I + sum_k off_k(.)            (unit diagonal blocks, four scaled neighbour blocks, like the fine level)

@@ -1,4 +1,4 @@
-"""GPU parity for the multigrid preconditioner (option preconditioner = 1, R12; SURVEY.md 8(f)
+"""GPU parity for the multigrid preconditioner (option preconditioner = 1, R15; SURVEY.md 8(f)
 row 4): the V-cycle itself element by element against the oracle's, then the preconditioned solves."""
 import numpy as np
 import pytest

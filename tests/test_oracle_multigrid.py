@@ -1,4 +1,4 @@
-"""Pins for the oracle's multigrid preconditioner (R12) -- CPU only.
+"""Pins for the oracle's multigrid preconditioner (R15) -- CPU only.
 
 The hierarchy and the V-cycle are checked against dense / scipy linear algebra built from the assembled fine blocks only
 (`OracleM1.assemble`), never from the multigrid code itself."""
