@@ -249,6 +249,8 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     g = ark.ArkM1(n, n, w["dx"], w["dy"], w["c"], bc=w["bc"], stream=stream)
     g.set_option("operator", args.operator)
+    if args.preconditioner == 1:
+        g.set_option("preconditioner", 1); g.set_option("mg_precision", args.mg_precision)
 
     def reset_device():
         g.set_state(devt["E"], devt["F"], devt["sigma_a"], devt["sigma_s"])
@@ -434,6 +436,19 @@ def run_ours(args):
                                                  "ms_per_iteration": tm["krylov_ms"] / max(its, 1),
                                                  "T_implicit_over_T_explicit": ms / ms_exp, "over_K": ms / ms_exp / ratio,
                                                  "implicit_wins": bool(res <= TOL and ms / ms_exp < ratio)}
+            # the bench step itself (reset + explicit + implicit 10x) with the multigrid preconditioner: a variant, not the headline
+            g.set_option("krylov", 0)
+            reset_device(); one_step()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(3):
+                reset_device()
+                its_v, res_v = one_step()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms_v = e0.elapsed_time(e1) / 3
+            mgo["bench_step_variant"] = {"step": "state reset + 1 explicit + 1 implicit (10x, GMRES(30) + multigrid V-cycle)", "ms_per_step": ms_v,
+                                         "cell_updates_per_s": 2.0 * N / (ms_v * 1e-3), "iterations": its_v, "final_residual": res_v}
             mgo["break_even_reached_at"] = [f"{lab}:{k}" for lab in ("rough_medium", "smooth_problem") for k, v in mgo[lab].items() if v["implicit_wins"]]
             line_extra["multigrid"] = mgo
             g.set_option("preconditioner", 0); g.set_option("krylov", 0)
@@ -506,7 +521,8 @@ def run_ours(args):
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"M1 random medium (BASELINE.json configs[3]) {n}x{n}, fp64, periodic, c=1, seed {args.seed}(+rank)",
-                       "step": "state reset (D2D) + 1 explicit step (CFL 0.4) + 1 implicit step (dt = 10x explicit, GMRES(30) + block-Jacobi, tol 1e-10)",
+                       "step": "state reset (D2D) + 1 explicit step (CFL 0.4) + 1 implicit step (dt = 10x explicit, GMRES(30) + "
+                               + ("block-Jacobi" if args.preconditioner == 0 else f"multigrid V-cycle (fp{args.mg_precision} blocks)") + ", tol 1e-10)",
                        "iterations_per_implicit_step": its_main,
                        "operator": "matrix-free coefficient planes" if args.operator == 1 else "pre-multiplied block stencil (BSR 3x3)", "parallelism": "replicas only (one independent problem per GPU)" if world > 1 else "1 GPU",
                        "l2": f"inputs larger than L2 (state+opacity {5 * N * 8 / 1e6:.0f} MB, Krylov basis {31 * 3 * N * 8 / 1e9:.1f} GB vs 126 MB L2)",
@@ -531,6 +547,9 @@ def main():
     ap.add_argument("--seed", type=int, default=1234)
     ap.add_argument("--operator", type=int, default=1, choices=[0, 1],
                     help="implicit operator: 0 = pre-multiplied block stencil, 1 = matrix-free coefficient planes (default, DESIGN.md)")
+    ap.add_argument("--preconditioner", type=int, default=0, choices=[0, 1],
+                    help="0: 3x3 block-Jacobi (north_star; the default line)  1: multigrid V-cycle (variant run; uses the block-stencil operator)")
+    ap.add_argument("--mg-precision", type=int, default=32, choices=[32, 64], help="storage precision of the multigrid blocks")
     ap.add_argument("--no-sweep", action="store_true", help="skip the dt = 50/100/200x implicit solves")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stage2", action="store_true", help="skip the config-5 (2048^2, matter coupling) implicit step")
