@@ -490,6 +490,23 @@ def run_ours(args):
             ms5e = e0.elapsed_time(e1) / 40
             line_extra["stage2"]["explicit"] = {"ms_per_step": ms5e, "cell_updates_per_s": N5 / (ms5e * 1e-3), "bytes_per_cell": 96,
                                                 "hbm_frac": 96.0 * N5 / (ms5e * 1e-3) / 1e9 / peak_gbs}
+            # the same coupled step with BiCGStab + the multigrid V-cycle (fp32 blocks), at 100x and 1000x
+            g5.set_option("preconditioner", 1); g5.set_option("mg_precision", 32); g5.set_option("krylov", 1)
+            s2mg = {}
+            for ratio in (100.0, 1000.0):
+                for rep in range(2):                          # first pass allocates the hierarchy
+                    g5.set_state(d5["E"], d5["F"], d5["sigma_a"], d5["sigma_s"], d5["T"])
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    its5m, res5m = g5.step_implicit(ratio * dte5, TOL, RESTART, 400)
+                    g5.add_velocity_sources(ratio * dte5)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                ms5m = e0.elapsed_time(e1)
+                s2mg[f"{ratio:g}x"] = {"iterations": its5m, "final_residual": res5m, "converged": bool(res5m <= TOL), "ms": ms5m,
+                                       "cell_updates_per_s": N5 / (ms5m * 1e-3), "T_implicit_over_T_explicit": ms5m / ms5e,
+                                       "over_K": ms5m / ms5e / ratio, "implicit_wins": bool(res5m <= TOL and ms5m / ms5e < ratio)}
+            line_extra["stage2"]["bicgstab_multigrid"] = s2mg
             g5.close()
             del d5
         # ---- roofline of the dominant kernel class ---------------------------------------------------------------
