@@ -41,3 +41,29 @@ def test_implicit_step_4096_satisfies_the_oracles_linear_system(w4096, krylov):
     assert np.linalg.norm((b - Ax).ravel()) <= 2e-10 * np.linalg.norm(b.ravel())
     # sampled cells: the implicit update is not the identity and not the explicit update
     assert rel_l2(x, b) > 1e-3
+
+
+@pytest.mark.parametrize("prec,krylov", [(64, 0), (32, 1)])
+def test_multigrid_step_4096_satisfies_the_oracles_linear_system(w4096, prec, krylov):
+    # the multigrid-preconditioned solve at the bench size, in the configurations bench.py times (fp32 blocks + BiCGStab on the
+    # rough medium; fp64 blocks + GMRES as the reference form): the solution must satisfy the ORACLE's flux-form system
+    w = w4096
+    dt = 10.0 * wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    g = make_gpu(w, dict(preconditioner=1, mg_precision=prec, krylov=krylov))
+    its, res = g.step_implicit(dt, 1e-10, 30, 400)
+    assert res <= 1e-10 and 0 < its < 40
+    E, F = g.get_state()
+    x = np.concatenate((E[None], F))
+    o = make_oracle(w)
+    Ax = o.apply_linear(dt, x, mode=0)
+    b = np.concatenate((w["E"][None], w["F"]))
+    assert np.linalg.norm((b - Ax).ravel()) <= 2e-10 * np.linalg.norm(b.ravel())
+
+
+def test_vcycle_1024_matches_oracle():
+    # 11 levels, many tiles: the cycle element by element against the oracle's at config 3's size
+    w = wl.random_medium(1024, seed=1234)
+    dt = 100.0 * wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    o, g = make_oracle(w, dict(preconditioner=1)), make_gpu(w, dict(preconditioner=1))
+    R = np.random.default_rng(11).standard_normal((3, 1024, 1024))
+    assert rel_l2(g.apply_preconditioner(dt, R), o.mg_apply(dt, R)) <= 1e-9
