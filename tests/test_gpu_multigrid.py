@@ -166,3 +166,26 @@ def test_single_precision_multigrid_solve_meets_the_fp64_tolerance(krylov):
     g.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
     ig2, rg2 = g.step_implicit(dt, 1e-10, 30, 1000)
     assert rg2 <= 1e-10 and abs(ig2 - io) <= max(3, 0.15 * io)
+
+
+def test_marshak_wave_with_multigrid():
+    # PAPER.md:377-383 with dt = 10^4 x explicit, sigma dx = 25 (the regime the paper's AMG is for): 12 BiCGStab iterations per step
+    # instead of 55 with block-Jacobi, same answer
+    from helpers import marshak_diffusion_reference
+    w = wl.marshak(400)
+    nsteps, dt = 300, 10.0
+    Tref = marshak_diffusion_reference(w, dt, nsteps)
+    opts = dict(krylov=1, preconditioner=1)
+    o, g, gj = make_oracle(w, opts), make_gpu(w, opts), make_gpu(w, dict(krylov=1))
+    tot_o = tot_g = tot_j = 0
+    for _ in range(nsteps):
+        tot_o += o.step_implicit(dt, 1e-11, 30, 20000)[0]
+        its, res = g.step_implicit(dt, 1e-11, 30, 20000)
+        assert res <= 1e-10
+        tot_g += its
+        tot_j += gj.step_implicit(dt, 1e-11, 30, 20000)[0]
+    Eg, Fg, Tg = g.get_state(with_T=True)
+    Eo, Fo, To = o.get_state(with_T=True)
+    assert rel_l2(Tg[0], Tref) <= 0.011
+    assert rel_l2(Tg, To) <= 1e-7 and rel_l2(Eg, Eo) <= 1e-7
+    assert abs(tot_g - tot_o) <= 0.05 * tot_o and tot_g * 3 < tot_j
