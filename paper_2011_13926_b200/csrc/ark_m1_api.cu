@@ -6,6 +6,7 @@
 #include <stdlib.h>
 #include <string.h>
 #include <new>
+#include <map>
 #include <vector>
 
 #include "../../include/ark_m1.h"
@@ -25,6 +26,7 @@ struct ark_m1 {
     int device, sm_count;
     long long N;
     long long bytes;
+    std::map<void*, size_t>* allocs;   // device allocations counted in `bytes`
     bool have_state, have_T;
     // state: two buffers of 3N doubles [E | Fx | Fy]; U[cur] is current
     double* U[2];
@@ -101,7 +103,18 @@ static int dmalloc(ark_m1* h, void** p, size_t bytes)
     cudaError_t e = cudaMalloc(p, bytes);
     if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return fail(h, ARK_M1_E_ALLOC, "cudaMalloc: %s", cudaGetErrorString(e)); }
     h->bytes += (long long)bytes;
+    if (h->allocs) (*h->allocs)[*p] = bytes;
     return 0;
+}
+
+// cudaFree of a dmalloc'ed pointer with the byte count kept right (null is fine)
+static void dfree(ark_m1* h, void* p)
+{
+    if (!p) return;
+    cudaFree(p);
+    if (!h->allocs) return;
+    auto it = h->allocs->find(p);
+    if (it != h->allocs->end()) { h->bytes -= (long long)it->second; h->allocs->erase(it); }
 }
 
 // the multigrid hierarchy is built from assembled blocks: it overrides the matrix-free operator
@@ -142,6 +155,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     h->hist_host = new std::vector<double>();
+    h->allocs = new std::map<void*, size_t>();
     h->kev = new std::vector<cudaEvent_t>(); h->kcls = new std::vector<int>(); h->kbytes = new std::vector<double>();
     const size_t N = (size_t)h->N;
     bool ok = true;
@@ -165,11 +179,11 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
 
 static void free_implicit(ark_m1* h)
 {
-    for (int l = 0; l < h->mg.nlev; ++l) { cudaFree(h->mg.lev[l].off32); h->mg.lev[l].off32 = nullptr; }
-    for (int l = 1; l < h->mg.nlev; ++l) { cudaFree(h->mg.lev[l].off); cudaFree(h->mg.lev[l].Dinv); cudaFree(h->mg.lev[l].r); cudaFree(h->mg.lev[l].e); }
-    h->mg.nlev = 0; cudaFree(h->mgz); h->mgz = nullptr;
-    cudaFree(h->A.off); cudaFree(h->A.C); cudaFree(h->A.Minv); cudaFree(h->A.b); cudaFree(h->V); cudaFree(h->tvec); cudaFree(h->wblock); cudaFree(h->nprev); h->nprev = nullptr;
-    cudaFree(h->mf.J); cudaFree(h->mf.fE); cudaFree(h->mf.fN); cudaFree(h->mf.dE); cudaFree(h->mf.dF); cudaFree(h->mf.xlo); cudaFree(h->mf.ylo);
+    for (int l = 0; l < h->mg.nlev; ++l) { dfree(h, h->mg.lev[l].off32); h->mg.lev[l].off32 = nullptr; }
+    for (int l = 1; l < h->mg.nlev; ++l) { dfree(h, h->mg.lev[l].off); dfree(h, h->mg.lev[l].Dinv); dfree(h, h->mg.lev[l].r); dfree(h, h->mg.lev[l].e); }
+    h->mg.nlev = 0; dfree(h, h->mgz); h->mgz = nullptr;
+    dfree(h, h->A.off); dfree(h, h->A.C); dfree(h, h->A.Minv); dfree(h, h->A.b); dfree(h, h->V); dfree(h, h->tvec); cudaFree(h->wblock); dfree(h, h->nprev); h->nprev = nullptr;
+    dfree(h, h->mf.J); dfree(h, h->mf.fE); dfree(h, h->mf.fN); dfree(h, h->mf.dE); dfree(h, h->mf.dF); dfree(h, h->mf.xlo); dfree(h, h->mf.ylo);
     memset(&h->mf, 0, sizeof h->mf);
     h->A.off = h->A.C = h->A.Minv = h->A.b = nullptr; h->V = h->tvec = nullptr; h->wblock = nullptr; h->m_alloc = 0; h->maxit_alloc = 0;
 }
@@ -185,7 +199,7 @@ void ark_m1_destroy(ark_m1* h)
     free_implicit(h);
     if (h->ctl_host) cudaFreeHost(h->ctl_host);
     for (int k = 0; k < 3; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
-    delete h->hist_host;
+    delete h->hist_host; delete h->allocs; h->allocs = nullptr;
     if (h->kev) for (cudaEvent_t e : *h->kev) cudaEventDestroy(e);
     delete h->kev; delete h->kcls; delete h->kbytes;
     cudaGetLastError();
@@ -270,7 +284,7 @@ int ark_m1_set_field(ark_m1* h, const char* name, const double* plane)
     else if (!strcmp(name, "uy")) dst = &h->uy; else if (!strcmp(name, "source_E")) dst = &h->source_E;
     else return fail(h, ARK_M1_E_ARG, "unknown field %s", name);
     const size_t B = (size_t)h->N * sizeof(double);
-    if (!plane) { CU(cudaStreamSynchronize(h->st)); if (*dst) { cudaFree(*dst); h->bytes -= (long long)B; } *dst = nullptr; return 0; }
+    if (!plane) { CU(cudaStreamSynchronize(h->st)); dfree(h, *dst); *dst = nullptr; return 0; }
     if (!*dst) { int rc = dmalloc(h, (void**)dst, B); if (rc) return rc; }
     CU(cudaMemcpyAsync(*dst, plane, B, cudaMemcpyDefault, h->st));
     return 0;
@@ -429,7 +443,7 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
     }
     h->stride = (long long)((n + 31) / 32 * 32) + h->basis_pad;
     if (h->m_alloc < m) {
-        if (h->V) { cudaFree(h->V); h->bytes -= (long long)((size_t)(h->m_alloc + 1) * h->stride * sizeof(double)); h->V = nullptr; }
+        dfree(h, h->V); h->V = nullptr;
         int rc = dmalloc(h, (void**)&h->V, (size_t)(m + 1) * h->stride * sizeof(double));
         if (rc) { h->m_alloc = 0; return rc; }
     }

@@ -189,3 +189,20 @@ def test_marshak_wave_with_multigrid():
     assert rel_l2(Tg[0], Tref) <= 0.011
     assert rel_l2(Tg, To) <= 1e-7 and rel_l2(Eg, Eo) <= 1e-7
     assert abs(tot_g - tot_o) <= 0.05 * tot_o and tot_g * 3 < tot_j
+
+
+def test_device_bytes_accounting_with_the_hierarchy():
+    w = small_random_state(64, 48, seed=3)
+    g = make_gpu(w)
+    b0 = g.device_bytes()
+    g.step_implicit(_dt(w, 20.0), 1e-10, 30, 500)
+    b1 = g.device_bytes()
+    g.set_option("preconditioner", 1); g.set_option("mg_precision", 32)
+    g.step_implicit(_dt(w, 20.0), 1e-10, 30, 500)
+    b2 = g.device_bytes()
+    N = 64 * 48
+    assert b1 > b0 and b2 - b1 >= (45 + 3) * 8 * N + 36 * 4 * N      # block stencil + V-cycle vector + fp32 copy at least
+    g.set_option("basis_pad", 32)                                     # releases the implicit workspace
+    assert g.device_bytes() == b0
+    its, res = g.step_implicit(_dt(w, 20.0), 1e-10, 30, 500)          # and it comes back
+    assert res <= 1e-10 and b0 < g.device_bytes() < b2            # this time without the matrix-free planes of the first solve
