@@ -410,6 +410,40 @@ def run_ours(args):
             bi["break_even_reached_at"] = wins
             line_extra["bicgstab"] = bi
             g.set_option("krylov", 0)
+        # ---- compressed-basis GMRES (option basis_precision = 32: Arnoldi vectors stored in fp32, fp64 arithmetic and fp64 exit test) ----
+        if not args.no_sweep:
+            g.set_option("basis_precision", 32)
+            cbo = {"rough_medium": {}, "smooth_problem": {}}
+            for label, tensors, ratios in (("rough_medium", devt, (10.0, 50.0)), ("smooth_problem", None, (100.0,))):
+                if tensors is None:
+                    ws = wl.gaussian_diffusion(n)
+                    tensors = {k: torch.from_numpy(np.ascontiguousarray(ws[k])).to(dev) for k in ("E", "F", "sigma_a", "sigma_s")}
+                for ratio in ratios:
+                    for rep in range(2 if (label == "rough_medium" and ratio == 10.0) else 1):      # first call allocates the fp32 basis
+                        g.set_state(tensors["E"], tensors["F"], tensors["sigma_a"], tensors["sigma_s"])
+                        torch.cuda.synchronize()
+                        e0.record(stream)
+                        its, res = g.step_implicit(ratio * dt_e, TOL, RESTART, MAXIT)
+                        e1.record(stream)
+                        torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1)
+                    tm = g.timings()
+                    cbo[label][f"{ratio:g}x"] = {"iterations": its, "final_residual": res, "converged": bool(res <= TOL), "ms": ms,
+                                                 "ms_per_iteration": tm["krylov_ms"] / max(its, 1),
+                                                 "bytes_per_cell_per_iteration_mean_m30": 684, "T_implicit_over_T_explicit": ms / ms_exp}
+            reset_device(); one_step()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(3):
+                reset_device()
+                its_v, res_v = one_step()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms_v = e0.elapsed_time(e1) / 3
+            cbo["bench_step_variant"] = {"step": "state reset + 1 explicit + 1 implicit (10x, GMRES(30) + block-Jacobi, fp32-stored basis)", "ms_per_step": ms_v,
+                                         "cell_updates_per_s": 2.0 * N / (ms_v * 1e-3), "iterations": its_v, "final_residual": res_v}
+            line_extra["compressed_basis"] = cbo
+            g.set_option("basis_precision", 64)
         # ---- multigrid preconditioner (SURVEY 8(f) row 4 "stronger preconditioner"): option preconditioner = 1,
         #      blocks stored in fp32 (mg_precision = 32); BiCGStab on the rough medium, GMRES(30) on the smooth problem ----------------
         if not args.no_sweep:

@@ -96,6 +96,10 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                       3: row-marching kernel with a three-slot register rotation (no window copies)
  *   "operator"          1: matrix-free coefficient planes, flux form (default: 5% faster per solve at 4096^2)
  *                       0: block stencil (BSR 3x3 on the 5-point graph, pre-multiplied by M^-1)
+ *   "basis_precision"   64 (default) or 32: storage precision of the GMRES Arnoldi basis.  32 = compressed-basis GMRES: the basis
+ *                       vectors are stored in single precision, every computation (operator, dots, updates, Hessenberg,
+ *                       solution, true residual at each restart) stays fp64 and the solve ends at the same fp64 tolerance;
+ *                       applies to GMRES + block-Jacobi + matrix-free operator + one-pass orthogonalisation, ignored otherwise
  *   "preconditioner"    0: 3x3 block-Jacobi (north_star; default)
  *                       1: multigrid V-cycle (R15): 2x2 cell aggregates down to one cell, Galerkin
  *                          coarse operators, one damped block-Jacobi sweep before and after; uses the block-stencil operator

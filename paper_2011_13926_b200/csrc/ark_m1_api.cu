@@ -37,6 +37,10 @@ struct ark_m1 {
     unsigned long long* counts;   // 2
     // options
     int ortho, explicit_kernel, op_kind, maxv, basis_pad, krylov, asm_kernel;
+    int basis_prec;    // 64, or 32: compressed-basis GMRES (krylov_cb.cu); applies to GMRES + block-Jacobi + matrix-free operator
+    float* V32;        // (m32_alloc + 1) basis vectors of `stride` floats
+    double* wk;        // 3N: the fp64 work vector of the compressed-basis path
+    int m32_alloc, vslots;
     int precond;       // 0: 3x3 block-Jacobi, 1: multigrid V-cycle (forces the assembled block-stencil operator)
     MgHier mg;         // hierarchy (levels >= 1 allocated lazily)
     double* mgz;       // 3N: V-cycle output (hat variable)
@@ -120,6 +124,9 @@ static void dfree(ark_m1* h, void* p)
 // the multigrid hierarchy is built from assembled blocks: it overrides the matrix-free operator
 static inline int opk(const ark_m1* h) { return h->precond == 1 ? 0 : h->op_kind; }
 
+// compressed-basis GMRES applies to the default solver configuration only; elsewhere the option is ignored
+static inline bool use_cb(const ark_m1* h) { return h->basis_prec == 32 && h->krylov == 0 && h->precond == 0 && h->op_kind == 1 && h->ortho == 1; }
+
 static Fields fields_of(const ark_m1* h)
 {
     Fields f;
@@ -151,7 +158,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
     h->ortho = 1; h->explicit_kernel = 1; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0; h->asm_kernel = 1;
-    h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
+    h->basis_prec = 64; h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     h->hist_host = new std::vector<double>();
@@ -182,6 +189,7 @@ static void free_implicit(ark_m1* h)
     for (int l = 0; l < h->mg.nlev; ++l) { dfree(h, h->mg.lev[l].off32); h->mg.lev[l].off32 = nullptr; }
     for (int l = 1; l < h->mg.nlev; ++l) { dfree(h, h->mg.lev[l].off); dfree(h, h->mg.lev[l].Dinv); dfree(h, h->mg.lev[l].r); dfree(h, h->mg.lev[l].e); }
     h->mg.nlev = 0; dfree(h, h->mgz); h->mgz = nullptr;
+    dfree(h, h->V32); h->V32 = nullptr; dfree(h, h->wk); h->wk = nullptr; h->m32_alloc = 0; h->vslots = 0;
     dfree(h, h->A.off); dfree(h, h->A.C); dfree(h, h->A.Minv); dfree(h, h->A.b); dfree(h, h->V); dfree(h, h->tvec); cudaFree(h->wblock); dfree(h, h->nprev); h->nprev = nullptr;
     dfree(h, h->mf.J); dfree(h, h->mf.fE); dfree(h, h->mf.fN); dfree(h, h->mf.dE); dfree(h, h->mf.dF); dfree(h, h->mf.xlo); dfree(h, h->mf.ylo);
     memset(&h->mf, 0, sizeof h->mf);
@@ -271,6 +279,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
     else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
     else if (!strcmp(key, "mg_coarse_sweeps")) { if (iv < 1) return fail(h, ARK_M1_E_ARG, "mg_coarse_sweeps must be >= 1%s", ""); h->mg.coarse_sweeps = iv; }
+    else if (!strcmp(key, "basis_precision")) { if (iv != 32 && iv != 64) return fail(h, ARK_M1_E_ARG, "basis_precision must be 64 or 32%s", ""); h->basis_prec = iv; }
     else if (!strcmp(key, "mg_precision")) { if (iv != 32 && iv != 64) return fail(h, ARK_M1_E_ARG, "mg_precision must be 64 or 32%s", ""); h->mg.precision = iv; }
     else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
     return 0;
@@ -387,7 +396,8 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
 {
     const size_t N = (size_t)h->N, n = 3 * N;
     const bool have_op = (opk(h) == 0) ? (h->A.off != nullptr) : (h->mf.J != nullptr);
-    if (h->m_alloc >= m && h->maxit_alloc >= maxit && have_op && (h->precond == 0 || (h->mg.nlev > 0 && (h->mg.precision == 64 || h->mg.lev[0].off32)))) return 0;
+    if (h->m_alloc >= m && h->maxit_alloc >= maxit && have_op && (h->precond == 0 || (h->mg.nlev > 0 && (h->mg.precision == 64 || h->mg.lev[0].off32)))
+        && h->vslots >= (use_cb(h) ? 6 : ((m + 1) > 6 ? (m + 1) : 6)) && (!use_cb(h) || (h->m32_alloc >= m && h->wk))) return 0;
     CU(cudaStreamSynchronize(h->st));
     const long long before = h->bytes;
     (void)before;
@@ -442,10 +452,23 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
         }
     }
     h->stride = (long long)((n + 31) / 32 * 32) + h->basis_pad;
-    if (h->m_alloc < m) {
-        dfree(h, h->V); h->V = nullptr;
-        int rc = dmalloc(h, (void**)&h->V, (size_t)(m + 1) * h->stride * sizeof(double));
-        if (rc) { h->m_alloc = 0; return rc; }
+    {   // fp64 vector slots: the whole basis, or (compressed-basis path) the six slots BiCGStab and the staging calls use
+        const int need = use_cb(h) ? 6 : ((m + 1) > 6 ? (m + 1) : 6);
+        if (h->vslots < need) {
+            dfree(h, h->V); h->V = nullptr; h->vslots = 0;
+            int rc = dmalloc(h, (void**)&h->V, (size_t)need * h->stride * sizeof(double));
+            if (rc) return rc;
+            h->vslots = need;
+        }
+        if (use_cb(h)) {
+            int rc;
+            if (h->m32_alloc < m) {
+                dfree(h, h->V32); h->V32 = nullptr; h->m32_alloc = 0;
+                if ((rc = dmalloc(h, (void**)&h->V32, (size_t)(m + 1) * h->stride * sizeof(float)))) return rc;
+                h->m32_alloc = m;
+            }
+            if (!h->wk && (rc = dmalloc(h, (void**)&h->wk, n * sizeof(double)))) return rc;
+        }
     }
     const int mm = m > h->m_alloc ? m : h->m_alloc;
     const int mi = maxit > h->maxit_alloc ? maxit : h->maxit_alloc;
@@ -582,6 +605,56 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
     return 0;
 }
 
+// Compressed-basis GMRES(m) (krylov_cb.cu; option "basis_precision" = 32): same algorithm and control flow as gmres_solve, the
+// Arnoldi vectors stored in single precision (h->V32), one fp64 work vector (h->wk) carrying w = A M^-1 v_j through the
+// orthogonalisation.  The true fp64 residual b - A x is recomputed at every restart, so the exit test is the same.
+static int true_residual_cb(ark_m1* h, const double* x)
+{
+    const long long n = 3 * h->N;
+    KL(KC_SPMV, 216.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, x, h->wk, nullptr, h->A.b, -1.0, nullptr, 0, h->sm_count, h->st));
+    KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->wk, h->wk, 0, 1, 0, n, h->W, DOT_RNORM, h->sm_count, h->st));
+    KL(KC_UPDATE, 36.0 * h->N, launch_mg_to_float(h->wk, h->V32, n, h->st));          // v_0 = r, rounded once
+    return 0;
+}
+
+static int gmres_solve_cb(ark_m1* h, double tol, int m, int maxit)
+{
+    int rc;
+    const long long n = 3 * h->N, S = h->stride;
+    const int sm = h->sm_count;
+    double* x = h->U[h->cur];
+    double* w = h->wk;
+    GmresWork W = h->W;
+    const int* stop = &W.ctl->inner_stop;
+    const int MV = h->maxv < 16 ? h->maxv : 16;
+    KL(KC_SMALL, 0.0, launch_begin_solve(W, tol, m, maxit, h->st));
+    KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
+    if ((rc = true_residual_cb(h, x))) return rc;
+    if ((rc = fetch_ctl(h))) return rc;
+    while (!h->ctl_host->inner_stop) {
+        for (int j = 0; j < m; ++j) {
+            float* vnext = h->V32 + (size_t)(j + 1) * S;
+            KL(KC_SPMV, 252.0 * h->N, launch_op_mf_f32(h->g, h->mf, h->A.Minv, h->V32 + (size_t)j * S, w, W.scale + j, stop, sm, h->st));
+            for (int c0 = 0; c0 <= j; c0 += MV) {
+                const int nv = (j + 1 - c0) < MV ? (j + 1 - c0) : MV;
+                KL(KC_DOT, (24.0 + 12.0 * nv) * h->N, launch_multi_dot32(w, h->V32 + (size_t)c0 * S, S, nv, c0, n, W, DOT_H, sm, h->st));
+            }
+            for (int c0 = 0; c0 <= j; c0 += MV) {
+                const int nv = (j + 1 - c0) < MV ? (j + 1 - c0) : MV;
+                const int last = (c0 + MV > j);
+                // intermediate chunks update w in place; the last one only stores the rounded result as v_{j+1} and its norm
+                KL(KC_UPDATE, (24.0 + 12.0 * nv + (last ? 12.0 : 24.0)) * h->N,
+                   launch_update32(w, h->V32 + (size_t)c0 * S, S, nv, c0, n, W, last, last ? 0 : 1, last ? vnext : nullptr, sm, h->st));
+            }
+        }
+        KL(KC_SMALL, 0.0, launch_solve_y(W, h->st));
+        KL(KC_COMBINE, 8.0 * (1.5 * m + 15.0) * h->N, launch_combine32(h->g, h->V32, S, h->A.Minv, x, W, sm, h->st));
+        if ((rc = true_residual_cb(h, x))) return rc;
+        if ((rc = fetch_ctl(h))) return rc;
+    }
+    return 0;
+}
+
 // Right-preconditioned BiCGStab (the paper's Krylov method) on the assembled system; same conventions as
 // gmres_solve.  Vector slots of h->V: 0 = r (and s), 1 = t, 2 = r^, 3 = p, 4 = v, 5 = y (x = x0 + M^-1 y).
 // Iterations are enqueued in batches of 8 without host round trips; one iteration = two operator applications.
@@ -680,7 +753,7 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
     CU(cudaEventRecord(h->ev[0], h->st));
     if ((rc = assemble_system(h, dt))) return rc;
     CU(cudaEventRecord(h->ev[1], h->st));
-    if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : gmres_solve(h, tol, restart, maxit))) return rc;
+    if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : (use_cb(h) ? gmres_solve_cb(h, tol, restart, maxit) : gmres_solve(h, tol, restart, maxit)))) return rc;
     CU(cudaEventRecord(h->ev[2], h->st));
     if ((rc = finish_implicit(h, dt, final_residual))) return rc;
     return h->ctl_host->its;
@@ -710,7 +783,7 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
     for (k = 0; k < max_newton; ++k) {
         CU(cudaMemcpyAsync(h->nprev, x, n * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
         if ((rc = assemble_system(h, dt, base))) return rc;
-        if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : gmres_solve(h, tol, restart, maxit))) return rc;
+        if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : (use_cb(h) ? gmres_solve_cb(h, tol, restart, maxit) : gmres_solve(h, tol, restart, maxit)))) return rc;
         total += h->ctl_host->its;
         if (h->ctl_host->nonfinite) break;
         KL(KC_SMALL, 72.0 * h->N, launch_sub(h->nprev, x, h->nprev, (long long)n, h->st));

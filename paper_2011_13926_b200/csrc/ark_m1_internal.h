@@ -95,6 +95,8 @@ cudaError_t launch_assemble_march(const Grid& g, const Scheme& s, const Fields& 
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
                          int sm_count, cudaStream_t st);
+cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Minv, const float* v, double* out,
+                             const double* scale_ptr, const int* skip_flag, int sm_count, cudaStream_t st);
 cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, cudaStream_t st);
 // t = C x
 cudaError_t launch_diag_mul(const Grid& g, const double* Cblk, const double* x, double* t, cudaStream_t st);
@@ -137,6 +139,13 @@ cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
 // x += Minv * (sum_{k<ctl->j} coef[k] V_k)  per cell;  Minv == nullptr: x = sum_{k<ctl->j} coef[k] V_k
 cudaError_t launch_combine(const Grid& g, const double* V, long long stride, const double* Minv, double* x,
                            GmresWork W, int sm_count, cudaStream_t st);
+// compressed-basis GMRES (krylov_cb.cu): basis vectors stored in single precision, fp64 arithmetic; nv <= 16
+cudaError_t launch_multi_dot32(const double* w, const float* V0, long long stride, int nv, int col0, long long n,
+                               GmresWork W, int mode, int sm_count, cudaStream_t st);
+cudaError_t launch_update32(double* w, const float* V0, long long stride, int nv, int col0, long long n, GmresWork W,
+                            int with_norm, int write_w, float* out32, int sm_count, cudaStream_t st);
+cudaError_t launch_combine32(const Grid& g, const float* V, long long stride, const double* Minv, double* x,
+                             GmresWork W, int sm_count, cudaStream_t st);
 // BiCGStab vector kernels (krylov_kernels.cu); every one returns at once when ctl->inner_stop is set
 cudaError_t launch_bicg_begin(double* r, double* rhat, double* p, double* v, long long n, GmresWork W, cudaStream_t st);
 cudaError_t launch_bicg_p(const double* r, double* p, const double* v, long long n, GmresWork W, cudaStream_t st);      // p = r + beta (p - omega v)

@@ -32,8 +32,8 @@ struct FC { double ap, Lam, alpha, sw; };            // face coefficients; sw = 
 
 // z and Pi of the cell in column (xmode, ii) and row j (j may be -1 or ny).  Dirichlet ghosts carry z = 0 (their
 // contribution is in b), outflow ghosts copy the adjacent cell, periodic ghosts wrap (R9).
-template <bool PRECOND>
-__device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const double* __restrict__ v, const double* __restrict__ Minv,
+template <bool PRECOND, typename TIN>
+__device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const TIN* __restrict__ v, const double* __restrict__ Minv,
                                       const double* __restrict__ J, double c2, int xmode, int ii, int j)
 {
     ZP r; r.zE = 0.0; r.zFx = 0.0; r.zFy = 0.0; r.Pxx = 0.0; r.Pxy = 0.0; r.Pyy = 0.0; r.v0 = 0.0; r.v1 = 0.0; r.v2 = 0.0;
@@ -45,7 +45,7 @@ __device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const double* 
         jj = (bc == BC_PERIODIC) ? ((j < 0) ? g.ny - 1 : 0) : ((j < 0) ? 0 : g.ny - 1);
     }
     const long long id = (long long)jj * g.nx + ii;
-    const double v0 = v[id], v1 = v[N + id], v2 = v[2 * N + id];
+    const double v0 = (double)v[id], v1 = (double)v[N + id], v2 = (double)v[2 * N + id];
     r.v0 = v0; r.v1 = v1; r.v2 = v2;
     if (PRECOND) {
         r.zE  = Minv[0 * N + id] * v0 + Minv[1 * N + id] * v1 + Minv[2 * N + id] * v2;
@@ -68,8 +68,9 @@ struct ZPub { double zE, zFx, zFy, Pxx, Pxy; };
 
 // DOT (BiCGStab fusions, saving the separate reduction passes): 0 none; 1: <out, aux> -> epilogue BICG_ALPHA;
 // 2: <out, v>, <out, out> -> epilogue BICG_OMEGA (v = the kernel's own input, already in registers).
-template <bool PRECOND, int DOT>
-__global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const double* __restrict__ v,
+// TIN = float: the input vector is a single-precision (compressed) Krylov basis vector (krylov_cb.cu); all arithmetic is fp64.
+template <bool PRECOND, int DOT, typename TIN = double>
+__global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
                                                     double* __restrict__ out, const double* __restrict__ scale_ptr,
                                                     const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
                                                     int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W)
@@ -98,8 +99,8 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
     const bool east_valid = (i < g.nx) && (xmode != 2);    // this thread owns the face between columns i and i+1
     const double sc = sgn * (scale_ptr ? *scale_ptr : 1.0);
 
-    ZP zS = load_zp<PRECOND>(g, N, v, Minv, mf.J, c2, xmode, ii, j0 - 1);
-    ZP zC = load_zp<PRECOND>(g, N, v, Minv, mf.J, c2, xmode, ii, j0);
+    ZP zS = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0 - 1);
+    ZP zC = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0);
     double Hs0 = 0.0, Hs1 = 0.0, Hs2 = 0.0, Ss = 0.0;
     if (upd) {
         // south face of row j0: the north face of row j0-1, or the stored low-side line / the wrapped last row
@@ -113,7 +114,7 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
     for (int j = j0; j < j1; ++j) {
         // issue every global load of this row first (north cell, face coefficients, source weights); they are consumed
         // after the two barriers of the x-face exchange, which needs only data already in registers
-        const ZP zN = load_zp<PRECOND>(g, N, v, Minv, mf.J, c2, xmode, ii, j + 1);
+        const ZP zN = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j + 1);
         const long long id = (long long)j * g.nx + (upd ? i : 0);
         FC fn; fn.ap = 0.5; fn.Lam = 0.0; fn.alpha = 1.0; fn.sw = 0.0;
         double dE = 0.0, dF = 0.0, a0 = 0.0, a1 = 0.0, a2 = 0.0;
@@ -180,6 +181,17 @@ cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Mi
     const double c2 = g.c * g.c;
     if (dot == 1) op_mf_kernel<true, 1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
     else op_mf_kernel<true, 2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+    return cudaGetLastError();
+}
+
+// out = s * A M^-1 v with v stored in single precision
+cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Minv, const float* v, double* out,
+                             const double* scale_ptr, const int* skip_flag, int sm_count, cudaStream_t st)
+{
+    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY);
+    const double c2 = g.c * g.c;
+    GmresWork none; memset(&none, 0, sizeof none);
+    op_mf_kernel<true, 0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     return cudaGetLastError();
 }
 
