@@ -526,7 +526,8 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
     } else {
         MfPlanes none; memset(&none, 0, sizeof none);
         KL(KC_ASSEMBLE, 496.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, none, bsrc, h->st));
-        KL(KC_SCALE, 648.0 * h->N, launch_scale_offdiag(h->g, h->A, h->st));
+        float* o32 = (h->precond == 1 && h->mg.precision == 32) ? h->mg.lev[0].off32 : nullptr;
+        KL(KC_SCALE, (648.0 + (o32 ? 144.0 : 0.0)) * h->N, launch_scale_offdiag(h->g, h->A, o32, h->st));
     }
     if (h->precond == 1) {       // Galerkin hierarchy: each level reads 36 doubles per finer cell, writes 45 (+ the scaling pass) per cell
         h->mg.lev[0].off = h->A.off;
@@ -534,13 +535,9 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
             const MgLevel& f = h->mg.lev[l - 1]; const MgLevel& c = h->mg.lev[l];
             const double Nf = (double)f.g.nx * f.g.ny, Nc = (double)c.g.nx * c.g.ny;
             h->launches++;      // two kernels per level
-            KL(KC_MGSETUP, 288.0 * Nf + (360.0 + 648.0) * Nc, launch_mg_galerkin(f.g, f.off, c.g, c.off, c.Dinv, h->st));
+            KL(KC_MGSETUP, 288.0 * Nf + (360.0 + 648.0) * Nc, launch_mg_galerkin(f.g, f.off, c.g, c.off, c.Dinv, h->mg.precision == 32 ? c.off32 : nullptr, h->st));
         }
-        if (h->mg.precision == 32)
-            for (int l = 0; l < h->mg.nlev; ++l) {
-                const long long cnt = 36LL * h->mg.lev[l].g.nx * h->mg.lev[l].g.ny;
-                KL(KC_MGSETUP, 12.0 * cnt, launch_mg_to_float(h->mg.lev[l].off, h->mg.lev[l].off32, cnt, h->st));
-            }
+
     }
     return 0;
 }

@@ -97,7 +97,7 @@ cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, 
                          int sm_count, cudaStream_t st);
 cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Minv, const float* v, double* out,
                              const double* scale_ptr, const int* skip_flag, int sm_count, cudaStream_t st);
-cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, cudaStream_t st);
+cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, float* off32, cudaStream_t st);   // off32: optional fp32 copy
 // t = C x
 cudaError_t launch_diag_mul(const Grid& g, const double* Cblk, const double* x, double* t, cudaStream_t st);
 // out = sgn*(s*(v + sum_k Ahat_k v_nbr)) + (add ? add : 0);  s = *scale_ptr[scale_idx] if scale_ptr else 1
@@ -121,8 +121,8 @@ struct MgLevel {
 };
 struct MgHier { int nlev; MgLevel lev[MG_MAXLEV]; double omega; int coarse_sweeps; int precision; };
 // coarse blocks of one level from the finer one (Galerkin, 2x2 aggregates): writes coff (scaled) and cDinv
-cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc, double* coff, double* cDinv, cudaStream_t st);
-cudaError_t launch_mg_to_float(const double* a, float* b, long long n, cudaStream_t st);
+cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc, double* coff, double* cDinv, float* coff32, cudaStream_t st);
+cudaError_t launch_mg_to_float(const double* a, float* b, long long n, cudaStream_t st);   // b = (float) a
 // zhat_out = one V-cycle on r_in (level-0 vectors of 3N doubles, distinct); *nl = kernels launched
 cudaError_t launch_mg_vcycle(const MgHier& H, const double* r_in, double* zhat_out, const int* skip_flag, cudaStream_t st, int* nl);
 

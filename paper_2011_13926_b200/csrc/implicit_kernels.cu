@@ -185,8 +185,8 @@ __device__ __forceinline__ long long nbr_index(const Grid& g, int i, int j, int 
     return (long long)jj * g.nx + ii;
 }
 
-// off_k <- off_k * Minv(neighbour k), in place.
-__global__ void __launch_bounds__(128) scale_offdiag_kernel(Grid g, BlockMatrix A)
+// off_k <- off_k * Minv(neighbour k), in place; off32 (may be null) receives a single-precision copy (multigrid, mg_precision = 32).
+__global__ void __launch_bounds__(128) scale_offdiag_kernel(Grid g, BlockMatrix A, float* __restrict__ off32)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -201,15 +201,18 @@ __global__ void __launch_bounds__(128) scale_offdiag_kernel(Grid g, BlockMatrix 
 #pragma unroll
         for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int cc = 0; cc < 3; ++cc)
-                A.off[(k * 9 + 3 * r + cc) * N + id] = a[3 * r] * m[cc] + a[3 * r + 1] * m[3 + cc] + a[3 * r + 2] * m[6 + cc];
+            for (int cc = 0; cc < 3; ++cc) {
+                const double v = a[3 * r] * m[cc] + a[3 * r + 1] * m[3 + cc] + a[3 * r + 2] * m[6 + cc];
+                A.off[(k * 9 + 3 * r + cc) * N + id] = v;
+                if (off32) off32[(k * 9 + 3 * r + cc) * N + id] = (float)v;
+            }
     }
 }
 
-cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, cudaStream_t st)
+cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, float* off32, cudaStream_t st)
 {
     dim3 blk(32, 4), grd((g.nx + 31) / 32, (g.ny + 3) / 4);
-    scale_offdiag_kernel<<<grd, blk, 0, st>>>(g, A);
+    scale_offdiag_kernel<<<grd, blk, 0, st>>>(g, A, off32);
     return cudaGetLastError();
 }
 

@@ -73,13 +73,13 @@ __global__ void __launch_bounds__(128) mg_galerkin_kernel(Grid gf, const double*
         for (int e = 0; e < 9; ++e) coff[(long long)(k * 9 + e) * Nc + a] = Ck[k].a[e];
 }
 
-cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc, double* coff, double* cDinv, cudaStream_t st)
+cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc, double* coff, double* cDinv, float* coff32, cudaStream_t st)
 {
     dim3 blk(32, 4), grd((gc.nx + 31) / 32, (gc.ny + 3) / 4);
     mg_galerkin_kernel<<<grd, blk, 0, st>>>(gf, off, gc, coff, cDinv);
     if (cudaGetLastError() != cudaSuccess) return cudaErrorLaunchFailure;
     BlockMatrix C; C.off = coff; C.C = nullptr; C.Minv = cDinv; C.b = nullptr;
-    return launch_scale_offdiag(gc, C, st);
+    return launch_scale_offdiag(gc, C, coff32, st);
 }
 
 // ---- V-cycle pass 1: r_c = P0^T ((1 - omega) r - omega sum_k off_k r_nbr) --------------------------------------------
