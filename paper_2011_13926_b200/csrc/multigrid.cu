@@ -17,6 +17,10 @@
 
 namespace ark {
 
+#ifndef ARK_MG_BY
+#define ARK_MG_BY 4          // rows of threads per block of the V-cycle kernels (32 x ARK_MG_BY threads)
+#endif
+
 // Neighbour k (0: W, 1: E, 2: S, 3: N) of cell (i, j): its index on the level and, through `agg`, its aggregate on the next
 // coarser level (cnx aggregates per row).  Non-periodic sides clamp (the block there is zero).
 __device__ __forceinline__ long long mg_nbr(const Grid& g, int i, int j, int k, int cnx, long long& agg)
@@ -85,7 +89,7 @@ cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc
 // ---- V-cycle pass 1: r_c = P0^T ((1 - omega) r - omega sum_k off_k r_nbr) --------------------------------------------
 // Thread (i, J) handles the fine cells (i, 2J) and (i, 2J+1); lane pairs (i even, i+1) add up through a shuffle.
 template <typename TB>
-__global__ void __launch_bounds__(128) mg_restrict_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(32 * ARK_MG_BY) mg_restrict_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                           double omega, int cnx, double* __restrict__ rc,
                                                           const int* __restrict__ skip_flag)
 {
@@ -126,7 +130,7 @@ __global__ void __launch_bounds__(128) mg_restrict_kernel(Grid g, const TB* __re
 
 // ---- V-cycle pass 2: t = omega r + P0 e_c;  z^ = t + omega (r - t - sum_k off_k t_nbr);  out = Dinv z^ (coarse levels) or z^ ----
 template <typename TB>
-__global__ void __launch_bounds__(128) mg_prolong_smooth_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(32 * ARK_MG_BY) mg_prolong_smooth_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                                 double omega, int cnx, const double* __restrict__ ec,
                                                                 const double* __restrict__ Dinv, double* __restrict__ out,
                                                                 const int* __restrict__ skip_flag)
@@ -159,6 +163,130 @@ __global__ void __launch_bounds__(128) mg_prolong_smooth_kernel(Grid g, const TB
     } else {
         out[id] = z0; out[N + id] = z1; out[2 * N + id] = z2;
     }
+}
+
+// ---- pair kernels: two adjacent cells (2I, 2I+1) per thread, blocks and vectors read as 2-element vectors ----------------
+// Used on every level with an even nx (all levels of a power-of-two grid): half as many load instructions per byte as the
+// one-cell kernels above (which remain the path for odd nx), and the restriction needs no shuffle: a thread owns a whole aggregate.
+template <typename T> struct Pair2;
+template <> struct Pair2<double> { typedef double2 type; };
+template <> struct Pair2<float> { typedef float2 type; };
+
+struct V3 { double e, fx, fy; };
+__device__ __forceinline__ V3 ld3(const double* __restrict__ r, long long N, long long id) { V3 v; v.e = r[id]; v.fx = r[N + id]; v.fy = r[2 * N + id]; return v; }
+__device__ __forceinline__ void ld3x2(const double* __restrict__ r, long long N, long long id, V3& a, V3& b)
+{
+    const double2 p0 = *reinterpret_cast<const double2*>(r + id), p1 = *reinterpret_cast<const double2*>(r + N + id),
+                  p2 = *reinterpret_cast<const double2*>(r + 2 * N + id);
+    a.e = p0.x; b.e = p0.y; a.fx = p1.x; b.fx = p1.y; a.fy = p2.x; b.fy = p2.y;
+}
+// acc += off_k(a) xa and off_k(b) xb for the cell pair at id (block k), one vector load per block entry
+template <typename TB>
+__device__ __forceinline__ void blk2_apply(const TB* __restrict__ off, long long N, long long id, int k, const V3& xa, const V3& xb,
+                                           double (&qa)[3], double (&qb)[3])
+{
+    typedef typename Pair2<TB>::type TB2;
+    const TB* base = off + (long long)(k * 9) * N + id;
+#pragma unroll
+    for (int row = 0; row < 3; ++row) {
+        const TB2 c0 = *reinterpret_cast<const TB2*>(base + (3 * row) * N), c1 = *reinterpret_cast<const TB2*>(base + (3 * row + 1) * N),
+                  c2 = *reinterpret_cast<const TB2*>(base + (3 * row + 2) * N);
+        qa[row] += (double)c0.x * xa.e + (double)c1.x * xa.fx + (double)c2.x * xa.fy;
+        qb[row] += (double)c0.y * xb.e + (double)c1.y * xb.fx + (double)c2.y * xb.fy;
+    }
+}
+// column and row neighbours of the pair (2I, 2I+1) in row j: indices on the level and aggregates on the next one
+struct PairNbr { long long w, e, s, n, aw, ae, as, an; };
+__device__ __forceinline__ PairNbr pair_nbr(const Grid& g, int I, int j, int cnx)
+{
+    PairNbr p;
+    int iw = 2 * I - 1, ie = 2 * I + 2, js = j - 1, jn = j + 1;
+    if (iw < 0) iw = (g.bc[XLO] == BC_PERIODIC) ? g.nx - 1 : 0;
+    if (ie >= g.nx) ie = (g.bc[XHI] == BC_PERIODIC) ? 0 : g.nx - 1;
+    if (js < 0) js = (g.bc[YLO] == BC_PERIODIC) ? g.ny - 1 : 0;
+    if (jn >= g.ny) jn = (g.bc[YHI] == BC_PERIODIC) ? 0 : g.ny - 1;
+    p.w = (long long)j * g.nx + iw; p.e = (long long)j * g.nx + ie;
+    p.s = (long long)js * g.nx + 2 * I; p.n = (long long)jn * g.nx + 2 * I;
+    p.aw = (long long)(j >> 1) * cnx + (iw >> 1); p.ae = (long long)(j >> 1) * cnx + (ie >> 1);
+    p.as = (long long)(js >> 1) * cnx + I; p.an = (long long)(jn >> 1) * cnx + I;
+    return p;
+}
+
+template <typename TB>
+__global__ void __launch_bounds__(128) mg_restrict2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+                                                           double omega, int cnx, double* __restrict__ rc,
+                                                           const int* __restrict__ skip_flag)
+{
+    if (skip_flag && *skip_flag) return;
+    const int I = blockIdx.x * blockDim.x + threadIdx.x;
+    const int J = blockIdx.y * blockDim.y + threadIdx.y;
+    const int cny = (g.ny + 1) / 2;
+    if (I >= cnx || J >= cny) return;
+    const long long N = (long long)g.nx * g.ny;
+    double s[3] = { 0.0, 0.0, 0.0 };
+#pragma unroll
+    for (int dj = 0; dj < 2; ++dj) {
+        const int j = 2 * J + dj;
+        if (j >= g.ny) continue;
+        const long long id = (long long)j * g.nx + 2 * I;
+        const PairNbr p = pair_nbr(g, I, j, cnx);
+        V3 ra, rb, sa, sb, na, nb;
+        ld3x2(r, N, id, ra, rb); ld3x2(r, N, p.s, sa, sb); ld3x2(r, N, p.n, na, nb);
+        const V3 rw = ld3(r, N, p.w), re = ld3(r, N, p.e);
+        double qa[3] = { 0.0, 0.0, 0.0 }, qb[3] = { 0.0, 0.0, 0.0 };
+        blk2_apply<TB>(off, N, id, 0, rw, ra, qa, qb);      // west: of a it is the outer column, of b it is a
+        blk2_apply<TB>(off, N, id, 1, rb, re, qa, qb);      // east: of a it is b, of b the outer column
+        blk2_apply<TB>(off, N, id, 2, sa, sb, qa, qb);
+        blk2_apply<TB>(off, N, id, 3, na, nb, qa, qb);
+        s[0] += (1.0 - omega) * (ra.e + rb.e) - omega * (qa[0] + qb[0]);
+        s[1] += (1.0 - omega) * (ra.fx + rb.fx) - omega * (qa[1] + qb[1]);
+        s[2] += (1.0 - omega) * (ra.fy + rb.fy) - omega * (qa[2] + qb[2]);
+    }
+    const long long Nc = (long long)cnx * cny, a = (long long)J * cnx + I;
+    rc[a] = s[0]; rc[Nc + a] = s[1]; rc[2 * Nc + a] = s[2];
+}
+
+template <typename TB>
+__global__ void __launch_bounds__(128) mg_prolong_smooth2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+                                                                 double omega, int cnx, const double* __restrict__ ec,
+                                                                 const double* __restrict__ Dinv, double* __restrict__ out,
+                                                                 const int* __restrict__ skip_flag)
+{
+    if (skip_flag && *skip_flag) return;
+    const int I = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (I >= cnx || j >= g.ny) return;
+    const long long N = (long long)g.nx * g.ny, id = (long long)j * g.nx + 2 * I;
+    const long long Nc = (long long)cnx * ((g.ny + 1) / 2), ag = (long long)(j >> 1) * cnx + I;
+    const PairNbr p = pair_nbr(g, I, j, cnx);
+    V3 ra, rb, sa, sb, na, nb;
+    ld3x2(r, N, id, ra, rb); ld3x2(r, N, p.s, sa, sb); ld3x2(r, N, p.n, na, nb);
+    V3 rw = ld3(r, N, p.w), re = ld3(r, N, p.e);
+    const V3 e0 = ld3(ec, Nc, ag), ew = ld3(ec, Nc, p.aw), ee = ld3(ec, Nc, p.ae), es = ld3(ec, Nc, p.as), en = ld3(ec, Nc, p.an);
+    // t = omega r + P0 e_c at the pair and its six neighbours
+#define ARK_T(v, c) do { (v).e = fma(omega, (v).e, (c).e); (v).fx = fma(omega, (v).fx, (c).fx); (v).fy = fma(omega, (v).fy, (c).fy); } while (0)
+    V3 ta = ra, tb = rb;
+    ARK_T(ta, e0); ARK_T(tb, e0); ARK_T(rw, ew); ARK_T(re, ee); ARK_T(sa, es); ARK_T(sb, es); ARK_T(na, en); ARK_T(nb, en);
+#undef ARK_T
+    double qa[3] = { ta.e, ta.fx, ta.fy }, qb[3] = { tb.e, tb.fx, tb.fy };
+    blk2_apply<TB>(off, N, id, 0, rw, ta, qa, qb);
+    blk2_apply<TB>(off, N, id, 1, tb, re, qa, qb);
+    blk2_apply<TB>(off, N, id, 2, sa, sb, qa, qb);
+    blk2_apply<TB>(off, N, id, 3, na, nb, qa, qb);
+    const double za0 = ta.e + omega * (ra.e - qa[0]), za1 = ta.fx + omega * (ra.fx - qa[1]), za2 = ta.fy + omega * (ra.fy - qa[2]);
+    const double zb0 = tb.e + omega * (rb.e - qb[0]), zb1 = tb.fx + omega * (rb.fx - qb[1]), zb2 = tb.fy + omega * (rb.fy - qb[2]);
+    double2 o0, o1, o2;
+    if (Dinv) {
+        double2 d[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) d[e] = *reinterpret_cast<const double2*>(Dinv + e * N + id);
+        o0 = make_double2(d[0].x * za0 + d[1].x * za1 + d[2].x * za2, d[0].y * zb0 + d[1].y * zb1 + d[2].y * zb2);
+        o1 = make_double2(d[3].x * za0 + d[4].x * za1 + d[5].x * za2, d[3].y * zb0 + d[4].y * zb1 + d[5].y * zb2);
+        o2 = make_double2(d[6].x * za0 + d[7].x * za1 + d[8].x * za2, d[6].y * zb0 + d[7].y * zb1 + d[8].y * zb2);
+    } else {
+        o0 = make_double2(za0, zb0); o1 = make_double2(za1, zb1); o2 = make_double2(za2, zb2);
+    }
+    *reinterpret_cast<double2*>(out + id) = o0; *reinterpret_cast<double2*>(out + N + id) = o1; *reinterpret_cast<double2*>(out + 2 * N + id) = o2;
 }
 
 // ---- coarsest level (a single cell): z^ = omega r, then sweeps-1 times z^ += omega (r - Ahat z^);  out = Dinv z^ ----------
@@ -196,8 +324,14 @@ static cudaError_t vcycle_t(const MgHier& H, const double* r_in, double* zhat_ou
     for (int l = 0; l + 1 < L; ++l) {                     // downward: restricted residuals
         const MgLevel& f = H.lev[l];
         const double* r = (l == 0) ? r_in : f.r;
-        dim3 blk(32, 4), grd((f.g.nx + 31) / 32, ((f.g.ny + 1) / 2 + 3) / 4);
-        mg_restrict_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].r, skip_flag);
+        if ((f.g.nx & 1) == 0) {          // pair kernel: one thread per aggregate
+            const int cnx = H.lev[l + 1].g.nx, cny = H.lev[l + 1].g.ny;
+            dim3 blk(32, 4), grd((cnx + 31) / 32, (cny + 3) / 4);
+            mg_restrict2_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, cnx, H.lev[l + 1].r, skip_flag);
+        } else {
+            dim3 blk(32, ARK_MG_BY), grd((f.g.nx + 31) / 32, ((f.g.ny + 1) / 2 + ARK_MG_BY - 1) / ARK_MG_BY);
+            mg_restrict_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].r, skip_flag);
+        }
         ++launches;
     }
     {
@@ -210,9 +344,16 @@ static cudaError_t vcycle_t(const MgHier& H, const double* r_in, double* zhat_ou
     for (int l = L - 2; l >= 0; --l) {                    // upward: interpolation + post-smoothing
         const MgLevel& f = H.lev[l];
         const double* r = (l == 0) ? r_in : f.r;
-        dim3 blk(32, 4), grd((f.g.nx + 31) / 32, (f.g.ny + 3) / 4);
-        mg_prolong_smooth_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].e,
-                                                          (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
+        if ((f.g.nx & 1) == 0) {
+            const int cnx = H.lev[l + 1].g.nx;
+            dim3 blk(32, 4), grd((cnx + 31) / 32, (f.g.ny + 3) / 4);
+            mg_prolong_smooth2_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, cnx, H.lev[l + 1].e,
+                                                               (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
+        } else {
+            dim3 blk(32, ARK_MG_BY), grd((f.g.nx + 31) / 32, (f.g.ny + ARK_MG_BY - 1) / ARK_MG_BY);
+            mg_prolong_smooth_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].e,
+                                                              (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
+        }
         ++launches;
     }
     if (nl) *nl = launches;
