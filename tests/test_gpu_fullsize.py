@@ -67,3 +67,32 @@ def test_vcycle_1024_matches_oracle():
     o, g = make_oracle(w, dict(preconditioner=1)), make_gpu(w, dict(preconditioner=1))
     R = np.random.default_rng(11).standard_normal((3, 1024, 1024))
     assert rel_l2(g.apply_preconditioner(dt, R), o.mg_apply(dt, R)) <= 1e-9
+
+
+def test_8192_grid_indices_beyond_32_bits():
+    # 67 M cells, 201 M unknowns: plane offsets (k N, k <= 36) exceed 2^31; explicit step against the oracle on every element,
+    # the implicit solution in the oracle's operator, multigrid and compressed-basis solves against it
+    n = 8192
+    w = wl.random_medium(n, seed=99)
+    dt = wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    o, g = make_oracle(w), make_gpu(w)
+    o.step_explicit(dt)
+    g.step_explicit(dt)
+    assert state_rel_l2(g.get_state(), o.get_state()) <= 1e-11
+    E0, F0 = g.get_state()
+    b = np.concatenate((E0[None], F0))
+    its, res = g.step_implicit(10.0 * dt, 1e-10, 30, 1000)
+    assert res <= 1e-10 and 0 < its < 200
+    E, F = g.get_state()
+    x = np.concatenate((E[None], F))
+    g.close()
+    Ax = o.apply_linear(10.0 * dt, x, mode=0)            # the oracle holds the same U^n (its own explicit step)
+    assert np.linalg.norm((b - Ax).ravel()) <= 2e-10 * np.linalg.norm(b.ravel())
+    del o, Ax
+    for opts in (dict(preconditioner=1, mg_precision=32, krylov=1), dict(basis_precision=32)):
+        g2 = make_gpu(dict(w, E=E0, F=F0), opts)
+        its2, res2 = g2.step_implicit(10.0 * dt, 1e-10, 30, 1000)
+        E2, F2 = g2.get_state()
+        g2.close()
+        assert res2 <= 1e-10
+        assert rel_l2(np.concatenate((E2[None], F2)), x) <= 1e-8
