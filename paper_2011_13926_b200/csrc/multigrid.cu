@@ -17,6 +17,9 @@
 
 namespace ark {
 
+#ifndef ARK_MG_MINB
+#define ARK_MG_MINB 3        // resident blocks per SM asked of the pair kernels: 168 registers let ptxas issue all block loads up front (measured best of 1, 3, 4, 8)
+#endif
 #ifndef ARK_MG_BY
 #define ARK_MG_BY 4          // rows of threads per block of the V-cycle kernels (32 x ARK_MG_BY threads)
 #endif
@@ -213,7 +216,7 @@ __device__ __forceinline__ PairNbr pair_nbr(const Grid& g, int I, int j, int cnx
 }
 
 template <typename TB>
-__global__ void __launch_bounds__(128) mg_restrict2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(128, ARK_MG_MINB) mg_restrict2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                            double omega, int cnx, double* __restrict__ rc,
                                                            const int* __restrict__ skip_flag)
 {
@@ -247,7 +250,7 @@ __global__ void __launch_bounds__(128) mg_restrict2_kernel(Grid g, const TB* __r
 }
 
 template <typename TB>
-__global__ void __launch_bounds__(128) mg_prolong_smooth2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(128, ARK_MG_MINB) mg_prolong_smooth2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                                  double omega, int cnx, const double* __restrict__ ec,
                                                                  const double* __restrict__ Dinv, double* __restrict__ out,
                                                                  const int* __restrict__ skip_flag)
