@@ -135,13 +135,29 @@ struct XPub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };   // what the we
 // What the march kernel keeps per cell: pressure, Eq. 14 eigenvalues for both face orientations, |f|.
 struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };   // Pxx.. hold c^2 P (what the flux needs)
 
+// max/min of two doubles as compare + select (2 fp64-pipe + 2 ALU issue slots).  fmax()/fmin() and the `x > K ? x : K` idiom
+// compile on sm_100a to DSETP.MAX + SEL + FSEL + a NaN-quieting LOP3 + register copies (~9 issue slots, one dependent chain);
+// the arguments here are never NaN.
+__device__ __forceinline__ double dmax_sel(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.gt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
+__device__ __forceinline__ double dmin_sel(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
+
 // Default-scheme closure with 2 reciprocals and 4 reciprocal square roots per cell:
 //   1/(cE);  rs = 1/sqrt(4 - 3 f^2) gives xi = s rs and 1/xi = rs;  one reciprocal of (2+xi)(5+2xi) gives both
 //   1/(5+2xi) (for chi) and 1/(2+xi) (for the anisotropic part and the eigenvalue prefactor);  |f| and the two
 //   eigenvalue roots as x rsqrt(x).
 __device__ __forceinline__ void closure_fast(double c, double E, double Fx, double Fy, CloF& q)
 {
-    const double Es = (E > ARK_E_FLOOR) ? E : ARK_E_FLOOR;
+    const double Es = dmax_sel(E, ARK_E_FLOOR);
     const double ice = rcp_fast(c * Es);
     double fx = Fx * ice, fy = Fy * ice;
     const double f2raw = fx * fx + fy * fy;
@@ -171,8 +187,11 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double crs = c * rs;                                // c/xi
     const double k = 0.81649658092772603273 * crs * i2;       // c sqrt(2/3)/(xi (xi+2))
     const double a2 = a + a;
-    const double rx = k * sqrt_fast(a * fma(3.0 * fy, fy, a2));
-    const double ry = k * sqrt_fast(a * fma(3.0 * fx, fx, a2));
+    // sqrt(x) = x' rsqrt(x') with x' = x + 1e-300 folded into the product's fma: branch-free, and x = 0 (f = 1) gives 1e-150
+    // instead of 0 (the oracle's eigenvalues are O(c); 1e-150 is below every rounding error of the path)
+    const double xr = fma(a, fma(3.0 * fy, fy, a2), 1e-300), yr = fma(a, fma(3.0 * fx, fx, a2), 1e-300);
+    const double rx = k * (xr * rsqrt_fast(xr));
+    const double ry = k * (yr * rsqrt_fast(yr));
     const double mx = fx * crs, my = fy * crs;
     q.lmaxx = mx + rx; q.lminx = mx - rx;
     q.lmaxy = my + ry; q.lminy = my - ry;
@@ -185,8 +204,8 @@ struct FaceF { double ap, Lam, alpha, sig; };
 __device__ __forceinline__ void face_fast(double k3, double lminL, double lmaxL, double fL, double stL,
                                           double lminR, double lmaxR, double fR, double stR, FaceF& fc)
 {
-    const double lp = fmax(0.0, fmax(lmaxL, lmaxR));
-    const double lm = fmin(0.0, fmin(lminL, lminR));
+    const double lp = dmax_sel(dmax_sel(lmaxL, lmaxR), 0.0);
+    const double lm = dmin_sel(dmin_sel(lminL, lminR), 0.0);
     const double dl = lp - lm;
     fc.sig = 0.5 * (stL + stR);
     const double ff = 0.5 * (fL + fR);

@@ -13,27 +13,58 @@
 
 namespace ark {
 
+// Block = ONE warp of 32 columns (30 updated + 1 halo lane each side), 16 blocks per SM (128 registers): measured fastest
+// (DESIGN.md section 6): no hardware barrier, no coupling between warps; 0.272 ms at 4096^2 against 0.284 (128 columns).
+#ifndef ARK_MARCH3_TX
+#define ARK_MARCH3_TX 32
+#endif
+#ifndef ARK_MARCH3_MINB
+#define ARK_MARCH3_MINB 16
+#endif
+#ifndef ARK_MARCH3_RY
+#define ARK_MARCH3_RY 33      // rows per block (cap; a multiple of 3)
+#endif
+static constexpr int TX3 = ARK_MARCH3_TX;
+
 struct Slot {
     Raw u;                      // raw state of the cell
     CloF q;                     // closure (c^2 P, eigenvalues, |f|)
     double H0, H1, H2, S;       // flux through the NORTH face of the cell (E, Fx, Fy rows) and sigma_n (Fy_j + Fy_j+1)
 };
 
+// a one-warp block needs no hardware barrier for the shared-memory exchange
+__device__ __forceinline__ void block_sync() { if (TX3 == 32) __syncwarp(); else __syncthreads(); }
+
 struct March3Ctx {
     double c, cdt, dt, rdx, rdy, k3x, k3y, qc;
     int xmode, ii, xside, t;
     bool upd, wb;
+    // branch-free loader of the hot loop: value of plane p in grid row j = bp[j * stride]
+    //   grid column: bp = plane + ii, stride = nx;  Dirichlet x-ghost: bp = ghost column, stride = 1;  inactive lane: cell 0, stride = 0
+    const double *bE, *bFx, *bFy, *bst, *bsa;
+    unsigned int stride;
 };
 
-template <bool SD>
+// The raw rows travel HBM -> shared memory with cp.async (LDGSTS), three rows ahead of their use, each thread into its own
+// slots of ring[row mod 3][field][thread]: the request holds no registers, so ptxas has no reason to sink it towards the
+// use (with plain loads it did, and the exposed latency cost more than the copies saved).
+// FAST: row j+3 is known to be a grid row (0 <= j+3 < ny): five unconditional copies from the thread's base pointers.
+template <bool SD, bool FAST>
 __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const Fields& f, const March3Ctx& k,
                                          Slot& C, Slot& N, Slot& P, int j, int j1, unsigned int row_off,
-                                         XPub* pub, double (*flx)[TX],
+                                         double (*ringN)[TX3], double (*ringC)[TX3],
+                                         XPub* pub, double (*flx)[TX3],
                                          double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
 {
-    // prefetch the raw state two rows ahead into the slot that was the centre one row ago (its flux P.H is still needed
-    // below as the south flux; only the raw fields are overwritten)
-    if (j + 1 < j1) P.u = load_row(f, g, k.xmode, k.ii, k.xside, j + 2);
+    // request row j+3 into the ring slot of row j (read one row ago), then take row j+1 (third youngest group) out of the ring
+    if (FAST) {
+        const unsigned int o = (unsigned int)(j + 3) * k.stride;
+        cp_async8(&ringC[0][k.t], k.bE + o); cp_async8(&ringC[1][k.t], k.bFx + o); cp_async8(&ringC[2][k.t], k.bFy + o);
+        cp_async8(&ringC[3][k.t], k.bst + o); cp_async8(&ringC[4][k.t], k.bsa + o);
+        cp_async_commit();
+    } else load_row_async<TX3>(ringC, k.t, f, g, k.xmode, k.ii, k.xside, j + 3, j + 2 < j1);
+    cp_async_wait<2>();
+    N.u.E = ringN[0][k.t]; N.u.Fx = ringN[1][k.t]; N.u.Fy = ringN[2][k.t]; N.u.st = ringN[3][k.t]; N.u.sa = ringN[4][k.t];
     // publish the x-face data of the centre cell
     XPub me; me.E = C.u.E; me.Fx = C.u.Fx; me.Fy = C.u.Fy; me.Pxx = C.q.Pxx; me.Pxy = C.q.Pxy;
     me.lmin = C.q.lminx; me.lmax = C.q.lmaxx; me.f = C.q.f; me.st = C.u.st;
@@ -43,7 +74,7 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
     FaceF fn;
     cell_face<SD>(s, k.c, g.dy, k.k3y, C.q.lminy, C.q.lmaxy, C.q.f, C.u.st, N.q.lminy, N.q.lmaxy, N.q.f, N.u.st, fn);
     ARK_FACE_FLUX(fn, C.u.E, N.u.E, C.u.Fy, N.u.Fy, C.u.Fx, N.u.Fx, C.q.Pyy, N.q.Pyy, C.q.Pxy, N.q.Pxy, C.H0, C.H2, C.H1, C.S);
-    __syncthreads();
+    block_sync();
     double Ge0, Ge1, Ge2, Se;
     {
         const XPub R = pub[k.t + 1];
@@ -52,7 +83,7 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
         ARK_FACE_FLUX(fe, me.E, R.E, me.Fx, R.Fx, me.Fy, R.Fy, me.Pxx, R.Pxx, me.Pxy, R.Pxy, Ge0, Ge1, Ge2, Se);
     }
     flx[0][k.t] = Ge0; flx[1][k.t] = Ge1; flx[2][k.t] = Ge2; flx[3][k.t] = Se;
-    __syncthreads();
+    block_sync();
     {
         const int tw = (k.t > 0) ? k.t - 1 : 0;
         const double Gw0 = flx[0][tw], Gw1 = flx[1][tw], Gw2 = flx[2][tw], Sw = flx[3][tw];
@@ -68,17 +99,18 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
 }
 
 template <bool SD>
-__global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march3_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
+__global__ void __launch_bounds__(TX3, ARK_MARCH3_MINB) explicit_march3_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
                                                             double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
 {
-    __shared__ XPub pub[TX + 1];
-    __shared__ double flx[4][TX];
+    __shared__ XPub pub[TX3 + 1];
+    __shared__ double flx[4][TX3];
+    __shared__ double ring[3][5][TX3];     // raw rows in flight: row r lives in ring[r mod 3]
     March3Ctx k;
     k.t = threadIdx.x;
-    const int i = blockIdx.x * (TX - 2) - 1 + k.t;
+    const int i = blockIdx.x * (TX3 - 2) - 1 + k.t;
     const int j0 = blockIdx.y * RY;
     const int j1 = min(j0 + RY, g.ny);
-    k.upd = (k.t >= 1 && k.t <= TX - 2 && i >= 0 && i < g.nx);
+    k.upd = (k.t >= 1 && k.t <= TX3 - 2 && i >= 0 && i < g.nx);
     k.c = g.c; k.dt = dt; k.cdt = g.c * dt;
     k.rdx = dt / g.dx; k.rdy = dt / g.dy;
     k.k3x = 3.0 * g.dx / g.c; k.k3y = 3.0 * g.dy / g.c;
@@ -94,11 +126,16 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march3_kernel(Gri
         else k.ii = (i < 0) ? 0 : g.nx - 1;
     }
 
+    if (k.xmode == 0) { k.bE = f.E + k.ii; k.bFx = f.Fx + k.ii; k.bFy = f.Fy + k.ii; k.bst = f.st + k.ii; k.bsa = f.sa + k.ii; k.stride = (unsigned int)g.nx; }
+    else if (k.xmode == 1) { k.bE = f.gh[k.xside][0]; k.bFx = f.gh[k.xside][1]; k.bFy = f.gh[k.xside][2]; k.bsa = f.gh[k.xside][3]; k.bst = f.gh[k.xside][4]; k.stride = 1u; }
+    else { k.bE = f.E; k.bFx = f.Fx; k.bFy = f.Fy; k.bst = f.st; k.bsa = f.sa; k.stride = 0u; }
+
     // prologue: Z = row j0-1 (its north flux = south flux of row j0), X = row j0, Y = raw of row j0+1
     Slot X, Y, Z;
     Z.u = load_row(f, g, k.xmode, k.ii, k.xside, j0 - 1);
     X.u = load_row(f, g, k.xmode, k.ii, k.xside, j0);
-    Y.u = load_row(f, g, k.xmode, k.ii, k.xside, j0 + 1);
+    load_row_async<TX3>(ring[(j0 + 1) % 3], k.t, f, g, k.xmode, k.ii, k.xside, j0 + 1, true);
+    load_row_async<TX3>(ring[(j0 + 2) % 3], k.t, f, g, k.xmode, k.ii, k.xside, j0 + 2, j0 + 1 < j1);
     cell_closure<SD>(s, k.c, Z.u, Z.q);
     cell_closure<SD>(s, k.c, X.u, X.q);
     {
@@ -110,29 +147,36 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march3_kernel(Gri
     const unsigned int nxu = (unsigned int)g.nx;
 
     int j = j0;
-    for (; j + 2 < j1; j += 3) {
-        row_step<SD>(g, s, f, k, X, Y, Z, j, j1, row_off, pub, flx, oE, oFx, oFy);
-        row_step<SD>(g, s, f, k, Y, Z, X, j + 1, j1, row_off + nxu, pub, flx, oE, oFx, oFy);
-        row_step<SD>(g, s, f, k, Z, X, Y, j + 2, j1, row_off + 2 * nxu, pub, flx, oE, oFx, oFy);
-        row_off += 3 * nxu;
+    // hot loop: three rows per trip, every requested row (j+3 .. j+5) inside the grid.  RY is a multiple of 3 (launcher), so
+    // j mod 3 == 0 at every trip and the ring slots are compile-time constants.
+    const int jfast = min(j1, g.ny - 3);
+    if (j0 % 3 == 0) {
+        for (; j + 2 < jfast; j += 3) {
+            row_step<SD, true>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[1], ring[0], pub, flx, oE, oFx, oFy);
+            row_step<SD, true>(g, s, f, k, Y, Z, X, j + 1, j1, row_off + nxu, ring[2], ring[1], pub, flx, oE, oFx, oFy);
+            row_step<SD, true>(g, s, f, k, Z, X, Y, j + 2, j1, row_off + 2 * nxu, ring[0], ring[2], pub, flx, oE, oFx, oFy);
+            row_off += 3 * nxu;
+        }
     }
-    if (j < j1) {       // one or two rows left (block-uniform)
-        row_step<SD>(g, s, f, k, X, Y, Z, j, j1, row_off, pub, flx, oE, oFx, oFy);
-        if (j + 1 < j1) row_step<SD>(g, s, f, k, Y, Z, X, j + 1, j1, row_off + nxu, pub, flx, oE, oFx, oFy);
+    // remaining rows (block-uniform trip count): general loader, the window is shifted by copies
+    for (; j < j1; ++j) {
+        row_step<SD, false>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[(j + 1) % 3], ring[j % 3], pub, flx, oE, oFx, oFy);
+        const Slot T = X; X = Y; Y = Z; Z = T;
+        row_off += nxu;
     }
 }
 
 cudaError_t launch_explicit_march3(const Grid& g, const Scheme& s, const Fields& f, double dt,
                                    double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st)
 {
-    const int strips = (g.nx + (TX - 2) - 1) / (TX - 2);
+    const int strips = (g.nx + (TX3 - 2) - 1) / (TX3 - 2);
     long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
-    int RY = (int)(want < 3 ? 3 : (want > 33 ? 33 : want));   // multiples of three rows avoid the remainder path
+    int RY = (int)(want < 3 ? 3 : (want > ARK_MARCH3_RY ? ARK_MARCH3_RY : want));   // multiples of three rows avoid the remainder path
     RY = (RY + 2) / 3 * 3;
     if (RY > g.ny) RY = g.ny;
     dim3 grd(strips, (g.ny + RY - 1) / RY);
-    if (s.is_default()) explicit_march3_kernel<true><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
-    else explicit_march3_kernel<false><<<grd, TX, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
+    if (s.is_default()) explicit_march3_kernel<true><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
+    else explicit_march3_kernel<false><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
     return cudaGetLastError();
 }
 
