@@ -160,16 +160,16 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double Es = dmax_sel(E, ARK_E_FLOOR);
     const double ice = rcp_fast(c * Es);
     double fx = Fx * ice, fy = Fy * ice;
-    const double f2raw = fx * fx + fy * fy;
+    // f^2 + 1e-300 (folded into the fma): the reciprocal square root below needs no guard for F = 0
+    const double f2raw = fma(fx, fx, fma(fy, fy, 1e-300));
     // |f| and the clamp of PAPER.md:513, branch-free: one rsqrt serves both (f = f2 rsqrt(f2); rescale by rsqrt(f2) if f2 > 1)
-    const bool tiny = !(f2raw > 1e-290);
     const bool huge = !(f2raw <= 1e300);          // E <= 0 (floored): F/(cE) overflows; 1/sqrt(inf) = 0 like IEEE
-    const double rf = rsqrt_fast((tiny || huge) ? 1.0 : f2raw);
+    const double rf = rsqrt_fast(huge ? 1.0 : f2raw);
     const bool clamp = f2raw > 1.0;
     const double sc = clamp ? (huge ? 0.0 : rf) : 1.0;
     fx *= sc; fy *= sc;
     const double f2 = clamp ? 1.0 : f2raw;
-    q.f = clamp ? 1.0 : (tiny ? 0.0 : f2raw * rf);
+    q.f = clamp ? 1.0 : f2raw * rf;
     const double s = 4.0 - 3.0 * f2;       // >= 1
     const double rs = rsqrt_fast(s);
     const double xi = s * rs;
@@ -187,9 +187,10 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double crs = c * rs;                                // c/xi
     const double k = 0.81649658092772603273 * crs * i2;       // c sqrt(2/3)/(xi (xi+2))
     const double a2 = a + a;
-    // sqrt(x) = x' rsqrt(x') with x' = x + 1e-300 folded into the product's fma: branch-free, and x = 0 (f = 1) gives 1e-150
-    // instead of 0 (the oracle's eigenvalues are O(c); 1e-150 is below every rounding error of the path)
-    const double xr = fma(a, fma(3.0 * fy, fy, a2), 1e-300), yr = fma(a, fma(3.0 * fx, fx, a2), 1e-300);
+    // sqrt(x) = x' rsqrt(x') with x' = x + 1e-300 folded into the product's fma: branch-free, and x = 0 (f = 1) gives 1e-100
+    // instead of 0 (the oracle's eigenvalues are O(c); 1e-100 is below every rounding error of the path).
+    // It also makes l+ - l- > 0 on every face (face_fast needs no zero-width guard).
+    const double xr = fma(a, fma(3.0 * fy, fy, a2), 1e-200), yr = fma(a, fma(3.0 * fx, fx, a2), 1e-200);
     const double rx = k * (xr * rsqrt_fast(xr));
     const double ry = k * (yr * rsqrt_fast(yr));
     const double mx = fx * crs, my = fy * crs;
@@ -210,14 +211,14 @@ __device__ __forceinline__ void face_fast(double k3, double lminL, double lmaxL,
     fc.sig = 0.5 * (stL + stR);
     const double ff = 0.5 * (fL + fR);
     const double kk = k3 * fc.sig * fma(-ff, ff, 1.0);
-    const bool ok = dl > 0.0;
-    const double dls = ok ? dl : 1.0;
-    const double D = fma(-kk * lp, lm, dls);
-    const double qq = rcp_fast(dls * D);
-    const double apv = lp * (qq * D);
-    fc.ap = ok ? apv : 0.5;
-    fc.Lam = lm * apv;                     // l+ l-/dl; 0 when dl == 0 (then l+ = l- = 0)
-    fc.alpha = dls * (dls * qq);           // 1 when dl == 0
+    // dl > 0 always: closure_fast's eigenvalue roots are >= ~1e-101 c, so (l+, l-) = (0, 0) cannot occur; on a face between
+    // cells with f = 1 exactly along the face, dl ~ 1e-100 c gives a+ = 1/2, Lambda ~ -1e-101 c, alpha = 1 (the oracle's guard
+    // values 1/2, 0, 1)
+    const double D = fma(-kk * lp, lm, dl);
+    const double qq = rcp_fast(dl * D);
+    fc.ap = lp * (qq * D);
+    fc.Lam = lm * fc.ap;                   // l+ l-/dl
+    fc.alpha = dl * (dl * qq);
 }
 
 // Scheme dispatch: the default scheme uses the fast forms above, every other switch combination the generic ones.
