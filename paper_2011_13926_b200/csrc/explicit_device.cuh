@@ -185,14 +185,13 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     // Eq. 14
     const double a = (xi - 1.0) * t2;
     const double crs = c * rs;                                // c/xi
-    const double k = 0.81649658092772603273 * crs * i2;       // c sqrt(2/3)/(xi (xi+2))
-    const double a2 = a + a;
-    // sqrt(x) = x' rsqrt(x') with x' = x + 1e-300 folded into the product's fma: branch-free, and x = 0 (f = 1) gives 1e-100
-    // instead of 0 (the oracle's eigenvalues are O(c); 1e-100 is below every rounding error of the path).
-    // It also makes l+ - l- > 0 on every face (face_fast needs no zero-width guard).
-    const double xr = fma(a, fma(3.0 * fy, fy, a2), 1e-200), yr = fma(a, fma(3.0 * fx, fx, a2), 1e-200);
-    const double rx = k * (xr * rsqrt_fast(xr));
-    const double ry = k * (yr * rsqrt_fast(yr));
+    const double k = 1.41421356237309504880 * crs * i2;       // c sqrt(2/3)/(xi (xi+2)) times the sqrt(3) taken out of the roots
+    const double a23 = 0.66666666666666666667 * a;
+    // roots of Eq. 14: sqrt(a (3 f_t^2 + 2a)) = sqrt(3) sqrt(a (f_t^2 + 2a/3)).  x' = x + 1e-200 folded into the product's fma:
+    // branch-free, and x = 0 (f = 1) gives ~1e-100 instead of 0 (the eigenvalues are O(c); 1e-100 is below every rounding
+    // error of the path).  It also makes l+ - l- > 0 on every face (face_fast needs no zero-width guard).
+    const double rx = k * sqrt_core(fma(a, fma(fy, fy, a23), 1e-200));
+    const double ry = k * sqrt_core(fma(a, fma(fx, fx, a23), 1e-200));
     const double mx = fx * crs, my = fy * crs;
     q.lmaxx = mx + rx; q.lminx = mx - rx;
     q.lmaxy = my + ry; q.lminy = my - ry;
@@ -201,16 +200,16 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
 // Face coefficients with ONE reciprocal.  With D = dl - kk l+ l- (kk = 3 sigma_f delta (1 - f_f^2)/c >= 0, l+ l- <= 0):
 //   1/dl = D/(dl D),  alpha = 1/(1 - kk Lambda) = dl/D = dl^2/(dl D).   a- = 1 - a+ is never formed: the fluxes use
 //   a+ x_L + a- x_R = x_R + a+ (x_L - x_R).
-struct FaceF { double ap, Lam, alpha, sig; };
-__device__ __forceinline__ void face_fast(double k3, double lminL, double lmaxL, double fL, double stL,
+struct FaceF { double ap, Lam, alpha, sig; };     // sig = sigma_L + sigma_R = TWICE the face opacity of Eq. 18 (the 1/2 sits in k3h and qc)
+__device__ __forceinline__ void face_fast(double k3h, double lminL, double lmaxL, double fL, double stL,
                                           double lminR, double lmaxR, double fR, double stR, FaceF& fc)
 {
     const double lp = dmax_sel(dmax_sel(lmaxL, lmaxR), 0.0);
     const double lm = dmin_sel(dmin_sel(lminL, lminR), 0.0);
     const double dl = lp - lm;
-    fc.sig = 0.5 * (stL + stR);
+    fc.sig = stL + stR;
     const double ff = 0.5 * (fL + fR);
-    const double kk = k3 * fc.sig * fma(-ff, ff, 1.0);
+    const double kk = k3h * fc.sig * fma(-ff, ff, 1.0);
     // dl > 0 always: closure_fast's eigenvalue roots are >= ~1e-101 c, so (l+, l-) = (0, 0) cannot occur; on a face between
     // cells with f = 1 exactly along the face, dl ~ 1e-100 c gives a+ = 1/2, Lambda ~ -1e-101 c, alpha = 1 (the oracle's guard
     // values 1/2, 0, 1)
@@ -233,20 +232,21 @@ __device__ __forceinline__ void cell_closure(const Scheme& s, double c, const Ra
         q.lminx = t.lmin[0]; q.lmaxx = t.lmax[0]; q.lminy = t.lmin[1]; q.lmaxy = t.lmax[1];
     }
 }
+// k3h = 3 delta/(2c): Eq. 25's 3 sigma_f delta (1 - f_f^2)/c = k3h (sigma_L + sigma_R)(1 - f_f^2)
 template <bool SD>
-__device__ __forceinline__ void cell_face(const Scheme& s, double c, double delta, double k3,
+__device__ __forceinline__ void cell_face(const Scheme& s, double c, double delta, double k3h,
                                           double lminL, double lmaxL, double fL, double stL,
                                           double lminR, double lmaxR, double fR, double stR, FaceF& fc)
 {
-    if (SD) face_fast(k3, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, fc);
+    if (SD) face_fast(k3h, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, fc);
     else {
         Face t; face_eval<false>(s, c, delta, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, t);
-        fc.ap = t.ap; fc.Lam = t.Lam; fc.alpha = t.alpha; fc.sig = t.sig;     // a+ + a- = 1 in every scheme variant
+        fc.ap = t.ap; fc.Lam = t.Lam; fc.alpha = t.alpha; fc.sig = 2.0 * t.sig;     // a+ + a- = 1 in every scheme variant
     }
 }
 
 // Flux of Eq. 13 through one face (normal component Fn, pressures already times c^2):
-//   G0 = alpha (a+ Fn_L + a- Fn_R + Lam (E_R - E_L)),  G1/G2 = a+ P_L + a- P_R + Lam (F_R - F_L),  S = sigma_f (Fn_L + Fn_R)
+//   G0 = alpha (a+ Fn_L + a- Fn_R + Lam (E_R - E_L)),  G1/G2 = a+ P_L + a- P_R + Lam (F_R - F_L),  S = (sigma_L + sigma_R)(Fn_L + Fn_R) = 2 sigma_f (Fn_L + Fn_R)
 #define ARK_FACE_FLUX(fc, EL, ER, FnL, FnR, FtL, FtR, PnL, PnR, PtL, PtR, G0, Gn, Gt, S)              \
     do {                                                                                             \
         const double dFn_ = (FnR) - (FnL);                                                           \

@@ -30,8 +30,8 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
     const bool upd = (t >= 1 && t <= TX - 2 && i >= 0 && i < g.nx);
     const double c = g.c, cdt = c * dt;
     const double rdx = dt / g.dx, rdy = dt / g.dy;
-    const double k3x = 3.0 * g.dx / c, k3y = 3.0 * g.dy / c;   // Eq. 25: 3 sigma dx (1-f^2)/c = k3 sigma (1-f^2)
-    const double qc = 0.25 * c * dt;                            // WB source weight (Eqs. 18-19) times dt
+    const double k3x = 1.5 * g.dx / c, k3y = 1.5 * g.dy / c;   // Eq. 25: 3 sigma_f dx (1-f^2)/c = k3 (sigma_L + sigma_R)(1-f^2)
+    const double qc = 0.125 * c * dt;                            // WB source weight 1/4 (Eqs. 18-19) times dt, times the 1/2 of sigma_f
     const bool wb = SD ? true : (s.wb != 0);
 
     // resolve the column once
@@ -167,8 +167,8 @@ __global__ void __launch_bounds__(32 * WPB, ARK_WARP_MINB) explicit_warp_kernel(
     const bool upd = (lane >= 1 && lane <= WCOLS && i >= 0 && i < g.nx);
     const double c = g.c, cdt = c * dt;
     const double rdx = dt / g.dx, rdy = dt / g.dy;
-    const double k3x = 3.0 * g.dx / c, k3y = 3.0 * g.dy / c;
-    const double qc = 0.25 * c * dt;
+    const double k3x = 1.5 * g.dx / c, k3y = 1.5 * g.dy / c;
+    const double qc = 0.125 * c * dt;
     const bool wb = SD ? true : (s.wb != 0);
 
     int xmode = 0, ii = i, xside = 0;

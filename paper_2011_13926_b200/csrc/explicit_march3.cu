@@ -113,8 +113,8 @@ __global__ void __launch_bounds__(TX3, ARK_MARCH3_MINB) explicit_march3_kernel(G
     k.upd = (k.t >= 1 && k.t <= TX3 - 2 && i >= 0 && i < g.nx);
     k.c = g.c; k.dt = dt; k.cdt = g.c * dt;
     k.rdx = dt / g.dx; k.rdy = dt / g.dy;
-    k.k3x = 3.0 * g.dx / g.c; k.k3y = 3.0 * g.dy / g.c;
-    k.qc = 0.25 * g.c * dt;
+    k.k3x = 1.5 * g.dx / g.c; k.k3y = 1.5 * g.dy / g.c;     // 3 delta/(2c): FaceF.sig is sigma_L + sigma_R
+    k.qc = 0.125 * g.c * dt;                                   // Eqs. 18-19: 1/4, times the 1/2 of sigma_f
     k.wb = SD ? true : (s.wb != 0);
     k.xmode = 0; k.ii = i; k.xside = 0;
     if (i > g.nx) k.xmode = 2;

@@ -98,8 +98,18 @@ __device__ __forceinline__ double rsqrt_fast(double x)
     const double p = fma(0.375, e, 0.5);              // y (1 + e/2 + 3 e^2/8): third order, 2^-60
     return fma(y * e, p, y);
 }
+// sqrt(x) for normal x > 0, the same third-order correction applied to t = x y ~ sqrt(x): one multiply less than x * rsqrt_fast(x)
+__device__ __forceinline__ double sqrt_core(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(t * e, p, t);
+}
 // sqrt(x) for x >= 0; exactly 0 for x below 1e-290 (the seed flushes subnormals)
-__device__ __forceinline__ double sqrt_fast(double x) { return (x > 1e-290) ? x * rsqrt_fast(x) : 0.0; }
+__device__ __forceinline__ double sqrt_fast(double x) { return (x > 1e-290) ? sqrt_core(x) : 0.0; }
 
 // IEEE or fast (<= 1 ulp) reciprocal / square root, selected at compile time (FAST is used by the assembly kernel).
 template <bool FAST> __device__ __forceinline__ double rcp_sel(double x) { return FAST ? rcp_fast(x) : 1.0 / x; }
