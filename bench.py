@@ -285,7 +285,7 @@ def run_ours(args):
     exp_gbs = 64.0 * N / (best * 1e-3) / 1e9
     explicit_info = {"cell_updates_per_s": N / (best * 1e-3), "ms_per_step": best, "steps_timed": n_exp, "repeats": 5, "bytes_per_cell": 64,
                      "achieved_gbs": exp_gbs, "hbm_frac": exp_gbs / peak_gbs, "clocks": exp_clocks,
-                     "bound": "fp64 issue (DESIGN.md section 6): the kernel needs ~190 fp64 + ~265 other instructions per cell"}
+                     "bound": "fp64 issue (DESIGN.md section 6): the kernel needs ~170 fp64 + ~110 other instructions per cell"}
 
     # ---- main timed region: W warm-up + exactly K steps, inputs resident in HBM ----------------------------------
     for _ in range(args.warmup):

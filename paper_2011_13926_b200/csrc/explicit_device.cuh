@@ -135,22 +135,6 @@ struct XPub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };   // what the we
 // What the march kernel keeps per cell: pressure, Eq. 14 eigenvalues for both face orientations, |f|.
 struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };   // Pxx.. hold c^2 P (what the flux needs)
 
-// max/min of two doubles as compare + select (2 fp64-pipe + 2 ALU issue slots).  fmax()/fmin() and the `x > K ? x : K` idiom
-// compile on sm_100a to DSETP.MAX + SEL + FSEL + a NaN-quieting LOP3 + register copies (~9 issue slots, one dependent chain);
-// the arguments here are never NaN.
-__device__ __forceinline__ double dmax_sel(double a, double b)
-{
-    double r;
-    asm("{\n\t.reg .pred p;\n\tsetp.gt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
-    return r;
-}
-__device__ __forceinline__ double dmin_sel(double a, double b)
-{
-    double r;
-    asm("{\n\t.reg .pred p;\n\tsetp.lt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
-    return r;
-}
-
 // Default-scheme closure with 2 reciprocals and 4 reciprocal square roots per cell:
 //   1/(cE);  rs = 1/sqrt(4 - 3 f^2) gives xi = s rs and 1/xi = rs;  one reciprocal of (2+xi)(5+2xi) gives both
 //   1/(5+2xi) (for chi) and 1/(2+xi) (for the anisotropic part and the eigenvalue prefactor);  |f| and the two

@@ -69,15 +69,16 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
     XPub me; me.E = C.u.E; me.Fx = C.u.Fx; me.Fy = C.u.Fy; me.Pxx = C.q.Pxx; me.Pxy = C.q.Pxy;
     me.lmin = C.q.lminx; me.lmax = C.q.lmaxx; me.f = C.q.f; me.st = C.u.st;
     pub[k.t] = me;
-    // closure of the north cell, north face
+    block_sync();
+    const XPub R = pub[k.t + 1];
+    // closure of the north cell, north face, east face: one basic block, so that the scheduler can overlap the east-face chain
+    // (which depends only on data of row j) with the closure chain of row j+1 (0.2605 -> 0.2576 ms at 4096^2)
     cell_closure<SD>(s, k.c, N.u, N.q);
     FaceF fn;
     cell_face<SD>(s, k.c, g.dy, k.k3y, C.q.lminy, C.q.lmaxy, C.q.f, C.u.st, N.q.lminy, N.q.lmaxy, N.q.f, N.u.st, fn);
     ARK_FACE_FLUX(fn, C.u.E, N.u.E, C.u.Fy, N.u.Fy, C.u.Fx, N.u.Fx, C.q.Pyy, N.q.Pyy, C.q.Pxy, N.q.Pxy, C.H0, C.H2, C.H1, C.S);
-    block_sync();
     double Ge0, Ge1, Ge2, Se;
     {
-        const XPub R = pub[k.t + 1];
         FaceF fe;
         cell_face<SD>(s, k.c, g.dx, k.k3x, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
         ARK_FACE_FLUX(fe, me.E, R.E, me.Fx, R.Fx, me.Fy, R.Fy, me.Pxx, R.Pxx, me.Pxy, R.Pxy, Ge0, Ge1, Ge2, Se);

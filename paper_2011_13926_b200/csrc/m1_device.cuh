@@ -98,6 +98,22 @@ __device__ __forceinline__ double rsqrt_fast(double x)
     const double p = fma(0.375, e, 0.5);              // y (1 + e/2 + 3 e^2/8): third order, 2^-60
     return fma(y * e, p, y);
 }
+// max/min of two doubles as compare + select (2 fp64-pipe + 2 ALU issue slots).  fmax()/fmin() and the `x > K ? x : K` idiom
+// compile on sm_100a to DSETP.MAX + SEL + FSEL + a NaN-quieting LOP3 + register copies (~9 issue slots, one dependent chain);
+// the arguments here are never NaN.
+__device__ __forceinline__ double dmax_sel(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.gt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
+__device__ __forceinline__ double dmin_sel(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
+
 // sqrt(x) for normal x > 0, the same third-order correction applied to t = x y ~ sqrt(x): one multiply less than x * rsqrt_fast(x)
 __device__ __forceinline__ double sqrt_core(double x)
 {
@@ -200,8 +216,8 @@ __device__ __forceinline__ void face_eval(const Scheme& s, double c, double delt
                                           double lminR, double lmaxR, double fR, double stR, Face& fc)
 {
     const double fl = SCHEME_DEFAULT ? 0.0 : s.eig_floor * c;
-    const double lp = fmax(fl, fmax(lmaxL, lmaxR));
-    const double lm = fmin(-fl, fmin(lminL, lminR));
+    const double lp = dmax_sel(dmax_sel(lmaxL, lmaxR), fl);
+    const double lm = dmin_sel(dmin_sel(lminL, lminR), -fl);
     const double dl = lp - lm;
     if (dl > 0.0) {
         const double idl = rcp_sel<FAST>(dl);
