@@ -92,10 +92,10 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *   "vectors_per_pass"  basis vectors handled per pass of the multi-dot / multi-axpy kernels, 1..32 (default 16, by measurement)
  *   "basis_pad"         extra doubles (multiple of 32) between consecutive Krylov basis vectors (default 0; measured: no effect)
  *   "kernel_timing"     1: time every kernel launch with CUDA events (see ark_m1_get_kernel_stats); default 0
- *   "explicit_kernel"   0: one-thread-per-cell kernel   1: row-marching kernel, 128-column blocks (used for the matter-coupled step)
- *                       2: barrier-free warp-shuffle kernel
+ *   "explicit_kernel"   0: one-thread-per-cell kernel   1: row-marching kernel, 128-column blocks
+ *                       2: barrier-free warp-shuffle kernel (pure radiation only; falls back to 1 when T or source_E is set)
  *                       3: row-marching kernel, one warp per block, three-slot register rotation (no window copies) and
- *                          cp.async row prefetch (default; falls back to 1 when T or source_E is set)
+ *                          cp.async row prefetch (default)
  *   "operator"          1: matrix-free coefficient planes, flux form (default: 5% faster per solve at 4096^2)
  *                       0: block stencil (BSR 3x3 on the 5-point graph, pre-multiplied by M^-1)
  *   "basis_precision"   64 (default) or 32: storage precision of the GMRES Arnoldi basis.  32 = compressed-basis GMRES: the basis

@@ -316,8 +316,9 @@ static int explicit_once(ark_m1* h, double dt)
     const Fields f = fields_of(h);
     double* O = h->U[h->cur ^ 1];
     const bool plain = !h->have_T && !h->source_E;
-    if (h->explicit_kernel == 3 && plain && h->N < (1LL << 31)) {
-        KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
+    if (h->explicit_kernel == 3 && h->N < (1LL << 31)) {
+        KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N,
+                                                                                   h->have_T ? h->T[h->cur ^ 1] : nullptr, h->sm_count, h->st));
     } else if (h->explicit_kernel == 2 && plain && h->N < (1LL << 31)) {
         KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_warp(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
     } else if (h->explicit_kernel >= 1 && h->N < (1LL << 31)) {   // the march kernels use 32-bit in-plane offsets
@@ -811,7 +812,9 @@ extern "C" int ark_m1_step_semi_implicit(ark_m1* h, double dt, double tol, int r
         const Fields f = fields_of(h);
         double* O = h->U[h->cur ^ 1];
         kmark(h, KC_EXPLICIT, 64.0 * h->N);
-        cudaError_t e = launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, nullptr, h->sm_count, h->st);
+        cudaError_t e = (h->explicit_kernel == 3)
+            ? launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, nullptr, h->sm_count, h->st)
+            : launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, nullptr, h->sm_count, h->st);
         h->s.src_off = 0;
         if (e != cudaSuccess) return fail(h, ARK_M1_E_CUDA, "launch_explicit_march: %s", cudaGetErrorString(e));
         if (h->have_T) CU(cudaMemcpyAsync(h->T[h->cur ^ 1], h->T[h->cur], (size_t)h->N * sizeof(double), cudaMemcpyDeviceToDevice, h->st));

@@ -56,7 +56,7 @@ cudaError_t launch_explicit_cell(const Grid& g, const Scheme& s, const Fields& f
 cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& f, double dt,
                                   double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st);
 cudaError_t launch_explicit_march3(const Grid& g, const Scheme& s, const Fields& f, double dt,
-                                   double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st);
+                                   double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st);
 cudaError_t launch_explicit_warp(const Grid& g, const Scheme& s, const Fields& f, double dt,
                                  double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st);
 cudaError_t launch_velocity_sources(const Grid& g, const Scheme& s, const Fields& f, const double* ux, const double* uy,

@@ -49,13 +49,22 @@ struct March3Ctx {
 // slots of ring[row mod 3][field][thread]: the request holds no registers, so ptxas has no reason to sink it towards the
 // use (with plain loads it did, and the exposed latency cost more than the copies saved).
 // FAST: row j+3 is known to be a grid row (0 <= j+3 < ny): five unconditional copies from the thread's base pointers.
-template <bool SD, bool FAST>
+template <bool SD, bool FAST, bool COUPLED>
 __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const Fields& f, const March3Ctx& k,
                                          Slot& C, Slot& N, Slot& P, int j, int j1, unsigned int row_off,
                                          double (*ringN)[TX3], double (*ringC)[TX3],
                                          XPub* pub, double (*flx)[TX3],
-                                         double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
+                                         double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy,
+                                         double* __restrict__ oT)
 {
+    // COUPLED (stage 2, Eq. 4): the matter planes of the centre row are only needed by the update at the end of the row step;
+    // their loads are issued here so that the closure work hides the latency
+    double Tm = 0.0, rcv = 1.0, srcE = 0.0;
+    const bool coupled_on = COUPLED && k.upd && !(!SD && s.src_off);
+    if (coupled_on) {
+        if (f.T) { Tm = f.T[row_off]; if (f.rho_cv) rcv = f.rho_cv[row_off]; }
+        if (f.source_E) srcE = f.source_E[row_off];
+    }
     // request row j+3 into the ring slot of row j (read one row ago), then take row j+1 (third youngest group) out of the ring
     if (FAST) {
         const unsigned int o = (unsigned int)(j + 3) * k.stride;
@@ -91,7 +100,16 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
         double dSFx, dSFy;   // -dt * S^F
         if (k.wb) { dSFx = k.qc * (Se + Sw); dSFy = k.qc * (C.S + P.S); }
         else { dSFx = k.dt * k.c * C.u.st * C.u.Fx; dSFy = k.dt * k.c * C.u.st * C.u.Fy; }
-        const double dSE = k.cdt * C.u.sa * C.u.E;
+        double dSE = k.cdt * C.u.sa * C.u.E;
+        if (coupled_on) {       // emission c sigma_a a_r T^4, source_E, explicit matter-energy update of Eq. 4
+            if (f.T) {
+                const double Theta = s.a_r * (Tm * Tm) * (Tm * Tm);
+                dSE -= k.cdt * C.u.sa * Theta;
+                if (oT) oT[row_off] = Tm - k.cdt * C.u.sa * (Theta - C.u.E) / rcv;
+            }
+            dSE -= k.dt * srcE;
+        }
+        if (!SD && s.src_off) { dSE = 0.0; dSFx = 0.0; dSFy = 0.0; }     // semi-implicit step: hyperbolic part only
         const double nE  = C.u.E  - fma(k.rdx, Ge0 - Gw0, fma(k.rdy, C.H0 - P.H0, dSE));
         const double nFx = C.u.Fx - fma(k.rdx, Ge1 - Gw1, fma(k.rdy, C.H1 - P.H1, dSFx));
         const double nFy = C.u.Fy - fma(k.rdx, Ge2 - Gw2, fma(k.rdy, C.H2 - P.H2, dSFy));
@@ -99,9 +117,10 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
     }
 }
 
-template <bool SD>
+template <bool SD, bool COUPLED>
 __global__ void __launch_bounds__(TX3, ARK_MARCH3_MINB) explicit_march3_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
-                                                            double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
+                                                            double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy,
+                                                            double* __restrict__ oT)
 {
     __shared__ XPub pub[TX3 + 1];
     __shared__ double flx[4][TX3];
@@ -153,22 +172,22 @@ __global__ void __launch_bounds__(TX3, ARK_MARCH3_MINB) explicit_march3_kernel(G
     const int jfast = min(j1, g.ny - 3);
     if (j0 % 3 == 0) {
         for (; j + 2 < jfast; j += 3) {
-            row_step<SD, true>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[1], ring[0], pub, flx, oE, oFx, oFy);
-            row_step<SD, true>(g, s, f, k, Y, Z, X, j + 1, j1, row_off + nxu, ring[2], ring[1], pub, flx, oE, oFx, oFy);
-            row_step<SD, true>(g, s, f, k, Z, X, Y, j + 2, j1, row_off + 2 * nxu, ring[0], ring[2], pub, flx, oE, oFx, oFy);
+            row_step<SD, true, COUPLED>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[1], ring[0], pub, flx, oE, oFx, oFy, oT);
+            row_step<SD, true, COUPLED>(g, s, f, k, Y, Z, X, j + 1, j1, row_off + nxu, ring[2], ring[1], pub, flx, oE, oFx, oFy, oT);
+            row_step<SD, true, COUPLED>(g, s, f, k, Z, X, Y, j + 2, j1, row_off + 2 * nxu, ring[0], ring[2], pub, flx, oE, oFx, oFy, oT);
             row_off += 3 * nxu;
         }
     }
     // remaining rows (block-uniform trip count): general loader, the window is shifted by copies
     for (; j < j1; ++j) {
-        row_step<SD, false>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[(j + 1) % 3], ring[j % 3], pub, flx, oE, oFx, oFy);
+        row_step<SD, false, COUPLED>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[(j + 1) % 3], ring[j % 3], pub, flx, oE, oFx, oFy, oT);
         const Slot T = X; X = Y; Y = Z; Z = T;
         row_off += nxu;
     }
 }
 
 cudaError_t launch_explicit_march3(const Grid& g, const Scheme& s, const Fields& f, double dt,
-                                   double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st)
+                                   double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st)
 {
     const int strips = (g.nx + (TX3 - 2) - 1) / (TX3 - 2);
     long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
@@ -176,8 +195,14 @@ cudaError_t launch_explicit_march3(const Grid& g, const Scheme& s, const Fields&
     RY = (RY + 2) / 3 * 3;
     if (RY > g.ny) RY = g.ny;
     dim3 grd(strips, (g.ny + RY - 1) / RY);
-    if (s.is_default()) explicit_march3_kernel<true><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
-    else explicit_march3_kernel<false><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
+    const bool coupled = (f.T != nullptr) || (f.source_E != nullptr);
+    if (coupled) {
+        if (s.is_default()) explicit_march3_kernel<true, true><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, outT);
+        else explicit_march3_kernel<false, true><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, outT);
+    } else {
+        if (s.is_default()) explicit_march3_kernel<true, false><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, nullptr);
+        else explicit_march3_kernel<false, false><<<grd, TX3, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy, nullptr);
+    }
     return cudaGetLastError();
 }
 

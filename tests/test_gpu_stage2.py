@@ -25,10 +25,10 @@ def _dt(w, k=1.0):
     return k * wl.explicit_dt(w["dx"], w["dy"], w["c"])
 
 
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [0, 1, 3])
 @pytest.mark.parametrize("bc", [(0, 0, 0, 0), (1, 2, 2, 1)])
 def test_explicit_step_with_temperature(bc, kernel):
-    # kernel 0: one thread per cell; kernel 1: the marching kernel with the stage-2 terms (emission, source_E, Eq. 4)
+    # kernel 0: one thread per cell; kernels 1 and 3 (default): the marching kernels with the stage-2 terms (emission, source_E, Eq. 4)
     w = _coupled_state(141, 37, seed=3, bc=bc)
     o, g = make_oracle(w, dict(a_r=0.7)), make_gpu(w, dict(a_r=0.7, explicit_kernel=kernel))
     dt = 0.2 * _dt(w)
