@@ -14,7 +14,11 @@
 
 namespace ark {
 
-static constexpr int TXA = 128;
+#ifndef ARK_ASM_TX
+#define ARK_ASM_TX 32      // one warp per block, like the explicit kernel: 1.104 -> 1.059 ms at 4096^2 (128 -> 64 -> 32 columns: 0.668 / 0.689 / 0.697 of HBM peak)
+#endif
+static constexpr int TXA = ARK_ASM_TX;
+__device__ __forceinline__ void asm_sync() { if (TXA == 32) __syncwarp(); else __syncthreads(); }
 
 struct ACell {                 // one cell: raw state, closure, Jacobian
     Raw u;
@@ -86,13 +90,13 @@ __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, F
         closure_eval<true, SD, true>(s, c, Nn.u.E, Nn.u.Fx, Nn.u.Fy, Nn.q, &Nn.J);
         Face fn;
         face_eval<SD, true>(s, c, g.dy, C.q.lmin[1], C.q.lmax[1], C.q.f, C.u.st, Nn.q.lmin[1], Nn.q.lmax[1], Nn.q.f, Nn.u.st, fn);
-        __syncthreads();
+        asm_sync();
         const APub R = pub[t + 1];
         const APub L = pub[t > 0 ? t - 1 : 0];
         Face fe;
         face_eval<SD, true>(s, c, g.dx, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
         fcs[0][t] = fe.ap; fcs[1][t] = fe.am; fcs[2][t] = fe.Lam; fcs[3][t] = fe.alpha; fcs[4][t] = fe.sig;
-        __syncthreads();
+        asm_sync();
         if (upd) {
             const int tw = t - 1;
             Face fw; fw.ap = fcs[0][tw]; fw.am = fcs[1][tw]; fw.Lam = fcs[2][tw]; fw.alpha = fcs[3][tw]; fw.sig = fcs[4][tw];
