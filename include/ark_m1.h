@@ -190,10 +190,11 @@ ARK_M1_API int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap);
 ARK_M1_API const char* ark_m1_kernel_class_name(int k);
 ARK_M1_API long long ark_m1_kernel_launches(const ark_m1* h);
 
-/* Self-test of the fast fp64 reciprocal / reciprocal square root of the hot kernels (MUFU seed + Newton steps): out3[0..2] =
- * max relative error of rcp_fast vs 1/x, rsqrt_fast vs 1/sqrt(x), x rsqrt_fast(x) vs sqrt(x) over n samples in 200 binades
- * (host pointer).  Expected: 0, <= 1 ulp, <= 1 ulp.  No handle needed. */
-ARK_M1_API int ark_m1_fastmath_errors(int n, double* out3);
+/* Self-test of the fast fp64 reciprocal / reciprocal square root of the hot kernels (MUFU seed + Newton steps): out4[0..3] =
+ * max relative error of rcp_fast vs 1/x, rsqrt_fast vs 1/sqrt(x), sqrt_fast vs sqrt(x) and rcp_fast3 (one third-order step,
+ * explicit kernel) vs 1/x over n samples in 200 binades (host pointer to 4 doubles).  Expected: 0, <= 1 ulp, <= 1 ulp, <= 1 ulp.
+ * No handle needed. */
+ARK_M1_API int ark_m1_fastmath_errors(int n, double* out4);
 
 /* Device bytes currently allocated by the handle. */
 ARK_M1_API long long ark_m1_device_bytes(const ark_m1* h);

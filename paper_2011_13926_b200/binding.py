@@ -250,8 +250,8 @@ class ArkM1:
 
 
 def fastmath_errors(n=1 << 20):
-    """Max relative errors (rcp_fast, rsqrt_fast, sqrt via rsqrt) of the kernels' fast fp64 forms against IEEE, measured on the GPU."""
-    buf = (C.c_double * 3)()
+    """Max relative errors (rcp_fast, rsqrt_fast, sqrt_fast, rcp_fast3) of the kernels' fast fp64 forms against IEEE, measured on the GPU."""
+    buf = (C.c_double * 4)()
     rc = load_library().ark_m1_fastmath_errors(int(n), buf)
     if rc < 0:
         raise RuntimeError(f"ark_m1_fastmath_errors failed ({rc})")

@@ -906,14 +906,14 @@ extern "C" long long ark_m1_kernel_launches(const ark_m1* h) { return h ? h->lau
 
 // Self-test of the fast reciprocal / reciprocal square root used by the hot kernels: max relative errors against the IEEE
 // sequences over n samples in 200 binades.  No handle needed.  Returns 0 or ARK_M1_E_CUDA.
-extern "C" int ark_m1_fastmath_errors(int n, double* out3)
+extern "C" int ark_m1_fastmath_errors(int n, double* out4)
 {
-    if (!out3 || n < 1) return ARK_M1_E_ARG;
+    if (!out4 || n < 1) return ARK_M1_E_ARG;
     double* d = nullptr;
-    if (cudaMalloc((void**)&d, 3 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return ARK_M1_E_ALLOC; }
-    cudaError_t e = cudaMemset(d, 0, 3 * sizeof(double));
+    if (cudaMalloc((void**)&d, 4 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return ARK_M1_E_ALLOC; }
+    cudaError_t e = cudaMemset(d, 0, 4 * sizeof(double));
     if (e == cudaSuccess) e = launch_fastmath_selftest(n, d, 0);
-    if (e == cudaSuccess) e = cudaMemcpy(out3, d, 3 * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(out4, d, 4 * sizeof(double), cudaMemcpyDeviceToHost);
     cudaFree(d);
     return e == cudaSuccess ? 0 : ARK_M1_E_CUDA;
 }

@@ -142,7 +142,7 @@ struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };   // Pxx..
 __device__ __forceinline__ void closure_fast(double c, double E, double Fx, double Fy, CloF& q)
 {
     const double Es = dmax_sel(E, ARK_E_FLOOR);
-    const double ice = rcp_fast(c * Es);
+    const double ice = rcp_fast3(c * Es);
     double fx = Fx * ice, fy = Fy * ice;
     // f^2 + 1e-300 (folded into the fma): the reciprocal square root below needs no guard for F = 0
     const double f2raw = fma(fx, fx, fma(fy, fy, 1e-300));
@@ -158,7 +158,7 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double rs = rsqrt_fast(s);
     const double xi = s * rs;
     const double t2 = 2.0 + xi, t5 = 5.0 + 2.0 * xi;
-    const double rp = rcp_fast(t2 * t5);
+    const double rp = rcp_fast3(t2 * t5);
     const double i2 = rp * t5, i5 = rp * t2;            // 1/(2+xi), 1/(5+2xi)
     const double chi = (3.0 + 4.0 * f2) * i5;
     const double q3 = 3.0 * i2;
@@ -198,7 +198,7 @@ __device__ __forceinline__ void face_fast(double k3h, double lminL, double lmaxL
     // cells with f = 1 exactly along the face, dl ~ 1e-100 c gives a+ = 1/2, Lambda ~ -1e-101 c, alpha = 1 (the oracle's guard
     // values 1/2, 0, 1)
     const double D = fma(-kk * lp, lm, dl);
-    const double qq = rcp_fast(dl * D);
+    const double qq = rcp_fast3(dl * D);
     fc.ap = lp * (qq * D);
     fc.Lam = lm * fc.ap;                   // l+ l-/dl
     fc.alpha = dl * (dl * qq);

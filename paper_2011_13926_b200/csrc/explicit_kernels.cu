@@ -153,24 +153,27 @@ cudaError_t launch_count_unrealizable(const Grid& g, const Fields& f, unsigned l
 }
 
 // Self-test of the fast reciprocal / reciprocal square root (m1_device.cuh) against the IEEE sequences, on n samples spread
-// over 200 binades: out[0..2] = max relative error of rcp_fast, rsqrt_fast and x * rsqrt_fast(x) (vs sqrt).
+// over 200 binades: out[0..3] = max relative error of rcp_fast, rsqrt_fast, sqrt_fast (vs sqrt) and rcp_fast3.
 __global__ void fastmath_selftest_kernel(int n, double* __restrict__ out3)
 {
-    double e0 = 0.0, e1 = 0.0, e2 = 0.0;
+    double e0 = 0.0, e1 = 0.0, e2 = 0.0, e3 = 0.0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const double x = exp2((double)(i % 200 - 100)) * (1.0 + (double)i / (double)n);
         e0 = fmax(e0, fabs(rcp_fast(x) - 1.0 / x) * x);
         const double rs = 1.0 / sqrt(x), sq = sqrt(x);
         e1 = fmax(e1, fabs(rsqrt_fast(x) - rs) * sq);
         e2 = fmax(e2, fabs(sqrt_fast(x) - sq) / sq);
+        e3 = fmax(e3, fabs(rcp_fast3(x) - 1.0 / x) * x);
     }
     for (int o = 16; o > 0; o >>= 1) {
         e0 = fmax(e0, __shfl_down_sync(0xffffffffu, e0, o)); e1 = fmax(e1, __shfl_down_sync(0xffffffffu, e1, o)); e2 = fmax(e2, __shfl_down_sync(0xffffffffu, e2, o));
+        e3 = fmax(e3, __shfl_down_sync(0xffffffffu, e3, o));
     }
     if ((threadIdx.x & 31) == 0) {      // errors are non-negative: their bit patterns order like unsigned integers
         atomicMax((unsigned long long*)&out3[0], (unsigned long long)__double_as_longlong(e0));
         atomicMax((unsigned long long*)&out3[1], (unsigned long long)__double_as_longlong(e1));
         atomicMax((unsigned long long*)&out3[2], (unsigned long long)__double_as_longlong(e2));
+        atomicMax((unsigned long long*)&out3[3], (unsigned long long)__double_as_longlong(e3));
     }
 }
 

@@ -89,6 +89,15 @@ __device__ __forceinline__ double rcp_fast(double x)
     e = fma(-x, y, 1.0); y = fma(y, e, y);            // 2^-80 -> rounding
     return y;
 }
+// Reciprocal with ONE third-order step, y (1 + e + e^2) with e = 1 - x y: 3 DFMA instead of 4, <= 1 ulp instead of
+// correctly rounded (the explicit kernel is fp64-issue bound and has four reciprocals per cell).
+__device__ __forceinline__ double rcp_fast3(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);                   // 2^-60 -> rounding
+}
 __device__ __forceinline__ double rsqrt_fast(double x)
 {
     double y;
