@@ -45,6 +45,21 @@ def test_explicit_step_ragged_shapes(shape, kernel):
     assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
 
 
+@pytest.mark.parametrize("kernel", [1, 3])
+@pytest.mark.parametrize("bc", [(1, 2, 2, 1), (2, 1, 1, 2), (0, 0, 1, 1)])
+def test_explicit_step_midsize_long_blocks(bc, kernel):
+    # 701 x 1003: blocks of 21 rows (kernel 3: seven trips of the three-row rotation loop, the last block with a ragged tail of
+    # rows handled by the general loader), 24 strips of 30 columns with a ragged last strip, Dirichlet and outflow ghost columns
+    # in the branch-free hot loop, y-ghost rows in the prologue and in the tail
+    w = small_random_state(701, 1003, seed=77, dx=0.011, dy=0.009, c=1.1, bc=bc, sig_range=(-2.0, 2.0))
+    o, g = make_oracle(w), make_gpu(w, dict(explicit_kernel=kernel))
+    dt = _dt(w)
+    for _ in range(2):
+        o.step_explicit(dt)
+        g.step_explicit(dt)
+    assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+
+
 def test_residual_matches_oracle():
     w = small_random_state(61, 47, seed=5, bc=(1, 2, 0, 0))
     o, g = make_oracle(w), make_gpu(w)
