@@ -15,7 +15,7 @@
 namespace ark {
 
 #ifndef ARK_ASM_TX
-#define ARK_ASM_TX 32      // one warp per block, like the explicit kernel: 1.104 -> 1.059 ms at 4096^2 (128 -> 64 -> 32 columns: 0.668 / 0.689 / 0.697 of HBM peak)
+#define ARK_ASM_TX 32      // one warp per block, like the explicit kernel: 1.104 -> 1.059 ms at 4096^2 (128 -> 64 -> 32 columns: 0.668 / 0.689 / 0.697 of HBM peak; with the shuffle exchange 1.008 ms = 0.73)
 #endif
 static constexpr int TXA = ARK_ASM_TX;
 __device__ __forceinline__ void asm_sync() { if (TXA == 32) __syncwarp(); else __syncthreads(); }
@@ -26,6 +26,8 @@ struct ACell {                 // one cell: raw state, closure, Jacobian
     Jac J;
 };
 struct APub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };
+__device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
 // A_k g for a Dirichlet ghost state g on the far side of face `fc` (right == true: the ghost is the R cell of the face).
 // Returns the contribution with weight w = +-dt/dx already applied, plus the WB source weight sw on the normal flux row.
@@ -86,6 +88,20 @@ __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, F
         const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
         APub me; me.E = C.u.E; me.Fx = C.u.Fx; me.Fy = C.u.Fy; me.Pxx = C.q.Pxx; me.Pxy = C.q.Pxy;
         me.lmin = C.q.lmin[0]; me.lmax = C.q.lmax[0]; me.f = C.q.f; me.st = C.u.st;
+#if ARK_ASM_TX == 32
+        // one-warp block: the neighbours' x-face data and the west face's coefficients travel by warp shuffles
+        APub R, L;
+        R.E = shfl_dn1(me.E); R.Fx = shfl_dn1(me.Fx); R.Fy = shfl_dn1(me.Fy); R.Pxx = shfl_dn1(me.Pxx); R.Pxy = shfl_dn1(me.Pxy);
+        R.lmin = shfl_dn1(me.lmin); R.lmax = shfl_dn1(me.lmax); R.f = shfl_dn1(me.f); R.st = shfl_dn1(me.st);
+        L.E = shfl_up1(me.E); L.Fx = shfl_up1(me.Fx); L.Fy = shfl_up1(me.Fy); L.Pxx = shfl_up1(me.Pxx); L.Pxy = shfl_up1(me.Pxy);
+        closure_eval<true, SD, true>(s, c, Nn.u.E, Nn.u.Fx, Nn.u.Fy, Nn.q, &Nn.J);
+        Face fn;
+        face_eval<SD, true>(s, c, g.dy, C.q.lmin[1], C.q.lmax[1], C.q.f, C.u.st, Nn.q.lmin[1], Nn.q.lmax[1], Nn.q.f, Nn.u.st, fn);
+        Face fe;
+        face_eval<SD, true>(s, c, g.dx, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
+        Face fw; fw.ap = shfl_up1(fe.ap); fw.am = shfl_up1(fe.am); fw.Lam = shfl_up1(fe.Lam); fw.alpha = shfl_up1(fe.alpha); fw.sig = shfl_up1(fe.sig);
+        if (upd) {
+#else
         pub[t] = me;
         closure_eval<true, SD, true>(s, c, Nn.u.E, Nn.u.Fx, Nn.u.Fy, Nn.q, &Nn.J);
         Face fn;
@@ -100,6 +116,7 @@ __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, F
         if (upd) {
             const int tw = t - 1;
             Face fw; fw.ap = fcs[0][tw]; fw.am = fcs[1][tw]; fw.Lam = fcs[2][tw]; fw.alpha = fcs[3][tw]; fw.sig = fcs[4][tw];
+#endif
             const long long id = (long long)j * g.nx + i;
             const bool fold_s = (j == 0 && g.bc[YLO] == BC_OUTFLOW) || (g.ny == 1 && g.bc[YLO] == BC_PERIODIC);
             const bool fold_n = (j == g.ny - 1 && g.bc[YHI] == BC_OUTFLOW) || (g.ny == 1 && g.bc[YHI] == BC_PERIODIC);
