@@ -196,6 +196,17 @@ ARK_M1_API long long ark_m1_kernel_launches(const ark_m1* h);
  * No handle needed. */
 ARK_M1_API int ark_m1_fastmath_errors(int n, double* out4);
 
+/* Self-test that MEASURES the issue rates of the instruction kinds the explicit and assembly kernels are bound by (they are
+ * fp64-issue bound, not HBM bound: DESIGN.md section 6), on the current device.  No handle needed; takes a few milliseconds.
+ * out (host, cap >= 12):
+ *   [0] DFMA lanes per clock per SM (every SM full, 8 independent chains per thread)   [1] DFMA dependent-issue latency, cycles
+ *   [2] DADD, [3] DMUL, [4] compare+select max (DSETP + SEL), [5] IMAD, [6] FFMA: lanes per clock per SM
+ *   [7] issue cycles per (DFMA + IMAD) pair per warp per SM sub-partition, [8] the same for (DFMA + FFMA)
+ *   [9] 64-bit warp shuffles, lanes per clock per SM      [10] SM clock during the test, MHz      [11] number of SMs
+ * The fp64 "alu" roofline of bench.py is out[0] * out[11] * clock lane-instructions per second.
+ * Returns 12, or ARK_M1_E_ARG / ARK_M1_E_ALLOC / ARK_M1_E_CUDA / ARK_M1_E_UNSUPPORTED. */
+ARK_M1_API int ark_m1_fp64_issue_rate(double* out, int cap);
+
 /* Device bytes currently allocated by the handle. */
 ARK_M1_API long long ark_m1_device_bytes(const ark_m1* h);
 

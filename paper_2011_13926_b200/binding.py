@@ -24,7 +24,7 @@ SYMBOLS = [
     "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
     "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_step_semi_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
-    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_fastmath_errors", "ark_m1_apply_preconditioner", "ark_m1_device_bytes",
+    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_fastmath_errors", "ark_m1_fp64_issue_rate", "ark_m1_apply_preconditioner", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
 ]
 
@@ -37,12 +37,11 @@ _lib = None
 
 
 def load_library(path: str | None = None):
-    """dlopen libark_m1.so and declare the prototypes.  Raises if the library is missing (no fallback).
-    `path` (or the environment variable ARK_M1_LIB) selects another build of the same library, e.g. a tuning variant."""
+    """dlopen libark_m1.so and declare the prototypes.  Raises if the library is missing (no fallback)."""
     global _lib
     if _lib is not None:
         return _lib
-    path = path or os.environ.get("ARK_M1_LIB") or LIB_PATH
+    path = path or LIB_PATH
     if not os.path.exists(path):
         raise RuntimeError(f"{path} not found: build it with `python -m paper_2011_13926_b200.build` "
                            "(the CUDA library is the only implementation; there is no CPU fallback)")
@@ -76,6 +75,7 @@ def load_library(path: str | None = None):
     L.ark_m1_kernel_launches.restype = C.c_longlong
     L.ark_m1_kernel_launches.argtypes = [vp]
     L.ark_m1_fastmath_errors.argtypes = [i, C.POINTER(C.c_double)]
+    L.ark_m1_fp64_issue_rate.argtypes = [C.POINTER(C.c_double), i]
     L.ark_m1_device_bytes.restype = C.c_longlong
     L.ark_m1_device_bytes.argtypes = [vp]
     L.ark_m1_last_error.restype = C.c_char_p
@@ -256,6 +256,20 @@ def fastmath_errors(n=1 << 20):
     if rc < 0:
         raise RuntimeError(f"ark_m1_fastmath_errors failed ({rc})")
     return tuple(buf)
+
+
+PIPE_RATE_KEYS = ("dfma_lanes_per_clk_sm", "dfma_latency_cycles", "dadd_lanes_per_clk_sm", "dmul_lanes_per_clk_sm",
+                  "dmax_sel_lanes_per_clk_sm", "imad_lanes_per_clk_sm", "ffma_lanes_per_clk_sm", "dfma_imad_pair_issue_cycles",
+                  "dfma_ffma_pair_issue_cycles", "shfl64_lanes_per_clk_sm", "sm_mhz", "sm_count")
+
+
+def fp64_issue_rate():
+    """Issue rates measured on the current GPU by ark_m1_fp64_issue_rate (see include/ark_m1.h), as a dict."""
+    buf = (C.c_double * 12)()
+    rc = load_library().ark_m1_fp64_issue_rate(buf, 12)
+    if rc < 0:
+        raise RuntimeError(f"ark_m1_fp64_issue_rate failed ({rc})")
+    return dict(zip(PIPE_RATE_KEYS, (float(v) for v in buf)))
 
 
 def version():

@@ -272,7 +272,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 3) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1, 2 or 3%s", ""); h->explicit_kernel = iv; }
     else if (!strcmp(key, "assembly_kernel")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "assembly_kernel must be 0 (tile) or 1 (marching)%s", ""); h->asm_kernel = iv; }
     else if (!strcmp(key, "krylov")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "krylov must be 0 (GMRES) or 1 (BiCGStab)%s", ""); h->krylov = iv; }
-    else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 32]%s", ""); h->maxv = iv; }
+    else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 16]%s", ""); h->maxv = iv; }
     else if (!strcmp(key, "basis_pad")) { if (iv < 0 || (iv & 31)) return fail(h, ARK_M1_E_ARG, "basis_pad must be a non-negative multiple of 32 doubles%s", ""); if (iv != h->basis_pad) { cudaStreamSynchronize(h->st); free_implicit(h); } h->basis_pad = iv; }
     else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
@@ -578,14 +578,16 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
                 KL(KC_SPMV, 264.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
             else
                 KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
+            // the j+1 basis vectors go through the multi-vector kernels in ceil((j+1)/MV) chunks of (nearly) equal size
+            const int nchunk = (j + MV) / MV, csize = (j + nchunk) / nchunk;
             for (int pass = 0; pass < h->ortho; ++pass) {
-                for (int c0 = 0; c0 <= j; c0 += MV) {
-                    const int nv = (j + 1 - c0) < MV ? (j + 1 - c0) : MV;
+                for (int c0 = 0; c0 <= j; c0 += csize) {
+                    const int nv = (j + 1 - c0) < csize ? (j + 1 - c0) : csize;
                     KL(KC_DOT, 24.0 * (nv + 1) * h->N, launch_multi_dot(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, pass == 0 ? DOT_H : DOT_H2, sm, h->st));
                 }
-                for (int c0 = 0; c0 <= j; c0 += MV) {
-                    const int nv = (j + 1 - c0) < MV ? (j + 1 - c0) : MV;
-                    const int last = (c0 + MV > j) && (pass == h->ortho - 1);
+                for (int c0 = 0; c0 <= j; c0 += csize) {
+                    const int nv = (j + 1 - c0) < csize ? (j + 1 - c0) : csize;
+                    const int last = (c0 + csize > j) && (pass == h->ortho - 1);
                     KL(KC_UPDATE, 24.0 * (nv + 2) * h->N, launch_update(w, h->V + (size_t)c0 * S, S, nv, c0, n, W, last, sm, h->st));
                 }
             }

@@ -41,7 +41,7 @@ struct GmresWork {                 // device pointers into one small allocation
     int caphist;
 };
 
-enum { MAXV = 32 };                // basis vectors handled per pass of the multi-vector kernels
+enum { MAXV = 16 };                // basis vectors handled per pass of the multi-vector kernels (the measured optimum: DESIGN.md section 5)
 
 enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5, DOT_AUX0 = 6, DOT_AUX1 = 7,
                BICG_ALPHA = 8, BICG_OMEGA = 9, BICG_RHO = 10 };

@@ -136,9 +136,8 @@ struct XPub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };   // what the we
 struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };   // Pxx.. hold c^2 P (what the flux needs)
 
 // Default-scheme closure with 2 reciprocals and 4 reciprocal square roots per cell:
-//   1/(cE);  rs = 1/sqrt(4 - 3 f^2) gives xi = s rs and 1/xi = rs;  one reciprocal of (2+xi)(5+2xi) gives both
-//   1/(5+2xi) (for chi) and 1/(2+xi) (for the anisotropic part and the eigenvalue prefactor);  |f| and the two
-//   eigenvalue roots as x rsqrt(x).
+//   1/(cE);  rs = 1/sqrt(4 - 3 f^2) gives xi = s rs and 1/xi = rs;  the reciprocal of 2 + xi (anisotropic part and the
+//   eigenvalue prefactor; chi itself is (5 - 2 xi)/3, no division);  |f| and the two eigenvalue roots as x rsqrt(x).
 __device__ __forceinline__ void closure_fast(double c, double E, double Fx, double Fy, CloF& q)
 {
     const double Es = dmax_sel(E, ARK_E_FLOOR);
@@ -157,17 +156,18 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     const double s = 4.0 - 3.0 * f2;       // >= 1
     const double rs = rsqrt_fast(s);
     const double xi = s * rs;
-    const double t2 = 2.0 + xi, t5 = 5.0 + 2.0 * xi;
-    const double rp = rcp_fast3(t2 * t5);
-    const double i2 = rp * t5, i5 = rp * t2;            // 1/(2+xi), 1/(5+2xi)
-    const double chi = (3.0 + 4.0 * f2) * i5;
+    // chi = (3 + 4 f^2)/(5 + 2 xi) needs no division: xi^2 = 4 - 3 f^2 gives 3 + 4 f^2 = (25 - 4 xi^2)/3 =
+    // (5 - 2 xi)(5 + 2 xi)/3, so chi = (5 - 2 xi)/3, the isotropic part (1 - chi)/2 = (xi - 1)/3 and the anisotropic
+    // coefficient (3 chi - 1)/(2 f^2) = (2 - xi)/f^2 = 3/(2 + xi): one reciprocal, of 2 + xi, serves the pressure and Eq. 14
+    const double t2 = 2.0 + xi, xm1 = xi - 1.0;
+    const double i2 = rcp_fast3(t2);                    // 1/(2+xi)
     const double q3 = 3.0 * i2;
-    const double iso = 0.5 - 0.5 * chi;
+    const double iso = 0.33333333333333333333 * xm1;
     const double Ec = (c * c) * E;                      // c^2 folded into the stored pressure
     const double Eq = Ec * q3, Ei = Ec * iso;
     q.Pxx = fma(Eq * fx, fx, Ei); q.Pxy = Eq * fx * fy; q.Pyy = fma(Eq * fy, fy, Ei);
     // Eq. 14
-    const double a = (xi - 1.0) * t2;
+    const double a = xm1 * t2;
     const double crs = c * rs;                                // c/xi
     const double k = 1.41421356237309504880 * crs * i2;       // c sqrt(2/3)/(xi (xi+2)) times the sqrt(3) taken out of the roots
     const double a23 = 0.66666666666666666667 * a;

@@ -16,22 +16,56 @@ namespace ark {
 
 int krylov_max_blocks(int sm_count) { return sm_count * 4; }
 
+// ---------------------------------------------------------------------------------------------------------
+// The two streaming kernels of the orthogonalisation.  Both are pure HBM streams (0.12 DFMA per byte), so the only thing that
+// matters is how many bytes each SM keeps in flight — and that must not depend on what ptxas does with a particular NV
+// (round 1: register counts between 40 and 166 over the 32 instances, loads serialised in some, 3 of the 4 blocks per SM
+// resident in others: 4.7-8.4 TB/s).  Shape used here, the same for every instance:
+//   * __launch_bounds__(256, 2): 2 blocks per SM always fit (<= 128 registers), grid = 2 x SMs, one wave, no tail;
+//   * a trip handles U elements (double2) per thread, U chosen so that (NV + 1) U >= 16: the trip first issues ALL its
+//     (NV + 1) U 16-byte loads into register arrays, then does the arithmetic -> 512 threads x >= 16 x 16 B >= 128 KB in
+//     flight per SM whatever NV is;
+//   * streaming loads (ld.global.cs: the basis is read once per kernel and is far larger than L2).
+// ---------------------------------------------------------------------------------------------------------
+// (measured at 4096^2 with 2, 3, 4 blocks per SM x 8, 12, 16, 24 loads per trip: 2.889-2.898 ms per GMRES iteration for all of
+// them — once every instance keeps > 100 KB per SM in flight the streams sit at what the HBM delivers, 7.6 TB/s read-only and
+// 7.0 TB/s with the write stream of the update)
+static constexpr int GS_BLOCKS_PER_SM = 2;
+__host__ __device__ constexpr int gs_unroll(int nv) { return (nv + 1) >= 16 ? 1 : (16 + nv) / (nv + 1); }   // ceil(16 / (nv + 1))
+
+__device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
+
 template <int NV>
-__global__ void __launch_bounds__(KTHREADS) multi_dot_kernel(const double* __restrict__ w, const double* __restrict__ V0,
-                                                             long long stride, long long n, GmresWork W, int mode, int col0)
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) multi_dot_kernel(const double* __restrict__ w, const double* __restrict__ V0,
+                                                                               long long stride, long long n, GmresWork W, int mode, int col0)
 {
     if ((mode == DOT_H || mode == DOT_H2 || mode == BICG_ALPHA || mode == BICG_OMEGA) && W.ctl->inner_stop) return;
+    constexpr int U = gs_unroll(NV);
     double acc[NV];
 #pragma unroll
     for (int k = 0; k < NV; ++k) acc[k] = 0.0;
-    const long long n2 = n >> 1;
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
     const double2* w2 = reinterpret_cast<const double2*>(w);
-    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
+    long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x;
+    for (; e + (U - 1) * T < n2; e += U * T) {
+        double2 a[U], b[U][NV];
+#pragma unroll
+        for (int u = 0; u < U; ++u) a[u] = ld_stream(w2 + e + u * T);
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) b[u][k] = ld_stream(reinterpret_cast<const double2*>(V0 + k * stride) + e + u * T);
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) acc[k] = fma(a[u].y, b[u][k].y, fma(a[u].x, b[u][k].x, acc[k]));
+    }
+    for (; e < n2; e += T) {                      // fewer than U elements left for this thread
         const double2 a = w2[e];
 #pragma unroll
         for (int k = 0; k < NV; ++k) {
             const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
-            acc[k] += a.x * b.x + a.y * b.y;
+            acc[k] = fma(a.y, b.y, fma(a.x, b.x, acc[k]));
         }
     }
     if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
@@ -42,25 +76,43 @@ __global__ void __launch_bounds__(KTHREADS) multi_dot_kernel(const double* __res
 }
 
 template <int NV, bool WITH_NORM>
-__global__ void __launch_bounds__(KTHREADS) update_kernel(double* __restrict__ w, const double* __restrict__ V0,
-                                                          long long stride, long long n, GmresWork W, int col0)
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) update_kernel(double* __restrict__ w, const double* __restrict__ V0,
+                                                                            long long stride, long long n, GmresWork W, int col0)
 {
     if (W.ctl->inner_stop) return;
+    constexpr int U = gs_unroll(NV);
     double cf[NV];
 #pragma unroll
     for (int k = 0; k < NV; ++k) cf[k] = W.coef[col0 + k];
     double acc[1] = { 0.0 };
-    const long long n2 = n >> 1;
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
     double2* w2 = reinterpret_cast<double2*>(w);
-    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += (long long)gridDim.x * KTHREADS) {
+    long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x;
+    for (; e + (U - 1) * T < n2; e += U * T) {
+        double2 a[U], b[U][NV];
+#pragma unroll
+        for (int u = 0; u < U; ++u) a[u] = ld_stream(w2 + e + u * T);
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) b[u][k] = ld_stream(reinterpret_cast<const double2*>(V0 + k * stride) + e + u * T);
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int k = 0; k < NV; ++k) { a[u].x = fma(-cf[k], b[u][k].x, a[u].x); a[u].y = fma(-cf[k], b[u][k].y, a[u].y); }
+            w2[e + u * T] = a[u];
+            if (WITH_NORM) acc[0] = fma(a[u].y, a[u].y, fma(a[u].x, a[u].x, acc[0]));
+        }
+    }
+    for (; e < n2; e += T) {
         double2 a = w2[e];
-        double2 b[NV];
 #pragma unroll
-        for (int k = 0; k < NV; ++k) b[k] = reinterpret_cast<const double2*>(V0 + k * stride)[e];
-#pragma unroll
-        for (int k = 0; k < NV; ++k) { a.x = fma(-cf[k], b[k].x, a.x); a.y = fma(-cf[k], b[k].y, a.y); }
+        for (int k = 0; k < NV; ++k) {
+            const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
+            a.x = fma(-cf[k], b.x, a.x); a.y = fma(-cf[k], b.y, a.y);
+        }
         w2[e] = a;
-        if (WITH_NORM) acc[0] += a.x * a.x + a.y * a.y;
+        if (WITH_NORM) acc[0] = fma(a.y, a.y, fma(a.x, a.x, acc[0]));
     }
     if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         double a = w[n - 1];
@@ -70,6 +122,14 @@ __global__ void __launch_bounds__(KTHREADS) update_kernel(double* __restrict__ w
         if (WITH_NORM) acc[0] += a * a;
     }
     if (WITH_NORM) reduce_and_finish<1, KTHREADS, true>(acc, W, DOT_UPD, 0);
+}
+
+// grid of the Gram-Schmidt streams: one wave of GS_BLOCKS_PER_SM blocks per SM (fewer on small vectors)
+static int gs_grid(long long n, int sm_count)
+{
+    const long long need = ((n >> 1) + KTHREADS - 1) / KTHREADS;
+    const long long cap = (long long)sm_count * GS_BLOCKS_PER_SM;
+    return (int)(need < 1 ? 1 : (need < cap ? need : cap));
 }
 
 static int grid_for(long long n, int sm_count)
@@ -89,13 +149,11 @@ static void dot_launch(int grd, const double* w, const double* V0, long long str
 cudaError_t launch_multi_dot(const double* w, const double* V0, long long stride, int nv, int col0, long long n,
                              GmresWork W, int mode, int sm_count, cudaStream_t st)
 {
-    const int grd = grid_for(n, sm_count);
+    const int grd = gs_grid(n, sm_count);
     switch (nv) {
 #define ARK_CASE(K) case K: dot_launch<K>(grd, w, V0, stride, n, W, mode, col0, st); break;
         ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
         ARK_CASE(9) ARK_CASE(10) ARK_CASE(11) ARK_CASE(12) ARK_CASE(13) ARK_CASE(14) ARK_CASE(15) ARK_CASE(16)
-        ARK_CASE(17) ARK_CASE(18) ARK_CASE(19) ARK_CASE(20) ARK_CASE(21) ARK_CASE(22) ARK_CASE(23) ARK_CASE(24)
-        ARK_CASE(25) ARK_CASE(26) ARK_CASE(27) ARK_CASE(28) ARK_CASE(29) ARK_CASE(30) ARK_CASE(31) ARK_CASE(32)
 #undef ARK_CASE
         default: return cudaErrorInvalidValue;
     }
@@ -113,13 +171,11 @@ static void upd_launch(int grd, double* w, const double* V0, long long stride, l
 cudaError_t launch_update(double* w, const double* V0, long long stride, int nv, int col0, long long n,
                           GmresWork W, int with_norm, int sm_count, cudaStream_t st)
 {
-    const int grd = grid_for(n, sm_count);
+    const int grd = gs_grid(n, sm_count);
     switch (nv) {
 #define ARK_CASE(K) case K: upd_launch<K>(grd, w, V0, stride, n, W, col0, with_norm, st); break;
         ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
         ARK_CASE(9) ARK_CASE(10) ARK_CASE(11) ARK_CASE(12) ARK_CASE(13) ARK_CASE(14) ARK_CASE(15) ARK_CASE(16)
-        ARK_CASE(17) ARK_CASE(18) ARK_CASE(19) ARK_CASE(20) ARK_CASE(21) ARK_CASE(22) ARK_CASE(23) ARK_CASE(24)
-        ARK_CASE(25) ARK_CASE(26) ARK_CASE(27) ARK_CASE(28) ARK_CASE(29) ARK_CASE(30) ARK_CASE(31) ARK_CASE(32)
 #undef ARK_CASE
         default: return cudaErrorInvalidValue;
     }
