@@ -56,8 +56,10 @@ enum {
 
 /* Create a solver for an nx*ny grid with cell sizes dx, dy and speed of light c.
  * bc == NULL means periodic on all sides; periodic must be set on both sides of a direction.
- * Uses the current CUDA device and the legacy default stream until ark_m1_set_stream.
- * Returns NULL on bad arguments or when no CUDA device is usable. */
+ * Uses the current CUDA device (every later call on the handle makes that device current for its duration and restores the
+ * caller's) and the legacy default stream until ark_m1_set_stream.  Limits: ny <= 262140 (several kernels map four rows to one
+ * gridDim.y slot); grids of 2^31 cells or more run on the generic explicit kernel only.
+ * Returns NULL on bad arguments, beyond the limits, or when no CUDA device is usable. */
 ARK_M1_API ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_m1_bc* bc);
 ARK_M1_API void    ark_m1_destroy(ark_m1* h);
 
@@ -89,13 +91,13 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *   "krylov"            0: restarted GMRES(restart) (north_star, default)   1: BiCGStab, the paper's solver,
  *                       right-preconditioned with the same block-Jacobi; `restart` is then ignored and the returned count is in
  *                       BiCGStab iterations (two operator applications each)
- *   "vectors_per_pass"  basis vectors handled per pass of the multi-dot / multi-axpy kernels, 1..32 (default 16, by measurement)
- *   "basis_pad"         extra doubles (multiple of 32) between consecutive Krylov basis vectors (default 0; measured: no effect)
+ *   "vectors_per_pass"  basis vectors handled per pass of the multi-dot / multi-axpy kernels, 1..16 (default 16, by measurement)
+ *   "release_workspace" non-zero: free the implicit workspace (operator planes, Krylov basis, multigrid hierarchy) now; the next
+ *                       implicit step allocates what it needs again.  Synchronises.
  *   "kernel_timing"     1: time every kernel launch with CUDA events (see ark_m1_get_kernel_stats); default 0
- *   "explicit_kernel"   0: one-thread-per-cell kernel   1: row-marching kernel, 128-column blocks
- *                       2: barrier-free warp-shuffle kernel (pure radiation only; falls back to 1 when T or source_E is set)
- *                       3: row-marching kernel, one warp per block, three-slot register rotation (no window copies) and
- *                          cp.async row prefetch (default)
+ *   "explicit_kernel"   0: one-thread-per-cell kernel (generic; all scheme switches)   1: row-marching kernel, 128-column blocks
+ *                       3: row-marching kernel, one warp per block, four-slot register rotation (no window copies), closure one
+ *                          row ahead of the faces, cp.async row prefetch (default)
  *   "operator"          1: matrix-free coefficient planes, flux form (default: 5% faster per solve at 4096^2)
  *                       0: block stencil (BSR 3x3 on the 5-point graph, pre-multiplied by M^-1)
  *   "basis_precision"   64 (default) or 32: storage precision of the GMRES Arnoldi basis.  32 = compressed-basis GMRES: the basis

@@ -33,19 +33,18 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, defines=(), out: str | None = None) -> str:
-    """Compile every .cu of csrc/ into one shared library.  Returns its path.
-    `defines` (e.g. ["ARK_MARCH_TX=256"]) and `out` build a tuning variant beside the default library."""
-    global_lib = LIB if out is None else out
-    if out is None and not defines and not force and not _stale():
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile every .cu of csrc/ into one shared library.  Returns its path."""
+    global_lib = LIB
+    if not force and not _stale():
         return LIB
     nvcc = _nvcc()
-    objdir = os.path.join(_HERE, "build" if out is None else "build_" + os.path.basename(out))
+    objdir = os.path.join(_HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     procs = []
     for s in SOURCES:
         obj = os.path.join(objdir, s.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_FLAGS, *[f"-D{d}" for d in defines], "-c", os.path.join(CSRC, s), "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, s), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((s, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))

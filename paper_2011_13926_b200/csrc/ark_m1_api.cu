@@ -36,7 +36,7 @@ struct ark_m1 {
     double *rho_cv, *ux, *uy, *source_E;
     unsigned long long* counts;   // 2
     // options
-    int ortho, explicit_kernel, op_kind, maxv, basis_pad, krylov, asm_kernel;
+    int ortho, explicit_kernel, op_kind, maxv, krylov, asm_kernel;
     int basis_prec;    // 64, or 32: compressed-basis GMRES (krylov_cb.cu); applies to GMRES + block-Jacobi + matrix-free operator
     float* V32;        // (m32_alloc + 1) basis vectors of `stride` floats
     double* wk;        // 3N: the fp64 work vector of the compressed-basis path
@@ -69,6 +69,30 @@ struct ark_m1 {
     long long launches;          // kernels launched by this handle
     char err[512];
 };
+
+// The handle lives on the device that was current at ark_m1_create.  Every entry point makes that device current for its
+// duration and restores the caller's (a multi-GPU process may have switched devices in between).
+struct DeviceGuard {
+    int prev;
+    bool switched;
+    explicit DeviceGuard(int dev) : prev(-1), switched(false)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+#define GUARD(h) DeviceGuard guard__((h)->device)
+
+namespace ark {
+int current_sm_count()
+{
+    static int cached[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    if (cached[dev] == 0) { int n = 0; cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); cached[dev] = n > 0 ? n : 148; }
+    return cached[dev];
+}
+}  // namespace ark
 
 static int fail(ark_m1* h, int code, const char* fmt, const char* detail)
 {
@@ -149,6 +173,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     if (bc) { b[0] = bc->xlo; b[1] = bc->xhi; b[2] = bc->ylo; b[3] = bc->yhi; }
     for (int s = 0; s < 4; ++s) if (b[s] < 0 || b[s] > 2) return nullptr;
     if ((b[0] == BC_PERIODIC) != (b[1] == BC_PERIODIC) || (b[2] == BC_PERIODIC) != (b[3] == BC_PERIODIC)) return nullptr;
+    if ((ny + 3) / 4 > 65535) return nullptr;      // several kernels map four rows to one gridDim.y slot (limit 65535): ny <= 262140
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     ark_m1* h = new (std::nothrow) ark_m1;
@@ -157,7 +182,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
-    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->basis_pad = 0; h->asm_kernel = 1;
+    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1;
     h->basis_prec = 64; h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -199,6 +224,7 @@ static void free_implicit(ark_m1* h)
 void ark_m1_destroy(ark_m1* h)
 {
     if (!h) return;
+    GUARD(h);
     cudaStreamSynchronize(h->st);
     for (int k = 0; k < 2; ++k) { cudaFree(h->U[k]); cudaFree(h->T[k]); }
     cudaFree(h->sa); cudaFree(h->ss_tmp); cudaFree(h->stot); cudaFree(h->counts);
@@ -217,6 +243,7 @@ void ark_m1_destroy(ark_m1* h)
 int ark_m1_set_stream(ark_m1* h, void* cuda_stream)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     CU(cudaStreamSynchronize(h->st));
     h->st = (cudaStream_t)cuda_stream;
     return 0;
@@ -225,6 +252,7 @@ int ark_m1_set_stream(ark_m1* h, void* cuda_stream)
 int ark_m1_set_state(ark_m1* h, const double* E, const double* F, const double* sigma_a, const double* sigma_s, const double* T)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!E || !F || !sigma_a || !sigma_s) return fail(h, ARK_M1_E_ARG, "set_state: NULL array%s", "");
     const size_t N = (size_t)h->N, B = N * sizeof(double);
     double* U = h->U[h->cur];
@@ -245,6 +273,7 @@ int ark_m1_set_state(ark_m1* h, const double* E, const double* F, const double* 
 int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const double* F_g, const double* sa_g, const double* ss_g)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (side < 0 || side > 3 || !E_g || !F_g || !sa_g || !ss_g) return fail(h, ARK_M1_E_ARG, "set_boundary: bad argument%s", "");
     const size_t len = (side < 2) ? h->g.ny : h->g.nx, B = len * sizeof(double);
     CU(cudaMemcpyAsync(h->gh[side][0], E_g, B, cudaMemcpyDefault, h->st));
@@ -260,6 +289,7 @@ int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const double* F_
 int ark_m1_set_option(ark_m1* h, const char* key, double value)
 {
     if (!h || !key) return ARK_M1_E_ARG;
+    GUARD(h);
     const int iv = (int)value;
     if (!strcmp(key, "well_balanced")) h->s.wb = (value != 0.0);
     else if (!strcmp(key, "ap_mode")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "ap_mode must be 0, 1 or 2%s", ""); h->s.ap = iv; }
@@ -269,11 +299,11 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "eig_floor")) { if (!(value >= 0.0)) return fail(h, ARK_M1_E_ARG, "eig_floor must be >= 0%s", ""); h->s.eig_floor = value; }
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
     else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
-    else if (!strcmp(key, "explicit_kernel")) { if (iv < 0 || iv > 3) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0, 1, 2 or 3%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "explicit_kernel")) { if (iv != 0 && iv != 1 && iv != 3) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0 (cell), 1 (128-column march) or 3 (one-warp march, default)%s", ""); h->explicit_kernel = iv; }
     else if (!strcmp(key, "assembly_kernel")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "assembly_kernel must be 0 (tile) or 1 (marching)%s", ""); h->asm_kernel = iv; }
     else if (!strcmp(key, "krylov")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "krylov must be 0 (GMRES) or 1 (BiCGStab)%s", ""); h->krylov = iv; }
     else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 16]%s", ""); h->maxv = iv; }
-    else if (!strcmp(key, "basis_pad")) { if (iv < 0 || (iv & 31)) return fail(h, ARK_M1_E_ARG, "basis_pad must be a non-negative multiple of 32 doubles%s", ""); if (iv != h->basis_pad) { cudaStreamSynchronize(h->st); free_implicit(h); } h->basis_pad = iv; }
+    else if (!strcmp(key, "release_workspace")) { if (value != 0.0) { cudaStreamSynchronize(h->st); free_implicit(h); } }
     else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
@@ -288,6 +318,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
 int ark_m1_set_field(ark_m1* h, const char* name, const double* plane)
 {
     if (!h || !name) return ARK_M1_E_ARG;
+    GUARD(h);
     double** dst = nullptr;
     if (!strcmp(name, "rho_cv")) dst = &h->rho_cv; else if (!strcmp(name, "ux")) dst = &h->ux;
     else if (!strcmp(name, "uy")) dst = &h->uy; else if (!strcmp(name, "source_E")) dst = &h->source_E;
@@ -302,6 +333,7 @@ int ark_m1_set_field(ark_m1* h, const char* name, const double* plane)
 int ark_m1_get_state(ark_m1* h, double* E, double* F, double* T)
 {
     if (!h || !E || !F) return ARK_M1_E_ARG;
+    GUARD(h);
     const size_t N = (size_t)h->N, B = N * sizeof(double);
     const double* U = h->U[h->cur];
     CU(cudaMemcpyAsync(E, U, B, cudaMemcpyDefault, h->st));
@@ -315,18 +347,16 @@ static int explicit_once(ark_m1* h, double dt)
 {
     const Fields f = fields_of(h);
     double* O = h->U[h->cur ^ 1];
-    const bool plain = !h->have_T && !h->source_E;
-    if (h->explicit_kernel == 3 && h->N < (1LL << 31)) {
-        KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N,
-                                                                                   h->have_T ? h->T[h->cur ^ 1] : nullptr, h->sm_count, h->st));
-    } else if (h->explicit_kernel == 2 && plain && h->N < (1LL << 31)) {
-        KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_warp(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, h->sm_count, h->st));
-    } else if (h->explicit_kernel >= 1 && h->N < (1LL << 31)) {   // the march kernels use 32-bit in-plane offsets
-        KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N,
-                                                                                  h->have_T ? h->T[h->cur ^ 1] : nullptr, h->sm_count, h->st));
-    } else {
-        KL(KC_EXPLICIT, (h->have_T ? 88.0 : 64.0) * h->N, launch_explicit_cell(h->g, h->s, f, dt, 0, O, O + h->N, O + 2 * h->N, h->have_T ? h->T[h->cur ^ 1] : nullptr, h->st));
-    }
+    double* OT = h->have_T ? h->T[h->cur ^ 1] : nullptr;
+    // algorithmic bytes per cell: 5 planes in, 3 out; the coupled step adds T in/out (16), rho c_v (8) and the source plane (8)
+    const double bpc = 64.0 + (h->have_T ? 16.0 + (h->rho_cv ? 8.0 : 0.0) : 0.0) + (h->source_E ? 8.0 : 0.0);
+    const bool small = h->N < (1LL << 31);          // the march kernels use 32-bit in-plane offsets (their launchers check it too)
+    if (h->explicit_kernel == 3 && small)
+        KL(KC_EXPLICIT, bpc * h->N, launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, OT, h->sm_count, h->st));
+    else if (h->explicit_kernel >= 1 && small)
+        KL(KC_EXPLICIT, bpc * h->N, launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, OT, h->sm_count, h->st));
+    else
+        KL(KC_EXPLICIT, bpc * h->N, launch_explicit_cell(h->g, h->s, f, dt, 0, O, O + h->N, O + 2 * h->N, OT, h->st));
     h->cur ^= 1;
     return 0;
 }
@@ -334,6 +364,7 @@ static int explicit_once(ark_m1* h, double dt)
 int ark_m1_step_explicit(ark_m1* h, double dt)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "step_explicit: dt must be > 0%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_explicit: no state set%s", "");
     return explicit_once(h, dt);
@@ -342,6 +373,7 @@ int ark_m1_step_explicit(ark_m1* h, double dt)
 int ark_m1_steps_explicit(ark_m1* h, double dt, int nsteps)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!(dt > 0.0) || nsteps < 0) return fail(h, ARK_M1_E_ARG, "steps_explicit: dt must be > 0 and nsteps >= 0%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "steps_explicit: no state set%s", "");
     for (int k = 0; k < nsteps; ++k) { int rc = explicit_once(h, dt); if (rc) return rc; }
@@ -351,6 +383,7 @@ int ark_m1_steps_explicit(ark_m1* h, double dt, int nsteps)
 int ark_m1_residual(ark_m1* h, double* RE, double* RF)
 {
     if (!h || !RE || !RF) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "residual: no state set%s", "");
     const Fields f = fields_of(h);
     double* O = h->U[h->cur ^ 1];
@@ -365,6 +398,7 @@ int ark_m1_residual(ark_m1* h, double* RE, double* RF)
 int ark_m1_add_velocity_sources(ark_m1* h, double dt)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!h->have_state || !h->ux || !h->uy) return fail(h, ARK_M1_E_NOTSET, "add_velocity_sources: state, ux, uy must be set%s", "");
     const Fields f = fields_of(h);
     double* U = h->U[h->cur];
@@ -375,6 +409,7 @@ int ark_m1_add_velocity_sources(ark_m1* h, double dt)
 int ark_m1_count_unrealizable(ark_m1* h, long long* nE, long long* nf)
 {
     if (!h || !nE || !nf) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "count_unrealizable: no state set%s", "");
     CU(cudaMemsetAsync(h->counts, 0, 2 * sizeof(unsigned long long), h->st));
     KL(KC_SMALL, 24.0 * h->N, launch_count_unrealizable(h->g, fields_of(h), h->counts, h->st));
@@ -452,7 +487,7 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
             if (rc) return rc;
         }
     }
-    h->stride = (long long)((n + 31) / 32 * 32) + h->basis_pad;
+    h->stride = (long long)((n + 31) / 32 * 32);
     {   // fp64 vector slots: the whole basis, or (compressed-basis path) the six slots BiCGStab and the staging calls use
         const int need = use_cb(h) ? 6 : ((m + 1) > 6 ? (m + 1) : 6);
         if (h->vslots < need) {
@@ -746,6 +781,7 @@ static int finish_implicit(ark_m1* h, double dt, double* final_residual)
 extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit: no state set%s", "");
     int rc = ensure_implicit(h, (h->krylov == 1 && restart < 5) ? 5 : restart, maxit);
@@ -766,6 +802,7 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
                                            int* newton_iterations, double* final_residual, double* final_update)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0 || !(newton_tol >= 0.0) || max_newton < 1)
         return fail(h, ARK_M1_E_ARG, "step_implicit_newton: need dt > 0, tol > 0, restart >= 1, maxit >= 0, newton_tol >= 0, max_newton >= 1%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit_newton: no state set%s", "");
@@ -806,6 +843,7 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
 extern "C" int ark_m1_step_semi_implicit(ark_m1* h, double dt, double tol, int restart, int maxit, double* final_residual)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_semi_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_semi_implicit: no state set%s", "");
     if (h->N >= (1LL << 31)) return fail(h, ARK_M1_E_UNSUPPORTED, "step_semi_implicit: grid too large for the marching kernels%s", "");
@@ -831,6 +869,7 @@ extern "C" int ark_m1_step_semi_implicit(ark_m1* h, double dt, double tol, int r
 extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, double* out, double* b_out)
 {
     if (!h || !Vin || !out) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "apply_operator: dt must be > 0%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "apply_operator: no state set%s", "");
     int rc = ensure_implicit(h, 1, 1);
@@ -857,6 +896,7 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
 extern "C" int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* Vin, double* out)
 {
     if (!h || !Vin || !out) return ARK_M1_E_ARG;
+    GUARD(h);
     if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "apply_preconditioner: dt must be > 0%s", "");
     if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "apply_preconditioner: no state set%s", "");
     int rc = ensure_implicit(h, 1, 1);
@@ -882,6 +922,7 @@ extern "C" int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* V
 extern "C" int ark_m1_get_history(ark_m1* h, double* buf, int cap)
 {
     if (!h) return ARK_M1_E_ARG;
+    GUARD(h);
     const int n = (int)h->hist_host->size();
     if (buf) for (int k = 0; k < n && k < cap; ++k) buf[k] = (*h->hist_host)[k];
     return n;
@@ -890,6 +931,7 @@ extern "C" int ark_m1_get_history(ark_m1* h, double* buf, int cap)
 extern "C" int ark_m1_get_timings(ark_m1* h, double* out3)
 {
     if (!h || !out3) return ARK_M1_E_ARG;
+    GUARD(h);
     for (int k = 0; k < 3; ++k) out3[k] = h->timings[k];
     return 0;
 }
@@ -899,6 +941,7 @@ extern "C" int ark_m1_get_timings(ark_m1* h, double* out3)
 extern "C" int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap)
 {
     if (!h || !out) return ARK_M1_E_ARG;
+    GUARD(h);
     kflush(h);
     for (int k = 0; k < KC_COUNT && 3 * k + 2 < cap; ++k) for (int q = 0; q < 3; ++q) out[3 * k + q] = h->kstat[k][q];
     return KC_COUNT;

@@ -47,6 +47,9 @@ enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4,
                BICG_ALPHA = 8, BICG_OMEGA = 9, BICG_RHO = 10 };
 enum { BS_RHO = 0, BS_ALPHA = 1, BS_OMEGA = 2, BS_RHO_NEW = 3, BS_RN = 4, BS_RESTART = 5 };
 
+// number of SMs of the CURRENT device (cached per device; ark_m1_api.cu) — grid sizes are multiples of it
+int current_sm_count();
+
 // ---------------------------------------------------------------------------------------------------------
 // Launchers (each enqueues on `st`, returns cudaGetLastError()).
 // ---------------------------------------------------------------------------------------------------------
@@ -57,13 +60,11 @@ cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& 
                                   double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st);
 cudaError_t launch_explicit_march3(const Grid& g, const Scheme& s, const Fields& f, double dt,
                                    double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st);
-cudaError_t launch_explicit_warp(const Grid& g, const Scheme& s, const Fields& f, double dt,
-                                 double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st);
 cudaError_t launch_velocity_sources(const Grid& g, const Scheme& s, const Fields& f, const double* ux, const double* uy,
                                     double dt, double* E, double* Fx, double* Fy, cudaStream_t st);
 cudaError_t launch_count_unrealizable(const Grid& g, const Fields& f, unsigned long long* counts2, cudaStream_t st);
 cudaError_t launch_fastmath_selftest(int n, double* out3, cudaStream_t st);
-cudaError_t launch_add_planes(double* st_out, const double* a, const double* b, long long n, cudaStream_t st);
+cudaError_t launch_add_planes(double* st_out, const double* a, const double* b, long long n, cudaStream_t st);   // st_out may be b
 
 // implicit_kernels.cu
 struct BlockMatrix {      // SoA planes of N doubles each
@@ -153,7 +154,7 @@ cudaError_t launch_bicg_s(double* r, const double* v, long long n, GmresWork W, 
 cudaError_t launch_bicg_xr(double* y, const double* p, double* r, const double* t, const double* rhat, long long n,
                            GmresWork W, int sm_count, cudaStream_t st);   // y += alpha p + omega r; r -= omega t; rho, ||r||
 cudaError_t launch_combine_y(const Grid& g, const double* Minv, double* y, double* x, cudaStream_t st);                  // x += M^-1 y; y = 0
-cudaError_t launch_sub(double* out, const double* a, const double* b, long long n, cudaStream_t st);   // out = a - b
+cudaError_t launch_sub(double* out, const double* a, const double* b, long long n, cudaStream_t st);   // out = a - b (out may be a or b)
 cudaError_t launch_begin_solve(GmresWork W, double tol, int m, int maxit, cudaStream_t st);
 
 }  // namespace ark

@@ -5,23 +5,8 @@
 
 namespace ark {
 
-// tuning knobs (defaults chosen by measurement on B200)
-#ifndef ARK_MARCH_TX
-#define ARK_MARCH_TX 128
-#endif
-#ifndef ARK_MARCH_UNROLL
-#define ARK_MARCH_UNROLL 1
-#endif
-#ifndef ARK_MARCH_MINB
-#define ARK_MARCH_MINB 4
-#endif
-#ifndef ARK_MARCH_RY
-#define ARK_MARCH_RY 32
-#endif
-#ifndef ARK_MARCH_ASYNC
-#define ARK_MARCH_ASYNC 0   // 1: prefetch rows with cp.async into a shared-memory ring
-#endif
-static constexpr int TX = ARK_MARCH_TX;
+static constexpr int TX = 128;         // columns per block of explicit_march_kernel (126 updated + 2 halo)
+static constexpr int MARCH_RY = 32;    // rows per block (cap)
 
 struct Raw { double E, Fx, Fy, st, sa; };
 
@@ -29,20 +14,6 @@ struct Raw { double E, Fx, Fy, st, sa; };
 // (interior row) costs one multiply-add and five loads.
 //   xmode 0: column ii of the grid (after periodic wrap / outflow clamp);  1: Dirichlet x-ghost of side xside;  2: inactive.
 // j may be -1 or ny (y ghost).  Corner ghosts are never used by a 5-point stencil and return a dummy state.
-#ifndef ARK_MARCH_PINLOAD
-#define ARK_MARCH_PINLOAD 0     // 1: the hot-path loads are volatile asm, so that ptxas cannot sink the prefetch
-#endif
-__device__ __forceinline__ double ld_pinned(const double* p)
-{
-#if ARK_MARCH_PINLOAD
-    double x;
-    asm volatile("ld.global.f64 %0, [%1];" : "=d"(x) : "l"(p) : "memory");
-    return x;
-#else
-    return *p;
-#endif
-}
-
 __device__ __forceinline__ Raw load_row_general(const Fields& f, const Grid& g, int xmode, int ii, int xside, int j);
 
 // Hot path first (interior row of a grid column: no default values are materialised), everything else in load_row_general.
@@ -51,7 +22,7 @@ __device__ __forceinline__ Raw load_row(const Fields& f, const Grid& g, int xmod
     if (xmode == 0 && (unsigned int)j < (unsigned int)g.ny) {
         Raw r;
         const unsigned int id = (unsigned int)j * (unsigned int)g.nx + (unsigned int)ii;
-        r.E = ld_pinned(f.E + id); r.Fx = ld_pinned(f.Fx + id); r.Fy = ld_pinned(f.Fy + id); r.st = ld_pinned(f.st + id); r.sa = ld_pinned(f.sa + id);
+        r.E = f.E[id]; r.Fx = f.Fx[id]; r.Fy = f.Fy[id]; r.st = f.st[id]; r.sa = f.sa[id];
         return r;
     }
     return load_row_general(f, g, xmode, ii, xside, j);
@@ -64,7 +35,7 @@ __device__ __forceinline__ Raw load_row_general(const Fields& f, const Grid& g, 
     if (j >= 0 && j < g.ny) {
         if (xmode == 0) {
             const unsigned int id = (unsigned int)j * (unsigned int)g.nx + (unsigned int)ii;
-            r.E = ld_pinned(f.E + id); r.Fx = ld_pinned(f.Fx + id); r.Fy = ld_pinned(f.Fy + id); r.st = ld_pinned(f.st + id); r.sa = ld_pinned(f.sa + id);
+            r.E = f.E[id]; r.Fx = f.Fx[id]; r.Fy = f.Fy[id]; r.st = f.st[id]; r.sa = f.sa[id];
         } else {
             r.E = f.gh[xside][0][j]; r.Fx = f.gh[xside][1][j]; r.Fy = f.gh[xside][2][j]; r.sa = f.gh[xside][3][j]; r.st = f.gh[xside][4][j];
         }
@@ -83,7 +54,7 @@ __device__ __forceinline__ Raw load_row_general(const Fields& f, const Grid& g, 
     return r;
 }
 
-// Asynchronous variant of load_row (ARK_MARCH_ASYNC): the five values of one cell go straight from global to this
+// Asynchronous variant of load_row: the five values of one cell go straight from global to this
 // thread's own slots of a shared-memory ring with cp.async (LDGSTS), so no registers are held while the request is in
 // flight and the compiler cannot sink the prefetch towards its use.  A thread only ever reads back its own slots,
 // hence cp.async.wait_group is the only synchronisation needed.  ring layout: [stage][field][thread].
@@ -133,7 +104,7 @@ __device__ __forceinline__ void load_row_async(double (*ring)[TXN], int t, const
 struct XPub { double E, Fx, Fy, Pxx, Pxy, lmin, lmax, f, st; };   // what the west neighbour needs for its east face
 
 // What the march kernel keeps per cell: pressure, Eq. 14 eigenvalues for both face orientations, |f|.
-struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };   // Pxx.. hold c^2 P (what the flux needs)
+struct CloF { double Pxx, Pxy, Pyy, lminx, lmaxx, lminy, lmaxy, f; };   // Pxx.. hold c^2 P (what the flux needs); f = |f|/2
 
 // Default-scheme closure with 2 reciprocals and 4 reciprocal square roots per cell:
 //   1/(cE);  rs = 1/sqrt(4 - 3 f^2) gives xi = s rs and 1/xi = rs;  the reciprocal of 2 + xi (anisotropic part and the
@@ -145,14 +116,16 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     double fx = Fx * ice, fy = Fy * ice;
     // f^2 + 1e-300 (folded into the fma): the reciprocal square root below needs no guard for F = 0
     const double f2raw = fma(fx, fx, fma(fy, fy, 1e-300));
-    // |f| and the clamp of PAPER.md:513, branch-free: one rsqrt serves both (f = f2 rsqrt(f2); rescale by rsqrt(f2) if f2 > 1)
+    // |f| and the clamp of PAPER.md:513, branch-free: one rsqrt serves both (f = f2 rsqrt(f2); rescale by rsqrt(f2) if f2 > 1).
+    // (A warp-uniform branch around the rare clamp/overflow selects was measured: no gain, it splits the row's basic block.)
     const bool huge = !(f2raw <= 1e300);          // E <= 0 (floored): F/(cE) overflows; 1/sqrt(inf) = 0 like IEEE
     const double rf = rsqrt_fast(huge ? 1.0 : f2raw);
     const bool clamp = f2raw > 1.0;
     const double sc = clamp ? (huge ? 0.0 : rf) : 1.0;
     fx *= sc; fy *= sc;
     const double f2 = clamp ? 1.0 : f2raw;
-    q.f = clamp ? 1.0 : f2raw * rf;
+    const double fh = clamp ? 0.5 : (0.5 * f2raw) * rf;      // |f|/2: the face needs (f_L + f_R)/2
+    q.f = fh;
     const double s = 4.0 - 3.0 * f2;       // >= 1
     const double rs = rsqrt_fast(s);
     const double xi = s * rs;
@@ -161,10 +134,8 @@ __device__ __forceinline__ void closure_fast(double c, double E, double Fx, doub
     // coefficient (3 chi - 1)/(2 f^2) = (2 - xi)/f^2 = 3/(2 + xi): one reciprocal, of 2 + xi, serves the pressure and Eq. 14
     const double t2 = 2.0 + xi, xm1 = xi - 1.0;
     const double i2 = rcp_fast3(t2);                    // 1/(2+xi)
-    const double q3 = 3.0 * i2;
-    const double iso = 0.33333333333333333333 * xm1;
-    const double Ec = (c * c) * E;                      // c^2 folded into the stored pressure
-    const double Eq = Ec * q3, Ei = Ec * iso;
+    const double c2 = c * c;                            // uniform: hoisted out of the row loop
+    const double Eq = E * ((3.0 * c2) * i2), Ei = E * ((0.33333333333333333333 * c2) * xm1);   // c^2 folded into the stored pressure
     q.Pxx = fma(Eq * fx, fx, Ei); q.Pxy = Eq * fx * fy; q.Pyy = fma(Eq * fy, fy, Ei);
     // Eq. 14
     const double a = xm1 * t2;
@@ -192,7 +163,7 @@ __device__ __forceinline__ void face_fast(double k3h, double lminL, double lmaxL
     const double lm = dmin_sel(dmin_sel(lminL, lminR), 0.0);
     const double dl = lp - lm;
     fc.sig = stL + stR;
-    const double ff = 0.5 * (fL + fR);
+    const double ff = fL + fR;             // the cells store |f|/2
     const double kk = k3h * fc.sig * fma(-ff, ff, 1.0);
     // dl > 0 always: closure_fast's eigenvalue roots are >= ~1e-101 c, so (l+, l-) = (0, 0) cannot occur; on a face between
     // cells with f = 1 exactly along the face, dl ~ 1e-100 c gives a+ = 1/2, Lambda ~ -1e-101 c, alpha = 1 (the oracle's guard
@@ -212,7 +183,7 @@ __device__ __forceinline__ void cell_closure(const Scheme& s, double c, const Ra
     else {
         Clo t; closure_eval<false, false>(s, c, u.E, u.Fx, u.Fy, t, nullptr);
         const double c2 = c * c;
-        q.Pxx = c2 * t.Pxx; q.Pxy = c2 * t.Pxy; q.Pyy = c2 * t.Pyy; q.f = t.f;
+        q.Pxx = c2 * t.Pxx; q.Pxy = c2 * t.Pxy; q.Pyy = c2 * t.Pyy; q.f = 0.5 * t.f;
         q.lminx = t.lmin[0]; q.lmaxx = t.lmax[0]; q.lminy = t.lmin[1]; q.lmaxy = t.lmax[1];
     }
 }
@@ -224,7 +195,7 @@ __device__ __forceinline__ void cell_face(const Scheme& s, double c, double delt
 {
     if (SD) face_fast(k3h, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, fc);
     else {
-        Face t; face_eval<false>(s, c, delta, lminL, lmaxL, fL, stL, lminR, lmaxR, fR, stR, t);
+        Face t; face_eval<false>(s, c, delta, lminL, lmaxL, 2.0 * fL, stL, lminR, lmaxR, 2.0 * fR, stR, t);
         fc.ap = t.ap; fc.Lam = t.Lam; fc.alpha = t.alpha; fc.sig = 2.0 * t.sig;     // a+ + a- = 1 in every scheme variant
     }
 }

@@ -122,7 +122,7 @@ cudaError_t launch_velocity_sources(const Grid& g, const Scheme& s, const Fields
                                     double dt, double* E, double* Fx, double* Fy, cudaStream_t st)
 {
     const long long N = (long long)g.nx * g.ny;
-    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < 148 * 8 ? (N + blk - 1) / blk : 148 * 8);
+    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < current_sm_count() * 8 ? (N + blk - 1) / blk : current_sm_count() * 8);
     velocity_sources_kernel<<<grd, blk, 0, st>>>(g, s, f, ux, uy, dt, E, Fx, Fy);
     return cudaGetLastError();
 }
@@ -147,7 +147,7 @@ __global__ void count_unrealizable_kernel(Grid g, Fields f, unsigned long long* 
 cudaError_t launch_count_unrealizable(const Grid& g, const Fields& f, unsigned long long* counts2, cudaStream_t st)
 {
     const long long N = (long long)g.nx * g.ny;
-    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < 148 * 8 ? (N + blk - 1) / blk : 148 * 8);
+    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < current_sm_count() * 8 ? (N + blk - 1) / blk : current_sm_count() * 8);
     count_unrealizable_kernel<<<grd, blk, 0, st>>>(g, f, counts2);
     return cudaGetLastError();
 }
@@ -179,18 +179,19 @@ __global__ void fastmath_selftest_kernel(int n, double* __restrict__ out3)
 
 cudaError_t launch_fastmath_selftest(int n, double* out3, cudaStream_t st)
 {
-    fastmath_selftest_kernel<<<148, 256, 0, st>>>(n, out3);
+    fastmath_selftest_kernel<<<current_sm_count(), 256, 0, st>>>(n, out3);
     return cudaGetLastError();
 }
 
-__global__ void add_planes_kernel(double* __restrict__ o, const double* __restrict__ a, const double* __restrict__ b, long long n)
+// o may alias a or b (set_boundary adds in place): no __restrict__
+__global__ void add_planes_kernel(double* o, const double* a, const double* b, long long n)
 {
     for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) o[k] = a[k] + b[k];
 }
 
 cudaError_t launch_add_planes(double* o, const double* a, const double* b, long long n, cudaStream_t st)
 {
-    const int blk = 256; const int grd = (int)((n + blk - 1) / blk < 148 * 8 ? (n + blk - 1) / blk : 148 * 8);
+    const int blk = 256; const int grd = (int)((n + blk - 1) / blk < current_sm_count() * 8 ? (n + blk - 1) / blk : current_sm_count() * 8);
     add_planes_kernel<<<grd, blk, 0, st>>>(o, a, b, n);
     return cudaGetLastError();
 }

@@ -16,7 +16,7 @@ namespace ark {
 
 // COUPLED: stage-2 terms of the cell kernel (emission c sigma_a a_r T^4, source_E, explicit matter-energy update of Eq. 4).
 template <bool SD, bool COUPLED>
-__global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
+__global__ void __launch_bounds__(TX, 4) explicit_march_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
                                                             double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy,
                                                             double* __restrict__ oT)
 {
@@ -46,17 +46,9 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
     }
 
     // prologue: rows j0-1 (south) and j0 (centre); flux through the south face of row j0
-#if ARK_MARCH_ASYNC
-    __shared__ double ring[3][5][TX];
-    load_row_async<TX>(ring[0], t, f, g, xmode, ii, xside, j0 + 1, true);      // slot 0 <- row j0+1
-    load_row_async<TX>(ring[1], t, f, g, xmode, ii, xside, j0 + 2, j0 + 1 < j1);
-    int slot_n = 0, slot_p = 2;     // slot holding row j+1; slot receiving row j+3
-#endif
     Raw uS = load_row(f, g, xmode, ii, xside, j0 - 1);
     Raw uC = load_row(f, g, xmode, ii, xside, j0);
-#if !ARK_MARCH_ASYNC
     Raw uN = load_row(f, g, xmode, ii, xside, j0 + 1);
-#endif
     CloF qS, qC;
     cell_closure<SD>(s, c, uS, qS);
     cell_closure<SD>(s, c, uC, qC);
@@ -70,20 +62,10 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
     // 32-bit in-plane offsets (host guarantees nx*ny < 2^31)
     unsigned int row_off = (unsigned int)j0 * (unsigned int)g.nx + (unsigned int)(i < 0 ? 0 : i);
 
-    constexpr int kUnroll = ARK_MARCH_UNROLL;
-#pragma unroll kUnroll
+#pragma unroll 1
     for (int j = j0; j < j1; ++j) {
-#if ARK_MARCH_ASYNC
-        // request row j+3, then take row j+1 out of the ring (its group is the third youngest)
-        load_row_async<TX>(ring[slot_p], t, f, g, xmode, ii, xside, j + 3, j + 2 < j1);
-        cp_async_wait<2>();
-        Raw uN;
-        uN.E = ring[slot_n][0][t]; uN.Fx = ring[slot_n][1][t]; uN.Fy = ring[slot_n][2][t]; uN.st = ring[slot_n][3][t]; uN.sa = ring[slot_n][4][t];
-        slot_p = slot_n; slot_n = (slot_n == 2) ? 0 : slot_n + 1;
-#else
         // prefetch the raw state two rows ahead
         const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
-#endif
         // publish the x-face data of this cell (computed one row ago)
         XPub me; me.E = uC.E; me.Fx = uC.Fx; me.Fy = uC.Fy; me.Pxx = qC.Pxx; me.Pxy = qC.Pxy;
         me.lmin = qC.lminx; me.lmax = qC.lmaxx; me.f = qC.f; me.st = uC.st;
@@ -130,127 +112,21 @@ __global__ void __launch_bounds__(TX, ARK_MARCH_MINB) explicit_march_kernel(Grid
         }
         row_off += (unsigned int)g.nx;
         // shift the window north
-#if ARK_MARCH_ASYNC
-        uC = uN; qC = qN;
-#else
-        uC = uN; qC = qN; uN = uNN;
-#endif
-        Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// Barrier-free variant: a WARP owns 30 columns (+1 halo lane each side) and exchanges the x-face data with
-// __shfl_down/__shfl_up, so warps never wait for one another and the row body is one basic block.
-// ---------------------------------------------------------------------------------------------------------
-#ifndef ARK_WARP_WPB
-#define ARK_WARP_WPB 4      // warps per block
-#endif
-#ifndef ARK_WARP_MINB
-#define ARK_WARP_MINB 4
-#endif
-static constexpr int WPB = ARK_WARP_WPB;
-static constexpr int WCOLS = 30;
-
-__device__ __forceinline__ double shfl_dn(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
-__device__ __forceinline__ double shfl_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
-
-template <bool SD>
-__global__ void __launch_bounds__(32 * WPB, ARK_WARP_MINB) explicit_warp_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
-                                                            double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int i = (blockIdx.x * WPB + warp) * WCOLS - 1 + lane;
-    const int j0 = blockIdx.y * RY;
-    const int j1 = min(j0 + RY, g.ny);
-    const bool col_active = (i <= g.nx);
-    const bool upd = (lane >= 1 && lane <= WCOLS && i >= 0 && i < g.nx);
-    const double c = g.c, cdt = c * dt;
-    const double rdx = dt / g.dx, rdy = dt / g.dy;
-    const double k3x = 1.5 * g.dx / c, k3y = 1.5 * g.dy / c;
-    const double qc = 0.125 * c * dt;
-    const bool wb = SD ? true : (s.wb != 0);
-
-    int xmode = 0, ii = i, xside = 0;
-    if (!col_active) xmode = 2;
-    else if (i < 0 || i >= g.nx) {
-        xside = (i < 0) ? XLO : XHI;
-        const int bc = g.bc[xside];
-        if (bc == BC_DIRICHLET) { xmode = 1; ii = 0; }
-        else if (bc == BC_PERIODIC) ii = (i < 0) ? g.nx - 1 : 0;
-        else ii = (i < 0) ? 0 : g.nx - 1;
-    }
-    Raw uS = load_row(f, g, xmode, ii, xside, j0 - 1);
-    Raw uC = load_row(f, g, xmode, ii, xside, j0);
-    Raw uN = load_row(f, g, xmode, ii, xside, j0 + 1);
-    CloF qS, qC;
-    cell_closure<SD>(s, c, uS, qS);
-    cell_closure<SD>(s, c, uC, qC);
-    double Hs0, Hs1, Hs2, Ss;
-    {
-        FaceF fs;
-        cell_face<SD>(s, c, g.dy, k3y, qS.lminy, qS.lmaxy, qS.f, uS.st, qC.lminy, qC.lmaxy, qC.f, uC.st, fs);
-        ARK_FACE_FLUX(fs, uS.E, uC.E, uS.Fy, uC.Fy, uS.Fx, uC.Fx, qS.Pyy, qC.Pyy, qS.Pxy, qC.Pxy, Hs0, Hs2, Hs1, Ss);
-    }
-    unsigned int row_off = (unsigned int)j0 * (unsigned int)g.nx + (unsigned int)(i < 0 ? 0 : i);
-
-    for (int j = j0; j < j1; ++j) {
-        const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
-        // east neighbour's x-face data (lane + 1)
-        const double RE = shfl_dn(uC.E), RFx = shfl_dn(uC.Fx), RFy = shfl_dn(uC.Fy), RPxx = shfl_dn(qC.Pxx), RPxy = shfl_dn(qC.Pxy);
-        const double Rlmin = shfl_dn(qC.lminx), Rlmax = shfl_dn(qC.lmaxx), Rf = shfl_dn(qC.f), Rst = shfl_dn(uC.st);
-        // north cell closure + north face
-        CloF qN;
-        cell_closure<SD>(s, c, uN, qN);
-        FaceF fn;
-        cell_face<SD>(s, c, g.dy, k3y, qC.lminy, qC.lmaxy, qC.f, uC.st, qN.lminy, qN.lmaxy, qN.f, uN.st, fn);
-        double Hn0, Hn1, Hn2, Sn;
-        ARK_FACE_FLUX(fn, uC.E, uN.E, uC.Fy, uN.Fy, uC.Fx, uN.Fx, qC.Pyy, qN.Pyy, qC.Pxy, qN.Pxy, Hn0, Hn2, Hn1, Sn);
-        // east face
-        double Ge0, Ge1, Ge2, Se;
-        {
-            FaceF fe;
-            cell_face<SD>(s, c, g.dx, k3x, qC.lminx, qC.lmaxx, qC.f, uC.st, Rlmin, Rlmax, Rf, Rst, fe);
-            ARK_FACE_FLUX(fe, uC.E, RE, uC.Fx, RFx, uC.Fy, RFy, qC.Pxx, RPxx, qC.Pxy, RPxy, Ge0, Ge1, Ge2, Se);
-        }
-        // west flux = east flux of lane - 1
-        const double Gw0 = shfl_up(Ge0), Gw1 = shfl_up(Ge1), Gw2 = shfl_up(Ge2), Sw = shfl_up(Se);
-        double dSFx, dSFy;
-        if (wb) { dSFx = qc * (Se + Sw); dSFy = qc * (Sn + Ss); }
-        else { dSFx = dt * c * uC.st * uC.Fx; dSFy = dt * c * uC.st * uC.Fy; }
-        const double dSE = cdt * uC.sa * uC.E;
-        const double nE  = uC.E  - fma(rdx, Ge0 - Gw0, fma(rdy, Hn0 - Hs0, dSE));
-        const double nFx = uC.Fx - fma(rdx, Ge1 - Gw1, fma(rdy, Hn1 - Hs1, dSFx));
-        const double nFy = uC.Fy - fma(rdx, Ge2 - Gw2, fma(rdy, Hn2 - Hs2, dSFy));
-        if (upd) { oE[row_off] = nE; oFx[row_off] = nFx; oFy[row_off] = nFy; }
-        row_off += (unsigned int)g.nx;
         uC = uN; qC = qN; uN = uNN;
         Hs0 = Hn0; Hs1 = Hn1; Hs2 = Hn2; Ss = Sn;
     }
-}
-
-cudaError_t launch_explicit_warp(const Grid& g, const Scheme& s, const Fields& f, double dt,
-                                 double* outE, double* outFx, double* outFy, int sm_count, cudaStream_t st)
-{
-    const int strips = (g.nx + WCOLS * WPB - 1) / (WCOLS * WPB);
-    long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
-    int RY = (int)(want < 4 ? 4 : (want > ARK_MARCH_RY ? ARK_MARCH_RY : want));
-    if (RY > g.ny) RY = g.ny;
-    dim3 grd(strips, (g.ny + RY - 1) / RY);
-    if (s.is_default()) explicit_warp_kernel<true><<<grd, 32 * WPB, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
-    else explicit_warp_kernel<false><<<grd, 32 * WPB, 0, st>>>(g, s, f, dt, RY, outE, outFx, outFy);
-    return cudaGetLastError();
 }
 
 cudaError_t launch_explicit_march(const Grid& g, const Scheme& s, const Fields& f, double dt,
                                   double* outE, double* outFx, double* outFy, double* outT, int sm_count, cudaStream_t st)
 {
     const int strips = (g.nx + (TX - 2) - 1) / (TX - 2);
-    // rows per block: enough blocks for ~8 per SM, between 4 and ARK_MARCH_RY rows.  (A single wave of
+    // rows per block: enough blocks for ~8 per SM, between 4 and MARCH_RY rows.  (A single wave of
     // SMs x resident-blocks blocks with ~240 rows each was measured 8% slower at 4096^2: uneven blocks per SM.)
     long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
-    int RY = (int)(want < 4 ? 4 : (want > ARK_MARCH_RY ? ARK_MARCH_RY : want));
+    int RY = (int)(want < 4 ? 4 : (want > MARCH_RY ? MARCH_RY : want));
     if (RY > g.ny) RY = g.ny;
+    if ((long long)g.nx * g.ny >= (1LL << 31) || (g.ny + RY - 1) / RY > 65535) return cudaErrorInvalidConfiguration;   // 32-bit in-plane offsets; gridDim.y
     dim3 grd(strips, (g.ny + RY - 1) / RY);
     const bool coupled = (f.T != nullptr) || (f.source_E != nullptr);
     if (coupled) {

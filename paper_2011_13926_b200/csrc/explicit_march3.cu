@@ -1,43 +1,31 @@
-// explicit_march3.cu — row-marching explicit kernel with a THREE-SLOT register rotation (explicit_kernel = 3).
+// explicit_march3.cu — row-marching explicit kernel with a FOUR-SLOT register rotation (explicit_kernel = 3, the default).
 //
 // Same arithmetic and organisation as explicit_march_kernel (column strips, rows marched, one closure per cell, one flux
-// per face, x-faces through shared memory).  The difference is purely in how the marching window is held:
-// explicit_march_kernel shifts (centre <- north <- prefetched) by register copies every row, which ptxas emits as ~45
-// IMAD.MOV per row — and IMAD issues at half rate on B200 (measured: 16 independent IMAD = 31 cycles per warp).  Here a
-// slot = {raw state, closure, north-face flux} and the three slots exchange ROLES instead of contents: the row body is a
-// forceinline function instantiated three times with permuted arguments, so no copy is ever made.
-//   row j   : centre = X, north = Y, prefetch target = Z   (south flux = Z.H, written one row ago when Z was the centre)
-//   row j+1 : centre = Y, north = Z, prefetch target = X
-//   row j+2 : centre = Z, north = X, prefetch target = Y
+// per face).  The differences are in how the marching window is held and in what a row step contains:
+//  * a slot = {raw state, closure, north-face flux}; the four slots exchange ROLES instead of contents (the row body is a
+//    forceinline function instantiated four times with permuted arguments), so no register copy is ever made
+//    (explicit_march_kernel shifts its window by ~45 IMAD.MOV per row);
+//      row j   : south = A (only its north flux is still alive), centre = B, north = C, closure target = D (row j+2)
+//      row j+1 : south = B, centre = C, north = D, target = A      ... and so on, period 4
+//  * the closure is computed one row further ahead than the faces need it, so that the closure chain of row j+2 and the
+//    face -> update chain of row j are independent inside one basic block (see row_step);
+//  * one warp per block: the x-face exchange is done with warp shuffles, there is no barrier at all.
 #include "explicit_device.cuh"
 
 namespace ark {
 
-// Block = ONE warp of 32 columns (30 updated + 1 halo lane each side), 16 blocks per SM (128 registers): measured fastest
-// (DESIGN.md section 6): no hardware barrier, no coupling between warps; 0.272 ms at 4096^2 against 0.284 (128 columns).
-#ifndef ARK_MARCH3_TX
-#define ARK_MARCH3_TX 32
-#endif
-#ifndef ARK_MARCH3_MINB
-#define ARK_MARCH3_MINB 16
-#endif
-#ifndef ARK_MARCH3_RY
-#define ARK_MARCH3_RY 33      // rows per block (cap; a multiple of 3)
-#endif
-#ifndef ARK_MARCH3_SHFL
-#define ARK_MARCH3_SHFL (ARK_MARCH3_TX == 32)      // one-warp blocks: the x-face exchange by warp shuffles instead of shared memory
-                                                  // (no synchronisation at all, the row step is one basic block): 0.2545 -> 0.2438 ms
-#endif
-static constexpr int TX3 = ARK_MARCH3_TX;
+// Block = ONE warp of 32 columns (30 updated + 1 halo lane each side): no hardware barrier, no coupling between warps
+// (0.272 ms at 4096^2 against 0.284 with 128 columns).  12 blocks per SM (150 registers) against 16
+// (128 registers): 0.2321 against 0.2357 ms with the four-slot window — the fp64 pipe, not the warp count, is the limit.
+static constexpr int TX3 = 32;          // threads = columns per block
+static constexpr int MARCH3_MINB = 12;   // resident blocks per SM asked of ptxas
+static constexpr int MARCH3_RY = 48;     // rows per block (cap; a multiple of 4)
 
 struct Slot {
     Raw u;                      // raw state of the cell
     CloF q;                     // closure (c^2 P, eigenvalues, |f|)
     double H0, H1, H2, S;       // flux through the NORTH face of the cell (E, Fx, Fy rows) and sigma_n (Fy_j + Fy_j+1)
 };
-
-// a one-warp block needs no hardware barrier for the shared-memory exchange
-__device__ __forceinline__ void block_sync() { if (TX3 == 32) __syncwarp(); else __syncthreads(); }
 
 struct March3Ctx {
     double c, cdt, dt, rdx, rdy, k3x, k3y, qc;
@@ -50,14 +38,20 @@ struct March3Ctx {
 };
 
 // The raw rows travel HBM -> shared memory with cp.async (LDGSTS), three rows ahead of their use, each thread into its own
-// slots of ring[row mod 3][field][thread]: the request holds no registers, so ptxas has no reason to sink it towards the
+// slots of ring[row mod 4][field][thread]: the request holds no registers, so ptxas has no reason to sink it towards the
 // use (with plain loads it did, and the exposed latency cost more than the copies saved).
-// FAST: row j+3 is known to be a grid row (0 <= j+3 < ny): five unconditional copies from the thread's base pointers.
+// FAST: row j+5 is known to be a grid row (0 <= j+5 < ny): five unconditional copies from the thread's base pointers.
+//
+// One row step = update of row j.  The closure is taken ONE ROW FURTHER AHEAD than the faces need it: the step computes the
+// closure of row j+2 (slot Q) while the north face (rows j, j+1), the east face and the update of row j use closures that
+// were finished in earlier steps.  The long closure chain (4 MUFU-seeded roots in sequence) and the face -> update chain are
+// then independent inside one basic block and overlap; with the closure of row j+1 computed in the same step (the three-slot
+// form) the step was one serial chain closure -> north face -> update per warp (DFMA dependent-issue latency on B200: 8.4
+// cycles, ark_m1_fp64_issue_rate).
 template <bool SD, bool FAST, bool COUPLED>
 __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const Fields& f, const March3Ctx& k,
-                                         Slot& C, Slot& N, Slot& P, int j, int j1, unsigned int row_off,
-                                         double (*ringN)[TX3], double (*ringC)[TX3],
-                                         XPub* pub, double (*flx)[TX3],
+                                         Slot& P, Slot& C, Slot& N, Slot& Q, int j, int j1, unsigned int row_off,
+                                         double (*ringQ)[TX3], double (*ringR)[TX3],
                                          double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy,
                                          double* __restrict__ oT)
 {
@@ -69,32 +63,26 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
         if (f.T) { Tm = f.T[row_off]; if (f.rho_cv) rcv = f.rho_cv[row_off]; }
         if (f.source_E) srcE = f.source_E[row_off];
     }
-    // request row j+3 into the ring slot of row j (read one row ago), then take row j+1 (third youngest group) out of the ring
+    // request row j+5 into the ring slot of row j+1 (read one step ago), then take row j+2 (fourth youngest group) out of the ring
     if (FAST) {
-        const unsigned int o = (unsigned int)(j + 3) * k.stride;
-        cp_async8(&ringC[0][k.t], k.bE + o); cp_async8(&ringC[1][k.t], k.bFx + o); cp_async8(&ringC[2][k.t], k.bFy + o);
-        cp_async8(&ringC[3][k.t], k.bst + o); cp_async8(&ringC[4][k.t], k.bsa + o);
+        const unsigned int o = (unsigned int)(j + 5) * k.stride;
+        cp_async8(&ringR[0][k.t], k.bE + o); cp_async8(&ringR[1][k.t], k.bFx + o); cp_async8(&ringR[2][k.t], k.bFy + o);
+        cp_async8(&ringR[3][k.t], k.bst + o); cp_async8(&ringR[4][k.t], k.bsa + o);
         cp_async_commit();
-    } else load_row_async<TX3>(ringC, k.t, f, g, k.xmode, k.ii, k.xside, j + 3, j + 2 < j1);
-    cp_async_wait<2>();
-    N.u.E = ringN[0][k.t]; N.u.Fx = ringN[1][k.t]; N.u.Fy = ringN[2][k.t]; N.u.st = ringN[3][k.t]; N.u.sa = ringN[4][k.t];
+    } else load_row_async<TX3>(ringR, k.t, f, g, k.xmode, k.ii, k.xside, j + 5, j + 5 <= j1);
+    cp_async_wait<3>();
+    Q.u.E = ringQ[0][k.t]; Q.u.Fx = ringQ[1][k.t]; Q.u.Fy = ringQ[2][k.t]; Q.u.st = ringQ[3][k.t]; Q.u.sa = ringQ[4][k.t];
     // publish the x-face data of the centre cell
     XPub me; me.E = C.u.E; me.Fx = C.u.Fx; me.Fy = C.u.Fy; me.Pxx = C.q.Pxx; me.Pxy = C.q.Pxy;
     me.lmin = C.q.lminx; me.lmax = C.q.lmaxx; me.f = C.q.f; me.st = C.u.st;
-#if ARK_MARCH3_SHFL
+    // ... to the west neighbour (lane t reads lane t+1) by warp shuffle: no shared memory, no synchronisation
     XPub R;
     R.E = __shfl_down_sync(0xffffffffu, me.E, 1); R.Fx = __shfl_down_sync(0xffffffffu, me.Fx, 1); R.Fy = __shfl_down_sync(0xffffffffu, me.Fy, 1);
     R.Pxx = __shfl_down_sync(0xffffffffu, me.Pxx, 1); R.Pxy = __shfl_down_sync(0xffffffffu, me.Pxy, 1);
     R.lmin = __shfl_down_sync(0xffffffffu, me.lmin, 1); R.lmax = __shfl_down_sync(0xffffffffu, me.lmax, 1);
     R.f = __shfl_down_sync(0xffffffffu, me.f, 1); R.st = __shfl_down_sync(0xffffffffu, me.st, 1);
-#else
-    pub[k.t] = me;
-    block_sync();
-    const XPub R = pub[k.t + 1];
-#endif
-    // closure of the north cell, north face, east face: one basic block, so that the scheduler can overlap the east-face chain
-    // (which depends only on data of row j) with the closure chain of row j+1 (0.2605 -> 0.2576 ms at 4096^2)
-    cell_closure<SD>(s, k.c, N.u, N.q);
+    // closure of row j+2, north face and east face of row j: one basic block of independent chains
+    cell_closure<SD>(s, k.c, Q.u, Q.q);
     FaceF fn;
     cell_face<SD>(s, k.c, g.dy, k.k3y, C.q.lminy, C.q.lmaxy, C.q.f, C.u.st, N.q.lminy, N.q.lmaxy, N.q.f, N.u.st, fn);
     ARK_FACE_FLUX(fn, C.u.E, N.u.E, C.u.Fy, N.u.Fy, C.u.Fx, N.u.Fx, C.q.Pyy, N.q.Pyy, C.q.Pxy, N.q.Pxy, C.H0, C.H2, C.H1, C.S);
@@ -104,17 +92,9 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
         cell_face<SD>(s, k.c, g.dx, k.k3x, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
         ARK_FACE_FLUX(fe, me.E, R.E, me.Fx, R.Fx, me.Fy, R.Fy, me.Pxx, R.Pxx, me.Pxy, R.Pxy, Ge0, Ge1, Ge2, Se);
     }
-#if ARK_MARCH3_SHFL
-    {
+    {   // the west flux is the east flux of lane t-1
         const double Gw0 = __shfl_up_sync(0xffffffffu, Ge0, 1), Gw1 = __shfl_up_sync(0xffffffffu, Ge1, 1);
         const double Gw2 = __shfl_up_sync(0xffffffffu, Ge2, 1), Sw = __shfl_up_sync(0xffffffffu, Se, 1);
-#else
-    flx[0][k.t] = Ge0; flx[1][k.t] = Ge1; flx[2][k.t] = Ge2; flx[3][k.t] = Se;
-    block_sync();
-    {
-        const int tw = (k.t > 0) ? k.t - 1 : 0;
-        const double Gw0 = flx[0][tw], Gw1 = flx[1][tw], Gw2 = flx[2][tw], Sw = flx[3][tw];
-#endif
         double dSFx, dSFy;   // -dt * S^F
         if (k.wb) { dSFx = k.qc * (Se + Sw); dSFy = k.qc * (C.S + P.S); }
         else { dSFx = k.dt * k.c * C.u.st * C.u.Fx; dSFy = k.dt * k.c * C.u.st * C.u.Fy; }
@@ -136,13 +116,11 @@ __device__ __forceinline__ void row_step(const Grid& g, const Scheme& s, const F
 }
 
 template <bool SD, bool COUPLED>
-__global__ void __launch_bounds__(TX3, ARK_MARCH3_MINB) explicit_march3_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
+__global__ void __launch_bounds__(TX3, MARCH3_MINB) explicit_march3_kernel(Grid g, Scheme s, Fields f, double dt, int RY,
                                                             double* __restrict__ oE, double* __restrict__ oFx, double* __restrict__ oFy,
                                                             double* __restrict__ oT)
 {
-    __shared__ XPub pub[TX3 + 1];
-    __shared__ double flx[4][TX3];
-    __shared__ double ring[3][5][TX3];     // raw rows in flight: row r lives in ring[r mod 3]
+    __shared__ double ring[4][5][TX3];     // raw rows in flight: row r lives in ring[r mod 4]
     March3Ctx k;
     k.t = threadIdx.x;
     const int i = blockIdx.x * (TX3 - 2) - 1 + k.t;
@@ -168,38 +146,43 @@ __global__ void __launch_bounds__(TX3, ARK_MARCH3_MINB) explicit_march3_kernel(G
     else if (k.xmode == 1) { k.bE = f.gh[k.xside][0]; k.bFx = f.gh[k.xside][1]; k.bFy = f.gh[k.xside][2]; k.bsa = f.gh[k.xside][3]; k.bst = f.gh[k.xside][4]; k.stride = 1u; }
     else { k.bE = f.E; k.bFx = f.Fx; k.bFy = f.Fy; k.bst = f.st; k.bsa = f.sa; k.stride = 0u; }
 
-    // prologue: Z = row j0-1 (its north flux = south flux of row j0), X = row j0, Y = raw of row j0+1
-    Slot X, Y, Z;
-    Z.u = load_row(f, g, k.xmode, k.ii, k.xside, j0 - 1);
-    X.u = load_row(f, g, k.xmode, k.ii, k.xside, j0);
-    load_row_async<TX3>(ring[(j0 + 1) % 3], k.t, f, g, k.xmode, k.ii, k.xside, j0 + 1, true);
-    load_row_async<TX3>(ring[(j0 + 2) % 3], k.t, f, g, k.xmode, k.ii, k.xside, j0 + 2, j0 + 1 < j1);
-    cell_closure<SD>(s, k.c, Z.u, Z.q);
-    cell_closure<SD>(s, k.c, X.u, X.q);
+    // prologue: A = row j0-1 (only its north flux = south flux of row j0 is kept), B = row j0, C = row j0+1 with closures;
+    // rows j0+2 .. j0+4 requested into the ring
+    Slot A, B, C, D;
+    A.u = load_row(f, g, k.xmode, k.ii, k.xside, j0 - 1);
+    B.u = load_row(f, g, k.xmode, k.ii, k.xside, j0);
+    C.u = load_row(f, g, k.xmode, k.ii, k.xside, j0 + 1);
+    load_row_async<TX3>(ring[(j0 + 2) % 4], k.t, f, g, k.xmode, k.ii, k.xside, j0 + 2, j0 + 2 <= j1);
+    load_row_async<TX3>(ring[(j0 + 3) % 4], k.t, f, g, k.xmode, k.ii, k.xside, j0 + 3, j0 + 3 <= j1);
+    load_row_async<TX3>(ring[(j0 + 4) % 4], k.t, f, g, k.xmode, k.ii, k.xside, j0 + 4, j0 + 4 <= j1);
+    cell_closure<SD>(s, k.c, A.u, A.q);
+    cell_closure<SD>(s, k.c, B.u, B.q);
+    cell_closure<SD>(s, k.c, C.u, C.q);
     {
         FaceF fs;
-        cell_face<SD>(s, k.c, g.dy, k.k3y, Z.q.lminy, Z.q.lmaxy, Z.q.f, Z.u.st, X.q.lminy, X.q.lmaxy, X.q.f, X.u.st, fs);
-        ARK_FACE_FLUX(fs, Z.u.E, X.u.E, Z.u.Fy, X.u.Fy, Z.u.Fx, X.u.Fx, Z.q.Pyy, X.q.Pyy, Z.q.Pxy, X.q.Pxy, Z.H0, Z.H2, Z.H1, Z.S);
+        cell_face<SD>(s, k.c, g.dy, k.k3y, A.q.lminy, A.q.lmaxy, A.q.f, A.u.st, B.q.lminy, B.q.lmaxy, B.q.f, B.u.st, fs);
+        ARK_FACE_FLUX(fs, A.u.E, B.u.E, A.u.Fy, B.u.Fy, A.u.Fx, B.u.Fx, A.q.Pyy, B.q.Pyy, A.q.Pxy, B.q.Pxy, A.H0, A.H2, A.H1, A.S);
     }
     unsigned int row_off = (unsigned int)j0 * (unsigned int)g.nx + (unsigned int)(i < 0 ? 0 : i);
     const unsigned int nxu = (unsigned int)g.nx;
 
     int j = j0;
-    // hot loop: three rows per trip, every requested row (j+3 .. j+5) inside the grid.  RY is a multiple of 3 (launcher), so
-    // j mod 3 == 0 at every trip and the ring slots are compile-time constants.
-    const int jfast = min(j1, g.ny - 3);
-    if (j0 % 3 == 0) {
-        for (; j + 2 < jfast; j += 3) {
-            row_step<SD, true, COUPLED>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[1], ring[0], pub, flx, oE, oFx, oFy, oT);
-            row_step<SD, true, COUPLED>(g, s, f, k, Y, Z, X, j + 1, j1, row_off + nxu, ring[2], ring[1], pub, flx, oE, oFx, oFy, oT);
-            row_step<SD, true, COUPLED>(g, s, f, k, Z, X, Y, j + 2, j1, row_off + 2 * nxu, ring[0], ring[2], pub, flx, oE, oFx, oFy, oT);
-            row_off += 3 * nxu;
+    // hot loop: four rows per trip, every requested row (j+5 .. j+8) inside the grid.  RY is a multiple of 4 (launcher), so
+    // j mod 4 == 0 at every trip and the ring slots are compile-time constants; the four slots exchange roles, not contents.
+    const int jfast = min(j1, g.ny - 5);
+    if (j0 % 4 == 0) {
+        for (; j + 3 < jfast; j += 4) {
+            row_step<SD, true, COUPLED>(g, s, f, k, A, B, C, D, j,     j1, row_off,           ring[2], ring[1], oE, oFx, oFy, oT);
+            row_step<SD, true, COUPLED>(g, s, f, k, B, C, D, A, j + 1, j1, row_off + nxu,     ring[3], ring[2], oE, oFx, oFy, oT);
+            row_step<SD, true, COUPLED>(g, s, f, k, C, D, A, B, j + 2, j1, row_off + 2 * nxu, ring[0], ring[3], oE, oFx, oFy, oT);
+            row_step<SD, true, COUPLED>(g, s, f, k, D, A, B, C, j + 3, j1, row_off + 3 * nxu, ring[1], ring[0], oE, oFx, oFy, oT);
+            row_off += 4 * nxu;
         }
     }
     // remaining rows (block-uniform trip count): general loader, the window is shifted by copies
     for (; j < j1; ++j) {
-        row_step<SD, false, COUPLED>(g, s, f, k, X, Y, Z, j, j1, row_off, ring[(j + 1) % 3], ring[j % 3], pub, flx, oE, oFx, oFy, oT);
-        const Slot T = X; X = Y; Y = Z; Z = T;
+        row_step<SD, false, COUPLED>(g, s, f, k, A, B, C, D, j, j1, row_off, ring[(j + 2) % 4], ring[(j + 1) % 4], oE, oFx, oFy, oT);
+        const Slot T = A; A = B; B = C; C = D; D = T;
         row_off += nxu;
     }
 }
@@ -209,9 +192,10 @@ cudaError_t launch_explicit_march3(const Grid& g, const Scheme& s, const Fields&
 {
     const int strips = (g.nx + (TX3 - 2) - 1) / (TX3 - 2);
     long long want = ((long long)g.ny * strips + (long long)sm_count * 8 - 1) / ((long long)sm_count * 8);
-    int RY = (int)(want < 3 ? 3 : (want > ARK_MARCH3_RY ? ARK_MARCH3_RY : want));   // multiples of three rows avoid the remainder path
-    RY = (RY + 2) / 3 * 3;
+    int RY = (int)(want < 4 ? 4 : (want > MARCH3_RY ? MARCH3_RY : want));   // multiples of four rows avoid the remainder path
+    RY = (RY + 3) / 4 * 4;
     if (RY > g.ny) RY = g.ny;
+    if ((long long)g.nx * g.ny >= (1LL << 31) || (g.ny + RY - 1) / RY > 65535) return cudaErrorInvalidConfiguration;   // 32-bit in-plane offsets; gridDim.y
     dim3 grd(strips, (g.ny + RY - 1) / RY);
     const bool coupled = (f.T != nullptr) || (f.source_E != nullptr);
     if (coupled) {

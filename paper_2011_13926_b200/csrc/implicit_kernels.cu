@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(256) diag_mul_kernel(long long N, const double
 cudaError_t launch_diag_mul(const Grid& g, const double* Cblk, const double* x, double* t, cudaStream_t st)
 {
     const long long N = (long long)g.nx * g.ny;
-    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < 148 * 8 ? (N + blk - 1) / blk : 148 * 8);
+    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < current_sm_count() * 8 ? (N + blk - 1) / blk : current_sm_count() * 8);
     diag_mul_kernel<<<grd, blk, 0, st>>>(N, Cblk, x, t);
     return cudaGetLastError();
 }
@@ -285,7 +285,7 @@ cudaError_t launch_matter_update(const Grid& g, const Scheme& s, double dt, cons
                                  const double* Enew, double* T, cudaStream_t st)
 {
     const long long N = (long long)g.nx * g.ny;
-    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < 148 * 8 ? (N + blk - 1) / blk : 148 * 8);
+    const int blk = 256; const int grd = (int)((N + blk - 1) / blk < current_sm_count() * 8 ? (N + blk - 1) / blk : current_sm_count() * 8);
     matter_update_kernel<<<grd, blk, 0, st>>>(N, g.c, s.a_r, dt, sa, rho_cv, Enew, T);
     return cudaGetLastError();
 }

@@ -324,17 +324,17 @@ __global__ void __launch_bounds__(KTHREADS) combine_y_kernel(long long N, const 
 
 cudaError_t launch_bicg_begin(double* r, double* rhat, double* p, double* v, long long n, GmresWork W, cudaStream_t st)
 {
-    bicg_begin_kernel<<<148 * 4, KTHREADS, 0, st>>>(r, rhat, p, v, n, W);
+    bicg_begin_kernel<<<current_sm_count() * 4, KTHREADS, 0, st>>>(r, rhat, p, v, n, W);
     return cudaGetLastError();
 }
 cudaError_t launch_bicg_p(const double* r, double* p, const double* v, long long n, GmresWork W, cudaStream_t st)
 {
-    bicg_p_kernel<<<148 * 4, KTHREADS, 0, st>>>(r, p, v, n, W);
+    bicg_p_kernel<<<current_sm_count() * 4, KTHREADS, 0, st>>>(r, p, v, n, W);
     return cudaGetLastError();
 }
 cudaError_t launch_bicg_s(double* r, const double* v, long long n, GmresWork W, cudaStream_t st)
 {
-    bicg_s_kernel<<<148 * 4, KTHREADS, 0, st>>>(r, v, n, W);
+    bicg_s_kernel<<<current_sm_count() * 4, KTHREADS, 0, st>>>(r, v, n, W);
     return cudaGetLastError();
 }
 cudaError_t launch_bicg_xr(double* y, const double* p, double* r, const double* t, const double* rhat, long long n,
@@ -347,11 +347,12 @@ cudaError_t launch_combine_y(const Grid& g, const double* Minv, double* y, doubl
 {
     const long long N = (long long)g.nx * g.ny;
     const long long need = (N + KTHREADS - 1) / KTHREADS;
-    combine_y_kernel<<<(int)(need < 148 * 8 ? need : 148 * 8), KTHREADS, 0, st>>>(N, Minv, y, x);
+    combine_y_kernel<<<(int)(need < current_sm_count() * 8 ? need : current_sm_count() * 8), KTHREADS, 0, st>>>(N, Minv, y, x);
     return cudaGetLastError();
 }
 
-__global__ void sub_kernel(double* __restrict__ o, const double* __restrict__ a, const double* __restrict__ b, long long n)
+// o may alias a or b (the Newton loop subtracts in place): no __restrict__
+__global__ void sub_kernel(double* o, const double* a, const double* b, long long n)
 {
     for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) o[k] = a[k] - b[k];
 }
@@ -359,7 +360,7 @@ __global__ void sub_kernel(double* __restrict__ o, const double* __restrict__ a,
 cudaError_t launch_sub(double* out, const double* a, const double* b, long long n, cudaStream_t st)
 {
     const long long need = (n + 255) / 256;
-    sub_kernel<<<(int)(need < 148 * 8 ? need : 148 * 8), 256, 0, st>>>(out, a, b, n);
+    sub_kernel<<<(int)(need < current_sm_count() * 8 ? need : current_sm_count() * 8), 256, 0, st>>>(out, a, b, n);
     return cudaGetLastError();
 }
 

@@ -378,7 +378,7 @@ __global__ void mg_to_float_kernel(const double* __restrict__ a, float* __restri
 cudaError_t launch_mg_to_float(const double* a, float* b, long long n, cudaStream_t st)
 {
     const long long need = (n + 255) / 256;
-    mg_to_float_kernel<<<(int)(need < 148 * 16 ? need : 148 * 16), 256, 0, st>>>(a, b, n);
+    mg_to_float_kernel<<<(int)(need < current_sm_count() * 16 ? need : current_sm_count() * 16), 256, 0, st>>>(a, b, n);
     return cudaGetLastError();
 }
 

@@ -36,6 +36,33 @@ def state_rel_l2(got, want):
     return max(rel_l2(a, b) for a, b in zip(got, want) if a is not None and b is not None)
 
 
+def max_abs_scaled(a, b):
+    """max |a - b| / max |b|: the element-wise bound beside the L2 norm (a single bad boundary cell vanishes in a 16 M-element norm)."""
+    a, b = np.asarray(a), np.asarray(b)
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)) if a.size else 0.0
+
+
+def state_max_abs(got, want):
+    """max over the fields (E, F[, T]) of the scaled element-wise difference."""
+    return max(max_abs_scaled(a, b) for a, b in zip(got, want) if a is not None and b is not None)
+
+
+def assert_parity(got, want, tol):
+    """Parity bar of the GPU tests: relative L2 <= tol per field (north_star) AND every element within tol * max|field|."""
+    l2, mx = state_rel_l2(got, want), state_max_abs(got, want)
+    assert l2 <= tol and mx <= tol, f"relative L2 {l2:.2e}, scaled max-abs {mx:.2e} (tol {tol:.0e})"
+
+
+# BiCGStab is not a minimal-residual method: its residual history is erratic and the iteration at which it crosses the
+# tolerance moves with the rounding order of the dot products (79 against 93 iterations seen for one system after a recompile).
+# The parity criterion is the state (<= 1e-8); the count band is a sanity check, one value everywhere (DESIGN.md R12).
+BICGSTAB_COUNT_TOL = 0.25
+
+
+def bicgstab_count_ok(ig, io):
+    return abs(ig - io) <= max(3, BICGSTAB_COUNT_TOL * io)
+
+
 def rel_l2(a, b):
     a, b = np.asarray(a), np.asarray(b)
     return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 import m1_workloads as wl
-from helpers import make_oracle, make_gpu, small_random_state, rel_l2, state_rel_l2
+from helpers import make_oracle, make_gpu, small_random_state, rel_l2, state_rel_l2, assert_parity
 
 pytestmark = pytest.mark.gpu
 
@@ -18,7 +18,7 @@ def _dt(w):
     return wl.explicit_dt(w["dx"], w["dy"], w["c"])
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
+@pytest.mark.parametrize("kernel", [0, 1, 3])
 @pytest.mark.parametrize("bc", BCS)
 def test_explicit_step_small_all_boundaries(bc, kernel):
     # 37 x 29: ragged in both directions, dx != dy, c != 1
@@ -28,10 +28,10 @@ def test_explicit_step_small_all_boundaries(bc, kernel):
     for _ in range(3):
         o.step_explicit(dt)
         g.step_explicit(dt)
-    assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+    assert_parity(g.get_state(), o.get_state(), TOL_EXPLICIT)
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
+@pytest.mark.parametrize("kernel", [0, 1, 3])
 @pytest.mark.parametrize("shape", [(300, 70), (127, 5), (126, 64), (1, 40), (40, 1), (2, 2), (253, 131)])
 def test_explicit_step_ragged_shapes(shape, kernel):
     # several 126-column strips plus a ragged tail; degenerate one-cell-wide grids
@@ -42,13 +42,13 @@ def test_explicit_step_ragged_shapes(shape, kernel):
     for _ in range(2):
         o.step_explicit(dt)
         g.step_explicit(dt)
-    assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+    assert_parity(g.get_state(), o.get_state(), TOL_EXPLICIT)
 
 
 @pytest.mark.parametrize("kernel", [1, 3])
 @pytest.mark.parametrize("bc", [(1, 2, 2, 1), (2, 1, 1, 2), (0, 0, 1, 1)])
 def test_explicit_step_midsize_long_blocks(bc, kernel):
-    # 701 x 1003: blocks of 21 rows (kernel 3: seven trips of the three-row rotation loop, the last block with a ragged tail of
+    # 701 x 1003: blocks of 48 rows (kernel 3: twelve trips of the four-row rotation loop, the last block with a ragged tail of
     # rows handled by the general loader), 24 strips of 30 columns with a ragged last strip, Dirichlet and outflow ghost columns
     # in the branch-free hot loop, y-ghost rows in the prologue and in the tail
     w = small_random_state(701, 1003, seed=77, dx=0.011, dy=0.009, c=1.1, bc=bc, sig_range=(-2.0, 2.0))
@@ -57,7 +57,7 @@ def test_explicit_step_midsize_long_blocks(bc, kernel):
     for _ in range(2):
         o.step_explicit(dt)
         g.step_explicit(dt)
-    assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+    assert_parity(g.get_state(), o.get_state(), TOL_EXPLICIT)
 
 
 def test_residual_matches_oracle():
@@ -82,23 +82,23 @@ def test_clamped_and_degenerate_cells():
     o, g = make_oracle(w), make_gpu(w)
     assert o.count_unrealizable() == g.count_unrealizable()
     assert o.count_unrealizable()[1] > 0
-    for kernel in (0, 1, 2, 3):
+    for kernel in (0, 1, 3):
         o, g = make_oracle(w), make_gpu(w, dict(explicit_kernel=kernel))
         o.step_explicit(1e-3)
         g.step_explicit(1e-3)
-        assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+        assert_parity(g.get_state(), o.get_state(), TOL_EXPLICIT)
 
 
 @pytest.mark.parametrize("opts", [dict(well_balanced=0), dict(ap_mode=0), dict(ap_mode=2), dict(eig_mode=1), dict(eig_mode=2),
                                   dict(closure=1), dict(eig_floor=0.1)])
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
+@pytest.mark.parametrize("kernel", [0, 1, 3])
 def test_scheme_switches(opts, kernel):
     w = small_random_state(45, 31, seed=13, bc=(1, 1, 0, 0), sig_range=(-1.0, 1.0))
     o, g = make_oracle(w, opts), make_gpu(w, dict(opts, explicit_kernel=kernel))
     dt = _dt(w)
     o.step_explicit(dt)
     g.step_explicit(dt)
-    assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+    assert_parity(g.get_state(), o.get_state(), TOL_EXPLICIT)
 
 
 def test_config2_opacity_jump_stays_steady():
@@ -118,7 +118,7 @@ def test_config2_opacity_jump_stays_steady():
         o.step_explicit(dt)
     g.steps_explicit(dt, 50)
     Eg, Fg = g.get_state()
-    assert state_rel_l2((Eg, Fg), o.get_state()) <= TOL_EXPLICIT
+    assert_parity((Eg, Fg), o.get_state(), TOL_EXPLICIT)
     drift = max(np.max(np.abs(Eg - w["E"])) / np.max(np.abs(w["E"])), np.max(np.abs(Fg[0] - w["F"][0])) / w["F0"])
     assert drift < 1e-9
 
@@ -130,7 +130,7 @@ def test_config3_random_medium_1024():
     dt = _dt(w)
     o.step_explicit(dt)
     g.step_explicit(dt)
-    assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+    assert_parity(g.get_state(), o.get_state(), TOL_EXPLICIT)
 
 
 def test_conservation_periodic():
@@ -185,13 +185,13 @@ def test_nonpositive_energy_cells_do_not_poison_the_step():
     w = small_random_state(40, 28, seed=19)
     w["E"][7, 9] = -0.3
     w["E"][20, 3] = 0.0
-    for kernel in (0, 1, 2, 3):
+    for kernel in (0, 1, 3):
         o, g = make_oracle(w), make_gpu(w, dict(explicit_kernel=kernel))
         o.step_explicit(1e-3)
         g.step_explicit(1e-3)
         Eg, Fg = g.get_state()
         assert np.all(np.isfinite(Eg)) and np.all(np.isfinite(Fg))
-        assert state_rel_l2((Eg, Fg), o.get_state()) <= TOL_EXPLICIT
+        assert_parity((Eg, Fg), o.get_state(), TOL_EXPLICIT)
     o, g = make_oracle(w), make_gpu(w)
     V = np.random.default_rng(2).standard_normal((3, 28, 40))
     assert rel_l2(g.apply_operator(0.02, V), o.apply_linear(0.02, V)) <= 1e-12
@@ -211,7 +211,7 @@ def test_beam_test_of_the_paper():
         for _ in range(300):
             o.step_explicit(dt)
         g.steps_explicit(dt, 300)
-        assert state_rel_l2(g.get_state(), o.get_state()) <= TOL_EXPLICIT
+        assert_parity(g.get_state(), o.get_state(), TOL_EXPLICIT)
     width = {}
     for eig in (0, 1):
         g = make_gpu(w, dict(eig_mode=eig))

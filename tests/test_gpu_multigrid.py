@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 import m1_workloads as wl
-from helpers import make_oracle, make_gpu, small_random_state, rel_l2, state_rel_l2
+from helpers import make_oracle, make_gpu, small_random_state, rel_l2, state_rel_l2, bicgstab_count_ok
 
 pytestmark = pytest.mark.gpu
 BCS = [(0, 0, 0, 0), (1, 1, 0, 0), (1, 2, 2, 1), (2, 2, 1, 1)]
@@ -63,8 +63,7 @@ def test_multigrid_solve_matches_oracle(bc, krylov):
     ig, rg = g.step_implicit(dt, 1e-10, 30, 1000)
     assert ro <= 1e-10 and rg <= 1e-10
     assert state_rel_l2(g.get_state(), o.get_state()) <= 1e-8
-    # BiCGStab counts move with the last bit of the assembled blocks (79 against 93 seen after a recompile): 25 %
-    assert abs(ig - io) <= (2 if krylov == 0 else max(3, 0.25 * io))
+    assert abs(ig - io) <= 2 if krylov == 0 else bicgstab_count_ok(ig, io)
 
 
 def test_multigrid_solve_equals_dense_direct_solve():
@@ -161,12 +160,12 @@ def test_single_precision_multigrid_solve_meets_the_fp64_tolerance(krylov):
     ig, rg = g.step_implicit(dt, 1e-10, 30, 1000)
     assert ro <= 1e-10 and rg <= 1e-10
     assert state_rel_l2(g.get_state(), o.get_state()) <= 1e-8
-    assert abs(ig - io) <= max(3, 0.15 * io)
+    assert bicgstab_count_ok(ig, io)
     # switching back to fp64 blocks on the same handle
     g.set_option("mg_precision", 64)
     g.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
     ig2, rg2 = g.step_implicit(dt, 1e-10, 30, 1000)
-    assert rg2 <= 1e-10 and abs(ig2 - io) <= max(3, 0.15 * io)
+    assert rg2 <= 1e-10 and bicgstab_count_ok(ig2, io)
 
 
 def test_marshak_wave_with_multigrid():
@@ -203,7 +202,7 @@ def test_device_bytes_accounting_with_the_hierarchy():
     b2 = g.device_bytes()
     N = 64 * 48
     assert b1 > b0 and b2 - b1 >= (45 + 3) * 8 * N + 36 * 4 * N      # block stencil + V-cycle vector + fp32 copy at least
-    g.set_option("basis_pad", 32)                                     # releases the implicit workspace
+    g.set_option("release_workspace", 1)                              # releases the implicit workspace
     assert g.device_bytes() == b0
     its, res = g.step_implicit(_dt(w, 20.0), 1e-10, 30, 500)          # and it comes back
     assert res <= 1e-10 and b0 < g.device_bytes() < b2            # this time without the matrix-free planes of the first solve
