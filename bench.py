@@ -45,6 +45,7 @@ TOL, RESTART, MAXIT = 1e-10, 30, 4000
 BENCH_DT_RATIO = 10.0
 SWEEP = (10.0, 50.0, 100.0, 200.0)
 PAPER_BREAK_EVEN = "50-100x (relaxation preconditioner; CPU 50, K80 GPU 100; PAPER.md:369)"
+FP64_INSTR_PER_CELL = 157       # fp64-pipe instructions (DFMA/DMUL/DADD/DSETP) per cell in the row loop of explicit_march3_kernel (SASS count)
 
 
 def load_ncu_traffic():
@@ -127,23 +128,77 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------------------------
 # reference arm / cpu baseline: the oracle on a bounded sample
 # --------------------------------------------------------------------------------------------------------------
-def oracle_step_time(n_sample, seed, steps, warmup):
-    """Times `steps` passes (explicit step + implicit 10x step from the same state) of the oracle at n_sample^2."""
+def oracle_set_threads(nthreads):
+    """Set the OpenMP team size of the oracle's next parallel regions (libgomp runtime call; None = leave as is)."""
+    if nthreads is None:
+        return
+    import ctypes
+    ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(nthreads))
+
+
+def oracle_step_time(n_sample, seed, steps, warmup, threads=None):
+    """Times `steps` passes (explicit step + implicit 10x step from the same state) of the oracle at n_sample^2; the explicit and
+    the implicit part are also timed separately."""
     from oracle.oracle_m1 import OracleM1, num_threads
+    all_cores = num_threads()
+    oracle_set_threads(threads)
     w = wl.random_medium(n_sample, seed=seed)
     dt = wl.explicit_dt(w["dx"], w["dy"], w["c"])
     o = OracleM1(w["nx"], w["ny"], w["dx"], w["dy"], w["c"], bc=w["bc"])
-    times, its = [], 0
+    times, t_exp, t_imp, its = [], [], [], 0
     for k in range(warmup + steps):
         o.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
         t0 = time.perf_counter()
         o.step_explicit(dt)
-        its, _ = o.step_implicit(BENCH_DT_RATIO * dt, TOL, RESTART, MAXIT)
         t1 = time.perf_counter()
+        its, _ = o.step_implicit(BENCH_DT_RATIO * dt, TOL, RESTART, MAXIT)
+        t2 = time.perf_counter()
         if k >= warmup:
-            times.append(t1 - t0)
+            times.append(t2 - t0); t_exp.append(t1 - t0); t_imp.append(t2 - t1)
     total = float(sum(times))
-    return dict(seconds=total, per_step=total / max(steps, 1), cells=n_sample * n_sample, iterations=its, cores=num_threads())
+    out = dict(seconds=total, per_step=total / max(steps, 1), cells=n_sample * n_sample, iterations=its,
+               cores=(threads if threads is not None else all_cores), explicit_s=float(sum(t_exp)) / max(steps, 1),
+               implicit_s=float(sum(t_imp)) / max(steps, 1))
+    oracle_set_threads(all_cores if threads is not None else None)
+    return out
+
+
+def oracle_protocol(n, seed):
+    """The oracle timings SURVEY.md 8(d) lists, at the bench size: explicit alone (3 steps) and one capped GMRES cycle
+    (maxit = restart = 30 -> seconds per iteration), with all cores and with 1 thread; full solves at 1024^2, dt = 50x
+    (config 3).  Takes minutes; opt-in (--oracle-protocol)."""
+    from oracle.oracle_m1 import OracleM1, num_threads
+    all_cores = num_threads()
+    out = {"grid": n, "all_cores": all_cores}
+    w = wl.random_medium(n, seed=seed)
+    dt = wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    N = n * n
+    for label, th in (("all_cores", all_cores), ("one_thread", 1)):
+        oracle_set_threads(th)
+        o = OracleM1(w["nx"], w["ny"], w["dx"], w["dy"], w["c"], bc=w["bc"])
+        o.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
+        nst = 3 if th > 1 else 1
+        t0 = time.perf_counter()
+        for _ in range(nst):
+            o.step_explicit(dt)
+        te = (time.perf_counter() - t0) / nst
+        o.set_state(w["E"], w["F"], w["sigma_a"], w["sigma_s"])
+        t0 = time.perf_counter()
+        its, res = o.step_implicit(BENCH_DT_RATIO * dt, TOL, RESTART, RESTART)       # one capped cycle
+        ti = time.perf_counter() - t0
+        out[label] = {"threads": th, "explicit_steps_timed": nst, "explicit_s_per_step": te, "explicit_cell_updates_per_s": N / te,
+                      "implicit_capped_cycle_s": ti, "implicit_iterations": its, "implicit_s_per_iteration": ti / max(its, 1),
+                      "implicit_extrapolated_s_per_solve_85_iterations": 85 * ti / max(its, 1)}
+        del o
+    oracle_set_threads(all_cores)
+    w3 = wl.random_medium(1024, seed=seed)
+    dt3 = wl.explicit_dt(w3["dx"], w3["dy"], w3["c"])
+    o = OracleM1(w3["nx"], w3["ny"], w3["dx"], w3["dy"], w3["c"], bc=w3["bc"])
+    o.set_state(w3["E"], w3["F"], w3["sigma_a"], w3["sigma_s"])
+    t0 = time.perf_counter()
+    its, res = o.step_implicit(50.0 * dt3, TOL, RESTART, MAXIT)
+    out["config3_1024_dt50"] = {"threads": all_cores, "iterations": its, "final_residual": res, "s_per_solve": time.perf_counter() - t0}
+    return out
 
 
 def run_reference(args):
@@ -264,7 +319,10 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- explicit kernel alone, first (a kernel timed in isolation: burst clocks), with its own clock record ----------
+    # ---- explicit kernel alone, first: BURST (best of 5 x >= 40 back-to-back steps, ~10 ms each, boost clock) and SUSTAINED
+    #      (one back-to-back run of >= 2 s, the regime of the paper's explicit route: 73 823 consecutive steps),
+    #      each with its own clock record.  The kernel is fp64-issue bound, so its time follows the SM clock.
+    rates = ark.fp64_issue_rate()      # measured fp64 issue rate of this GPU (the "alu" roofline below)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     reset_device()
     g.steps_explicit(dt_e, 10)
@@ -273,19 +331,41 @@ def run_ours(args):
     smp = ClockSampler(local)
     smp.start()
     time.sleep(0.3)
-    best = None
+    best, all_ms = None, []
     for _ in range(5):
         e0.record(stream)
         g.steps_explicit(dt_e, n_exp)
         e1.record(stream)
         torch.cuda.synchronize()
         t_ms = e0.elapsed_time(e1) / n_exp
+        all_ms.append(t_ms)
         best = t_ms if best is None else min(best, t_ms)
     exp_clocks = smp.stop()
+    n_sus = int(max(200, args.sustain_s * 1e3 / best))
+    smp = ClockSampler(local)
+    smp.start()
+    e0.record(stream)
+    g.steps_explicit(dt_e, n_sus)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    sus_ms = e0.elapsed_time(e1) / n_sus
+    sus_clocks = smp.stop()
     exp_gbs = 64.0 * N / (best * 1e-3) / 1e9
-    explicit_info = {"cell_updates_per_s": N / (best * 1e-3), "ms_per_step": best, "steps_timed": n_exp, "repeats": 5, "bytes_per_cell": 64,
-                     "achieved_gbs": exp_gbs, "hbm_frac": exp_gbs / peak_gbs, "clocks": exp_clocks,
-                     "bound": "fp64 issue (DESIGN.md section 6): the kernel needs ~170 fp64 + ~110 other instructions per cell"}
+    sus_gbs = 64.0 * N / (sus_ms * 1e-3) / 1e9
+    alu_peak = rates["dfma_lanes_per_clk_sm"] * rates["sm_count"] * rates["sm_mhz"] * 1e6       # fp64 lane-instructions per second
+    alu_work = FP64_INSTR_PER_CELL * (32.0 / 30.0) * N                                           # halo lanes compute too
+    explicit_info = {"cell_updates_per_s": N / (sus_ms * 1e-3), "ms_per_step": sus_ms, "bytes_per_cell": 64,
+                     "achieved_gbs": sus_gbs, "hbm_frac": sus_gbs / peak_gbs,
+                     "sustained": {"ms_per_step": sus_ms, "steps_timed": n_sus, "hbm_frac": sus_gbs / peak_gbs, "clocks": sus_clocks},
+                     "burst": {"ms_per_step": best, "median_ms_per_step": float(np.median(all_ms)), "steps_timed": n_exp, "repeats": 5,
+                               "cell_updates_per_s": N / (best * 1e-3), "hbm_frac": exp_gbs / peak_gbs, "clocks": exp_clocks},
+                     "alu": {"bound": "alu", "pipe": "fp64", "unit": "fp64 lane-instructions/s",
+                             "fp64_instr_per_cell": FP64_INSTR_PER_CELL, "lanes_factor": 32.0 / 30.0,
+                             "peak": alu_peak, "achieved_sustained": alu_work / (sus_ms * 1e-3), "achieved_burst": alu_work / (best * 1e-3),
+                             "frac_sustained": alu_work / (sus_ms * 1e-3) / alu_peak, "frac_burst": alu_work / (best * 1e-3) / alu_peak,
+                             "peak_source": "ark_m1_fp64_issue_rate on this GPU in this run: DFMA lanes/clk/SM x SMs x SM clock measured during the test",
+                             "issue_rates": rates},
+                     "bound": "fp64 issue (DESIGN.md section 6): 157 fp64 + 110 other instructions per cell"}
 
     # ---- main timed region: W warm-up + exactly K steps, inputs resident in HBM ----------------------------------
     for _ in range(args.warmup):
@@ -329,15 +409,11 @@ def run_ours(args):
     line_extra = {}
     if rank == 0:
         line_extra["explicit"] = explicit_info
-        ms_exp = explicit_info["ms_per_step"]
+        ms_exp = explicit_info["ms_per_step"]          # SUSTAINED explicit step: the denominator of every break-even statement
         traffic = load_ncu_traffic()
-        if n == 4096:
-            _te = traffic.get("explicit", {})
-            if "fp64_pipe_busy_frac" in _te:   # the kernel is ALU bound: fp64 pipe occupancy from the committed ncu capture
-                explicit_info["alu"] = {"bound": "alu", "pipe": "fp64", "frac": _te["fp64_pipe_busy_frac"],
-                                        "issue_slots_frac": _te.get("issue_slots_busy_frac"),
-                                        "peak": "148 SMs x 64 fp64 lanes/clk x SM clock (DESIGN.md section 6)", "source": _te.get("alu_note")}
-                explicit_info["traffic"] = _te.get("dram_bytes")
+        if n == 4096 and "explicit" in traffic:
+            explicit_info["traffic"] = traffic["explicit"]["dram_bytes"]
+            explicit_info["alu"]["ncu_fp64_pipe_busy_frac"] = traffic["explicit"].get("fp64_pipe_busy_frac")
         # ---- implicit sweep ----------------------------------------------------------------------------------------
         imp, brk = {}, {}
         ratios = SWEEP if not args.no_sweep else (BENCH_DT_RATIO,)
@@ -363,6 +439,31 @@ def run_ours(args):
         wins = [k for k, v in brk.items() if v["implicit_wins"]]
         line_extra["break_even"] = {"per_ratio": brk, "reached_in_sweep": bool(wins), "first_winning_ratio": wins[0] if wins else None,
                                     "paper": PAPER_BREAK_EVEN}
+        # ---- restart length (the one free parameter north_star leaves the solver; SURVEY 8(f) row 4 "longer restart") ------------
+        if args.restart_sweep:
+            rsw = {}
+            for ngrid in (1024, n):
+                wr = w if ngrid == n else wl.random_medium(ngrid, seed=args.seed)
+                dtr = wl.explicit_dt(wr["dx"], wr["dy"], wr["c"])
+                tr_ = devt if ngrid == n else {k: torch.from_numpy(np.ascontiguousarray(wr[k])).to(dev) for k in ("E", "F", "sigma_a", "sigma_s")}
+                gr = g if ngrid == n else ark.ArkM1(ngrid, ngrid, wr["dx"], wr["dy"], wr["c"], bc=wr["bc"], stream=stream)
+                tab = {}
+                for m_ in (30, 60, 100):
+                    for ratio in (50.0, 100.0, 200.0):
+                        gr.set_state(tr_["E"], tr_["F"], tr_["sigma_a"], tr_["sigma_s"])
+                        torch.cuda.synchronize()
+                        e0.record(stream)
+                        its, res = gr.step_implicit(ratio * dtr, TOL, m_, MAXIT)
+                        e1.record(stream)
+                        torch.cuda.synchronize()
+                        tab[f"m{m_}_{ratio:g}x"] = {"restart": m_, "dt_ratio": ratio, "iterations": its, "final_residual": res, "converged": bool(res <= TOL),
+                                                    "ms": e0.elapsed_time(e1), "device_bytes": gr.device_bytes()}
+                rsw[f"{ngrid}x{ngrid}"] = tab
+                if ngrid != n:
+                    gr.close()
+                else:
+                    g.set_option("release_workspace", 1)      # give the 100-vector basis back before the remaining sections
+            line_extra["restart_sweep"] = rsw
         # ---- smooth problem (config-1 type: Gaussian, sigma_s = 1e3, at the bench resolution): where implicit comes closest --
         if not args.no_sweep:
             ws = wl.gaussian_diffusion(n)
@@ -569,9 +670,19 @@ def run_ours(args):
         if world == 1 and not args.no_cpu_baseline:
             n_s = args.cpu_n
             r = oracle_step_time(n_s, args.seed, 1, 0)
+            r1 = oracle_step_time(512, args.seed, 1, 0, threads=1)
             line_extra["cpu_baseline"] = {"value": 2.0 * r["cells"] / r["seconds"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
                                           "sample": f"1 step (explicit + implicit 10x, {r['iterations']} GMRES iterations) on a {n_s}x{n_s} grid of "
-                                                    f"the same generator = {r['cells'] / N:.4f} of the workload's cells; {r['seconds']:.1f} s"}
+                                                    f"the same generator = {r['cells'] / N:.4f} of the workload's cells; {r['seconds']:.1f} s",
+                                          "explicit_cell_updates_per_s": r["cells"] / r["explicit_s"],
+                                          "implicit_cell_updates_per_s": r["cells"] / r["implicit_s"],
+                                          "implicit_s_per_iteration_per_Mcell": r["implicit_s"] / max(r["iterations"], 1) / (r["cells"] / 1e6),
+                                          "one_thread": {"sample": "the same step on a 512x512 grid, 1 thread", "value": 2.0 * r1["cells"] / r1["seconds"],
+                                                         "explicit_cell_updates_per_s": r1["cells"] / r1["explicit_s"],
+                                                         "implicit_cell_updates_per_s": r1["cells"] / r1["implicit_s"]},
+                                          "protocol": "bounded sample; the full SURVEY 8(d) protocol (bench size, explicit alone, capped cycle, 1 thread) runs with --oracle-protocol"}
+            if args.oracle_protocol:
+                line_extra["cpu_baseline"]["full_protocol"] = oracle_protocol(n, args.seed)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -607,6 +718,9 @@ def main():
                     help="0: 3x3 block-Jacobi (north_star; the default line)  1: multigrid V-cycle (variant run; uses the block-stencil operator)")
     ap.add_argument("--mg-precision", type=int, default=32, choices=[32, 64], help="storage precision of the multigrid blocks")
     ap.add_argument("--no-sweep", action="store_true", help="skip the dt = 50/100/200x implicit solves")
+    ap.add_argument("--sustain-s", type=float, default=2.0, help="length of the sustained back-to-back explicit run, seconds")
+    ap.add_argument("--restart-sweep", action="store_true", help="also sweep the GMRES restart length (30/60/100) at 50/100/200x on the bench medium and at 1024^2 (takes ~3 min)")
+    ap.add_argument("--oracle-protocol", action="store_true", help="also time the oracle as SURVEY 8(d) lists it: explicit alone and one capped GMRES cycle at the bench size, all cores and 1 thread (takes several minutes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stage2", action="store_true", help="skip the config-5 (2048^2, matter coupling) implicit step")
     ap.add_argument("--cpu-n", type=int, default=2048, help="grid size of the oracle's bounded sample (cpu_baseline)")

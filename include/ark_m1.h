@@ -209,6 +209,64 @@ ARK_M1_API int ark_m1_fastmath_errors(int n, double* out4);
  * Returns 12, or ARK_M1_E_ARG / ARK_M1_E_ALLOC / ARK_M1_E_CUDA / ARK_M1_E_UNSUPPORTED. */
 ARK_M1_API int ark_m1_fp64_issue_rate(double* out, int cap);
 
+/* ---------------------------------------------------------------------------------------------------------------------------
+ * Domain-decomposed step: 1-D slabs in y, one slab per rank ("regular domain decomposition with ghost cells";
+ * PAPER.md:315 rows of the linear system distributed over the ranks; "several communications per iteration").
+ * Rank r of nranks owns the global rows [y0, y1) of ark_m1_slab_range.  Per explicit step and per assembly the boundary rows of
+ * (E, Fx, Fy, sigma_a, sigma_t) are exchanged with the two neighbours; per operator application the boundary rows of
+ * (z, c^2 J z), z = M^-1 v; per GMRES iteration the j+1 Gram-Schmidt dot products and ||w||^2 are all-reduced (fp64).
+ * Everything else runs in the one-GPU kernels on the slab.  Supported: ark_m1_group_step_explicit (all explicit kernels, matter
+ * terms included) and ark_m1_group_step_implicit with the default solver configuration (GMRES(m) + block-Jacobi, matrix-free
+ * operator); other solver options return ARK_M1_E_UNSUPPORTED.
+ *
+ * A group owns its slab solvers.  ark_m1_group_slab returns them: use ark_m1_set_state / ark_m1_set_field / ark_m1_set_boundary
+ * (x sides, and the y sides that are global boundaries) / ark_m1_set_option / ark_m1_get_state on a slab handle with LOCAL arrays
+ * of (y1 - y0) x nx cells; the stepping calls on a slab handle return ARK_M1_E_UNSUPPORTED (the halos must be exchanged).
+ * --------------------------------------------------------------------------------------------------------------------------- */
+typedef struct ark_m1_group ark_m1_group;
+
+/* Rows [*y0, *y1) of rank `rank` of `nranks` on a grid of ny rows: y0 = floor(ny rank / nranks).  Host arithmetic only (no GPU). */
+ARK_M1_API int ark_m1_slab_range(int ny, int nranks, int rank, int* y0, int* y1);
+
+/* Caller-supplied transport for ark_m1_group_create_host: HOST buffers, blocking calls, 0 on success.
+ *   sendrecv     : send `n` doubles of send_lo to rank `lo` and of send_hi to rank `hi`; receive `n` doubles from `lo` into recv_lo
+ *                  and from `hi` into recv_hi.  lo / hi < 0: no such neighbour (its buffers are not touched).  What a rank sends to
+ *                  its `lo` neighbour arrives in that neighbour's recv_hi, and vice versa (with two ranks and a periodic direction lo
+ *                  and hi are the same peer).
+ *   allreduce_sum: buf[0..n) <- sum over all ranks, the same result on every rank. */
+typedef struct {
+    void* ctx;
+    int (*sendrecv)(void* ctx, int lo, int hi, const double* send_lo, const double* send_hi, double* recv_lo, double* recv_hi, long long n);
+    int (*allreduce_sum)(void* ctx, double* buf, int n);
+} ark_m1_host_transport;
+
+/* All nranks slabs in this process on the current device (exchange = device copies, all-reduce = a kernel; nothing ever waits on
+ * another rank): the form the decomposition is tested in on one GPU.  Global arguments as for ark_m1_create. */
+ARK_M1_API ark_m1_group* ark_m1_group_create_local(int nx, int ny, double dx, double dy, double c, const ark_m1_bc* bc, int nranks);
+/* One slab (rank `rank`) in this process; halos and sums staged through pinned host memory and the caller's transport. */
+ARK_M1_API ark_m1_group* ark_m1_group_create_host(int nx, int ny, double dx, double dy, double c, const ark_m1_bc* bc, int rank, int nranks,
+                                                  const ark_m1_host_transport* transport);
+/* One slab in this process on the current GPU; ncclSend/ncclRecv + ncclAllReduce on the solver's stream.  unique_id128: the 128 bytes
+ * of ark_m1_nccl_unique_id obtained on one rank and distributed to all by the caller.  libnccl.so.2 is opened with dlopen. */
+ARK_M1_API int ark_m1_nccl_unique_id(void* out128);
+ARK_M1_API ark_m1_group* ark_m1_group_create_nccl(int nx, int ny, double dx, double dy, double c, const ark_m1_bc* bc, int rank, int nranks,
+                                                  const void* unique_id128);
+ARK_M1_API void ark_m1_group_destroy(ark_m1_group* g);
+ARK_M1_API int ark_m1_group_set_stream(ark_m1_group* g, void* cuda_stream);
+
+/* Number of slabs held by this process (nranks for a local group, 1 otherwise) and the k-th of them with its rank and rows. */
+ARK_M1_API int ark_m1_group_local_slabs(const ark_m1_group* g);
+ARK_M1_API ark_m1* ark_m1_group_slab(ark_m1_group* g, int k, int* rank, int* y0, int* y1);
+
+/* The decomposed steps; arguments, return values and error behaviour as ark_m1_step_explicit / ark_m1_step_implicit (collective:
+ * every rank calls them with the same arguments). */
+ARK_M1_API int ark_m1_group_step_explicit(ark_m1_group* g, double dt);
+ARK_M1_API int ark_m1_group_step_implicit(ark_m1_group* g, double dt, double tol, int restart, int maxit, double* final_residual);
+
+/* Communication counters since creation: halo bytes sent by this process, exchanges, all-reduces. */
+ARK_M1_API int ark_m1_group_comm_stats(const ark_m1_group* g, long long* halo_bytes, long long* exchanges, long long* allreduces);
+ARK_M1_API const char* ark_m1_group_last_error(const ark_m1_group* g);
+
 /* Device bytes currently allocated by the handle. */
 ARK_M1_API long long ark_m1_device_bytes(const ark_m1* h);
 

@@ -26,11 +26,23 @@ SYMBOLS = [
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
     "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_fastmath_errors", "ark_m1_fp64_issue_rate", "ark_m1_apply_preconditioner", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
+    "ark_m1_slab_range", "ark_m1_group_create_local", "ark_m1_group_create_host", "ark_m1_nccl_unique_id", "ark_m1_group_create_nccl",
+    "ark_m1_group_destroy", "ark_m1_group_set_stream", "ark_m1_group_local_slabs", "ark_m1_group_slab", "ark_m1_group_step_explicit",
+    "ark_m1_group_step_implicit", "ark_m1_group_comm_stats", "ark_m1_group_last_error",
 ]
 
 
 class ArkBc(C.Structure):
     _fields_ = [("xlo", C.c_int), ("xhi", C.c_int), ("ylo", C.c_int), ("yhi", C.c_int)]
+
+
+_SENDRECV = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                        C.POINTER(C.c_double), C.c_longlong)
+_ALLREDUCE = C.CFUNCTYPE(C.c_int, C.c_void_p, C.POINTER(C.c_double), C.c_int)
+
+
+class ArkHostTransport(C.Structure):
+    _fields_ = [("ctx", C.c_void_p), ("sendrecv", _SENDRECV), ("allreduce_sum", _ALLREDUCE)]
 
 
 _lib = None
@@ -82,6 +94,26 @@ def load_library(path: str | None = None):
     L.ark_m1_last_error.argtypes = [vp]
     L.ark_m1_version.restype = C.c_char_p
     L.ark_m1_version.argtypes = []
+    ip = C.POINTER(C.c_int)
+    L.ark_m1_slab_range.argtypes = [i, i, i, ip, ip]
+    L.ark_m1_group_create_local.restype = vp
+    L.ark_m1_group_create_local.argtypes = [i, i, d, d, d, C.POINTER(ArkBc), i]
+    L.ark_m1_group_create_host.restype = vp
+    L.ark_m1_group_create_host.argtypes = [i, i, d, d, d, C.POINTER(ArkBc), i, i, C.POINTER(ArkHostTransport)]
+    L.ark_m1_nccl_unique_id.argtypes = [vp]
+    L.ark_m1_group_create_nccl.restype = vp
+    L.ark_m1_group_create_nccl.argtypes = [i, i, d, d, d, C.POINTER(ArkBc), i, i, vp]
+    L.ark_m1_group_destroy.restype = None
+    L.ark_m1_group_destroy.argtypes = [vp]
+    L.ark_m1_group_set_stream.argtypes = [vp, vp]
+    L.ark_m1_group_local_slabs.argtypes = [vp]
+    L.ark_m1_group_slab.restype = vp
+    L.ark_m1_group_slab.argtypes = [vp, i, ip, ip, ip]
+    L.ark_m1_group_step_explicit.argtypes = [vp, d]
+    L.ark_m1_group_step_implicit.argtypes = [vp, d, d, i, i, C.POINTER(C.c_double)]
+    L.ark_m1_group_comm_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    L.ark_m1_group_last_error.restype = C.c_char_p
+    L.ark_m1_group_last_error.argtypes = [vp]
     for name in SYMBOLS:
         getattr(L, name)
     _lib = L
@@ -111,10 +143,14 @@ def _ptr(a, nelem=None):
 class ArkM1:
     """One solver handle.  Method names follow include/ark_m1.h without the ark_m1_ prefix."""
 
-    def __init__(self, nx, ny, dx, dy, c=1.0, bc=(0, 0, 0, 0), stream=None):
+    def __init__(self, nx, ny, dx, dy, c=1.0, bc=(0, 0, 0, 0), stream=None, _borrowed=None):
         self._L = load_library()
         self.nx, self.ny, self.dx, self.dy, self.c = int(nx), int(ny), float(dx), float(dy), float(c)
         self.bc = tuple(int(b) for b in bc)
+        self._owned = _borrowed is None
+        if _borrowed is not None:          # a slab of an ArkM1Group: the group owns the handle
+            self._h = _borrowed
+            return
         b = ArkBc(*self.bc)
         self._h = self._L.ark_m1_create(self.nx, self.ny, self.dx, self.dy, self.c, C.byref(b))
         if not self._h:
@@ -124,7 +160,8 @@ class ArkM1:
 
     def close(self):
         if getattr(self, "_h", None):
-            self._L.ark_m1_destroy(self._h)
+            if self._owned:
+                self._L.ark_m1_destroy(self._h)
             self._h = None
 
     __del__ = close
@@ -247,6 +284,165 @@ class ArkM1:
 
     def device_bytes(self):
         return int(self._L.ark_m1_device_bytes(self._h))
+
+
+def slab_range(ny, nranks, rank):
+    """Rows [y0, y1) of slab `rank` (ark_m1_slab_range; host arithmetic, works without a GPU)."""
+    y0, y1 = C.c_int(0), C.c_int(0)
+    if load_library().ark_m1_slab_range(int(ny), int(nranks), int(rank), C.byref(y0), C.byref(y1)) < 0:
+        raise ValueError("ark_m1_slab_range: bad arguments")
+    return y0.value, y1.value
+
+
+def gloo_host_transport(dist, rank, nranks):
+    """ArkHostTransport whose callbacks move the host buffers with torch.distributed (any backend with CPU tensors, e.g. gloo).
+    Returns (transport struct, keepalive)."""
+    import torch
+
+    def _view(ptr, n):
+        return torch.from_numpy(np.ctypeslib.as_array(ptr, shape=(int(n),)))
+
+    def sendrecv(ctx, lo, hi, send_lo, send_hi, recv_lo, recv_hi, n):
+        try:
+            ops, keep = [], []
+            # what goes to `lo` is that rank's upper halo (tag 1); what goes to `hi` is its lower halo (tag 0)
+            if lo >= 0:
+                t = _view(send_lo, n).clone(); keep.append(t); ops.append(dist.P2POp(dist.isend, t, lo, tag=1))
+            if hi >= 0:
+                t = _view(send_hi, n).clone(); keep.append(t); ops.append(dist.P2POp(dist.isend, t, hi, tag=0))
+            rl = rh = None
+            if hi >= 0:
+                rh = torch.empty(int(n), dtype=torch.float64); ops.append(dist.P2POp(dist.irecv, rh, hi, tag=1))
+            if lo >= 0:
+                rl = torch.empty(int(n), dtype=torch.float64); ops.append(dist.P2POp(dist.irecv, rl, lo, tag=0))
+            if ops:
+                for req in dist.batch_isend_irecv(ops):
+                    req.wait()
+            if rl is not None:
+                _view(recv_lo, n).copy_(rl)
+            if rh is not None:
+                _view(recv_hi, n).copy_(rh)
+            return 0
+        except Exception as exc:      # never let an exception cross the C boundary
+            print(f"gloo_host_transport.sendrecv failed on rank {rank}: {exc!r}")
+            return -1
+
+    def allreduce(ctx, buf, n):
+        try:
+            t = _view(buf, n).clone()
+            dist.all_reduce(t)
+            _view(buf, n).copy_(t)
+            return 0
+        except Exception as exc:
+            print(f"gloo_host_transport.allreduce failed on rank {rank}: {exc!r}")
+            return -1
+
+    cb1, cb2 = _SENDRECV(sendrecv), _ALLREDUCE(allreduce)
+    return ArkHostTransport(None, cb1, cb2), (cb1, cb2)
+
+
+class ArkM1Group:
+    """Slab-decomposed solver (include/ark_m1.h, "Domain-decomposed step").  kind = "local" (all slabs in this process, one
+    GPU), "host" (one slab per process, `transport` = ArkHostTransport) or "nccl" (one slab per process and GPU,
+    `unique_id` = the 128 bytes of nccl_unique_id() of one rank)."""
+
+    def __init__(self, nx, ny, dx, dy, c=1.0, bc=(0, 0, 0, 0), nranks=1, kind="local", rank=0, transport=None, unique_id=None, stream=None):
+        self._L = load_library()
+        self.nx, self.ny, self.nranks, self.rank, self.kind = int(nx), int(ny), int(nranks), int(rank), kind
+        b = ArkBc(*[int(v) for v in bc])
+        self._keep = transport
+        if kind == "local":
+            self._g = self._L.ark_m1_group_create_local(self.nx, self.ny, float(dx), float(dy), float(c), C.byref(b), self.nranks)
+        elif kind == "host":
+            self._g = self._L.ark_m1_group_create_host(self.nx, self.ny, float(dx), float(dy), float(c), C.byref(b), self.rank, self.nranks,
+                                                       C.byref(transport[0] if isinstance(transport, tuple) else transport))
+        elif kind == "nccl":
+            self._idbuf = C.create_string_buffer(bytes(unique_id), 128)
+            self._g = self._L.ark_m1_group_create_nccl(self.nx, self.ny, float(dx), float(dy), float(c), C.byref(b), self.rank, self.nranks,
+                                                       C.cast(self._idbuf, C.c_void_p))
+        else:
+            raise ValueError("kind must be local, host or nccl")
+        if not self._g:
+            raise ValueError("ark_m1_group_create failed (bad arguments, no CUDA device, or the transport could not be set up)")
+        self.slabs = []
+        for k in range(self._L.ark_m1_group_local_slabs(self._g)):
+            r, y0, y1 = C.c_int(0), C.c_int(0), C.c_int(0)
+            h = self._L.ark_m1_group_slab(self._g, k, C.byref(r), C.byref(y0), C.byref(y1))
+            s = ArkM1(self.nx, y1.value - y0.value, dx, dy, c, bc, _borrowed=h)
+            s.rank, s.y0, s.y1 = r.value, y0.value, y1.value
+            self.slabs.append(s)
+        if stream is not None:
+            self.set_stream(stream)
+
+    def close(self):
+        if getattr(self, "_g", None):
+            for s in self.slabs:
+                s.close()
+            self._L.ark_m1_group_destroy(self._g)
+            self._g = None
+
+    __del__ = close
+
+    def _check(self, rc):
+        if rc < 0:
+            raise RuntimeError(f"ark_m1_group error {rc}: {self._L.ark_m1_group_last_error(self._g).decode()}")
+        return rc
+
+    def set_stream(self, stream):
+        addr = getattr(stream, "cuda_stream", stream)
+        self._check(self._L.ark_m1_group_set_stream(self._g, C.c_void_p(addr)))
+
+    def set_option(self, key, value):
+        for s in self.slabs:
+            s.set_option(key, value)
+
+    def scatter(self, w):
+        """Give every local slab its rows of a GLOBAL workload dict (E, F, sigma_a, sigma_s[, T, rho_cv, source_E, ux, uy], x-side
+        ghosts per row, y-side ghosts on the end slabs)."""
+        for s in self.slabs:
+            rows = slice(s.y0, s.y1)
+            cut = lambda a: None if a is None else np.ascontiguousarray(np.asarray(a)[..., rows, :])
+            s.set_state(cut(w["E"]), cut(w["F"]), cut(w["sigma_a"]), cut(w["sigma_s"]), cut(w.get("T")))
+            for name in ("rho_cv", "ux", "uy", "source_E"):
+                if w.get(name) is not None:
+                    s.set_field(name, cut(w[name]))
+            for side, gh in (w.get("ghosts") or {}).items():
+                if side < 2:           # x sides: one value per row of the slab
+                    s.set_boundary(side, *[np.ascontiguousarray(np.asarray(a)[..., rows]) for a in gh])
+                elif (side == 2 and s.y0 == 0) or (side == 3 and s.y1 == self.ny):
+                    s.set_boundary(side, *gh)
+
+    def gather(self, with_T=False):
+        """Rows held by this process: list of (y0, y1, E, F[, T])."""
+        return [(s.y0, s.y1) + tuple(s.get_state(with_T=with_T)) for s in self.slabs]
+
+    def get_state(self, with_T=False):
+        """The stitched global state (local groups only)."""
+        parts = self.gather(with_T)
+        E = np.concatenate([p[2] for p in parts], axis=0)
+        F = np.concatenate([p[3] for p in parts], axis=1)
+        return (E, F, np.concatenate([p[4] for p in parts], axis=0)) if with_T else (E, F)
+
+    def step_explicit(self, dt):
+        self._check(self._L.ark_m1_group_step_explicit(self._g, float(dt)))
+
+    def step_implicit(self, dt, tol=1e-10, restart=30, maxit=4000):
+        res = C.c_double(0.0)
+        its = self._check(self._L.ark_m1_group_step_implicit(self._g, float(dt), float(tol), int(restart), int(maxit), C.byref(res)))
+        return its, res.value
+
+    def comm_stats(self):
+        a, b, c_ = C.c_longlong(0), C.c_longlong(0), C.c_longlong(0)
+        self._check(self._L.ark_m1_group_comm_stats(self._g, C.byref(a), C.byref(b), C.byref(c_)))
+        return dict(halo_bytes=a.value, exchanges=b.value, allreduces=c_.value)
+
+
+def nccl_unique_id():
+    buf = C.create_string_buffer(128)
+    rc = load_library().ark_m1_nccl_unique_id(C.cast(buf, C.c_void_p))
+    if rc < 0:
+        raise RuntimeError(f"ark_m1_nccl_unique_id failed ({rc}): libnccl.so.2 not loadable?")
+    return bytes(buf.raw)
 
 
 def fastmath_errors(n=1 << 20):

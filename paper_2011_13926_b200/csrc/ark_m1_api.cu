@@ -9,79 +9,17 @@
 #include <map>
 #include <vector>
 
-#include "../../include/ark_m1.h"
-#include "ark_m1_internal.h"
+#include "ark_m1_handle.h"
 
 using namespace ark;
 
-// kernel classes for the launch statistics
-enum { KC_EXPLICIT = 0, KC_ASSEMBLE, KC_SCALE, KC_DIAGMUL, KC_SPMV, KC_DOT, KC_UPDATE, KC_COMBINE, KC_SMALL, KC_MG, KC_MGSETUP, KC_COUNT };
-static const char* const kc_names[KC_COUNT] = { "explicit", "assemble", "scale_offdiag", "diag_mul", "spmv_hat", "multi_dot",
-                                                 "update_norm", "combine", "small", "mg_vcycle", "mg_setup" };
-
-struct ark_m1 {
-    Grid g;
-    Scheme s;
-    cudaStream_t st;
-    int device, sm_count;
-    long long N;
-    long long bytes;
-    std::map<void*, size_t>* allocs;   // device allocations counted in `bytes`
-    bool have_state, have_T;
-    // state: two buffers of 3N doubles [E | Fx | Fy]; U[cur] is current
-    double* U[2];
-    int cur;
-    double *sa, *ss_tmp, *stot, *T[2];
-    double* gh[4][5];
-    double *rho_cv, *ux, *uy, *source_E;
-    unsigned long long* counts;   // 2
-    // options
-    int ortho, explicit_kernel, op_kind, maxv, krylov, asm_kernel;
-    int basis_prec;    // 64, or 32: compressed-basis GMRES (krylov_cb.cu); applies to GMRES + block-Jacobi + matrix-free operator
-    float* V32;        // (m32_alloc + 1) basis vectors of `stride` floats
-    double* wk;        // 3N: the fp64 work vector of the compressed-basis path
-    int m32_alloc, vslots;
-    int precond;       // 0: 3x3 block-Jacobi, 1: multigrid V-cycle (forces the assembled block-stencil operator)
-    MgHier mg;         // hierarchy (levels >= 1 allocated lazily)
-    double* mgz;       // 3N: V-cycle output (hat variable)
-    double mg_cells;   // sum over levels of cells / N (for the byte counts)
-    // implicit workspace (lazy)
-    BlockMatrix A;
-    MfPlanes mf;       // matrix-free coefficient planes (op_kind == 1)
-    double* V;         // (m+1) vectors of `stride` doubles
-    double* tvec;      // 3N
-    double* nprev;     // 3N, previous Newton iterate (lazy)
-    long long stride;
-    int m_alloc, maxit_alloc;
-    GmresWork W;
-    void* wblock;      // allocation behind W
-    GmresCtl* ctl_host;  // pinned
-    std::vector<double>* hist_host;
-    cudaEvent_t ev[3];
-    double timings[3];
-    // per-kernel-class timing (option "kernel_timing"): one event before every launch + one at the end
-    int ktiming;
-    std::vector<cudaEvent_t>* kev;
-    std::vector<int>* kcls;
-    std::vector<double>* kbytes;
-    size_t kused;
-    double kstat[KC_COUNT][3];   // launches, milliseconds, algorithmic bytes
-    long long launches;          // kernels launched by this handle
-    char err[512];
-};
-
 // The handle lives on the device that was current at ark_m1_create.  Every entry point makes that device current for its
 // duration and restores the caller's (a multi-GPU process may have switched devices in between).
-struct DeviceGuard {
-    int prev;
-    bool switched;
-    explicit DeviceGuard(int dev) : prev(-1), switched(false)
-    {
-        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
-    }
-    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
-};
-#define GUARD(h) DeviceGuard guard__((h)->device)
+DeviceGuard::DeviceGuard(int dev) : prev(-1), switched(false)
+{
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+}
+DeviceGuard::~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 
 namespace ark {
 int current_sm_count()
@@ -94,15 +32,14 @@ int current_sm_count()
 }
 }  // namespace ark
 
-static int fail(ark_m1* h, int code, const char* fmt, const char* detail)
+int ark_fail(ark_m1* h, int code, const char* fmt, const char* detail)
 {
     if (h) snprintf(h->err, sizeof h->err, fmt, detail ? detail : "");
     return code;
 }
-#define CU(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(h, ARK_M1_E_CUDA, #call ": %s", cudaGetErrorString(e__)); } while (0)
 
 // Record the start of a launch of class `cls` moving `bytes` algorithmic bytes (only when kernel timing is on).
-static void kmark(ark_m1* h, int cls, double bytes)
+void ark_kmark(ark_m1* h, int cls, double bytes)
 {
     h->launches++;
     if (!h->ktiming) return;
@@ -111,7 +48,7 @@ static void kmark(ark_m1* h, int cls, double bytes)
     h->kcls->push_back(cls); h->kbytes->push_back(bytes);
 }
 // Close the open series: one final event, then (after a sync) accumulate per-class elapsed times.
-static void kflush(ark_m1* h)
+void ark_kflush(ark_m1* h)
 {
     if (!h->ktiming || h->kcls->empty()) return;
     if (h->kused == h->kev->size()) { cudaEvent_t e; cudaEventCreate(&e); h->kev->push_back(e); }
@@ -124,19 +61,18 @@ static void kflush(ark_m1* h)
     }
     h->kcls->clear(); h->kbytes->clear(); h->kused = 0;
 }
-#define KL(cls, bytes, call) do { kmark(h, (cls), (double)(bytes)); CU(call); } while (0)
 
-static int dmalloc(ark_m1* h, void** p, size_t bytes)
+int ark_dmalloc(ark_m1* h, void** p, size_t bytes)
 {
     cudaError_t e = cudaMalloc(p, bytes);
-    if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return fail(h, ARK_M1_E_ALLOC, "cudaMalloc: %s", cudaGetErrorString(e)); }
+    if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return ark_fail(h, ARK_M1_E_ALLOC, "cudaMalloc: %s", cudaGetErrorString(e)); }
     h->bytes += (long long)bytes;
     if (h->allocs) (*h->allocs)[*p] = bytes;
     return 0;
 }
 
 // cudaFree of a dmalloc'ed pointer with the byte count kept right (null is fine)
-static void dfree(ark_m1* h, void* p)
+void ark_dfree(ark_m1* h, void* p)
 {
     if (!p) return;
     cudaFree(p);
@@ -151,16 +87,22 @@ static inline int opk(const ark_m1* h) { return h->precond == 1 ? 0 : h->op_kind
 // compressed-basis GMRES applies to the default solver configuration only; elsewhere the option is ignored
 static inline bool use_cb(const ark_m1* h) { return h->basis_prec == 32 && h->krylov == 0 && h->precond == 0 && h->op_kind == 1 && h->ortho == 1; }
 
-static Fields fields_of(const ark_m1* h)
+Fields ark_fields_of(const ark_m1* h)
 {
     Fields f;
     const double* U = h->U[h->cur];
     f.E = U; f.Fx = U + h->N; f.Fy = U + 2 * h->N; f.sa = h->sa; f.st = h->stot;
     for (int s = 0; s < 4; ++s) for (int k = 0; k < 5; ++k) f.gh[s][k] = h->gh[s][k];
+    for (int s = 0; s < 2; ++s)      // halo sides of a slab: the ghost lines are the received boundary rows of the neighbour rank
+        if (h->g.bc[YLO + s] == BC_HALO) for (int k = 0; k < 5; ++k) f.gh[YLO + s][k] = h->halo_state[s] + (size_t)k * h->g.nx;
     f.T = h->have_T ? h->T[h->cur] : nullptr;
     f.rho_cv = h->rho_cv; f.source_E = h->source_E;
     return f;
 }
+
+// a slab with halo sides can only be advanced through its group (the halos must be exchanged first)
+static inline bool needs_group(const ark_m1* h) { return h->g.bc[YLO] == BC_HALO || h->g.bc[YHI] == BC_HALO; }
+#define NO_SLAB(h, what) do { if (needs_group(h)) return ark_fail(h, ARK_M1_E_UNSUPPORTED, what ": this handle is a slab of an ark_m1_group; use the ark_m1_group_* call%s", ""); } while (0)
 
 extern "C" {
 
@@ -191,15 +133,15 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->kev = new std::vector<cudaEvent_t>(); h->kcls = new std::vector<int>(); h->kbytes = new std::vector<double>();
     const size_t N = (size_t)h->N;
     bool ok = true;
-    for (int k = 0; k < 2 && ok; ++k) ok = dmalloc(h, (void**)&h->U[k], 3 * N * sizeof(double)) == 0;
-    ok = ok && dmalloc(h, (void**)&h->sa, N * sizeof(double)) == 0;
-    ok = ok && dmalloc(h, (void**)&h->ss_tmp, N * sizeof(double)) == 0;
-    ok = ok && dmalloc(h, (void**)&h->stot, N * sizeof(double)) == 0;
-    ok = ok && dmalloc(h, (void**)&h->counts, 2 * sizeof(unsigned long long)) == 0;
+    for (int k = 0; k < 2 && ok; ++k) ok = ark_dmalloc(h, (void**)&h->U[k], 3 * N * sizeof(double)) == 0;
+    ok = ok && ark_dmalloc(h, (void**)&h->sa, N * sizeof(double)) == 0;
+    ok = ok && ark_dmalloc(h, (void**)&h->ss_tmp, N * sizeof(double)) == 0;
+    ok = ok && ark_dmalloc(h, (void**)&h->stot, N * sizeof(double)) == 0;
+    ok = ok && ark_dmalloc(h, (void**)&h->counts, 2 * sizeof(unsigned long long)) == 0;
     for (int s = 0; s < 4 && ok; ++s) {
         const size_t len = (s < 2) ? ny : nx;
         for (int k = 0; k < 5 && ok; ++k) {
-            ok = dmalloc(h, (void**)&h->gh[s][k], len * sizeof(double)) == 0;
+            ok = ark_dmalloc(h, (void**)&h->gh[s][k], len * sizeof(double)) == 0;
             if (ok) cudaMemset(h->gh[s][k], 0, len * sizeof(double));
         }
     }
@@ -211,12 +153,12 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
 
 static void free_implicit(ark_m1* h)
 {
-    for (int l = 0; l < h->mg.nlev; ++l) { dfree(h, h->mg.lev[l].off32); h->mg.lev[l].off32 = nullptr; }
-    for (int l = 1; l < h->mg.nlev; ++l) { dfree(h, h->mg.lev[l].off); dfree(h, h->mg.lev[l].Dinv); dfree(h, h->mg.lev[l].r); dfree(h, h->mg.lev[l].e); }
-    h->mg.nlev = 0; dfree(h, h->mgz); h->mgz = nullptr;
-    dfree(h, h->V32); h->V32 = nullptr; dfree(h, h->wk); h->wk = nullptr; h->m32_alloc = 0; h->vslots = 0;
-    dfree(h, h->A.off); dfree(h, h->A.C); dfree(h, h->A.Minv); dfree(h, h->A.b); dfree(h, h->V); dfree(h, h->tvec); cudaFree(h->wblock); dfree(h, h->nprev); h->nprev = nullptr;
-    dfree(h, h->mf.J); dfree(h, h->mf.fE); dfree(h, h->mf.fN); dfree(h, h->mf.dE); dfree(h, h->mf.dF); dfree(h, h->mf.xlo); dfree(h, h->mf.ylo);
+    for (int l = 0; l < h->mg.nlev; ++l) { ark_dfree(h, h->mg.lev[l].off32); h->mg.lev[l].off32 = nullptr; }
+    for (int l = 1; l < h->mg.nlev; ++l) { ark_dfree(h, h->mg.lev[l].off); ark_dfree(h, h->mg.lev[l].Dinv); ark_dfree(h, h->mg.lev[l].r); ark_dfree(h, h->mg.lev[l].e); }
+    h->mg.nlev = 0; ark_dfree(h, h->mgz); h->mgz = nullptr;
+    ark_dfree(h, h->V32); h->V32 = nullptr; ark_dfree(h, h->wk); h->wk = nullptr; h->m32_alloc = 0; h->vslots = 0;
+    ark_dfree(h, h->A.off); ark_dfree(h, h->A.C); ark_dfree(h, h->A.Minv); ark_dfree(h, h->A.b); ark_dfree(h, h->V); ark_dfree(h, h->tvec); cudaFree(h->wblock); ark_dfree(h, h->nprev); h->nprev = nullptr;
+    ark_dfree(h, h->mf.J); ark_dfree(h, h->mf.fE); ark_dfree(h, h->mf.fN); ark_dfree(h, h->mf.dE); ark_dfree(h, h->mf.dF); ark_dfree(h, h->mf.xlo); ark_dfree(h, h->mf.ylo);
     memset(&h->mf, 0, sizeof h->mf);
     h->A.off = h->A.C = h->A.Minv = h->A.b = nullptr; h->V = h->tvec = nullptr; h->wblock = nullptr; h->m_alloc = 0; h->maxit_alloc = 0;
 }
@@ -253,7 +195,7 @@ int ark_m1_set_state(ark_m1* h, const double* E, const double* F, const double* 
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!E || !F || !sigma_a || !sigma_s) return fail(h, ARK_M1_E_ARG, "set_state: NULL array%s", "");
+    if (!E || !F || !sigma_a || !sigma_s) return ark_fail(h, ARK_M1_E_ARG, "set_state: NULL array%s", "");
     const size_t N = (size_t)h->N, B = N * sizeof(double);
     double* U = h->U[h->cur];
     CU(cudaMemcpyAsync(U, E, B, cudaMemcpyDefault, h->st));
@@ -262,7 +204,7 @@ int ark_m1_set_state(ark_m1* h, const double* E, const double* F, const double* 
     CU(cudaMemcpyAsync(h->ss_tmp, sigma_s, B, cudaMemcpyDefault, h->st));
     CU(launch_add_planes(h->stot, h->sa, h->ss_tmp, (long long)N, h->st));
     if (T) {
-        for (int k = 0; k < 2; ++k) if (!h->T[k]) { int rc = dmalloc(h, (void**)&h->T[k], B); if (rc) return rc; }
+        for (int k = 0; k < 2; ++k) if (!h->T[k]) { int rc = ark_dmalloc(h, (void**)&h->T[k], B); if (rc) return rc; }
         CU(cudaMemcpyAsync(h->T[h->cur], T, B, cudaMemcpyDefault, h->st));
     }
     h->have_T = (T != nullptr);
@@ -274,7 +216,7 @@ int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const double* F_
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
-    if (side < 0 || side > 3 || !E_g || !F_g || !sa_g || !ss_g) return fail(h, ARK_M1_E_ARG, "set_boundary: bad argument%s", "");
+    if (side < 0 || side > 3 || !E_g || !F_g || !sa_g || !ss_g) return ark_fail(h, ARK_M1_E_ARG, "set_boundary: bad argument%s", "");
     const size_t len = (side < 2) ? h->g.ny : h->g.nx, B = len * sizeof(double);
     CU(cudaMemcpyAsync(h->gh[side][0], E_g, B, cudaMemcpyDefault, h->st));
     CU(cudaMemcpyAsync(h->gh[side][1], F_g, B, cudaMemcpyDefault, h->st));
@@ -292,26 +234,26 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     GUARD(h);
     const int iv = (int)value;
     if (!strcmp(key, "well_balanced")) h->s.wb = (value != 0.0);
-    else if (!strcmp(key, "ap_mode")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "ap_mode must be 0, 1 or 2%s", ""); h->s.ap = iv; }
-    else if (!strcmp(key, "eig_mode")) { if (iv < 0 || iv > 2) return fail(h, ARK_M1_E_ARG, "eig_mode must be 0, 1 or 2%s", ""); h->s.eig = iv; }
-    else if (!strcmp(key, "closure")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "closure must be 0 or 1%s", ""); h->s.closure = iv; }
-    else if (!strcmp(key, "linearisation")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "linearisation must be 0 or 1%s", ""); h->s.lin = iv; }
-    else if (!strcmp(key, "eig_floor")) { if (!(value >= 0.0)) return fail(h, ARK_M1_E_ARG, "eig_floor must be >= 0%s", ""); h->s.eig_floor = value; }
+    else if (!strcmp(key, "ap_mode")) { if (iv < 0 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "ap_mode must be 0, 1 or 2%s", ""); h->s.ap = iv; }
+    else if (!strcmp(key, "eig_mode")) { if (iv < 0 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "eig_mode must be 0, 1 or 2%s", ""); h->s.eig = iv; }
+    else if (!strcmp(key, "closure")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "closure must be 0 or 1%s", ""); h->s.closure = iv; }
+    else if (!strcmp(key, "linearisation")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "linearisation must be 0 or 1%s", ""); h->s.lin = iv; }
+    else if (!strcmp(key, "eig_floor")) { if (!(value >= 0.0)) return ark_fail(h, ARK_M1_E_ARG, "eig_floor must be >= 0%s", ""); h->s.eig_floor = value; }
     else if (!strcmp(key, "a_r")) h->s.a_r = value;
-    else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
-    else if (!strcmp(key, "explicit_kernel")) { if (iv != 0 && iv != 1 && iv != 3) return fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0 (cell), 1 (128-column march) or 3 (one-warp march, default)%s", ""); h->explicit_kernel = iv; }
-    else if (!strcmp(key, "assembly_kernel")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "assembly_kernel must be 0 (tile) or 1 (marching)%s", ""); h->asm_kernel = iv; }
-    else if (!strcmp(key, "krylov")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "krylov must be 0 (GMRES) or 1 (BiCGStab)%s", ""); h->krylov = iv; }
-    else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 16]%s", ""); h->maxv = iv; }
+    else if (!strcmp(key, "orthogonalisation")) { if (iv < 1 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "orthogonalisation must be 1 or 2%s", ""); h->ortho = iv; }
+    else if (!strcmp(key, "explicit_kernel")) { if (iv != 0 && iv != 1 && iv != 3) return ark_fail(h, ARK_M1_E_ARG, "explicit_kernel must be 0 (cell), 1 (128-column march) or 3 (one-warp march, default)%s", ""); h->explicit_kernel = iv; }
+    else if (!strcmp(key, "assembly_kernel")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "assembly_kernel must be 0 (tile) or 1 (marching)%s", ""); h->asm_kernel = iv; }
+    else if (!strcmp(key, "krylov")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "krylov must be 0 (GMRES) or 1 (BiCGStab)%s", ""); h->krylov = iv; }
+    else if (!strcmp(key, "vectors_per_pass")) { if (iv < 1 || iv > MAXV) return ark_fail(h, ARK_M1_E_ARG, "vectors_per_pass must be in [1, 16]%s", ""); h->maxv = iv; }
     else if (!strcmp(key, "release_workspace")) { if (value != 0.0) { cudaStreamSynchronize(h->st); free_implicit(h); } }
-    else if (!strcmp(key, "kernel_timing")) { kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
-    else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
-    else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
-    else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
-    else if (!strcmp(key, "mg_coarse_sweeps")) { if (iv < 1) return fail(h, ARK_M1_E_ARG, "mg_coarse_sweeps must be >= 1%s", ""); h->mg.coarse_sweeps = iv; }
-    else if (!strcmp(key, "basis_precision")) { if (iv != 32 && iv != 64) return fail(h, ARK_M1_E_ARG, "basis_precision must be 64 or 32%s", ""); h->basis_prec = iv; }
-    else if (!strcmp(key, "mg_precision")) { if (iv != 32 && iv != 64) return fail(h, ARK_M1_E_ARG, "mg_precision must be 64 or 32%s", ""); h->mg.precision = iv; }
-    else return fail(h, ARK_M1_E_ARG, "unknown option %s", key);
+    else if (!strcmp(key, "kernel_timing")) { ark_kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
+    else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
+    else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
+    else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return ark_fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
+    else if (!strcmp(key, "mg_coarse_sweeps")) { if (iv < 1) return ark_fail(h, ARK_M1_E_ARG, "mg_coarse_sweeps must be >= 1%s", ""); h->mg.coarse_sweeps = iv; }
+    else if (!strcmp(key, "basis_precision")) { if (iv != 32 && iv != 64) return ark_fail(h, ARK_M1_E_ARG, "basis_precision must be 64 or 32%s", ""); h->basis_prec = iv; }
+    else if (!strcmp(key, "mg_precision")) { if (iv != 32 && iv != 64) return ark_fail(h, ARK_M1_E_ARG, "mg_precision must be 64 or 32%s", ""); h->mg.precision = iv; }
+    else return ark_fail(h, ARK_M1_E_ARG, "unknown option %s", key);
     return 0;
 }
 
@@ -322,10 +264,10 @@ int ark_m1_set_field(ark_m1* h, const char* name, const double* plane)
     double** dst = nullptr;
     if (!strcmp(name, "rho_cv")) dst = &h->rho_cv; else if (!strcmp(name, "ux")) dst = &h->ux;
     else if (!strcmp(name, "uy")) dst = &h->uy; else if (!strcmp(name, "source_E")) dst = &h->source_E;
-    else return fail(h, ARK_M1_E_ARG, "unknown field %s", name);
+    else return ark_fail(h, ARK_M1_E_ARG, "unknown field %s", name);
     const size_t B = (size_t)h->N * sizeof(double);
-    if (!plane) { CU(cudaStreamSynchronize(h->st)); dfree(h, *dst); *dst = nullptr; return 0; }
-    if (!*dst) { int rc = dmalloc(h, (void**)dst, B); if (rc) return rc; }
+    if (!plane) { CU(cudaStreamSynchronize(h->st)); ark_dfree(h, *dst); *dst = nullptr; return 0; }
+    if (!*dst) { int rc = ark_dmalloc(h, (void**)dst, B); if (rc) return rc; }
     CU(cudaMemcpyAsync(*dst, plane, B, cudaMemcpyDefault, h->st));
     return 0;
 }
@@ -343,9 +285,11 @@ int ark_m1_get_state(ark_m1* h, double* E, double* F, double* T)
     return 0;
 }
 
-static int explicit_once(ark_m1* h, double dt)
+}  // extern "C"
+
+int ark_explicit_once(ark_m1* h, double dt)
 {
-    const Fields f = fields_of(h);
+    const Fields f = ark_fields_of(h);
     double* O = h->U[h->cur ^ 1];
     double* OT = h->have_T ? h->T[h->cur ^ 1] : nullptr;
     // algorithmic bytes per cell: 5 planes in, 3 out; the coupled step adds T in/out (16), rho c_v (8) and the source plane (8)
@@ -361,22 +305,26 @@ static int explicit_once(ark_m1* h, double dt)
     return 0;
 }
 
+extern "C" {
+
 int ark_m1_step_explicit(ark_m1* h, double dt)
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "step_explicit: dt must be > 0%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_explicit: no state set%s", "");
-    return explicit_once(h, dt);
+    NO_SLAB(h, "step_explicit");
+    if (!(dt > 0.0)) return ark_fail(h, ARK_M1_E_ARG, "step_explicit: dt must be > 0%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "step_explicit: no state set%s", "");
+    return ark_explicit_once(h, dt);
 }
 
 int ark_m1_steps_explicit(ark_m1* h, double dt, int nsteps)
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!(dt > 0.0) || nsteps < 0) return fail(h, ARK_M1_E_ARG, "steps_explicit: dt must be > 0 and nsteps >= 0%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "steps_explicit: no state set%s", "");
-    for (int k = 0; k < nsteps; ++k) { int rc = explicit_once(h, dt); if (rc) return rc; }
+    NO_SLAB(h, "steps_explicit");
+    if (!(dt > 0.0) || nsteps < 0) return ark_fail(h, ARK_M1_E_ARG, "steps_explicit: dt must be > 0 and nsteps >= 0%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "steps_explicit: no state set%s", "");
+    for (int k = 0; k < nsteps; ++k) { int rc = ark_explicit_once(h, dt); if (rc) return rc; }
     return 0;
 }
 
@@ -384,8 +332,9 @@ int ark_m1_residual(ark_m1* h, double* RE, double* RF)
 {
     if (!h || !RE || !RF) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "residual: no state set%s", "");
-    const Fields f = fields_of(h);
+    NO_SLAB(h, "residual");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "residual: no state set%s", "");
+    const Fields f = ark_fields_of(h);
     double* O = h->U[h->cur ^ 1];
     const size_t N = (size_t)h->N;
     KL(KC_EXPLICIT, 64.0 * h->N, launch_explicit_cell(h->g, h->s, f, 0.0, 1, O, O + N, O + 2 * N, nullptr, h->st));
@@ -399,8 +348,8 @@ int ark_m1_add_velocity_sources(ark_m1* h, double dt)
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!h->have_state || !h->ux || !h->uy) return fail(h, ARK_M1_E_NOTSET, "add_velocity_sources: state, ux, uy must be set%s", "");
-    const Fields f = fields_of(h);
+    if (!h->have_state || !h->ux || !h->uy) return ark_fail(h, ARK_M1_E_NOTSET, "add_velocity_sources: state, ux, uy must be set%s", "");
+    const Fields f = ark_fields_of(h);
     double* U = h->U[h->cur];
     KL(KC_SMALL, 88.0 * h->N, launch_velocity_sources(h->g, h->s, f, h->ux, h->uy, dt, U, U + h->N, U + 2 * h->N, h->st));
     return 0;
@@ -410,9 +359,9 @@ int ark_m1_count_unrealizable(ark_m1* h, long long* nE, long long* nf)
 {
     if (!h || !nE || !nf) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "count_unrealizable: no state set%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "count_unrealizable: no state set%s", "");
     CU(cudaMemsetAsync(h->counts, 0, 2 * sizeof(unsigned long long), h->st));
-    KL(KC_SMALL, 24.0 * h->N, launch_count_unrealizable(h->g, fields_of(h), h->counts, h->st));
+    KL(KC_SMALL, 24.0 * h->N, launch_count_unrealizable(h->g, ark_fields_of(h), h->counts, h->st));
     unsigned long long out[2];
     CU(cudaMemcpyAsync(out, h->counts, sizeof out, cudaMemcpyDeviceToHost, h->st));
     CU(cudaStreamSynchronize(h->st));
@@ -428,7 +377,7 @@ const char* ark_m1_last_error(const ark_m1* h) { return h ? h->err : "null handl
 // ---------------------------------------------------------------------------------------------------------
 // Implicit step
 // ---------------------------------------------------------------------------------------------------------
-static int ensure_implicit(ark_m1* h, int m, int maxit)
+int ark_ensure_implicit(ark_m1* h, int m, int maxit)
 {
     const size_t N = (size_t)h->N, n = 3 * N;
     const bool have_op = (opk(h) == 0) ? (h->A.off != nullptr) : (h->mf.J != nullptr);
@@ -439,28 +388,28 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
     (void)before;
     if (h->A.Minv == nullptr) {
         int rc;
-        if ((rc = dmalloc(h, (void**)&h->A.Minv, 9 * N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->A.b, n * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->tvec, n * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->A.Minv, 9 * N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->A.b, n * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->tvec, n * sizeof(double)))) return rc;
     }
     if (opk(h) == 0 && h->A.off == nullptr) {
         int rc;
-        if ((rc = dmalloc(h, (void**)&h->A.off, 36 * N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->A.C, 9 * N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->A.off, 36 * N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->A.C, 9 * N * sizeof(double)))) return rc;
     }
     if (opk(h) == 1 && h->mf.J == nullptr) {
         int rc;
-        if ((rc = dmalloc(h, (void**)&h->mf.J, 9 * N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->mf.fE, 4 * N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->mf.fN, 4 * N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->mf.dE, N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->mf.dF, N * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->mf.xlo, 4 * (size_t)h->g.ny * sizeof(double)))) return rc;
-        if ((rc = dmalloc(h, (void**)&h->mf.ylo, 4 * (size_t)h->g.nx * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.J, 9 * N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.fE, 4 * N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.fN, 4 * N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.dE, N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.dF, N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.xlo, 4 * (size_t)h->g.ny * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.ylo, 4 * (size_t)h->g.nx * sizeof(double)))) return rc;
     }
     if (h->precond == 1 && h->mg.nlev == 0) {       // levels 1.. of the multigrid hierarchy (about 1/3 of the fine storage)
         int rc;
-        if ((rc = dmalloc(h, (void**)&h->mgz, n * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mgz, n * sizeof(double)))) return rc;
         MgHier& H = h->mg;
         H.lev[0].g = h->g; H.lev[0].off = nullptr; H.lev[0].off32 = nullptr; H.lev[0].Dinv = nullptr; H.lev[0].r = nullptr; H.lev[0].e = nullptr;
         int L = 1; double cells = 1.0;
@@ -470,20 +419,20 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
             const size_t Nc = (size_t)c.g.nx * c.g.ny;
             c.off = c.Dinv = c.r = c.e = nullptr; c.off32 = nullptr;
             H.nlev = L + 1;                          // so that a failure below frees what was allocated
-            if ((rc = dmalloc(h, (void**)&c.off, 36 * Nc * sizeof(double)))) return rc;
-            if ((rc = dmalloc(h, (void**)&c.Dinv, 9 * Nc * sizeof(double)))) return rc;
-            if ((rc = dmalloc(h, (void**)&c.r, 3 * Nc * sizeof(double)))) return rc;
-            if ((rc = dmalloc(h, (void**)&c.e, 3 * Nc * sizeof(double)))) return rc;
+            if ((rc = ark_dmalloc(h, (void**)&c.off, 36 * Nc * sizeof(double)))) return rc;
+            if ((rc = ark_dmalloc(h, (void**)&c.Dinv, 9 * Nc * sizeof(double)))) return rc;
+            if ((rc = ark_dmalloc(h, (void**)&c.r, 3 * Nc * sizeof(double)))) return rc;
+            if ((rc = ark_dmalloc(h, (void**)&c.e, 3 * Nc * sizeof(double)))) return rc;
             cells += (double)Nc / (double)N;
             ++L;
         }
-        if (H.lev[L - 1].g.nx > 1 || H.lev[L - 1].g.ny > 1) return fail(h, ARK_M1_E_UNSUPPORTED, "multigrid: grid too large for %s levels", "24");
+        if (H.lev[L - 1].g.nx > 1 || H.lev[L - 1].g.ny > 1) return ark_fail(h, ARK_M1_E_UNSUPPORTED, "multigrid: grid too large for %s levels", "24");
         H.nlev = L; h->mg_cells = cells;
     }
     if (h->precond == 1 && h->mg.precision == 32 && h->mg.lev[0].off32 == nullptr) {
         for (int l = 0; l < h->mg.nlev; ++l) {
             const size_t Nl = (size_t)h->mg.lev[l].g.nx * h->mg.lev[l].g.ny;
-            int rc = dmalloc(h, (void**)&h->mg.lev[l].off32, 36 * Nl * sizeof(float));
+            int rc = ark_dmalloc(h, (void**)&h->mg.lev[l].off32, 36 * Nl * sizeof(float));
             if (rc) return rc;
         }
     }
@@ -491,19 +440,19 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
     {   // fp64 vector slots: the whole basis, or (compressed-basis path) the six slots BiCGStab and the staging calls use
         const int need = use_cb(h) ? 6 : ((m + 1) > 6 ? (m + 1) : 6);
         if (h->vslots < need) {
-            dfree(h, h->V); h->V = nullptr; h->vslots = 0;
-            int rc = dmalloc(h, (void**)&h->V, (size_t)need * h->stride * sizeof(double));
+            ark_dfree(h, h->V); h->V = nullptr; h->vslots = 0;
+            int rc = ark_dmalloc(h, (void**)&h->V, (size_t)need * h->stride * sizeof(double));
             if (rc) return rc;
             h->vslots = need;
         }
         if (use_cb(h)) {
             int rc;
             if (h->m32_alloc < m) {
-                dfree(h, h->V32); h->V32 = nullptr; h->m32_alloc = 0;
-                if ((rc = dmalloc(h, (void**)&h->V32, (size_t)(m + 1) * h->stride * sizeof(float)))) return rc;
+                ark_dfree(h, h->V32); h->V32 = nullptr; h->m32_alloc = 0;
+                if ((rc = ark_dmalloc(h, (void**)&h->V32, (size_t)(m + 1) * h->stride * sizeof(float)))) return rc;
                 h->m32_alloc = m;
             }
-            if (!h->wk && (rc = dmalloc(h, (void**)&h->wk, n * sizeof(double)))) return rc;
+            if (!h->wk && (rc = ark_dmalloc(h, (void**)&h->wk, n * sizeof(double)))) return rc;
         }
     }
     const int mm = m > h->m_alloc ? m : h->m_alloc;
@@ -516,7 +465,7 @@ static int ensure_implicit(ark_m1* h, int m, int maxit)
     const size_t nd = (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 2 * (size_t)(mm + 1) + caphist
                       + (size_t)(krylov_max_blocks(h->sm_count) > op_mf_blocks(h->g, h->sm_count) ? krylov_max_blocks(h->sm_count) : op_mf_blocks(h->g, h->sm_count)) * MAXV;
     const size_t ctl_bytes = (sizeof(GmresCtl) + 255) / 256 * 256;
-    if (cudaMalloc(&h->wblock, ctl_bytes + nd * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(h, ARK_M1_E_ALLOC, "cudaMalloc (solver scalars)%s", ""); }
+    if (cudaMalloc(&h->wblock, ctl_bytes + nd * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return ark_fail(h, ARK_M1_E_ALLOC, "cudaMalloc (solver scalars)%s", ""); }
     CU(cudaMemset(h->wblock, 0, ctl_bytes + nd * sizeof(double)));
     GmresWork& W = h->W;
     W.ctl = (GmresCtl*)h->wblock;
@@ -543,16 +492,16 @@ static int true_residual(ark_m1* h, const double* x)
     return 0;
 }
 
-static int fetch_ctl(ark_m1* h)
+int ark_fetch_ctl(ark_m1* h)
 {
     CU(cudaMemcpyAsync(h->ctl_host, h->W.ctl, sizeof(GmresCtl), cudaMemcpyDeviceToHost, h->st));
     CU(cudaStreamSynchronize(h->st));
     return 0;
 }
 
-static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
+int ark_assemble_system(ark_m1* h, double dt, const double* bsrc)
 {
-    const Fields f = fields_of(h);
+    const Fields f = ark_fields_of(h);
     if (opk(h) == 1) {
         h->mf.rx = h->s.hyp_off ? 0.0 : dt / h->g.dx; h->mf.ry = h->s.hyp_off ? 0.0 : dt / h->g.dy;
         if (h->asm_kernel == 1 && h->N < (1LL << 31))
@@ -582,7 +531,7 @@ static int assemble_system(ark_m1* h, double dt, const double* bsrc = nullptr)
 static int mg_apply(ark_m1* h, const double* v, double* zhat, const int* stop)
 {
     int nl = 0;
-    kmark(h, KC_MG, (h->mg.precision == 32 ? (168.0 + 192.0) : (312.0 + 336.0)) * h->N * h->mg_cells);
+    ark_kmark(h, KC_MG, (h->mg.precision == 32 ? (168.0 + 192.0) : (312.0 + 336.0)) * h->N * h->mg_cells);
     CU(launch_mg_vcycle(h->mg, v, zhat, stop, h->st, &nl));
     h->launches += nl - 1;
     return 0;
@@ -602,7 +551,7 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
     KL(KC_SMALL, 0.0, launch_begin_solve(W, tol, m, maxit, h->st));
     KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
     if ((rc = true_residual(h, x))) return rc;
-    if ((rc = fetch_ctl(h))) return rc;
+    if ((rc = ark_fetch_ctl(h))) return rc;
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
@@ -635,7 +584,7 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
         } else
             KL(KC_COMBINE, 8.0 * (3.0 * m + 15.0) * h->N, launch_combine(h->g, h->V, S, h->A.Minv, x, W, sm, h->st));
         if ((rc = true_residual(h, x))) return rc;
-        if ((rc = fetch_ctl(h))) return rc;
+        if ((rc = ark_fetch_ctl(h))) return rc;
     }
     return 0;
 }
@@ -665,7 +614,7 @@ static int gmres_solve_cb(ark_m1* h, double tol, int m, int maxit)
     KL(KC_SMALL, 0.0, launch_begin_solve(W, tol, m, maxit, h->st));
     KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
     if ((rc = true_residual_cb(h, x))) return rc;
-    if ((rc = fetch_ctl(h))) return rc;
+    if ((rc = ark_fetch_ctl(h))) return rc;
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             float* vnext = h->V32 + (size_t)(j + 1) * S;
@@ -685,7 +634,7 @@ static int gmres_solve_cb(ark_m1* h, double tol, int m, int maxit)
         KL(KC_SMALL, 0.0, launch_solve_y(W, h->st));
         KL(KC_COMBINE, 8.0 * (1.5 * m + 15.0) * h->N, launch_combine32(h->g, h->V32, S, h->A.Minv, x, W, sm, h->st));
         if ((rc = true_residual_cb(h, x))) return rc;
-        if ((rc = fetch_ctl(h))) return rc;
+        if ((rc = ark_fetch_ctl(h))) return rc;
     }
     return 0;
 }
@@ -721,7 +670,7 @@ static int bicgstab_solve(ark_m1* h, double tol, int maxit)
     KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
     CU(cudaMemsetAsync(y, 0, (size_t)n * sizeof(double), h->st));
     if ((rc = true_residual(h, x))) return rc;
-    if ((rc = fetch_ctl(h))) return rc;
+    if ((rc = ark_fetch_ctl(h))) return rc;
     while (!h->ctl_host->inner_stop) {
         const int its0 = h->ctl_host->its;
         KL(KC_UPDATE, 96.0 * h->N, launch_bicg_begin(r, rh, p, v, n, W, h->st));
@@ -741,7 +690,7 @@ static int bicgstab_solve(ark_m1* h, double tol, int maxit)
                 }
                 KL(KC_UPDATE, 168.0 * h->N, launch_bicg_xr(y, p, r, t, rh, n, W, sm, h->st));
             }
-            if ((rc = fetch_ctl(h))) return rc;
+            if ((rc = ark_fetch_ctl(h))) return rc;
             if (h->ctl_host->inner_stop) break;
         }
         if (h->precond == 1) {
@@ -751,14 +700,14 @@ static int bicgstab_solve(ark_m1* h, double tol, int maxit)
         } else
             KL(KC_COMBINE, 168.0 * h->N, launch_combine_y(h->g, h->A.Minv, y, x, h->st));
         if ((rc = true_residual(h, x))) return rc;      // resets inner_stop unless converged / out of iterations
-        if ((rc = fetch_ctl(h))) return rc;
+        if ((rc = ark_fetch_ctl(h))) return rc;
         if (h->ctl_host->its == its0) break;            // breakdown without progress
     }
     return 0;
 }
 
 // History copy, matter update, timings, error mapping shared by the implicit entry points.
-static int finish_implicit(ark_m1* h, double dt, double* final_residual)
+int ark_finish_implicit(ark_m1* h, double dt, double* final_residual)
 {
     GmresWork W = h->W;
     const GmresCtl c = *h->ctl_host;
@@ -769,11 +718,11 @@ static int finish_implicit(ark_m1* h, double dt, double* final_residual)
         KL(KC_SMALL, 40.0 * h->N, launch_matter_update(h->g, h->s, dt, h->sa, h->rho_cv, h->U[h->cur], h->T[h->cur], h->st));
     }
     CU(cudaStreamSynchronize(h->st));
-    kflush(h);
+    ark_kflush(h);
     float ms01 = 0, ms12 = 0;
     cudaEventElapsedTime(&ms01, h->ev[0], h->ev[1]); cudaEventElapsedTime(&ms12, h->ev[1], h->ev[2]);
     h->timings[0] = ms01; h->timings[1] = ms12; h->timings[2] = (double)ms01 + ms12;
-    if (c.nonfinite) return fail(h, ARK_M1_E_NONFINITE, "step_implicit: non-finite norm in the solver (state or opacity holds NaN/Inf?)%s", "");
+    if (c.nonfinite) return ark_fail(h, ARK_M1_E_NONFINITE, "step_implicit: non-finite norm in the solver (state or opacity holds NaN/Inf?)%s", "");
     if (final_residual) *final_residual = (c.bnorm > 0.0) ? c.rnorm / c.bnorm : c.rnorm;
     return 0;
 }
@@ -782,16 +731,17 @@ extern "C" int ark_m1_step_implicit(ark_m1* h, double dt, double tol, int restar
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit: no state set%s", "");
-    int rc = ensure_implicit(h, (h->krylov == 1 && restart < 5) ? 5 : restart, maxit);
+    NO_SLAB(h, "ark_m1_step_implicit");
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return ark_fail(h, ARK_M1_E_ARG, "step_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "step_implicit: no state set%s", "");
+    int rc = ark_ensure_implicit(h, (h->krylov == 1 && restart < 5) ? 5 : restart, maxit);
     if (rc) return rc;
     CU(cudaEventRecord(h->ev[0], h->st));
-    if ((rc = assemble_system(h, dt))) return rc;
+    if ((rc = ark_assemble_system(h, dt, nullptr))) return rc;
     CU(cudaEventRecord(h->ev[1], h->st));
     if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : (use_cb(h) ? gmres_solve_cb(h, tol, restart, maxit) : gmres_solve(h, tol, restart, maxit)))) return rc;
     CU(cudaEventRecord(h->ev[2], h->st));
-    if ((rc = finish_implicit(h, dt, final_residual))) return rc;
+    if ((rc = ark_finish_implicit(h, dt, final_residual))) return rc;
     return h->ctl_host->its;
 }
 
@@ -803,13 +753,14 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
+    NO_SLAB(h, "ark_m1_step_implicit_newton");
     if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0 || !(newton_tol >= 0.0) || max_newton < 1)
-        return fail(h, ARK_M1_E_ARG, "step_implicit_newton: need dt > 0, tol > 0, restart >= 1, maxit >= 0, newton_tol >= 0, max_newton >= 1%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_implicit_newton: no state set%s", "");
-    int rc = ensure_implicit(h, (h->krylov == 1 && restart < 5) ? 5 : restart, maxit);
+        return ark_fail(h, ARK_M1_E_ARG, "step_implicit_newton: need dt > 0, tol > 0, restart >= 1, maxit >= 0, newton_tol >= 0, max_newton >= 1%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "step_implicit_newton: no state set%s", "");
+    int rc = ark_ensure_implicit(h, (h->krylov == 1 && restart < 5) ? 5 : restart, maxit);
     if (rc) return rc;
     const size_t n = 3 * (size_t)h->N;
-    if (!h->nprev && (rc = dmalloc(h, (void**)&h->nprev, n * sizeof(double)))) return rc;
+    if (!h->nprev && (rc = ark_dmalloc(h, (void**)&h->nprev, n * sizeof(double)))) return rc;
     double* x = h->U[h->cur];
     double* base = h->U[h->cur ^ 1];                 // U^n lives in the other state buffer during the iteration
     CU(cudaMemcpyAsync(base, x, n * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
@@ -819,20 +770,20 @@ extern "C" int ark_m1_step_implicit_newton(ark_m1* h, double dt, double tol, int
     double upd = 0.0;
     for (k = 0; k < max_newton; ++k) {
         CU(cudaMemcpyAsync(h->nprev, x, n * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
-        if ((rc = assemble_system(h, dt, base))) return rc;
+        if ((rc = ark_assemble_system(h, dt, base))) return rc;
         if ((rc = (h->krylov == 1) ? bicgstab_solve(h, tol, maxit) : (use_cb(h) ? gmres_solve_cb(h, tol, restart, maxit) : gmres_solve(h, tol, restart, maxit)))) return rc;
         total += h->ctl_host->its;
         if (h->ctl_host->nonfinite) break;
         KL(KC_SMALL, 72.0 * h->N, launch_sub(h->nprev, x, h->nprev, (long long)n, h->st));
         KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->nprev, h->nprev, 0, 1, 0, (long long)n, h->W, DOT_AUX0, h->sm_count, h->st));
         KL(KC_DOT, 24.0 * h->N, launch_multi_dot(x, x, 0, 1, 0, (long long)n, h->W, DOT_AUX1, h->sm_count, h->st));
-        if ((rc = fetch_ctl(h))) return rc;
+        if ((rc = ark_fetch_ctl(h))) return rc;
         const double d = h->ctl_host->aux[0], nrm = h->ctl_host->aux[1];
         upd = (nrm > 0.0) ? d / nrm : d;
         if (upd <= newton_tol) { ++k; break; }
     }
     CU(cudaEventRecord(h->ev[2], h->st));
-    if ((rc = finish_implicit(h, dt, final_residual))) return rc;
+    if ((rc = ark_finish_implicit(h, dt, final_residual))) return rc;
     if (newton_iterations) *newton_iterations = k;
     if (final_update) *final_update = upd;
     return total;
@@ -844,19 +795,20 @@ extern "C" int ark_m1_step_semi_implicit(ark_m1* h, double dt, double tol, int r
 {
     if (!h) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return fail(h, ARK_M1_E_ARG, "step_semi_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "step_semi_implicit: no state set%s", "");
-    if (h->N >= (1LL << 31)) return fail(h, ARK_M1_E_UNSUPPORTED, "step_semi_implicit: grid too large for the marching kernels%s", "");
+    NO_SLAB(h, "ark_m1_step_semi_implicit");
+    if (!(dt > 0.0) || !(tol > 0.0) || restart < 1 || maxit < 0) return ark_fail(h, ARK_M1_E_ARG, "step_semi_implicit: need dt > 0, tol > 0, restart >= 1, maxit >= 0%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "step_semi_implicit: no state set%s", "");
+    if (h->N >= (1LL << 31)) return ark_fail(h, ARK_M1_E_UNSUPPORTED, "step_semi_implicit: grid too large for the marching kernels%s", "");
     {   // U* = U^n - dt div(flux): marching kernel with the sources off (T untouched)
         h->s.src_off = 1;
-        const Fields f = fields_of(h);
+        const Fields f = ark_fields_of(h);
         double* O = h->U[h->cur ^ 1];
-        kmark(h, KC_EXPLICIT, 64.0 * h->N);
+        ark_kmark(h, KC_EXPLICIT, 64.0 * h->N);
         cudaError_t e = (h->explicit_kernel == 3)
             ? launch_explicit_march3(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, nullptr, h->sm_count, h->st)
             : launch_explicit_march(h->g, h->s, f, dt, O, O + h->N, O + 2 * h->N, nullptr, h->sm_count, h->st);
         h->s.src_off = 0;
-        if (e != cudaSuccess) return fail(h, ARK_M1_E_CUDA, "launch_explicit_march: %s", cudaGetErrorString(e));
+        if (e != cudaSuccess) return ark_fail(h, ARK_M1_E_CUDA, "launch_explicit_march: %s", cudaGetErrorString(e));
         if (h->have_T) CU(cudaMemcpyAsync(h->T[h->cur ^ 1], h->T[h->cur], (size_t)h->N * sizeof(double), cudaMemcpyDeviceToDevice, h->st));
         h->cur ^= 1;
     }
@@ -870,12 +822,13 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
 {
     if (!h || !Vin || !out) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "apply_operator: dt must be > 0%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "apply_operator: no state set%s", "");
-    int rc = ensure_implicit(h, 1, 1);
+    NO_SLAB(h, "ark_m1_apply_operator");
+    if (!(dt > 0.0)) return ark_fail(h, ARK_M1_E_ARG, "apply_operator: dt must be > 0%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "apply_operator: no state set%s", "");
+    int rc = ark_ensure_implicit(h, 1, 1);
     if (rc) return rc;
     const size_t n = 3 * (size_t)h->N;
-    if ((rc = assemble_system(h, dt))) return rc;
+    if ((rc = ark_assemble_system(h, dt, nullptr))) return rc;
     double* vin = h->V;                       // slot 0 as staging for the input, slot 1 for the output
     double* vout = h->V + h->stride;
     CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
@@ -897,12 +850,13 @@ extern "C" int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* V
 {
     if (!h || !Vin || !out) return ARK_M1_E_ARG;
     GUARD(h);
-    if (!(dt > 0.0)) return fail(h, ARK_M1_E_ARG, "apply_preconditioner: dt must be > 0%s", "");
-    if (!h->have_state) return fail(h, ARK_M1_E_NOTSET, "apply_preconditioner: no state set%s", "");
-    int rc = ensure_implicit(h, 1, 1);
+    NO_SLAB(h, "ark_m1_apply_preconditioner");
+    if (!(dt > 0.0)) return ark_fail(h, ARK_M1_E_ARG, "apply_preconditioner: dt must be > 0%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "apply_preconditioner: no state set%s", "");
+    int rc = ark_ensure_implicit(h, 1, 1);
     if (rc) return rc;
     const size_t n = 3 * (size_t)h->N;
-    if ((rc = assemble_system(h, dt))) return rc;
+    if ((rc = ark_assemble_system(h, dt, nullptr))) return rc;
     double* vin = h->V;
     double* vout = h->V + h->stride;
     CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
@@ -915,7 +869,7 @@ extern "C" int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* V
     }
     CU(cudaMemcpyAsync(out, vout, n * sizeof(double), cudaMemcpyDefault, h->st));
     CU(cudaStreamSynchronize(h->st));
-    kflush(h);
+    ark_kflush(h);
     return 0;
 }
 
@@ -942,7 +896,7 @@ extern "C" int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap)
 {
     if (!h || !out) return ARK_M1_E_ARG;
     GUARD(h);
-    kflush(h);
+    ark_kflush(h);
     for (int k = 0; k < KC_COUNT && 3 * k + 2 < cap; ++k) for (int q = 0; q < 3; ++q) out[3 * k + q] = h->kstat[k][q];
     return KC_COUNT;
 }

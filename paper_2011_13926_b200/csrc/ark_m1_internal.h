@@ -39,6 +39,8 @@ struct GmresWork {                 // device pointers into one small allocation
     double* hist;   // caphist
     double* partial;// [max_blocks][MAXV] block partial sums
     int caphist;
+    double* red_out;// null: the reduction kernels run their scalar epilogue themselves (one GPU).  Non-null (slab decomposition):
+                    // they store this rank's sums here instead; all-reduce and launch_epilogue follow
 };
 
 enum { MAXV = 16 };                // basis vectors handled per pass of the multi-vector kernels (the measured optimum: DESIGN.md section 5)
@@ -83,6 +85,7 @@ struct MfPlanes {
     double* xlo;   // [4][ny] : west face of column 0 (non-periodic x)
     double* ylo;   // [4][nx] : south face of row 0 (non-periodic y)
     double rx, ry; // dt/dx, dt/dy of the assembled step
+    const double* halo[2];   // slab decomposition (BC_HALO sides): received (z, c^2 J z) of the row below / above, [6][nx] each
 };
 // A.off / A.C may be null when mf.J is set (then only Minv, b and the coefficient planes are written)
 // bsrc: planes [E|Fx|Fy] that supply the U^n part of the right-hand side (null: the state in `f`; non-null in Newton
@@ -96,6 +99,9 @@ cudaError_t launch_assemble_march(const Grid& g, const Scheme& s, const Fields& 
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
                          int sm_count, cudaStream_t st);
+// (z, c^2 J z) of the slab's first and last row for the neighbour ranks (out_lo / out_hi: [6][nx], either may be null)
+cudaError_t launch_halo_pack_zp(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, int precond,
+                                double* out_lo, double* out_hi, const int* skip_flag, cudaStream_t st);
 cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Minv, const float* v, double* out,
                              const double* scale_ptr, const int* skip_flag, int sm_count, cudaStream_t st);
 cudaError_t launch_scale_offdiag(const Grid& g, BlockMatrix A, float* off32, cudaStream_t st);   // off32: optional fp32 copy
@@ -137,6 +143,8 @@ cudaError_t launch_update(double* w, const double* V0, long long stride, int nv,
                           GmresWork W, int with_norm, int sm_count, cudaStream_t st);
 // the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
 cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
+// the scalar epilogue of reduction `mode` on nv sums d[0..nv) (device; after an all-reduce over the ranks)
+cudaError_t launch_epilogue(GmresWork W, int mode, int nv, int col0, const double* d, const int* skip_flag, cudaStream_t st);
 // x += Minv * (sum_{k<ctl->j} coef[k] V_k)  per cell;  Minv == nullptr: x = sum_{k<ctl->j} coef[k] V_k
 cudaError_t launch_combine(const Grid& g, const double* V, long long stride, const double* Minv, double* x,
                            GmresWork W, int sm_count, cudaStream_t st);

@@ -44,7 +44,7 @@ __device__ __forceinline__ Raw load_row_general(const Fields& f, const Grid& g, 
     if (xmode != 0) return r;                       // corner
     const int side = (j < 0) ? YLO : YHI;
     const int bc = g.bc[side];
-    if (bc == BC_DIRICHLET) {
+    if (bc == BC_DIRICHLET || bc == BC_HALO) {
         r.E = f.gh[side][0][ii]; r.Fx = f.gh[side][1][ii]; r.Fy = f.gh[side][2][ii]; r.sa = f.gh[side][3][ii]; r.st = f.gh[side][4][ii];
         return r;
     }
@@ -83,7 +83,7 @@ __device__ __forceinline__ void load_row_async(double (*ring)[TXN], int t, const
         } else if (xmode == 0) {
             const int side = (j < 0) ? YLO : YHI;
             const int bc = g.bc[side];
-            if (bc == BC_DIRICHLET) {
+            if (bc == BC_DIRICHLET || bc == BC_HALO) {
                 p0 = f.gh[side][0] + ii; p1 = f.gh[side][1] + ii; p2 = f.gh[side][2] + ii; p3 = f.gh[side][4] + ii; p4 = f.gh[side][3] + ii;
             } else {
                 const int jj = (bc == BC_PERIODIC) ? ((j < 0) ? g.ny - 1 : 0) : ((j < 0) ? 0 : g.ny - 1);

@@ -152,6 +152,13 @@ __device__ __forceinline__ void reduce_and_finish(double (&acc)[NV], const Gmres
         s = warp_sum(s);
         if (lane == 0) dres[k] = s;
     }
+    if (W.red_out) {
+        // domain-decomposed solve (dist.cu): this rank's sums go to W.red_out; the all-reduce over the ranks and the scalar
+        // epilogue (launch_epilogue) follow as separate steps on the stream
+        __syncthreads();
+        if (threadIdx.x < NV) W.red_out[threadIdx.x] = dres[threadIdx.x];
+        return;
+    }
     if constexpr (STAGE) if (mode == DOT_UPD) {
         // stage column j of H (rows 0..j; row j+1 is ||w|| itself), cs and sn for the scalar epilogue
         __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];

@@ -182,6 +182,28 @@ cudaError_t launch_update(double* w, const double* V0, long long stride, int nv,
     return cudaGetLastError();
 }
 
+// Scalar epilogue as a kernel of its own (slab decomposition: the sums were all-reduced over the ranks in between).
+__global__ void __launch_bounds__(128) epilogue_kernel(GmresWork W, int mode, int nv, int col0, const double* __restrict__ d, const int* __restrict__ skip_flag)
+{
+    if (skip_flag && *skip_flag) return;
+    __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX], dd[MAXV];
+    if (threadIdx.x < nv) dd[threadIdx.x] = d[threadIdx.x];
+    bool staged = false;
+    if (mode == DOT_UPD) {
+        const int j = W.ctl->j, m = W.ctl->m;
+        staged = (j < EPI_MAX);
+        if (staged) for (int i = threadIdx.x; i <= j; i += blockDim.x) { hcol[i] = W.H[i * m + j]; if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; } }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) epilogue(W, mode, dd, nv, col0, staged ? hcol : nullptr, ccs, ssn);
+}
+
+cudaError_t launch_epilogue(GmresWork W, int mode, int nv, int col0, const double* d, const int* skip_flag, cudaStream_t st)
+{
+    epilogue_kernel<<<1, 128, 0, st>>>(W, mode, nv, col0, d, skip_flag);
+    return cudaGetLastError();
+}
+
 // Cycle end: back substitution H y = g over the ctl->j columns built in this cycle; coef_i = y_i scale_i.
 __global__ void solve_y_kernel(GmresWork W)
 {

@@ -20,7 +20,11 @@
 
 namespace ark {
 
-enum { BC_PERIODIC = 0, BC_DIRICHLET = 1, BC_OUTFLOW = 2 };
+// BC_HALO (internal, y sides of a slab of the domain-decomposed step, dist.cu): the ghost line holds the neighbour rank's
+// boundary row, refreshed by the halo exchange.  For the closure/flux kernels it is a Dirichlet ghost (a ghost enters like an
+// interior cell, R9); for the linear system it is an UNKNOWN: nothing moves to b, and the operator takes the
+// neighbour's z = M^-1 v and c^2 J z from the halo buffer of MfPlanes.
+enum { BC_PERIODIC = 0, BC_DIRICHLET = 1, BC_OUTFLOW = 2, BC_HALO = 3 };
 enum { XLO = 0, XHI = 1, YLO = 2, YHI = 3 };
 
 struct Scheme {

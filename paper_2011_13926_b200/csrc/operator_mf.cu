@@ -32,9 +32,12 @@ struct FC { double ap, Lam, alpha, sw; };            // face coefficients; sw = 
 
 // z and Pi of the cell in column (xmode, ii) and row j (j may be -1 or ny).  Dirichlet ghosts carry z = 0 (their
 // contribution is in b), outflow ghosts copy the adjacent cell, periodic ghosts wrap (R9).
+// Halo ghosts (BC_HALO, slab decomposition) carry the neighbour rank's (z, c^2 J z), packed by halo_pack_zp_kernel and exchanged
+// before the launch: halo[0] = row below the slab, halo[1] = row above, six lines of nx doubles each.
 template <bool PRECOND, typename TIN>
 __device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const TIN* __restrict__ v, const double* __restrict__ Minv,
-                                      const double* __restrict__ J, double c2, int xmode, int ii, int j)
+                                      const double* __restrict__ J, double c2, int xmode, int ii, int j,
+                                      const double* __restrict__ halo_lo, const double* __restrict__ halo_hi)
 {
     ZP r; r.zE = 0.0; r.zFx = 0.0; r.zFy = 0.0; r.Pxx = 0.0; r.Pxy = 0.0; r.Pyy = 0.0; r.v0 = 0.0; r.v1 = 0.0; r.v2 = 0.0;
     if (xmode != 0) return r;
@@ -42,6 +45,12 @@ __device__ __forceinline__ ZP load_zp(const Grid& g, long long N, const TIN* __r
     if (j < 0 || j >= g.ny) {
         const int bc = g.bc[(j < 0) ? YLO : YHI];
         if (bc == BC_DIRICHLET) return r;
+        if (bc == BC_HALO) {
+            const double* hz = (j < 0) ? halo_lo : halo_hi;
+            r.zE = hz[ii]; r.zFx = hz[g.nx + ii]; r.zFy = hz[2 * g.nx + ii];
+            r.Pxx = hz[3 * g.nx + ii]; r.Pxy = hz[4 * g.nx + ii]; r.Pyy = hz[5 * g.nx + ii];
+            return r;
+        }
         jj = (bc == BC_PERIODIC) ? ((j < 0) ? g.ny - 1 : 0) : ((j < 0) ? 0 : g.ny - 1);
     }
     const long long id = (long long)jj * g.nx + ii;
@@ -99,8 +108,8 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
     const bool east_valid = (i < g.nx) && (xmode != 2);    // this thread owns the face between columns i and i+1
     const double sc = sgn * (scale_ptr ? *scale_ptr : 1.0);
 
-    ZP zS = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0 - 1);
-    ZP zC = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0);
+    ZP zS = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0 - 1, mf.halo[0], mf.halo[1]);
+    ZP zC = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0, mf.halo[0], mf.halo[1]);
     double Hs0 = 0.0, Hs1 = 0.0, Hs2 = 0.0, Ss = 0.0;
     if (upd) {
         // south face of row j0: the north face of row j0-1, or the stored low-side line / the wrapped last row
@@ -114,7 +123,7 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
     for (int j = j0; j < j1; ++j) {
         // issue every global load of this row first (north cell, face coefficients, source weights); they are consumed
         // after the two barriers of the x-face exchange, which needs only data already in registers
-        const ZP zN = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j + 1);
+        const ZP zN = load_zp<PRECOND, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j + 1, mf.halo[0], mf.halo[1]);
         const long long id = (long long)j * g.nx + (upd ? i : 0);
         FC fn; fn.ap = 0.5; fn.Lam = 0.0; fn.alpha = 1.0; fn.sw = 0.0;
         double dE = 0.0, dF = 0.0, a0 = 0.0, a1 = 0.0, a2 = 0.0;
@@ -192,6 +201,34 @@ cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Mi
     const double c2 = g.c * g.c;
     GmresWork none; memset(&none, 0, sizeof none);
     op_mf_kernel<true, 0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    return cudaGetLastError();
+}
+
+// Slab decomposition: what the neighbour ranks need of this slab for one operator application — (z, c^2 J z) of the first row
+// (sent to the rank below) and of the last row (sent to the rank above): out_lo, out_hi = six lines of nx doubles each.
+template <bool PRECOND>
+__global__ void halo_pack_zp_kernel(Grid g, const double* __restrict__ J, const double* __restrict__ Minv, const double* __restrict__ v,
+                                    double c2, double* __restrict__ out_lo, double* __restrict__ out_hi, const int* __restrict__ skip_flag)
+{
+    if (skip_flag && *skip_flag) return;
+    const long long N = (long long)g.nx * g.ny;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < g.nx; i += gridDim.x * blockDim.x) {
+        for (int side = 0; side < 2; ++side) {
+            double* o = side == 0 ? out_lo : out_hi;
+            if (!o) continue;
+            const ZP r = load_zp<PRECOND, double>(g, N, v, Minv, J, c2, 0, i, side == 0 ? 0 : g.ny - 1, nullptr, nullptr);
+            o[i] = r.zE; o[g.nx + i] = r.zFx; o[2 * g.nx + i] = r.zFy; o[3 * g.nx + i] = r.Pxx; o[4 * g.nx + i] = r.Pxy; o[5 * g.nx + i] = r.Pyy;
+        }
+    }
+}
+
+cudaError_t launch_halo_pack_zp(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, int precond,
+                                double* out_lo, double* out_hi, const int* skip_flag, cudaStream_t st)
+{
+    const int blk = 128, grd = (g.nx + blk - 1) / blk;
+    const double c2 = g.c * g.c;
+    if (precond) halo_pack_zp_kernel<true><<<grd, blk, 0, st>>>(g, mf.J, Minv, v, c2, out_lo, out_hi, skip_flag);
+    else halo_pack_zp_kernel<false><<<grd, blk, 0, st>>>(g, mf.J, Minv, v, c2, out_lo, out_hi, skip_flag);
     return cudaGetLastError();
 }
 
