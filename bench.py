@@ -704,6 +704,114 @@ def run_ours(args):
     return 0
 
 
+def run_decomposed(args):
+    """Strong-scaling form of the same step: ONE global grid cut into y-slabs (include/ark_m1.h "Domain-decomposed step").
+    Under torchrun: one slab per rank and GPU, halos and Gram-Schmidt sums over NCCL.  With --decomposed-local R on one GPU: R slabs
+    in this process (the emulated form the tests use): measures what the decomposition itself costs (extra launches, halo packing)."""
+    import torch
+    import torch.distributed as dist
+    import paper_2011_13926_b200 as ark
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the CUDA library is the only implementation (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    n = args.n
+    N = n * n
+    w = wl.random_medium(n, seed=args.seed)           # the SAME global problem on every rank; each keeps its rows
+    dt_e = wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    stream = torch.cuda.current_stream()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+        box = [ark.nccl_unique_id() if rank == 0 else None]
+        dist.broadcast_object_list(box, src=0)
+        grp = ark.ArkM1Group(n, n, w["dx"], w["dy"], w["c"], bc=w["bc"], nranks=world, kind="nccl", rank=rank, unique_id=box[0], stream=stream)
+        nslab_total, kind = world, "nccl"
+    else:
+        grp = ark.ArkM1Group(n, n, w["dx"], w["dy"], w["c"], bc=w["bc"], nranks=args.decomposed_local, kind="local", stream=stream)
+        nslab_total, kind = args.decomposed_local, "local"
+    peak_gbs, peak_src = peaks()
+    devs = []
+    for s_ in grp.slabs:
+        rows = slice(s_.y0, s_.y1)
+        devs.append({k: torch.from_numpy(np.ascontiguousarray(np.asarray(w[k])[..., rows, :])).to(dev) for k in ("E", "F", "sigma_a", "sigma_s")})
+
+    def reset():
+        for s_, d_ in zip(grp.slabs, devs):
+            s_.set_state(d_["E"], d_["F"], d_["sigma_a"], d_["sigma_s"])
+
+    def one_step():
+        grp.step_explicit(dt_e)
+        return grp.step_implicit(BENCH_DT_RATIO * dt_e, TOL, RESTART, MAXIT)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        reset(); one_step()
+    st0 = grp.comm_stats()
+    l0 = sum(s_.kernel_launches() for s_ in grp.slabs)
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    its = 0
+    for _ in range(args.steps):
+        reset()
+        its, res = one_step()
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    elapsed = e0.elapsed_time(e1) * 1e-3
+    st1 = grp.comm_stats()
+    launches = sum(s_.kernel_launches() for s_ in grp.slabs) - l0
+    # explicit alone, sustained for ~1 s
+    reset()
+    grp.step_explicit(dt_e)
+    barrier()
+    n_e = 400
+    e0.record(stream)
+    for _ in range(n_e):
+        grp.step_explicit(dt_e)
+    e1.record(stream)
+    barrier()
+    t_exp = e0.elapsed_time(e1) / n_e
+    t_max, _ = aggregate_over_ranks(elapsed, 0.0, dist if world > 1 else None)
+    t_exp_max, _ = aggregate_over_ranks(t_exp, 0.0, dist if world > 1 else None)
+    if rank == 0:
+        halo_per_step = (st1["halo_bytes"] - st0["halo_bytes"]) / args.steps
+        interior = iteration_bytes_per_cell(its, operator=1) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
+        line = {
+            "metric": METRIC, "value": 2.0 * N * args.steps / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": f"M1 random medium (BASELINE.json configs[3]) {n}x{n}, fp64, periodic, c=1, seed {args.seed}: ONE global grid "
+                                   f"in {nslab_total} y-slabs ({kind} transport)",
+                       "step": "state reset (D2D) + 1 explicit step (CFL 0.4) + 1 implicit step (dt = 10x explicit, GMRES(30) + block-Jacobi, tol 1e-10)",
+                       "iterations_per_implicit_step": its, "final_residual": res,
+                       "parallelism": f"domain decomposition, {nslab_total} slabs of {n // nslab_total} rows, 1-cell halos, all-reduced Gram-Schmidt sums",
+                       "l2": "inputs larger than L2"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "explicit": {"ms_per_step": t_exp_max, "cell_updates_per_s": N / (t_exp_max * 1e-3), "hbm_frac_per_gpu": 64.0 * N / max(world, 1) / (t_exp_max * 1e-3) / 1e9 / peak_gbs},
+            "communication": {"halo_bytes_sent_per_step_this_rank": halo_per_step, "exchanges_per_step": (st1["exchanges"] - st0["exchanges"]) / args.steps,
+                              "allreduces_per_step": (st1["allreduces"] - st0["allreduces"]) / args.steps,
+                              "interior_algorithmic_bytes_per_step_per_slab": interior, "halo_over_interior": halo_per_step / interior},
+            "e2e": None,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    grp.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -719,6 +827,8 @@ def main():
     ap.add_argument("--mg-precision", type=int, default=32, choices=[32, 64], help="storage precision of the multigrid blocks")
     ap.add_argument("--no-sweep", action="store_true", help="skip the dt = 50/100/200x implicit solves")
     ap.add_argument("--sustain-s", type=float, default=2.0, help="length of the sustained back-to-back explicit run, seconds")
+    ap.add_argument("--decomposed", action="store_true", help="under torchrun: ONE global grid cut into y-slabs, one per rank, halos and sums over NCCL (strong scaling) instead of independent replicas")
+    ap.add_argument("--decomposed-local", type=int, default=0, metavar="R", help="one GPU: the same global grid in R slabs inside this process (what the decomposition itself costs)")
     ap.add_argument("--restart-sweep", action="store_true", help="also sweep the GMRES restart length (30/60/100) at 50/100/200x on the bench medium and at 1024^2 (takes ~3 min)")
     ap.add_argument("--oracle-protocol", action="store_true", help="also time the oracle as SURVEY 8(d) lists it: explicit alone and one capped GMRES cycle at the bench size, all cores and 1 thread (takes several minutes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -730,6 +840,8 @@ def main():
         print(f"bench.py: note: warmup {args.warmup} < 3 (timing rule wants >= 3)", file=sys.stderr)
     if args.impl == "reference":
         return run_reference(args)
+    if args.decomposed or args.decomposed_local > 1:
+        return run_decomposed(args)
     return run_ours(args)
 
 
