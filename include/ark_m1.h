@@ -267,6 +267,28 @@ ARK_M1_API int ark_m1_group_step_implicit(ark_m1_group* g, double dt, double tol
 ARK_M1_API int ark_m1_group_comm_stats(const ark_m1_group* g, long long* halo_bytes, long long* exchanges, long long* allreduces);
 ARK_M1_API const char* ark_m1_group_last_error(const ark_m1_group* g);
 
+/* ---------------------------------------------------------------------------------------------------------------------------
+ * Three space dimensions ("its extension to higher dimensions is straightforward"; (2+d)N unknowns):
+ * the same scheme direction by direction on (E, Fx, Fy, Fz), 7-point stencil, explicit step and one linearised implicit step
+ * solved by GMRES(restart) right-preconditioned with the 4x4 diagonal blocks.  Generic kernels (one thread per cell).
+ * Arrays: planes [nz][ny][nx], x fastest; F = [Fx | Fy | Fz] (3 nx ny nz doubles); host or device pointers.
+ * Boundaries: ARK_M1_BC_PERIODIC or ARK_M1_BC_OUTFLOW per side.  Arguments, return values and error behaviour as the 2-D calls.
+ * --------------------------------------------------------------------------------------------------------------------------- */
+typedef struct ark_m1_3d ark_m1_3d;
+typedef struct { int xlo, xhi, ylo, yhi, zlo, zhi; } ark_m1_bc3;
+ARK_M1_API ark_m1_3d* ark_m1_3d_create(int nx, int ny, int nz, double dx, double dy, double dz, double c, const ark_m1_bc3* bc);
+ARK_M1_API void ark_m1_3d_destroy(ark_m1_3d* h);
+ARK_M1_API int ark_m1_3d_set_stream(ark_m1_3d* h, void* cuda_stream);
+ARK_M1_API int ark_m1_3d_set_state(ark_m1_3d* h, const double* E, const double* F, const double* sigma_a, const double* sigma_s);
+ARK_M1_API int ark_m1_3d_get_state(ark_m1_3d* h, double* E, double* F);
+ARK_M1_API int ark_m1_3d_step_explicit(ark_m1_3d* h, double dt);
+ARK_M1_API int ark_m1_3d_step_implicit(ark_m1_3d* h, double dt, double tol, int restart, int maxit, double* final_residual);
+/* out = A V (precond == 0) or A M^-1 V (precond != 0), A = I + dt L_n of the stored state, through the solver's own assembly and
+ * operator kernels; V, out: 4 nx ny nz doubles [E | Fx | Fy | Fz].  Synchronises. */
+ARK_M1_API int ark_m1_3d_apply_operator(ark_m1_3d* h, double dt, const double* V, double* out, int precond);
+ARK_M1_API long long ark_m1_3d_kernel_launches(const ark_m1_3d* h);
+ARK_M1_API const char* ark_m1_3d_last_error(const ark_m1_3d* h);
+
 /* Device bytes currently allocated by the handle. */
 ARK_M1_API long long ark_m1_device_bytes(const ark_m1* h);
 

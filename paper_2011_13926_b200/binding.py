@@ -29,6 +29,8 @@ SYMBOLS = [
     "ark_m1_slab_range", "ark_m1_group_create_local", "ark_m1_group_create_host", "ark_m1_nccl_unique_id", "ark_m1_group_create_nccl",
     "ark_m1_group_destroy", "ark_m1_group_set_stream", "ark_m1_group_local_slabs", "ark_m1_group_slab", "ark_m1_group_step_explicit",
     "ark_m1_group_step_implicit", "ark_m1_group_comm_stats", "ark_m1_group_last_error",
+    "ark_m1_3d_create", "ark_m1_3d_destroy", "ark_m1_3d_set_stream", "ark_m1_3d_set_state", "ark_m1_3d_get_state", "ark_m1_3d_step_explicit",
+    "ark_m1_3d_step_implicit", "ark_m1_3d_apply_operator", "ark_m1_3d_kernel_launches", "ark_m1_3d_last_error",
 ]
 
 
@@ -39,6 +41,10 @@ class ArkBc(C.Structure):
 _SENDRECV = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
                         C.POINTER(C.c_double), C.c_longlong)
 _ALLREDUCE = C.CFUNCTYPE(C.c_int, C.c_void_p, C.POINTER(C.c_double), C.c_int)
+
+
+class ArkBc3(C.Structure):
+    _fields_ = [("xlo", C.c_int), ("xhi", C.c_int), ("ylo", C.c_int), ("yhi", C.c_int), ("zlo", C.c_int), ("zhi", C.c_int)]
 
 
 class ArkHostTransport(C.Structure):
@@ -114,6 +120,20 @@ def load_library(path: str | None = None):
     L.ark_m1_group_comm_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.ark_m1_group_last_error.restype = C.c_char_p
     L.ark_m1_group_last_error.argtypes = [vp]
+    L.ark_m1_3d_create.restype = vp
+    L.ark_m1_3d_create.argtypes = [i, i, i, d, d, d, d, C.POINTER(ArkBc3)]
+    L.ark_m1_3d_destroy.restype = None
+    L.ark_m1_3d_destroy.argtypes = [vp]
+    L.ark_m1_3d_set_stream.argtypes = [vp, vp]
+    L.ark_m1_3d_set_state.argtypes = [vp, dp, dp, dp, dp]
+    L.ark_m1_3d_get_state.argtypes = [vp, dp, dp]
+    L.ark_m1_3d_step_explicit.argtypes = [vp, d]
+    L.ark_m1_3d_step_implicit.argtypes = [vp, d, d, i, i, C.POINTER(C.c_double)]
+    L.ark_m1_3d_apply_operator.argtypes = [vp, d, dp, dp, i]
+    L.ark_m1_3d_kernel_launches.restype = C.c_longlong
+    L.ark_m1_3d_kernel_launches.argtypes = [vp]
+    L.ark_m1_3d_last_error.restype = C.c_char_p
+    L.ark_m1_3d_last_error.argtypes = [vp]
     for name in SYMBOLS:
         getattr(L, name)
     _lib = L
@@ -435,6 +455,64 @@ class ArkM1Group:
         a, b, c_ = C.c_longlong(0), C.c_longlong(0), C.c_longlong(0)
         self._check(self._L.ark_m1_group_comm_stats(self._g, C.byref(a), C.byref(b), C.byref(c_)))
         return dict(halo_bytes=a.value, exchanges=b.value, allreduces=c_.value)
+
+
+class ArkM1_3D:
+    """The 3-D solver (include/ark_m1.h "Three space dimensions").  Arrays [nz, ny, nx]; F is [3, nz, ny, nx]."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, c=1.0, bc=(0, 0, 0, 0, 0, 0), stream=None):
+        self._L = load_library()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        b = ArkBc3(*[int(v) for v in bc])
+        self._h = self._L.ark_m1_3d_create(self.nx, self.ny, self.nz, float(dx), float(dy), float(dz), float(c), C.byref(b))
+        if not self._h:
+            raise ValueError("ark_m1_3d_create failed (bad arguments or no CUDA device)")
+        if stream is not None:
+            self._check(self._L.ark_m1_3d_set_stream(self._h, C.c_void_p(getattr(stream, "cuda_stream", stream))))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.ark_m1_3d_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _check(self, rc):
+        if rc < 0:
+            raise RuntimeError(f"ark_m1_3d error {rc}: {self._L.ark_m1_3d_last_error(self._h).decode()}")
+        return rc
+
+    @property
+    def N(self):
+        return self.nx * self.ny * self.nz
+
+    def set_state(self, E, F, sigma_a, sigma_s):
+        N = self.N
+        pe, k0 = _ptr(E, N); pf, k1 = _ptr(F, 3 * N); pa, k2 = _ptr(sigma_a, N); ps, k3 = _ptr(sigma_s, N)
+        self._check(self._L.ark_m1_3d_set_state(self._h, pe, pf, pa, ps))
+        self._keep = (k0, k1, k2, k3)
+
+    def get_state(self):
+        E = np.empty((self.nz, self.ny, self.nx)); F = np.empty((3, self.nz, self.ny, self.nx))
+        self._check(self._L.ark_m1_3d_get_state(self._h, E.ctypes.data, F.ctypes.data))
+        return E, F
+
+    def step_explicit(self, dt):
+        self._check(self._L.ark_m1_3d_step_explicit(self._h, float(dt)))
+
+    def step_implicit(self, dt, tol=1e-10, restart=30, maxit=4000):
+        res = C.c_double(0.0)
+        its = self._check(self._L.ark_m1_3d_step_implicit(self._h, float(dt), float(tol), int(restart), int(maxit), C.byref(res)))
+        return its, res.value
+
+    def apply_operator(self, dt, V, precond=False):
+        p, keep = _ptr(V, 4 * self.N)
+        out = np.empty((4, self.nz, self.ny, self.nx))
+        self._check(self._L.ark_m1_3d_apply_operator(self._h, float(dt), p, out.ctypes.data, int(bool(precond))))
+        return out
+
+    def kernel_launches(self):
+        return int(self._L.ark_m1_3d_kernel_launches(self._h))
 
 
 def nccl_unique_id():
