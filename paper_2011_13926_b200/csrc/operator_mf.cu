@@ -6,16 +6,22 @@
 //   = 18 doubles against the 36 of the pre-multiplied block stencil; with M^-1 (9), v (3) and out (3):
 //   264 B per cell per application instead of 336.
 //
-// Organisation = the explicit march kernel's: a block owns a strip of TXO-2 columns (+1 halo column each side) and
+// Organisation = the explicit march kernel's: a block is ONE warp that owns a strip of 30 columns (+1 halo lane each side) and
 // marches over the rows; a thread keeps z = M^-1 v and Pi = c^2 J z of its cell in rows j and j+1 in registers (the
-// y-face flux needs no other thread; the north flux of row j is the south flux of row j+1); x-faces go through
-// shared memory: publish (z, Pi_xx, Pi_xy), compute the EAST flux, publish it, read the WEST flux from the left thread.
+// y-face flux needs no other thread; the north flux of row j is the south flux of row j+1); x-faces go through warp
+// shuffles: take (z, Pi_xx, Pi_xy) of the east lane, compute the EAST flux, hand it to the east lane as its WEST flux.
+// No shared memory, no barrier: the kernel is a latency-bound stream (ncu: 75 % of the stall samples wait for global loads),
+// and many small independent blocks keep more loads in flight than a few 128-thread blocks that meet at two barriers per row
+// (128 / 64 / 32 columns at 4096^2: 5.82 / 6.21 / 6.51 TB/s on the same box).
 #include <string.h>
 #include "krylov_device.cuh"
 
 namespace ark {
 
-static constexpr int TXO = 128;
+static constexpr int TXO = 32;         // one warp per block: the x-face exchange is done by warp shuffles, no barrier
+static constexpr int OP_RY = 32;       // rows per block (cap)
+static constexpr int OP_MINB = 24;     // resident blocks per SM asked of ptxas (80 registers): 32 rows x 16 / 20 / 24 blocks: 5.96 / 6.45 / 6.51 TB/s;
+                                       // 28 and 32 blocks spill (5.4-5.7); 48-256 rows: 6.15-6.48
 
 struct ZP { double zE, zFx, zFy, Pxx, Pxy, Pyy, v0, v1, v2; };   // z = [M^-1] v, c^2 J z and the raw input v of one cell
 struct FC { double ap, Lam, alpha, sw; };            // face coefficients; sw = c dt sigma_f / 4
@@ -79,15 +85,13 @@ struct ZPub { double zE, zFx, zFy, Pxx, Pxy; };
 // 2: <out, v>, <out, out> -> epilogue BICG_OMEGA (v = the kernel's own input, already in registers).
 // TIN = float: the input vector is a single-precision (compressed) Krylov basis vector (krylov_cb.cu); all arithmetic is fp64.
 template <bool PRECOND, int DOT, typename TIN = double>
-__global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
+__global__ void __launch_bounds__(TXO, DOT ? 16 : OP_MINB) op_mf_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
                                                     double* __restrict__ out, const double* __restrict__ scale_ptr,
                                                     const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
                                                     int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W)
 {
     if (skip_flag && *skip_flag) return;
     double acc[2] = { 0.0, 0.0 };
-    __shared__ ZPub pub[TXO + 1];
-    __shared__ double flx[4][TXO];
     const int t = threadIdx.x;
     const int i = blockIdx.x * (TXO - 2) - 1 + t;
     const int j0 = blockIdx.y * RY;
@@ -139,18 +143,18 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
             if (use_xlo || xmode == 1) { if (i < 0) fe = load_fc(mf.xlo, g.ny, j); }
             else fe = load_fc(mf.fE, N, (long long)j * g.nx + ii);
         }
+        // x-face exchange inside the warp: lane t takes the x-face data of lane t+1, computes its EAST flux, and hands it to
+        // lane t+1 as that lane's WEST flux
         ZPub me; me.zE = zC.zE; me.zFx = zC.zFx; me.zFy = zC.zFy; me.Pxx = zC.Pxx; me.Pxy = zC.Pxy;
-        pub[t] = me;
-        __syncthreads();
         double Ge0, Ge1, Ge2, Se;
         {
-            const ZPub R = pub[t + 1];
+            ZPub R;
+            R.zE = __shfl_down_sync(0xffffffffu, me.zE, 1); R.zFx = __shfl_down_sync(0xffffffffu, me.zFx, 1); R.zFy = __shfl_down_sync(0xffffffffu, me.zFy, 1);
+            R.Pxx = __shfl_down_sync(0xffffffffu, me.Pxx, 1); R.Pxy = __shfl_down_sync(0xffffffffu, me.Pxy, 1);
             ARK_LIN_FLUX(fe, me.zE, R.zE, me.zFx, R.zFx, me.zFy, R.zFy, me.Pxx, R.Pxx, me.Pxy, R.Pxy, Ge0, Ge1, Ge2, Se);
         }
-        flx[0][t] = Ge0; flx[1][t] = Ge1; flx[2][t] = Ge2; flx[3][t] = Se;
-        __syncthreads();
-        const int tw = (t > 0) ? t - 1 : 0;
-        const double Gw0 = flx[0][tw], Gw1 = flx[1][tw], Gw2 = flx[2][tw], Sw = flx[3][tw];
+        const double Gw0 = __shfl_up_sync(0xffffffffu, Ge0, 1), Gw1 = __shfl_up_sync(0xffffffffu, Ge1, 1);
+        const double Gw2 = __shfl_up_sync(0xffffffffu, Ge2, 1), Sw = __shfl_up_sync(0xffffffffu, Se, 1);
         // north face (own column)
         double Hn0, Hn1, Hn2, Sn;
         ARK_LIN_FLUX(fn, zC.zE, zN.zE, zC.zFy, zN.zFy, zC.zFx, zN.zFx, zC.Pyy, zN.Pyy, zC.Pxy, zN.Pxy, Hn0, Hn2, Hn1, Sn);
@@ -173,8 +177,8 @@ __global__ void __launch_bounds__(TXO) op_mf_kernel(Grid g, MfPlanes mf, const d
 static dim3 op_mf_grid(const Grid& g, int sm_count, int* RYout)
 {
     const int strips = (g.nx + (TXO - 2) - 1) / (TXO - 2);
-    long long want = ((long long)g.ny * strips + (long long)sm_count * 16 - 1) / ((long long)sm_count * 16);
-    int RY = (int)(want < 4 ? 4 : (want > 64 ? 64 : want));
+    long long want = ((long long)g.ny * strips + (long long)sm_count * 64 - 1) / ((long long)sm_count * 64);
+    int RY = (int)(want < 4 ? 4 : (want > OP_RY ? OP_RY : want));
     if (RY > g.ny) RY = g.ny;
     *RYout = RY;
     return dim3(strips, (g.ny + RY - 1) / RY);
