@@ -45,7 +45,7 @@ TOL, RESTART, MAXIT = 1e-10, 30, 4000
 BENCH_DT_RATIO = 10.0
 SWEEP = (10.0, 50.0, 100.0, 200.0)
 PAPER_BREAK_EVEN = "50-100x (relaxation preconditioner; CPU 50, K80 GPU 100; PAPER.md:369)"
-FP64_INSTR_PER_CELL = 157       # fp64-pipe instructions (DFMA/DMUL/DADD/DSETP) per cell in the row loop of explicit_march3_kernel (SASS count)
+FP64_INSTR_PER_CELL = 156       # fp64-pipe instructions (DFMA/DMUL/DADD/DSETP) per cell in the row loop of explicit_march3_kernel (SASS count)
 
 
 def load_ncu_traffic():
@@ -365,7 +365,7 @@ def run_ours(args):
                              "frac_sustained": alu_work / (sus_ms * 1e-3) / alu_peak, "frac_burst": alu_work / (best * 1e-3) / alu_peak,
                              "peak_source": "ark_m1_fp64_issue_rate on this GPU in this run: DFMA lanes/clk/SM x SMs x SM clock measured during the test",
                              "issue_rates": rates},
-                     "bound": "fp64 issue (DESIGN.md section 6): 157 fp64 + 110 other instructions per cell"}
+                     "bound": "fp64 issue (DESIGN.md section 6): 156 fp64 + 106 other instructions per cell"}
 
     # ---- main timed region: W warm-up + exactly K steps, inputs resident in HBM ----------------------------------
     for _ in range(args.warmup):
