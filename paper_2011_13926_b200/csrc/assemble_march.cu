@@ -14,11 +14,9 @@
 
 namespace ark {
 
-#ifndef ARK_ASM_TX
-#define ARK_ASM_TX 32      // one warp per block, like the explicit kernel: 1.104 -> 1.059 ms at 4096^2 (128 -> 64 -> 32 columns: 0.668 / 0.689 / 0.697 of HBM peak; with the shuffle exchange 1.008 ms = 0.73)
-#endif
-static constexpr int TXA = ARK_ASM_TX;
-__device__ __forceinline__ void asm_sync() { if (TXA == 32) __syncwarp(); else __syncthreads(); }
+// one warp per block, like the explicit kernel: 1.104 -> 1.059 ms at 4096^2 (128 -> 64 -> 32 columns: 0.668 / 0.689 / 0.697 of HBM peak);
+// with the shuffle exchange 1.008 ms = 0.73
+static constexpr int TXA = 32;
 
 struct ACell {                 // one cell: raw state, closure, Jacobian
     Raw u;
@@ -47,8 +45,6 @@ template <bool SD>
 __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, Fields f, double dt, BlockMatrix A, MfPlanes mf,
                                                              const double* __restrict__ bsrc, int RY)
 {
-    __shared__ APub pub[TXA + 1];
-    __shared__ double fcs[5][TXA];          // east-face coefficients of every thread: a+, a-, Lambda, alpha, sigma_f
     const int t = threadIdx.x;
     const int i = blockIdx.x * (TXA - 2) - 1 + t;
     const int j0 = blockIdx.y * RY;
@@ -88,7 +84,6 @@ __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, F
         const Raw uNN = load_row(f, g, (j + 1 < j1) ? xmode : 2, ii, xside, j + 2);
         APub me; me.E = C.u.E; me.Fx = C.u.Fx; me.Fy = C.u.Fy; me.Pxx = C.q.Pxx; me.Pxy = C.q.Pxy;
         me.lmin = C.q.lmin[0]; me.lmax = C.q.lmax[0]; me.f = C.q.f; me.st = C.u.st;
-#if ARK_ASM_TX == 32
         // one-warp block: the neighbours' x-face data and the west face's coefficients travel by warp shuffles
         APub R, L;
         R.E = shfl_dn1(me.E); R.Fx = shfl_dn1(me.Fx); R.Fy = shfl_dn1(me.Fy); R.Pxx = shfl_dn1(me.Pxx); R.Pxy = shfl_dn1(me.Pxy);
@@ -101,22 +96,6 @@ __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, F
         face_eval<SD, true>(s, c, g.dx, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
         Face fw; fw.ap = shfl_up1(fe.ap); fw.am = shfl_up1(fe.am); fw.Lam = shfl_up1(fe.Lam); fw.alpha = shfl_up1(fe.alpha); fw.sig = shfl_up1(fe.sig);
         if (upd) {
-#else
-        pub[t] = me;
-        closure_eval<true, SD, true>(s, c, Nn.u.E, Nn.u.Fx, Nn.u.Fy, Nn.q, &Nn.J);
-        Face fn;
-        face_eval<SD, true>(s, c, g.dy, C.q.lmin[1], C.q.lmax[1], C.q.f, C.u.st, Nn.q.lmin[1], Nn.q.lmax[1], Nn.q.f, Nn.u.st, fn);
-        asm_sync();
-        const APub R = pub[t + 1];
-        const APub L = pub[t > 0 ? t - 1 : 0];
-        Face fe;
-        face_eval<SD, true>(s, c, g.dx, me.lmin, me.lmax, me.f, me.st, R.lmin, R.lmax, R.f, R.st, fe);
-        fcs[0][t] = fe.ap; fcs[1][t] = fe.am; fcs[2][t] = fe.Lam; fcs[3][t] = fe.alpha; fcs[4][t] = fe.sig;
-        asm_sync();
-        if (upd) {
-            const int tw = t - 1;
-            Face fw; fw.ap = fcs[0][tw]; fw.am = fcs[1][tw]; fw.Lam = fcs[2][tw]; fw.alpha = fcs[3][tw]; fw.sig = fcs[4][tw];
-#endif
             const long long id = (long long)j * g.nx + i;
             const bool fold_s = (j == 0 && g.bc[YLO] == BC_OUTFLOW) || (g.ny == 1 && g.bc[YLO] == BC_PERIODIC);
             const bool fold_n = (j == g.ny - 1 && g.bc[YHI] == BC_OUTFLOW) || (g.ny == 1 && g.bc[YHI] == BC_PERIODIC);

@@ -24,10 +24,7 @@ namespace ark {
 // Tile assembly: a block owns ATX x ATY cells.  Phase 1 evaluates closure + pressure Jacobian ONCE per cell of the tile and
 // of its one-cell halo (corners excluded) into shared memory; phase 2 builds the five blocks of each cell from the five
 // shared entries.  (The first version evaluated five closures per cell: 3.5 ms at 4096^2; fast reciprocals: 2.4 ms.)
-#ifndef ARK_ASM_TY
-#define ARK_ASM_TY 4
-#endif
-static constexpr int ATX = 32, ATY = ARK_ASM_TY, AW = ATX + 2, AH = ATY + 2, ACELLS = AW * AH;
+static constexpr int ATX = 32, ATY = 4, AW = ATX + 2, AH = ATY + 2, ACELLS = AW * AH;
 enum { TC_E = 0, TC_FX, TC_FY, TC_SA, TC_ST, TC_F, TC_LMINX, TC_LMAXX, TC_LMINY, TC_LMAXY, TC_J0, TC_FIELDS = TC_J0 + 9 };
 
 template <bool SD>

@@ -6,10 +6,7 @@
 namespace ark {
 
 static constexpr int KTHREADS = 256;
-#ifndef ARK_EPI_MAX
-#define ARK_EPI_MAX 128
-#endif
-static constexpr int EPI_MAX = ARK_EPI_MAX;      // Hessenberg columns up to this length are staged in shared memory for the Givens epilogue
+static constexpr int EPI_MAX = 128;      // Hessenberg columns up to this length are staged in shared memory for the Givens epilogue
 
 
 __device__ __forceinline__ double warp_sum(double v)

@@ -17,12 +17,8 @@
 
 namespace ark {
 
-#ifndef ARK_MG_MINB
-#define ARK_MG_MINB 3        // resident blocks per SM asked of the pair kernels: 168 registers let ptxas issue all block loads up front (measured best of 1, 3, 4, 8)
-#endif
-#ifndef ARK_MG_BY
-#define ARK_MG_BY 4          // rows of threads per block of the V-cycle kernels (32 x ARK_MG_BY threads)
-#endif
+static constexpr int MG_MINB = 3;      // resident blocks per SM asked of the pair kernels: 168 registers let ptxas issue all block loads up front (measured best of 1, 3, 4, 8)
+static constexpr int MG_BY = 4;        // rows of threads per block of the V-cycle kernels (32 x MG_BY threads)
 
 // Neighbour k (0: W, 1: E, 2: S, 3: N) of cell (i, j): its index on the level and, through `agg`, its aggregate on the next
 // coarser level (cnx aggregates per row).  Non-periodic sides clamp (the block there is zero).
@@ -92,7 +88,7 @@ cudaError_t launch_mg_galerkin(const Grid& gf, const double* off, const Grid& gc
 // ---- V-cycle pass 1: r_c = P0^T ((1 - omega) r - omega sum_k off_k r_nbr) --------------------------------------------
 // Thread (i, J) handles the fine cells (i, 2J) and (i, 2J+1); lane pairs (i even, i+1) add up through a shuffle.
 template <typename TB>
-__global__ void __launch_bounds__(32 * ARK_MG_BY) mg_restrict_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(32 * MG_BY) mg_restrict_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                           double omega, int cnx, double* __restrict__ rc,
                                                           const int* __restrict__ skip_flag)
 {
@@ -133,7 +129,7 @@ __global__ void __launch_bounds__(32 * ARK_MG_BY) mg_restrict_kernel(Grid g, con
 
 // ---- V-cycle pass 2: t = omega r + P0 e_c;  z^ = t + omega (r - t - sum_k off_k t_nbr);  out = Dinv z^ (coarse levels) or z^ ----
 template <typename TB>
-__global__ void __launch_bounds__(32 * ARK_MG_BY) mg_prolong_smooth_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(32 * MG_BY) mg_prolong_smooth_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                                 double omega, int cnx, const double* __restrict__ ec,
                                                                 const double* __restrict__ Dinv, double* __restrict__ out,
                                                                 const int* __restrict__ skip_flag)
@@ -216,7 +212,7 @@ __device__ __forceinline__ PairNbr pair_nbr(const Grid& g, int I, int j, int cnx
 }
 
 template <typename TB>
-__global__ void __launch_bounds__(128, ARK_MG_MINB) mg_restrict2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(128, MG_MINB) mg_restrict2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                            double omega, int cnx, double* __restrict__ rc,
                                                            const int* __restrict__ skip_flag)
 {
@@ -250,7 +246,7 @@ __global__ void __launch_bounds__(128, ARK_MG_MINB) mg_restrict2_kernel(Grid g, 
 }
 
 template <typename TB>
-__global__ void __launch_bounds__(128, ARK_MG_MINB) mg_prolong_smooth2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
+__global__ void __launch_bounds__(128, MG_MINB) mg_prolong_smooth2_kernel(Grid g, const TB* __restrict__ off, const double* __restrict__ r,
                                                                  double omega, int cnx, const double* __restrict__ ec,
                                                                  const double* __restrict__ Dinv, double* __restrict__ out,
                                                                  const int* __restrict__ skip_flag)
@@ -332,7 +328,7 @@ static cudaError_t vcycle_t(const MgHier& H, const double* r_in, double* zhat_ou
             dim3 blk(32, 4), grd((cnx + 31) / 32, (cny + 3) / 4);
             mg_restrict2_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, cnx, H.lev[l + 1].r, skip_flag);
         } else {
-            dim3 blk(32, ARK_MG_BY), grd((f.g.nx + 31) / 32, ((f.g.ny + 1) / 2 + ARK_MG_BY - 1) / ARK_MG_BY);
+            dim3 blk(32, MG_BY), grd((f.g.nx + 31) / 32, ((f.g.ny + 1) / 2 + MG_BY - 1) / MG_BY);
             mg_restrict_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].r, skip_flag);
         }
         ++launches;
@@ -353,7 +349,7 @@ static cudaError_t vcycle_t(const MgHier& H, const double* r_in, double* zhat_ou
             mg_prolong_smooth2_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, cnx, H.lev[l + 1].e,
                                                                (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
         } else {
-            dim3 blk(32, ARK_MG_BY), grd((f.g.nx + 31) / 32, (f.g.ny + ARK_MG_BY - 1) / ARK_MG_BY);
+            dim3 blk(32, MG_BY), grd((f.g.nx + 31) / 32, (f.g.ny + MG_BY - 1) / MG_BY);
             mg_prolong_smooth_kernel<TB><<<grd, blk, 0, st>>>(f.g, blocks(f), r, H.omega, H.lev[l + 1].g.nx, H.lev[l + 1].e,
                                                               (l == 0) ? nullptr : f.Dinv, (l == 0) ? zhat_out : f.e, skip_flag);
         }
