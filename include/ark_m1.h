@@ -280,6 +280,9 @@ ARK_M1_API ark_m1_3d* ark_m1_3d_create(int nx, int ny, int nz, double dx, double
 ARK_M1_API void ark_m1_3d_destroy(ark_m1_3d* h);
 ARK_M1_API int ark_m1_3d_set_stream(ark_m1_3d* h, void* cuda_stream);
 ARK_M1_API int ark_m1_3d_set_state(ark_m1_3d* h, const double* E, const double* F, const double* sigma_a, const double* sigma_s);
+/* "explicit_kernel": 1 = two streaming passes, closure once per cell then the flux-form stencil (default); 0 = one thread per cell
+ * evaluating its seven closures itself (IEEE divisions and roots). */
+ARK_M1_API int ark_m1_3d_set_option(ark_m1_3d* h, const char* key, double value);
 ARK_M1_API int ark_m1_3d_get_state(ark_m1_3d* h, double* E, double* F);
 ARK_M1_API int ark_m1_3d_step_explicit(ark_m1_3d* h, double dt);
 ARK_M1_API int ark_m1_3d_step_implicit(ark_m1_3d* h, double dt, double tol, int restart, int maxit, double* final_residual);

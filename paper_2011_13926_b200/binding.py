@@ -29,7 +29,7 @@ SYMBOLS = [
     "ark_m1_slab_range", "ark_m1_group_create_local", "ark_m1_group_create_host", "ark_m1_nccl_unique_id", "ark_m1_group_create_nccl",
     "ark_m1_group_destroy", "ark_m1_group_set_stream", "ark_m1_group_local_slabs", "ark_m1_group_slab", "ark_m1_group_step_explicit",
     "ark_m1_group_step_implicit", "ark_m1_group_comm_stats", "ark_m1_group_last_error",
-    "ark_m1_3d_create", "ark_m1_3d_destroy", "ark_m1_3d_set_stream", "ark_m1_3d_set_state", "ark_m1_3d_get_state", "ark_m1_3d_step_explicit",
+    "ark_m1_3d_create", "ark_m1_3d_destroy", "ark_m1_3d_set_stream", "ark_m1_3d_set_state", "ark_m1_3d_set_option", "ark_m1_3d_get_state", "ark_m1_3d_step_explicit",
     "ark_m1_3d_step_implicit", "ark_m1_3d_apply_operator", "ark_m1_3d_kernel_launches", "ark_m1_3d_last_error",
 ]
 
@@ -126,6 +126,7 @@ def load_library(path: str | None = None):
     L.ark_m1_3d_destroy.argtypes = [vp]
     L.ark_m1_3d_set_stream.argtypes = [vp, vp]
     L.ark_m1_3d_set_state.argtypes = [vp, dp, dp, dp, dp]
+    L.ark_m1_3d_set_option.argtypes = [vp, C.c_char_p, d]
     L.ark_m1_3d_get_state.argtypes = [vp, dp, dp]
     L.ark_m1_3d_step_explicit.argtypes = [vp, d]
     L.ark_m1_3d_step_implicit.argtypes = [vp, d, d, i, i, C.POINTER(C.c_double)]
@@ -491,6 +492,9 @@ class ArkM1_3D:
         pe, k0 = _ptr(E, N); pf, k1 = _ptr(F, 3 * N); pa, k2 = _ptr(sigma_a, N); ps, k3 = _ptr(sigma_s, N)
         self._check(self._L.ark_m1_3d_set_state(self._h, pe, pf, pa, ps))
         self._keep = (k0, k1, k2, k3)
+
+    def set_option(self, key, value):
+        self._check(self._L.ark_m1_3d_set_option(self._h, key.encode(), float(value)))
 
     def get_state(self):
         E = np.empty((self.nz, self.ny, self.nx)); F = np.empty((3, self.nz, self.ny, self.nx))

@@ -37,22 +37,26 @@ def pair(shape, d, c, bc, state):
 BCS3 = [(0, 0, 0, 0, 0, 0), (2, 2, 0, 0, 0, 0), (0, 0, 2, 2, 2, 2), (2, 2, 2, 2, 2, 2)]
 
 
+@pytest.mark.parametrize("kernel", [1, 0])
 @pytest.mark.parametrize("bc", BCS3)
 @pytest.mark.parametrize("shape", [(19, 13, 11), (33, 5, 7), (1, 9, 1), (130, 3, 2)])
-def test_explicit_3d_parity(shape, bc):
+def test_explicit_3d_parity(shape, bc, kernel):
     c, d = 1.3, (0.013, 0.021, 0.017)
     o, g = pair(shape, d, c, bc, rough3(*shape, seed=501 + shape[0], c=c))
+    g.set_option("explicit_kernel", kernel)
     dt = 0.4 * min(d) / c / 1.5            # the unsplit 3-D limit is a third, not a half
     for _ in range(3):
         o.step_explicit(dt); g.step_explicit(dt)
     assert_parity(g.get_state(), o.get_state(), 1e-11)
 
 
-def test_explicit_3d_clamped_and_nonpositive_cells():
+@pytest.mark.parametrize("kernel", [1, 0])
+def test_explicit_3d_clamped_and_nonpositive_cells(kernel):
     shape, c, d = (12, 9, 8), 1.0, (0.1, 0.1, 0.1)
     E, F, sa, ss = rough3(*shape, seed=502, fmax=1.6)          # |F| > cE in many cells: clamp
     E[2, 3, 4] = -0.5; E[1, 1, 1] = 0.0; F[:, 5, 5, 5] = 0.0      # E <= 0 guard, F = 0
     o, g = pair(shape, d, c, (0, 0, 2, 2, 0, 0), (E, F, sa, ss))
+    g.set_option("explicit_kernel", kernel)
     o.step_explicit(0.02); g.step_explicit(0.02)
     assert_parity(g.get_state(), o.get_state(), 1e-11)
 
