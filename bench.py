@@ -768,10 +768,11 @@ def run_decomposed(args):
     w = wl.random_medium(n, seed=args.seed)           # the SAME global problem on every rank; each keeps its rows
     dt_e = wl.explicit_dt(w["dx"], w["dy"], w["c"])
     stream = torch.cuda.current_stream()
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    if world > 1 or args.decomposed_local < 2:          # --decomposed: one slab per rank over NCCL (a single rank still goes through NCCL)
         box = [ark.nccl_unique_id() if rank == 0 else None]
-        dist.broadcast_object_list(box, src=0)
+        if world > 1:
+            dist.init_process_group("nccl", device_id=dev)
+            dist.broadcast_object_list(box, src=0)
         grp = ark.ArkM1Group(n, n, w["dx"], w["dy"], w["c"], bc=w["bc"], nranks=world, kind="nccl", rank=rank, unique_id=box[0], stream=stream)
         nslab_total, kind = world, "nccl"
     else:
