@@ -649,18 +649,8 @@ def run_ours(args):
         # ---- 3-D (SURVEY 8(f) row 4 tail; generic kernels, csrc/m1_3d.cu): the same number of cells as the 2-D workload ---------------
         if not args.no_sweep and not args.no_3d:
             n3 = int(round(N ** (1.0 / 3.0)))
-            rng = np.random.default_rng(args.seed)
-            shp = (n3, n3, n3)
-            E3 = np.exp(rng.standard_normal(shp))
-            v3 = rng.standard_normal((3,) + shp); v3 /= np.linalg.norm(v3, axis=0)
-            F3 = rng.uniform(0.0, 0.9, shp) * E3 * v3
-            k5 = np.ones(5) / 5.0
-            def smooth(a):
-                for ax in range(3):
-                    a = sum(np.roll(a, sh, axis=ax) for sh in (-2, -1, 0, 1, 2)) / 5.0
-                return a
-            sa3 = 10.0 ** smooth(rng.uniform(-3.0, 3.0, shp)); ss3 = 10.0 ** smooth(rng.uniform(-3.0, 3.0, shp))
-            d3 = {k: torch.from_numpy(np.ascontiguousarray(a)).to(dev) for k, a in (("E", E3), ("F", F3), ("sa", sa3), ("ss", ss3))}
+            w3 = wl.random_medium_3d(n3, seed=args.seed)
+            d3 = {k: torch.from_numpy(np.ascontiguousarray(a)).to(dev) for k, a in (("E", w3["E"]), ("F", w3["F"]), ("sa", w3["sigma_a"]), ("ss", w3["sigma_s"]))}
             g3 = ark.ArkM1_3D(n3, n3, n3, 1.0 / n3, 1.0 / n3, 1.0 / n3, 1.0, stream=stream)
             N3 = n3 ** 3
             dt3 = 0.4 / n3 / 1.5
@@ -683,8 +673,8 @@ def run_ours(args):
             e1.record(stream)
             torch.cuda.synchronize()
             ms3i = e0.elapsed_time(e1)
-            line_extra["three_d"] = {"workload": f"{n3}^3 cells ({N3 / 1e6:.1f} M), periodic, the config-3 recipe in three dimensions (E lognormal, |F| = u c E with u ~ U[0, 0.9] in a random "
-                                                 "direction, log10 sigma ~ U[-3, 3] box-smoothed over 5 cells per direction)",
+            line_extra["three_d"] = {"workload": f"m1_workloads.random_medium_3d: {n3}^3 cells ({N3 / 1e6:.1f} M), periodic, the config-3 recipe in three dimensions (E lognormal, |F| = u c E with u ~ U[0, 0.9] in a "
+                                                 "random direction, log10 sigma ~ U[-3, 3] box-smoothed over 5 cells per direction)",
                                      "explicit": {"ms_per_step": ms3e, "cell_updates_per_s": N3 / (ms3e * 1e-3), "bytes_per_cell": 80, "hbm_frac": 80.0 * N3 / (ms3e * 1e-3) / 1e9 / peak_gbs,
                                                   "note": "two streaming passes (closure once per cell into 13 planes, then the flux-form stencil; ~320 B/cell of DRAM traffic against the algorithmic 80): not the marching organisation of the 2-D kernel"},
                                      "implicit_10x": {"iterations": its3, "final_residual": res3, "ms": ms3i, "ms_per_iteration": ms3i / max(its3, 1), "cell_updates_per_s": N3 / (ms3i * 1e-3)}}

@@ -17,6 +17,10 @@ five configs.  Recipes (also in DESIGN.md, "Input recipe"):
                                    both log10-opacity fields are smoothed with a separable periodic 5x5 box mean
                                    (applied to the log field) and exponentiated; |F| = u c E, direction theta.
   config 5  stratified_coupled   : see the function docstring.
+  3-D       random_medium_3d     : the config-3 recipe in three dimensions (planes [nz, ny, nx], F = [3, nz, ny, nx]): draw order
+                                   (1) g ~ N(0,1) -> E = exp(g)  (2) u ~ U[0, fmax]  (3) a direction vector N(0,1)^3, normalised
+                                   (4) log10 sigma_a ~ U[lo, hi]  (5) log10 sigma_s ~ U[lo, hi]; with smooth=True both log fields get
+                                   a separable periodic 5-point box mean per direction before exponentiation.
 """
 from __future__ import annotations
 
@@ -115,6 +119,28 @@ def random_medium(n=1024, seed=1234, c=1.0, ny=None):
     F[1] = u * c * E * np.sin(th)
     dx, dy = 1.0 / nx, 1.0 / ny
     return dict(nx=nx, ny=ny, dx=dx, dy=dy, c=c, bc=(0, 0, 0, 0), E=E, F=F, sigma_a=sigma_a, sigma_s=sigma_s, seed=seed)
+
+
+def random_medium_3d(nx, ny=None, nz=None, seed=1234, c=1.0, fmax=0.9, log_sigma=(-3.0, 3.0), smooth=True):
+    """The random medium in three dimensions (SURVEY 8(f) row 4 tail); see the module docstring for the draw order."""
+    ny = nx if ny is None else ny
+    nz = nx if nz is None else nz
+    rng = np.random.default_rng(seed)
+    shp = (nz, ny, nx)
+    E = np.exp(rng.standard_normal(shp))
+    u = rng.uniform(0.0, fmax, shp)
+    v = rng.standard_normal((3,) + shp)
+    v /= np.linalg.norm(v, axis=0)
+    F = u * c * E * v
+
+    def box(a):
+        for ax in range(3):
+            a = sum(np.roll(a, sh, axis=ax) for sh in (-2, -1, 0, 1, 2)) / 5.0
+        return a
+    la, ls = rng.uniform(*log_sigma, shp), rng.uniform(*log_sigma, shp)
+    if smooth:
+        la, ls = box(la), box(ls)
+    return dict(nx=nx, ny=ny, nz=nz, c=c, E=E, F=F, sigma_a=10.0 ** la, sigma_s=10.0 ** ls, seed=seed)
 
 
 def stratified_coupled(n=2048, seed=4321, c=1.0, gamma=5.0 / 3.0, H=0.1, kappa=1e3, u_rms=1e-3, a_r=1.0):

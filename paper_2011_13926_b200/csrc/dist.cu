@@ -220,6 +220,9 @@ static ark_m1_group* group_create(int nx, int ny, double dx, double dy, double c
     if (nx < 1 || ny < 1 || nranks < 1 || nranks > ny || rank < 0 || rank >= nranks) return nullptr;
     ark_m1_bc gb = { 0, 0, 0, 0 };
     if (bc) gb = *bc;
+    const int kinds[4] = { gb.xlo, gb.xhi, gb.ylo, gb.yhi };
+    for (int k = 0; k < 4; ++k) if (kinds[k] < BC_PERIODIC || kinds[k] > BC_OUTFLOW) return nullptr;
+    if ((gb.xlo == BC_PERIODIC) != (gb.xhi == BC_PERIODIC) || (gb.ylo == BC_PERIODIC) != (gb.yhi == BC_PERIODIC)) return nullptr;   // periodic comes in pairs
     ark_m1_group* G = new (std::nothrow) ark_m1_group;
     if (!G) return nullptr;
     memset(G, 0, sizeof *G);

@@ -4,6 +4,7 @@ GMRES residual converged, iteration counts within 2 or 2 %."""
 import numpy as np
 import pytest
 
+import m1_workloads as wl
 import paper_2011_13926_b200 as ark
 from helpers import assert_parity, state_rel_l2
 from oracle.oracle_m1_3d import OracleM1_3D
@@ -18,12 +19,8 @@ def _build():
 
 
 def rough3(nx, ny, nz, seed, c=1.0, fmax=0.9, sig=(-1.0, 1.0)):
-    rng = np.random.default_rng(seed)
-    shp = (nz, ny, nx)
-    E = np.exp(rng.standard_normal(shp))
-    u = rng.uniform(0.0, fmax, shp)
-    v = rng.standard_normal((3,) + shp); v /= np.linalg.norm(v, axis=0)
-    return E, u * c * E * v, 10.0 ** rng.uniform(*sig, shp), 10.0 ** rng.uniform(*sig, shp)
+    w = wl.random_medium_3d(nx, ny, nz, seed=seed, c=c, fmax=fmax, log_sigma=sig, smooth=False)
+    return w["E"], w["F"], w["sigma_a"], w["sigma_s"]
 
 
 def pair(shape, d, c, bc, state):

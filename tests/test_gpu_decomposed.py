@@ -131,6 +131,8 @@ def test_unsupported_options_and_slab_handles_are_rejected():
         grp.step_implicit(_dt(w, 10.0))
     with pytest.raises(ValueError):
         ark.ArkM1Group(20, 4, 0.1, 0.1, nranks=5)                # more slabs than rows
+    with pytest.raises(ValueError):
+        ark.ArkM1Group(20, 16, 0.1, 0.1, bc=(0, 0, 0, 1), nranks=2)   # periodic on one side of y only
 
 
 def test_nccl_transport_single_rank():

@@ -66,14 +66,8 @@ def test_a_state_independent_of_one_coordinate_evolves_like_the_2d_oracle(axis, 
 
 
 def _rough3(nx, ny, nz, seed, c=1.0, fmax=0.9):
-    rng = np.random.default_rng(seed)
-    shp = (nz, ny, nx)
-    E = np.exp(rng.standard_normal(shp))
-    u = rng.uniform(0.0, fmax, shp)
-    v = rng.standard_normal((3,) + shp); v /= np.linalg.norm(v, axis=0)
-    F = u * c * E * v
-    sa = 10.0 ** rng.uniform(-1.0, 1.0, shp); ss = 10.0 ** rng.uniform(-1.0, 1.0, shp)
-    return E, F, sa, ss
+    w = wl.random_medium_3d(nx, ny, nz, seed=seed, c=c, fmax=fmax, log_sigma=(-1.0, 1.0), smooth=False)
+    return w["E"], w["F"], w["sigma_a"], w["sigma_s"]
 
 
 def test_relabelling_the_axes_relabels_the_result():
