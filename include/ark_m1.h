@@ -292,6 +292,32 @@ ARK_M1_API int ark_m1_3d_apply_operator(ark_m1_3d* h, double dt, const double* V
 ARK_M1_API long long ark_m1_3d_kernel_launches(const ark_m1_3d* h);
 ARK_M1_API const char* ark_m1_3d_last_error(const ark_m1_3d* h);
 
+/* ---------------------------------------------------------------------------------------------------------------------------
+ * The realizability guard without any allocation (row a7), for callers that cannot call cudaMalloc: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it.  No handle.  Same predicate and arithmetic as
+ * ark_m1_count_unrealizable; the scratch (one pair of partial counts per block of 4096 cells and the "last block" ticket) lives
+ * in a static __device__ array of 262 400 bytes inside the library, held by every GPU that loads libark_m1.so until the process
+ * exits.  The call enqueues one 256-byte memset of the ticket and one kernel on `cuda_stream` and returns; it never synchronises
+ * and calls no cudaMalloc / cudaFree / allocating routine.
+ *   E, Fx, Fy : DEVICE pointers on the current device, ncells doubles each (any plane layout; [ny][nx] flattened), read only
+ *   c         : speed of light
+ *   counts2   : DEVICE pointer, 2 x unsigned long long, written by the kernel: [0] cells with E <= 0 (or NaN), [1] cells with
+ *               E > 0 and |F| > cE.  Valid once `cuda_stream` has reached the kernel's end.  ncells == 0 writes two zeros.
+ * Limit: ncells <= ark_m1_noalloc_max_cells() = 67 108 864 (8192^2); beyond it the call returns ARK_M1_E_UNSUPPORTED and
+ * launches nothing.  Other errors: ARK_M1_E_ARG (null pointer, ncells < 0), ARK_M1_E_CUDA.  ark_m1_noalloc_last_error() holds
+ * the calling thread's last message.
+ * Sharing: every call on a device uses the same array, which keeps the previous call's contents (the call clears what must
+ * start at zero).  Calls that can overlap on the GPU — different streams, different host threads, two captured graphs launched
+ * concurrently — race on it and return wrong counts: order them on one stream or with events.
+ * ark_m1_noalloc_setup() resolves the array's device address for the CURRENT device (cudaGetSymbolAddress, once per device;
+ * may load the module): call it once per device before capturing; ark_m1_count_unrealizable_noalloc calls it itself otherwise.
+ * --------------------------------------------------------------------------------------------------------------------------- */
+ARK_M1_API int ark_m1_noalloc_setup(void);
+ARK_M1_API long long ark_m1_noalloc_max_cells(void);
+ARK_M1_API int ark_m1_count_unrealizable_noalloc(const double* E, const double* Fx, const double* Fy, long long ncells, double c,
+                                                 unsigned long long* counts2, void* cuda_stream);
+ARK_M1_API const char* ark_m1_noalloc_last_error(void);
+
 /* Device bytes currently allocated by the handle. */
 ARK_M1_API long long ark_m1_device_bytes(const ark_m1* h);
 

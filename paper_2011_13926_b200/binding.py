@@ -31,6 +31,7 @@ SYMBOLS = [
     "ark_m1_group_step_implicit", "ark_m1_group_comm_stats", "ark_m1_group_last_error",
     "ark_m1_3d_create", "ark_m1_3d_destroy", "ark_m1_3d_set_stream", "ark_m1_3d_set_state", "ark_m1_3d_set_option", "ark_m1_3d_get_state", "ark_m1_3d_step_explicit",
     "ark_m1_3d_step_implicit", "ark_m1_3d_apply_operator", "ark_m1_3d_kernel_launches", "ark_m1_3d_last_error",
+    "ark_m1_noalloc_setup", "ark_m1_noalloc_max_cells", "ark_m1_count_unrealizable_noalloc", "ark_m1_noalloc_last_error",
 ]
 
 
@@ -135,6 +136,12 @@ def load_library(path: str | None = None):
     L.ark_m1_3d_kernel_launches.argtypes = [vp]
     L.ark_m1_3d_last_error.restype = C.c_char_p
     L.ark_m1_3d_last_error.argtypes = [vp]
+    L.ark_m1_noalloc_setup.argtypes = []
+    L.ark_m1_noalloc_max_cells.restype = C.c_longlong
+    L.ark_m1_noalloc_max_cells.argtypes = []
+    L.ark_m1_count_unrealizable_noalloc.argtypes = [dp, dp, dp, C.c_longlong, d, vp, vp]
+    L.ark_m1_noalloc_last_error.restype = C.c_char_p
+    L.ark_m1_noalloc_last_error.argtypes = []
     for name in SYMBOLS:
         getattr(L, name)
     _lib = L
@@ -548,6 +555,38 @@ def fp64_issue_rate():
     if rc < 0:
         raise RuntimeError(f"ark_m1_fp64_issue_rate failed ({rc})")
     return dict(zip(PIPE_RATE_KEYS, (float(v) for v in buf)))
+
+
+def noalloc_setup():
+    """Resolve the static scratch array of the no-allocation entry point on the current device (once per device, before a capture)."""
+    L = load_library()
+    rc = L.ark_m1_noalloc_setup()
+    if rc < 0:
+        raise RuntimeError(f"ark_m1_noalloc_setup failed ({rc}): {L.ark_m1_noalloc_last_error().decode()}")
+
+
+def noalloc_max_cells():
+    return int(load_library().ark_m1_noalloc_max_cells())
+
+
+def count_unrealizable_noalloc(E, Fx, Fy, c, counts2, stream=None):
+    """ark_m1_count_unrealizable_noalloc: E, Fx, Fy float64 CUDA tensors of equal size, counts2 a CUDA tensor of 2 x int64 (the two
+    unsigned 64-bit counts), all on the current device.  Enqueues on `stream` (torch stream or raw address; default: torch's current
+    stream) and returns without synchronising; allocates nothing."""
+    import torch
+    L = load_library()
+    for t in (E, Fx, Fy):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == E.numel()):
+            raise TypeError("E, Fx, Fy must be contiguous float64 CUDA tensors of equal size")
+    if not (isinstance(counts2, torch.Tensor) and counts2.is_cuda and counts2.dtype == torch.int64 and counts2.is_contiguous() and counts2.numel() == 2):
+        raise TypeError("counts2 must be a contiguous int64 CUDA tensor of 2 elements")
+    st = torch.cuda.current_stream() if stream is None else stream
+    st = getattr(st, "cuda_stream", st)
+    n = E.numel()
+    rc = L.ark_m1_count_unrealizable_noalloc(E.data_ptr() if n else None, Fx.data_ptr() if n else None, Fy.data_ptr() if n else None,
+                                             n, float(c), counts2.data_ptr(), st)
+    if rc < 0:
+        raise RuntimeError(f"ark_m1 error {rc}: {L.ark_m1_noalloc_last_error().decode()}")
 
 
 def version():
