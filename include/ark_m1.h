@@ -100,6 +100,12 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                          row ahead of the faces, cp.async row prefetch (default)
  *   "operator"          1: matrix-free coefficient planes, flux form (default: 5% faster per solve at 4096^2)
  *                       0: block stencil (BSR 3x3 on the 5-point graph, pre-multiplied by M^-1)
+ *   "op_recompute"      1 (default): the preconditioned matrix-free operator rebuilds each cell's diagonal block from J and the
+ *                          four faces' coefficients, which it loads anyway, and solves the 3 x 3 system in registers: 192 B per
+ *                          cell per application.  0: it loads the nine stored M^-1 planes (264 B).  Same operator up to the
+ *                          rounding of M^-1; cells with folded neighbours (outflow sides) always use the stored inverse
+ *   "apply_operator_precond"  1: ark_m1_apply_operator returns A M^-1 V through the solver's preconditioned kernel (matrix-free
+ *                          operator only); 0 (default): A V
  *   "basis_precision"   64 (default) or 32: storage precision of the GMRES Arnoldi basis.  32 = compressed-basis GMRES: the basis
  *                       vectors are stored in single precision, every computation (operator, dots, updates, Hessenberg,
  *                       solution, true residual at each restart) stays fp64 and the solve ends at the same fp64 tolerance;

@@ -83,6 +83,8 @@ void ark_dfree(ark_m1* h, void* p)
 
 // the multigrid hierarchy is built from assembled blocks: it overrides the matrix-free operator
 static inline int opk(const ark_m1* h) { return h->precond == 1 ? 0 : h->op_kind; }
+// bytes per cell the preconditioned matrix-free operator does not move when it rebuilds the diagonal block (the nine M^-1 planes)
+static inline double mf_saved(const ark_m1* h) { return h->mf.rc ? 72.0 : 0.0; }
 
 // compressed-basis GMRES applies to the default solver configuration only; elsewhere the option is ignored
 static inline bool use_cb(const ark_m1* h) { return h->basis_prec == 32 && h->krylov == 0 && h->precond == 0 && h->op_kind == 1 && h->ortho == 1; }
@@ -124,7 +126,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
-    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1;
+    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 1; h->apply_precond = 0;
     h->basis_prec = 64; h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -248,6 +250,8 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "release_workspace")) { if (value != 0.0) { cudaStreamSynchronize(h->st); free_implicit(h); } }
     else if (!strcmp(key, "kernel_timing")) { ark_kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
+    else if (!strcmp(key, "apply_operator_precond")) h->apply_precond = (value != 0.0);
+    else if (!strcmp(key, "op_recompute")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "op_recompute must be 0 (load M^-1) or 1 (rebuild the diagonal block in the operator)%s", ""); h->op_recompute = iv; }
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
     else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return ark_fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
     else if (!strcmp(key, "mg_coarse_sweeps")) { if (iv < 1) return ark_fail(h, ARK_M1_E_ARG, "mg_coarse_sweeps must be >= 1%s", ""); h->mg.coarse_sweeps = iv; }
@@ -504,6 +508,7 @@ int ark_assemble_system(ark_m1* h, double dt, const double* bsrc)
     const Fields f = ark_fields_of(h);
     if (opk(h) == 1) {
         h->mf.rx = h->s.hyp_off ? 0.0 : dt / h->g.dx; h->mf.ry = h->s.hyp_off ? 0.0 : dt / h->g.dy;
+        h->mf.rc = h->op_recompute; h->mf.has_dF = (h->s.wb == 0);
         if (h->asm_kernel == 1 && h->N < (1LL << 31))
             KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble_march(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->sm_count, h->st));
         else
@@ -559,7 +564,7 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
                 if ((rc = mg_apply(h, h->V + (size_t)j * S, h->mgz, stop))) return rc;
                 KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->mgz, w, W.scale + j, nullptr, 1.0, stop, h->st));
             } else if (opk(h) == 1)
-                KL(KC_SPMV, 264.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
+                KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
             else
                 KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, h->st));
             // the j+1 basis vectors go through the multi-vector kernels in ceil((j+1)/MV) chunks of (nearly) equal size
@@ -618,7 +623,7 @@ static int gmres_solve_cb(ark_m1* h, double tol, int m, int maxit)
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             float* vnext = h->V32 + (size_t)(j + 1) * S;
-            KL(KC_SPMV, 252.0 * h->N, launch_op_mf_f32(h->g, h->mf, h->A.Minv, h->V32 + (size_t)j * S, w, W.scale + j, stop, sm, h->st));
+            KL(KC_SPMV, (252.0 - mf_saved(h)) * h->N, launch_op_mf_f32(h->g, h->mf, h->A.Minv, h->V32 + (size_t)j * S, w, W.scale + j, stop, sm, h->st));
             for (int c0 = 0; c0 <= j; c0 += MV) {
                 const int nv = (j + 1 - c0) < MV ? (j + 1 - c0) : MV;
                 KL(KC_DOT, (24.0 + 12.0 * nv) * h->N, launch_multi_dot32(w, h->V32 + (size_t)c0 * S, S, nv, c0, n, W, DOT_H, sm, h->st));
@@ -651,7 +656,7 @@ static int op_apply_hat(ark_m1* h, const double* vin, double* vout, const int* s
         return 0;
     }
     if (opk(h) == 1)
-        KL(KC_SPMV, 264.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, stop, 1, h->sm_count, h->st));
+        KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, stop, 1, h->sm_count, h->st));
     else
         KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, vin, vout, nullptr, nullptr, 1.0, stop, h->st));
     return 0;
@@ -678,9 +683,9 @@ static int bicgstab_solve(ark_m1* h, double tol, int maxit)
             for (int k = 0; k < 8; ++k) {
                 KL(KC_UPDATE, 96.0 * h->N, launch_bicg_p(r, p, v, n, W, h->st));
                 if (opk(h) == 1) {   // matrix-free operator with the reductions fused in
-                    KL(KC_SPMV, 288.0 * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, p, v, stop, 1, rh, W, sm, h->st));
+                    KL(KC_SPMV, (288.0 - mf_saved(h)) * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, p, v, stop, 1, rh, W, sm, h->st));
                     KL(KC_UPDATE, 72.0 * h->N, launch_bicg_s(r, v, n, W, h->st));
-                    KL(KC_SPMV, 264.0 * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, r, t, stop, 2, nullptr, W, sm, h->st));
+                    KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf_dot(h->g, h->mf, h->A.Minv, r, t, stop, 2, nullptr, W, sm, h->st));
                 } else {
                     if ((rc = op_apply_hat(h, p, v, stop))) return rc;
                     KL(KC_DOT, 48.0 * h->N, launch_multi_dot(v, rh, S, 1, 0, n, W, BICG_ALPHA, sm, h->st));
@@ -833,7 +838,8 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
     double* vout = h->V + h->stride;
     CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
     if (opk(h) == 1) {
-        KL(KC_SPMV, 192.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, nullptr, 0, h->sm_count, h->st));
+        if (h->apply_precond) KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, nullptr, 1, h->sm_count, h->st));
+        else KL(KC_SPMV, 192.0 * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, vout, nullptr, nullptr, 1.0, nullptr, 0, h->sm_count, h->st));
     } else {
         KL(KC_DIAGMUL, 120.0 * h->N, launch_diag_mul(h->g, h->A.C, vin, h->tvec, h->st));
         KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->tvec, vout, nullptr, nullptr, 1.0, nullptr, h->st));

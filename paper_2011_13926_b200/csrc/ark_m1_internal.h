@@ -86,6 +86,8 @@ struct MfPlanes {
     double* ylo;   // [4][nx] : south face of row 0 (non-periodic y)
     double rx, ry; // dt/dx, dt/dy of the assembled step
     const double* halo[2];   // slab decomposition (BC_HALO sides): received (z, c^2 J z) of the row below / above, [6][nx] each
+    int rc;        // 1: the preconditioned operator rebuilds the diagonal block from J and the faces instead of loading M^-1 (operator_mf.cu)
+    int has_dF;    // 0: dF is identically zero (WB source) and is not loaded
 };
 // A.off / A.C may be null when mf.J is set (then only Minv, b and the coefficient planes are written)
 // bsrc: planes [E|Fx|Fy] that supply the U^n part of the right-hand side (null: the state in `f`; non-null in Newton

@@ -15,6 +15,7 @@
 // (128 / 64 / 32 columns at 4096^2: 5.82 / 6.21 / 6.51 TB/s on the same box).
 #include <string.h>
 #include "krylov_device.cuh"
+#include "explicit_device.cuh"
 
 namespace ark {
 
@@ -174,11 +175,257 @@ __global__ void __launch_bounds__(TXO, DOT ? 16 : OP_MINB) op_mf_kernel(Grid g, 
     if (DOT == 2) reduce_and_finish<2, TXO>(acc, W, BICG_OMEGA, 0);
 }
 
-static dim3 op_mf_grid(const Grid& g, int sm_count, int* RYout)
+// ---------------------------------------------------------------------------------------------------------
+// The same operator WITHOUT the M^-1 planes (MfPlanes::rc, option "op_recompute", the default): the diagonal block of
+// A = I + dt L_n is the coefficient of z_C in the flux form below, i.e. a function of the cell's J, its four faces' coefficients
+// and dE (dF) — all of which this kernel loads anyway — so z = M^-1 v is obtained by building M and solving the 3 x 3 system
+// in registers (76 fp64 instructions per cell) instead of loading nine more planes: 192 B per cell per application instead
+// of 264.  The kernel waits for HBM (85 % of the stall samples), the arithmetic is free.
+//   m00 = 1 + dE - rx (al_e L_e + al_w L_w) - ry (al_n L_n + al_s L_s)      m01 = rx (al_e a+_e - al_w a-_w)      m02 = ry (al_n a+_n - al_s a-_s)
+//   rows 1, 2 = (1 + dF - rx (L_e + L_w) - ry (L_n + L_s) + source weights) e_k + c^2 [rx (a+_e - a-_w) J^{x.} + ry (a+_n - a-_s) J^{y.}]
+// (assemble_march.cu's add_G terms, a- = 1 - a+).  Faces of the row AHEAD (j+1) are loaded in step j — east and north from the
+// cell's own planes, west from the west lane's east face (lane 0 loads it), south = the current row's north face — and kept
+// as the current row's faces of step j+1.  Cells whose diagonal block holds folded neighbours (outflow sides, R9), ghost
+// rows and the two prologue rows of a block take z from the stored M^-1 as before (assembly still writes it: combine needs it).
+// ---------------------------------------------------------------------------------------------------------
+struct JC { double xx0, xx1, xx2, xy0, xy1, xy2, yy0, yy1, yy2; };
+
+__device__ __forceinline__ void solve_diag(const FC& e, const FC& w, const FC& n, const FC& s, const JC& J, double dE, double dF,
+                                           double rx, double ry, double c2, double v0, double v1, double v2,
+                                           double& zE, double& zFx, double& zFy)
+{
+    const double lam = fma(rx, e.Lam + w.Lam, ry * (n.Lam + s.Lam));
+    const double m00 = (1.0 + dE) - fma(rx, fma(e.alpha, e.Lam, w.alpha * w.Lam), ry * fma(n.alpha, n.Lam, s.alpha * s.Lam));
+    const double m01 = rx * fma(e.alpha, e.ap, w.alpha * (w.ap - 1.0));
+    const double m02 = ry * fma(n.alpha, n.ap, s.alpha * (s.ap - 1.0));
+    const double ax = (c2 * rx) * ((e.ap + w.ap) - 1.0), ay = (c2 * ry) * ((n.ap + s.ap) - 1.0);
+    const double dd = (1.0 + dF) - lam;
+    const double m10 = fma(ax, J.xx0, ay * J.xy0), m11 = fma(ax, J.xx1, fma(ay, J.xy1, dd + (e.sw + w.sw))), m12 = fma(ax, J.xx2, ay * J.xy2);
+    const double m20 = fma(ax, J.xy0, ay * J.yy0), m21 = fma(ax, J.xy1, ay * J.yy1), m22 = fma(ax, J.xy2, fma(ay, J.yy2, dd + (n.sw + s.sw)));
+    const double c00 = m11 * m22 - m12 * m21, c01 = m12 * m20 - m10 * m22, c02 = m10 * m21 - m11 * m20;
+    const double id = rcp_fast(m00 * c00 + m01 * c01 + m02 * c02);
+    zE  = (c00 * v0 + (m02 * m21 - m01 * m22) * v1 + (m01 * m12 - m02 * m11) * v2) * id;
+    zFx = (c01 * v0 + (m00 * m22 - m02 * m20) * v1 + (m02 * m10 - m00 * m12) * v2) * id;
+    zFy = (c02 * v0 + (m01 * m20 - m00 * m21) * v1 + (m00 * m11 - m01 * m10) * v2) * id;
+}
+
+// 12 resident blocks per SM (160 registers) and 64 rows per block (the two prologue rows of a block take z from the stored M^-1):
+// 16 blocks x 32 rows 0.630 ms, 16 x 64 0.618, 12 x 32 0.578, 12 x 64 0.573, 10 x 64 0.574, 20 x 32 (spills) 1.10 at 4096^2.
+static constexpr int OP_RC_MINB = 12;
+static constexpr int OP_RC_RY = 64;
+static constexpr int RC_NST = 2;          // ring stages: row j+1 landed, row j+2 in flight during step j
+static constexpr int RC_NF = 21;          // ring fields per cell: J (9), east face (4), north face (4), dE, v (3)
+
+// The row after the row ahead travels HBM -> shared memory with cp.async while the block works (the explicit kernel's ring):
+// a warp's row step is one long dependent chain (loads -> block -> 3 x 3 solve -> c^2 J z -> fluxes -> store), and with the loads
+// issued at the start of the step that consumes them the kernel ran at 4.1 TB/s (0.79 ms, slower than loading M^-1).  Each thread
+// reads back only its own slots, so cp.async.wait_group is the only synchronisation.
+// Measured and not kept: a third ring stage (0.57 -> 0.91 ms: cp.async.ca holds an L1 line per request in flight and the shared-
+// memory carve-out leaves too few); the same ring filled by 1-D bulk copies (cp.async.bulk + mbarrier, one 272-byte copy per plane
+// row: ptxas serialises the 21 copies of a row in an ELECT loop, 0.61 / 0.63 / 0.71 ms with 2 / 3 / 4 stages); a branch-free row
+// step for interior strips (0.570 against 0.574).
+template <typename TIN>
+__device__ __forceinline__ void rc_issue(double (*ring)[TXO], double* ringw, int t, const MfPlanes& mf, const TIN* __restrict__ v,
+                                         long long N, long long idn, bool want)
+{
+    if (want) {
+#pragma unroll
+        for (int e = 0; e < 9; ++e) cp_async8(&ring[e][t], mf.J + e * N + idn);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { cp_async8(&ring[9 + e][t], mf.fE + e * N + idn); cp_async8(&ring[13 + e][t], mf.fN + e * N + idn); }
+        cp_async8(&ring[17][t], mf.dE + idn);
+        if (sizeof(TIN) == 8) {
+#pragma unroll
+            for (int e = 0; e < 3; ++e) cp_async8(&ring[18 + e][t], reinterpret_cast<const double*>(v) + e * N + idn);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 3; ++e) {
+                const unsigned int d = (unsigned int)__cvta_generic_to_shared(&ring[18 + e][t]);
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(d), "l"(v + e * N + idn) : "memory");
+            }
+        }
+        if (t == 0) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) cp_async8(&ringw[e], mf.fE + e * N + idn - 1);
+        }
+    }
+    cp_async_commit();
+}
+
+// State a block carries from row to row: z and c^2 J z of the current row, the south flux, the current row's own faces and
+// source weights.
+struct RcState { ZP zC; double Hs0, Hs1, Hs2, Ss; FC fe, fn; double dE, dF; };
+
+// Second half of a row step: east flux with the east lane's data, west flux from the west lane, north flux with the row ahead,
+// the output of row j; then the row ahead becomes the current row.
+template <int DOT>
+__device__ __forceinline__ void rc_current_row(RcState& S, const ZP& zN, const FC& feN, const FC& fnN, double dEN, double dFN, bool upd,
+                                               long long id, long long N, const double* __restrict__ add, const double* __restrict__ aux,
+                                               double* __restrict__ out, double rx, double ry, double sc, double (&acc)[2])
+{
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+    if (upd && add) { a0 = add[id]; a1 = add[N + id]; a2 = add[2 * N + id]; }
+    double x0 = 0.0, x1 = 0.0, x2 = 0.0;
+    if (DOT == 1 && upd) { x0 = aux[id]; x1 = aux[N + id]; x2 = aux[2 * N + id]; }
+    const ZP& zC = S.zC;
+    ZPub me; me.zE = zC.zE; me.zFx = zC.zFx; me.zFy = zC.zFy; me.Pxx = zC.Pxx; me.Pxy = zC.Pxy;
+    double Ge0, Ge1, Ge2, Se;
+    {
+        ZPub R;
+        R.zE = __shfl_down_sync(0xffffffffu, me.zE, 1); R.zFx = __shfl_down_sync(0xffffffffu, me.zFx, 1); R.zFy = __shfl_down_sync(0xffffffffu, me.zFy, 1);
+        R.Pxx = __shfl_down_sync(0xffffffffu, me.Pxx, 1); R.Pxy = __shfl_down_sync(0xffffffffu, me.Pxy, 1);
+        ARK_LIN_FLUX(S.fe, me.zE, R.zE, me.zFx, R.zFx, me.zFy, R.zFy, me.Pxx, R.Pxx, me.Pxy, R.Pxy, Ge0, Ge1, Ge2, Se);
+    }
+    const double Gw0 = __shfl_up_sync(0xffffffffu, Ge0, 1), Gw1 = __shfl_up_sync(0xffffffffu, Ge1, 1);
+    const double Gw2 = __shfl_up_sync(0xffffffffu, Ge2, 1), Sw = __shfl_up_sync(0xffffffffu, Se, 1);
+    double Hn0, Hn1, Hn2, Sn;
+    ARK_LIN_FLUX(S.fn, zC.zE, zN.zE, zC.zFy, zN.zFy, zC.zFx, zN.zFx, zC.Pyy, zN.Pyy, zC.Pxy, zN.Pxy, Hn0, Hn2, Hn1, Sn);
+    if (upd) {
+        double o0 = zC.zE  + fma(rx, Ge0 - Gw0, fma(ry, Hn0 - S.Hs0, S.dE * zC.zE));
+        double o1 = zC.zFx + fma(rx, Ge1 - Gw1, fma(ry, Hn1 - S.Hs1, fma(S.dF, zC.zFx, Se + Sw)));
+        double o2 = zC.zFy + fma(rx, Ge2 - Gw2, fma(ry, Hn2 - S.Hs2, fma(S.dF, zC.zFy, Sn + S.Ss)));
+        o0 = fma(sc, o0, a0); o1 = fma(sc, o1, a1); o2 = fma(sc, o2, a2);
+        out[id] = o0; out[N + id] = o1; out[2 * N + id] = o2;
+        if (DOT == 1) acc[0] += o0 * x0 + o1 * x1 + o2 * x2;
+        if (DOT == 2) { acc[0] += o0 * zC.v0 + o1 * zC.v1 + o2 * zC.v2; acc[1] += o0 * o0 + o1 * o1 + o2 * o2; }
+    }
+    S.zC = zN;
+    S.Hs0 = Hn0; S.Hs1 = Hn1; S.Hs2 = Hn2; S.Ss = Sn;
+    S.fe = feN; S.fn = fnN; S.dE = dEN; S.dF = dFN;
+}
+
+template <int DOT, typename TIN = double>
+__global__ void __launch_bounds__(TXO, OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
+                                                    double* __restrict__ out, const double* __restrict__ scale_ptr,
+                                                    const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
+                                                    int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W)
+{
+    if (skip_flag && *skip_flag) return;
+    __shared__ double ring[RC_NST][RC_NF][TXO];     // row r lives in ring[r % RC_NST]
+    __shared__ double ringw[RC_NST][4];             // lane 0: the east face of the column west of the strip
+    double acc[2] = { 0.0, 0.0 };
+    const int t = threadIdx.x;
+    const int i = blockIdx.x * (TXO - 2) - 1 + t;
+    const int j0 = blockIdx.y * RY;
+    const int j1 = min(j0 + RY, g.ny);
+    const long long N = (long long)g.nx * g.ny;
+    const bool upd = (t >= 1 && t <= TXO - 2 && i >= 0 && i < g.nx);
+    int xmode = 0, ii = i;
+    bool use_xlo = false;
+    if (i > g.nx) xmode = 2;
+    else if (i < 0 || i >= g.nx) {
+        const int bc = g.bc[(i < 0) ? XLO : XHI];
+        if (bc == BC_DIRICHLET) { xmode = 1; ii = 0; }
+        else if (bc == BC_PERIODIC) ii = (i < 0) ? g.nx - 1 : 0;
+        else ii = (i < 0) ? 0 : g.nx - 1;
+        use_xlo = (i < 0) && (bc != BC_PERIODIC);
+    }
+    const bool east_valid = (i < g.nx) && (xmode != 2);
+    // this lane's column has a plain diagonal block (no folded neighbour) and, for lane 0, a west column to take the west face from
+    const bool col_ok = xmode == 0 && g.nx >= 2 && g.ny >= 2 && !(ii == 0 && g.bc[XLO] == BC_OUTFLOW) && !(ii == g.nx - 1 && g.bc[XHI] == BC_OUTFLOW)
+                        && (t > 0 || ii >= 1);
+    const int last_ok = (g.bc[YHI] == BC_OUTFLOW) ? g.ny - 2 : g.ny - 1;      // last row whose block is built here (block-uniform)
+    const double sc = sgn * (scale_ptr ? *scale_ptr : 1.0);
+    const bool has_dF = mf.has_dF != 0;
+
+    const int last_row = min(j1, last_ok);      // last row requested into the ring
+    // request rows j0+1 .. j0+RC_NST-1 first: row j0+1 is consumed by the first row step
+#pragma unroll
+    for (int r = 1; r < RC_NST; ++r)
+        rc_issue<TIN>(ring[(j0 + r) % RC_NST], ringw[(j0 + r) % RC_NST], t, mf, v, N, (long long)(j0 + r) * g.nx + ii, col_ok && j0 + r <= last_row);
+
+    RcState S;
+    {
+        const ZP zS = load_zp<true, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0 - 1, mf.halo[0], mf.halo[1]);
+        S.zC = load_zp<true, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, j0, mf.halo[0], mf.halo[1]);
+        S.Hs0 = 0.0; S.Hs1 = 0.0; S.Hs2 = 0.0; S.Ss = 0.0;
+        if (upd) {
+            FC fs;
+            if (j0 > 0) fs = load_fc(mf.fN, N, (long long)(j0 - 1) * g.nx + i);
+            else if (g.bc[YLO] == BC_PERIODIC) fs = load_fc(mf.fN, N, (long long)(g.ny - 1) * g.nx + i);
+            else fs = load_fc(mf.ylo, g.nx, i);
+            ARK_LIN_FLUX(fs, zS.zE, S.zC.zE, zS.zFy, S.zC.zFy, zS.zFx, S.zC.zFx, zS.Pyy, S.zC.Pyy, zS.Pxy, S.zC.Pxy, S.Hs0, S.Hs2, S.Hs1, S.Ss);
+        }
+    }
+    // faces and source weights of the current row (row j0 here; afterwards handed over from the row ahead)
+    S.fe.ap = 0.5; S.fe.Lam = 0.0; S.fe.alpha = 1.0; S.fe.sw = 0.0;
+    S.fn = S.fe;
+    S.dE = 0.0; S.dF = 0.0;
+    if (east_valid || col_ok) {
+        if (use_xlo || xmode == 1) { if (i < 0) S.fe = load_fc(mf.xlo, g.ny, j0); }
+        else S.fe = load_fc(mf.fE, N, (long long)j0 * g.nx + ii);
+    }
+    if (xmode == 0) {
+        const long long id0 = (long long)j0 * g.nx + ii;
+        S.fn = load_fc(mf.fN, N, id0);
+        S.dE = mf.dE[id0];
+        if (has_dF) S.dF = mf.dF[id0];
+    }
+
+    for (int j = j0; j < j1; ++j) {
+        const int jn = j + 1;
+        const long long id = (long long)j * g.nx + (upd ? i : 0);
+        // ---- request row j+RC_NST into the slot of row j (read one step ago), then wait for row j+1
+        rc_issue<TIN>(ring[j % RC_NST], ringw[j % RC_NST], t, mf, v, N, (long long)(j + RC_NST) * g.nx + ii, col_ok && j + RC_NST <= last_row);
+        cp_async_wait<RC_NST - 1>();
+        double (*rg)[TXO] = ring[jn % RC_NST];
+        // ---- the row ahead: its faces, then z = M^-1 v either from the block built here or from the stored inverse
+        FC feN; feN.ap = 0.5; feN.Lam = 0.0; feN.alpha = 1.0; feN.sw = 0.0;
+        FC fnN = feN;
+        double dEN = 0.0, dFN = 0.0;
+        ZP zN;
+        const bool row_in = jn < g.ny;                 // block-uniform
+        const bool row_ok = jn <= last_ok;             // block-uniform
+        const bool ringed = row_ok && col_ok;
+        if (ringed) {
+            feN.ap = rg[9][t]; feN.Lam = rg[10][t]; feN.alpha = rg[11][t]; feN.sw = rg[12][t];
+            fnN.ap = rg[13][t]; fnN.Lam = rg[14][t]; fnN.alpha = rg[15][t]; fnN.sw = rg[16][t];
+            dEN = rg[17][t];
+            if (has_dF) dFN = mf.dF[(long long)jn * g.nx + ii];
+        } else if (row_in) {
+            if (east_valid || col_ok) {
+                if (use_xlo || xmode == 1) { if (i < 0) feN = load_fc(mf.xlo, g.ny, jn); }
+                else feN = load_fc(mf.fE, N, (long long)jn * g.nx + ii);
+            }
+            if (xmode == 0) {
+                const long long idn = (long long)jn * g.nx + ii;
+                fnN = load_fc(mf.fN, N, idn);
+                dEN = mf.dE[idn];
+                if (has_dF) dFN = mf.dF[idn];
+            }
+        }
+        if (row_ok) {
+            FC fwN;
+            fwN.ap = __shfl_up_sync(0xffffffffu, feN.ap, 1); fwN.Lam = __shfl_up_sync(0xffffffffu, feN.Lam, 1);
+            fwN.alpha = __shfl_up_sync(0xffffffffu, feN.alpha, 1); fwN.sw = __shfl_up_sync(0xffffffffu, feN.sw, 1);
+            if (col_ok) {
+                if (t == 0) { const double* rw = ringw[jn % RC_NST]; fwN.ap = rw[0]; fwN.Lam = rw[1]; fwN.alpha = rw[2]; fwN.sw = rw[3]; }
+                JC J;
+                J.xx0 = rg[0][t]; J.xx1 = rg[1][t]; J.xx2 = rg[2][t]; J.xy0 = rg[3][t]; J.xy1 = rg[4][t]; J.xy2 = rg[5][t];
+                J.yy0 = rg[6][t]; J.yy1 = rg[7][t]; J.yy2 = rg[8][t];
+                if (sizeof(TIN) == 8) { zN.v0 = rg[18][t]; zN.v1 = rg[19][t]; zN.v2 = rg[20][t]; }
+                else {
+                    zN.v0 = (double)*reinterpret_cast<const float*>(&rg[18][t]); zN.v1 = (double)*reinterpret_cast<const float*>(&rg[19][t]);
+                    zN.v2 = (double)*reinterpret_cast<const float*>(&rg[20][t]);
+                }
+                solve_diag(feN, fwN, fnN, S.fn, J, dEN, dFN, rx, ry, c2, zN.v0, zN.v1, zN.v2, zN.zE, zN.zFx, zN.zFy);
+                zN.Pxx = c2 * (J.xx0 * zN.zE + J.xx1 * zN.zFx + J.xx2 * zN.zFy);
+                zN.Pxy = c2 * (J.xy0 * zN.zE + J.xy1 * zN.zFx + J.xy2 * zN.zFy);
+                zN.Pyy = c2 * (J.yy0 * zN.zE + J.yy1 * zN.zFx + J.yy2 * zN.zFy);
+            } else zN = load_zp<true, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, jn, mf.halo[0], mf.halo[1]);
+        } else zN = load_zp<true, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, jn, mf.halo[0], mf.halo[1]);
+        rc_current_row<DOT>(S, zN, feN, fnN, dEN, dFN, upd, id, N, add, aux, out, rx, ry, sc, acc);
+    }
+    cp_async_wait<0>();
+    if (DOT == 1) reduce_and_finish<2, TXO>(acc, W, BICG_ALPHA, 0);
+    if (DOT == 2) reduce_and_finish<2, TXO>(acc, W, BICG_OMEGA, 0);
+}
+
+static dim3 op_mf_grid(const Grid& g, int sm_count, int* RYout, int ry_cap = OP_RY)
 {
     const int strips = (g.nx + (TXO - 2) - 1) / (TXO - 2);
     long long want = ((long long)g.ny * strips + (long long)sm_count * 64 - 1) / ((long long)sm_count * 64);
-    int RY = (int)(want < 4 ? 4 : (want > OP_RY ? OP_RY : want));
+    int RY = (int)(want < 4 ? 4 : (want > ry_cap ? ry_cap : want));
     if (RY > g.ny) RY = g.ny;
     *RYout = RY;
     return dim3(strips, (g.ny + RY - 1) / RY);
@@ -190,9 +437,13 @@ int op_mf_blocks(const Grid& g, int sm_count) { int RY; const dim3 d = op_mf_gri
 cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                              const int* skip_flag, int dot, const double* aux, GmresWork W, int sm_count, cudaStream_t st)
 {
-    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY);
+    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, mf.rc ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
-    if (dot == 1) op_mf_kernel<true, 1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+    if (mf.rc) {
+        if (dot == 1) op_mf_rc_kernel<1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+        else op_mf_rc_kernel<2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+    }
+    else if (dot == 1) op_mf_kernel<true, 1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
     else op_mf_kernel<true, 2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
     return cudaGetLastError();
 }
@@ -201,10 +452,11 @@ cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Mi
 cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Minv, const float* v, double* out,
                              const double* scale_ptr, const int* skip_flag, int sm_count, cudaStream_t st)
 {
-    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY);
+    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, mf.rc ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
     GmresWork none; memset(&none, 0, sizeof none);
-    op_mf_kernel<true, 0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    if (mf.rc) op_mf_rc_kernel<0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    else op_mf_kernel<true, 0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     return cudaGetLastError();
 }
 
@@ -240,10 +492,11 @@ cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, 
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
                          int sm_count, cudaStream_t st)
 {
-    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY);
+    int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, (precond && mf.rc) ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
     GmresWork none; memset(&none, 0, sizeof none);
-    if (precond) op_mf_kernel<true, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    if (precond && mf.rc) op_mf_rc_kernel<0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    else if (precond) op_mf_kernel<true, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     else op_mf_kernel<false, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     return cudaGetLastError();
 }
