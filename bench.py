@@ -243,10 +243,10 @@ def aggregate_over_ranks(elapsed_s, units, dist=None):
 
 def iteration_bytes_per_cell(iters, m=RESTART, operator=0):
     """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
-    operator 336 (block stencil) or 192 (matrix-free with the diagonal block rebuilt in the kernel, the default; 264 when it loads M^-1); one-pass classical Gram-Schmidt at inner index j: dots 24 (j+2),
+    operator 336 (block stencil) or 136 (matrix-free with the diagonal block and J rebuilt in the kernel, the default; 264 when it loads M^-1 and J); one-pass classical Gram-Schmidt at inner index j: dots 24 (j+2),
     update+norm 24 (j+3); one extra read of w per 16-vector pass (option vectors_per_pass, default 16 by measurement); per cycle: combine 8 (3 jj + 15) + true residual
     (block stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24."""
-    op = 336.0 if operator == 0 else 192.0
+    op = 336.0 if operator == 0 else 136.0
     res = 480.0 if operator == 0 else 216.0
     total, done = 0.0, 0
     while done < iters:
@@ -261,10 +261,10 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0):
 
 def bicgstab_bytes_per_cell(iters, operator=1):
     """Algorithmic bytes per cell of `iters` BiCGStab iterations as built.  Matrix-free operator (reductions fused into the
-    operator kernel): p update 96 + [A M^-1 p with <r^,v>] 216 + s update 72 + [A M^-1 s with <t,s>,<t,t>] 192 + y/r update with
-    rho, ||r|| 168 = 744.  Block stencil: 2 x 336 + 96 + 48 + 72 + 72 + 168 = 1128.  One cycle end: x += M^-1 y (168), true
+    operator kernel): p update 96 + [A M^-1 p with <r^,v>] 160 + s update 72 + [A M^-1 s with <t,s>,<t,t>] 136 + y/r update with
+    rho, ||r|| 168 = 632.  Block stencil: 2 x 336 + 96 + 48 + 72 + 72 + 168 = 1128.  One cycle end: x += M^-1 y (168), true
     residual, norm (24), cycle start (96)."""
-    per_it = 744.0 if operator == 1 else 1128.0
+    per_it = 632.0 if operator == 1 else 1128.0
     res = 480.0 if operator == 0 else 216.0
     return iters * per_it + 168.0 + res + 24.0 + 96.0
 
@@ -531,7 +531,7 @@ def run_ours(args):
                     tm = g.timings()
                     cbo[label][f"{ratio:g}x"] = {"iterations": its, "final_residual": res, "converged": bool(res <= TOL), "ms": ms,
                                                  "ms_per_iteration": tm["krylov_ms"] / max(its, 1),
-                                                 "bytes_per_cell_per_iteration_mean_m30": 612, "T_implicit_over_T_explicit": ms / ms_exp}
+                                                 "bytes_per_cell_per_iteration_mean_m30": 556, "T_implicit_over_T_explicit": ms / ms_exp}
             reset_device(); one_step()
             torch.cuda.synchronize()
             e0.record(stream)

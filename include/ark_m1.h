@@ -100,10 +100,12 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                          row ahead of the faces, cp.async row prefetch (default)
  *   "operator"          1: matrix-free coefficient planes, flux form (default: 5% faster per solve at 4096^2)
  *                       0: block stencil (BSR 3x3 on the 5-point graph, pre-multiplied by M^-1)
- *   "op_recompute"      1 (default): the preconditioned matrix-free operator rebuilds each cell's diagonal block from J and the
- *                          four faces' coefficients, which it loads anyway, and solves the 3 x 3 system in registers: 192 B per
- *                          cell per application.  0: it loads the nine stored M^-1 planes (264 B).  Same operator up to the
- *                          rounding of M^-1; cells with folded neighbours (outflow sides) always use the stored inverse
+ *   "op_recompute"      what the preconditioned matrix-free operator rebuilds in registers instead of loading it (same operator up
+ *                          to rounding; cells with folded neighbours (outflow sides) and clamped cells always use the stored values):
+ *                          2 (default): each cell's diagonal block, from J and the four faces' coefficients (3 x 3 solve in place of
+ *                             the nine M^-1 planes), and J itself from the cell's reduced flux (2 planes in place of 9):
+ *                             136 B per cell per application; needs the default scheme and the marching assembly, else acts as 1
+ *                          1: the diagonal block only: 192 B     0: nothing, M^-1 and J are loaded: 264 B
  *   "apply_operator_precond"  1: ark_m1_apply_operator returns A M^-1 V through the solver's preconditioned kernel (matrix-free
  *                          operator only); 0 (default): A V
  *   "basis_precision"   64 (default) or 32: storage precision of the GMRES Arnoldi basis.  32 = compressed-basis GMRES: the basis

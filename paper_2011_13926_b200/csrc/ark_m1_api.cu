@@ -84,7 +84,7 @@ void ark_dfree(ark_m1* h, void* p)
 // the multigrid hierarchy is built from assembled blocks: it overrides the matrix-free operator
 static inline int opk(const ark_m1* h) { return h->precond == 1 ? 0 : h->op_kind; }
 // bytes per cell the preconditioned matrix-free operator does not move when it rebuilds the diagonal block (the nine M^-1 planes)
-static inline double mf_saved(const ark_m1* h) { return h->mf.rc ? 72.0 : 0.0; }
+static inline double mf_saved(const ark_m1* h) { return h->mf.rc ? (h->mf.rcj ? 128.0 : 72.0) : 0.0; }
 
 // compressed-basis GMRES applies to the default solver configuration only; elsewhere the option is ignored
 static inline bool use_cb(const ark_m1* h) { return h->basis_prec == 32 && h->krylov == 0 && h->precond == 0 && h->op_kind == 1 && h->ortho == 1; }
@@ -126,7 +126,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
-    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 1; h->apply_precond = 0;
+    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 2; h->apply_precond = 0;
     h->basis_prec = 64; h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -160,7 +160,7 @@ static void free_implicit(ark_m1* h)
     h->mg.nlev = 0; ark_dfree(h, h->mgz); h->mgz = nullptr;
     ark_dfree(h, h->V32); h->V32 = nullptr; ark_dfree(h, h->wk); h->wk = nullptr; h->m32_alloc = 0; h->vslots = 0;
     ark_dfree(h, h->A.off); ark_dfree(h, h->A.C); ark_dfree(h, h->A.Minv); ark_dfree(h, h->A.b); ark_dfree(h, h->V); ark_dfree(h, h->tvec); cudaFree(h->wblock); ark_dfree(h, h->nprev); h->nprev = nullptr;
-    ark_dfree(h, h->mf.J); ark_dfree(h, h->mf.fE); ark_dfree(h, h->mf.fN); ark_dfree(h, h->mf.dE); ark_dfree(h, h->mf.dF); ark_dfree(h, h->mf.xlo); ark_dfree(h, h->mf.ylo);
+    ark_dfree(h, h->mf.J); ark_dfree(h, h->mf.fE); ark_dfree(h, h->mf.fN); ark_dfree(h, h->mf.dE); ark_dfree(h, h->mf.dF); ark_dfree(h, h->mf.fxy); ark_dfree(h, h->mf.xlo); ark_dfree(h, h->mf.ylo);
     memset(&h->mf, 0, sizeof h->mf);
     h->A.off = h->A.C = h->A.Minv = h->A.b = nullptr; h->V = h->tvec = nullptr; h->wblock = nullptr; h->m_alloc = 0; h->maxit_alloc = 0;
 }
@@ -251,7 +251,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "kernel_timing")) { ark_kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
     else if (!strcmp(key, "apply_operator_precond")) h->apply_precond = (value != 0.0);
-    else if (!strcmp(key, "op_recompute")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "op_recompute must be 0 (load M^-1) or 1 (rebuild the diagonal block in the operator)%s", ""); h->op_recompute = iv; }
+    else if (!strcmp(key, "op_recompute")) { if (iv < 0 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "op_recompute must be 0 (load M^-1), 1 (rebuild the diagonal block in the operator) or 2 (rebuild J as well)%s", ""); h->op_recompute = iv; }
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
     else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return ark_fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
     else if (!strcmp(key, "mg_coarse_sweeps")) { if (iv < 1) return ark_fail(h, ARK_M1_E_ARG, "mg_coarse_sweeps must be >= 1%s", ""); h->mg.coarse_sweeps = iv; }
@@ -408,6 +408,7 @@ int ark_ensure_implicit(ark_m1* h, int m, int maxit)
         if ((rc = ark_dmalloc(h, (void**)&h->mf.fN, 4 * N * sizeof(double)))) return rc;
         if ((rc = ark_dmalloc(h, (void**)&h->mf.dE, N * sizeof(double)))) return rc;
         if ((rc = ark_dmalloc(h, (void**)&h->mf.dF, N * sizeof(double)))) return rc;
+        if ((rc = ark_dmalloc(h, (void**)&h->mf.fxy, 2 * N * sizeof(double)))) return rc;
         if ((rc = ark_dmalloc(h, (void**)&h->mf.xlo, 4 * (size_t)h->g.ny * sizeof(double)))) return rc;
         if ((rc = ark_dmalloc(h, (void**)&h->mf.ylo, 4 * (size_t)h->g.nx * sizeof(double)))) return rc;
     }
@@ -509,6 +510,9 @@ int ark_assemble_system(ark_m1* h, double dt, const double* bsrc)
     if (opk(h) == 1) {
         h->mf.rx = h->s.hyp_off ? 0.0 : dt / h->g.dx; h->mf.ry = h->s.hyp_off ? 0.0 : dt / h->g.dy;
         h->mf.rc = h->op_recompute; h->mf.has_dF = (h->s.wb == 0);
+        // the reduced-flux planes are written by the marching assembly; the M1 Jacobian formula holds for the default scheme
+        h->mf.rcj = (h->op_recompute == 2 && h->s.is_default() && h->asm_kernel == 1 && h->N < (1LL << 31)) ? 1 : 0;
+        h->mf.rc = h->op_recompute ? 1 : 0;
         if (h->asm_kernel == 1 && h->N < (1LL << 31))
             KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble_march(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->sm_count, h->st));
         else

@@ -86,7 +86,9 @@ struct MfPlanes {
     double* ylo;   // [4][nx] : south face of row 0 (non-periodic y)
     double rx, ry; // dt/dx, dt/dy of the assembled step
     const double* halo[2];   // slab decomposition (BC_HALO sides): received (z, c^2 J z) of the row below / above, [6][nx] each
+    double* fxy;   // 2 planes: reduced flux (fx, fy) of the cell; fx = 4 marks a cell whose J is not the M1 closure's (clamped)
     int rc;        // 1: the preconditioned operator rebuilds the diagonal block from J and the faces instead of loading M^-1 (operator_mf.cu)
+    int rcj;       // 1 (with rc): it also rebuilds J from (fx, fy) instead of loading its nine planes (default scheme, marching assembly)
     int has_dF;    // 0: dF is identically zero (WB source) and is not loaded
 };
 // A.off / A.C may be null when mf.J is set (then only Minv, b and the coefficient planes are written)

@@ -141,6 +141,14 @@ __global__ void __launch_bounds__(TXA) assemble_march_kernel(Grid g, Scheme s, F
             mf.fE[id] = fe.ap; mf.fE[N + id] = fe.Lam; mf.fE[2 * N + id] = fe.alpha; mf.fE[3 * N + id] = se;
             mf.fN[id] = fn.ap; mf.fN[N + id] = fn.Lam; mf.fN[2 * N + id] = fn.alpha; mf.fN[3 * N + id] = sn;
             mf.dE[id] = dE;
+            {   // reduced flux for the operator that rebuilds J (operator_mf.cu): the same sequence as closure_eval's, so that the
+                // clamp decision is the one the stored J was formed with
+                const double Es = (C.u.E > ARK_E_FLOOR) ? C.u.E : ARK_E_FLOOR;
+                const double ice = rcp_sel<true>(c * Es);
+                const double fx = C.u.Fx * ice, fy = C.u.Fy * ice;
+                const double f2 = fx * fx + fy * fy;
+                mf.fxy[id] = (f2 > 1.0) ? 4.0 : fx; mf.fxy[N + id] = fy;
+            }
             mf.dF[id] = wb ? 0.0 : cdt * C.u.st;
             if (i == 0) { mf.xlo[j] = fw.ap; mf.xlo[g.ny + j] = fw.Lam; mf.xlo[2 * g.ny + j] = fw.alpha; mf.xlo[3 * g.ny + j] = sw; }
             if (j == 0) { mf.ylo[i] = fs.ap; mf.ylo[g.nx + i] = fs.Lam; mf.ylo[2 * g.nx + i] = fs.alpha; mf.ylo[3 * g.nx + i] = ss; }

@@ -399,7 +399,7 @@ static int group_operator(ark_m1_group* G, size_t v_off, bool v_is_x, size_t out
         ark_m1* h = s.h;
         const double* v = v_is_x ? h->U[h->cur] : h->V + v_off * h->stride;
         const int* stop = use_stop ? &h->W.ctl->inner_stop : nullptr;
-        ark_kmark(h, KC_SPMV, (precond ? (h->mf.rc ? 192.0 : 264.0) : 216.0) * h->N);
+        ark_kmark(h, KC_SPMV, (precond ? (h->mf.rc ? (h->mf.rcj ? 136.0 : 192.0) : 264.0) : 216.0) * h->N);
         GCU(launch_op_mf(h->g, h->mf, h->A.Minv, v, h->V + out_off * h->stride, scale_idx >= 0 ? h->W.scale + scale_idx : nullptr,
                          add_b ? h->A.b : nullptr, sgn, stop, precond, h->sm_count, G->st));
     }

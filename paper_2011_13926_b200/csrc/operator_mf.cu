@@ -209,12 +209,35 @@ __device__ __forceinline__ void solve_diag(const FC& e, const FC& w, const FC& n
     zFy = (c02 * v0 + (m01 * m20 - m00 * m21) * v1 + (m00 * m11 - m01 * m10) * v2) * id;
 }
 
+// The pressure Jacobian of the M1 closure from the reduced flux (closure_eval's formulas, m1_device.cuh; |f| <= 1, not clamped):
+// with it the operator loads (fx, fy) instead of the nine J planes, 192 -> 136 B per cell per application.
+__device__ __forceinline__ void jac_from_f(double fx, double fy, double ic, JC& J)
+{
+    const double f2 = fma(fx, fx, fy * fy);
+    const double s = fma(-3.0, f2, 4.0);                  // xi^2 >= 1
+    const double ixi = rsqrt_fast(s), xi = s * ixi;
+    const double q3 = 3.0 * rcp_fast(2.0 + xi);           // (3 chi - 1)/(2 f^2) = 3/(2 + xi)
+    const double iso = 0.33333333333333333333 * (xi - 1.0);   // (1 - chi)/2 with chi = (5 - 2 xi)/3
+    const double qx = q3 * fx, qy = q3 * fy;
+    const double Dxx = fma(qx, fx, iso), Dxy = qx * fy, Dyy = fma(qy, fy, iso);
+    const double t3 = q3 * q3 * ixi;
+    const double txx = t3 * fx * fx, txy = t3 * fx * fy, tyy = t3 * fy * fy, fxi = fx * ixi, fyi = fy * ixi;
+    J.xx0 = fma(f2 - 3.0 * fx * fx, ixi, Dxx); J.xy0 = fma(-3.0 * fx * fy, ixi, Dxy); J.yy0 = fma(f2 - 3.0 * fy * fy, ixi, Dyy);
+    J.xx1 = ic * (fma(txx, fx, 2.0 * qx) - fxi); J.xx2 = ic * fma(txx, fy, -fyi);
+    J.xy1 = ic * fma(txy, fx, qy);               J.xy2 = ic * fma(txy, fy, qx);
+    J.yy1 = ic * fma(tyy, fx, -fxi);             J.yy2 = ic * (fma(tyy, fy, 2.0 * qy) - fyi);
+}
+
 // 12 resident blocks per SM (160 registers) and 64 rows per block (the two prologue rows of a block take z from the stored M^-1):
 // 16 blocks x 32 rows 0.630 ms, 16 x 64 0.618, 12 x 32 0.578, 12 x 64 0.573, 10 x 64 0.574, 20 x 32 (spills) 1.10 at 4096^2.
 static constexpr int OP_RC_MINB = 12;
+static constexpr int OP_RCJ_MINB = 14;    // with J rebuilt too (128 registers, 7 KB ring): 10 / 12 / 13 / 14 / 15 / 16 blocks: 0.508 / 0.506 / 0.482 / 0.473 / 0.487 / 0.486 ms;
+                                          // rows per block 44 / 59 / 96 / 128: 0.471 / 0.474 / 0.480 / 0.498; a third ring stage 0.516
 static constexpr int OP_RC_RY = 64;
 static constexpr int RC_NST = 2;          // ring stages: row j+1 landed, row j+2 in flight during step j
-static constexpr int RC_NF = 21;          // ring fields per cell: J (9), east face (4), north face (4), dE, v (3)
+// ring fields per cell: J (9) — or, when J is rebuilt too, the reduced flux (2) —, east face (4), north face (4), dE, v (3)
+__host__ __device__ constexpr int rc_nj(bool jrc) { return jrc ? 2 : 9; }
+__host__ __device__ constexpr int rc_nf(bool jrc) { return rc_nj(jrc) + 12; }
 
 // The row after the row ahead travels HBM -> shared memory with cp.async while the block works (the explicit kernel's ring):
 // a warp's row step is one long dependent chain (loads -> block -> 3 x 3 solve -> c^2 J z -> fluxes -> store), and with the loads
@@ -224,23 +247,27 @@ static constexpr int RC_NF = 21;          // ring fields per cell: J (9), east f
 // memory carve-out leaves too few); the same ring filled by 1-D bulk copies (cp.async.bulk + mbarrier, one 272-byte copy per plane
 // row: ptxas serialises the 21 copies of a row in an ELECT loop, 0.61 / 0.63 / 0.71 ms with 2 / 3 / 4 stages); a branch-free row
 // step for interior strips (0.570 against 0.574).
-template <typename TIN>
+template <bool JRC, typename TIN>
 __device__ __forceinline__ void rc_issue(double (*ring)[TXO], double* ringw, int t, const MfPlanes& mf, const TIN* __restrict__ v,
                                          long long N, long long idn, bool want)
 {
+    constexpr int NJ = rc_nj(JRC);
     if (want) {
+        if (JRC) { cp_async8(&ring[0][t], mf.fxy + idn); cp_async8(&ring[1][t], mf.fxy + N + idn); }
+        else {
 #pragma unroll
-        for (int e = 0; e < 9; ++e) cp_async8(&ring[e][t], mf.J + e * N + idn);
+            for (int e = 0; e < 9; ++e) cp_async8(&ring[e][t], mf.J + e * N + idn);
+        }
 #pragma unroll
-        for (int e = 0; e < 4; ++e) { cp_async8(&ring[9 + e][t], mf.fE + e * N + idn); cp_async8(&ring[13 + e][t], mf.fN + e * N + idn); }
-        cp_async8(&ring[17][t], mf.dE + idn);
+        for (int e = 0; e < 4; ++e) { cp_async8(&ring[NJ + e][t], mf.fE + e * N + idn); cp_async8(&ring[NJ + 4 + e][t], mf.fN + e * N + idn); }
+        cp_async8(&ring[NJ + 8][t], mf.dE + idn);
         if (sizeof(TIN) == 8) {
 #pragma unroll
-            for (int e = 0; e < 3; ++e) cp_async8(&ring[18 + e][t], reinterpret_cast<const double*>(v) + e * N + idn);
+            for (int e = 0; e < 3; ++e) cp_async8(&ring[NJ + 9 + e][t], reinterpret_cast<const double*>(v) + e * N + idn);
         } else {
 #pragma unroll
             for (int e = 0; e < 3; ++e) {
-                const unsigned int d = (unsigned int)__cvta_generic_to_shared(&ring[18 + e][t]);
+                const unsigned int d = (unsigned int)__cvta_generic_to_shared(&ring[NJ + 9 + e][t]);
                 asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(d), "l"(v + e * N + idn) : "memory");
             }
         }
@@ -294,13 +321,14 @@ __device__ __forceinline__ void rc_current_row(RcState& S, const ZP& zN, const F
     S.fe = feN; S.fn = fnN; S.dE = dEN; S.dF = dFN;
 }
 
-template <int DOT, typename TIN = double>
-__global__ void __launch_bounds__(TXO, OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
+template <int DOT, typename TIN = double, bool JRC = false>
+__global__ void __launch_bounds__(TXO, JRC ? OP_RCJ_MINB : OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
                                                     double* __restrict__ out, const double* __restrict__ scale_ptr,
                                                     const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
                                                     int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W)
 {
     if (skip_flag && *skip_flag) return;
+    constexpr int NJ = rc_nj(JRC), RC_NF = rc_nf(JRC);
     __shared__ double ring[RC_NST][RC_NF][TXO];     // row r lives in ring[r % RC_NST]
     __shared__ double ringw[RC_NST][4];             // lane 0: the east face of the column west of the strip
     double acc[2] = { 0.0, 0.0 };
@@ -327,12 +355,13 @@ __global__ void __launch_bounds__(TXO, OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPla
     const int last_ok = (g.bc[YHI] == BC_OUTFLOW) ? g.ny - 2 : g.ny - 1;      // last row whose block is built here (block-uniform)
     const double sc = sgn * (scale_ptr ? *scale_ptr : 1.0);
     const bool has_dF = mf.has_dF != 0;
+    const double ic = 1.0 / g.c;
 
     const int last_row = min(j1, last_ok);      // last row requested into the ring
     // request rows j0+1 .. j0+RC_NST-1 first: row j0+1 is consumed by the first row step
 #pragma unroll
     for (int r = 1; r < RC_NST; ++r)
-        rc_issue<TIN>(ring[(j0 + r) % RC_NST], ringw[(j0 + r) % RC_NST], t, mf, v, N, (long long)(j0 + r) * g.nx + ii, col_ok && j0 + r <= last_row);
+        rc_issue<JRC, TIN>(ring[(j0 + r) % RC_NST], ringw[(j0 + r) % RC_NST], t, mf, v, N, (long long)(j0 + r) * g.nx + ii, col_ok && j0 + r <= last_row);
 
     RcState S;
     {
@@ -366,7 +395,7 @@ __global__ void __launch_bounds__(TXO, OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPla
         const int jn = j + 1;
         const long long id = (long long)j * g.nx + (upd ? i : 0);
         // ---- request row j+RC_NST into the slot of row j (read one step ago), then wait for row j+1
-        rc_issue<TIN>(ring[j % RC_NST], ringw[j % RC_NST], t, mf, v, N, (long long)(j + RC_NST) * g.nx + ii, col_ok && j + RC_NST <= last_row);
+        rc_issue<JRC, TIN>(ring[j % RC_NST], ringw[j % RC_NST], t, mf, v, N, (long long)(j + RC_NST) * g.nx + ii, col_ok && j + RC_NST <= last_row);
         cp_async_wait<RC_NST - 1>();
         double (*rg)[TXO] = ring[jn % RC_NST];
         // ---- the row ahead: its faces, then z = M^-1 v either from the block built here or from the stored inverse
@@ -378,9 +407,9 @@ __global__ void __launch_bounds__(TXO, OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPla
         const bool row_ok = jn <= last_ok;             // block-uniform
         const bool ringed = row_ok && col_ok;
         if (ringed) {
-            feN.ap = rg[9][t]; feN.Lam = rg[10][t]; feN.alpha = rg[11][t]; feN.sw = rg[12][t];
-            fnN.ap = rg[13][t]; fnN.Lam = rg[14][t]; fnN.alpha = rg[15][t]; fnN.sw = rg[16][t];
-            dEN = rg[17][t];
+            feN.ap = rg[NJ][t]; feN.Lam = rg[NJ + 1][t]; feN.alpha = rg[NJ + 2][t]; feN.sw = rg[NJ + 3][t];
+            fnN.ap = rg[NJ + 4][t]; fnN.Lam = rg[NJ + 5][t]; fnN.alpha = rg[NJ + 6][t]; fnN.sw = rg[NJ + 7][t];
+            dEN = rg[NJ + 8][t];
             if (has_dF) dFN = mf.dF[(long long)jn * g.nx + ii];
         } else if (row_in) {
             if (east_valid || col_ok) {
@@ -401,12 +430,22 @@ __global__ void __launch_bounds__(TXO, OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPla
             if (col_ok) {
                 if (t == 0) { const double* rw = ringw[jn % RC_NST]; fwN.ap = rw[0]; fwN.Lam = rw[1]; fwN.alpha = rw[2]; fwN.sw = rw[3]; }
                 JC J;
-                J.xx0 = rg[0][t]; J.xx1 = rg[1][t]; J.xx2 = rg[2][t]; J.xy0 = rg[3][t]; J.xy1 = rg[4][t]; J.xy2 = rg[5][t];
-                J.yy0 = rg[6][t]; J.yy1 = rg[7][t]; J.yy2 = rg[8][t];
-                if (sizeof(TIN) == 8) { zN.v0 = rg[18][t]; zN.v1 = rg[19][t]; zN.v2 = rg[20][t]; }
+                if (JRC) {
+                    const double fx = rg[0][t], fy = rg[1][t];
+                    if (fx > 2.0) {      // clamped cell: its J is not the M1 closure's; take the stored one
+                        const long long idn = (long long)jn * g.nx + ii;
+                        J.xx0 = mf.J[0 * N + idn]; J.xx1 = mf.J[1 * N + idn]; J.xx2 = mf.J[2 * N + idn];
+                        J.xy0 = mf.J[3 * N + idn]; J.xy1 = mf.J[4 * N + idn]; J.xy2 = mf.J[5 * N + idn];
+                        J.yy0 = mf.J[6 * N + idn]; J.yy1 = mf.J[7 * N + idn]; J.yy2 = mf.J[8 * N + idn];
+                    } else jac_from_f(fx, fy, ic, J);
+                } else {
+                    J.xx0 = rg[0][t]; J.xx1 = rg[1][t]; J.xx2 = rg[2][t]; J.xy0 = rg[3][t]; J.xy1 = rg[4][t]; J.xy2 = rg[5][t];
+                    J.yy0 = rg[6][t]; J.yy1 = rg[7][t]; J.yy2 = rg[8][t];
+                }
+                if (sizeof(TIN) == 8) { zN.v0 = rg[NJ + 9][t]; zN.v1 = rg[NJ + 10][t]; zN.v2 = rg[NJ + 11][t]; }
                 else {
-                    zN.v0 = (double)*reinterpret_cast<const float*>(&rg[18][t]); zN.v1 = (double)*reinterpret_cast<const float*>(&rg[19][t]);
-                    zN.v2 = (double)*reinterpret_cast<const float*>(&rg[20][t]);
+                    zN.v0 = (double)*reinterpret_cast<const float*>(&rg[NJ + 9][t]); zN.v1 = (double)*reinterpret_cast<const float*>(&rg[NJ + 10][t]);
+                    zN.v2 = (double)*reinterpret_cast<const float*>(&rg[NJ + 11][t]);
                 }
                 solve_diag(feN, fwN, fnN, S.fn, J, dEN, dFN, rx, ry, c2, zN.v0, zN.v1, zN.v2, zN.zE, zN.zFx, zN.zFy);
                 zN.Pxx = c2 * (J.xx0 * zN.zE + J.xx1 * zN.zFx + J.xx2 * zN.zFy);
@@ -439,7 +478,10 @@ cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Mi
 {
     int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, mf.rc ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
-    if (mf.rc) {
+    if (mf.rc && mf.rcj) {
+        if (dot == 1) op_mf_rc_kernel<1, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+        else op_mf_rc_kernel<2, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+    } else if (mf.rc) {
         if (dot == 1) op_mf_rc_kernel<1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
         else op_mf_rc_kernel<2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
     }
@@ -455,7 +497,8 @@ cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Mi
     int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, mf.rc ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
     GmresWork none; memset(&none, 0, sizeof none);
-    if (mf.rc) op_mf_rc_kernel<0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    if (mf.rc && mf.rcj) op_mf_rc_kernel<0, float, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    else if (mf.rc) op_mf_rc_kernel<0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     else op_mf_kernel<true, 0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     return cudaGetLastError();
 }
@@ -495,7 +538,8 @@ cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, 
     int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, (precond && mf.rc) ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
     GmresWork none; memset(&none, 0, sizeof none);
-    if (precond && mf.rc) op_mf_rc_kernel<0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    if (precond && mf.rc && mf.rcj) op_mf_rc_kernel<0, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    else if (precond && mf.rc) op_mf_rc_kernel<0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     else if (precond) op_mf_kernel<true, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     else op_mf_kernel<false, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
     return cudaGetLastError();

@@ -22,7 +22,7 @@ def _check(w, opts=None, K=20.0):
     ref_solver = make_gpu(w, dict(base, op_recompute=0))
     ref = ref_solver.apply_operator(dt, ref_solver.apply_preconditioner(dt, V))
     scale = np.max(np.abs(ref))
-    for rc in (0, 1):
+    for rc in (0, 1, 2):
         g = make_gpu(w, dict(base, op_recompute=rc, apply_operator_precond=1))
         got = g.apply_operator(dt, V)
         err = np.max(np.abs(got - ref)) / scale
@@ -58,16 +58,29 @@ def test_recomputed_block_with_matter_coupling_and_large_dt():
     _check(w, K=200.0)
 
 
+def test_recomputed_jacobian_with_clamped_and_nonpositive_cells():
+    # |F| > cE in many cells (their J is the clamped closure's, taken from the stored planes), E <= 0 in a few, f = 1 exactly in a row
+    w = small_random_state(157, 90, seed=41, fmax=1.7, bc=(0, 0, 2, 1), c=1.3)
+    rng = np.random.default_rng(8)
+    bad = rng.integers(0, w["nx"] * w["ny"], size=40)
+    w["E"].reshape(-1)[bad] = -w["E"].reshape(-1)[bad]
+    w["E"][7, :] = 2.0 ** rng.integers(-2, 3, w["nx"])
+    w["F"][0, 7, :] = 0.0
+    w["F"][1, 7, :] = w["c"] * w["E"][7, :]
+    _check(w, K=5.0)
+
+
 def test_solver_iteration_counts_do_not_depend_on_the_variant():
     import m1_workloads as wl
     w = wl.random_medium(256, seed=5)
     dt = 20 * wl.explicit_dt(w["dx"], w["dy"], w["c"])
     res = []
-    for rc in (0, 1):
+    for rc in (0, 1, 2):
         g = make_gpu(w, dict(op_recompute=rc))
         its, r = g.step_implicit(dt, 1e-10, 30, 2000)
         res.append((its, g.get_state()))
         assert r <= 1e-10
-    assert abs(res[0][0] - res[1][0]) <= 1
-    for a, b in zip(res[0][1], res[1][1]):
-        assert np.max(np.abs(a - b)) <= 1e-9 * np.max(np.abs(b))
+    for k in (1, 2):
+        assert abs(res[0][0] - res[k][0]) <= 1
+        for a, b in zip(res[0][1], res[k][1]):
+            assert np.max(np.abs(a - b)) <= 1e-9 * np.max(np.abs(b))
