@@ -126,7 +126,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
-    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 2; h->apply_precond = 0;
+    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 2; h->apply_precond = 0; h->arnoldi_block = 2;
     h->basis_prec = 64; h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -251,6 +251,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "kernel_timing")) { ark_kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
     else if (!strcmp(key, "apply_operator_precond")) h->apply_precond = (value != 0.0);
+    else if (!strcmp(key, "arnoldi_block")) { if (iv < 1 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "arnoldi_block must be 1 (one column per pass over the basis) or 2 (two columns)%s", ""); h->arnoldi_block = iv; }
     else if (!strcmp(key, "op_recompute")) { if (iv < 0 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "op_recompute must be 0 (load M^-1), 1 (rebuild the diagonal block in the operator) or 2 (rebuild J as well)%s", ""); h->op_recompute = iv; }
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
     else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return ark_fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
@@ -467,7 +468,7 @@ int ark_ensure_implicit(ark_m1* h, int m, int maxit)
     long long caph = (long long)mi + mi / (mm > 0 ? mm : 1) + 8;
     if (caph > (1LL << 20)) caph = (1LL << 20);     // the history keeps at most 2^20 entries (later ones are counted, not stored)
     const int caphist = (int)caph;
-    const size_t nd = (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 2 * (size_t)(mm + 1) + caphist
+    const size_t nd = 2 * (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 5 * (size_t)(mm + 1) + caphist
                       + (size_t)(krylov_max_blocks(h->sm_count) > op_mf_blocks(h->g, h->sm_count) ? krylov_max_blocks(h->sm_count) : op_mf_blocks(h->g, h->sm_count)) * MAXV;
     const size_t ctl_bytes = (sizeof(GmresCtl) + 255) / 256 * 256;
     if (cudaMalloc(&h->wblock, ctl_bytes + nd * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return ark_fail(h, ARK_M1_E_ALLOC, "cudaMalloc (solver scalars)%s", ""); }
@@ -477,7 +478,9 @@ int ark_ensure_implicit(ark_m1* h, int m, int maxit)
     double* p = (double*)((char*)h->wblock + ctl_bytes);
     W.H = p; p += (size_t)(mm + 1) * mm;
     W.cs = p; p += mm; W.sn = p; p += mm; W.g = p; p += mm + 1; W.y = p; p += mm;
-    W.scale = p; p += mm + 1; W.coef = p; p += mm + 1; W.hist = p; p += caphist; W.partial = p;
+    W.scale = p; p += mm + 1; W.coef = p; p += mm + 1; W.hist = p; p += caphist;
+    W.Hraw = p; p += (size_t)(mm + 1) * mm; W.c1 = p; p += mm + 1; W.c2 = p; p += mm + 1; W.coef2 = p; p += mm + 1;
+    W.partial = p;
     W.caphist = caphist;
     h->m_alloc = mm; h->maxit_alloc = mi;
     return 0;
@@ -561,9 +564,32 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
     KL(KC_DOT, 24.0 * h->N, launch_multi_dot(h->A.b, h->A.b, 0, 1, 0, n, W, DOT_BNORM, sm, h->st));
     if ((rc = true_residual(h, x))) return rc;
     if ((rc = ark_fetch_ctl(h))) return rc;
+    // two columns per pass over the basis: GMRES + block-Jacobi + matrix-free operator + one-pass Gram-Schmidt, m within the staged epilogue
+    const bool pair = (h->arnoldi_block == 2 && h->precond == 0 && opk(h) == 1 && h->ortho == 1 && m >= 2 && m <= 128);
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
+            if (pair && j + 1 < m) {
+                // two-column Arnoldi step: W1 = A M^-1 v_j, W2 = A M^-1 W1, both
+                // orthogonalised against v_0..v_j in the same passes over the basis, then W2 against W1'
+                double* w2 = h->V + (size_t)(j + 2) * S;
+                KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
+                KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, w, w2, nullptr, nullptr, 1.0, stop, 1, sm, h->st));
+                const int MV2 = krylov_pair_max_vectors();
+                const int nchunk2 = (j + MV2) / MV2, csize2 = (j + nchunk2) / nchunk2;
+                for (int c0 = 0; c0 <= j; c0 += csize2) {
+                    const int nv = (j + 1 - c0) < csize2 ? (j + 1 - c0) : csize2;
+                    KL(KC_DOT, 24.0 * (nv + 2) * h->N, launch_multi_dot2(w, w2, h->V + (size_t)c0 * S, S, nv, c0, n, W, sm, h->st));
+                }
+                for (int c0 = 0; c0 <= j; c0 += csize2) {
+                    const int nv = (j + 1 - c0) < csize2 ? (j + 1 - c0) : csize2;
+                    const int last = (c0 + csize2 > j);
+                    KL(KC_UPDATE, 24.0 * (nv + 4) * h->N, launch_update2(w, w2, h->V + (size_t)c0 * S, S, nv, c0, n, W, last, sm, h->st));
+                }
+                KL(KC_UPDATE, 72.0 * h->N, launch_update(w2, w, S, 1, j + 1, n, W, 1, sm, h->st, UPD_B2B));
+                ++j;
+                continue;
+            }
             if (h->precond == 1) {          // w = Ahat Mhat^-1 (scale_j v_j): the V-cycle is linear, the scale goes on last
                 if ((rc = mg_apply(h, h->V + (size_t)j * S, h->mgz, stop))) return rc;
                 KL(KC_SPMV, 336.0 * h->N, launch_spmv_hat(h->g, h->A.off, h->mgz, w, W.scale + j, nullptr, 1.0, stop, h->st));

@@ -25,6 +25,7 @@ struct GmresCtl {
     int pad;
     double aux[2];                 // scratch norms (Newton update size)
     double bs[8];                  // BiCGStab scalars: rho, alpha, omega, rho_new, ||r|| (recursive), flag "restart after this iteration"
+    double blk[4];                 // two-column Arnoldi step: r11 = ||W1'||, <W1', W2'>, <W1', W1'>
 };
 
 struct GmresWork {                 // device pointers into one small allocation
@@ -39,6 +40,10 @@ struct GmresWork {                 // device pointers into one small allocation
     double* hist;   // caphist
     double* partial;// [max_blocks][MAXV] block partial sums
     int caphist;
+    double* Hraw;   // (m+1) x m: the Arnoldi columns before the Givens rotations (two-column step only; may be null)
+    double* c1;     // m+1 : <W1, v_i> of the two-column step
+    double* c2;     // m+1 : <W2, v_i>
+    double* coef2;  // m+1 : coefficients of the second vector's update
     double* red_out;// null: the reduction kernels run their scalar epilogue themselves (one GPU).  Non-null (slab decomposition):
                     // they store this rank's sums here instead; all-reduce and launch_epilogue follow
 };
@@ -46,7 +51,10 @@ struct GmresWork {                 // device pointers into one small allocation
 enum { MAXV = 16 };                // basis vectors handled per pass of the multi-vector kernels (the measured optimum: DESIGN.md section 5)
 
 enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4, DOT_NONE = 5, DOT_AUX0 = 6, DOT_AUX1 = 7,
-               BICG_ALPHA = 8, BICG_OMEGA = 9, BICG_RHO = 10 };
+               BICG_ALPHA = 8, BICG_OMEGA = 9, BICG_RHO = 10,
+               DOT_B2 = 11,      // two-column step: <W1, V_i>, <W2, V_i> of a chunk
+               UPD_B2A = 12,     // ... first column finished: <W1', W1'>, <W1', W2'>
+               UPD_B2B = 13 };   // ... second column finished: ||W2''||^2
 enum { BS_RHO = 0, BS_ALPHA = 1, BS_OMEGA = 2, BS_RHO_NEW = 3, BS_RN = 4, BS_RESTART = 5 };
 
 // number of SMs of the CURRENT device (cached per device; ark_m1_api.cu) — grid sizes are multiples of it
@@ -144,7 +152,13 @@ cudaError_t launch_multi_dot(const double* w, const double* V0, long long stride
                              GmresWork W, int mode, int sm_count, cudaStream_t st);
 // w -= sum_k coef[col0+k] V_k ; if with_norm: ||w||^2 -> epilogue DOT_UPD
 cudaError_t launch_update(double* w, const double* V0, long long stride, int nv, int col0, long long n,
-                          GmresWork W, int with_norm, int sm_count, cudaStream_t st);
+                          GmresWork W, int with_norm, int sm_count, cudaStream_t st, int mode = DOT_UPD);
+// the pair kernels of the two-column Arnoldi step: nv <= krylov_pair_max_vectors() basis vectors per pass
+int krylov_pair_max_vectors();
+cudaError_t launch_multi_dot2(const double* w1, const double* w2, const double* V0, long long stride, int nv, int col0, long long n,
+                              GmresWork W, int sm_count, cudaStream_t st);
+cudaError_t launch_update2(double* w1, double* w2, const double* V0, long long stride, int nv, int col0, long long n,
+                           GmresWork W, int with_norm, int sm_count, cudaStream_t st);
 // the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
 cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
 // the scalar epilogue of reduction `mode` on nv sums d[0..nv) (device; after an all-reduce over the ranks)

@@ -22,6 +22,46 @@ __device__ __forceinline__ void hist_push(const GmresWork& W, GmresCtl* c, doubl
     c->nhist++;
 }
 
+// Column j of the Hessenberg matrix is complete: rows 0..j (raw, in hcol when staged, else already in W.H) and h_{j+1,j} = hn.
+// Apply the rotations 0..j-1, form rotation j, advance the residual estimate and the stop flag (Saad 2003, Sect. 6.5.3).
+// vnorm = norm of the stored (unnormalised) vector j+1; it differs from hn in the second column of a two-column step.
+__device__ __forceinline__ void finish_column(const GmresWork& W, GmresCtl* c, int j, double hn, const double* hcol, const double* ccs,
+                                              const double* ssn, double vnorm = -1.0)
+{
+    const int m = c->m;
+    double* H = W.H;
+    H[(j + 1) * m + j] = hn;
+    if (hcol) {
+        // column j, cs, sn were staged in shared memory by the whole block: the rotation chain runs on registers and
+        // shared memory instead of a dependent global load/store pair per step (it was ~1 us per previous rotation)
+        double carry = hcol[0];
+        for (int i = 0; i < j; ++i) {
+            const double nxt = hcol[i + 1];
+            H[i * m + j] = ccs[i] * carry + ssn[i] * nxt;
+            carry = -ssn[i] * carry + ccs[i] * nxt;
+        }
+        H[j * m + j] = carry;
+    } else {
+        for (int i = 0; i < j; ++i) {
+            const double a = H[i * m + j], b = H[(i + 1) * m + j];
+            H[i * m + j] = W.cs[i] * a + W.sn[i] * b;
+            H[(i + 1) * m + j] = -W.sn[i] * a + W.cs[i] * b;
+        }
+    }
+    const double a = H[j * m + j], b = H[(j + 1) * m + j];
+    const double r = hypot(a, b);
+    W.cs[j] = a / r; W.sn[j] = b / r;
+    H[j * m + j] = r; H[(j + 1) * m + j] = 0.0;
+    W.g[j + 1] = -W.sn[j] * W.g[j];
+    W.g[j] = W.cs[j] * W.g[j];
+    W.scale[j + 1] = 1.0 / (vnorm >= 0.0 ? vnorm : hn);
+    c->j = j + 1; c->its += 1;
+    c->est = fabs(W.g[j + 1]);
+    hist_push(W, c, c->est);
+    if (!isfinite(hn) || !isfinite(c->est)) c->nonfinite = 1;
+    if (c->est <= c->target || hn == 0.0 || c->its >= c->maxit || j + 1 >= m || c->nonfinite) c->inner_stop = 1;
+}
+
 // Scalar epilogues, run by one thread after a reduction has produced d[0..nv).
 __device__ __forceinline__ void epilogue(const GmresWork& W, int mode, const double* d, int nv, int col0,
                                          const double* hcol = nullptr, const double* ccs = nullptr, const double* ssn = nullptr)
@@ -71,40 +111,28 @@ __device__ __forceinline__ void epilogue(const GmresWork& W, int mode, const dou
         if (rn <= c->target || c->its >= c->maxit || d[0] == 0.0 || c->bs[BS_RESTART] != 0.0 || c->nonfinite) c->inner_stop = 1;
     } else if (mode == DOT_AUX0 || mode == DOT_AUX1) {
         c->aux[mode - DOT_AUX0] = sqrt(d[0]);
-    } else if (mode == DOT_UPD) {           // h_{j+1,j} = ||w||, Givens rotations (Saad 2003, Sect. 6.5.3)
-        const int j = c->j;
-        const double hn = sqrt(d[0]);
-        double* H = W.H;
-        H[(j + 1) * m + j] = hn;
-        if (hcol) {
-            // column j, cs, sn were staged in shared memory by the whole block: the rotation chain runs on registers and
-            // shared memory instead of a dependent global load/store pair per step (it was ~1 us per previous rotation)
-            double carry = hcol[0];
-            for (int i = 0; i < j; ++i) {
-                const double nxt = hcol[i + 1];
-                H[i * m + j] = ccs[i] * carry + ssn[i] * nxt;
-                carry = -ssn[i] * carry + ccs[i] * nxt;
-            }
-            H[j * m + j] = carry;
-        } else {
-            for (int i = 0; i < j; ++i) {
-                const double a = H[i * m + j], b = H[(i + 1) * m + j];
-                H[i * m + j] = W.cs[i] * a + W.sn[i] * b;
-                H[(i + 1) * m + j] = -W.sn[i] * a + W.cs[i] * b;
-            }
+    } else if (mode == DOT_UPD) {           // h_{j+1,j} = ||w||
+        finish_column(W, c, c->j, sqrt(d[0]), hcol, ccs, ssn);
+    } else if (mode == DOT_B2) {            // two-column step: c1_i = <W1, v_i>, c2_i = <W2, v_i> of one chunk of the basis
+        const int nb = nv / 2;              // d = [<W1, V_i>, i in the chunk | <W2, V_i>]
+        for (int k = 0; k < nb; ++k) {
+            const int i = col0 + k;
+            const double a = d[k] * W.scale[i], b = d[nb + k] * W.scale[i];
+            W.c1[i] = a; W.c2[i] = b;
+            W.coef[i] = a * W.scale[i]; W.coef2[i] = b * W.scale[i];
         }
-        const double a = H[j * m + j], b = H[(j + 1) * m + j];
-        const double r = hypot(a, b);
-        W.cs[j] = a / r; W.sn[j] = b / r;
-        H[j * m + j] = r; H[(j + 1) * m + j] = 0.0;
-        W.g[j + 1] = -W.sn[j] * W.g[j];
-        W.g[j] = W.cs[j] * W.g[j];
-        W.scale[j + 1] = 1.0 / hn;
-        c->j = j + 1; c->its += 1;
-        c->est = fabs(W.g[j + 1]);
-        hist_push(W, c, c->est);
-        if (!isfinite(hn) || !isfinite(c->est)) c->nonfinite = 1;
-        if (c->est <= c->target || hn == 0.0 || c->its >= c->maxit || j + 1 >= m || c->nonfinite) c->inner_stop = 1;
+    } else if (mode == UPD_B2A) {           // first column: h_{.,j} = (c1, r11); the coefficient of the W2'' = W2' - (b/a) W1' pass
+        const int j = c->j;
+        const double a = d[0], b = d[1], r11 = sqrt(a);
+        c->blk[0] = r11; c->blk[1] = b; c->blk[2] = a;
+        W.coef[j + 1] = (a > 0.0) ? b / a : 0.0;
+        W.Hraw[(j + 1) * c->m + j] = r11;
+        finish_column(W, c, j, r11, hcol, ccs, ssn);
+    } else if (mode == UPD_B2B) {           // second column (c->j is its index): rows 0..j of the raw column are staged in hcol
+        const int j = c->j, m = c->m;
+        const double hn = sqrt(d[0]) / c->blk[0];       // h_{j+1,j} = r22 / r11
+        W.Hraw[(j + 1) * m + j] = hn;
+        finish_column(W, c, j, hn, hcol, ccs, ssn, sqrt(d[0]));
     }
 }
 
@@ -156,12 +184,31 @@ __device__ __forceinline__ void reduce_and_finish(double (&acc)[NV], const Gmres
         if (threadIdx.x < NV) W.red_out[threadIdx.x] = dres[threadIdx.x];
         return;
     }
-    if constexpr (STAGE) if (mode == DOT_UPD) {
-        // stage column j of H (rows 0..j; row j+1 is ||w|| itself), cs and sn for the scalar epilogue
+    if constexpr (STAGE) if (mode == DOT_UPD || mode == UPD_B2A || mode == UPD_B2B) {
+        // stage column j of H (rows 0..j; row j+1 comes from the norm just reduced), cs and sn for the scalar epilogue
         __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
         const int j = W.ctl->j, m = W.ctl->m;
-        const bool staged = (j < EPI_MAX);
-        if (staged) for (int i = threadIdx.x; i <= j; i += NT) { hcol[i] = W.H[i * m + j]; if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; } }
+        const bool staged = (j < EPI_MAX);       // the two-column step is only used with m <= EPI_MAX
+        if (mode == DOT_UPD) {
+            if (staged) for (int i = threadIdx.x; i <= j; i += NT) { hcol[i] = W.H[i * m + j]; if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; } }
+        } else if (mode == UPD_B2A) {            // first column of the pair: rows 0..j are the c1 of the dot pass
+            for (int i = threadIdx.x; i <= j; i += NT) {
+                const double h = W.c1[i];
+                hcol[i] = h; W.Hraw[i * m + j] = h;
+                if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
+            }
+        } else {
+            // second column (index j; the pair started at j-1).  A v_j = (W2 - sum_{i<j} c1_i A v_i) / r11 with W2 = V c2 + r12 v_j +
+            // r22 v_{j+1} and A v_i = sum_{k<=i+1} Hraw_{k,i} v_k:  h_{k,j} = (c2ext_k - sum_{i>=k-1, i<j} Hraw_{k,i} c1_i) / r11, k <= j
+            const double r11 = W.ctl->blk[0], r12 = W.ctl->blk[1] / r11;
+            for (int k = threadIdx.x; k <= j; k += NT) {
+                double sacc = (k < j) ? W.c2[k] : r12;
+                for (int i = (k > 0 ? k - 1 : 0); i < j; ++i) sacc = fma(-W.Hraw[k * m + i], W.c1[i], sacc);
+                const double h = sacc / r11;
+                hcol[k] = h; W.Hraw[k * m + j] = h;
+                if (k < j) { ccs[k] = W.cs[k]; ssn[k] = W.sn[k]; }
+            }
+        }
         __syncthreads();
         if (threadIdx.x == 0) epilogue(W, mode, dres, NV, col0, staged ? hcol : nullptr, ccs, ssn);
         return;

@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) multi_dot_kernel(c
 
 template <int NV, bool WITH_NORM>
 __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) update_kernel(double* __restrict__ w, const double* __restrict__ V0,
-                                                                            long long stride, long long n, GmresWork W, int col0)
+                                                                            long long stride, long long n, GmresWork W, int col0, int mode)
 {
     if (W.ctl->inner_stop) return;
     constexpr int U = gs_unroll(NV);
@@ -121,7 +121,119 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) update_kernel(doub
         w[n - 1] = a;
         if (WITH_NORM) acc[0] += a * a;
     }
-    if (WITH_NORM) reduce_and_finish<1, KTHREADS, true>(acc, W, DOT_UPD, 0);
+    if (WITH_NORM) reduce_and_finish<1, KTHREADS, true>(acc, W, mode, 0);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The pair kernels of the two-column Arnoldi step (ark_m1_api.cu gmres_solve):
+// W1 = A v_j and W2 = A W1 are orthogonalised against the basis TOGETHER, so the basis is read once per pass for two columns.
+// Same in-flight shape as the single-vector kernels: (NV + 2) U >= 16 batched 16-byte loads per trip.
+// ---------------------------------------------------------------------------------------------------------
+static constexpr int MAXV2 = MAXV / 2;      // basis vectors per pass of the pair kernels (2 MAXV2 sums per block)
+__host__ __device__ constexpr int gs_unroll2(int nv) { return (nv + 2) >= 16 ? 1 : (15 + nv + 2) / (nv + 2); }
+
+template <int NV>
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) multi_dot2_kernel(const double* __restrict__ w1, const double* __restrict__ w2,
+                                                                                const double* __restrict__ V0, long long stride, long long n,
+                                                                                GmresWork W, int col0)
+{
+    if (W.ctl->inner_stop) return;
+    constexpr int U = gs_unroll2(NV);
+    double acc[2 * NV];
+#pragma unroll
+    for (int k = 0; k < 2 * NV; ++k) acc[k] = 0.0;
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
+    const double2* p1 = reinterpret_cast<const double2*>(w1);
+    const double2* p2 = reinterpret_cast<const double2*>(w2);
+    long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x;
+    for (; e + (U - 1) * T < n2; e += U * T) {
+        double2 a1[U], a2[U], b[U][NV];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { a1[u] = ld_stream(p1 + e + u * T); a2[u] = ld_stream(p2 + e + u * T); }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) b[u][k] = ld_stream(reinterpret_cast<const double2*>(V0 + k * stride) + e + u * T);
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) {
+                acc[k] = fma(a1[u].y, b[u][k].y, fma(a1[u].x, b[u][k].x, acc[k]));
+                acc[NV + k] = fma(a2[u].y, b[u][k].y, fma(a2[u].x, b[u][k].x, acc[NV + k]));
+            }
+    }
+    for (; e < n2; e += T) {
+        const double2 a1 = p1[e], a2 = p2[e];
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
+            acc[k] = fma(a1.y, b.y, fma(a1.x, b.x, acc[k]));
+            acc[NV + k] = fma(a2.y, b.y, fma(a2.x, b.x, acc[NV + k]));
+        }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) { acc[k] += w1[n - 1] * V0[k * stride + n - 1]; acc[NV + k] += w2[n - 1] * V0[k * stride + n - 1]; }
+    }
+    reduce_and_finish<2 * NV>(acc, W, DOT_B2, col0);
+}
+
+// W1 -= sum coef[col0+k] V_k, W2 -= sum coef2[col0+k] V_k; WITH_NORM (last chunk): <W1', W1'> and <W1', W2'> -> epilogue UPD_B2A
+template <int NV, bool WITH_NORM>
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) update2_kernel(double* __restrict__ w1, double* __restrict__ w2, const double* __restrict__ V0,
+                                                                             long long stride, long long n, GmresWork W, int col0)
+{
+    if (W.ctl->inner_stop) return;
+    constexpr int U = gs_unroll2(NV);
+    double cf1[NV], cf2[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) { cf1[k] = W.coef[col0 + k]; cf2[k] = W.coef2[col0 + k]; }
+    double acc[2] = { 0.0, 0.0 };
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
+    double2* p1 = reinterpret_cast<double2*>(w1);
+    double2* p2 = reinterpret_cast<double2*>(w2);
+    long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x;
+    for (; e + (U - 1) * T < n2; e += U * T) {
+        double2 a1[U], a2[U], b[U][NV];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { a1[u] = ld_stream(p1 + e + u * T); a2[u] = ld_stream(p2 + e + u * T); }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) b[u][k] = ld_stream(reinterpret_cast<const double2*>(V0 + k * stride) + e + u * T);
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int k = 0; k < NV; ++k) {
+                a1[u].x = fma(-cf1[k], b[u][k].x, a1[u].x); a1[u].y = fma(-cf1[k], b[u][k].y, a1[u].y);
+                a2[u].x = fma(-cf2[k], b[u][k].x, a2[u].x); a2[u].y = fma(-cf2[k], b[u][k].y, a2[u].y);
+            }
+            p1[e + u * T] = a1[u]; p2[e + u * T] = a2[u];
+            if (WITH_NORM) {
+                acc[0] = fma(a1[u].y, a1[u].y, fma(a1[u].x, a1[u].x, acc[0]));
+                acc[1] = fma(a1[u].y, a2[u].y, fma(a1[u].x, a2[u].x, acc[1]));
+            }
+        }
+    }
+    for (; e < n2; e += T) {
+        double2 a1 = p1[e], a2 = p2[e];
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
+            a1.x = fma(-cf1[k], b.x, a1.x); a1.y = fma(-cf1[k], b.y, a1.y);
+            a2.x = fma(-cf2[k], b.x, a2.x); a2.y = fma(-cf2[k], b.y, a2.y);
+        }
+        p1[e] = a1; p2[e] = a2;
+        if (WITH_NORM) { acc[0] = fma(a1.y, a1.y, fma(a1.x, a1.x, acc[0])); acc[1] = fma(a1.y, a2.y, fma(a1.x, a2.x, acc[1])); }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        double a1 = w1[n - 1], a2 = w2[n - 1];
+#pragma unroll
+        for (int k = 0; k < NV; ++k) { a1 -= cf1[k] * V0[k * stride + n - 1]; a2 -= cf2[k] * V0[k * stride + n - 1]; }
+        w1[n - 1] = a1; w2[n - 1] = a2;
+        if (WITH_NORM) { acc[0] += a1 * a1; acc[1] += a1 * a2; }
+    }
+    if (WITH_NORM) reduce_and_finish<2, KTHREADS, true>(acc, W, UPD_B2A, 0);
 }
 
 // grid of the Gram-Schmidt streams: one wave of GS_BLOCKS_PER_SM blocks per SM (fewer on small vectors)
@@ -162,20 +274,49 @@ cudaError_t launch_multi_dot(const double* w, const double* V0, long long stride
 
 template <int NV>
 static void upd_launch(int grd, double* w, const double* V0, long long stride, long long n, GmresWork W, int col0,
-                       int with_norm, cudaStream_t st)
+                       int with_norm, int mode, cudaStream_t st)
 {
-    if (with_norm) update_kernel<NV, true><<<grd, KTHREADS, 0, st>>>(w, V0, stride, n, W, col0);
-    else update_kernel<NV, false><<<grd, KTHREADS, 0, st>>>(w, V0, stride, n, W, col0);
+    if (with_norm) update_kernel<NV, true><<<grd, KTHREADS, 0, st>>>(w, V0, stride, n, W, col0, mode);
+    else update_kernel<NV, false><<<grd, KTHREADS, 0, st>>>(w, V0, stride, n, W, col0, mode);
 }
 
 cudaError_t launch_update(double* w, const double* V0, long long stride, int nv, int col0, long long n,
-                          GmresWork W, int with_norm, int sm_count, cudaStream_t st)
+                          GmresWork W, int with_norm, int sm_count, cudaStream_t st, int mode)
 {
     const int grd = gs_grid(n, sm_count);
     switch (nv) {
-#define ARK_CASE(K) case K: upd_launch<K>(grd, w, V0, stride, n, W, col0, with_norm, st); break;
+#define ARK_CASE(K) case K: upd_launch<K>(grd, w, V0, stride, n, W, col0, with_norm, mode, st); break;
         ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
         ARK_CASE(9) ARK_CASE(10) ARK_CASE(11) ARK_CASE(12) ARK_CASE(13) ARK_CASE(14) ARK_CASE(15) ARK_CASE(16)
+#undef ARK_CASE
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+int krylov_pair_max_vectors() { return MAXV2; }
+
+cudaError_t launch_multi_dot2(const double* w1, const double* w2, const double* V0, long long stride, int nv, int col0, long long n,
+                              GmresWork W, int sm_count, cudaStream_t st)
+{
+    const int grd = gs_grid(n, sm_count);
+    switch (nv) {
+#define ARK_CASE(K) case K: multi_dot2_kernel<K><<<grd, KTHREADS, 0, st>>>(w1, w2, V0, stride, n, W, col0); break;
+        ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
+#undef ARK_CASE
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_update2(double* w1, double* w2, const double* V0, long long stride, int nv, int col0, long long n,
+                           GmresWork W, int with_norm, int sm_count, cudaStream_t st)
+{
+    const int grd = gs_grid(n, sm_count);
+    switch (nv) {
+#define ARK_CASE(K) case K: if (with_norm) update2_kernel<K, true><<<grd, KTHREADS, 0, st>>>(w1, w2, V0, stride, n, W, col0); \
+                            else update2_kernel<K, false><<<grd, KTHREADS, 0, st>>>(w1, w2, V0, stride, n, W, col0); break;
+        ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
 #undef ARK_CASE
         default: return cudaErrorInvalidValue;
     }

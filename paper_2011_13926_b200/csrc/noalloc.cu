@@ -4,7 +4,7 @@
 // The handle path (ark_m1_count_unrealizable, explicit_kernels.cu) keeps its two counters in memory the handle cudaMalloc'ed at
 // create.  This variant takes the caller's planes and the caller's output and keeps its scratch — one partial pair per block and the
 // "last block done" ticket — in a file-scope __device__ array of fixed size.  Every GPU that loads libark_m1.so holds that array
-// (NOALLOC_SCRATCH_BYTES = 256 KB + 256 B) until the process exits.  Nothing here calls cudaMalloc, cudaFree or a library routine
+// (256 KB + 256 B) until the process exits.  Nothing here calls cudaMalloc, cudaFree or a library routine
 // that allocates.
 //
 // Consequences of the one shared array (ark_m1.h says the same):
@@ -30,7 +30,6 @@ static constexpr int NOALLOC_MAX_BLOCKS = 16384;
 static constexpr long long NOALLOC_MAX_CELLS = (long long)NOALLOC_MAX_BLOCKS * NOALLOC_CHUNK;
 static constexpr int NOALLOC_HEADER_WORDS = 32;                                        // 256 B: word 0 is the ticket
 static constexpr int NOALLOC_WORDS = NOALLOC_HEADER_WORDS + 2 * NOALLOC_MAX_BLOCKS;
-static constexpr size_t NOALLOC_SCRATCH_BYTES = sizeof(unsigned long long) * NOALLOC_WORDS;
 
 // [0] ticket, [1..31] unused, then partial[block][2]
 static __device__ __align__(256) unsigned long long noalloc_scratch[NOALLOC_WORDS];
