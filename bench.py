@@ -241,19 +241,31 @@ def aggregate_over_ranks(elapsed_s, units, dist=None):
     return float(t.item()), float(u.item())
 
 
-def iteration_bytes_per_cell(iters, m=RESTART, operator=0):
+def iteration_bytes_per_cell(iters, m=RESTART, operator=0, pair=None):
     """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
-    operator 336 (block stencil) or 136 (matrix-free with the diagonal block and J rebuilt in the kernel, the default; 264 when it loads M^-1 and J); one-pass classical Gram-Schmidt at inner index j: dots 24 (j+2),
-    update+norm 24 (j+3); one extra read of w per 16-vector pass (option vectors_per_pass, default 16 by measurement); per cycle: combine 8 (3 jj + 15) + true residual
-    (block stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24."""
+    operator 336 (block stencil) or 136 (matrix-free with the diagonal block and J rebuilt in the kernel, the default; 264 when it
+    loads M^-1 and J).  Matrix-free default = two Arnoldi columns per pass over the basis (`pair`): per pair at inner index j two
+    operator applications, dots of both vectors against the j+1 basis vectors 24 (j+1) + 48 per chunk of 8 vectors, one update pass
+    24 (j+1) + 96, the W2 - gamma W1 pass 72; a trailing single column and the block-stencil path use the one-column step: dots
+    24 (j+2), update+norm 24 (j+3), one extra read of w per 16-vector pass.  Per cycle: combine 8 (3 jj + 15) + true residual (block
+    stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24."""
+    if pair is None:
+        pair = (operator == 1)
     op = 336.0 if operator == 0 else 136.0
     res = 480.0 if operator == 0 else 216.0
     total, done = 0.0, 0
     while done < iters:
         jj = min(m, iters - done)
-        for j in range(jj):
-            passes = j // 16 + 1
-            total += op + 24.0 * (j + 1 + passes) + 24.0 * (j + 1 + 2 * passes)
+        j = 0
+        while j < jj:
+            if pair and j + 1 < m:          # the pair is enqueued whole even when the cycle stops after its first column
+                chunks = j // 8 + 1
+                total += 2.0 * op + 24.0 * (j + 1) + 48.0 * chunks + 24.0 * (j + 1) + 96.0 + (72.0 if j + 1 < jj else 0.0)
+                j += 2
+            else:
+                passes = j // 16 + 1
+                total += op + 24.0 * (j + 1 + passes) + 24.0 * (j + 1 + 2 * passes)
+                j += 1
         total += 8.0 * (3 * jj + 15) + res + 24.0
         done += jj
     return total
@@ -821,7 +833,7 @@ def run_decomposed(args):
     t_exp_max, _ = aggregate_over_ranks(t_exp, 0.0, dist if world > 1 else None)
     if rank == 0:
         halo_per_step = (st1["halo_bytes"] - st0["halo_bytes"]) / args.steps
-        interior = iteration_bytes_per_cell(its, operator=1) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
+        interior = iteration_bytes_per_cell(its, operator=1, pair=False) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
         line = {
             "metric": METRIC, "value": 2.0 * N * args.steps / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",

@@ -581,11 +581,7 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
                     const int nv = (j + 1 - c0) < csize2 ? (j + 1 - c0) : csize2;
                     KL(KC_DOT, 24.0 * (nv + 2) * h->N, launch_multi_dot2(w, w2, h->V + (size_t)c0 * S, S, nv, c0, n, W, sm, h->st));
                 }
-                for (int c0 = 0; c0 <= j; c0 += csize2) {
-                    const int nv = (j + 1 - c0) < csize2 ? (j + 1 - c0) : csize2;
-                    const int last = (c0 + csize2 > j);
-                    KL(KC_UPDATE, 24.0 * (nv + 4) * h->N, launch_update2(w, w2, h->V + (size_t)c0 * S, S, nv, c0, n, W, last, sm, h->st));
-                }
+                KL(KC_UPDATE, 24.0 * (j + 1 + 4) * h->N, launch_update2_all(w, w2, h->V, S, j + 1, n, W, sm, h->st));
                 KL(KC_UPDATE, 72.0 * h->N, launch_update(w2, w, S, 1, j + 1, n, W, 1, sm, h->st, UPD_B2B));
                 ++j;
                 continue;

@@ -236,6 +236,91 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) update2_kernel(dou
     if (WITH_NORM) reduce_and_finish<2, KTHREADS, true>(acc, W, UPD_B2A, 0);
 }
 
+// The same update over ALL nv <= MAXALL basis vectors in one pass: W1 and W2 are read and written once per pair of columns instead of
+// once per chunk of MAXV2 vectors (with chunks of 8 the two vectors moved 96 B per cell per chunk, up to four times per pair).  The
+// 2 nv coefficients sit in shared memory as (coef, coef2) pairs (one broadcast LDS.128 per vector); the basis goes through the
+// registers in batches of UB vectors x U elements, every batch's loads issued before its arithmetic.
+static constexpr int MAXALL = 128;
+static constexpr int UB = 8;
+template <int NB, int U>
+__device__ __forceinline__ void update2_batch(double2 (&a1)[U], double2 (&a2)[U], const double* __restrict__ Vb, long long stride, long long e, long long T,
+                                              const double2* __restrict__ cf)
+{
+    double2 b[U][NB];
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int k = 0; k < NB; ++k) b[u][k] = ld_stream(reinterpret_cast<const double2*>(Vb + k * stride) + e + u * T);
+#pragma unroll
+    for (int k = 0; k < NB; ++k) {
+        const double2 c = cf[k];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            a1[u].x = fma(-c.x, b[u][k].x, a1[u].x); a1[u].y = fma(-c.x, b[u][k].y, a1[u].y);
+            a2[u].x = fma(-c.y, b[u][k].x, a2[u].x); a2[u].y = fma(-c.y, b[u][k].y, a2[u].y);
+        }
+    }
+}
+
+template <int U>
+__device__ __forceinline__ void update2_sweep(double2 (&a1)[U], double2 (&a2)[U], const double* __restrict__ V0, long long stride, long long e, long long T,
+                                              const double2* __restrict__ cf, int nv)
+{
+    int k0 = 0;
+    for (; k0 + UB <= nv; k0 += UB) update2_batch<UB, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0);
+    switch (nv - k0) {
+        case 1: update2_batch<1, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0); break;
+        case 2: update2_batch<2, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0); break;
+        case 3: update2_batch<3, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0); break;
+        case 4: update2_batch<4, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0); break;
+        case 5: update2_batch<5, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0); break;
+        case 6: update2_batch<6, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0); break;
+        case 7: update2_batch<7, U>(a1, a2, V0 + k0 * stride, stride, e, T, cf + k0); break;
+        default: break;
+    }
+}
+
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) update2_all_kernel(double* __restrict__ w1, double* __restrict__ w2, const double* __restrict__ V0,
+                                                                                 long long stride, long long n, GmresWork W, int nv)
+{
+    if (W.ctl->inner_stop) return;
+    constexpr int U = 2;
+    __shared__ double2 cf[MAXALL];
+    for (int k = threadIdx.x; k < nv; k += KTHREADS) cf[k] = make_double2(W.coef[k], W.coef2[k]);
+    __syncthreads();
+    double acc[2] = { 0.0, 0.0 };
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
+    double2* p1 = reinterpret_cast<double2*>(w1);
+    double2* p2 = reinterpret_cast<double2*>(w2);
+    long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x;
+    for (; e + (U - 1) * T < n2; e += U * T) {
+        double2 a1[U], a2[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { a1[u] = ld_stream(p1 + e + u * T); a2[u] = ld_stream(p2 + e + u * T); }
+        update2_sweep<U>(a1, a2, V0, stride, e, T, cf, nv);
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            p1[e + u * T] = a1[u]; p2[e + u * T] = a2[u];
+            acc[0] = fma(a1[u].y, a1[u].y, fma(a1[u].x, a1[u].x, acc[0]));
+            acc[1] = fma(a1[u].y, a2[u].y, fma(a1[u].x, a2[u].x, acc[1]));
+        }
+    }
+    for (; e < n2; e += T) {
+        double2 a1[1] = { p1[e] }, a2[1] = { p2[e] };
+        update2_sweep<1>(a1, a2, V0, stride, e, T, cf, nv);
+        p1[e] = a1[0]; p2[e] = a2[0];
+        acc[0] = fma(a1[0].y, a1[0].y, fma(a1[0].x, a1[0].x, acc[0]));
+        acc[1] = fma(a1[0].y, a2[0].y, fma(a1[0].x, a2[0].x, acc[1]));
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        double a1 = w1[n - 1], a2 = w2[n - 1];
+        for (int k = 0; k < nv; ++k) { a1 -= cf[k].x * V0[k * stride + n - 1]; a2 -= cf[k].y * V0[k * stride + n - 1]; }
+        w1[n - 1] = a1; w2[n - 1] = a2;
+        acc[0] += a1 * a1; acc[1] += a1 * a2;
+    }
+    reduce_and_finish<2, KTHREADS, true>(acc, W, UPD_B2A, 0);
+}
+
 // grid of the Gram-Schmidt streams: one wave of GS_BLOCKS_PER_SM blocks per SM (fewer on small vectors)
 static int gs_grid(long long n, int sm_count)
 {
@@ -320,6 +405,14 @@ cudaError_t launch_update2(double* w1, double* w2, const double* V0, long long s
 #undef ARK_CASE
         default: return cudaErrorInvalidValue;
     }
+    return cudaGetLastError();
+}
+
+// W1, W2 -= their projections on all nv basis vectors V0 .. V0 + (nv-1) stride, one pass; <W1', W1'>, <W1', W2'> -> epilogue UPD_B2A
+cudaError_t launch_update2_all(double* w1, double* w2, const double* V0, long long stride, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st)
+{
+    if (nv < 1 || nv > MAXALL) return cudaErrorInvalidValue;
+    update2_all_kernel<<<gs_grid(n, sm_count), KTHREADS, 0, st>>>(w1, w2, V0, stride, n, W, nv);
     return cudaGetLastError();
 }
 
