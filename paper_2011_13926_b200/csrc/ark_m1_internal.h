@@ -157,8 +157,6 @@ cudaError_t launch_update(double* w, const double* V0, long long stride, int nv,
 int krylov_pair_max_vectors();
 cudaError_t launch_multi_dot2(const double* w1, const double* w2, const double* V0, long long stride, int nv, int col0, long long n,
                               GmresWork W, int sm_count, cudaStream_t st);
-cudaError_t launch_update2(double* w1, double* w2, const double* V0, long long stride, int nv, int col0, long long n,
-                           GmresWork W, int with_norm, int sm_count, cudaStream_t st);
 cudaError_t launch_update2_all(double* w1, double* w2, const double* V0, long long stride, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st);
 // the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
 cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);

@@ -178,66 +178,9 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) multi_dot2_kernel(
     reduce_and_finish<2 * NV>(acc, W, DOT_B2, col0);
 }
 
-// W1 -= sum coef[col0+k] V_k, W2 -= sum coef2[col0+k] V_k; WITH_NORM (last chunk): <W1', W1'> and <W1', W2'> -> epilogue UPD_B2A
-template <int NV, bool WITH_NORM>
-__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM) update2_kernel(double* __restrict__ w1, double* __restrict__ w2, const double* __restrict__ V0,
-                                                                             long long stride, long long n, GmresWork W, int col0)
-{
-    if (W.ctl->inner_stop) return;
-    constexpr int U = gs_unroll2(NV);
-    double cf1[NV], cf2[NV];
-#pragma unroll
-    for (int k = 0; k < NV; ++k) { cf1[k] = W.coef[col0 + k]; cf2[k] = W.coef2[col0 + k]; }
-    double acc[2] = { 0.0, 0.0 };
-    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
-    double2* p1 = reinterpret_cast<double2*>(w1);
-    double2* p2 = reinterpret_cast<double2*>(w2);
-    long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x;
-    for (; e + (U - 1) * T < n2; e += U * T) {
-        double2 a1[U], a2[U], b[U][NV];
-#pragma unroll
-        for (int u = 0; u < U; ++u) { a1[u] = ld_stream(p1 + e + u * T); a2[u] = ld_stream(p2 + e + u * T); }
-#pragma unroll
-        for (int u = 0; u < U; ++u)
-#pragma unroll
-            for (int k = 0; k < NV; ++k) b[u][k] = ld_stream(reinterpret_cast<const double2*>(V0 + k * stride) + e + u * T);
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-#pragma unroll
-            for (int k = 0; k < NV; ++k) {
-                a1[u].x = fma(-cf1[k], b[u][k].x, a1[u].x); a1[u].y = fma(-cf1[k], b[u][k].y, a1[u].y);
-                a2[u].x = fma(-cf2[k], b[u][k].x, a2[u].x); a2[u].y = fma(-cf2[k], b[u][k].y, a2[u].y);
-            }
-            p1[e + u * T] = a1[u]; p2[e + u * T] = a2[u];
-            if (WITH_NORM) {
-                acc[0] = fma(a1[u].y, a1[u].y, fma(a1[u].x, a1[u].x, acc[0]));
-                acc[1] = fma(a1[u].y, a2[u].y, fma(a1[u].x, a2[u].x, acc[1]));
-            }
-        }
-    }
-    for (; e < n2; e += T) {
-        double2 a1 = p1[e], a2 = p2[e];
-#pragma unroll
-        for (int k = 0; k < NV; ++k) {
-            const double2 b = reinterpret_cast<const double2*>(V0 + k * stride)[e];
-            a1.x = fma(-cf1[k], b.x, a1.x); a1.y = fma(-cf1[k], b.y, a1.y);
-            a2.x = fma(-cf2[k], b.x, a2.x); a2.y = fma(-cf2[k], b.y, a2.y);
-        }
-        p1[e] = a1; p2[e] = a2;
-        if (WITH_NORM) { acc[0] = fma(a1.y, a1.y, fma(a1.x, a1.x, acc[0])); acc[1] = fma(a1.y, a2.y, fma(a1.x, a2.x, acc[1])); }
-    }
-    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
-        double a1 = w1[n - 1], a2 = w2[n - 1];
-#pragma unroll
-        for (int k = 0; k < NV; ++k) { a1 -= cf1[k] * V0[k * stride + n - 1]; a2 -= cf2[k] * V0[k * stride + n - 1]; }
-        w1[n - 1] = a1; w2[n - 1] = a2;
-        if (WITH_NORM) { acc[0] += a1 * a1; acc[1] += a1 * a2; }
-    }
-    if (WITH_NORM) reduce_and_finish<2, KTHREADS, true>(acc, W, UPD_B2A, 0);
-}
-
-// The same update over ALL nv <= MAXALL basis vectors in one pass: W1 and W2 are read and written once per pair of columns instead of
-// once per chunk of MAXV2 vectors (with chunks of 8 the two vectors moved 96 B per cell per chunk, up to four times per pair).  The
+// W1 -= sum coef[k] V_k, W2 -= sum coef2[k] V_k over ALL nv <= MAXALL basis vectors in one pass, with <W1', W1'> and <W1', W2'> ->
+// epilogue UPD_B2A: W1 and W2 are read and written once per pair of columns (in chunks of 8 vectors the two vectors moved 96 B per
+// cell per chunk, up to four times per pair: 74 -> 59 ms of update time per solve at 4096^2).  The
 // 2 nv coefficients sit in shared memory as (coef, coef2) pairs (one broadcast LDS.128 per vector); the basis goes through the
 // registers in batches of UB vectors x U elements, every batch's loads issued before its arithmetic.
 static constexpr int MAXALL = 128;
@@ -387,20 +330,6 @@ cudaError_t launch_multi_dot2(const double* w1, const double* w2, const double* 
     const int grd = gs_grid(n, sm_count);
     switch (nv) {
 #define ARK_CASE(K) case K: multi_dot2_kernel<K><<<grd, KTHREADS, 0, st>>>(w1, w2, V0, stride, n, W, col0); break;
-        ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
-#undef ARK_CASE
-        default: return cudaErrorInvalidValue;
-    }
-    return cudaGetLastError();
-}
-
-cudaError_t launch_update2(double* w1, double* w2, const double* V0, long long stride, int nv, int col0, long long n,
-                           GmresWork W, int with_norm, int sm_count, cudaStream_t st)
-{
-    const int grd = gs_grid(n, sm_count);
-    switch (nv) {
-#define ARK_CASE(K) case K: if (with_norm) update2_kernel<K, true><<<grd, KTHREADS, 0, st>>>(w1, w2, V0, stride, n, W, col0); \
-                            else update2_kernel<K, false><<<grd, KTHREADS, 0, st>>>(w1, w2, V0, stride, n, W, col0); break;
         ARK_CASE(1) ARK_CASE(2) ARK_CASE(3) ARK_CASE(4) ARK_CASE(5) ARK_CASE(6) ARK_CASE(7) ARK_CASE(8)
 #undef ARK_CASE
         default: return cudaErrorInvalidValue;
