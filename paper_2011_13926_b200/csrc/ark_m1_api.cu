@@ -126,7 +126,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
-    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 2; h->apply_precond = 0; h->arnoldi_block = 2;
+    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 2; h->apply_precond = 0; h->arnoldi_block = 5;
     h->basis_prec = 64; h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -251,7 +251,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "kernel_timing")) { ark_kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
     else if (!strcmp(key, "apply_operator_precond")) h->apply_precond = (value != 0.0);
-    else if (!strcmp(key, "arnoldi_block")) { if (iv < 1 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "arnoldi_block must be 1 (one column per pass over the basis) or 2 (two columns)%s", ""); h->arnoldi_block = iv; }
+    else if (!strcmp(key, "arnoldi_block")) { if (iv < 1 || iv > SMAX) return ark_fail(h, ARK_M1_E_ARG, "arnoldi_block must be 1 (one column per pass over the basis), 2 (two columns) or 3..5 (s-step block)%s", ""); h->arnoldi_block = iv; }
     else if (!strcmp(key, "op_recompute")) { if (iv < 0 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "op_recompute must be 0 (load M^-1), 1 (rebuild the diagonal block in the operator) or 2 (rebuild J as well)%s", ""); h->op_recompute = iv; }
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
     else if (!strcmp(key, "mg_omega")) { if (!(value > 0.0) || !(value < 2.0)) return ark_fail(h, ARK_M1_E_ARG, "mg_omega must be in (0, 2)%s", ""); h->mg.omega = value; }
@@ -469,6 +469,7 @@ int ark_ensure_implicit(ark_m1* h, int m, int maxit)
     if (caph > (1LL << 20)) caph = (1LL << 20);     // the history keeps at most 2^20 entries (later ones are counted, not stored)
     const int caphist = (int)caph;
     const size_t nd = 2 * (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 5 * (size_t)(mm + 1) + caphist
+                      + 2 * (size_t)SMAX * (mm + 1) + 2 * SMAX * SMAX + (size_t)sstep_partial_doubles(h->sm_count)
                       + (size_t)(krylov_max_blocks(h->sm_count) > op_mf_blocks(h->g, h->sm_count) ? krylov_max_blocks(h->sm_count) : op_mf_blocks(h->g, h->sm_count)) * MAXV;
     const size_t ctl_bytes = (sizeof(GmresCtl) + 255) / 256 * 256;
     if (cudaMalloc(&h->wblock, ctl_bytes + nd * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return ark_fail(h, ARK_M1_E_ALLOC, "cudaMalloc (solver scalars)%s", ""); }
@@ -480,6 +481,8 @@ int ark_ensure_implicit(ark_m1* h, int m, int maxit)
     W.cs = p; p += mm; W.sn = p; p += mm; W.g = p; p += mm + 1; W.y = p; p += mm;
     W.scale = p; p += mm + 1; W.coef = p; p += mm + 1; W.hist = p; p += caphist;
     W.Hraw = p; p += (size_t)(mm + 1) * mm; W.c1 = p; p += mm + 1; W.c2 = p; p += mm + 1; W.coef2 = p; p += mm + 1;
+    W.cS = p; p += (size_t)SMAX * (mm + 1); W.coefS = p; p += (size_t)SMAX * (mm + 1); W.Rb = p; p += SMAX * SMAX; W.tb = p; p += SMAX * SMAX;
+    W.partialS = p; p += sstep_partial_doubles(h->sm_count);
     W.partial = p;
     W.caphist = caphist;
     h->m_alloc = mm; h->maxit_alloc = mi;
@@ -565,10 +568,27 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
     if ((rc = true_residual(h, x))) return rc;
     if ((rc = ark_fetch_ctl(h))) return rc;
     // two columns per pass over the basis: GMRES + block-Jacobi + matrix-free operator + one-pass Gram-Schmidt, m within the staged epilogue
-    const bool pair = (h->arnoldi_block == 2 && h->precond == 0 && opk(h) == 1 && h->ortho == 1 && m >= 2 && m <= 128);
+    const bool blk_ok = (h->precond == 0 && opk(h) == 1 && h->ortho == 1 && m <= 120);
+    const bool pair = (h->arnoldi_block >= 2 && blk_ok && m >= 2);
+    const int SB = (h->arnoldi_block >= 3 && blk_ok) ? h->arnoldi_block : 0;     // columns per s-step block (krylov_sstep.cu)
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
+            if (SB && j + SB <= m) {
+                // s-step Arnoldi block (krylov_sstep.cu): W_1 = A^ v_j, W_k = (A^ - 1) W_{k-1} in the slots j+1 .. j+SB, one dot pass and one
+                // update pass over the basis for all SB vectors, in-block solve, Hessenberg columns recovered on the device
+                for (int k = 0; k < SB; ++k)
+                    KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)(j + k) * S, h->V + (size_t)(j + k + 1) * S,
+                                                                          k == 0 ? W.scale + j : nullptr, nullptr, 1.0, stop, 1, sm, h->st, k == 0 ? 0.0 : 1.0));
+                for (int c0 = 0; c0 <= j; c0 += 32) {
+                    const int nv = (j + 1 - c0) < 32 ? (j + 1 - c0) : 32;
+                    KL(KC_DOT, 24.0 * (nv + SB) * h->N, launch_dotS(w, h->V + (size_t)c0 * S, S, SB, nv, c0, n, W, sm, h->st));
+                }
+                KL(KC_UPDATE, (24.0 * (j + 1) + 48.0 * SB) * h->N, launch_updateS(w, h->V, S, SB, j + 1, n, W, sm, h->st));
+                KL(KC_UPDATE, 24.0 * (2 * SB - 1) * h->N, launch_qrS(w, S, SB, n, W, 1.0, sm, h->st));
+                j += SB - 1;
+                continue;
+            }
             if (pair && j + 1 < m) {
                 // two-column Arnoldi step: W1 = A M^-1 v_j, W2 = A M^-1 W1, both
                 // orthogonalised against v_0..v_j in the same passes over the basis, then W2 against W1'

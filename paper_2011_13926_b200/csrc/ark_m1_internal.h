@@ -44,6 +44,12 @@ struct GmresWork {                 // device pointers into one small allocation
     double* c1;     // m+1 : <W1, v_i> of the two-column step
     double* c2;     // m+1 : <W2, v_i>
     double* coef2;  // m+1 : coefficients of the second vector's update
+    // s-step Arnoldi block (krylov_sstep.cu), SB = 3..5 columns per pass over the basis; ld = m + 1
+    double* cS;     // SMAX x ld : C_{i,k} = <W_{k+1}, v_i>
+    double* coefS;  // SMAX x ld : C_{i,k} scale_i, the update coefficients
+    double* Rb;     // SMAX x SMAX: Cholesky factor of the Gram matrix of the block after the projection (upper triangular, row-major)
+    double* tb;     // SMAX x SMAX: t_{l,k} = R_{l,k} / R_{l,l}, the coefficients of the in-block triangular solve
+    double* partialS;// [gs blocks][SMAX * 32]: block partial sums of the s-step dot kernel
     double* red_out;// null: the reduction kernels run their scalar epilogue themselves (one GPU).  Non-null (slab decomposition):
                     // they store this rank's sums here instead; all-reduce and launch_epilogue follow
 };
@@ -55,6 +61,7 @@ enum DotMode { DOT_BNORM = 0, DOT_RNORM = 1, DOT_H = 2, DOT_H2 = 3, DOT_UPD = 4,
                DOT_B2 = 11,      // two-column step: <W1, V_i>, <W2, V_i> of a chunk
                UPD_B2A = 12,     // ... first column finished: <W1', W1'>, <W1', W2'>
                UPD_B2B = 13 };   // ... second column finished: ||W2''||^2
+enum { SMAX = 5 };                // columns per s-step Arnoldi block (Gram matrix of SMAX (SMAX + 1) / 2 <= MAXV sums)
 enum { BS_RHO = 0, BS_ALPHA = 1, BS_OMEGA = 2, BS_RHO_NEW = 3, BS_RN = 4, BS_RESTART = 5 };
 
 // number of SMs of the CURRENT device (cached per device; ark_m1_api.cu) — grid sizes are multiples of it
@@ -108,9 +115,10 @@ cudaError_t launch_assemble(const Grid& g, const Scheme& s, const Fields& f, dou
 cudaError_t launch_assemble_march(const Grid& g, const Scheme& s, const Fields& f, double dt, BlockMatrix A, MfPlanes mf,
                                   const double* bsrc, int sm_count, cudaStream_t st);
 // out = sgn * s * (A [M^-1] v) + add, flux form from the coefficient planes; precond = 1 applies M^-1 (Minv) first
+// theta: the result is reduced by theta * v (shifted operator for the s-step Krylov basis; 0 = plain)
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
-                         int sm_count, cudaStream_t st);
+                         int sm_count, cudaStream_t st, double theta = 0.0);
 // (z, c^2 J z) of the slab's first and last row for the neighbour ranks (out_lo / out_hi: [6][nx], either may be null)
 cudaError_t launch_halo_pack_zp(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, int precond,
                                 double* out_lo, double* out_hi, const int* skip_flag, cudaStream_t st);
@@ -158,6 +166,14 @@ int krylov_pair_max_vectors();
 cudaError_t launch_multi_dot2(const double* w1, const double* w2, const double* V0, long long stride, int nv, int col0, long long n,
                               GmresWork W, int sm_count, cudaStream_t st);
 cudaError_t launch_update2_all(double* w1, double* w2, const double* V0, long long stride, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st);
+// krylov_sstep.cu — the s-step Arnoldi block: sb = 3..SMAX vectors W_1..W_sb in consecutive slots w1, w1 + stride, ...
+int sstep_partial_doubles(int sm_count);
+// C_{i,k} = <W_{k+1}, V_i> scale_i for nv <= 32 basis vectors starting at index col0 (V0 = their first slot)
+cudaError_t launch_dotS(const double* w1, const double* V0, long long stride, int sb, int nv, int col0, long long n, GmresWork W, int sm_count, cudaStream_t st);
+// W_k -= sum_i coefS_{i,k} V_i over all nv basis vectors; Gram matrix of the result -> Cholesky, first column of the block finished
+cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int sb, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st);
+// in-block triangular solve with the Cholesky coefficients, norms of the results -> columns 2..sb of the block finished (theta = shift)
+cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int sm_count, cudaStream_t st);
 // the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
 cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
 // the scalar epilogue of reduction `mode` on nv sums d[0..nv) (device; after an all-reduce over the ranks)

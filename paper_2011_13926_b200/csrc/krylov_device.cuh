@@ -136,6 +136,47 @@ __device__ __forceinline__ void epilogue(const GmresWork& W, int mode, const dou
     }
 }
 
+// The same deterministic two-stage reduction without an epilogue: returns true in the last block to finish, with the NV sums in
+// dres (shared memory, visible to every thread of that block); false in every other block.  For kernels that run an epilogue of
+// their own (krylov_sstep.cu).  NV <= MAXV.
+template <int NV, int NT = KTHREADS>
+__device__ __forceinline__ bool reduce_to_last(double (&acc)[NV], const GmresWork& W, double* dres)
+{
+    __shared__ double sh[NT / 32][MAXV];
+    __shared__ bool is_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned int bid = blockIdx.y * gridDim.x + blockIdx.x, nb = gridDim.x * gridDim.y;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        const double s = warp_sum(acc[k]);
+        if (lane == 0) sh[warp][k] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < NV) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < NT / 32; ++w) s += sh[w][threadIdx.x];
+        W.partial[(size_t)bid * MAXV + threadIdx.x] = s;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int t = atomicInc(&W.ctl->ticket, nb - 1);   // wraps to 0 after the last block
+        is_last = (t == nb - 1);
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    __threadfence();
+    for (int k = warp; k < NV; k += NT / 32) {
+        double s = 0.0;
+        for (unsigned int b = lane; b < nb; b += 32) s += __ldcg(&W.partial[(size_t)b * MAXV + k]);
+        s = warp_sum(s);
+        if (lane == 0) dres[k] = s;
+    }
+    __syncthreads();
+    return true;
+}
+
 // Block reduction of acc[0..NV) -> partial[block][.]; the last block sums the partials in a fixed order and
 // runs the epilogue.
 // NT = threads per block; blocks may be a 2-D grid (linear block id).

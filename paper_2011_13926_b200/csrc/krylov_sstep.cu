@@ -1,0 +1,374 @@
+// krylov_sstep.cu — row a6: the s-step Arnoldi block of restarted GMRES(m) (option "arnoldi_block" = 3..5).
+//
+// Orthogonalisation against the basis is most of an iteration's traffic (PAPER.md:263-272 fixes the solver, not how its basis is
+// built), and every Arnoldi column reads the whole basis twice.  A block builds SB columns per pass:
+//   W_1 = A^ v_j,  W_k = (A^ - theta) W_{k-1}  (theta = 1: A^ = A M^-1 has its spectrum around 1; the shifted powers stay well
+//   conditioned where the plain powers of A^ do not — numpy model of this file: in-block orthogonality defect 1e-6 against 4e-2 at s = 6);
+//   C = V^T W  (ONE pass over v_0..v_j for all SB vectors: multi_dotS_kernel);
+//   W' = W - V C with the Gram matrix G = W'^T W'  (ONE pass: updateS_kernel);  G = R^T R (Cholesky, on the device);
+//   q~_k = W'_k - sum_{l<k} (R_lk / R_ll) q~_l element by element with the norms n_k = ||q~_k|| MEASURED (qrS_kernel), v_{j+k} = q~_k / n_k.
+// The Hessenberg columns are those of Arnoldi.  With B = [v_j, W_1 .. W_{SB-1}]:  A^ B = W + theta B D (D = diag(0, 1, .., 1)),
+// B = [V Q] G^ and W = [V Q] K in the orthonormal basis (K = [C; R~], R~ = the factor actually applied: R~_lk = R_lk n_l / R_ll,
+// R~_kk = n_k), and A^ v_i = sum_k Hraw_ki v_k for i < j, so the new columns U_0 .. U_{SB-1} solve the triangular system
+//   U_b = ( K_b + theta G^_b - Hraw(:, 0..j-1) C(0..j-1, b-1) - U_0 C(j, b-1) - sum_{1<=l<b} U_l R~(l-1, b-1) ) / R~(b-1, b-1),   U_0 = K_0,
+// evaluated by the last block of the reduction (one thread per row), each followed by the Givens rotations / residual estimate /
+// stop test of the one-column step (finish_column).  In exact arithmetic the iterates are GMRES(m)'s.
+// A Cholesky pivot that is not positive (the Krylov space is exhausted inside the block) truncates the block there and ends the cycle.
+#include "krylov_device.cuh"
+
+namespace ark {
+
+static constexpr int GS_BLOCKS_PER_SM_SS = 2;   // one wave of two 256-thread blocks per SM, like the other Gram-Schmidt streams
+static constexpr int SS_NVW = 4;              // basis vectors per warp of the dot kernel (8 warps -> 32 vectors per launch)
+static constexpr int SS_CH = 8 * SS_NVW;      // basis vectors per launch of the dot kernel
+__host__ __device__ constexpr int ss_ng(int s) { return s * (s + 1) / 2; }
+
+int sstep_partial_doubles(int sm_count) { return sm_count * GS_BLOCKS_PER_SM_SS * SMAX * SS_CH; }
+
+__device__ __forceinline__ double2 ld_cs2(const double2* p) { return __ldcs(p); }
+
+// ---------------------------------------------------------------------------------------------------------
+// Dots of SB vectors against up to 32 basis vectors in one pass.  The basis vectors are dealt to the 8 warps of a block (warp g of G
+// groups takes i = g, g + G, ..): a warp keeps SB x NVW accumulators, whatever j is, and every warp of a block reads the same
+// elements of W_1..W_SB (once from HBM, the rest from L1).  With fewer than 8 vectors the spare warps take other elements (replicas).
+// ---------------------------------------------------------------------------------------------------------
+template <int SB, int NVW, int U>
+__device__ __forceinline__ void dotS_body(const double* __restrict__ w1, const double* __restrict__ V0, long long stride, long long n2,
+                                          int grp, int G, int rep, int R, int lane, double (&acc)[SB][SS_NVW])
+{
+    const long long tile = 32LL * U;
+    for (long long t = (long long)rep * gridDim.x + blockIdx.x; t * tile < n2; t += (long long)R * gridDim.x) {
+        const long long e0 = t * tile + lane;
+        double2 a[U][SB], b[U][NVW];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long e = e0 + 32LL * u;
+            const bool in = e < n2;
+#pragma unroll
+            for (int k = 0; k < SB; ++k) a[u][k] = in ? reinterpret_cast<const double2*>(w1 + k * stride)[e] : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int q = 0; q < NVW; ++q) b[u][q] = in ? ld_cs2(reinterpret_cast<const double2*>(V0 + (long long)(grp + q * G) * stride) + e) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k = 0; k < SB; ++k)
+#pragma unroll
+                for (int q = 0; q < NVW; ++q) acc[k][q] = fma(a[u][k].y, b[u][q].y, fma(a[u][k].x, b[u][q].x, acc[k][q]));
+    }
+}
+
+template <int SB>
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) multi_dotS_kernel(const double* __restrict__ w1, const double* __restrict__ V0,
+                                                                                    long long stride, long long n, GmresWork W, int nv, int col0)
+{
+    if (W.ctl->inner_stop) return;
+    __shared__ double sred[KTHREADS / 32][SB * SS_NVW];
+    __shared__ bool is_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int G = nv < 8 ? nv : 8, R = 8 / G;
+    const int grp = warp % G, rep = warp / G;
+    const int nvw = (rep < R) ? (nv - grp + G - 1) / G : 0;          // vectors of this warp (0: spare warp)
+    const long long n2 = n >> 1;
+    double acc[SB][SS_NVW];
+#pragma unroll
+    for (int k = 0; k < SB; ++k)
+#pragma unroll
+        for (int q = 0; q < SS_NVW; ++q) acc[k][q] = 0.0;
+    switch (nvw) {      // loads in flight per lane: (SB + nvw) U >= 14
+        case 1: dotS_body<SB, 1, 3>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
+        case 2: dotS_body<SB, 2, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
+        case 3: dotS_body<SB, 3, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
+        case 4: dotS_body<SB, 4, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
+        default: break;
+    }
+#pragma unroll
+    for (int k = 0; k < SB; ++k)
+#pragma unroll
+        for (int q = 0; q < SS_NVW; ++q) {
+            const double s = warp_sum(acc[k][q]);
+            if (lane == 0) sred[warp][k * SS_NVW + q] = s;
+        }
+    __syncthreads();
+    // entry (k, i): vector i of the chunk belongs to group i % G, slot i / G; its replicas are the warps grp + G r
+    const unsigned int bid = blockIdx.x, nb = gridDim.x;
+    const int ent = threadIdx.x;
+    if (ent < SB * SS_CH) {
+        const int k = ent / SS_CH, i = ent % SS_CH;
+        double s = 0.0;
+        if (i < nv) { const int g = i % G, q = i / G; for (int r = 0; r < R; ++r) s += sred[g + G * r][k * SS_NVW + q]; }
+        W.partialS[(size_t)bid * (SMAX * SS_CH) + ent] = s;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int t = atomicInc(&W.ctl->ticket, nb - 1);
+        is_last = (t == nb - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    if (ent < SB * SS_CH) {
+        const int k = ent / SS_CH, i = ent % SS_CH;
+        if (i < nv) {
+            double s = 0.0;
+            for (unsigned int b = 0; b < nb; ++b) s += __ldcg(&W.partialS[(size_t)b * (SMAX * SS_CH) + ent]);
+            if (n & 1) s += w1[k * stride + n - 1] * V0[(long long)i * stride + n - 1];
+            const int ld = W.ctl->m + 1, col = col0 + i;
+            const double c = s * W.scale[col];
+            W.cS[k * ld + col] = c;
+            W.coefS[k * ld + col] = c * W.scale[col];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// W_k -= sum_i coefS_{i,k} V_i over all nv basis vectors in one pass (coefficients in shared memory, the basis through the registers in
+// batches of SS_UB vectors), Gram matrix of the result; epilogue: Cholesky, coefficients of the in-block solve, first column of the block.
+// ---------------------------------------------------------------------------------------------------------
+static constexpr int SS_UB = 8;
+static constexpr int SS_MAXNV = 128;
+
+template <int SB, int NB>
+__device__ __forceinline__ void updS_batch(double2 (&a)[SB], const double* __restrict__ Vb, long long stride, long long e, const double* __restrict__ cf)
+{
+    double2 b[NB];
+#pragma unroll
+    for (int q = 0; q < NB; ++q) b[q] = ld_cs2(reinterpret_cast<const double2*>(Vb + q * stride) + e);
+#pragma unroll
+    for (int q = 0; q < NB; ++q)
+#pragma unroll
+        for (int k = 0; k < SB; ++k) { const double c = cf[q * SB + k]; a[k].x = fma(-c, b[q].x, a[k].x); a[k].y = fma(-c, b[q].y, a[k].y); }
+}
+
+// the scalar part of the epilogue after the update pass (thread 0 of the last block); G = upper triangle of the Gram matrix, row-major
+template <int SB>
+__device__ void sstep_cholesky(const GmresWork& W, const double* __restrict__ G, const double* hcol, const double* ccs, const double* ssn)
+{
+    GmresCtl* c = W.ctl;
+    const int j = c->j, m = c->m;
+    double Gm[SB][SB], R[SB][SB];
+    {
+        int p = 0;
+        for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) { Gm[k][l] = G[p]; Gm[l][k] = G[p]; ++p; }
+    }
+    int nacc = SB;
+    for (int k = 0; k < SB; ++k) for (int l = 0; l < SB; ++l) R[k][l] = 0.0;
+    for (int k = 0; k < SB; ++k) {
+        double d = Gm[k][k];
+        for (int l = 0; l < k; ++l) d -= R[l][k] * R[l][k];
+        // the pivot is ||q~_k||^2: when it has lost all its digits against ||W'_k||^2 the block is exhausted at column k
+        if (!(d > 1e-24 * Gm[k][k]) || !isfinite(d)) { nacc = k; break; }
+        R[k][k] = sqrt(d);
+        for (int l = k + 1; l < SB; ++l) {
+            double v = Gm[k][l];
+            for (int q = 0; q < k; ++q) v -= R[q][k] * R[q][l];
+            R[k][l] = v / R[k][k];
+        }
+    }
+    for (int k = 0; k < SB; ++k)
+        for (int l = 0; l < SB; ++l) {
+            W.Rb[k * SMAX + l] = R[k][l];
+            W.tb[k * SMAX + l] = (l > k && k < nacc && l < nacc) ? R[k][l] / R[k][k] : 0.0;
+        }
+    c->blk[3] = (double)nacc;
+    if (nacc == 0) {        // W'_1 = 0: the space is exhausted at column j (h_{j+1,j} = 0 ends the cycle like the one-column step)
+        W.Hraw[(j + 1) * m + j] = 0.0;
+        finish_column(W, c, j, 0.0, hcol, ccs, ssn);
+        return;
+    }
+    c->blk[0] = R[0][0];
+    W.Hraw[(j + 1) * m + j] = R[0][0];
+    finish_column(W, c, j, R[0][0], hcol, ccs, ssn);
+    if (nacc == 1) c->inner_stop = 1;
+}
+
+template <int SB>
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) updateS_kernel(double* __restrict__ w1, const double* __restrict__ V0, long long stride,
+                                                                                 long long n, GmresWork W, int nv)
+{
+    if (W.ctl->inner_stop) return;
+    constexpr int NG = ss_ng(SB);
+    __shared__ double cf[SS_MAXNV * SB];
+    __shared__ double dres[MAXV];
+    __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
+    const int ld = W.ctl->m + 1;
+    for (int q = threadIdx.x; q < nv * SB; q += KTHREADS) cf[q] = W.coefS[(q % SB) * ld + q / SB];
+    __syncthreads();
+    double acc[NG];
+#pragma unroll
+    for (int p = 0; p < NG; ++p) acc[p] = 0.0;
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += T) {
+        double2 a[SB];
+#pragma unroll
+        for (int k = 0; k < SB; ++k) a[k] = ld_cs2(reinterpret_cast<const double2*>(w1 + k * stride) + e);
+        int q0 = 0;
+        for (; q0 + SS_UB <= nv; q0 += SS_UB) updS_batch<SB, SS_UB>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB);
+        switch (nv - q0) {
+            case 1: updS_batch<SB, 1>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
+            case 2: updS_batch<SB, 2>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
+            case 3: updS_batch<SB, 3>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
+            case 4: updS_batch<SB, 4>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
+            case 5: updS_batch<SB, 5>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
+            case 6: updS_batch<SB, 6>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
+            case 7: updS_batch<SB, 7>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
+            default: break;
+        }
+        int p = 0;
+#pragma unroll
+        for (int k = 0; k < SB; ++k) {
+            reinterpret_cast<double2*>(w1 + k * stride)[e] = a[k];
+#pragma unroll
+            for (int l = k; l < SB; ++l) { acc[p] = fma(a[k].y, a[l].y, fma(a[k].x, a[l].x, acc[p])); ++p; }
+        }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        double a[SB];
+        for (int k = 0; k < SB; ++k) { a[k] = w1[k * stride + n - 1]; for (int q = 0; q < nv; ++q) a[k] -= cf[q * SB + k] * V0[(long long)q * stride + n - 1]; w1[k * stride + n - 1] = a[k]; }
+        int p = 0;
+        for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) acc[p++] += a[k] * a[l];
+    }
+    if (!reduce_to_last<NG>(acc, W, dres)) return;
+    // last block: stage column j (the c of the first vector, also the raw Hessenberg column), then the scalar part
+    const int j = W.ctl->j, m = W.ctl->m;
+    for (int i = threadIdx.x; i <= j; i += KTHREADS) {
+        const double h = W.cS[i];
+        hcol[i] = h; W.Hraw[i * m + j] = h;
+        if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) sstep_cholesky<SB>(W, dres, hcol, ccs, ssn);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// In-block triangular solve element by element, measured norms; epilogue: the remaining columns of the block.
+// ---------------------------------------------------------------------------------------------------------
+template <int SB>
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(double* __restrict__ w1, long long stride, long long n, GmresWork W, double theta)
+{
+    if (W.ctl->inner_stop) return;
+    __shared__ double tsh[SMAX * SMAX];
+    __shared__ double dres[MAXV];
+    __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
+    __shared__ double Ush[SMAX][EPI_MAX + SMAX + 1];
+    __shared__ double Rt[SMAX][SMAX], nrm[SMAX];
+    __shared__ int stop_sh;
+    if (threadIdx.x < SMAX * SMAX) tsh[threadIdx.x] = W.tb[threadIdx.x];
+    __syncthreads();
+    double acc[SB - 1];
+#pragma unroll
+    for (int k = 0; k < SB - 1; ++k) acc[k] = 0.0;
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += T) {
+        double2 a[SB];
+#pragma unroll
+        for (int k = 0; k < SB; ++k) a[k] = ld_cs2(reinterpret_cast<const double2*>(w1 + k * stride) + e);
+#pragma unroll
+        for (int k = 1; k < SB; ++k) {
+#pragma unroll
+            for (int l = 0; l < k; ++l) { const double t = tsh[l * SMAX + k]; a[k].x = fma(-t, a[l].x, a[k].x); a[k].y = fma(-t, a[l].y, a[k].y); }
+            reinterpret_cast<double2*>(w1 + k * stride)[e] = a[k];
+            acc[k - 1] = fma(a[k].y, a[k].y, fma(a[k].x, a[k].x, acc[k - 1]));
+        }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        double a[SB];
+        for (int k = 0; k < SB; ++k) a[k] = w1[k * stride + n - 1];
+        for (int k = 1; k < SB; ++k) { for (int l = 0; l < k; ++l) a[k] -= tsh[l * SMAX + k] * a[l]; w1[k * stride + n - 1] = a[k]; acc[k - 1] += a[k] * a[k]; }
+    }
+    if (!reduce_to_last<SB - 1>(acc, W, dres)) return;
+    // ---- last block: columns j0+1 .. j0+nacc-1 of the Hessenberg matrix (c->j = j0 + 1 here: the update pass finished column j0)
+    GmresCtl* c = W.ctl;
+    const int m = c->m, ld = m + 1, j0 = c->j - 1, nacc = (int)c->blk[3];
+    const int rows = j0 + 1 + SB;
+    if (threadIdx.x == 0) {
+        // R~: the factor actually applied: off-diagonals scaled by the measured norm of their row's vector, measured diagonal
+        nrm[0] = W.Rb[0];
+        for (int k = 1; k < SB; ++k) nrm[k] = sqrt(dres[k - 1]);
+        for (int l = 0; l < SB; ++l)
+            for (int k = 0; k < SB; ++k) {
+                const double rll = W.Rb[l * SMAX + l];
+                Rt[l][k] = (k == l) ? nrm[l] : ((k > l && rll > 0.0) ? W.Rb[l * SMAX + k] * (nrm[l] / rll) : 0.0);
+            }
+        stop_sh = 0;
+    }
+    for (int i = threadIdx.x; i < c->j; i += KTHREADS) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
+    __syncthreads();
+    // U_0 = K_0 = [C(:, 0); R~(:, 0)]
+    for (int r = threadIdx.x; r < rows; r += KTHREADS) Ush[0][r] = (r <= j0) ? W.cS[r] : Rt[r - j0 - 1][0];
+    __syncthreads();
+    for (int b = 1; b < nacc; ++b) {
+        const int col = j0 + b;
+        const double piv = Rt[b - 1][b - 1];
+        for (int r = threadIdx.x; r < rows; r += KTHREADS) {
+            // K_b + theta G^_b
+            double s = (r <= j0) ? fma(theta, W.cS[(b - 1) * ld + r], W.cS[b * ld + r]) : fma(theta, Rt[r - j0 - 1][b - 1], Rt[r - j0 - 1][b]);
+            // - Hraw(:, 0..j0-1) C(0..j0-1, b-1): row r of Hraw is non-zero from column r-1 on
+            if (r <= j0) for (int i = (r > 0 ? r - 1 : 0); i < j0; ++i) s = fma(-W.Hraw[r * m + i], W.cS[(b - 1) * ld + i], s);
+            s = fma(-Ush[0][r], W.cS[(b - 1) * ld + j0], s);
+            for (int l = 1; l < b; ++l) s = fma(-Ush[l][r], Rt[l - 1][b - 1], s);
+            const double u = s / piv;
+            Ush[b][r] = u;
+            if (r <= col + 1) W.Hraw[r * m + col] = u;
+            if (r <= col) hcol[r] = u;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            finish_column(W, c, col, Ush[b][col + 1], hcol, ccs, ssn, nrm[b]);
+            ccs[col] = W.cs[col]; ssn[col] = W.sn[col];
+            stop_sh = c->inner_stop;
+        }
+        __syncthreads();
+        if (stop_sh) break;
+    }
+    if (threadIdx.x == 0 && nacc < SB) c->inner_stop = 1;      // truncated block: the cycle ends here
+}
+
+// ---------------------------------------------------------------------------------------------------------
+static int ss_grid(long long n, int sm_count)
+{
+    const long long need = ((n >> 1) + KTHREADS - 1) / KTHREADS;
+    const long long cap = (long long)sm_count * GS_BLOCKS_PER_SM_SS;
+    return (int)(need < 1 ? 1 : (need < cap ? need : cap));
+}
+
+cudaError_t launch_dotS(const double* w1, const double* V0, long long stride, int sb, int nv, int col0, long long n, GmresWork W, int sm_count, cudaStream_t st)
+{
+    if (nv < 1 || nv > SS_CH) return cudaErrorInvalidValue;
+    const int grd = ss_grid(n, sm_count);
+    switch (sb) {
+        case 3: multi_dotS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0); break;
+        case 4: multi_dotS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0); break;
+        case 5: multi_dotS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int sb, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st)
+{
+    if (nv < 1 || nv > SS_MAXNV) return cudaErrorInvalidValue;
+    const int grd = ss_grid(n, sm_count);
+    switch (sb) {
+        case 3: updateS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv); break;
+        case 4: updateS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv); break;
+        case 5: updateS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int sm_count, cudaStream_t st)
+{
+    const int grd = ss_grid(n, sm_count);
+    switch (sb) {
+        case 3: qrS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta); break;
+        case 4: qrS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta); break;
+        case 5: qrS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace ark

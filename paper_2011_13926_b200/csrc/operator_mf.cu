@@ -89,7 +89,7 @@ template <bool PRECOND, int DOT, typename TIN = double>
 __global__ void __launch_bounds__(TXO, DOT ? 16 : OP_MINB) op_mf_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
                                                     double* __restrict__ out, const double* __restrict__ scale_ptr,
                                                     const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
-                                                    int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W)
+                                                    int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W, double theta)
 {
     if (skip_flag && *skip_flag) return;
     double acc[2] = { 0.0, 0.0 };
@@ -164,6 +164,7 @@ __global__ void __launch_bounds__(TXO, DOT ? 16 : OP_MINB) op_mf_kernel(Grid g, 
             double o1 = zC.zFx + fma(rx, Ge1 - Gw1, fma(ry, Hn1 - Hs1, fma(dF, zC.zFx, Se + Sw)));
             double o2 = zC.zFy + fma(rx, Ge2 - Gw2, fma(ry, Hn2 - Hs2, fma(dF, zC.zFy, Sn + Ss)));
             o0 = fma(sc, o0, a0); o1 = fma(sc, o1, a1); o2 = fma(sc, o2, a2);
+            o0 = fma(-theta, zC.v0, o0); o1 = fma(-theta, zC.v1, o1); o2 = fma(-theta, zC.v2, o2);     // shifted operator (s-step basis)
             out[id] = o0; out[N + id] = o1; out[2 * N + id] = o2;
             if (DOT == 1) acc[0] += o0 * x0 + o1 * x1 + o2 * x2;
             if (DOT == 2) { acc[0] += o0 * zC.v0 + o1 * zC.v1 + o2 * zC.v2; acc[1] += o0 * o0 + o1 * o1 + o2 * o2; }
@@ -288,7 +289,7 @@ struct RcState { ZP zC; double Hs0, Hs1, Hs2, Ss; FC fe, fn; double dE, dF; };
 template <int DOT>
 __device__ __forceinline__ void rc_current_row(RcState& S, const ZP& zN, const FC& feN, const FC& fnN, double dEN, double dFN, bool upd,
                                                long long id, long long N, const double* __restrict__ add, const double* __restrict__ aux,
-                                               double* __restrict__ out, double rx, double ry, double sc, double (&acc)[2])
+                                               double* __restrict__ out, double rx, double ry, double sc, double theta, double (&acc)[2])
 {
     double a0 = 0.0, a1 = 0.0, a2 = 0.0;
     if (upd && add) { a0 = add[id]; a1 = add[N + id]; a2 = add[2 * N + id]; }
@@ -312,6 +313,7 @@ __device__ __forceinline__ void rc_current_row(RcState& S, const ZP& zN, const F
         double o1 = zC.zFx + fma(rx, Ge1 - Gw1, fma(ry, Hn1 - S.Hs1, fma(S.dF, zC.zFx, Se + Sw)));
         double o2 = zC.zFy + fma(rx, Ge2 - Gw2, fma(ry, Hn2 - S.Hs2, fma(S.dF, zC.zFy, Sn + S.Ss)));
         o0 = fma(sc, o0, a0); o1 = fma(sc, o1, a1); o2 = fma(sc, o2, a2);
+        o0 = fma(-theta, zC.v0, o0); o1 = fma(-theta, zC.v1, o1); o2 = fma(-theta, zC.v2, o2);     // shifted operator (s-step basis)
         out[id] = o0; out[N + id] = o1; out[2 * N + id] = o2;
         if (DOT == 1) acc[0] += o0 * x0 + o1 * x1 + o2 * x2;
         if (DOT == 2) { acc[0] += o0 * zC.v0 + o1 * zC.v1 + o2 * zC.v2; acc[1] += o0 * o0 + o1 * o1 + o2 * o2; }
@@ -325,7 +327,7 @@ template <int DOT, typename TIN = double, bool JRC = false>
 __global__ void __launch_bounds__(TXO, JRC ? OP_RCJ_MINB : OP_RC_MINB) op_mf_rc_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const TIN* __restrict__ v,
                                                     double* __restrict__ out, const double* __restrict__ scale_ptr,
                                                     const double* __restrict__ add, double sgn, const int* __restrict__ skip_flag,
-                                                    int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W)
+                                                    int RY, double rx, double ry, double c2, const double* __restrict__ aux, GmresWork W, double theta)
 {
     if (skip_flag && *skip_flag) return;
     constexpr int NJ = rc_nj(JRC), RC_NF = rc_nf(JRC);
@@ -453,7 +455,7 @@ __global__ void __launch_bounds__(TXO, JRC ? OP_RCJ_MINB : OP_RC_MINB) op_mf_rc_
                 zN.Pyy = c2 * (J.yy0 * zN.zE + J.yy1 * zN.zFx + J.yy2 * zN.zFy);
             } else zN = load_zp<true, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, jn, mf.halo[0], mf.halo[1]);
         } else zN = load_zp<true, TIN>(g, N, v, Minv, mf.J, c2, xmode, ii, jn, mf.halo[0], mf.halo[1]);
-        rc_current_row<DOT>(S, zN, feN, fnN, dEN, dFN, upd, id, N, add, aux, out, rx, ry, sc, acc);
+        rc_current_row<DOT>(S, zN, feN, fnN, dEN, dFN, upd, id, N, add, aux, out, rx, ry, sc, theta, acc);
     }
     cp_async_wait<0>();
     if (DOT == 1) reduce_and_finish<2, TXO>(acc, W, BICG_ALPHA, 0);
@@ -479,14 +481,14 @@ cudaError_t launch_op_mf_dot(const Grid& g, const MfPlanes& mf, const double* Mi
     int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, mf.rc ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
     if (mf.rc && mf.rcj) {
-        if (dot == 1) op_mf_rc_kernel<1, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
-        else op_mf_rc_kernel<2, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+        if (dot == 1) op_mf_rc_kernel<1, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W, 0.0);
+        else op_mf_rc_kernel<2, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W, 0.0);
     } else if (mf.rc) {
-        if (dot == 1) op_mf_rc_kernel<1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
-        else op_mf_rc_kernel<2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+        if (dot == 1) op_mf_rc_kernel<1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W, 0.0);
+        else op_mf_rc_kernel<2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W, 0.0);
     }
-    else if (dot == 1) op_mf_kernel<true, 1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
-    else op_mf_kernel<true, 2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W);
+    else if (dot == 1) op_mf_kernel<true, 1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W, 0.0);
+    else op_mf_kernel<true, 2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, nullptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, aux, W, 0.0);
     return cudaGetLastError();
 }
 
@@ -497,9 +499,9 @@ cudaError_t launch_op_mf_f32(const Grid& g, const MfPlanes& mf, const double* Mi
     int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, mf.rc ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
     GmresWork none; memset(&none, 0, sizeof none);
-    if (mf.rc && mf.rcj) op_mf_rc_kernel<0, float, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
-    else if (mf.rc) op_mf_rc_kernel<0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
-    else op_mf_kernel<true, 0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    if (mf.rc && mf.rcj) op_mf_rc_kernel<0, float, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none, 0.0);
+    else if (mf.rc) op_mf_rc_kernel<0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none, 0.0);
+    else op_mf_kernel<true, 0, float><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, nullptr, 1.0, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none, 0.0);
     return cudaGetLastError();
 }
 
@@ -533,15 +535,15 @@ cudaError_t launch_halo_pack_zp(const Grid& g, const MfPlanes& mf, const double*
 
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
-                         int sm_count, cudaStream_t st)
+                         int sm_count, cudaStream_t st, double theta)
 {
     int RY; const dim3 grd = op_mf_grid(g, sm_count, &RY, (precond && mf.rc) ? OP_RC_RY : OP_RY);
     const double c2 = g.c * g.c;
     GmresWork none; memset(&none, 0, sizeof none);
-    if (precond && mf.rc && mf.rcj) op_mf_rc_kernel<0, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
-    else if (precond && mf.rc) op_mf_rc_kernel<0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
-    else if (precond) op_mf_kernel<true, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
-    else op_mf_kernel<false, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none);
+    if (precond && mf.rc && mf.rcj) op_mf_rc_kernel<0, double, true><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none, theta);
+    else if (precond && mf.rc) op_mf_rc_kernel<0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none, theta);
+    else if (precond) op_mf_kernel<true, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none, theta);
+    else op_mf_kernel<false, 0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out, scale_ptr, add, sgn, skip_flag, RY, mf.rx, mf.ry, c2, nullptr, none, theta);
     return cudaGetLastError();
 }
 
