@@ -241,16 +241,21 @@ def aggregate_over_ranks(elapsed_s, units, dist=None):
     return float(t.item()), float(u.item())
 
 
-def iteration_bytes_per_cell(iters, m=RESTART, operator=0, pair=None):
+ARNOLDI_BLOCK = 5      # the library's default (option arnoldi_block): columns per pass over the basis
+
+
+def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None):
     """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
     operator 336 (block stencil) or 136 (matrix-free with the diagonal block and J rebuilt in the kernel, the default; 264 when it
-    loads M^-1 and J).  Matrix-free default = two Arnoldi columns per pass over the basis (`pair`): per pair at inner index j two
-    operator applications, dots of both vectors against the j+1 basis vectors 24 (j+1) + 48 per chunk of 8 vectors, one update pass
-    24 (j+1) + 96, the W2 - gamma W1 pass 72; a trailing single column and the block-stencil path use the one-column step: dots
-    24 (j+2), update+norm 24 (j+3), one extra read of w per 16-vector pass.  Per cycle: combine 8 (3 jj + 15) + true residual (block
-    stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24."""
-    if pair is None:
-        pair = (operator == 1)
+    loads M^-1 and J).  Matrix-free default = s-step Arnoldi blocks of `block` = 5 columns per pass over the basis: per block at inner
+    index j five operator applications, one dot pass 24 (j+1 + 5) (per 32 basis vectors), one update pass 24 (j+1) + 48*5, the
+    in-block solve 24 (2*5 - 1); columns left over go through the two-column step (two operator applications, dots 24 (j+1) + 48 per
+    chunk of 8 vectors, update 24 (j+1) + 96, the W2 - gamma W1 pass 72) or the one-column step (dots 24 (j+2), update+norm 24 (j+3), one
+    extra read of w per 16-vector pass), which the block-stencil path uses throughout.  Per cycle: combine 8 (3 jj + 15) + true residual
+    (block stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24.  A block is enqueued whole: its operator applications, dot
+    and update passes are paid even when the cycle stops after its first column."""
+    if block is None:
+        block = ARNOLDI_BLOCK if operator == 1 else 1
     op = 336.0 if operator == 0 else 136.0
     res = 480.0 if operator == 0 else 216.0
     total, done = 0.0, 0
@@ -258,7 +263,11 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0, pair=None):
         jj = min(m, iters - done)
         j = 0
         while j < jj:
-            if pair and j + 1 < m:          # the pair is enqueued whole even when the cycle stops after its first column
+            if block >= 3 and j + block <= m:
+                total += block * op + 24.0 * (j + 1) + 24.0 * block * (j // 32 + 1) + 24.0 * (j + 1) + 48.0 * block
+                total += 24.0 * (2 * block - 1) if j + 1 < jj else 0.0
+                j += block
+            elif block >= 2 and j + 1 < m:
                 chunks = j // 8 + 1
                 total += 2.0 * op + 24.0 * (j + 1) + 48.0 * chunks + 24.0 * (j + 1) + 96.0 + (72.0 if j + 1 < jj else 0.0)
                 j += 2
@@ -833,7 +842,7 @@ def run_decomposed(args):
     t_exp_max, _ = aggregate_over_ranks(t_exp, 0.0, dist if world > 1 else None)
     if rank == 0:
         halo_per_step = (st1["halo_bytes"] - st0["halo_bytes"]) / args.steps
-        interior = iteration_bytes_per_cell(its, operator=1, pair=False) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
+        interior = iteration_bytes_per_cell(its, operator=1, block=1) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
         line = {
             "metric": METRIC, "value": 2.0 * N * args.steps / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",

@@ -585,7 +585,10 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
                     KL(KC_DOT, 24.0 * (nv + SB) * h->N, launch_dotS(w, h->V + (size_t)c0 * S, S, SB, nv, c0, n, W, sm, h->st));
                 }
                 KL(KC_UPDATE, (24.0 * (j + 1) + 48.0 * SB) * h->N, launch_updateS(w, h->V, S, SB, j + 1, n, W, sm, h->st));
-                KL(KC_UPDATE, 24.0 * (2 * SB - 1) * h->N, launch_qrS(w, S, SB, n, W, 1.0, sm, h->st));
+                KL(KC_UPDATE, 24.0 * (2 * SB - 1) * h->N, launch_qrS(w, S, SB, n, W, 1.0, 1, sm, h->st));
+                // second round for a block flagged ill-conditioned (both kernels return at once otherwise)
+                KL(KC_SMALL, 0.0, launch_gramS(w, S, SB, n, W, sm, h->st));
+                KL(KC_SMALL, 0.0, launch_qrS(w, S, SB, n, W, 1.0, 2, sm, h->st));
                 j += SB - 1;
                 continue;
             }

@@ -25,7 +25,7 @@ struct GmresCtl {
     int pad;
     double aux[2];                 // scratch norms (Newton update size)
     double bs[8];                  // BiCGStab scalars: rho, alpha, omega, rho_new, ||r|| (recursive), flag "restart after this iteration"
-    double blk[4];                 // two-column Arnoldi step: r11 = ||W1'||, <W1', W2'>, <W1', W1'>
+    double blk[8];                 // two-column Arnoldi step: r11 = ||W1'||, <W1', W2'>, <W1', W1'>; s-step block: [3] accepted columns, [4] refine flag
 };
 
 struct GmresWork {                 // device pointers into one small allocation
@@ -47,8 +47,8 @@ struct GmresWork {                 // device pointers into one small allocation
     // s-step Arnoldi block (krylov_sstep.cu), SB = 3..5 columns per pass over the basis; ld = m + 1
     double* cS;     // SMAX x ld : C_{i,k} = <W_{k+1}, v_i>
     double* coefS;  // SMAX x ld : C_{i,k} scale_i, the update coefficients
-    double* Rb;     // SMAX x SMAX: Cholesky factor of the Gram matrix of the block after the projection (upper triangular, row-major)
-    double* tb;     // SMAX x SMAX: t_{l,k} = R_{l,k} / R_{l,l}, the coefficients of the in-block triangular solve
+    double* Rb;     // SMAX x SMAX: T, the unit upper-triangular factor applied so far in the block (W' = Q~ T; T = T2 T1 after a refinement round)
+    double* tb;     // SMAX x SMAX: t_{l,k} = R_{l,k} / R_{l,l} of the current round's Cholesky factor, the coefficients of the in-block solve
     double* partialS;// [gs blocks][SMAX * 32]: block partial sums of the s-step dot kernel
     double* red_out;// null: the reduction kernels run their scalar epilogue themselves (one GPU).  Non-null (slab decomposition):
                     // they store this rank's sums here instead; all-reduce and launch_epilogue follow
@@ -173,7 +173,10 @@ cudaError_t launch_dotS(const double* w1, const double* V0, long long stride, in
 // W_k -= sum_i coefS_{i,k} V_i over all nv basis vectors; Gram matrix of the result -> Cholesky, first column of the block finished
 cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int sb, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st);
 // in-block triangular solve with the Cholesky coefficients, norms of the results -> columns 2..sb of the block finished (theta = shift)
-cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int sm_count, cudaStream_t st);
+// round 1 follows the update pass; round 2 (after launch_gramS) runs only when the block was flagged ill-conditioned (refinement)
+cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int round, int sm_count, cudaStream_t st);
+// Gram matrix of the block after round 1, second Cholesky factor (returns at once unless the block was flagged for refinement)
+cudaError_t launch_gramS(const double* w1, long long stride, int sb, long long n, GmresWork W, int sm_count, cudaStream_t st);
 // the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
 cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
 // the scalar epilogue of reduction `mode` on nv sums d[0..nv) (device; after an all-reduce over the ranks)

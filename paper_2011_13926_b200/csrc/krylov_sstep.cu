@@ -13,12 +13,20 @@
 //   U_b = ( K_b + theta G^_b - Hraw(:, 0..j-1) C(0..j-1, b-1) - U_0 C(j, b-1) - sum_{1<=l<b} U_l R~(l-1, b-1) ) / R~(b-1, b-1),   U_0 = K_0,
 // evaluated by the last block of the reduction (one thread per row), each followed by the Givens rotations / residual estimate /
 // stop test of the one-column step (finish_column).  In exact arithmetic the iterates are GMRES(m)'s.
-// A Cholesky pivot that is not positive (the Krylov space is exhausted inside the block) truncates the block there and ends the cycle.
+// Conditioning.  The pivot ratios rho_k = R_kk^2 / G_kk (the part of W'_k that is new) measure the block: the coefficients of the
+// in-block solve carry a relative error of about eps / rho.  On the bench medium rho >= 0.04; on the smooth diffusive problem at
+// 1024^2, whose residual falls tenfold per iteration, the first block has rho = (1, 1.6e-4, 3.5e-6, 7.9e-9, 4.0e-12) and one round
+// left the basis orthogonal to 1e-5 only (29 iterations instead of 17).  A block with min rho < SS_RHO_REFINE therefore gets a SECOND
+// round (gramS_kernel + qrS_kernel round 2: Gram matrix of the q~, Cholesky, solve; "CholQR2"), whose kernels return at once for every
+// other block; W' = Q~ T with T = T2 T1 the product of the unit triangular factors, R~ = diag(n) T.  A pivot below SS_RHO_DROP (the
+// Krylov space is exhausted inside the block, or beyond what two rounds repair) truncates the block there and ends the cycle.
+#include <stdio.h>
 #include "krylov_device.cuh"
 
 namespace ark {
 
 static constexpr int GS_BLOCKS_PER_SM_SS = 2;   // one wave of two 256-thread blocks per SM, like the other Gram-Schmidt streams
+static constexpr double SS_RHO_REFINE = 1e-5, SS_RHO_DROP = 1e-13;     // thresholds 1e-5 .. 0.5 give the same iteration counts on every system tried
 static constexpr int SS_NVW = 4;              // basis vectors per warp of the dot kernel (8 warps -> 32 vectors per launch)
 static constexpr int SS_CH = 8 * SS_NVW;      // basis vectors per launch of the dot kernel
 __host__ __device__ constexpr int ss_ng(int s) { return s * (s + 1) / 2; }
@@ -141,24 +149,22 @@ __device__ __forceinline__ void updS_batch(double2 (&a)[SB], const double* __res
         for (int k = 0; k < SB; ++k) { const double c = cf[q * SB + k]; a[k].x = fma(-c, b[q].x, a[k].x); a[k].y = fma(-c, b[q].y, a[k].y); }
 }
 
-// the scalar part of the epilogue after the update pass (thread 0 of the last block); G = upper triangle of the Gram matrix, row-major
+// Cholesky factor of a Gram matrix given as its upper triangle (row-major): t_{l,k} = R_{l,k} / R_{l,l} for l < k < nacc (0 elsewhere),
+// rho_k = R_kk^2 / G_kk.  Returns the number of leading columns whose pivot is at least drop * G_kk.
 template <int SB>
-__device__ void sstep_cholesky(const GmresWork& W, const double* __restrict__ G, const double* hcol, const double* ccs, const double* ssn)
+__device__ int sstep_factor(const double* __restrict__ G, double drop, double (&t)[SB][SB], double (&rho)[SB], double& r00)
 {
-    GmresCtl* c = W.ctl;
-    const int j = c->j, m = c->m;
     double Gm[SB][SB], R[SB][SB];
-    {
-        int p = 0;
-        for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) { Gm[k][l] = G[p]; Gm[l][k] = G[p]; ++p; }
-    }
+    int p = 0;
+    for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) { Gm[k][l] = G[p]; Gm[l][k] = G[p]; ++p; }
+    for (int k = 0; k < SB; ++k) for (int l = 0; l < SB; ++l) { R[k][l] = 0.0; t[k][l] = 0.0; }
+    for (int k = 0; k < SB; ++k) rho[k] = 0.0;
     int nacc = SB;
-    for (int k = 0; k < SB; ++k) for (int l = 0; l < SB; ++l) R[k][l] = 0.0;
     for (int k = 0; k < SB; ++k) {
         double d = Gm[k][k];
         for (int l = 0; l < k; ++l) d -= R[l][k] * R[l][k];
-        // the pivot is ||q~_k||^2: when it has lost all its digits against ||W'_k||^2 the block is exhausted at column k
-        if (!(d > 1e-24 * Gm[k][k]) || !isfinite(d)) { nacc = k; break; }
+        if (!(d > drop * Gm[k][k]) || !isfinite(d)) { nacc = k; break; }
+        rho[k] = d / Gm[k][k];
         R[k][k] = sqrt(d);
         for (int l = k + 1; l < SB; ++l) {
             double v = Gm[k][l];
@@ -166,20 +172,36 @@ __device__ void sstep_cholesky(const GmresWork& W, const double* __restrict__ G,
             R[k][l] = v / R[k][k];
         }
     }
+    for (int k = 0; k < nacc; ++k) for (int l = k + 1; l < nacc; ++l) t[k][l] = R[k][l] / R[k][k];
+    r00 = R[0][0];
+    return nacc;
+}
+
+// the scalar part of the epilogue after the update pass (thread 0 of the last block)
+template <int SB>
+__device__ void sstep_first_round(const GmresWork& W, const double* __restrict__ G, const double* hcol, const double* ccs, const double* ssn)
+{
+    GmresCtl* c = W.ctl;
+    const int j = c->j, m = c->m;
+    double t[SB][SB], rho[SB], r00;
+    const int nacc = sstep_factor<SB>(G, SS_RHO_DROP, t, rho, r00);
+    double rmin = 1.0;
+    for (int k = 0; k < nacc; ++k) rmin = rho[k] < rmin ? rho[k] : rmin;
     for (int k = 0; k < SB; ++k)
-        for (int l = 0; l < SB; ++l) {
-            W.Rb[k * SMAX + l] = R[k][l];
-            W.tb[k * SMAX + l] = (l > k && k < nacc && l < nacc) ? R[k][l] / R[k][k] : 0.0;
-        }
+        for (int l = 0; l < SB; ++l) { W.tb[k * SMAX + l] = t[k][l]; W.Rb[k * SMAX + l] = (k == l) ? 1.0 : t[k][l]; }
     c->blk[3] = (double)nacc;
+    c->blk[4] = (nacc > 1 && rmin < SS_RHO_REFINE) ? 1.0 : 0.0;
+#ifdef SS_DEBUG
+    printf("blk j=%d nacc=%d refine=%d rho:", j, nacc, (int)c->blk[4]); for (int k = 0; k < SB; ++k) printf(" %.2e", rho[k]); printf("\n");
+#endif
     if (nacc == 0) {        // W'_1 = 0: the space is exhausted at column j (h_{j+1,j} = 0 ends the cycle like the one-column step)
         W.Hraw[(j + 1) * m + j] = 0.0;
         finish_column(W, c, j, 0.0, hcol, ccs, ssn);
         return;
     }
-    c->blk[0] = R[0][0];
-    W.Hraw[(j + 1) * m + j] = R[0][0];
-    finish_column(W, c, j, R[0][0], hcol, ccs, ssn);
+    c->blk[0] = r00;
+    W.Hraw[(j + 1) * m + j] = r00;
+    finish_column(W, c, j, r00, hcol, ccs, ssn);
     if (nacc == 1) c->inner_stop = 1;
 }
 
@@ -238,16 +260,18 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) updateS_kernel(
         if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
     }
     __syncthreads();
-    if (threadIdx.x == 0) sstep_cholesky<SB>(W, dres, hcol, ccs, ssn);
+    if (threadIdx.x == 0) sstep_first_round<SB>(W, dres, hcol, ccs, ssn);
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // In-block triangular solve element by element, measured norms; epilogue: the remaining columns of the block.
 // ---------------------------------------------------------------------------------------------------------
 template <int SB>
-__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(double* __restrict__ w1, long long stride, long long n, GmresWork W, double theta)
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(double* __restrict__ w1, long long stride, long long n, GmresWork W, double theta, int round)
 {
     if (W.ctl->inner_stop) return;
+    const bool refine = W.ctl->blk[4] != 0.0;
+    if (round == 2 && !refine) return;
     __shared__ double tsh[SMAX * SMAX];
     __shared__ double dres[MAXV];
     __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
@@ -278,19 +302,17 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(doub
         for (int k = 1; k < SB; ++k) { for (int l = 0; l < k; ++l) a[k] -= tsh[l * SMAX + k] * a[l]; w1[k * stride + n - 1] = a[k]; acc[k - 1] += a[k] * a[k]; }
     }
     if (!reduce_to_last<SB - 1>(acc, W, dres)) return;
+    if (round == 1 && refine) return;        // the block goes through a second round first: its columns are finished by that round's epilogue
     // ---- last block: columns j0+1 .. j0+nacc-1 of the Hessenberg matrix (c->j = j0 + 1 here: the update pass finished column j0)
     GmresCtl* c = W.ctl;
     const int m = c->m, ld = m + 1, j0 = c->j - 1, nacc = (int)c->blk[3];
     const int rows = j0 + 1 + SB;
     if (threadIdx.x == 0) {
-        // R~: the factor actually applied: off-diagonals scaled by the measured norm of their row's vector, measured diagonal
-        nrm[0] = W.Rb[0];
+        // R~ = diag(n) T: the factor actually applied (W' = Q~ T with the unit triangular T of the solve(s), q_k = q~_k / n_k measured)
+        nrm[0] = c->blk[0];
         for (int k = 1; k < SB; ++k) nrm[k] = sqrt(dres[k - 1]);
         for (int l = 0; l < SB; ++l)
-            for (int k = 0; k < SB; ++k) {
-                const double rll = W.Rb[l * SMAX + l];
-                Rt[l][k] = (k == l) ? nrm[l] : ((k > l && rll > 0.0) ? W.Rb[l * SMAX + k] * (nrm[l] / rll) : 0.0);
-            }
+            for (int k = 0; k < SB; ++k) Rt[l][k] = (k >= l) ? nrm[l] * W.Rb[l * SMAX + k] : 0.0;
         stop_sh = 0;
     }
     for (int i = threadIdx.x; i < c->j; i += KTHREADS) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
@@ -323,6 +345,55 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(doub
         if (stop_sh) break;
     }
     if (threadIdx.x == 0 && nacc < SB) c->inner_stop = 1;      // truncated block: the cycle ends here
+}
+
+// Second round for an ill-conditioned block: Gram matrix of the q~ of round 1, Cholesky, coefficients of round 2, T = T2 T1.
+template <int SB>
+__global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) gramS_kernel(const double* __restrict__ w1, long long stride, long long n, GmresWork W)
+{
+    if (W.ctl->inner_stop || W.ctl->blk[4] == 0.0) return;
+    constexpr int NG = ss_ng(SB);
+    __shared__ double dres[MAXV];
+    double acc[NG];
+#pragma unroll
+    for (int p = 0; p < NG; ++p) acc[p] = 0.0;
+    const long long n2 = n >> 1, T = (long long)gridDim.x * KTHREADS;
+    for (long long e = blockIdx.x * (long long)KTHREADS + threadIdx.x; e < n2; e += T) {
+        double2 a[SB];
+#pragma unroll
+        for (int k = 0; k < SB; ++k) a[k] = ld_cs2(reinterpret_cast<const double2*>(w1 + k * stride) + e);
+        int p = 0;
+#pragma unroll
+        for (int k = 0; k < SB; ++k)
+#pragma unroll
+            for (int l = k; l < SB; ++l) { acc[p] = fma(a[k].y, a[l].y, fma(a[k].x, a[l].x, acc[p])); ++p; }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        int p = 0;
+        for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) acc[p++] += w1[k * stride + n - 1] * w1[l * stride + n - 1];
+    }
+    if (!reduce_to_last<NG>(acc, W, dres)) return;
+    if (threadIdx.x == 0) {
+        GmresCtl* c = W.ctl;
+        double t2[SB][SB], rho[SB], r00;
+        int nacc = sstep_factor<SB>(dres, SS_RHO_DROP, t2, rho, r00);
+        const int nacc1 = (int)c->blk[3];
+        if (nacc > nacc1) nacc = nacc1;
+        // T <- T2 T1 (unit upper triangular), coefficients of round 2
+        double T1[SB][SB], Tn[SB][SB];
+        for (int k = 0; k < SB; ++k) for (int l = 0; l < SB; ++l) T1[k][l] = W.Rb[k * SMAX + l];
+        for (int k = 0; k < SB; ++k)
+            for (int l = 0; l < SB; ++l) {
+                double v = 0.0;
+                for (int q = k; q <= l; ++q) v += ((q == k) ? 1.0 : t2[k][q]) * T1[q][l];
+                Tn[k][l] = (l >= k) ? v : 0.0;
+            }
+        for (int k = 0; k < SB; ++k) for (int l = 0; l < SB; ++l) { W.Rb[k * SMAX + l] = Tn[k][l]; W.tb[k * SMAX + l] = t2[k][l]; }
+        c->blk[3] = (double)nacc;
+#ifdef SS_DEBUG
+        printf("   round 2: nacc=%d rho:", nacc); for (int k = 0; k < SB; ++k) printf(" %.2e", rho[k]); printf("\n");
+#endif
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -359,13 +430,25 @@ cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int s
     return cudaGetLastError();
 }
 
-cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int sm_count, cudaStream_t st)
+cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int round, int sm_count, cudaStream_t st)
 {
     const int grd = ss_grid(n, sm_count);
     switch (sb) {
-        case 3: qrS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta); break;
-        case 4: qrS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta); break;
-        case 5: qrS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta); break;
+        case 3: qrS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta, round); break;
+        case 4: qrS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta, round); break;
+        case 5: qrS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W, theta, round); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gramS(const double* w1, long long stride, int sb, long long n, GmresWork W, int sm_count, cudaStream_t st)
+{
+    const int grd = ss_grid(n, sm_count);
+    switch (sb) {
+        case 3: gramS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W); break;
+        case 4: gramS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W); break;
+        case 5: gramS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, stride, n, W); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

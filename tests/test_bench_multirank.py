@@ -44,7 +44,13 @@ def test_single_process_aggregate_is_identity():
 def test_iteration_byte_formula():
     sys.path.insert(0, ROOT)
     import bench
-    # one iteration at j = 0: operator 336 + dots 24 (1 + 1) + update 24 (1 + 2); one cycle end: combine 8 (3 + 15) + 120 + 360 + 24
+    # one iteration at j = 0, one column per pass over the basis: operator + dots 24 (1 + 1) + update 24 (1 + 2); one cycle end:
+    # combine 8 (3 + 15) + true residual + norm 24
     assert bench.iteration_bytes_per_cell(1, operator=0) == 336 + 48 + 72 + 8 * 18 + 120 + 360 + 24
-    assert bench.iteration_bytes_per_cell(1, operator=1) == 264 + 48 + 72 + 8 * 18 + 216 + 24
+    assert bench.iteration_bytes_per_cell(1, operator=1, block=1) == 136 + 48 + 72 + 8 * 18 + 216 + 24
+    # matrix-free default: blocks of five columns.  First block (j = 0) of a cycle that needs all five: five operator applications,
+    # dots 24 (1 + 5), update 24 + 240, in-block solve 24 * 9
+    assert bench.iteration_bytes_per_cell(5, operator=1) == 5 * 136 + 144 + 264 + 216 + 8 * (15 + 15) + 216 + 24
+    # two columns per pass: two operator applications, dots 24 + 48, update 24 + 96, the W2 - gamma W1 pass 72
+    assert bench.iteration_bytes_per_cell(2, operator=1, block=2) == 2 * 136 + 72 + 120 + 72 + 8 * (6 + 15) + 216 + 24
     assert bench.iteration_bytes_per_cell(60) == 2 * bench.iteration_bytes_per_cell(30)
