@@ -100,10 +100,13 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                          row ahead of the faces, cp.async row prefetch (default)
  *   "operator"          1: matrix-free coefficient planes, flux form (default: 5% faster per solve at 4096^2)
  *                       0: block stencil (BSR 3x3 on the 5-point graph, pre-multiplied by M^-1)
- *   "arnoldi_block"     2 (default): GMRES builds two Arnoldi columns per pass over the basis (W1 = A M^-1 v_j, W2 = A M^-1 W1
- *                          orthogonalised together; the Hessenberg columns are recovered on the device, the iterates are GMRES(m)'s);
- *                          applies to GMRES + block-Jacobi + matrix-free operator + one-pass orthogonalisation, restart <= 128
- *                       1: one column per pass
+ *   "arnoldi_block"     columns of the Arnoldi process built per pass over the basis (the iterates and the iteration count are
+ *                          GMRES(m)'s in every case; the stop test and the iteration limit act per column):
+ *                          5 (default), 4, 3: s-step blocks (W_1 = A M^-1 v_j, W_k = (A M^-1 - 1) W_{k-1}; one dot pass, one update
+ *                             pass, Cholesky-based in-block solve with a second round for ill-conditioned blocks, Hessenberg columns
+ *                             recovered on the device); columns a restart length leaves over use the two-column step
+ *                          2: two columns per pass     1: one
+ *                          applies to GMRES + block-Jacobi + matrix-free operator + one-pass orthogonalisation, restart <= 120
  *   "op_recompute"      what the preconditioned matrix-free operator rebuilds in registers instead of loading it (same operator up
  *                          to rounding; cells with folded neighbours (outflow sides) and clamped cells always use the stored values):
  *                          2 (default): each cell's diagonal block, from J and the four faces' coefficients (3 x 3 solve in place of
