@@ -520,7 +520,7 @@ int ark_assemble_system(ark_m1* h, double dt, const double* bsrc)
         h->mf.rcj = (h->op_recompute == 2 && h->s.is_default() && h->asm_kernel == 1 && h->N < (1LL << 31)) ? 1 : 0;
         h->mf.rc = h->op_recompute ? 1 : 0;
         if (h->asm_kernel == 1 && h->N < (1LL << 31))
-            KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble_march(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->sm_count, h->st));
+            KL(KC_ASSEMBLE, 304.0 * h->N, launch_assemble_march(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->sm_count, h->st));     // 288 + the two reduced-flux planes
         else
             KL(KC_ASSEMBLE, 288.0 * h->N, launch_assemble(h->g, h->s, f, dt, h->A, h->mf, bsrc, h->st));
     } else {

@@ -38,7 +38,8 @@ __device__ __forceinline__ double2 ld_cs2(const double2* p) { return __ldcs(p); 
 // ---------------------------------------------------------------------------------------------------------
 // Dots of SB vectors against up to 32 basis vectors in one pass.  The basis vectors are dealt to the 8 warps of a block (warp g of G
 // groups takes i = g, g + G, ..): a warp keeps SB x NVW accumulators, whatever j is, and every warp of a block reads the same
-// elements of W_1..W_SB (once from HBM, the rest from L1).  With fewer than 8 vectors the spare warps take other elements (replicas).
+// elements of W_1..W_SB (once from HBM, the rest from L1).  With fewer than 32 vectors there are fewer groups and the other warps
+// take other elements (replicas of the groups).
 // ---------------------------------------------------------------------------------------------------------
 template <int SB, int NVW, int U>
 __device__ __forceinline__ void dotS_body(const double* __restrict__ w1, const double* __restrict__ V0, long long stride, long long n2,
@@ -74,7 +75,9 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) multi_dotS_kern
     __shared__ double sred[KTHREADS / 32][SB * SS_NVW];
     __shared__ bool is_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int G = nv < 8 ? nv : 8, R = 8 / G;
+    // groups: the smallest power of two that leaves a warp at most SS_NVW vectors, so that 8 / G replicas keep every warp busy and the
+    // vectors per warp are as even as they can be (6 vectors: 2 groups x 3 vectors x 4 replicas, not 6 x 1 with two warps idle)
+    const int G = nv <= SS_NVW ? 1 : (nv <= 2 * SS_NVW ? 2 : (nv <= 4 * SS_NVW ? 4 : 8)), R = 8 / G;
     const int grp = warp % G, rep = warp / G;
     const int nvw = (rep < R) ? (nv - grp + G - 1) / G : 0;          // vectors of this warp (0: spare warp)
     const long long n2 = n >> 1;
