@@ -717,6 +717,9 @@ def run_ours(args):
                                   "frac": kern[dom]["hbm_frac"], "traffic": tr_bytes, "peak_source": peak_src,
                                   "share_of_step": kern[dom]["share"], "alg_bytes_per_launch": kern[dom]["alg_bytes_per_launch"],
                                   "traffic_note": tr.get("note"),
+                                  "pipes_note": (f"ncu of the same kernel: fp64 pipe {float(tr['fp64_pipe_busy_frac']):.2f}, issue slots {float(tr['issue_slots_busy_frac']):.2f} "
+                                                 "busy: the operator moves 136 instead of 264 B per cell by rebuilding J and the 3x3 diagonal block in registers and sits "
+                                                 "between the HBM roof and the issue roof (DESIGN.md section 5)") if tr.get("fp64_pipe_busy_frac") and dom == "spmv_hat" else None,
                                   "frac_of_nominal": kern[dom]["achieved_gbs"] / 7700.0,
                                   "nominal_note": "the measured peak is a torch copy (6544 GB/s here); these kernels are read-dominated and exceed it, "
                                                   "so the fraction of the 7.7 TB/s HGX figure (B200_PROFILING.md) is given as well"}
