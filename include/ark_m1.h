@@ -296,7 +296,9 @@ ARK_M1_API void ark_m1_3d_destroy(ark_m1_3d* h);
 ARK_M1_API int ark_m1_3d_set_stream(ark_m1_3d* h, void* cuda_stream);
 ARK_M1_API int ark_m1_3d_set_state(ark_m1_3d* h, const double* E, const double* F, const double* sigma_a, const double* sigma_s);
 /* "explicit_kernel": 1 = two streaming passes, closure once per cell then the flux-form stencil (default); 0 = one thread per cell
- * evaluating its seven closures itself (IEEE divisions and roots). */
+ * evaluating its seven closures itself (IEEE divisions and roots).
+ * "arnoldi_block": 5 (default), 4, 3 = s-step Arnoldi blocks as in the 2-D solver (columns a restart length leaves over use the
+ * two-column step); 1 = one column per pass over the basis. */
 ARK_M1_API int ark_m1_3d_set_option(ark_m1_3d* h, const char* key, double value);
 ARK_M1_API int ark_m1_3d_get_state(ark_m1_3d* h, double* E, double* F);
 ARK_M1_API int ark_m1_3d_step_explicit(ark_m1_3d* h, double dt);

@@ -347,7 +347,8 @@ __global__ void __launch_bounds__(256) zp3d_kernel(long long N, Op3 op, const do
 
 // out = sgn * s * (I + dt L_n) z + add, flux form, from the (z, c^2 J z) planes
 __global__ void __launch_bounds__(128) op3d_kernel(Grid3 g, Op3 op, double* __restrict__ out, const double* __restrict__ scale_ptr,
-                                                   const double* __restrict__ add, double sgn, double dt, const int* __restrict__ skip)
+                                                   const double* __restrict__ add, double sgn, double dt, const int* __restrict__ skip,
+                                                   const double* __restrict__ vshift, double theta)
 {
     if (skip && *skip) return;
     const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
@@ -381,7 +382,11 @@ __global__ void __launch_bounds__(128) op3d_kernel(Grid3 g, Op3 op, double* __re
         o[1 + dir] += swp * (zC[1 + dir] + zH[1 + dir]) + swm * (zL[1 + dir] + zC[1 + dir]);
     }
 #pragma unroll
-    for (int e = 0; e < 4; ++e) out[e * N + id] = fma(sc, o[e], add ? add[e * N + id] : 0.0);
+    for (int e = 0; e < 4; ++e) {
+        double r = fma(sc, o[e], add ? add[e * N + id] : 0.0);
+        if (vshift) r = fma(-theta, vshift[e * N + id], r);        // shifted operator (s-step Krylov basis, krylov_sstep.cu)
+        out[e * N + id] = r;
+    }
 }
 
 // x += M^-1 (sum_k coef_k V_k)
@@ -414,6 +419,7 @@ struct ark_m1_3d {
     double *sa, *ss_tmp, *stot;
     double* CL;               // 13 closure planes of the two-pass explicit step (lazy)
     int explicit_kernel;      // 1: two streaming passes (default), 0: one thread per cell with seven closures (IEEE forms)
+    int arnoldi_block;        // 5 (default): s-step Arnoldi blocks as in the 2-D solver; 3, 4: shorter blocks; 1: one column per pass over the basis
     bool have_state;
     Op3 op;
     double* V; long long stride; int m_alloc, maxit_alloc;
@@ -454,7 +460,8 @@ static int ensure3(ark_m1_3d* h, int m, int maxit)
     cudaFree(h->wblock); h->wblock = nullptr;
     long long caph = (long long)mi + mi / (mm > 0 ? mm : 1) + 8;
     if (caph > (1LL << 20)) caph = (1LL << 20);
-    const size_t nd = (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 2 * (size_t)(mm + 1) + (size_t)caph + (size_t)krylov_max_blocks(h->sm_count) * MAXV;
+    const size_t nd = 2 * (size_t)(mm + 1) * mm + 2 * (size_t)mm + (mm + 1) + mm + 5 * (size_t)(mm + 1) + (size_t)caph + (size_t)krylov_max_blocks(h->sm_count) * MAXV
+                      + 2 * (size_t)SMAX * (mm + 1) + 2 * SMAX * SMAX + (size_t)sstep_partial_doubles(h->sm_count);
     const size_t ctl_bytes = (sizeof(GmresCtl) + 255) / 256 * 256;
     if (cudaMalloc(&h->wblock, ctl_bytes + nd * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail3(h, ARK_M1_E_ALLOC, "cudaMalloc (solver scalars)", nullptr); }
     CU3(cudaMemset(h->wblock, 0, ctl_bytes + nd * sizeof(double)));
@@ -463,18 +470,23 @@ static int ensure3(ark_m1_3d* h, int m, int maxit)
     W.ctl = (GmresCtl*)h->wblock;
     double* p = (double*)((char*)h->wblock + ctl_bytes);
     W.H = p; p += (size_t)(mm + 1) * mm; W.cs = p; p += mm; W.sn = p; p += mm; W.g = p; p += mm + 1; W.y = p; p += mm;
-    W.scale = p; p += mm + 1; W.coef = p; p += mm + 1; W.hist = p; p += caph; W.partial = p;
+    W.scale = p; p += mm + 1; W.coef = p; p += mm + 1; W.hist = p; p += caph;
+    W.Hraw = p; p += (size_t)(mm + 1) * mm; W.c1 = p; p += mm + 1; W.c2 = p; p += mm + 1; W.coef2 = p; p += mm + 1;
+    W.cS = p; p += (size_t)SMAX * (mm + 1); W.coefS = p; p += (size_t)SMAX * (mm + 1); W.Rb = p; p += SMAX * SMAX; W.tb = p; p += SMAX * SMAX;
+    W.partialS = p; p += sstep_partial_doubles(h->sm_count);
+    W.partial = p;
     W.caphist = (int)caph;
     h->m_alloc = mm; h->maxit_alloc = mi;
     return 0;
 }
 
-static int apply3(ark_m1_3d* h, const double* v, double* out, const double* scale_ptr, const double* add, double sgn, double dt, int precond, const int* stop)
+static int apply3(ark_m1_3d* h, const double* v, double* out, const double* scale_ptr, const double* add, double sgn, double dt, int precond, const int* stop,
+                  double theta = 0.0)
 {
     const long long N = h->N;
     zp3d_kernel<<<(unsigned)((N + 255) / 256), 256, 0, h->st>>>(N, h->op, v, precond, h->g.c * h->g.c, stop);
     CU3(cudaGetLastError());
-    op3d_kernel<<<(unsigned)((N + 127) / 128), 128, 0, h->st>>>(h->g, h->op, out, scale_ptr, add, sgn, dt, stop);
+    op3d_kernel<<<(unsigned)((N + 127) / 128), 128, 0, h->st>>>(h->g, h->op, out, scale_ptr, add, sgn, dt, stop, theta != 0.0 ? v : nullptr, theta);
     CU3(cudaGetLastError());
     h->launches += 2;
     return 0;
@@ -507,7 +519,7 @@ ark_m1_3d* ark_m1_3d_create(int nx, int ny, int nz, double dx, double dy, double
     memset(h, 0, sizeof *h);
     h->g.n[0] = nx; h->g.n[1] = ny; h->g.n[2] = nz; h->g.d[0] = dx; h->g.d[1] = dy; h->g.d[2] = dz; h->g.c = c;
     for (int s = 0; s < 6; ++s) h->g.bc[s] = b[s];
-    h->N = N; h->device = dev; h->explicit_kernel = 1;
+    h->N = N; h->device = dev; h->explicit_kernel = 1; h->arnoldi_block = 5;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     bool ok = true;
     for (int k = 0; k < 2 && ok; ++k) ok = cudaMalloc((void**)&h->U[k], 4 * (size_t)N * sizeof(double)) == cudaSuccess;
@@ -555,6 +567,7 @@ int ark_m1_3d_set_option(ark_m1_3d* h, const char* key, double value)
 {
     if (!h || !key) return ARK_M1_E_ARG;
     if (!strcmp(key, "explicit_kernel")) { if (value != 0.0 && value != 1.0) return fail3(h, ARK_M1_E_ARG, "explicit_kernel must be 0 or 1", nullptr); h->explicit_kernel = (int)value; }
+    else if (!strcmp(key, "arnoldi_block")) { const int iv = (int)value; if (iv != 1 && (iv < 3 || iv > SMAX)) return fail3(h, ARK_M1_E_ARG, "arnoldi_block must be 1 or 3..5", nullptr); h->arnoldi_block = iv; }
     else return fail3(h, ARK_M1_E_ARG, "unknown option", key);
     return 0;
 }
@@ -611,9 +624,44 @@ int ark_m1_3d_step_implicit(ark_m1_3d* h, double dt, double tol, int restart, in
     CU3(cudaMemcpyAsync(h->ctl_host, W.ctl, sizeof(GmresCtl), cudaMemcpyDeviceToHost, h->st));
     CU3(cudaStreamSynchronize(h->st));
     const int MV = MAXV;
+    const int SB = (h->arnoldi_block >= 3 && m <= 120) ? h->arnoldi_block : 0;      // columns per s-step block (0: one column per pass)
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
+            if (SB && j + SB <= m) {
+                // s-step Arnoldi block, as in the 2-D solver (krylov_sstep.cu; the vector kernels only see vectors of 4N doubles)
+                for (int k = 0; k < SB; ++k)
+                    if ((rc = apply3(h, h->V + (size_t)(j + k) * S, h->V + (size_t)(j + k + 1) * S, k == 0 ? W.scale + j : nullptr, nullptr, 1.0, dt, 1, stop, k == 0 ? 0.0 : 1.0))) return rc;
+                for (int c0 = 0; c0 <= j; c0 += 32) {
+                    const int nv = (j + 1 - c0) < 32 ? (j + 1 - c0) : 32;
+                    CU3(launch_dotS(w, h->V + (size_t)c0 * S, S, SB, nv, c0, n, W, sm, h->st));
+                    h->launches++;
+                }
+                CU3(launch_updateS(w, h->V, S, SB, j + 1, n, W, sm, h->st));
+                CU3(launch_qrS(w, S, SB, n, W, 1.0, 1, sm, h->st));
+                CU3(launch_gramS(w, S, SB, n, W, sm, h->st));
+                CU3(launch_qrS(w, S, SB, n, W, 1.0, 2, sm, h->st));
+                h->launches += 4;
+                j += SB - 1;
+                continue;
+            }
+            if (SB && j + 1 < m) {      // columns a restart length leaves over: the two-column step
+                double* w2 = h->V + (size_t)(j + 2) * S;
+                if ((rc = apply3(h, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, dt, 1, stop))) return rc;
+                if ((rc = apply3(h, w, w2, nullptr, nullptr, 1.0, dt, 1, stop))) return rc;
+                const int MV2 = krylov_pair_max_vectors();
+                const int nchunk2 = (j + MV2) / MV2, csize2 = (j + nchunk2) / nchunk2;
+                for (int c0 = 0; c0 <= j; c0 += csize2) {
+                    const int nv = (j + 1 - c0) < csize2 ? (j + 1 - c0) : csize2;
+                    CU3(launch_multi_dot2(w, w2, h->V + (size_t)c0 * S, S, nv, c0, n, W, sm, h->st));
+                    h->launches++;
+                }
+                CU3(launch_update2_all(w, w2, h->V, S, j + 1, n, W, sm, h->st));
+                CU3(launch_update(w2, w, S, 1, j + 1, n, W, 1, sm, h->st, UPD_B2B));
+                h->launches += 2;
+                ++j;
+                continue;
+            }
             if ((rc = apply3(h, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, dt, 1, stop))) return rc;
             const int nchunk = (j + MV) / MV, csize = (j + nchunk) / nchunk;
             for (int c0 = 0; c0 <= j; c0 += csize) {

@@ -112,3 +112,22 @@ def test_operator_and_preconditioner_3d_against_the_oracle(bc):
     Z = np.stack([np.linalg.solve(B[k], V.reshape(4, N)[:, k]) for k in range(N)], axis=1).reshape(V.shape)
     AMo = o.apply_linear(dt, Z)
     assert np.max(np.abs(g.apply_operator(dt, V, precond=True) - AMo)) <= 1e-12 * np.max(np.abs(AMo))
+
+
+@pytest.mark.parametrize("restart", [30, 7])
+def test_3d_block_arnoldi_reproduces_the_one_column_solver(restart):
+    # arnoldi_block = 5 (default) / 3 against 1: same iteration count, same state (the s-step kernels of krylov_sstep.cu on 4N-vectors)
+    shape, d, c, bc = (40, 23, 17), (0.02, 0.03, 0.025), 1.2, (0, 0, 2, 2, 0, 0)
+    state = rough3(*shape, seed=21, c=c)
+    dt = 20 * 0.4 * min(d) / c
+    res = {}
+    for blk in (1, 3, 5):
+        g = ark.ArkM1_3D(*shape, *d, c, bc)
+        g.set_option("arnoldi_block", blk)
+        g.set_state(*state)
+        its, r = g.step_implicit(dt, 1e-10, restart, 2000)
+        assert r <= 1e-10
+        res[blk] = (its, g.get_state())
+    for blk in (3, 5):
+        assert abs(res[blk][0] - res[1][0]) <= 1
+        assert state_rel_l2(res[blk][1], res[1][1]) <= 1e-9
