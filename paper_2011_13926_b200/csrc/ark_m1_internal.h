@@ -177,6 +177,9 @@ cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int s
 cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int round, int sm_count, cudaStream_t st);
 // Gram matrix of the block after round 1, second Cholesky factor (returns at once unless the block was flagged for refinement)
 cudaError_t launch_gramS(const double* w1, long long stride, int sb, long long n, GmresWork W, int sm_count, cudaStream_t st);
+// slab decomposition: with W.red_out set the four kernels above leave this rank's sums there (dots: [sb][m + 1] raw sums); after the
+// all-reduce, the epilogue of step `which` (0 dots, 1 update pass, 2 in-block solve of `round`, 3 second-round Gram matrix) on `red`
+cudaError_t launch_sstep_epilogue(GmresWork W, int which, int sb, int nv, const double* red, double theta, int round, cudaStream_t st);
 // the whole inner orthogonalisation step for index j decided on the device (j = ctl->j): see krylov_kernels.cu
 cudaError_t launch_solve_y(GmresWork W, cudaStream_t st);
 // the scalar epilogue of reduction `mode` on nv sums d[0..nv) (device; after an all-reduce over the ranks)

@@ -176,7 +176,7 @@ static int group_allreduce(ark_m1_group* G, int n)
     std::vector<Slab>& S = *G->slabs;
     G->reduce_calls++;
     if (G->transport == TR_LOCAL) {
-        sum_slabs_kernel<<<1, 64, 0, G->st>>>(G->red_ptrs, (int)S.size(), n);
+        sum_slabs_kernel<<<(n + 63) / 64, 64, 0, G->st>>>(G->red_ptrs, (int)S.size(), n);      // one thread per sum (a single block of 64 silently left sums 64.. unreduced)
         GCU(cudaGetLastError());
         return 0;
     }
@@ -384,7 +384,7 @@ extern "C" int ark_m1_group_step_explicit(ark_m1_group* G, double dt)
 
 // w_out = sgn * scale * A [M^-1] v + add on every slab, after the halo exchange of (z, c^2 J z)
 static int group_operator(ark_m1_group* G, size_t v_off, bool v_is_x, size_t out_off, int scale_idx, bool add_b, double sgn,
-                          bool use_stop, int precond)
+                          bool use_stop, int precond, double theta = 0.0)
 {
     for (Slab& s : *G->slabs) {
         ark_m1* h = s.h;
@@ -401,7 +401,19 @@ static int group_operator(ark_m1_group* G, size_t v_off, bool v_is_x, size_t out
         const int* stop = use_stop ? &h->W.ctl->inner_stop : nullptr;
         ark_kmark(h, KC_SPMV, (precond ? (h->mf.rc ? (h->mf.rcj ? 136.0 : 192.0) : 264.0) : 216.0) * h->N);
         GCU(launch_op_mf(h->g, h->mf, h->A.Minv, v, h->V + out_off * h->stride, scale_idx >= 0 ? h->W.scale + scale_idx : nullptr,
-                         add_b ? h->A.b : nullptr, sgn, stop, precond, h->sm_count, G->st));
+                         add_b ? h->A.b : nullptr, sgn, stop, precond, h->sm_count, G->st, theta));
+    }
+    return 0;
+}
+
+// one all-reduce of n sums followed by the s-step epilogue `which` on every slab (krylov_sstep.cu)
+static int group_sstep_epilogue(ark_m1_group* G, int n, int which, int sb, int nv, int round)
+{
+    int rc = group_allreduce(G, n);
+    if (rc) return rc;
+    for (Slab& s : *G->slabs) {
+        s.h->launches++;
+        GCU(launch_sstep_epilogue(s.h->W, which, sb, nv, s.red, 1.0, round, G->st));
     }
     return 0;
 }
@@ -466,8 +478,55 @@ extern "C" int ark_m1_group_step_implicit(ark_m1_group* G, double dt, double tol
     if ((rc = group_true_residual(G))) return rc;
     if ((rc = group_fetch_ctl(G))) return rc;
     const int MV = S[0].h->maxv;
+    // s-step Arnoldi blocks (krylov_sstep.cu), as in the one-GPU solver: per block of SB columns SB halo exchanges (one per operator
+    // application) and FIVE all-reduces (dots, Gram matrix, norms, and the two of the refinement round, whose kernels return at once
+    // for a well-conditioned block) instead of 2 SB with one column per pass.  Columns a restart length leaves over use the one-column step.
+    const int SB = (S[0].h->arnoldi_block >= 3 && m <= 120 && SMAX * (m + 1) <= RED_CAP) ? S[0].h->arnoldi_block : 0;
     while (!S[0].h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
+            if (SB && j + SB <= m) {
+                for (int k = 0; k < SB; ++k)
+                    if ((rc = group_operator(G, (size_t)(j + k), false, (size_t)(j + k + 1), k == 0 ? j : -1, false, 1.0, true, 1, k == 0 ? 0.0 : 1.0))) return rc;
+                const int ld = m + 1;
+                for (Slab& s : S) {
+                    ark_m1* h = s.h;
+                    double* w = h->V + (size_t)(j + 1) * h->stride;
+                    GmresWork W = h->W; W.red_out = s.red;
+                    for (int c0 = 0; c0 <= j; c0 += 32) {
+                        const int nv = (j + 1 - c0) < 32 ? (j + 1 - c0) : 32;
+                        ark_kmark(h, KC_DOT, 24.0 * (nv + SB) * h->N);
+                        GCU(launch_dotS(w, h->V + (size_t)c0 * h->stride, h->stride, SB, nv, c0, 3 * h->N, W, h->sm_count, G->st));
+                    }
+                }
+                if ((rc = group_sstep_epilogue(G, SB * ld, 0, SB, j + 1, 0))) return rc;
+                for (Slab& s : S) {
+                    ark_m1* h = s.h;
+                    GmresWork W = h->W; W.red_out = s.red;
+                    ark_kmark(h, KC_UPDATE, (24.0 * (j + 1) + 48.0 * SB) * h->N);
+                    GCU(launch_updateS(h->V + (size_t)(j + 1) * h->stride, h->V, h->stride, SB, j + 1, 3 * h->N, W, h->sm_count, G->st));
+                }
+                if ((rc = group_sstep_epilogue(G, SB * (SB + 1) / 2, 1, SB, j + 1, 0))) return rc;
+                for (int round = 1; round <= 2; ++round) {
+                    if (round == 2) {
+                        for (Slab& s : S) {
+                            ark_m1* h = s.h;
+                            GmresWork W = h->W; W.red_out = s.red;
+                            ark_kmark(h, KC_SMALL, 0.0);
+                            GCU(launch_gramS(h->V + (size_t)(j + 1) * h->stride, h->stride, SB, 3 * h->N, W, h->sm_count, G->st));
+                        }
+                        if ((rc = group_sstep_epilogue(G, SB * (SB + 1) / 2, 3, SB, j + 1, 2))) return rc;
+                    }
+                    for (Slab& s : S) {
+                        ark_m1* h = s.h;
+                        GmresWork W = h->W; W.red_out = s.red;
+                        ark_kmark(h, round == 1 ? KC_UPDATE : KC_SMALL, round == 1 ? 24.0 * (2 * SB - 1) * h->N : 0.0);
+                        GCU(launch_qrS(h->V + (size_t)(j + 1) * h->stride, h->stride, SB, 3 * h->N, W, 1.0, round, h->sm_count, G->st));
+                    }
+                    if ((rc = group_sstep_epilogue(G, SB - 1, 2, SB, j + 1, round))) return rc;
+                }
+                j += SB - 1;
+                continue;
+            }
             if ((rc = group_operator(G, (size_t)j, false, (size_t)j + 1, j, false, 1.0, true, 1))) return rc;
             const int nchunk = (j + MV) / MV, csize = (j + nchunk) / nchunk;
             for (Slab& s : S) {

@@ -126,6 +126,7 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) multi_dotS_kern
             for (unsigned int b = 0; b < nb; ++b) s += __ldcg(&W.partialS[(size_t)b * (SMAX * SS_CH) + ent]);
             if (n & 1) s += w1[k * stride + n - 1] * V0[(long long)i * stride + n - 1];
             const int ld = W.ctl->m + 1, col = col0 + i;
+            if (W.red_out) { W.red_out[k * ld + col] = s; return; }      // slab decomposition: this rank's sums; all-reduce and epilogue follow
             const double c = s * W.scale[col];
             W.cS[k * ld + col] = c;
             W.coefS[k * ld + col] = c * W.scale[col];
@@ -208,6 +209,21 @@ __device__ void sstep_first_round(const GmresWork& W, const double* __restrict__
     if (nacc == 1) c->inner_stop = 1;
 }
 
+// last block of the update pass (or the epilogue kernel of the slab decomposition): stage column j (the c of the first vector, also the
+// raw Hessenberg column), then the scalar part
+template <int SB>
+__device__ __forceinline__ void sstep_update_epilogue(const GmresWork& W, const double* dres, double* hcol, double* ccs, double* ssn)
+{
+    const int j = W.ctl->j, m = W.ctl->m;
+    for (int i = threadIdx.x; i <= j; i += blockDim.x) {
+        const double h = W.cS[i];
+        hcol[i] = h; W.Hraw[i * m + j] = h;
+        if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) sstep_first_round<SB>(W, dres, hcol, ccs, ssn);
+}
+
 template <int SB>
 __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) updateS_kernel(double* __restrict__ w1, const double* __restrict__ V0, long long stride,
                                                                                  long long n, GmresWork W, int nv)
@@ -255,15 +271,60 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) updateS_kernel(
         for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) acc[p++] += a[k] * a[l];
     }
     if (!reduce_to_last<NG>(acc, W, dres)) return;
-    // last block: stage column j (the c of the first vector, also the raw Hessenberg column), then the scalar part
-    const int j = W.ctl->j, m = W.ctl->m;
-    for (int i = threadIdx.x; i <= j; i += KTHREADS) {
-        const double h = W.cS[i];
-        hcol[i] = h; W.Hraw[i * m + j] = h;
-        if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
+    if (W.red_out) { if (threadIdx.x < NG) W.red_out[threadIdx.x] = dres[threadIdx.x]; return; }
+    sstep_update_epilogue<SB>(W, dres, hcol, ccs, ssn);
+}
+
+// Columns j0+1 .. j0+nacc-1 of the Hessenberg matrix from the measured norms of the in-block solve (c->j = j0 + 1 here: the update pass
+// finished column j0).  Run by one block: the last block of qrS_kernel, or the epilogue kernel of the slab decomposition.
+template <int SB>
+__device__ __forceinline__ void sstep_finish_block(const GmresWork& W, const double* dres, double theta)
+{
+    __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
+    __shared__ double Ush[SMAX][EPI_MAX + SMAX + 1];
+    __shared__ double Rt[SMAX][SMAX], nrm[SMAX];
+    __shared__ int stop_sh;
+    GmresCtl* c = W.ctl;
+    const int m = c->m, ld = m + 1, j0 = c->j - 1, nacc = (int)c->blk[3];
+    const int rows = j0 + 1 + SB;
+    if (threadIdx.x == 0) {
+        // R~ = diag(n) T: the factor actually applied (W' = Q~ T with the unit triangular T of the solve(s), q_k = q~_k / n_k measured)
+        nrm[0] = c->blk[0];
+        for (int k = 1; k < SB; ++k) nrm[k] = sqrt(dres[k - 1]);
+        for (int l = 0; l < SB; ++l)
+            for (int k = 0; k < SB; ++k) Rt[l][k] = (k >= l) ? nrm[l] * W.Rb[l * SMAX + k] : 0.0;
+        stop_sh = 0;
     }
+    for (int i = threadIdx.x; i < c->j; i += (int)blockDim.x) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
     __syncthreads();
-    if (threadIdx.x == 0) sstep_first_round<SB>(W, dres, hcol, ccs, ssn);
+    // U_0 = K_0 = [C(:, 0); R~(:, 0)]
+    for (int r = threadIdx.x; r < rows; r += (int)blockDim.x) Ush[0][r] = (r <= j0) ? W.cS[r] : Rt[r - j0 - 1][0];
+    __syncthreads();
+    for (int b = 1; b < nacc; ++b) {
+        const int col = j0 + b;
+        const double piv = Rt[b - 1][b - 1];
+        for (int r = threadIdx.x; r < rows; r += (int)blockDim.x) {
+            // K_b + theta G^_b
+            double s = (r <= j0) ? fma(theta, W.cS[(b - 1) * ld + r], W.cS[b * ld + r]) : fma(theta, Rt[r - j0 - 1][b - 1], Rt[r - j0 - 1][b]);
+            // - Hraw(:, 0..j0-1) C(0..j0-1, b-1): row r of Hraw is non-zero from column r-1 on
+            if (r <= j0) for (int i = (r > 0 ? r - 1 : 0); i < j0; ++i) s = fma(-W.Hraw[r * m + i], W.cS[(b - 1) * ld + i], s);
+            s = fma(-Ush[0][r], W.cS[(b - 1) * ld + j0], s);
+            for (int l = 1; l < b; ++l) s = fma(-Ush[l][r], Rt[l - 1][b - 1], s);
+            const double u = s / piv;
+            Ush[b][r] = u;
+            if (r <= col + 1) W.Hraw[r * m + col] = u;
+            if (r <= col) hcol[r] = u;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            finish_column(W, c, col, Ush[b][col + 1], hcol, ccs, ssn, nrm[b]);
+            ccs[col] = W.cs[col]; ssn[col] = W.sn[col];
+            stop_sh = c->inner_stop;
+        }
+        __syncthreads();
+        if (stop_sh) break;
+    }
+    if (threadIdx.x == 0 && nacc < SB) c->inner_stop = 1;      // truncated block: the cycle ends here
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -277,10 +338,6 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(doub
     if (round == 2 && !refine) return;
     __shared__ double tsh[SMAX * SMAX];
     __shared__ double dres[MAXV];
-    __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
-    __shared__ double Ush[SMAX][EPI_MAX + SMAX + 1];
-    __shared__ double Rt[SMAX][SMAX], nrm[SMAX];
-    __shared__ int stop_sh;
     if (threadIdx.x < SMAX * SMAX) tsh[threadIdx.x] = W.tb[threadIdx.x];
     __syncthreads();
     double acc[SB - 1];
@@ -305,50 +362,12 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(doub
         for (int k = 1; k < SB; ++k) { for (int l = 0; l < k; ++l) a[k] -= tsh[l * SMAX + k] * a[l]; w1[k * stride + n - 1] = a[k]; acc[k - 1] += a[k] * a[k]; }
     }
     if (!reduce_to_last<SB - 1>(acc, W, dres)) return;
+    if (W.red_out) { if (threadIdx.x < SB - 1) W.red_out[threadIdx.x] = dres[threadIdx.x]; return; }
     if (round == 1 && refine) return;        // the block goes through a second round first: its columns are finished by that round's epilogue
-    // ---- last block: columns j0+1 .. j0+nacc-1 of the Hessenberg matrix (c->j = j0 + 1 here: the update pass finished column j0)
-    GmresCtl* c = W.ctl;
-    const int m = c->m, ld = m + 1, j0 = c->j - 1, nacc = (int)c->blk[3];
-    const int rows = j0 + 1 + SB;
-    if (threadIdx.x == 0) {
-        // R~ = diag(n) T: the factor actually applied (W' = Q~ T with the unit triangular T of the solve(s), q_k = q~_k / n_k measured)
-        nrm[0] = c->blk[0];
-        for (int k = 1; k < SB; ++k) nrm[k] = sqrt(dres[k - 1]);
-        for (int l = 0; l < SB; ++l)
-            for (int k = 0; k < SB; ++k) Rt[l][k] = (k >= l) ? nrm[l] * W.Rb[l * SMAX + k] : 0.0;
-        stop_sh = 0;
-    }
-    for (int i = threadIdx.x; i < c->j; i += KTHREADS) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
-    __syncthreads();
-    // U_0 = K_0 = [C(:, 0); R~(:, 0)]
-    for (int r = threadIdx.x; r < rows; r += KTHREADS) Ush[0][r] = (r <= j0) ? W.cS[r] : Rt[r - j0 - 1][0];
-    __syncthreads();
-    for (int b = 1; b < nacc; ++b) {
-        const int col = j0 + b;
-        const double piv = Rt[b - 1][b - 1];
-        for (int r = threadIdx.x; r < rows; r += KTHREADS) {
-            // K_b + theta G^_b
-            double s = (r <= j0) ? fma(theta, W.cS[(b - 1) * ld + r], W.cS[b * ld + r]) : fma(theta, Rt[r - j0 - 1][b - 1], Rt[r - j0 - 1][b]);
-            // - Hraw(:, 0..j0-1) C(0..j0-1, b-1): row r of Hraw is non-zero from column r-1 on
-            if (r <= j0) for (int i = (r > 0 ? r - 1 : 0); i < j0; ++i) s = fma(-W.Hraw[r * m + i], W.cS[(b - 1) * ld + i], s);
-            s = fma(-Ush[0][r], W.cS[(b - 1) * ld + j0], s);
-            for (int l = 1; l < b; ++l) s = fma(-Ush[l][r], Rt[l - 1][b - 1], s);
-            const double u = s / piv;
-            Ush[b][r] = u;
-            if (r <= col + 1) W.Hraw[r * m + col] = u;
-            if (r <= col) hcol[r] = u;
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            finish_column(W, c, col, Ush[b][col + 1], hcol, ccs, ssn, nrm[b]);
-            ccs[col] = W.cs[col]; ssn[col] = W.sn[col];
-            stop_sh = c->inner_stop;
-        }
-        __syncthreads();
-        if (stop_sh) break;
-    }
-    if (threadIdx.x == 0 && nacc < SB) c->inner_stop = 1;      // truncated block: the cycle ends here
+    sstep_finish_block<SB>(W, dres, theta);
 }
+
+template <int SB> __device__ __forceinline__ void sstep_second_round(const GmresWork& W, const double* dres);
 
 // Second round for an ill-conditioned block: Gram matrix of the q~ of round 1, Cholesky, coefficients of round 2, T = T2 T1.
 template <int SB>
@@ -376,6 +395,14 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) gramS_kernel(co
         for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) acc[p++] += w1[k * stride + n - 1] * w1[l * stride + n - 1];
     }
     if (!reduce_to_last<NG>(acc, W, dres)) return;
+    if (W.red_out) { if (threadIdx.x < NG) W.red_out[threadIdx.x] = dres[threadIdx.x]; return; }
+    sstep_second_round<SB>(W, dres);
+}
+
+// Cholesky of the second round's Gram matrix, T <- T2 T1 (thread 0 of one block)
+template <int SB>
+__device__ __forceinline__ void sstep_second_round(const GmresWork& W, const double* dres)
+{
     if (threadIdx.x == 0) {
         GmresCtl* c = W.ctl;
         double t2[SB][SB], rho[SB], r00;
@@ -397,6 +424,49 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) gramS_kernel(co
         printf("   round 2: nacc=%d rho:", nacc); for (int k = 0; k < SB; ++k) printf(" %.2e", rho[k]); printf("\n");
 #endif
     }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Slab decomposition (dist.cu): the kernels above leave this rank's sums in W.red_out; after the all-reduce over the ranks these
+// one-block kernels run the epilogues on the summed values `red` (every rank holds the same solver state).
+//   which 0: dots (red = [SB][m + 1] raw sums of the nv = j + 1 basis vectors)   1: update pass (Gram matrix)
+//         2: in-block solve (norms; round 1 or 2)                                 3: second-round Gram matrix
+// ---------------------------------------------------------------------------------------------------------
+template <int SB>
+__global__ void __launch_bounds__(KTHREADS) sstep_epilogue_kernel(GmresWork W, int which, int nv, const double* __restrict__ red, double theta, int round)
+{
+    GmresCtl* c = W.ctl;
+    if (c->inner_stop) return;
+    __shared__ double dres[MAXV];
+    __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
+    const int ld = c->m + 1;
+    if (which == 0) {
+        for (int ent = threadIdx.x; ent < SB * nv; ent += KTHREADS) {
+            const int k = ent / nv, i = ent % nv;
+            const double cc = red[k * ld + i] * W.scale[i];
+            W.cS[k * ld + i] = cc; W.coefS[k * ld + i] = cc * W.scale[i];
+        }
+        return;
+    }
+    const bool refine = c->blk[4] != 0.0;
+    if ((which == 3 || (which == 2 && round == 2)) && !refine) return;
+    const int nsum = (which == 2) ? SB - 1 : ss_ng(SB);
+    if (threadIdx.x < nsum) dres[threadIdx.x] = red[threadIdx.x];
+    __syncthreads();
+    if (which == 1) sstep_update_epilogue<SB>(W, dres, hcol, ccs, ssn);
+    else if (which == 3) sstep_second_round<SB>(W, dres);
+    else { if (round == 1 && refine) return; sstep_finish_block<SB>(W, dres, theta); }
+}
+
+cudaError_t launch_sstep_epilogue(GmresWork W, int which, int sb, int nv, const double* red, double theta, int round, cudaStream_t st)
+{
+    switch (sb) {
+        case 3: sstep_epilogue_kernel<3><<<1, KTHREADS, 0, st>>>(W, which, nv, red, theta, round); break;
+        case 4: sstep_epilogue_kernel<4><<<1, KTHREADS, 0, st>>>(W, which, nv, red, theta, round); break;
+        case 5: sstep_epilogue_kernel<5><<<1, KTHREADS, 0, st>>>(W, which, nv, red, theta, round); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------------------
