@@ -248,8 +248,10 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None):
     """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
     operator 336 (block stencil) or 136 (matrix-free with the diagonal block and J rebuilt in the kernel, the default; 264 when it
     loads M^-1 and J).  Matrix-free default = s-step Arnoldi blocks of `block` = 5 columns per pass over the basis: per block at inner
-    index j five operator applications, one dot pass 24 (j+1 + 5) (per 32 basis vectors), one update pass 24 (j+1) + 48*5, the
-    in-block solve 24 (2*5 - 1); columns left over go through the two-column step (two operator applications, dots 24 (j+1) + 48 per
+    index j five operator applications, one dot pass 24 (j+1 + 5) (per 32 vectors; the block's own slots are dotted like basis vectors
+    from L1 / L2 and predict the in-block solve), one update pass 24 (j+1) + 48*5 that applies the predicted solve; a block whose
+    prediction is not used adds a pass of 24 (2*5 - 1) (none on the bench medium: `block_stats` in the line; not in this model);
+    columns left over go through the two-column step (two operator applications, dots 24 (j+1) + 48 per
     chunk of 8 vectors, update 24 (j+1) + 96, the W2 - gamma W1 pass 72) or the one-column step (dots 24 (j+2), update+norm 24 (j+3), one
     extra read of w per 16-vector pass), which the block-stencil path uses throughout.  Per cycle: combine 8 (3 jj + 15) + true residual
     (block stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24.  A block is enqueued whole: its operator applications, dot
@@ -264,8 +266,7 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None):
         j = 0
         while j < jj:
             if block >= 3 and j + block <= m:
-                total += block * op + 24.0 * (j + 1) + 24.0 * block * (j // 32 + 1) + 24.0 * (j + 1) + 48.0 * block
-                total += 24.0 * (2 * block - 1) if j + 1 < jj else 0.0
+                total += block * op + 24.0 * (j + 1) + 24.0 * block * ((j + block) // 32 + 1) + 24.0 * (j + 1) + 48.0 * block
                 j += block
             elif block >= 2 and j + 1 < m:
                 chunks = j // 8 + 1
@@ -454,7 +455,7 @@ def run_ours(args):
                                   "ms_per_iteration": tm["krylov_ms"] / max(its, 1), "cell_updates_per_s": N / (ms * 1e-3),
                                   "cell_iterations_per_s": N * its / (ms * 1e-3), "bytes_per_cell_per_iteration": bpc / max(its, 1),
                                   "krylov_achieved_gbs": kry_gbs, "krylov_hbm_frac": (kry_gbs / peak_gbs) if kry_gbs else None,
-                                  "cells_E_nonpositive": nE, "cells_f_above_one": nf}
+                                  "cells_E_nonpositive": nE, "cells_f_above_one": nf, "block_stats": g.block_stats()}
             brk[f"{ratio:g}x"] = {"T_implicit_over_T_explicit": ms / ms_exp, "implicit_wins": bool(ms / ms_exp < ratio)}
         line_extra["implicit"] = imp
         wins = [k for k, v in brk.items() if v["implicit_wins"]]
@@ -845,7 +846,7 @@ def run_decomposed(args):
     t_exp_max, _ = aggregate_over_ranks(t_exp, 0.0, dist if world > 1 else None)
     if rank == 0:
         halo_per_step = (st1["halo_bytes"] - st0["halo_bytes"]) / args.steps
-        interior = iteration_bytes_per_cell(its, operator=1, block=1) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
+        interior = iteration_bytes_per_cell(its, operator=1) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
         line = {
             "metric": METRIC, "value": 2.0 * N * args.steps / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",

@@ -206,6 +206,11 @@ ARK_M1_API int ark_m1_get_timings(ark_m1* h, double* out3);
 ARK_M1_API int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap);
 ARK_M1_API const char* ark_m1_kernel_class_name(int k);
 ARK_M1_API long long ark_m1_kernel_launches(const ark_m1* h);
+/* s-step Arnoldi blocks of the LAST linear solve, by the way their in-block factorisation went:
+ * out4[0] finished by the update pass (solve predicted by the dot pass, measured Gram matrix within tolerance),
+ * out4[1] predicted, then a second round from the measured Gram matrix, out4[2] measured factorisation and a separate in-block pass,
+ * out4[3] the same with a second round.  out4 is a host array of 4.  Zeros when the solve built no blocks. */
+ARK_M1_API int ark_m1_block_stats(const ark_m1* h, long long* out4);
 
 /* Self-test of the fast fp64 reciprocal / reciprocal square root of the hot kernels (MUFU seed + Newton steps): out4[0..3] =
  * max relative error of rcp_fast vs 1/x, rsqrt_fast vs 1/sqrt(x), sqrt_fast vs sqrt(x) and rcp_fast3 (one third-order step,

@@ -24,7 +24,7 @@ SYMBOLS = [
     "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
     "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_step_semi_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
-    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_fastmath_errors", "ark_m1_fp64_issue_rate", "ark_m1_apply_preconditioner", "ark_m1_device_bytes",
+    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_block_stats", "ark_m1_fastmath_errors", "ark_m1_fp64_issue_rate", "ark_m1_apply_preconditioner", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
     "ark_m1_slab_range", "ark_m1_group_create_local", "ark_m1_group_create_host", "ark_m1_nccl_unique_id", "ark_m1_group_create_nccl",
     "ark_m1_group_destroy", "ark_m1_group_set_stream", "ark_m1_group_local_slabs", "ark_m1_group_slab", "ark_m1_group_step_explicit",
@@ -93,6 +93,8 @@ def load_library(path: str | None = None):
     L.ark_m1_kernel_class_name.argtypes = [i]
     L.ark_m1_kernel_launches.restype = C.c_longlong
     L.ark_m1_kernel_launches.argtypes = [vp]
+    L.ark_m1_block_stats.restype = C.c_int
+    L.ark_m1_block_stats.argtypes = [vp, C.POINTER(C.c_longlong)]
     L.ark_m1_fastmath_errors.argtypes = [i, C.POINTER(C.c_double)]
     L.ark_m1_fp64_issue_rate.argtypes = [C.POINTER(C.c_double), i]
     L.ark_m1_device_bytes.restype = C.c_longlong
@@ -309,6 +311,12 @@ class ArkM1:
 
     def kernel_launches(self):
         return int(self._L.ark_m1_kernel_launches(self._h))
+
+    def block_stats(self):
+        """s-step Arnoldi blocks of the last linear solve: dict(update_pass, predicted_refined, separate_pass, separate_refined)."""
+        buf = (C.c_longlong * 4)()
+        self._check(self._L.ark_m1_block_stats(self._h, buf))
+        return dict(update_pass=int(buf[0]), predicted_refined=int(buf[1]), separate_pass=int(buf[2]), separate_refined=int(buf[3]))
 
     def device_bytes(self):
         return int(self._L.ark_m1_device_bytes(self._h))

@@ -580,12 +580,17 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
                 for (int k = 0; k < SB; ++k)
                     KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)(j + k) * S, h->V + (size_t)(j + k + 1) * S,
                                                                           k == 0 ? W.scale + j : nullptr, nullptr, 1.0, stop, 1, sm, h->st, k == 0 ? 0.0 : 1.0));
-                for (int c0 = 0; c0 <= j; c0 += 32) {
-                    const int nv = (j + 1 - c0) < 32 ? (j + 1 - c0) : 32;
-                    KL(KC_DOT, 24.0 * (nv + SB) * h->N, launch_dotS(w, h->V + (size_t)c0 * S, S, SB, nv, c0, n, W, sm, h->st));
+                // the dot pass takes the block's own slots j+1 .. j+SB as basis vectors as well (W^T W, read from L1/L2): it predicts the
+                // in-block solve, the update pass applies it and checks the result (krylov_sstep.cu: sstep_predict)
+                const int nd = j + 1 + SB;
+                for (int c0 = 0; c0 < nd; c0 += 32) {
+                    const int nv = (nd - c0) < 32 ? (nd - c0) : 32, nbasis = (j + 1 - c0) < 0 ? 0 : ((j + 1 - c0) < nv ? (j + 1 - c0) : nv);
+                    KL(KC_DOT, 24.0 * (nbasis + SB) * h->N, launch_dotS(w, h->V + (size_t)c0 * S, S, SB, nv, c0, n, W, sm, h->st, j));
                 }
-                KL(KC_UPDATE, (24.0 * (j + 1) + 48.0 * SB) * h->N, launch_updateS(w, h->V, S, SB, j + 1, n, W, sm, h->st));
-                KL(KC_UPDATE, 24.0 * (2 * SB - 1) * h->N, launch_qrS(w, S, SB, n, W, 1.0, 1, sm, h->st));
+                KL(KC_UPDATE, (24.0 * (j + 1) + 48.0 * SB) * h->N, launch_updateS(w, h->V, S, SB, j + 1, n, W, sm, h->st, 1.0));
+                // in-block solve as a pass of its own: only for a block whose prediction was not used (returns at once otherwise; its
+                // 24 (2 SB - 1) B per cell are not booked)
+                KL(KC_SMALL, 0.0, launch_qrS(w, S, SB, n, W, 1.0, 1, sm, h->st));
                 // second round for a block flagged ill-conditioned (both kernels return at once otherwise)
                 KL(KC_SMALL, 0.0, launch_gramS(w, S, SB, n, W, sm, h->st));
                 KL(KC_SMALL, 0.0, launch_qrS(w, S, SB, n, W, 1.0, 2, sm, h->st));
@@ -957,6 +962,13 @@ extern "C" int ark_m1_get_kernel_stats(ark_m1* h, double* out, int cap)
 }
 extern "C" const char* ark_m1_kernel_class_name(int k) { return (k >= 0 && k < KC_COUNT) ? kc_names[k] : ""; }
 extern "C" long long ark_m1_kernel_launches(const ark_m1* h) { return h ? h->launches : 0; }
+
+extern "C" int ark_m1_block_stats(const ark_m1* h, long long* out4)
+{
+    if (!h || !out4) return ARK_M1_E_ARG;
+    for (int k = 0; k < 4; ++k) out4[k] = h->ctl_host ? h->ctl_host->blk_stat[k] : 0;
+    return ARK_M1_OK;
+}
 
 // Self-test of the fast reciprocal / reciprocal square root used by the hot kernels: max relative errors against the IEEE
 // sequences over n samples in 200 binades.  No handle needed.  Returns 0 or ARK_M1_E_CUDA.

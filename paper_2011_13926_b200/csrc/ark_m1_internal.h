@@ -25,7 +25,10 @@ struct GmresCtl {
     int pad;
     double aux[2];                 // scratch norms (Newton update size)
     double bs[8];                  // BiCGStab scalars: rho, alpha, omega, rho_new, ||r|| (recursive), flag "restart after this iteration"
-    double blk[8];                 // two-column Arnoldi step: r11 = ||W1'||, <W1', W2'>, <W1', W1'>; s-step block: [3] accepted columns, [4] refine flag
+    double blk[8];                 // two-column Arnoldi step: r11 = ||W1'||, <W1', W2'>, <W1', W1'>; s-step block: [3] accepted columns, [4] refine flag,
+                                   // [5] in-block solve predicted by the dot pass (applied by the update pass), [6] block finished by the update pass
+    double gram[25];               // s-step block: W^T W from the dot pass (the block's own slots dotted like basis vectors)
+    int blk_stat[4];               // s-step blocks of this solve: finished in the update pass / predicted, then refined / classic / classic, refined
 };
 
 struct GmresWork {                 // device pointers into one small allocation
@@ -169,9 +172,11 @@ cudaError_t launch_update2_all(double* w1, double* w2, const double* V0, long lo
 // krylov_sstep.cu — the s-step Arnoldi block: sb = 3..SMAX vectors W_1..W_sb in consecutive slots w1, w1 + stride, ...
 int sstep_partial_doubles(int sm_count);
 // C_{i,k} = <W_{k+1}, V_i> scale_i for nv <= 32 basis vectors starting at index col0 (V0 = their first slot)
-cudaError_t launch_dotS(const double* w1, const double* V0, long long stride, int sb, int nv, int col0, long long n, GmresWork W, int sm_count, cudaStream_t st);
+cudaError_t launch_dotS(const double* w1, const double* V0, long long stride, int sb, int nv, int col0, long long n, GmresWork W, int sm_count, cudaStream_t st,
+                        int jpred = -1);
 // W_k -= sum_i coefS_{i,k} V_i over all nv basis vectors; Gram matrix of the result -> Cholesky, first column of the block finished
-cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int sb, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st);
+cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int sb, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st,
+                           double theta = 1.0);
 // in-block triangular solve with the Cholesky coefficients, norms of the results -> columns 2..sb of the block finished (theta = shift)
 // round 1 follows the update pass; round 2 (after launch_gramS) runs only when the block was flagged ill-conditioned (refinement)
 cudaError_t launch_qrS(double* w1, long long stride, int sb, long long n, GmresWork W, double theta, int round, int sm_count, cudaStream_t st);

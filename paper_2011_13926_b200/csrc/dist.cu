@@ -492,13 +492,15 @@ extern "C" int ark_m1_group_step_implicit(ark_m1_group* G, double dt, double tol
                     ark_m1* h = s.h;
                     double* w = h->V + (size_t)(j + 1) * h->stride;
                     GmresWork W = h->W; W.red_out = s.red;
-                    for (int c0 = 0; c0 <= j; c0 += 32) {
-                        const int nv = (j + 1 - c0) < 32 ? (j + 1 - c0) : 32;
-                        ark_kmark(h, KC_DOT, 24.0 * (nv + SB) * h->N);
-                        GCU(launch_dotS(w, h->V + (size_t)c0 * h->stride, h->stride, SB, nv, c0, 3 * h->N, W, h->sm_count, G->st));
+                    // the block's own slots are dotted like basis vectors (W^T W): the in-block solve is predicted from the reduced sums
+                    const int nd = j + 1 + SB;
+                    for (int c0 = 0; c0 < nd; c0 += 32) {
+                        const int nv = (nd - c0) < 32 ? (nd - c0) : 32, nbasis = (j + 1 - c0) < 0 ? 0 : ((j + 1 - c0) < nv ? (j + 1 - c0) : nv);
+                        ark_kmark(h, KC_DOT, 24.0 * (nbasis + SB) * h->N);
+                        GCU(launch_dotS(w, h->V + (size_t)c0 * h->stride, h->stride, SB, nv, c0, 3 * h->N, W, h->sm_count, G->st, j));
                     }
                 }
-                if ((rc = group_sstep_epilogue(G, SB * ld, 0, SB, j + 1, 0))) return rc;
+                if ((rc = group_sstep_epilogue(G, SB * ld, 0, SB, j + 1 + SB, 1))) return rc;
                 for (Slab& s : S) {
                     ark_m1* h = s.h;
                     GmresWork W = h->W; W.red_out = s.red;
@@ -519,7 +521,7 @@ extern "C" int ark_m1_group_step_implicit(ark_m1_group* G, double dt, double tol
                     for (Slab& s : S) {
                         ark_m1* h = s.h;
                         GmresWork W = h->W; W.red_out = s.red;
-                        ark_kmark(h, round == 1 ? KC_UPDATE : KC_SMALL, round == 1 ? 24.0 * (2 * SB - 1) * h->N : 0.0);
+                        ark_kmark(h, KC_SMALL, 0.0);      // a pass of its own only for a block whose predicted solve was not used
                         GCU(launch_qrS(h->V + (size_t)(j + 1) * h->stride, h->stride, SB, 3 * h->N, W, 1.0, round, h->sm_count, G->st));
                     }
                     if ((rc = group_sstep_epilogue(G, SB - 1, 2, SB, j + 1, round))) return rc;

@@ -556,6 +556,8 @@ __global__ void begin_solve_kernel(GmresWork W, double tol, int m, int maxit)
     c->bnorm = 0.0; c->target = 0.0; c->rnorm = 0.0; c->est = tol;
     c->m = m; c->maxit = maxit; c->its = 0; c->j = 0; c->inner_stop = 0; c->converged = 0; c->nonfinite = 0;
     c->nhist = 0; c->ticket = 0;
+    for (int k = 0; k < 8; ++k) c->blk[k] = 0.0;
+    for (int k = 0; k < 4; ++k) c->blk_stat[k] = 0;
 }
 
 cudaError_t launch_begin_solve(GmresWork W, double tol, int m, int maxit, cudaStream_t st)

@@ -20,6 +20,10 @@
 // round (gramS_kernel + qrS_kernel round 2: Gram matrix of the q~, Cholesky, solve; "CholQR2"), whose kernels return at once for every
 // other block; W' = Q~ T with T = T2 T1 the product of the unit triangular factors, R~ = diag(n) T.  A pivot below SS_RHO_DROP (the
 // Krylov space is exhausted inside the block, or beyond what two rounds repair) truncates the block there and ends the cycle.
+// Prediction.  The dot pass also dots the block's own slots (S = W^T W, the operands already in L1), so G' = S - C^T C gives the
+// Cholesky factor BEFORE the update pass; for a well-conditioned block (predicted rho >= SS_RHO_PRED) the update pass applies the
+// in-block solve to the registers it holds and measures the Gram matrix of the q~; if that is orthogonal to SS_PRED_TOL the block is
+// finished there and the separate in-block pass (216 of ~1900 B per cell and block) is not run (sstep_predict, sstep_pred_epilogue).
 #include <stdio.h>
 #include "krylov_device.cuh"
 
@@ -27,6 +31,10 @@ namespace ark {
 
 static constexpr int GS_BLOCKS_PER_SM_SS = 2;   // one wave of two 256-thread blocks per SM, like the other Gram-Schmidt streams
 static constexpr double SS_RHO_REFINE = 1e-5, SS_RHO_DROP = 1e-13;     // thresholds 1e-5 .. 0.5 give the same iteration counts on every system tried
+// prediction of the in-block solve (sstep_predict): used when every predicted pivot ratio is at least SS_RHO_PRED and no diagonal entry of
+// S - C^T C lost more than three digits; the block counts as finished when the MEASURED Gram matrix of the q~ has every
+// |<q~_k, q~_l>| <= SS_PRED_TOL ||q~_k|| ||q~_l|| (what one round of the measured factorisation reaches for rho >= SS_RHO_REFINE)
+static constexpr double SS_RHO_PRED = 1e-3, SS_PRED_CANCEL = 1e-3, SS_PRED_TOL = 1e-10;
 static constexpr int SS_NVW = 4;              // basis vectors per warp of the dot kernel (8 warps -> 32 vectors per launch)
 static constexpr int SS_CH = 8 * SS_NVW;      // basis vectors per launch of the dot kernel
 __host__ __device__ constexpr int ss_ng(int s) { return s * (s + 1) / 2; }
@@ -43,8 +51,13 @@ __device__ __forceinline__ double2 ld_cs2(const double2* p) { return __ldcs(p); 
 // ---------------------------------------------------------------------------------------------------------
 template <int SB, int NVW, int U>
 __device__ __forceinline__ void dotS_body(const double* __restrict__ w1, const double* __restrict__ V0, long long stride, long long n2,
-                                          int grp, int G, int rep, int R, int lane, double (&acc)[SB][SS_NVW])
+                                          int grp, int G, int rep, int R, int lane, int wfirst, double (&acc)[SB][SS_NVW])
 {
+    // vectors wfirst.. of the chunk are the block's own slots: the same lines the `a` loads of this block bring into L1, so they are
+    // read through L1 (the basis streams past it)
+    bool own[NVW];
+#pragma unroll
+    for (int q = 0; q < NVW; ++q) own[q] = (grp + q * G) >= wfirst;
     const long long tile = 32LL * U;
     for (long long t = (long long)rep * gridDim.x + blockIdx.x; t * tile < n2; t += (long long)R * gridDim.x) {
         const long long e0 = t * tile + lane;
@@ -56,7 +69,10 @@ __device__ __forceinline__ void dotS_body(const double* __restrict__ w1, const d
 #pragma unroll
             for (int k = 0; k < SB; ++k) a[u][k] = in ? reinterpret_cast<const double2*>(w1 + k * stride)[e] : make_double2(0.0, 0.0);
 #pragma unroll
-            for (int q = 0; q < NVW; ++q) b[u][q] = in ? ld_cs2(reinterpret_cast<const double2*>(V0 + (long long)(grp + q * G) * stride) + e) : make_double2(0.0, 0.0);
+            for (int q = 0; q < NVW; ++q) {
+                const double2* pb = reinterpret_cast<const double2*>(V0 + (long long)(grp + q * G) * stride) + e;
+                b[u][q] = in ? (own[q] ? *pb : ld_cs2(pb)) : make_double2(0.0, 0.0);
+            }
         }
 #pragma unroll
         for (int u = 0; u < U; ++u)
@@ -67,9 +83,11 @@ __device__ __forceinline__ void dotS_body(const double* __restrict__ w1, const d
     }
 }
 
+template <int SB> __device__ __forceinline__ void sstep_predict(const GmresWork& W, int j);
+
 template <int SB>
 __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) multi_dotS_kernel(const double* __restrict__ w1, const double* __restrict__ V0,
-                                                                                    long long stride, long long n, GmresWork W, int nv, int col0)
+                                                                                    long long stride, long long n, GmresWork W, int nv, int col0, int jpred)
 {
     if (W.ctl->inner_stop) return;
     __shared__ double sred[KTHREADS / 32][SB * SS_NVW];
@@ -81,16 +99,17 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) multi_dotS_kern
     const int grp = warp % G, rep = warp / G;
     const int nvw = (rep < R) ? (nv - grp + G - 1) / G : 0;          // vectors of this warp (0: spare warp)
     const long long n2 = n >> 1;
+    const int wfirst = (jpred >= 0) ? jpred + 1 - col0 : (1 << 30);
     double acc[SB][SS_NVW];
 #pragma unroll
     for (int k = 0; k < SB; ++k)
 #pragma unroll
         for (int q = 0; q < SS_NVW; ++q) acc[k][q] = 0.0;
     switch (nvw) {      // loads in flight per lane: (SB + nvw) U >= 14
-        case 1: dotS_body<SB, 1, 3>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
-        case 2: dotS_body<SB, 2, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
-        case 3: dotS_body<SB, 3, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
-        case 4: dotS_body<SB, 4, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, acc); break;
+        case 1: dotS_body<SB, 1, 3>(w1, V0, stride, n2, grp, G, rep, R, lane, wfirst, acc); break;
+        case 2: dotS_body<SB, 2, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, wfirst, acc); break;
+        case 3: dotS_body<SB, 3, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, wfirst, acc); break;
+        case 4: dotS_body<SB, 4, 2>(w1, V0, stride, n2, grp, G, rep, R, lane, wfirst, acc); break;
         default: break;
     }
 #pragma unroll
@@ -127,11 +146,17 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) multi_dotS_kern
             if (n & 1) s += w1[k * stride + n - 1] * V0[(long long)i * stride + n - 1];
             const int ld = W.ctl->m + 1, col = col0 + i;
             if (W.red_out) { W.red_out[k * ld + col] = s; return; }      // slab decomposition: this rank's sums; all-reduce and epilogue follow
-            const double c = s * W.scale[col];
-            W.cS[k * ld + col] = c;
-            W.coefS[k * ld + col] = c * W.scale[col];
+            if (jpred >= 0 && col > jpred) W.ctl->gram[k * SMAX + (col - jpred - 1)] = s;      // a slot of the block itself: <W_k, W_l>
+            else {
+                const double c = s * W.scale[col];
+                W.cS[k * ld + col] = c;
+                W.coefS[k * ld + col] = c * W.scale[col];
+            }
         }
     }
+    if (W.red_out || jpred < 0 || col0 + nv != jpred + 1 + SB) return;      // (uniform) no prediction here, or more chunks of this block follow
+    __syncthreads();
+    sstep_predict<SB>(W, jpred);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -181,6 +206,50 @@ __device__ int sstep_factor(const double* __restrict__ G, double drop, double (&
     return nacc;
 }
 
+// Prediction of the in-block solve by the dot pass (its last block, all threads).  The dot pass also dots the block's own slots like
+// basis vectors, S = W^T W; with C = V^T W and V orthonormal the Gram matrix of W' = W - V C is G' = S - C^T C, so the Cholesky factor and
+// the coefficients t of the solve are known BEFORE the update pass, which then applies the solve to the registers it already holds
+// the block in (q~ = W' T^-1 element by element) and measures the Gram matrix of the q~.  Whatever T is, W' = Q~ T holds by
+// construction and the recovery of the Hessenberg columns uses the T applied and the norms measured; T only decides how orthogonal
+// the q~ are, and that is CHECKED on the measured Gram matrix (sstep_pred_epilogue): a block that passes is finished without the
+// separate in-block pass (216 B per cell less), one that fails goes through the second round with the Gram matrix just measured.
+template <int SB>
+__device__ __forceinline__ void sstep_predict(const GmresWork& W, int j)
+{
+    __shared__ double Gp[SMAX * SMAX];
+    GmresCtl* c = W.ctl;
+    const int ld = c->m + 1;
+    if (threadIdx.x < SB * SB) {
+        const int k = threadIdx.x / SB, l = threadIdx.x % SB;
+        double s = 0.0;
+        for (int i = 0; i <= j; ++i) s = fma(W.cS[k * ld + i], W.cS[l * ld + i], s);
+        Gp[k * SMAX + l] = 0.5 * (c->gram[k * SMAX + l] + c->gram[l * SMAX + k]) - s;
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    double G[ss_ng(SB)], t[SB][SB], rho[SB], r00;
+    int p = 0;
+    bool ok = true;
+    for (int k = 0; k < SB; ++k) {
+        for (int l = k; l < SB; ++l) G[p++] = Gp[k * SMAX + l];
+        ok = ok && (Gp[k * SMAX + k] > SS_PRED_CANCEL * c->gram[k * SMAX + k]);
+    }
+    const int nacc = sstep_factor<SB>(G, SS_RHO_DROP, t, rho, r00);
+    ok = ok && nacc == SB;
+    for (int k = 0; k < SB; ++k) ok = ok && (rho[k] >= SS_RHO_PRED);
+#ifdef SS_DEBUG
+    printf("pred j=%d ok=%d rho:", j, (int)ok); for (int k = 0; k < SB; ++k) printf(" %.2e", rho[k]);
+    printf("  G'/S:"); for (int k = 0; k < SB; ++k) printf(" %.2e", Gp[k * SMAX + k] / c->gram[k * SMAX + k]); printf("\n");
+#endif
+    c->blk[5] = ok ? 1.0 : 0.0;
+    c->blk[6] = 0.0;
+    if (!ok) return;
+    for (int k = 0; k < SB; ++k)
+        for (int l = 0; l < SB; ++l) { W.tb[k * SMAX + l] = t[k][l]; W.Rb[k * SMAX + l] = (k == l) ? 1.0 : t[k][l]; }
+    c->blk[3] = (double)SB;
+    c->blk[4] = 0.0;
+}
+
 // the scalar part of the epilogue after the update pass (thread 0 of the last block)
 template <int SB>
 __device__ void sstep_first_round(const GmresWork& W, const double* __restrict__ G, const double* hcol, const double* ccs, const double* ssn)
@@ -195,6 +264,7 @@ __device__ void sstep_first_round(const GmresWork& W, const double* __restrict__
         for (int l = 0; l < SB; ++l) { W.tb[k * SMAX + l] = t[k][l]; W.Rb[k * SMAX + l] = (k == l) ? 1.0 : t[k][l]; }
     c->blk[3] = (double)nacc;
     c->blk[4] = (nacc > 1 && rmin < SS_RHO_REFINE) ? 1.0 : 0.0;
+    c->blk_stat[c->blk[4] != 0.0 ? 3 : 2] += 1;
 #ifdef SS_DEBUG
     printf("blk j=%d nacc=%d refine=%d rho:", j, nacc, (int)c->blk[4]); for (int k = 0; k < SB; ++k) printf(" %.2e", rho[k]); printf("\n");
 #endif
@@ -224,17 +294,77 @@ __device__ __forceinline__ void sstep_update_epilogue(const GmresWork& W, const 
     if (threadIdx.x == 0) sstep_first_round<SB>(W, dres, hcol, ccs, ssn);
 }
 
+template <int SB> __device__ __forceinline__ void sstep_finish_block(const GmresWork& W, const double* dres, double theta);
+template <int SB> __device__ __forceinline__ void sstep_second_round(const GmresWork& W, const double* dres);
+
+// last block of an update pass that applied the predicted solve: column j from the measured ||q~_1||, then the check of the measured
+// Gram matrix: orthogonal -> the remaining columns of the block here; not -> second round from this Gram matrix (qrS_kernel round 2)
+template <int SB>
+__device__ __forceinline__ void sstep_pred_epilogue(const GmresWork& W, const double* dres, double theta, double* hcol, double* ccs, double* ssn)
+{
+    __shared__ double nrm2[SMAX];
+    __shared__ int verdict;          // 0: the block is orthogonal, finish it here   1: second round   2: nothing more to do
+    GmresCtl* c = W.ctl;
+    const int j = c->j, m = c->m;
+    for (int i = threadIdx.x; i <= j; i += blockDim.x) {
+        const double h = W.cS[i];
+        hcol[i] = h; W.Hraw[i * m + j] = h;
+        if (i < j) { ccs[i] = W.cs[i]; ssn[i] = W.sn[i]; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double Gd[SB];
+        int p = 0;
+        double defect = 0.0;
+        for (int k = 0; k < SB; ++k) { Gd[k] = dres[p]; p += SB - k; }
+        p = 0;
+        for (int k = 0; k < SB; ++k)
+            for (int l = k; l < SB; ++l) { if (l > k) { const double d = fabs(dres[p]) / sqrt(Gd[k] * Gd[l]); defect = (d > defect || !(d == d)) ? d : defect; } ++p; }
+        const bool orth = defect <= SS_PRED_TOL;        // false for a NaN as well
+#ifdef SS_DEBUG
+        printf("  pred-applied j=%d defect=%.2e\n", j, defect);
+#endif
+        if (!(Gd[0] > 0.0)) {          // W'_1 = 0: the space is exhausted at column j
+            W.Hraw[(j + 1) * m + j] = 0.0;
+            finish_column(W, c, j, 0.0, hcol, ccs, ssn);
+            c->blk[6] = 1.0;
+            verdict = 2;
+        } else {
+            const double r00 = sqrt(Gd[0]);
+            c->blk[0] = r00;
+            W.Hraw[(j + 1) * m + j] = r00;
+            finish_column(W, c, j, r00, hcol, ccs, ssn);
+            if (c->inner_stop) { c->blk[6] = 1.0; verdict = 2; }
+            else if (orth) {
+                for (int k = 1; k < SB; ++k) nrm2[k - 1] = Gd[k];
+                c->blk[6] = 1.0; c->blk_stat[0] += 1;
+                verdict = 0;
+            } else {
+                sstep_second_round<SB>(W, dres);      // T <- T2 T1, coefficients of round 2 from the Gram matrix measured here
+                c->blk[4] = 1.0; c->blk_stat[1] += 1;
+                if ((int)c->blk[3] <= 1) c->inner_stop = 1;
+                verdict = 1;
+            }
+        }
+    }
+    __syncthreads();
+    if (verdict == 0) sstep_finish_block<SB>(W, nrm2, theta);
+}
+
 template <int SB>
 __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) updateS_kernel(double* __restrict__ w1, const double* __restrict__ V0, long long stride,
-                                                                                 long long n, GmresWork W, int nv)
+                                                                                 long long n, GmresWork W, int nv, double theta)
 {
     if (W.ctl->inner_stop) return;
     constexpr int NG = ss_ng(SB);
     __shared__ double cf[SS_MAXNV * SB];
+    __shared__ double tsh[SMAX * SMAX];
     __shared__ double dres[MAXV];
     __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
     const int ld = W.ctl->m + 1;
+    const bool pred = W.ctl->blk[5] != 0.0;      // the dot pass predicted the in-block solve: apply it here
     for (int q = threadIdx.x; q < nv * SB; q += KTHREADS) cf[q] = W.coefS[(q % SB) * ld + q / SB];
+    if (threadIdx.x < SMAX * SMAX) tsh[threadIdx.x] = pred ? W.tb[threadIdx.x] : 0.0;
     __syncthreads();
     double acc[NG];
 #pragma unroll
@@ -256,6 +386,12 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) updateS_kernel(
             case 7: updS_batch<SB, 7>(a, V0 + (long long)q0 * stride, stride, e, cf + q0 * SB); break;
             default: break;
         }
+        if (pred) {
+#pragma unroll
+            for (int k = 1; k < SB; ++k)
+#pragma unroll
+                for (int l = 0; l < k; ++l) { const double t = tsh[l * SMAX + k]; a[k].x = fma(-t, a[l].x, a[k].x); a[k].y = fma(-t, a[l].y, a[k].y); }
+        }
         int p = 0;
 #pragma unroll
         for (int k = 0; k < SB; ++k) {
@@ -266,13 +402,16 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) updateS_kernel(
     }
     if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         double a[SB];
-        for (int k = 0; k < SB; ++k) { a[k] = w1[k * stride + n - 1]; for (int q = 0; q < nv; ++q) a[k] -= cf[q * SB + k] * V0[(long long)q * stride + n - 1]; w1[k * stride + n - 1] = a[k]; }
+        for (int k = 0; k < SB; ++k) { a[k] = w1[k * stride + n - 1]; for (int q = 0; q < nv; ++q) a[k] -= cf[q * SB + k] * V0[(long long)q * stride + n - 1]; }
+        for (int k = 1; k < SB; ++k) for (int l = 0; l < k; ++l) a[k] -= tsh[l * SMAX + k] * a[l];
+        for (int k = 0; k < SB; ++k) w1[k * stride + n - 1] = a[k];
         int p = 0;
         for (int k = 0; k < SB; ++k) for (int l = k; l < SB; ++l) acc[p++] += a[k] * a[l];
     }
     if (!reduce_to_last<NG>(acc, W, dres)) return;
     if (W.red_out) { if (threadIdx.x < NG) W.red_out[threadIdx.x] = dres[threadIdx.x]; return; }
-    sstep_update_epilogue<SB>(W, dres, hcol, ccs, ssn);
+    if (pred) sstep_pred_epilogue<SB>(W, dres, theta, hcol, ccs, ssn);
+    else sstep_update_epilogue<SB>(W, dres, hcol, ccs, ssn);
 }
 
 // Columns j0+1 .. j0+nacc-1 of the Hessenberg matrix from the measured norms of the in-block solve (c->j = j0 + 1 here: the update pass
@@ -333,9 +472,10 @@ __device__ __forceinline__ void sstep_finish_block(const GmresWork& W, const dou
 template <int SB>
 __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(double* __restrict__ w1, long long stride, long long n, GmresWork W, double theta, int round)
 {
-    if (W.ctl->inner_stop) return;
+    if (W.ctl->inner_stop || W.ctl->blk[6] != 0.0) return;      // [6]: the update pass finished the block (predicted solve, verified)
     const bool refine = W.ctl->blk[4] != 0.0;
     if (round == 2 && !refine) return;
+    if (round == 1 && W.ctl->blk[5] != 0.0) return;             // [5]: round 1 was applied by the update pass; round 2 follows
     __shared__ double tsh[SMAX * SMAX];
     __shared__ double dres[MAXV];
     if (threadIdx.x < SMAX * SMAX) tsh[threadIdx.x] = W.tb[threadIdx.x];
@@ -367,13 +507,11 @@ __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) qrS_kernel(doub
     sstep_finish_block<SB>(W, dres, theta);
 }
 
-template <int SB> __device__ __forceinline__ void sstep_second_round(const GmresWork& W, const double* dres);
-
 // Second round for an ill-conditioned block: Gram matrix of the q~ of round 1, Cholesky, coefficients of round 2, T = T2 T1.
 template <int SB>
 __global__ void __launch_bounds__(KTHREADS, GS_BLOCKS_PER_SM_SS) gramS_kernel(const double* __restrict__ w1, long long stride, long long n, GmresWork W)
 {
-    if (W.ctl->inner_stop || W.ctl->blk[4] == 0.0) return;
+    if (W.ctl->inner_stop || W.ctl->blk[4] == 0.0 || W.ctl->blk[5] != 0.0 || W.ctl->blk[6] != 0.0) return;   // ([5]: that Gram matrix came with the update pass)
     constexpr int NG = ss_ng(SB);
     __shared__ double dres[MAXV];
     double acc[NG];
@@ -440,20 +578,30 @@ __global__ void __launch_bounds__(KTHREADS) sstep_epilogue_kernel(GmresWork W, i
     __shared__ double dres[MAXV];
     __shared__ double hcol[EPI_MAX + 1], ccs[EPI_MAX], ssn[EPI_MAX];
     const int ld = c->m + 1;
-    if (which == 0) {
+    if (which == 0) {       // round = 1: the last SB of the nv vectors are the block's own slots (W^T W) and the in-block solve is predicted
+        const int jp = (round == 1) ? nv - 1 - SB : -1;
         for (int ent = threadIdx.x; ent < SB * nv; ent += KTHREADS) {
             const int k = ent / nv, i = ent % nv;
+            if (jp >= 0 && i > jp) { c->gram[k * SMAX + (i - jp - 1)] = red[k * ld + i]; continue; }
             const double cc = red[k * ld + i] * W.scale[i];
             W.cS[k * ld + i] = cc; W.coefS[k * ld + i] = cc * W.scale[i];
         }
+        if (jp < 0) return;
+        __syncthreads();
+        sstep_predict<SB>(W, jp);
         return;
     }
     const bool refine = c->blk[4] != 0.0;
+    if (c->blk[6] != 0.0 && which != 1) return;                              // the update pass finished the block
     if ((which == 3 || (which == 2 && round == 2)) && !refine) return;
+    if ((which == 3 || (which == 2 && round == 1)) && c->blk[5] != 0.0) return;   // round 1 and its Gram matrix came with the update pass
     const int nsum = (which == 2) ? SB - 1 : ss_ng(SB);
     if (threadIdx.x < nsum) dres[threadIdx.x] = red[threadIdx.x];
     __syncthreads();
-    if (which == 1) sstep_update_epilogue<SB>(W, dres, hcol, ccs, ssn);
+    if (which == 1) {
+        if (c->blk[5] != 0.0) sstep_pred_epilogue<SB>(W, dres, theta, hcol, ccs, ssn);
+        else sstep_update_epilogue<SB>(W, dres, hcol, ccs, ssn);
+    }
     else if (which == 3) sstep_second_round<SB>(W, dres);
     else { if (round == 1 && refine) return; sstep_finish_block<SB>(W, dres, theta); }
 }
@@ -477,27 +625,27 @@ static int ss_grid(long long n, int sm_count)
     return (int)(need < 1 ? 1 : (need < cap ? need : cap));
 }
 
-cudaError_t launch_dotS(const double* w1, const double* V0, long long stride, int sb, int nv, int col0, long long n, GmresWork W, int sm_count, cudaStream_t st)
+cudaError_t launch_dotS(const double* w1, const double* V0, long long stride, int sb, int nv, int col0, long long n, GmresWork W, int sm_count, cudaStream_t st, int jpred)
 {
     if (nv < 1 || nv > SS_CH) return cudaErrorInvalidValue;
     const int grd = ss_grid(n, sm_count);
     switch (sb) {
-        case 3: multi_dotS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0); break;
-        case 4: multi_dotS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0); break;
-        case 5: multi_dotS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0); break;
+        case 3: multi_dotS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0, jpred); break;
+        case 4: multi_dotS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0, jpred); break;
+        case 5: multi_dotS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, col0, jpred); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
 }
 
-cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int sb, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st)
+cudaError_t launch_updateS(double* w1, const double* V0, long long stride, int sb, int nv, long long n, GmresWork W, int sm_count, cudaStream_t st, double theta)
 {
     if (nv < 1 || nv > SS_MAXNV) return cudaErrorInvalidValue;
     const int grd = ss_grid(n, sm_count);
     switch (sb) {
-        case 3: updateS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv); break;
-        case 4: updateS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv); break;
-        case 5: updateS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv); break;
+        case 3: updateS_kernel<3><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, theta); break;
+        case 4: updateS_kernel<4><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, theta); break;
+        case 5: updateS_kernel<5><<<grd, KTHREADS, 0, st>>>(w1, V0, stride, n, W, nv, theta); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

@@ -632,9 +632,10 @@ int ark_m1_3d_step_implicit(ark_m1_3d* h, double dt, double tol, int restart, in
                 // s-step Arnoldi block, as in the 2-D solver (krylov_sstep.cu; the vector kernels only see vectors of 4N doubles)
                 for (int k = 0; k < SB; ++k)
                     if ((rc = apply3(h, h->V + (size_t)(j + k) * S, h->V + (size_t)(j + k + 1) * S, k == 0 ? W.scale + j : nullptr, nullptr, 1.0, dt, 1, stop, k == 0 ? 0.0 : 1.0))) return rc;
-                for (int c0 = 0; c0 <= j; c0 += 32) {
-                    const int nv = (j + 1 - c0) < 32 ? (j + 1 - c0) : 32;
-                    CU3(launch_dotS(w, h->V + (size_t)c0 * S, S, SB, nv, c0, n, W, sm, h->st));
+                const int nd = j + 1 + SB;          // the block's own slots are dotted like basis vectors: the in-block solve is predicted
+                for (int c0 = 0; c0 < nd; c0 += 32) {
+                    const int nv = (nd - c0) < 32 ? (nd - c0) : 32;
+                    CU3(launch_dotS(w, h->V + (size_t)c0 * S, S, SB, nv, c0, n, W, sm, h->st, j));
                     h->launches++;
                 }
                 CU3(launch_updateS(w, h->V, S, SB, j + 1, n, W, sm, h->st));

@@ -100,3 +100,35 @@ def test_ill_conditioned_blocks_are_refined(k):
     dt = k * wl.explicit_dt(w["dx"], w["dy"], w["c"])
     # histories: equal to 1e-5 relative down to a residual of 1e-8, within 0.3 % at 1e-10 (eleven orders below the start)
     _check_against_one_column(w, dt, dcount=1, hist_tol=1e-2)
+
+
+def _stats(w, dt, blk, restart=30, tol=1e-10, maxit=4000):
+    g = make_gpu(w, dict(arnoldi_block=blk))
+    its, res = g.step_implicit(dt, tol, restart, maxit)
+    return its, res, g.block_stats()
+
+
+@pytest.mark.parametrize("blk", [3, 4, 5])
+def test_well_conditioned_blocks_finish_in_the_update_pass(blk):
+    # bench medium (small): the dot pass predicts the in-block solve from S - C^T C, the update pass applies it and the measured Gram
+    # matrix of the result passes the orthogonality check: no block takes the separate in-block pass, and the count is that of the
+    # one-column solver (checked for the same systems above).  Every full block of the solve is accounted for in the four counters.
+    w = wl.random_medium(192, seed=21)
+    dt = 10 * wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    i1, r1, s1 = _stats(w, dt, 1)
+    assert s1 == dict(update_pass=0, predicted_refined=0, separate_pass=0, separate_refined=0)
+    ib, rb, sb = _stats(w, dt, blk)
+    assert rb <= 1e-10 and abs(ib - i1) <= 1
+    assert sb["update_pass"] >= 1 and sb["separate_pass"] == 0 and sb["separate_refined"] == 0 and sb["predicted_refined"] == 0
+    full_blocks_per_cycle = 30 // blk
+    assert sum(sb.values()) <= -(-ib // 30) * full_blocks_per_cycle and sum(sb.values()) >= (ib // 30) * full_blocks_per_cycle
+
+
+def test_ill_conditioned_blocks_do_not_use_the_prediction():
+    # smooth diffusive problem (see test_ill_conditioned_blocks_are_refined): the predicted pivot ratios of the first block fall below
+    # 1e-3, so the prediction is not applied and the block takes the measured factorisation with its second round
+    w = wl.gaussian_diffusion(1024)
+    dt = 100 * wl.explicit_dt(w["dx"], w["dy"], w["c"])
+    its, res, st = _stats(w, dt, 5)
+    assert res <= 1e-10 and its <= 18
+    assert st["separate_refined"] >= 1 and st["update_pass"] + st["predicted_refined"] < sum(st.values())
