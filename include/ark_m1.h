@@ -190,6 +190,14 @@ ARK_M1_API int ark_m1_apply_operator(ark_m1* h, double dt, const double* V, doub
  * the inverse 3x3 diagonal blocks (Eq. 27 block-wise; option "preconditioner" = 0, default) or one multigrid V-cycle
  * ("preconditioner" = 1, R15).  V, out: 3*nx*ny doubles, host or device.  Synchronises. */
 ARK_M1_API int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* V, double* out);
+/* Two applications of the preconditioned operator in a row, as the s-step Arnoldi block issues them (DESIGN.md "Two applications
+ * per pass"): out1 = A M^-1 V - theta1 V, out2 = A M^-1 out1 - theta2 out1 for the linearisation of a step dt at the current
+ * state (A = I + dt L_n; M = its 3x3 block diagonal).  V, out1, out2: 3 planes of nx*ny doubles
+ * each (E, Fx, Fy), host or device.  With option "op_pair" = 1 (default) on a grid periodic on all four sides and the default
+ * matrix-free operator (op_recompute = 2) both come from ONE pass over the coefficient planes; otherwise from two passes.
+ * Returns 1 if the one-pass kernel ran, 0 if two passes did, < 0 on error (ARK_M1_E_UNSUPPORTED with option operator = 0).
+ * Synchronises the handle's stream. */
+ARK_M1_API int ark_m1_apply_operator_pair(ark_m1* h, double dt, const double* V, double* out1, double* out2, double theta1, double theta2);
 
 /* Relative residual history of the last implicit solve: entry 0 = true residual of the initial guess, then one
  * estimate per inner iteration.  Copies min(cap, n) values into buf (host) and returns n. */

@@ -24,7 +24,7 @@ SYMBOLS = [
     "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
     "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_step_semi_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
-    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_block_stats", "ark_m1_fastmath_errors", "ark_m1_fp64_issue_rate", "ark_m1_apply_preconditioner", "ark_m1_device_bytes",
+    "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_block_stats", "ark_m1_fastmath_errors", "ark_m1_fp64_issue_rate", "ark_m1_apply_preconditioner", "ark_m1_apply_operator_pair", "ark_m1_device_bytes",
     "ark_m1_last_error", "ark_m1_version",
     "ark_m1_slab_range", "ark_m1_group_create_local", "ark_m1_group_create_host", "ark_m1_nccl_unique_id", "ark_m1_group_create_nccl",
     "ark_m1_group_destroy", "ark_m1_group_set_stream", "ark_m1_group_local_slabs", "ark_m1_group_slab", "ark_m1_group_step_explicit",
@@ -86,6 +86,7 @@ def load_library(path: str | None = None):
     L.ark_m1_residual.argtypes = [vp, dp, dp]
     L.ark_m1_apply_operator.argtypes = [vp, d, dp, dp, dp]
     L.ark_m1_apply_preconditioner.argtypes = [vp, d, dp, dp]
+    L.ark_m1_apply_operator_pair.argtypes = [vp, d, dp, dp, dp, d, d]
     L.ark_m1_get_history.argtypes = [vp, C.POINTER(C.c_double), i]
     L.ark_m1_get_timings.argtypes = [vp, C.POINTER(C.c_double)]
     L.ark_m1_get_kernel_stats.argtypes = [vp, C.POINTER(C.c_double), i]
@@ -290,6 +291,13 @@ class ArkM1:
         out = np.empty((3, self.ny, self.nx))
         self._check(self._L.ark_m1_apply_preconditioner(self._h, float(dt), p, out.ctypes.data))
         return out
+
+    def apply_operator_pair(self, dt, V, theta1=0.0, theta2=0.0):
+        """(out1, out2, fused): out1 = A M^-1 V - theta1 V, out2 = A M^-1 out1 - theta2 out1; fused = the one-pass kernel ran."""
+        p, keep = _ptr(V, 3 * self.N)
+        o1 = np.empty((3, self.ny, self.nx)); o2 = np.empty((3, self.ny, self.nx))
+        fused = self._check(self._L.ark_m1_apply_operator_pair(self._h, float(dt), p, o1.ctypes.data, o2.ctypes.data, float(theta1), float(theta2)))
+        return o1, o2, bool(fused)
 
     def history(self):
         n = self._L.ark_m1_get_history(self._h, None, 0)

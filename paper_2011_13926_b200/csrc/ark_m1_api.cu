@@ -126,7 +126,7 @@ ark_m1* ark_m1_create(int nx, int ny, double dx, double dy, double c, const ark_
     h->g.nx = nx; h->g.ny = ny; h->g.dx = dx; h->g.dy = dy; h->g.c = c;
     for (int s = 0; s < 4; ++s) h->g.bc[s] = b[s];
     h->s.wb = 1; h->s.ap = 1; h->s.eig = 0; h->s.closure = 0; h->s.lin = 0; h->s.eig_floor = 0.0; h->s.a_r = 1.0; h->s.src_off = 0; h->s.hyp_off = 0;
-    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 2; h->apply_precond = 0; h->arnoldi_block = 5;
+    h->ortho = 1; h->explicit_kernel = 3; h->op_kind = 1; h->maxv = 16; h->asm_kernel = 1; h->op_recompute = 2; h->apply_precond = 0; h->arnoldi_block = 5; h->op_pair = 1;
     h->basis_prec = 64; h->precond = 0; h->mg.omega = 0.8; h->mg.coarse_sweeps = 2; h->mg.nlev = 0; h->mg.precision = 64;
     h->device = dev; h->N = (long long)nx * ny; h->st = 0;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -251,6 +251,7 @@ int ark_m1_set_option(ark_m1* h, const char* key, double value)
     else if (!strcmp(key, "kernel_timing")) { ark_kflush(h); h->ktiming = (value != 0.0); if (h->ktiming) memset(h->kstat, 0, sizeof h->kstat); }
     else if (!strcmp(key, "operator")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "operator must be 0 (block stencil) or 1 (matrix-free)%s", ""); h->op_kind = iv; }
     else if (!strcmp(key, "apply_operator_precond")) h->apply_precond = (value != 0.0);
+    else if (!strcmp(key, "op_pair")) h->op_pair = (value != 0.0);
     else if (!strcmp(key, "arnoldi_block")) { if (iv < 1 || iv > SMAX) return ark_fail(h, ARK_M1_E_ARG, "arnoldi_block must be 1 (one column per pass over the basis), 2 (two columns) or 3..5 (s-step block)%s", ""); h->arnoldi_block = iv; }
     else if (!strcmp(key, "op_recompute")) { if (iv < 0 || iv > 2) return ark_fail(h, ARK_M1_E_ARG, "op_recompute must be 0 (load M^-1), 1 (rebuild the diagonal block in the operator) or 2 (rebuild J as well)%s", ""); h->op_recompute = iv; }
     else if (!strcmp(key, "preconditioner")) { if (iv < 0 || iv > 1) return ark_fail(h, ARK_M1_E_ARG, "preconditioner must be 0 (block-Jacobi) or 1 (multigrid)%s", ""); h->precond = iv; }
@@ -571,15 +572,24 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
     const bool blk_ok = (h->precond == 0 && opk(h) == 1 && h->ortho == 1 && m <= 120);
     const bool pair = (h->arnoldi_block >= 2 && blk_ok && m >= 2);
     const int SB = (h->arnoldi_block >= 3 && blk_ok) ? h->arnoldi_block : 0;     // columns per s-step block (krylov_sstep.cu)
+    const bool pair2 = SB && h->op_pair && op_mf2_ok(h->g, h->mf);               // two operator applications per pass inside a block
     while (!h->ctl_host->inner_stop) {
         for (int j = 0; j < m; ++j) {
             double* w = h->V + (size_t)(j + 1) * S;
             if (SB && j + SB <= m) {
                 // s-step Arnoldi block (krylov_sstep.cu): W_1 = A^ v_j, W_k = (A^ - 1) W_{k-1} in the slots j+1 .. j+SB, one dot pass and one
                 // update pass over the basis for all SB vectors, in-block solve, Hessenberg columns recovered on the device
-                for (int k = 0; k < SB; ++k)
+                // (pairs of applications in one pass where the two-application kernel applies: operator_mf.cu, op_mf_rc2_kernel)
+                for (int k = 0; k < SB; ++k) {
+                    if (pair2 && k + 1 < SB) {
+                        KL(KC_SPMV, 160.0 * h->N, launch_op_mf2(h->g, h->mf, h->A.Minv, h->V + (size_t)(j + k) * S, h->V + (size_t)(j + k + 1) * S, h->V + (size_t)(j + k + 2) * S,
+                                                               k == 0 ? W.scale + j : nullptr, stop, sm, h->st, k == 0 ? 0.0 : 1.0, 1.0));
+                        ++k;
+                        continue;
+                    }
                     KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)(j + k) * S, h->V + (size_t)(j + k + 1) * S,
                                                                           k == 0 ? W.scale + j : nullptr, nullptr, 1.0, stop, 1, sm, h->st, k == 0 ? 0.0 : 1.0));
+                }
                 // the dot pass takes the block's own slots j+1 .. j+SB as basis vectors as well (W^T W, read from L1/L2): it predicts the
                 // in-block solve, the update pass applies it and checks the result (krylov_sstep.cu: sstep_predict)
                 const int nd = j + 1 + SB;
@@ -902,6 +912,37 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
     if (b_out) CU(cudaMemcpyAsync(b_out, h->A.b, n * sizeof(double), cudaMemcpyDefault, h->st));
     CU(cudaStreamSynchronize(h->st));
     return 0;
+}
+
+// out1 = A M^-1 V - theta1 V, out2 = A M^-1 out1 - theta2 out1: the two-application kernel of the s-step block where it applies
+// (matrix-free operator with J and the block rebuilt, periodic grid, option "op_pair" 1), else two single applications.
+// Returns 1 if the fused kernel ran, 0 if not.
+extern "C" int ark_m1_apply_operator_pair(ark_m1* h, double dt, const double* Vin, double* out1, double* out2, double theta1, double theta2)
+{
+    if (!h || !Vin || !out1 || !out2) return ARK_M1_E_ARG;
+    GUARD(h);
+    NO_SLAB(h, "ark_m1_apply_operator_pair");
+    if (!(dt > 0.0)) return ark_fail(h, ARK_M1_E_ARG, "apply_operator_pair: dt must be > 0%s", "");
+    if (!h->have_state) return ark_fail(h, ARK_M1_E_NOTSET, "apply_operator_pair: no state set%s", "");
+    if (opk(h) != 1) return ark_fail(h, ARK_M1_E_UNSUPPORTED, "apply_operator_pair: the matrix-free operator only (option operator = 1)%s", "");
+    int rc = ark_ensure_implicit(h, 1, 2);
+    if (rc) return rc;
+    const size_t n = 3 * (size_t)h->N;
+    if ((rc = ark_assemble_system(h, dt, nullptr))) return rc;
+    double* vin = h->V;
+    double* v1 = h->V + h->stride;
+    double* v2 = h->V + 2 * h->stride;
+    CU(cudaMemcpyAsync(vin, Vin, n * sizeof(double), cudaMemcpyDefault, h->st));
+    const int fused = h->op_pair && op_mf2_ok(h->g, h->mf);
+    if (fused) KL(KC_SPMV, 160.0 * h->N, launch_op_mf2(h->g, h->mf, h->A.Minv, vin, v1, v2, nullptr, nullptr, h->sm_count, h->st, theta1, theta2));
+    else {
+        KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, vin, v1, nullptr, nullptr, 1.0, nullptr, 1, h->sm_count, h->st, theta1));
+        KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, v1, v2, nullptr, nullptr, 1.0, nullptr, 1, h->sm_count, h->st, theta2));
+    }
+    CU(cudaMemcpyAsync(out1, v1, n * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(cudaMemcpyAsync(out2, v2, n * sizeof(double), cudaMemcpyDefault, h->st));
+    CU(cudaStreamSynchronize(h->st));
+    return fused;
 }
 
 // out = M^-1 V with the right preconditioner the solver would use for a step dt: the inverse 3x3 diagonal blocks

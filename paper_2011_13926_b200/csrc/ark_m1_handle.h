@@ -34,6 +34,7 @@ struct ark_m1 {
     // options
     int ortho, explicit_kernel, op_kind, maxv, krylov, asm_kernel;
     int arnoldi_block; // 2 (default): GMRES builds two Arnoldi columns per pass over the basis (gmres_solve); 1: one
+    int op_pair;       // 1 (default): inside an s-step block two operator applications go through ONE pass where the grid allows (op_mf_rc2_kernel)
     int apply_precond; // 1: ark_m1_apply_operator returns A M^-1 V through the solver's preconditioned matrix-free kernel (matrix-free operator only)
     int op_recompute;  // 1 (default): the matrix-free operator rebuilds the diagonal block instead of loading M^-1 (MfPlanes::rc)
     int basis_prec;    // 64, or 32: compressed-basis GMRES (krylov_cb.cu); applies to GMRES + block-Jacobi + matrix-free operator

@@ -122,6 +122,9 @@ cudaError_t launch_assemble_march(const Grid& g, const Scheme& s, const Fields& 
 cudaError_t launch_op_mf(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out,
                          const double* scale_ptr, const double* add, double sgn, const int* skip_flag, int precond,
                          int sm_count, cudaStream_t st, double theta = 0.0);
+bool op_mf2_ok(const Grid& g, const MfPlanes& mf);
+cudaError_t launch_op_mf2(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out1, double* out2,
+                          const double* scale_ptr, const int* skip_flag, int sm_count, cudaStream_t st, double th1, double th2);
 // (z, c^2 J z) of the slab's first and last row for the neighbour ranks (out_lo / out_hi: [6][nx], either may be null)
 cudaError_t launch_halo_pack_zp(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, int precond,
                                 double* out_lo, double* out_hi, const int* skip_flag, cudaStream_t st);

@@ -462,6 +462,234 @@ __global__ void __launch_bounds__(TXO, JRC ? OP_RCJ_MINB : OP_RC_MINB) op_mf_rc_
     if (DOT == 2) reduce_and_finish<2, TXO>(acc, W, BICG_OMEGA, 0);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// TWO applications in one pass: out1 = s A^ v - th1 v, out2 = A^ out1 - th2 out1 (A^ = A M^-1) — the matrix-powers kernel of the
+// s-step Arnoldi block (krylov_sstep.cu), which applies A^ five times in a row.  The rebuild of J and of the 3 x 3 block is ~130 of
+// the operator's ~200 fp64 instructions per cell and the coefficient planes are 88 of its 136 B: both are paid ONCE for the two
+// applications here (the inverse block is formed explicitly, adj(M) / det, and kept with J for one row step), 160 B per cell
+// per pair instead of 272.  The second application trails the first by one row: with row j+1 built, the first application emits
+// o1(j); z2(j) = M^-1(j) o1(j) and the second emits o2(j-1) from z2(j-2..j).  A strip is 28 columns (+2 halo lanes each side: o1 is
+// valid on lanes 1..30, o2 on 2..29) and a block marches rows j0-1 .. j1 for the first application (rows j0-1 and j1 belong to the
+// neighbours and are not stored).  Grids periodic on all four sides (every column and row has a plain diagonal block, ghosts wrap);
+// anything else takes two single applications.
+// ---------------------------------------------------------------------------------------------------------
+// 8 resident one-warp blocks per SM (two per sub-partition, 240 registers, no spills).  Measured on the bench solve at 4096^2 (58 operator
+// launches, 34 of them pairs, against 94 single applications at 49.2 ms): 8 blocks 38.1 ms; 12 blocks (168 registers, 216 B of spills)
+// 53.6; 16 blocks 60.0; the inverse block and J parked in shared memory between the two row steps (218 registers) 39.4; rows per
+// block 32 / 64 / 128: 39.4 / 38.1 / 37.9; a third ring stage 38.3.  A pair costs 0.75 ms against 2 x 0.52.
+static constexpr int OP2_MINB = 8;
+static constexpr int OP2_NST = 2;
+static constexpr int OP2_RY = 64;
+static constexpr int OP2_W = TXO - 4;
+
+__device__ __forceinline__ void build_inv(const FC& e, const FC& w, const FC& n, const FC& s, const JC& J, double dE, double dF,
+                                          double rx, double ry, double c2, double (&I)[9])
+{
+    const double lam = fma(rx, e.Lam + w.Lam, ry * (n.Lam + s.Lam));
+    const double m00 = (1.0 + dE) - fma(rx, fma(e.alpha, e.Lam, w.alpha * w.Lam), ry * fma(n.alpha, n.Lam, s.alpha * s.Lam));
+    const double m01 = rx * fma(e.alpha, e.ap, w.alpha * (w.ap - 1.0));
+    const double m02 = ry * fma(n.alpha, n.ap, s.alpha * (s.ap - 1.0));
+    const double ax = (c2 * rx) * ((e.ap + w.ap) - 1.0), ay = (c2 * ry) * ((n.ap + s.ap) - 1.0);
+    const double dd = (1.0 + dF) - lam;
+    const double m10 = fma(ax, J.xx0, ay * J.xy0), m11 = fma(ax, J.xx1, fma(ay, J.xy1, dd + (e.sw + w.sw))), m12 = fma(ax, J.xx2, ay * J.xy2);
+    const double m20 = fma(ax, J.xy0, ay * J.yy0), m21 = fma(ax, J.xy1, ay * J.yy1), m22 = fma(ax, J.xy2, fma(ay, J.yy2, dd + (n.sw + s.sw)));
+    const double c00 = m11 * m22 - m12 * m21, c01 = m12 * m20 - m10 * m22, c02 = m10 * m21 - m11 * m20;
+    const double id = rcp_fast(m00 * c00 + m01 * c01 + m02 * c02);
+    I[0] = c00 * id; I[1] = (m02 * m21 - m01 * m22) * id; I[2] = (m01 * m12 - m02 * m11) * id;
+    I[3] = c01 * id; I[4] = (m00 * m22 - m02 * m20) * id; I[5] = (m02 * m10 - m00 * m12) * id;
+    I[6] = c02 * id; I[7] = (m01 * m20 - m00 * m21) * id; I[8] = (m00 * m11 - m01 * m10) * id;
+}
+
+// z = I v, Pi = c^2 J z of one cell
+__device__ __forceinline__ void zp_from(const double (&I)[9], const JC& J, double c2, double v0, double v1, double v2, ZP& z)
+{
+    z.v0 = v0; z.v1 = v1; z.v2 = v2;
+    z.zE  = fma(I[0], v0, fma(I[1], v1, I[2] * v2));
+    z.zFx = fma(I[3], v0, fma(I[4], v1, I[5] * v2));
+    z.zFy = fma(I[6], v0, fma(I[7], v1, I[8] * v2));
+    z.Pxx = c2 * (J.xx0 * z.zE + J.xx1 * z.zFx + J.xx2 * z.zFy);
+    z.Pxy = c2 * (J.xy0 * z.zE + J.xy1 * z.zFx + J.xy2 * z.zFy);
+    z.Pyy = c2 * (J.yy0 * z.zE + J.yy1 * z.zFx + J.yy2 * z.zFy);
+}
+
+// one row of one application (rc_current_row without the fusions): o = s (A z)(row of S) - theta v, then the row ahead becomes S's row
+__device__ __forceinline__ void rc2_row(RcState& S, const ZP& zN, const FC& feN, const FC& fnN, double dEN, double dFN,
+                                        double rx, double ry, double sc, double theta, double& o0, double& o1, double& o2)
+{
+    const ZP& zC = S.zC;
+    double Ge0, Ge1, Ge2, Se;
+    {
+        const double RzE = __shfl_down_sync(0xffffffffu, zC.zE, 1), RzFx = __shfl_down_sync(0xffffffffu, zC.zFx, 1), RzFy = __shfl_down_sync(0xffffffffu, zC.zFy, 1);
+        const double RPxx = __shfl_down_sync(0xffffffffu, zC.Pxx, 1), RPxy = __shfl_down_sync(0xffffffffu, zC.Pxy, 1);
+        ARK_LIN_FLUX(S.fe, zC.zE, RzE, zC.zFx, RzFx, zC.zFy, RzFy, zC.Pxx, RPxx, zC.Pxy, RPxy, Ge0, Ge1, Ge2, Se);
+    }
+    const double Gw0 = __shfl_up_sync(0xffffffffu, Ge0, 1), Gw1 = __shfl_up_sync(0xffffffffu, Ge1, 1);
+    const double Gw2 = __shfl_up_sync(0xffffffffu, Ge2, 1), Sw = __shfl_up_sync(0xffffffffu, Se, 1);
+    double Hn0, Hn1, Hn2, Sn;
+    ARK_LIN_FLUX(S.fn, zC.zE, zN.zE, zC.zFy, zN.zFy, zC.zFx, zN.zFx, zC.Pyy, zN.Pyy, zC.Pxy, zN.Pxy, Hn0, Hn2, Hn1, Sn);
+    o0 = zC.zE  + fma(rx, Ge0 - Gw0, fma(ry, Hn0 - S.Hs0, S.dE * zC.zE));
+    o1 = zC.zFx + fma(rx, Ge1 - Gw1, fma(ry, Hn1 - S.Hs1, fma(S.dF, zC.zFx, Se + Sw)));
+    o2 = zC.zFy + fma(rx, Ge2 - Gw2, fma(ry, Hn2 - S.Hs2, fma(S.dF, zC.zFy, Sn + S.Ss)));
+    o0 = fma(-theta, zC.v0, sc * o0); o1 = fma(-theta, zC.v1, sc * o1); o2 = fma(-theta, zC.v2, sc * o2);
+    S.zC = zN;
+    S.Hs0 = Hn0; S.Hs1 = Hn1; S.Hs2 = Hn2; S.Ss = Sn;
+    S.fe = feN; S.fn = fnN; S.dE = dEN; S.dF = dFN;
+}
+
+__device__ __forceinline__ void rc2_issue(double (*ring)[TXO], double* ringw, int t, const MfPlanes& mf, const double* __restrict__ v,
+                                          long long N, long long idn, long long idw, bool want)
+{
+    if (want) {
+        cp_async8(&ring[0][t], mf.fxy + idn); cp_async8(&ring[1][t], mf.fxy + N + idn);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { cp_async8(&ring[2 + e][t], mf.fE + e * N + idn); cp_async8(&ring[6 + e][t], mf.fN + e * N + idn); }
+        cp_async8(&ring[10][t], mf.dE + idn);
+#pragma unroll
+        for (int e = 0; e < 3; ++e) cp_async8(&ring[11 + e][t], v + e * N + idn);
+        if (t == 0) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) cp_async8(&ringw[e], mf.fE + e * N + idw);
+        }
+    }
+    cp_async_commit();
+}
+
+__device__ __forceinline__ void load_jc(const double* __restrict__ Jp, long long N, long long id, JC& J)
+{
+    J.xx0 = Jp[0 * N + id]; J.xx1 = Jp[1 * N + id]; J.xx2 = Jp[2 * N + id];
+    J.xy0 = Jp[3 * N + id]; J.xy1 = Jp[4 * N + id]; J.xy2 = Jp[5 * N + id];
+    J.yy0 = Jp[6 * N + id]; J.yy1 = Jp[7 * N + id]; J.yy2 = Jp[8 * N + id];
+}
+
+__global__ void __launch_bounds__(TXO, OP2_MINB) op_mf_rc2_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const double* __restrict__ v,
+                                                                  double* __restrict__ out1, double* __restrict__ out2,
+                                                                  const double* __restrict__ scale_ptr, const int* __restrict__ skip_flag,
+                                                                  int RY, double rx, double ry, double c2, double th1, double th2)
+{
+    if (skip_flag && *skip_flag) return;
+    __shared__ double ring[OP2_NST][14][TXO];        // row-ahead number q lives in ring[q % OP2_NST]: (fx, fy), east face, north face, dE, v
+    __shared__ double ringw[OP2_NST][4];             // lane 0: the east face of the column west of the strip
+    const int t = threadIdx.x, nx = g.nx, ny = g.ny;
+    const int i = blockIdx.x * OP2_W - 2 + t;
+    const int ii = ((i % nx) + nx) % nx;
+    const int iw = (ii == 0) ? nx - 1 : ii - 1;
+    const int j0 = blockIdx.y * RY;
+    const int j1 = min(j0 + RY, ny);
+    const long long N = (long long)nx * ny;
+    const bool st_lane = (t >= 2 && t <= TXO - 3 && i >= 0 && i < nx);
+    const double sc = scale_ptr ? *scale_ptr : 1.0;
+    const bool has_dF = mf.has_dF != 0;
+    const double ic = 1.0 / g.c;
+    const int qlast = j1 + 1 - j0;                  // rows ahead j0 .. j1+1 (wrapped)
+#define ARK_WR(j) ((j) < 0 ? (j) + ny : ((j) >= ny ? (j) - ny : (j)))
+#pragma unroll
+    for (int r = 0; r < OP2_NST - 1; ++r) {
+        const int rr = ARK_WR(j0 + r);
+        rc2_issue(ring[r], ringw[r], t, mf, v, N, (long long)rr * nx + ii, (long long)rr * nx + iw, r <= qlast);
+    }
+
+    // first application: rows j0-2 (south of the first marched row) and j0-1 from the stored inverse
+    const int rS = ARK_WR(j0 - 2), rC = ARK_WR(j0 - 1);
+    const long long idC = (long long)rC * nx + ii;
+    RcState S1, S2;
+    {
+        const ZP zS = load_zp<true, double>(g, N, v, Minv, mf.J, c2, 0, ii, rS, nullptr, nullptr);
+        S1.zC = load_zp<true, double>(g, N, v, Minv, mf.J, c2, 0, ii, rC, nullptr, nullptr);
+        const FC fs = load_fc(mf.fN, N, (long long)rS * nx + ii);
+        ARK_LIN_FLUX(fs, zS.zE, S1.zC.zE, zS.zFy, S1.zC.zFy, zS.zFx, S1.zC.zFx, zS.Pyy, S1.zC.Pyy, zS.Pxy, S1.zC.Pxy, S1.Hs0, S1.Hs2, S1.Hs1, S1.Ss);
+    }
+    S1.fe = load_fc(mf.fE, N, idC);
+    S1.fn = load_fc(mf.fN, N, idC);
+    S1.dE = mf.dE[idC];
+    S1.dF = has_dF ? mf.dF[idC] : 0.0;
+    // inverse block and J of the current row of the first application (row j0-1: stored; afterwards handed over from the row ahead)
+    double IC[9];
+    JC Jc;
+#pragma unroll
+    for (int e = 0; e < 9; ++e) IC[e] = Minv[e * N + idC];
+    load_jc(mf.J, N, idC, Jc);
+    S2 = S1;       // (overwritten at q = 0)
+
+    for (int q = 0; q <= qlast; ++q) {
+        const int jm = j0 - 1 + q;
+        const int rn = ARK_WR(jm + 1);
+        {
+            const int qa = q + OP2_NST - 1, r2 = ARK_WR(j0 + qa);       // the slot read one step ago
+            rc2_issue(ring[qa % OP2_NST], ringw[qa % OP2_NST], t, mf, v, N, (long long)r2 * nx + ii, (long long)r2 * nx + iw, qa <= qlast);
+        }
+        cp_async_wait<OP2_NST - 1>();
+        double (*rg)[TXO] = ring[q % OP2_NST];
+        // ---- the row ahead: faces, J, inverse block, z1 = M^-1 v
+        const long long idn = (long long)rn * nx + ii;
+        FC feN, fnN, fwN;
+        feN.ap = rg[2][t]; feN.Lam = rg[3][t]; feN.alpha = rg[4][t]; feN.sw = rg[5][t];
+        fnN.ap = rg[6][t]; fnN.Lam = rg[7][t]; fnN.alpha = rg[8][t]; fnN.sw = rg[9][t];
+        const double dEN = rg[10][t];
+        const double dFN = has_dF ? mf.dF[idn] : 0.0;
+        fwN.ap = __shfl_up_sync(0xffffffffu, feN.ap, 1); fwN.Lam = __shfl_up_sync(0xffffffffu, feN.Lam, 1);
+        fwN.alpha = __shfl_up_sync(0xffffffffu, feN.alpha, 1); fwN.sw = __shfl_up_sync(0xffffffffu, feN.sw, 1);
+        if (t == 0) { const double* rw = ringw[q % OP2_NST]; fwN.ap = rw[0]; fwN.Lam = rw[1]; fwN.alpha = rw[2]; fwN.sw = rw[3]; }
+        JC Jn;
+        {
+            const double fx = rg[0][t], fy = rg[1][t];
+            if (fx > 2.0) load_jc(mf.J, N, idn, Jn);      // clamped cell: the stored J
+            else jac_from_f(fx, fy, ic, Jn);
+        }
+        double IN[9];
+        build_inv(feN, fwN, fnN, S1.fn, Jn, dEN, dFN, rx, ry, c2, IN);
+        ZP zN;
+        zp_from(IN, Jn, c2, rg[11][t], rg[12][t], rg[13][t], zN);
+        // ---- first application, row jm
+        const FC fe1 = S1.fe, fn1 = S1.fn;
+        const double dE1 = S1.dE, dF1 = S1.dF;
+        double o0, o1, o2;
+        rc2_row(S1, zN, feN, fnN, dEN, dFN, rx, ry, sc, th1, o0, o1, o2);
+        if (st_lane && q >= 1 && jm < j1) {
+            const long long id = (long long)jm * nx + i;
+            out1[id] = o0; out1[N + id] = o1; out1[2 * N + id] = o2;
+        }
+        // ---- second application: z2 of row jm, then row jm-1
+        ZP y;
+        zp_from(IC, Jc, c2, o0, o1, o2, y);
+        if (q >= 1) {
+            double p0, p1, p2;
+            rc2_row(S2, y, fe1, fn1, dE1, dF1, rx, ry, 1.0, th2, p0, p1, p2);
+            if (st_lane && q >= 2) {
+                const long long id = (long long)(jm - 1) * nx + i;
+                out2[id] = p0; out2[N + id] = p1; out2[2 * N + id] = p2;
+            }
+        } else {
+            S2.zC = y; S2.Hs0 = 0.0; S2.Hs1 = 0.0; S2.Hs2 = 0.0; S2.Ss = 0.0;
+            S2.fe = fe1; S2.fn = fn1; S2.dE = dE1; S2.dF = dF1;
+        }
+#pragma unroll
+        for (int e = 0; e < 9; ++e) IC[e] = IN[e];
+        Jc = Jn;
+    }
+    cp_async_wait<0>();
+#undef ARK_WR
+}
+
+bool op_mf2_ok(const Grid& g, const MfPlanes& mf)
+{
+    return mf.rc && mf.rcj && g.nx >= 4 && g.ny >= 4 && g.bc[XLO] == BC_PERIODIC && g.bc[XHI] == BC_PERIODIC
+           && g.bc[YLO] == BC_PERIODIC && g.bc[YHI] == BC_PERIODIC;
+}
+
+// out1 = s A M^-1 v - th1 v, out2 = A M^-1 out1 - th2 out1 in one pass (op_mf2_ok grids only)
+cudaError_t launch_op_mf2(const Grid& g, const MfPlanes& mf, const double* Minv, const double* v, double* out1, double* out2,
+                          const double* scale_ptr, const int* skip_flag, int sm_count, cudaStream_t st, double th1, double th2)
+{
+    if (!op_mf2_ok(g, mf)) return cudaErrorNotSupported;
+    const int strips = (g.nx + OP2_W - 1) / OP2_W;
+    long long want = ((long long)g.ny * strips + (long long)sm_count * 64 - 1) / ((long long)sm_count * 64);
+    int RY = (int)(want < 8 ? 8 : (want > OP2_RY ? OP2_RY : want));
+    if (RY > g.ny) RY = g.ny;
+    const dim3 grd(strips, (g.ny + RY - 1) / RY);
+    op_mf_rc2_kernel<<<grd, TXO, 0, st>>>(g, mf, Minv, v, out1, out2, scale_ptr, skip_flag, RY, mf.rx, mf.ry, g.c * g.c, th1, th2);
+    return cudaGetLastError();
+}
+
 static dim3 op_mf_grid(const Grid& g, int sm_count, int* RYout, int ry_cap = OP_RY)
 {
     const int strips = (g.nx + (TXO - 2) - 1) / (TXO - 2);
