@@ -244,7 +244,7 @@ def aggregate_over_ranks(elapsed_s, units, dist=None):
 ARNOLDI_BLOCK = 5      # the library's default (option arnoldi_block): columns per pass over the basis
 
 
-def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None):
+def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None, pair=None):
     """Algorithmic HBM bytes per cell of `iters` GMRES iterations with the kernels as built:
     operator 336 (block stencil) or 136 (matrix-free with the diagonal block and J rebuilt in the kernel, the default; 264 when it
     loads M^-1 and J).  Matrix-free default = s-step Arnoldi blocks of `block` = 5 columns per pass over the basis: per block at inner
@@ -255,9 +255,13 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None):
     chunk of 8 vectors, update 24 (j+1) + 96, the W2 - gamma W1 pass 72) or the one-column step (dots 24 (j+2), update+norm 24 (j+3), one
     extra read of w per 16-vector pass), which the block-stencil path uses throughout.  Per cycle: combine 8 (3 jj + 15) + true residual
     (block stencil: diag_mul 120 + spmv 360; matrix-free: 216) + norm 24.  A block is enqueued whole: its operator applications, dot
-    and update passes are paid even when the cycle stops after its first column."""
+    and update passes are paid even when the cycle stops after its first column.  `pair` (default: with the matrix-free operator; the
+    bench medium is periodic): inside a block two operator applications go through one pass (160 B per pair instead of 2 x 136:
+    coefficient planes read once, the intermediate vector written but not read back)."""
     if block is None:
         block = ARNOLDI_BLOCK if operator == 1 else 1
+    if pair is None:
+        pair = operator == 1
     op = 336.0 if operator == 0 else 136.0
     res = 480.0 if operator == 0 else 216.0
     total, done = 0.0, 0
@@ -266,7 +270,8 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None):
         j = 0
         while j < jj:
             if block >= 3 and j + block <= m:
-                total += block * op + 24.0 * (j + 1) + 24.0 * block * ((j + block) // 32 + 1) + 24.0 * (j + 1) + 48.0 * block
+                total += ((block // 2) * 160.0 + (block % 2) * op) if pair else block * op
+                total += 24.0 * (j + 1) + 24.0 * block * ((j + block) // 32 + 1) + 24.0 * (j + 1) + 48.0 * block
                 j += block
             elif block >= 2 and j + 1 < m:
                 chunks = j // 8 + 1
@@ -718,9 +723,10 @@ def run_ours(args):
                                   "frac": kern[dom]["hbm_frac"], "traffic": tr_bytes, "peak_source": peak_src,
                                   "share_of_step": kern[dom]["share"], "alg_bytes_per_launch": kern[dom]["alg_bytes_per_launch"],
                                   "traffic_note": tr.get("note"),
-                                  "pipes_note": (f"ncu of the same kernel: fp64 pipe {float(tr['fp64_pipe_busy_frac']):.2f}, issue slots {float(tr['issue_slots_busy_frac']):.2f} "
-                                                 "busy: the operator moves 136 instead of 264 B per cell by rebuilding J and the 3x3 diagonal block in registers and sits "
-                                                 "between the HBM roof and the issue roof (DESIGN.md section 5)") if tr.get("fp64_pipe_busy_frac") and dom == "spmv_hat" else None,
+                                  "pipes_note": (f"ncu of the kernel named in traffic_note: fp64 pipe {float(tr['fp64_pipe_busy_frac']):.2f}, issue slots "
+                                                 f"{float(tr['issue_slots_busy_frac']):.2f} busy: the operator rebuilds J and the 3x3 diagonal block in registers instead of "
+                                                 "loading them (136 instead of 264 B per cell; 160 B per PAIR of applications inside an s-step block) and sits between "
+                                                 "the HBM roof and the issue roof (DESIGN.md section 5)") if tr.get("fp64_pipe_busy_frac") and dom == "spmv_hat" else None,
                                   "frac_of_nominal": kern[dom]["achieved_gbs"] / 7700.0,
                                   "nominal_note": "the measured peak is a torch copy (6544 GB/s here); these kernels are read-dominated and exceed it, "
                                                   "so the fraction of the 7.7 TB/s HGX figure (B200_PROFILING.md) is given as well"}
@@ -846,7 +852,7 @@ def run_decomposed(args):
     t_exp_max, _ = aggregate_over_ranks(t_exp, 0.0, dist if world > 1 else None)
     if rank == 0:
         halo_per_step = (st1["halo_bytes"] - st0["halo_bytes"]) / args.steps
-        interior = iteration_bytes_per_cell(its, operator=1) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
+        interior = iteration_bytes_per_cell(its, operator=1, pair=False) * N / nslab_total + (64.0 + 288.0) * N / nslab_total
         line = {
             "metric": METRIC, "value": 2.0 * N * args.steps / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",

@@ -50,7 +50,9 @@ def test_iteration_byte_formula():
     assert bench.iteration_bytes_per_cell(1, operator=1, block=1) == 136 + 48 + 72 + 8 * 18 + 216 + 24
     # matrix-free default: blocks of five columns.  First block (j = 0) of a cycle that needs all five: five operator applications,
     # dots 24 (1 + 5), update 24 + 240 (the in-block solve rides on the update pass: predicted by the dot pass)
-    assert bench.iteration_bytes_per_cell(5, operator=1) == 5 * 136 + 144 + 264 + 8 * (15 + 15) + 216 + 24
+    assert bench.iteration_bytes_per_cell(5, operator=1, pair=False) == 5 * 136 + 144 + 264 + 8 * (15 + 15) + 216 + 24
+    # ... and two operator applications per pass inside the block (periodic grids): 2 x 160 + 136
+    assert bench.iteration_bytes_per_cell(5, operator=1) == 2 * 160 + 136 + 144 + 264 + 8 * (15 + 15) + 216 + 24
     # two columns per pass: two operator applications, dots 24 + 48, update 24 + 96, the W2 - gamma W1 pass 72
     assert bench.iteration_bytes_per_cell(2, operator=1, block=2) == 2 * 136 + 72 + 120 + 72 + 8 * (6 + 15) + 216 + 24
     assert bench.iteration_bytes_per_cell(60) == 2 * bench.iteration_bytes_per_cell(30)
