@@ -103,8 +103,9 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *   "arnoldi_block"     columns of the Arnoldi process built per pass over the basis (the iterates and the iteration count are
  *                          GMRES(m)'s in every case; the stop test and the iteration limit act per column):
  *                          5 (default), 4, 3: s-step blocks (W_1 = A M^-1 v_j, W_k = (A M^-1 - 1) W_{k-1}; one dot pass, one update
- *                             pass, Cholesky-based in-block solve with a second round for ill-conditioned blocks, Hessenberg columns
- *                             recovered on the device); columns a restart length leaves over use the two-column step
+ *                             pass, Cholesky-based in-block solve — predicted by the dot pass and applied by the update pass for
+ *                             well-conditioned blocks, a pass of its own with a second round for ill-conditioned ones —, Hessenberg
+ *                             columns recovered on the device); columns a restart length leaves over use the two-column step
  *                          2: two columns per pass     1: one
  *                          applies to GMRES + block-Jacobi + matrix-free operator + one-pass orthogonalisation, restart <= 120
  *   "op_recompute"      what the preconditioned matrix-free operator rebuilds in registers instead of loading it (same operator up
@@ -113,6 +114,9 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                             the nine M^-1 planes), and J itself from the cell's reduced flux (2 planes in place of 9):
  *                             136 B per cell per application; needs the default scheme and the marching assembly, else acts as 1
  *                          1: the diagonal block only: 192 B     0: nothing, M^-1 and J are loaded: 264 B
+ *   "op_pair"           1 (default): inside an s-step block two applications of the preconditioned operator go through ONE pass over
+ *                          the coefficient planes (160 instead of 2 x 136 B per cell) where the grid is periodic on all four sides
+ *                          and op_recompute = 2 is in effect; two passes everywhere else.  0: always two passes.  Same results.
  *   "apply_operator_precond"  1: ark_m1_apply_operator returns A M^-1 V through the solver's preconditioned kernel (matrix-free
  *                          operator only); 0 (default): A V
  *   "basis_precision"   64 (default) or 32: storage precision of the GMRES Arnoldi basis.  32 = compressed-basis GMRES: the basis
