@@ -672,6 +672,7 @@ __global__ void __launch_bounds__(TXO, OP2_MINB) op_mf_rc2_kernel(Grid g, MfPlan
 
 bool op_mf2_ok(const Grid& g, const MfPlanes& mf)
 {
+    if ((g.ny + OP2_RY - 1) / OP2_RY > 65535) return false;      // rows of blocks on gridDim.y
     return mf.rc && mf.rcj && g.nx >= 4 && g.ny >= 4 && g.bc[XLO] == BC_PERIODIC && g.bc[XHI] == BC_PERIODIC
            && g.bc[YLO] == BC_PERIODIC && g.bc[YHI] == BC_PERIODIC;
 }
