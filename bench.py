@@ -16,7 +16,9 @@ The JSON line also carries, each measured in the same run with CUDA events:
     roofline  : the dominant kernel class of the step (by device time), from per-launch CUDA events inside the timed region
     kernels   : the same for every kernel class
     e2e       : the same step through the C ABI with HOST (pinned) buffers: H2D of the 5 input planes and D2H of the 3
-                state planes inside the timed region
+                state planes of EVERY step inside the timed region, with the library's overlapped transfers (the next step's
+                upload and the last step's download run on the handle's copy stream beside the solve); `e2e.blocking` = the same
+                with ark_m1_set_state / ark_m1_get_state, copies and solve in series
     cpu_baseline : the oracle (oracle/oracle_m1.c, as it stands) on a bounded sample of the same workload
 Multi-GPU (torchrun): the path does not exchange data between GPUs (one-GPU north star): every rank runs an independent
 replica with its own seed, value = sum of units / max-over-ranks time ("scaling": "weak", no collective on the data path).
@@ -418,6 +420,7 @@ def run_ours(args):
     value = units / t_max
 
     # ---- e2e: same step through the C ABI with pinned HOST buffers -------------------------------------------------
+    # (a) blocking calls: upload, step, download in series (ark_m1_set_state / ark_m1_get_state)
     def e2e_step():
         g.set_state(host["E"], host["F"], host["sigma_a"], host["sigma_s"])
         one_step()
@@ -430,8 +433,31 @@ def run_ours(args):
         e2e_step()
     e1.record(stream)
     barrier()
-    t_e2e, u_e2e = aggregate_over_ranks(e0.elapsed_time(e1) * 1e-3, 2.0 * N * k_e2e, dist if world > 1 else None)
-    e2e = {"value": u_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": 5 * N * 8, "d2h_bytes_per_step": 3 * N * 8, "steps": k_e2e}
+    t_ser, u_ser = aggregate_over_ranks(e0.elapsed_time(e1) * 1e-3, 2.0 * N * k_e2e, dist if world > 1 else None)
+    # (b) the same loop with the library's overlapped transfers (csrc/pipeline.cu): every step's 5 input planes still come from the
+    # pinned host buffers and its 3 result planes still go back to them inside the timed region, but step k+1's upload and step k's
+    # download run on the handle's copy stream beside the solve.  The first upload and the last download are exposed and timed.
+    def e2e_pipelined(k):
+        g.prefetch_state(host["E"], host["F"], host["sigma_a"], host["sigma_s"])
+        for s_ in range(k):
+            g.commit_state()
+            if s_ + 1 < k:
+                g.prefetch_state(host["E"], host["F"], host["sigma_a"], host["sigma_s"])
+            one_step()
+            g.get_state_async((out_E, out_F))
+        g.wait_transfers()
+    e2e_pipelined(1)
+    barrier()
+    k_pipe = max(1, args.steps)
+    e0.record(stream)
+    e2e_pipelined(k_pipe)
+    e1.record(stream)
+    barrier()
+    t_e2e, u_e2e = aggregate_over_ranks(e0.elapsed_time(e1) * 1e-3, 2.0 * N * k_pipe, dist if world > 1 else None)
+    e2e = {"value": u_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": 5 * N * 8, "d2h_bytes_per_step": 3 * N * 8, "steps": k_pipe,
+           "api": "ark_m1_prefetch_state / commit_state / step_explicit / step_implicit / get_state_async / wait_transfers: the next step's upload and "
+                  "the last step's download overlap the solve; first upload and last download exposed",
+           "blocking": {"value": u_ser / t_ser, "steps": k_e2e, "api": "ark_m1_set_state / step_explicit / step_implicit / ark_m1_get_state, in series"}}
 
     line_extra = {}
     if rank == 0:

@@ -140,6 +140,27 @@ ARK_M1_API int ark_m1_set_field(ark_m1* h, const char* name, const double* plane
 /* Copy out E [nx*ny], F [2*nx*ny] and, if T != NULL and a temperature was set, T [nx*ny].  Synchronises. */
 ARK_M1_API int ark_m1_get_state(ark_m1* h, double* E, double* F, double* T);
 
+/* Overlapped transfers (csrc/pipeline.cu): the same set_state / get_state for a caller that steps one state after another from HOST
+ * buffers, with the upload of the NEXT state and the download of the LAST result on a copy stream of the handle's own, beside the
+ * solve that is running instead of in series with it.  Nothing of the method is computed here (PAPER.md:152-173, 263-272 are the
+ * steps in between); results are those of the blocking calls, bit for bit.
+ *   ark_m1_prefetch_state   starts copying E (nx*ny), F (2 planes), sigma_a, sigma_s (host — pinned for a real overlap — or device)
+ *                           into a staging buffer; returns at once; the arrays stay the library's until ark_m1_commit_state has
+ *                           been called AND (host arrays) ark_m1_wait_transfers or a synchronisation of the handle's stream after it.
+ *   ark_m1_commit_state     enqueues, on the handle's stream, "wait for that upload, then take the staged state" (= ark_m1_set_state
+ *                           with T = NULL: a radiation-only state; matter coupling uses ark_m1_set_state).  ARK_M1_E_NOTSET without
+ *                           a prefetch.  A new prefetch may be started right after it: it waits on the device for this commit.
+ *   ark_m1_get_state_async  snapshots the current state on the handle's stream (device copy) and copies the snapshot to E, F on the
+ *                           copy stream; returns at once; the handle's stream is free for the next step.  A second call waits on the
+ *                           device for the first download.  E, F are valid after ark_m1_wait_transfers.
+ *   ark_m1_wait_transfers   blocks the host until every copy started by the two calls above is done.
+ * Device memory: 8 planes (staging 5, snapshot 3), allocated at the first call, counted in ark_m1_device_bytes.  Not for slabs of an
+ * ark_m1_group (ARK_M1_E_UNSUPPORTED).  Calls on one handle must not overlap in time, as everywhere in this API. */
+ARK_M1_API int ark_m1_prefetch_state(ark_m1* h, const double* E, const double* F, const double* sigma_a, const double* sigma_s);
+ARK_M1_API int ark_m1_commit_state(ark_m1* h);
+ARK_M1_API int ark_m1_get_state_async(ark_m1* h, double* E, double* F);
+ARK_M1_API int ark_m1_wait_transfers(ark_m1* h);
+
 /* Explicit step (rows a1-a4 of the hot path): U^{n+1} = U^n - dt R(U^n), R = divergence of the AP HLL fluxes
  * (Eqs. 12-14, 25) minus the sources (WB Eqs. 18-19 and -c sigma_a E).  One fused
  * kernel; asynchronous (no host synchronisation).  dt <= 0: ARK_M1_E_ARG. */

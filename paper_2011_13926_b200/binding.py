@@ -21,7 +21,7 @@ XLO, XHI, YLO, YHI = 0, 1, 2, 3
 # every symbol include/ark_m1.h declares
 SYMBOLS = [
     "ark_m1_create", "ark_m1_destroy", "ark_m1_set_stream", "ark_m1_set_state", "ark_m1_set_boundary",
-    "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_step_explicit", "ark_m1_steps_explicit",
+    "ark_m1_set_option", "ark_m1_set_field", "ark_m1_get_state", "ark_m1_prefetch_state", "ark_m1_commit_state", "ark_m1_get_state_async", "ark_m1_wait_transfers", "ark_m1_step_explicit", "ark_m1_steps_explicit",
     "ark_m1_step_implicit", "ark_m1_step_implicit_newton", "ark_m1_step_semi_implicit", "ark_m1_add_velocity_sources", "ark_m1_count_unrealizable", "ark_m1_residual",
     "ark_m1_apply_operator", "ark_m1_get_history", "ark_m1_get_timings", "ark_m1_get_kernel_stats",
     "ark_m1_kernel_class_name", "ark_m1_kernel_launches", "ark_m1_block_stats", "ark_m1_fastmath_errors", "ark_m1_fp64_issue_rate", "ark_m1_apply_preconditioner", "ark_m1_apply_operator_pair", "ark_m1_device_bytes",
@@ -76,6 +76,10 @@ def load_library(path: str | None = None):
     L.ark_m1_set_option.argtypes = [vp, C.c_char_p, d]
     L.ark_m1_set_field.argtypes = [vp, C.c_char_p, dp]
     L.ark_m1_get_state.argtypes = [vp, dp, dp, dp]
+    L.ark_m1_prefetch_state.argtypes = [vp, dp, dp, dp, dp]
+    L.ark_m1_commit_state.argtypes = [vp]
+    L.ark_m1_get_state_async.argtypes = [vp, dp, dp]
+    L.ark_m1_wait_transfers.argtypes = [vp]
     L.ark_m1_step_explicit.argtypes = [vp, d]
     L.ark_m1_steps_explicit.argtypes = [vp, d, i]
     L.ark_m1_step_implicit.argtypes = [vp, d, d, i, i, C.POINTER(C.c_double)]
@@ -242,6 +246,27 @@ class ArkM1:
         pe, _ = _ptr(E, self.N); pf, _ = _ptr(F, 2 * self.N); pt, _ = _ptr(T, self.N)
         self._check(self._L.ark_m1_get_state(self._h, pe, pf, pt))
         return (E, F, T) if (with_T or (out is not None and len(out) > 2)) else (E, F)
+
+    # ---- overlapped transfers (csrc/pipeline.cu): the next state goes up and the last result comes down beside the running solve
+    def prefetch_state(self, E, F, sigma_a, sigma_s):
+        """Starts the upload of the NEXT state into a staging buffer on the handle's copy stream; returns at once."""
+        N = self.N
+        pe, k0 = _ptr(E, N); pf, k1 = _ptr(F, 2 * N); pa, k2 = _ptr(sigma_a, N); ps, k3 = _ptr(sigma_s, N)
+        self._check(self._L.ark_m1_prefetch_state(self._h, pe, pf, pa, ps))
+        self._keep_up = (k0, k1, k2, k3)
+
+    def commit_state(self):
+        """The handle's stream waits for the prefetched upload and takes the staged state (radiation-only: T unset)."""
+        self._check(self._L.ark_m1_commit_state(self._h))
+
+    def get_state_async(self, out):
+        """Snapshot of the current state copied to out = (E, F) on the copy stream; valid after wait_transfers()."""
+        pe, k0 = _ptr(out[0], self.N); pf, k1 = _ptr(out[1], 2 * self.N)
+        self._check(self._L.ark_m1_get_state_async(self._h, pe, pf))
+        self._keep_down = (k0, k1)
+
+    def wait_transfers(self):
+        self._check(self._L.ark_m1_wait_transfers(self._h))
 
     def step_explicit(self, dt):
         self._check(self._L.ark_m1_step_explicit(self._h, float(dt)))

@@ -12,7 +12,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libark_m1.so")
-SOURCES = ["ark_m1_api.cu", "explicit_kernels.cu", "explicit_march.cu", "explicit_march3.cu", "implicit_kernels.cu", "assemble_march.cu", "operator_mf.cu", "krylov_kernels.cu", "krylov_sstep.cu", "krylov_cb.cu", "multigrid.cu", "pipe_rates.cu", "dist.cu", "m1_3d.cu", "noalloc.cu"]
+SOURCES = ["ark_m1_api.cu", "explicit_kernels.cu", "explicit_march.cu", "explicit_march3.cu", "implicit_kernels.cu", "assemble_march.cu", "operator_mf.cu", "krylov_kernels.cu", "krylov_sstep.cu", "krylov_cb.cu", "multigrid.cu", "pipe_rates.cu", "dist.cu", "m1_3d.cu", "noalloc.cu", "pipeline.cu"]
 HEADERS = ["ark_m1_internal.h", "ark_m1_handle.h", "m1_device.cuh", "explicit_device.cuh", "krylov_device.cuh", "implicit_device.cuh", os.path.join("..", "..", "include", "ark_m1.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "--expt-relaxed-constexpr"]

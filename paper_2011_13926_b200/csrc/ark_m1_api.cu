@@ -170,6 +170,7 @@ void ark_m1_destroy(ark_m1* h)
     if (!h) return;
     GUARD(h);
     cudaStreamSynchronize(h->st);
+    ark_pipe_free(h);
     for (int k = 0; k < 2; ++k) { cudaFree(h->U[k]); cudaFree(h->T[k]); }
     cudaFree(h->sa); cudaFree(h->ss_tmp); cudaFree(h->stot); cudaFree(h->counts);
     for (int s = 0; s < 4; ++s) for (int k = 0; k < 5; ++k) cudaFree(h->gh[s][k]);

@@ -72,6 +72,7 @@ struct ark_m1 {
     double* halo_state[2];       // [5][nx]: row below (0) / above (1) the slab
     double* halo_zp[2];          // [6][nx]: (z, c^2 J z) of the same rows, refreshed before every operator application
     long long launches;          // kernels launched by this handle
+    void* pipe;                  // overlapped state transfers (pipeline.cu): copy stream, staging and snapshot buffers; null until first used
     char err[512];
 };
 
@@ -98,3 +99,4 @@ int ark_assemble_system(ark_m1* h, double dt, const double* bsrc);
 int ark_fetch_ctl(ark_m1* h);
 int ark_finish_implicit(ark_m1* h, double dt, double* final_residual);
 int ark_explicit_once(ark_m1* h, double dt);
+void ark_pipe_free(ark_m1* h);      // pipeline.cu
