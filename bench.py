@@ -277,7 +277,7 @@ def iteration_bytes_per_cell(iters, m=RESTART, operator=0, block=None, pair=None
                 j += block
             elif block >= 2 and j + 1 < m:
                 chunks = j // 8 + 1
-                total += 2.0 * op + 24.0 * (j + 1) + 48.0 * chunks + 24.0 * (j + 1) + 96.0 + (72.0 if j + 1 < jj else 0.0)
+                total += (160.0 if pair else 2.0 * op) + 24.0 * (j + 1) + 48.0 * chunks + 24.0 * (j + 1) + 96.0 + (72.0 if j + 1 < jj else 0.0)
                 j += 2
             else:
                 passes = j // 16 + 1

@@ -612,8 +612,12 @@ static int gmres_solve(ark_m1* h, double tol, int m, int maxit)
                 // two-column Arnoldi step: W1 = A M^-1 v_j, W2 = A M^-1 W1, both
                 // orthogonalised against v_0..v_j in the same passes over the basis, then W2 against W1'
                 double* w2 = h->V + (size_t)(j + 2) * S;
-                KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
-                KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, w, w2, nullptr, nullptr, 1.0, stop, 1, sm, h->st));
+                if (h->op_pair && op_mf2_ok(h->g, h->mf))      // both applications in one pass (operator_mf.cu, op_mf_rc2_kernel)
+                    KL(KC_SPMV, 160.0 * h->N, launch_op_mf2(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, w2, W.scale + j, stop, sm, h->st, 0.0, 0.0));
+                else {
+                    KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, h->V + (size_t)j * S, w, W.scale + j, nullptr, 1.0, stop, 1, sm, h->st));
+                    KL(KC_SPMV, (264.0 - mf_saved(h)) * h->N, launch_op_mf(h->g, h->mf, h->A.Minv, w, w2, nullptr, nullptr, 1.0, stop, 1, sm, h->st));
+                }
                 const int MV2 = krylov_pair_max_vectors();
                 const int nchunk2 = (j + MV2) / MV2, csize2 = (j + nchunk2) / nchunk2;
                 for (int c0 = 0; c0 <= j; c0 += csize2) {

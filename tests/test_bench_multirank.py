@@ -54,5 +54,6 @@ def test_iteration_byte_formula():
     # ... and two operator applications per pass inside the block (periodic grids): 2 x 160 + 136
     assert bench.iteration_bytes_per_cell(5, operator=1) == 2 * 160 + 136 + 144 + 264 + 8 * (15 + 15) + 216 + 24
     # two columns per pass: two operator applications, dots 24 + 48, update 24 + 96, the W2 - gamma W1 pass 72
-    assert bench.iteration_bytes_per_cell(2, operator=1, block=2) == 2 * 136 + 72 + 120 + 72 + 8 * (6 + 15) + 216 + 24
+    assert bench.iteration_bytes_per_cell(2, operator=1, block=2, pair=False) == 2 * 136 + 72 + 120 + 72 + 8 * (6 + 15) + 216 + 24
+    assert bench.iteration_bytes_per_cell(2, operator=1, block=2) == 160 + 72 + 120 + 72 + 8 * (6 + 15) + 216 + 24
     assert bench.iteration_bytes_per_cell(60) == 2 * bench.iteration_bytes_per_cell(30)
