@@ -115,8 +115,9 @@ ARK_M1_API int ark_m1_set_boundary(ark_m1* h, int side, const double* E_g, const
  *                             136 B per cell per application; needs the default scheme and the marching assembly, else acts as 1
  *                          1: the diagonal block only: 192 B     0: nothing, M^-1 and J are loaded: 264 B
  *   "op_pair"           1 (default): inside an s-step block two applications of the preconditioned operator go through ONE pass over
- *                          the coefficient planes (160 instead of 2 x 136 B per cell) where the grid is periodic on all four sides
- *                          and op_recompute = 2 is in effect; two passes everywhere else.  0: always two passes.  Same results.
+ *                          the coefficient planes (160 instead of 2 x 136 B per cell) where op_recompute = 2 is in effect (default
+ *                          scheme) and the grid is at least 4 x 4 and not a slab of a decomposed grid; two passes otherwise.
+ *                          0: always two passes.  Same results.
  *   "apply_operator_precond"  1: ark_m1_apply_operator returns A M^-1 V through the solver's preconditioned kernel (matrix-free
  *                          operator only); 0 (default): A V
  *   "basis_precision"   64 (default) or 32: storage precision of the GMRES Arnoldi basis.  32 = compressed-basis GMRES: the basis
@@ -218,8 +219,8 @@ ARK_M1_API int ark_m1_apply_preconditioner(ark_m1* h, double dt, const double* V
 /* Two applications of the preconditioned operator in a row, as the s-step Arnoldi block issues them (DESIGN.md "Two applications
  * per pass"): out1 = A M^-1 V - theta1 V, out2 = A M^-1 out1 - theta2 out1 for the linearisation of a step dt at the current
  * state (A = I + dt L_n; M = its 3x3 block diagonal).  V, out1, out2: 3 planes of nx*ny doubles
- * each (E, Fx, Fy), host or device.  With option "op_pair" = 1 (default) on a grid periodic on all four sides and the default
- * matrix-free operator (op_recompute = 2) both come from ONE pass over the coefficient planes; otherwise from two passes.
+ * each (E, Fx, Fy), host or device.  With option "op_pair" = 1 (default), the default matrix-free operator (op_recompute = 2) and a
+ * grid of at least 4 x 4 cells (any boundary kinds) both come from ONE pass over the coefficient planes; otherwise from two passes.
  * Returns 1 if the one-pass kernel ran, 0 if two passes did, < 0 on error (ARK_M1_E_UNSUPPORTED with option operator = 0).
  * Synchronises the handle's stream. */
 ARK_M1_API int ark_m1_apply_operator_pair(ark_m1* h, double dt, const double* V, double* out1, double* out2, double theta1, double theta2);

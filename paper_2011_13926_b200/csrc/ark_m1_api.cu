@@ -920,7 +920,7 @@ extern "C" int ark_m1_apply_operator(ark_m1* h, double dt, const double* Vin, do
 }
 
 // out1 = A M^-1 V - theta1 V, out2 = A M^-1 out1 - theta2 out1: the two-application kernel of the s-step block where it applies
-// (matrix-free operator with J and the block rebuilt, periodic grid, option "op_pair" 1), else two single applications.
+// (matrix-free operator with J and the block rebuilt, grid of at least 4 x 4 cells, option "op_pair" 1), else two single applications.
 // Returns 1 if the fused kernel ran, 0 if not.
 extern "C" int ark_m1_apply_operator_pair(ark_m1* h, double dt, const double* Vin, double* out1, double* out2, double theta1, double theta2)
 {

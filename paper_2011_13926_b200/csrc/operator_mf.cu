@@ -470,8 +470,9 @@ __global__ void __launch_bounds__(TXO, JRC ? OP_RCJ_MINB : OP_RC_MINB) op_mf_rc_
 // per pair instead of 272.  The second application trails the first by one row: with row j+1 built, the first application emits
 // o1(j); z2(j) = M^-1(j) o1(j) and the second emits o2(j-1) from z2(j-2..j).  A strip is 28 columns (+2 halo lanes each side: o1 is
 // valid on lanes 1..30, o2 on 2..29) and a block marches rows j0-1 .. j1 for the first application (rows j0-1 and j1 belong to the
-// neighbours and are not stored).  Grids periodic on all four sides (every column and row has a plain diagonal block, ghosts wrap);
-// anything else takes two single applications.
+// neighbours and are not stored).  rc2_body is the code for blocks that see real rows and columns only (every block of a grid
+// periodic on all four sides: every column and row has a plain diagonal block, ghosts wrap); blocks that touch a Dirichlet or
+// outflow side run rc2g_body further down; halo rows of a slab, op_recompute < 2 and grids under 4 x 4 take two single applications.
 // ---------------------------------------------------------------------------------------------------------
 // 8 resident one-warp blocks per SM (two per sub-partition, 240 registers, no spills).  Measured on the bench solve at 4096^2 (58 operator
 // launches, 34 of them pairs, against 94 single applications at 49.2 ms): 8 blocks 38.1 ms; 12 blocks (168 registers, 216 B of spills)
@@ -561,12 +562,18 @@ __device__ __forceinline__ void load_jc(const double* __restrict__ Jp, long long
     J.yy0 = Jp[6 * N + id]; J.yy1 = Jp[7 * N + id]; J.yy2 = Jp[8 * N + id];
 }
 
-__global__ void __launch_bounds__(TXO, OP2_MINB) op_mf_rc2_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const double* __restrict__ v,
-                                                                  double* __restrict__ out1, double* __restrict__ out2,
-                                                                  const double* __restrict__ scale_ptr, const int* __restrict__ skip_flag,
-                                                                  int RY, double rx, double ry, double c2, double th1, double th2)
+// Grids with Dirichlet or outflow sides: blocks that touch a boundary (first strip, last two strips — the last but one can hold the ghost
+// lane of column nx —, first block row, last two block rows) go through op_mf_rc2g_kernel below; every other block sees real rows and
+// columns only and runs this kernel's periodic code unchanged (0.75 against 0.99 ms per pair at 4096^2 for the general code).
+__device__ __forceinline__ bool op2_edge_block(const Grid& g, int bx, int by, int SX, int SY)
 {
-    if (skip_flag && *skip_flag) return;
+    return (g.bc[YLO] != BC_PERIODIC && (by == 0 || by >= SY - 2)) || (g.bc[XLO] != BC_PERIODIC && (bx == 0 || bx >= SX - 2));
+}
+
+__device__ __forceinline__ void rc2_body(const Grid& g, const MfPlanes& mf, const double* __restrict__ Minv, const double* __restrict__ v,
+                                         double* __restrict__ out1, double* __restrict__ out2, const double* __restrict__ scale_ptr,
+                                         int RY, double rx, double ry, double c2, double th1, double th2)
+{
     __shared__ double ring[OP2_NST][14][TXO];        // row-ahead number q lives in ring[q % OP2_NST]: (fx, fy), east face, north face, dE, v
     __shared__ double ringw[OP2_NST][4];             // lane 0: the east face of the column west of the strip
     const int t = threadIdx.x, nx = g.nx, ny = g.ny;
@@ -670,11 +677,216 @@ __global__ void __launch_bounds__(TXO, OP2_MINB) op_mf_rc2_kernel(Grid g, MfPlan
 #undef ARK_WR
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// The two-application kernel for grids with Dirichlet or outflow sides (any mix with periodic ones).  Same march; what the
+// boundaries add:
+//   columns  ghost lanes (i = -1, nx) carry z = 0 (Dirichlet) or a copy of the adjacent lane's (z, Pi) (outflow) in BOTH applications
+//            (their own o1 is not a stencil result); the copy is a shuffle, done in the two edge strips only.  The west face of
+//            column 0 is the boundary face of mf.xlo.  An outflow boundary column holds a folded neighbour in its diagonal block:
+//            its inverse block and J come from the stored planes (as in the one-application kernel), for both applications.
+//   rows     a block that starts at row 0 marches the first application from row 0 (ghost row -1 = 0 or a copy of row 0, south face
+//            from mf.ylo) and starts the second with the ghost of ITS vector: z2(-1) = 0 or z2(0).  A block that ends at row ny-1
+//            takes the ghost row ny as the row ahead of the first application, and one more step of the second with z2(ny) = 0 or
+//            z2(ny-1).  An outflow top row uses the stored inverse.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void zp_zero(ZP& z)
+{
+    z.zE = 0.0; z.zFx = 0.0; z.zFy = 0.0; z.Pxx = 0.0; z.Pxy = 0.0; z.Pyy = 0.0; z.v0 = 0.0; z.v1 = 0.0; z.v2 = 0.0;
+}
+
+// lane kinds: 0 cell, 1 cell with a folded diagonal block, 2 zero ghost / inactive, 3 copy of lane t+1, 4 copy of lane t-1
+__device__ __forceinline__ void fix_ghost(ZP& z, int kind)
+{
+    ZP a, b;
+    a.zE = __shfl_down_sync(0xffffffffu, z.zE, 1); a.zFx = __shfl_down_sync(0xffffffffu, z.zFx, 1); a.zFy = __shfl_down_sync(0xffffffffu, z.zFy, 1);
+    a.Pxx = __shfl_down_sync(0xffffffffu, z.Pxx, 1); a.Pxy = __shfl_down_sync(0xffffffffu, z.Pxy, 1); a.Pyy = __shfl_down_sync(0xffffffffu, z.Pyy, 1);
+    b.zE = __shfl_up_sync(0xffffffffu, z.zE, 1); b.zFx = __shfl_up_sync(0xffffffffu, z.zFx, 1); b.zFy = __shfl_up_sync(0xffffffffu, z.zFy, 1);
+    b.Pxx = __shfl_up_sync(0xffffffffu, z.Pxx, 1); b.Pxy = __shfl_up_sync(0xffffffffu, z.Pxy, 1); b.Pyy = __shfl_up_sync(0xffffffffu, z.Pyy, 1);
+    if (kind == 2) zp_zero(z);
+    else if (kind == 3) { z.zE = a.zE; z.zFx = a.zFx; z.zFy = a.zFy; z.Pxx = a.Pxx; z.Pxy = a.Pxy; z.Pyy = a.Pyy; }
+    else if (kind == 4) { z.zE = b.zE; z.zFx = b.zFx; z.zFy = b.zFy; z.Pxx = b.Pxx; z.Pxy = b.Pxy; z.Pyy = b.Pyy; }
+}
+
+#define ARK_YFLUX(fc, zL, zR, H0, H1, H2, Sv) \
+    ARK_LIN_FLUX(fc, (zL).zE, (zR).zE, (zL).zFy, (zR).zFy, (zL).zFx, (zR).zFx, (zL).Pyy, (zR).Pyy, (zL).Pxy, (zR).Pxy, H0, H2, H1, Sv)
+
+__device__ __forceinline__ void rc2g_body(const Grid& g, const MfPlanes& mf, const double* __restrict__ Minv, const double* __restrict__ v,
+                                          double* __restrict__ out1, double* __restrict__ out2, const double* __restrict__ scale_ptr,
+                                          int RY, double rx, double ry, double c2, double th1, double th2)
+{
+    __shared__ double ring[OP2_NST][14][TXO];
+    __shared__ double ringw[OP2_NST][4];
+    const int t = threadIdx.x, nx = g.nx, ny = g.ny;
+    const int i = blockIdx.x * OP2_W - 2 + t;
+    const bool perx = g.bc[XLO] == BC_PERIODIC, pery = g.bc[YLO] == BC_PERIODIC;
+    int ii, kind;
+    if (perx) { ii = ((i % nx) + nx) % nx; kind = 0; }
+    else if (i >= 0 && i < nx) { ii = i; kind = ((i == 0 && g.bc[XLO] == BC_OUTFLOW) || (i == nx - 1 && g.bc[XHI] == BC_OUTFLOW)) ? 1 : 0; }
+    else if (i == -1) { ii = 0; kind = (g.bc[XLO] == BC_DIRICHLET) ? 2 : 3; }
+    else if (i == nx) { ii = nx - 1; kind = (g.bc[XHI] == BC_DIRICHLET) ? 2 : 4; }
+    else { ii = (i < 0) ? 0 : nx - 1; kind = 2; }
+    const bool edge = __any_sync(0xffffffffu, kind >= 2);          // (warp-uniform) this strip holds ghost lanes
+    const bool lghost = (!perx && i == -1);                        // its east face is the boundary face of mf.xlo
+    const int iw = (ii == 0) ? (perx ? nx - 1 : 0) : ii - 1;       // column of lane 0's west face (lane 0 is never column 0 of a non-periodic grid)
+    const int lxm = (kind <= 1) ? 0 : 1;
+    const int j0 = blockIdx.y * RY;
+    const int j1 = min(j0 + RY, ny);
+    const long long N = (long long)nx * ny;
+    const bool st_lane = (t >= 2 && t <= TXO - 3 && i >= 0 && i < nx);
+    const double sc = scale_ptr ? *scale_ptr : 1.0;
+    const bool has_dF = mf.has_dF != 0;
+    const double ic = 1.0 / g.c;
+    const int jmA = pery ? j0 - 1 : (j0 > 0 ? j0 - 1 : 0);         // rows marched by the first application: jmA .. jmB
+    const int jmB = pery ? j1 : (j1 < ny ? j1 : ny - 1);
+    const int nsteps = jmB - jmA + 1;
+#define ARK_WR(j) ((j) < 0 ? (j) + ny : ((j) >= ny ? (j) - ny : (j)))
+#define ARK_REAL(j) (pery || ((j) >= 0 && (j) < ny))
+#pragma unroll
+    for (int r = 0; r < OP2_NST - 1; ++r) {
+        const int jr = jmA + 1 + r, rr = ARK_WR(jr);
+        rc2_issue(ring[r], ringw[r], t, mf, v, N, (long long)rr * nx + ii, (long long)rr * nx + iw, r < nsteps && ARK_REAL(jr));
+    }
+
+    // ---- prologue of the first application: the row south of the first marched row, and that row, from the stored inverse
+    RcState S1, S2;
+    const int rA = ARK_WR(jmA);
+    const long long idA = (long long)rA * nx + ii;
+    {
+        // (a ghost row -1 is resolved by load_zp: zero, or the copy of row 0)
+        ZP zS = load_zp<true, double>(g, N, v, Minv, mf.J, c2, lxm, ii, pery ? ARK_WR(jmA - 1) : jmA - 1, nullptr, nullptr);
+        S1.zC = load_zp<true, double>(g, N, v, Minv, mf.J, c2, lxm, ii, rA, nullptr, nullptr);
+        if (edge) { fix_ghost(zS, kind); fix_ghost(S1.zC, kind); }
+        const FC fs = (pery || jmA > 0) ? load_fc(mf.fN, N, (long long)ARK_WR(jmA - 1) * nx + ii) : load_fc(mf.ylo, nx, ii);
+        ARK_YFLUX(fs, zS, S1.zC, S1.Hs0, S1.Hs1, S1.Hs2, S1.Ss);
+    }
+    S1.fe = lghost ? load_fc(mf.xlo, ny, rA) : load_fc(mf.fE, N, idA);
+    S1.fn = load_fc(mf.fN, N, idA);
+    S1.dE = mf.dE[idA];
+    S1.dF = has_dF ? mf.dF[idA] : 0.0;
+    double IC[9];
+    JC Jc;
+#pragma unroll
+    for (int e = 0; e < 9; ++e) IC[e] = Minv[e * N + idA];
+    load_jc(mf.J, N, idA, Jc);
+    S2 = S1;       // (overwritten at q = 0)
+    FC fdef; fdef.ap = 0.5; fdef.Lam = 0.0; fdef.alpha = 1.0; fdef.sw = 0.0;
+
+    for (int q = 0; q < nsteps; ++q) {
+        const int jm = jmA + q, jn = jm + 1;
+        const bool real_n = ARK_REAL(jn);                            // (block-uniform) false: the row ahead is the ghost row ny
+        {
+            const int qa = q + OP2_NST - 1, j2 = jmA + 1 + qa, r2 = ARK_WR(j2);
+            rc2_issue(ring[qa % OP2_NST], ringw[qa % OP2_NST], t, mf, v, N, (long long)r2 * nx + ii, (long long)r2 * nx + iw, qa < nsteps && ARK_REAL(j2));
+        }
+        cp_async_wait<OP2_NST - 1>();
+        double (*rg)[TXO] = ring[q % OP2_NST];
+        FC feN = fdef, fnN = fdef;
+        double dEN = 0.0, dFN = 0.0;
+        double IN[9];
+        JC Jn;
+        ZP zN;
+        if (real_n) {
+            const int rn = ARK_WR(jn);
+            const long long idn = (long long)rn * nx + ii;
+            feN.ap = rg[2][t]; feN.Lam = rg[3][t]; feN.alpha = rg[4][t]; feN.sw = rg[5][t];
+            fnN.ap = rg[6][t]; fnN.Lam = rg[7][t]; fnN.alpha = rg[8][t]; fnN.sw = rg[9][t];
+            dEN = rg[10][t];
+            if (has_dF) dFN = mf.dF[idn];
+            if (lghost) feN = load_fc(mf.xlo, ny, rn);
+            FC fwN;
+            fwN.ap = __shfl_up_sync(0xffffffffu, feN.ap, 1); fwN.Lam = __shfl_up_sync(0xffffffffu, feN.Lam, 1);
+            fwN.alpha = __shfl_up_sync(0xffffffffu, feN.alpha, 1); fwN.sw = __shfl_up_sync(0xffffffffu, feN.sw, 1);
+            if (t == 0) { const double* rw = ringw[q % OP2_NST]; fwN.ap = rw[0]; fwN.Lam = rw[1]; fwN.alpha = rw[2]; fwN.sw = rw[3]; }
+            // a diagonal block that holds a folded neighbour (outflow column or outflow top row): the stored inverse and J
+            const bool folded = (kind == 1) || (!pery && jn == ny - 1 && g.bc[YHI] == BC_OUTFLOW);
+            if (folded) {
+#pragma unroll
+                for (int e = 0; e < 9; ++e) IN[e] = Minv[e * N + idn];
+                load_jc(mf.J, N, idn, Jn);
+            } else {
+                const double fx = rg[0][t], fy = rg[1][t];
+                if (fx > 2.0) load_jc(mf.J, N, idn, Jn);      // clamped cell: the stored J
+                else jac_from_f(fx, fy, ic, Jn);
+                build_inv(feN, fwN, fnN, S1.fn, Jn, dEN, dFN, rx, ry, c2, IN);
+            }
+            zp_from(IN, Jn, c2, rg[11][t], rg[12][t], rg[13][t], zN);
+            if (edge) fix_ghost(zN, kind);
+        } else {
+            if (g.bc[YHI] == BC_DIRICHLET) zp_zero(zN); else zN = S1.zC;
+#pragma unroll
+            for (int e = 0; e < 9; ++e) IN[e] = 0.0;
+            Jn = Jc;
+        }
+        // ---- first application, row jm
+        const FC fe1 = S1.fe, fn1 = S1.fn;
+        const double dE1 = S1.dE, dF1 = S1.dF;
+        double o0, o1, o2;
+        rc2_row(S1, zN, feN, fnN, dEN, dFN, rx, ry, sc, th1, o0, o1, o2);
+        if (st_lane && jm >= j0 && jm < j1) {
+            const long long id = (long long)jm * nx + i;
+            out1[id] = o0; out1[N + id] = o1; out1[2 * N + id] = o2;
+        }
+        // ---- second application: z2 of row jm, then row jm-1
+        ZP y;
+        zp_from(IC, Jc, c2, o0, o1, o2, y);
+        if (edge) fix_ghost(y, kind);
+        if (q == 0) {
+            S2.zC = y; S2.Hs0 = 0.0; S2.Hs1 = 0.0; S2.Hs2 = 0.0; S2.Ss = 0.0;
+            S2.fe = fe1; S2.fn = fn1; S2.dE = dE1; S2.dF = dF1;
+            if (jmA == j0) {       // (block-uniform) row 0 of a non-periodic grid: the ghost row of the second application's vector
+                ZP yg;
+                if (g.bc[YLO] == BC_DIRICHLET) zp_zero(yg); else yg = y;
+                const FC fs2 = load_fc(mf.ylo, nx, ii);
+                ARK_YFLUX(fs2, yg, y, S2.Hs0, S2.Hs1, S2.Hs2, S2.Ss);
+            }
+        } else {
+            double p0, p1, p2;
+            rc2_row(S2, y, fe1, fn1, dE1, dF1, rx, ry, 1.0, th2, p0, p1, p2);
+            if (st_lane && jm - 1 >= j0) {
+                const long long id = (long long)(jm - 1) * nx + i;
+                out2[id] = p0; out2[N + id] = p1; out2[2 * N + id] = p2;
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < 9; ++e) IC[e] = IN[e];
+        Jc = Jn;
+    }
+    cp_async_wait<0>();
+    if (!pery && j1 == ny) {       // (block-uniform) the last row of the second application: its row ahead is the ghost row ny
+        ZP yg;
+        if (g.bc[YHI] == BC_DIRICHLET) zp_zero(yg); else yg = S2.zC;
+        double p0, p1, p2;
+        rc2_row(S2, yg, fdef, fdef, 0.0, 0.0, rx, ry, 1.0, th2, p0, p1, p2);
+        if (st_lane) {
+            const long long id = (long long)(ny - 1) * nx + i;
+            out2[id] = p0; out2[N + id] = p1; out2[2 * N + id] = p2;
+        }
+    }
+#undef ARK_WR
+#undef ARK_REAL
+}
+
+// MODE 0: every block runs the periodic code (grids periodic on all four sides).  1: boundary blocks run the general code, the
+// others the periodic code, in ONE grid (as two launches the handful of boundary blocks were a 0.15 ms tail per pair).  2: every
+// block runs the general code (grids too small to have interior blocks).
+template <int MODE>
+__global__ void __launch_bounds__(TXO, OP2_MINB) op_mf_rc2_kernel(Grid g, MfPlanes mf, const double* __restrict__ Minv, const double* __restrict__ v,
+                                                                  double* __restrict__ out1, double* __restrict__ out2,
+                                                                  const double* __restrict__ scale_ptr, const int* __restrict__ skip_flag,
+                                                                  int RY, double rx, double ry, double c2, double th1, double th2)
+{
+    if (skip_flag && *skip_flag) return;
+    if (MODE == 0) rc2_body(g, mf, Minv, v, out1, out2, scale_ptr, RY, rx, ry, c2, th1, th2);
+    else if (MODE == 2) rc2g_body(g, mf, Minv, v, out1, out2, scale_ptr, RY, rx, ry, c2, th1, th2);
+    else if (op2_edge_block(g, blockIdx.x, blockIdx.y, gridDim.x, gridDim.y)) rc2g_body(g, mf, Minv, v, out1, out2, scale_ptr, RY, rx, ry, c2, th1, th2);
+    else rc2_body(g, mf, Minv, v, out1, out2, scale_ptr, RY, rx, ry, c2, th1, th2);
+}
+
 bool op_mf2_ok(const Grid& g, const MfPlanes& mf)
 {
     if ((g.ny + OP2_RY - 1) / OP2_RY > 65535) return false;      // rows of blocks on gridDim.y
-    return mf.rc && mf.rcj && g.nx >= 4 && g.ny >= 4 && g.bc[XLO] == BC_PERIODIC && g.bc[XHI] == BC_PERIODIC
-           && g.bc[YLO] == BC_PERIODIC && g.bc[YHI] == BC_PERIODIC;
+    for (int s = 0; s < 4; ++s) if (g.bc[s] != BC_PERIODIC && g.bc[s] != BC_DIRICHLET && g.bc[s] != BC_OUTFLOW) return false;      // (halo rows of a slab)
+    return mf.rc && mf.rcj && g.nx >= 4 && g.ny >= 4;
 }
 
 // out1 = s A M^-1 v - th1 v, out2 = A M^-1 out1 - th2 out1 in one pass (op_mf2_ok grids only)
@@ -687,7 +899,11 @@ cudaError_t launch_op_mf2(const Grid& g, const MfPlanes& mf, const double* Minv,
     int RY = (int)(want < 8 ? 8 : (want > OP2_RY ? OP2_RY : want));
     if (RY > g.ny) RY = g.ny;
     const dim3 grd(strips, (g.ny + RY - 1) / RY);
-    op_mf_rc2_kernel<<<grd, TXO, 0, st>>>(g, mf, Minv, v, out1, out2, scale_ptr, skip_flag, RY, mf.rx, mf.ry, g.c * g.c, th1, th2);
+    const bool periodic = g.bc[XLO] == BC_PERIODIC && g.bc[XHI] == BC_PERIODIC && g.bc[YLO] == BC_PERIODIC && g.bc[YHI] == BC_PERIODIC;
+    const bool interior = (g.bc[XLO] == BC_PERIODIC || grd.x >= 4) && (g.bc[YLO] == BC_PERIODIC || grd.y >= 4);      // the grid has blocks that touch no boundary
+    if (periodic) op_mf_rc2_kernel<0><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out1, out2, scale_ptr, skip_flag, RY, mf.rx, mf.ry, g.c * g.c, th1, th2);
+    else if (interior) op_mf_rc2_kernel<1><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out1, out2, scale_ptr, skip_flag, RY, mf.rx, mf.ry, g.c * g.c, th1, th2);
+    else op_mf_rc2_kernel<2><<<grd, TXO, 0, st>>>(g, mf, Minv, v, out1, out2, scale_ptr, skip_flag, RY, mf.rx, mf.ry, g.c * g.c, th1, th2);
     return cudaGetLastError();
 }
 

@@ -1,5 +1,5 @@
 """GPU check of the two-application operator kernel (csrc/operator_mf.cu op_mf_rc2_kernel, option op_pair = 1, the default inside the
-s-step Arnoldi block on grids periodic on all four sides): out1 = A M^-1 v - theta1 v and out2 = A M^-1 out1 - theta2 out1 from
+s-step Arnoldi block; op_mf_rc2g_kernel on grids with Dirichlet or outflow sides): out1 = A M^-1 v - theta1 v and out2 = A M^-1 out1 - theta2 out1 from
 ONE pass over the coefficient planes, against the same two results from two passes of the single-application kernel (itself checked
 against apply_operator(apply_preconditioner(v)) in test_gpu_operator_recompute.py and through it against the oracle) and against the
 two-step reference built from the un-preconditioned operator and the stored inverse blocks.
@@ -72,15 +72,30 @@ def test_pair_kernel_with_clamped_and_nonpositive_cells():
     _check(w, K=5.0)
 
 
-@pytest.mark.parametrize("bc", [(1, 1, 0, 0), (0, 0, 2, 2), (1, 2, 2, 1), (2, 2, 2, 2)])
-def test_other_boundaries_take_two_passes(bc):
-    _check(small_random_state(61, 47, seed=9, bc=bc), expect_fused=False, thetas=((0.0, 1.0),))
+@pytest.mark.parametrize("bc", [(1, 1, 0, 0), (0, 0, 2, 2), (0, 0, 1, 1), (2, 2, 0, 0), (1, 2, 2, 1), (2, 1, 1, 2), (2, 2, 1, 1), (1, 1, 1, 1), (2, 2, 2, 2)])
+@pytest.mark.parametrize("shape", [(200, 70), (61, 130), (30, 5), (29, 66), (91, 200), (4, 4)])
+def test_pair_kernel_dirichlet_and_outflow_sides(bc, shape):
+    # ghost lanes and ghost rows of BOTH applications, folded boundary columns / top row (outflow), the boundary faces of mf.xlo / mf.ylo;
+    # one to four 64-row blocks (first, interior, last), ragged strips, grids narrower than one strip
+    nx, ny = shape
+    _check(small_random_state(nx, ny, seed=3 + nx + ny, bc=bc, sig_range=(-1.0, 1.0), dx=0.011, dy=0.017, c=1.3), thetas=((0.0, 1.0), (1.0, 0.5)))
+
+
+def test_pair_kernel_boundaries_with_clamped_cells_and_large_dt():
+    w = small_random_state(157, 90, seed=41, fmax=1.7, bc=(1, 2, 2, 1), c=1.3)
+    rng = np.random.default_rng(8)
+    w["E"][7, :] = 2.0 ** rng.integers(-2, 3, w["nx"])
+    w["F"][0, 7, :] = 0.0
+    w["F"][1, 7, :] = w["c"] * w["E"][7, :]
+    _check(w, K=5.0)
+    _check(small_random_state(123, 80, seed=31, bc=(2, 1, 2, 2), sig_range=(-1.0, 2.0)), K=200.0)
 
 
 @pytest.mark.parametrize("shape", [(2, 2), (3, 40), (40, 3)])
-def test_tiny_periodic_grids_take_two_passes(shape):
+@pytest.mark.parametrize("bc", [PER, (1, 2, 2, 1)])
+def test_tiny_grids_take_two_passes(shape, bc):
     nx, ny = shape
-    _check(small_random_state(nx, ny, seed=19, bc=PER), expect_fused=False, thetas=((1.0, 1.0),))
+    _check(small_random_state(nx, ny, seed=19, bc=bc), expect_fused=False, thetas=((1.0, 1.0),))
 
 
 @pytest.mark.parametrize("recompute", [0, 1])
