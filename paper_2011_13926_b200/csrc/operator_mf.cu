@@ -474,7 +474,7 @@ __global__ void __launch_bounds__(TXO, JRC ? OP_RCJ_MINB : OP_RC_MINB) op_mf_rc_
 // periodic on all four sides: every column and row has a plain diagonal block, ghosts wrap); blocks that touch a Dirichlet or
 // outflow side run rc2g_body further down; halo rows of a slab, op_recompute < 2 and grids under 4 x 4 take two single applications.
 // ---------------------------------------------------------------------------------------------------------
-// 8 resident one-warp blocks per SM (two per sub-partition, 240 registers, no spills).  Measured on the bench solve at 4096^2 (58 operator
+// 8 resident one-warp blocks per SM (two per sub-partition, 240-255 registers, no spills).  Measured on the bench solve at 4096^2 (58 operator
 // launches, 34 of them pairs, against 94 single applications at 49.2 ms): 8 blocks 38.1 ms; 12 blocks (168 registers, 216 B of spills)
 // 53.6; 16 blocks 60.0; the inverse block and J parked in shared memory between the two row steps (218 registers) 39.4; rows per
 // block 32 / 64 / 128: 39.4 / 38.1 / 37.9; a third ring stage 38.3.  A pair costs 0.75 ms against 2 x 0.52.
