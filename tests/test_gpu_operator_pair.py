@@ -118,3 +118,11 @@ def test_solver_is_the_same_with_and_without_the_pair_kernel():
     assert np.max(np.abs(np.log10(h1[1:k] / h0[1:k]))) <= 1e-3
     E1, F1 = s1; E0, F0 = s0
     assert np.linalg.norm(E1 - E0) <= 1e-10 * np.linalg.norm(E0) and np.linalg.norm(F1 - F0) <= 1e-10 * np.linalg.norm(F0)
+
+
+@pytest.mark.parametrize("bc", [(1, 2, 2, 1), (0, 0, 2, 2), (2, 2, 0, 0)])
+def test_pair_kernel_boundaries_on_a_grid_of_several_waves(bc):
+    # 37 strips x 13 block rows: interior blocks (periodic code) and boundary blocks (general code) side by side in one grid
+    w = wl.random_medium(1030, seed=77, ny=777)
+    w["bc"] = bc
+    _check(w, K=10.0, thetas=((1.0, 1.0),))
